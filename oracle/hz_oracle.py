@@ -1,0 +1,440 @@
+"""CPU ORACLE for the block-level DDM / WaveHoltz hot path of arxiv/paper_2606_21695.
+
+THIS IS TEST INFRASTRUCTURE, NOT THE PRODUCT.  It is a plain, slow, fp64 numpy/scipy
+restatement of what the paper computes, written from /root/reference/PAPER.md only.
+Only `tests/`, `__graft_entry__.smoke()` and `bench.py`'s `cpu_baseline` /
+`--impl reference` legs may import it.  It shares no code, table or constant
+generator with `paper_2606_21695_b200/` (the CUDA path) and never imports it.
+
+Citations are "PAPER.md:<line> (section / equation)".  Where the paper is silent,
+garbled or inconsistent the reading is the one listed in DESIGN.md ("Readings", R1..R23).
+
+What is pinned (tests/test_oracle_pins.py; none of the pins re-types a formula below):
+  gll()                      sum(w)=2, D exact on polynomials, symmetry, Lambda_1=4, Lambda_2=24
+  element_stiffness()        A_e 1 = 0, symmetric, exact energy of a polynomial field
+  assemble_global()/direct   plane wave recovered at order ~h^(2p) (eq. (1))
+  wh_tables()                filter orthogonality identities
+  waveholtz_iteration()      fixed point == dense direct solve of (4),
+                             leapfrog evolves e^{-i w t} exactly at every step
+  ddm_*()                    converged DDM == dense direct solve <=1e-8,
+                             L=1 DDM == WaveHoltz on the whole domain, hand-sized 2x1 case,
+                             wrong sign of eq. (2) diverges (reading R3)
+Nothing here is "parity unpinned".
+
+Conventions
+  mesh      nx*ny rectangular elements on [x0,x1]x[y0,y1], degree p, GLL nodes;
+            global node (I,J), I in 0..nx*p, J in 0..ny*p, flat index J*(nx*p+1)+I (x fastest).
+  sides     0=W (I=0), 1=E (I=max), 2=S (J=0), 3=N (J=max); an edge array runs along
+            increasing J (W,E) or increasing I (S,N) and INCLUDES both end nodes.
+"""
+from __future__ import annotations
+
+import math
+from dataclasses import dataclass, field
+
+import numpy as np
+import scipy.sparse as sp
+import scipy.sparse.linalg as spla
+
+W_, E_, S_, N_ = 0, 1, 2, 3
+OPPOSITE = (E_, W_, N_, S_)
+
+
+# --------------------------------------------------------------------------------------
+# O1  Discretisation: GLL nodal basis (Section IV)
+# --------------------------------------------------------------------------------------
+def gll(p: int):
+    """Gauss-Lobatto-Legendre nodes xi_0..xi_p on [-1,1] (roots of (1-x^2) P_p'(x)),
+    weights w_a = 2 / (p (p+1) P_p(xi_a)^2) and the Lagrange differentiation matrix
+    D[a,b] = l_b'(xi_a).  PAPER.md:113 ("GLL quadrature rule on which the nodal basis is
+    defined"), PAPER.md:199 ("1D differentiation matrix D of size (P+1)^2")."""
+    if p < 1:
+        raise ValueError("p >= 1")
+    Pp = np.polynomial.legendre.Legendre.basis(p)
+    interior = np.sort(np.real(Pp.deriv().roots())) if p > 1 else np.array([])
+    xi = np.concatenate(([-1.0], interior, [1.0]))
+    # polish the interior roots with Newton on P_p'(x)
+    d1, d2 = Pp.deriv(), Pp.deriv(2)
+    for _ in range(4):
+        if p > 1:
+            xi[1:-1] -= d1(xi[1:-1]) / d2(xi[1:-1])
+    w = 2.0 / (p * (p + 1) * Pp(xi) ** 2)
+    D = np.zeros((p + 1, p + 1))
+    # barycentric form of the derivative of the Lagrange basis
+    bw = np.array([1.0 / np.prod([xi[a] - xi[b] for b in range(p + 1) if b != a])
+                   for a in range(p + 1)])
+    for a in range(p + 1):
+        for b in range(p + 1):
+            if a != b:
+                D[a, b] = (bw[b] / bw[a]) / (xi[a] - xi[b])
+        D[a, a] = -np.sum(D[a, :])
+    return xi, w, D
+
+
+def stiffness_1d(p: int):
+    """Reference 1-D stiffness K = D^T W D on [-1,1] (A_ij=(grad phi_j, grad phi_i)
+    with GLL quadrature, evaluated through D as in PAPER.md:201)."""
+    _, w, D = gll(p)
+    return D.T @ np.diag(w) @ D
+
+
+def lambda_p(p: int) -> float:
+    """Largest eigenvalue of the 1-D element pencil (K_h, W_h) at element length h=1
+    (reading R9: it bounds the spectrum of M^-1 A and fixes the stable time step)."""
+    _, w, _ = gll(p)
+    K = stiffness_1d(p)
+    # physical element of length h: K_h = (2/h) K, W_h = (h/2) W  ->  W_h^-1 K_h = (2/h)^2 W^-1 K
+    ev = np.linalg.eigvals(np.diag(1.0 / w) @ K)
+    return float(4.0 * np.max(np.real(ev)))
+
+
+def element_stiffness(p: int, hx: float, hy: float):
+    """(p+1)^2 x (p+1)^2 stiffness of one hx-by-hy rectangle, local node (a,b) -> b*(p+1)+a.
+    int grad(phi_j).grad(phi_i) with GLL quadrature: (hy/hx) W(x)K  [d/dx part]
+    + (hx/hy) K(x)W [d/dy part]; np.kron(Y, X)[b*(p+1)+a, ...] = Y[b,.] X[a,.].
+    PAPER.md:109 (definition of A), PAPER.md:199-201 (gradient via D, then D^T)."""
+    _, w, _ = gll(p)
+    K = stiffness_1d(p)
+    Wm = np.diag(w)
+    return (hy / hx) * np.kron(Wm, K) + (hx / hy) * np.kron(K, Wm)
+
+
+# --------------------------------------------------------------------------------------
+# Problem description (eq. (1); arguments mirror include/hz.h)
+# --------------------------------------------------------------------------------------
+@dataclass
+class Problem:
+    nx: int
+    ny: int
+    p: int
+    x0: float
+    y0: float
+    x1: float
+    y1: float
+    c_nodes: np.ndarray          # (ny*p+1, nx*p+1) wave speed AT the global GLL nodes (R14)
+    omega: float
+    f: np.ndarray                # (ny*p+1, nx*p+1) complex source AT the nodes
+    bc_lambda: list | None = None  # 4 complex edge arrays (W,E,S,N) or None (=0)
+
+    @property
+    def hx(self):
+        return (self.x1 - self.x0) / self.nx
+
+    @property
+    def hy(self):
+        return (self.y1 - self.y0) / self.ny
+
+    @property
+    def npx(self):
+        return self.nx * self.p + 1
+
+    @property
+    def npy(self):
+        return self.ny * self.p + 1
+
+    def node_coords(self):
+        xi, _, _ = gll(self.p)
+        x = np.concatenate([self.x0 + self.hx * (e + (xi[:-1] + 1) / 2) for e in range(self.nx)]
+                           + [[self.x1]])
+        y = np.concatenate([self.y0 + self.hy * (e + (xi[:-1] + 1) / 2) for e in range(self.ny)]
+                           + [[self.y1]])
+        return x, y
+
+
+def _region_operators(p, ex, ey, hx, hy):
+    """Assemble, by summation over the ex*ey elements of a rectangular region, the
+    stiffness A (sparse), the geometric lumped mass m (one value per region node) and the
+    geometric edge weights s[side] (one value per edge node) of that region.
+    PAPER.md:109-113: GLL quadrature makes M and H diagonal.  Lumped mass of element node
+    (a,b): (hx/2)(hy/2) w_a w_b; edge weight of an element-edge node: (h_edge/2) w_a."""
+    _, w, _ = gll(p)
+    Ae = element_stiffness(p, hx, hy)
+    npx, npy = ex * p + 1, ey * p + 1
+    rows, cols, vals = [], [], []
+    m = np.zeros((npy, npx))
+    la = np.arange(p + 1)
+    for fy in range(ey):
+        for fx in range(ex):
+            gi = (fy * p + la)[:, None] * npx + (fx * p + la)[None, :]   # [b,a] -> global
+            gi = gi.reshape(-1)
+            rows.append(np.repeat(gi, (p + 1) ** 2))
+            cols.append(np.tile(gi, (p + 1) ** 2))
+            vals.append(Ae.reshape(-1))
+            m[fy * p:fy * p + p + 1, fx * p:fx * p + p + 1] += (hx / 2) * (hy / 2) * np.outer(w, w)
+    A = sp.csr_matrix((np.concatenate(vals), (np.concatenate(rows), np.concatenate(cols))),
+                      shape=(npx * npy, npx * npy))
+    A.sum_duplicates()
+    sy = np.zeros(npy)
+    for fy in range(ey):
+        sy[fy * p:fy * p + p + 1] += (hy / 2) * w
+    sx = np.zeros(npx)
+    for fx in range(ex):
+        sx[fx * p:fx * p + p + 1] += (hx / 2) * w
+    s = [sy.copy(), sy.copy(), sx.copy(), sx.copy()]
+    return A, m, s
+
+
+def edge_index(npx, npy, side):
+    """Flat region indices of the nodes of one side, in the edge-array order."""
+    if side == W_:
+        return np.arange(npy) * npx
+    if side == E_:
+        return np.arange(npy) * npx + (npx - 1)
+    if side == S_:
+        return np.arange(npx)
+    return (npy - 1) * npx + np.arange(npx)
+
+
+# --------------------------------------------------------------------------------------
+# O2  Global reference system (4) and direct solve (eq. (4))
+# --------------------------------------------------------------------------------------
+def assemble_global(pr: Problem):
+    """Returns A (sparse real), M (diag, real), H (diag, real; outer boundary only), b (complex)
+    of  (A - i w H - w^2 M) u = b,  PAPER.md:105-111."""
+    A, m, s = _region_operators(pr.p, pr.nx, pr.ny, pr.hx, pr.hy)
+    c = np.asarray(pr.c_nodes, dtype=float).reshape(-1)
+    M = m.reshape(-1) / c ** 2
+    H = np.zeros_like(M)
+    b = np.asarray(pr.f, dtype=complex).reshape(-1) * m.reshape(-1)
+    for side in range(4):
+        idx = edge_index(pr.npx, pr.npy, side)
+        H[idx] += s[side] / c[idx]
+        if pr.bc_lambda is not None:
+            b[idx] += s[side] * np.asarray(pr.bc_lambda[side], dtype=complex)
+    return A, M, H, b
+
+
+def helmholtz_matrix(A, M, H, omega):
+    return (A.astype(complex) - sp.diags(1j * omega * H + omega ** 2 * M)).tocsc()
+
+
+def direct_solve(pr: Problem):
+    """Sparse LU of the global discrete Helmholtz system (4): the plain definition of the
+    converged answer."""
+    A, M, H, b = assemble_global(pr)
+    u = spla.splu(helmholtz_matrix(A, M, H, pr.omega)).solve(b)
+    return u.reshape(pr.npy, pr.npx)
+
+
+def residual(pr: Problem, u):
+    """|| b - (A - i w H - w^2 M) u ||_2 / || b ||_2 on the global system (row A10 of the scope
+    table; the operator is the paper's "Operator time" normaliser)."""
+    A, M, H, b = assemble_global(pr)
+    u = np.asarray(u, dtype=complex).reshape(-1)
+    r = b - (A @ u - (1j * pr.omega * H + pr.omega ** 2 * M) * u)
+    return float(np.linalg.norm(r) / np.linalg.norm(b))
+
+
+# --------------------------------------------------------------------------------------
+# O4  WaveHoltz (Section V; Algorithm 1 at PAPER.md:160-183)
+# --------------------------------------------------------------------------------------
+def choose_nt(p, hx, hy, c_max, omega, cfl_frac):
+    """Number of time steps per period T = 2 pi / w (reading R9).  The stable step of the
+    leapfrog is dt_stab = 2 / sqrt(lmax) with lmax = c_max^2 Lambda_p (1/hx^2 + 1/hy^2) the
+    bound on the spectrum of M^-1 A; N_t = ceil(T / (cfl_frac dt_stab)), at least 4.  The
+    paper prints only dt <= 2h/(p^2 c_max), which is not a bound in 2-D."""
+    lmax = c_max ** 2 * lambda_p(p) * (1.0 / hx ** 2 + 1.0 / hy ** 2)
+    dt_stab = 2.0 / math.sqrt(lmax)
+    T = 2.0 * math.pi / omega
+    return max(4, int(math.ceil(T / (cfl_frac * dt_stab) * (1.0 - 1e-12))))
+
+
+@dataclass
+class WHTables:
+    n_t: int
+    dt: float
+    theta: float
+    sigma: float
+    kappa: np.ndarray        # kappa_nu,       nu = 0..N_t-1
+    kappa_half: np.ndarray   # kappa_{nu+1/2}, nu = 0..N_t-1
+    cos_nu: np.ndarray       # cos(2 pi nu / N_t)
+    sin_nu: np.ndarray       # sin(2 pi nu / N_t)
+
+
+def wh_tables(n_t: int, omega: float) -> WHTables:
+    """Filter kappa_nu = cos(2 pi nu/N_t) - 1/4 + 1/4 tan^2(pi/N_t), evaluated at
+    nu and at nu+1/2 (reading R6); theta = tan(w dt/2)/w, sigma = sin(w dt/2)/(w/2)
+    (PAPER.md:144)."""
+    dt = 2.0 * math.pi / omega / n_t
+    nu = np.arange(n_t, dtype=float)
+
+    def kap(x):
+        return np.cos(2 * np.pi * x / n_t) - 0.25 + 0.25 * math.tan(math.pi / n_t) ** 2
+
+    return WHTables(n_t=n_t, dt=dt,
+                    theta=math.tan(omega * dt / 2) / omega,
+                    sigma=math.sin(omega * dt / 2) / (omega / 2),
+                    kappa=kap(nu), kappa_half=kap(nu + 0.5),
+                    cos_nu=np.cos(2 * np.pi * nu / n_t), sin_nu=np.sin(2 * np.pi * nu / n_t))
+
+
+def waveholtz_iteration(A, M, H, b, u, omega, tab: WHTables, trace=None):
+    """One application of Pi (eq. (7)) in the order of Algorithm 1
+    (PAPER.md:168-178).  A sparse real, M/H real diagonals, b/u complex vectors.
+    If `trace` is a list, (p^nu, pdot^{nu+1/2}) of every step is appended to it."""
+    N = tab.n_t
+    alpha = (M - tab.theta * H) / (M + tab.theta * H)
+    beta = tab.sigma / (M + tab.theta * H)
+    # Initialise p <- Re u ; pdot <- Re{-i w u e^{-pi i / N_t}}  (reading R8)
+    p = np.real(u).copy()
+    pdot = np.real(-1j * omega * u * np.exp(-1j * math.pi / N))
+    # v <- kappa_0 p - (1/(i w)) kappa_{1/2} pdot   (eq. (7) sign, reading R2)
+    v = tab.kappa[0] * p - (1.0 / (1j * omega)) * tab.kappa_half[0] * pdot
+    if trace is not None:
+        trace.append((p.copy(), pdot.copy()))
+    for nu in range(1, N):                                     # PAPER.md:170 (reading R5)
+        p = p + tab.sigma * pdot                               # PAPER.md:142 / 172
+        Ap = A @ p
+        src = np.real(b * np.exp(-2j * math.pi * nu / N))      # PAPER.md:140 (reading R7)
+        pdot = alpha * pdot + beta * (-Ap + src)               # PAPER.md:140 / 176
+        v = v + tab.kappa[nu] * p - (1.0 / (1j * omega)) * tab.kappa_half[nu] * pdot  # 177
+        if trace is not None:
+            trace.append((p.copy(), pdot.copy()))
+    return (2.0 / N) * v                                       # eq. (7) prefactor (reading R4)
+
+
+# --------------------------------------------------------------------------------------
+# O3/O5/O6/O7  Domain decomposition (Section III; Algorithm 1)
+# --------------------------------------------------------------------------------------
+@dataclass
+class Subdomain:
+    ix: int                      # position in the sx*sy subdomain grid
+    iy: int
+    I0: int                      # global node offset of the local node (0,0)
+    J0: int
+    npx: int
+    npy: int
+    A: sp.csr_matrix             # local stiffness (own elements only)
+    M: np.ndarray                # c^-2 * local lumped mass
+    H: np.ndarray                # c^-1 * edge weight on the WHOLE subdomain boundary (O3)
+    bf: np.ndarray               # f(x_j) * local lumped mass (+ physical-side bc_lambda), complex
+    s: list                      # geometric edge weights per side
+    k_edge: list                 # k_j = omega / c_j on each side's nodes (reading R15)
+    neighbour: list              # subdomain index across each side, or -1 (physical boundary)
+    edge_idx: list = field(default_factory=list)
+
+
+@dataclass
+class DDMState:
+    pr: Problem
+    sx: int
+    sy: int
+    tab: WHTables
+    subs: list
+    lam: list                    # lam[l][side] complex edge array (zeros on physical sides)
+    u: list                      # u[l] complex local vector (previous WaveHoltz iterate)
+    n_sweeps: int = 0
+
+
+def ddm_setup(pr: Problem, sx: int, sy: int, cfl_frac: float = 0.5, n_t: int | None = None) -> DDMState:
+    """Partition into sx*sy rectangular subdomains of (nx/sx)*(ny/sy) elements and build the
+    subdomain systems (O3): A_l, M_l from the subdomain's own elements; H_l on its whole
+    boundary (interfaces carry the same impedance operator as the outer boundary,
+    PAPER.md:70-75, 83); load f(x_j) m^l_j with the LOCAL mass."""
+    if pr.nx % sx or pr.ny % sy:
+        raise ValueError("subdomain grid must divide the element grid (reading R23)")
+    ex, ey = pr.nx // sx, pr.ny // sy
+    A, m, s = _region_operators(pr.p, ex, ey, pr.hx, pr.hy)
+    npx, npy = ex * pr.p + 1, ey * pr.p + 1
+    c = np.asarray(pr.c_nodes, dtype=float)
+    f = np.asarray(pr.f, dtype=complex)
+    if n_t is None:
+        n_t = choose_nt(pr.p, pr.hx, pr.hy, float(c.max()), pr.omega, cfl_frac)
+    tab = wh_tables(n_t, pr.omega)
+    subs = []
+    for iy in range(sy):
+        for ix in range(sx):
+            I0, J0 = ix * ex * pr.p, iy * ey * pr.p
+            cl = c[J0:J0 + npy, I0:I0 + npx].reshape(-1)
+            fl = f[J0:J0 + npy, I0:I0 + npx].reshape(-1)
+            M = m.reshape(-1) / cl ** 2
+            H = np.zeros_like(M)
+            bf = fl * m.reshape(-1)
+            nb = [-1, -1, -1, -1]
+            if ix > 0:
+                nb[W_] = iy * sx + ix - 1
+            if ix < sx - 1:
+                nb[E_] = iy * sx + ix + 1
+            if iy > 0:
+                nb[S_] = (iy - 1) * sx + ix
+            if iy < sy - 1:
+                nb[N_] = (iy + 1) * sx + ix
+            eidx, kedge = [], []
+            for side in range(4):
+                idx = edge_index(npx, npy, side)
+                eidx.append(idx)
+                H[idx] += s[side] / cl[idx]
+                kedge.append(pr.omega / cl[idx])
+                if nb[side] < 0 and pr.bc_lambda is not None:
+                    full = np.asarray(pr.bc_lambda[side], dtype=complex)
+                    off = J0 if side in (W_, E_) else I0
+                    bf[idx] += s[side] * full[off:off + len(idx)]
+            subs.append(Subdomain(ix, iy, I0, J0, npx, npy, A, M, H, bf, s, kedge, nb, eidx))
+    lam = [[np.zeros(len(sd.edge_idx[side]), dtype=complex) for side in range(4)] for sd in subs]
+    u = [np.zeros(sd.npx * sd.npy, dtype=complex) for sd in subs]
+    return DDMState(pr, sx, sy, tab, subs, lam, u)
+
+
+def ddm_cycle(st: DDMState, l: int, n_wh: int, warm_start: bool, sign_2ik: float = -1.0):
+    """Algorithm 1 on subdomain l.  Returns (u_l, g) where g[side] is the
+    outgoing interface datum of each non-physical side (None on physical sides):
+        g = -lambda^n_{l,side} - 2 i k u_l      (eq. (2), sign per reading R3;
+    `sign_2ik=+1` reproduces the printed sign and is used only by the pin that shows it
+    diverges)."""
+    sd = st.subs[l]
+    # Assemble b from f and lambda^n: b_j = f_j m_j + sum_sides s_j lambda_j
+    b = sd.bf.copy()
+    for side in range(4):
+        if sd.neighbour[side] >= 0:
+            b[sd.edge_idx[side]] += sd.s[side] * st.lam[l][side]
+    # u^(0) <- 0 or the previous iterate (warm start, reading R11)
+    u = st.u[l].copy() if warm_start else np.zeros_like(st.u[l])
+    for _ in range(n_wh):                                   # fixed count (reading R10)
+        u = waveholtz_iteration(sd.A, sd.M, sd.H, b, u, st.pr.omega, st.tab)
+    g = [None] * 4
+    for side in range(4):
+        if sd.neighbour[side] >= 0:
+            g[side] = -st.lam[l][side] + sign_2ik * 2j * sd.k_edge[side] * u[sd.edge_idx[side]]
+    return u, g
+
+
+def ddm_sweep(st: DDMState, n_wh: int, warm_start: bool, relax: float, sign_2ik: float = -1.0):
+    """One outer iteration: the DDM cycle on every subdomain from the SAME lambda^n (all
+    subdomains concurrently), then the exchange (O6): subdomain l's outgoing g
+    on `side` lands in neighbour r's slot on the opposite side, with relaxation rho (R12):
+        lambda^{n+1}_{r,opp} = (1-rho) lambda^n_{r,opp} + rho g_{l,side}."""
+    L = len(st.subs)
+    new_u, gs = [None] * L, [None] * L
+    for l in range(L):
+        new_u[l], gs[l] = ddm_cycle(st, l, n_wh, warm_start, sign_2ik)
+    new_lam = [[a.copy() for a in st.lam[l]] for l in range(L)]
+    for l in range(L):
+        for side in range(4):
+            r = st.subs[l].neighbour[side]
+            if r >= 0:
+                o = OPPOSITE[side]
+                new_lam[r][o] = (1.0 - relax) * st.lam[r][o] + relax * gs[l][side]
+    st.lam, st.u = new_lam, new_u
+    st.n_sweeps += 1
+    return st
+
+
+def ddm_gather(st: DDMState):
+    """Global nodal field: mean of the copies at nodes shared by several subdomains (R19)."""
+    pr = st.pr
+    acc = np.zeros((pr.npy, pr.npx), dtype=complex)
+    cnt = np.zeros((pr.npy, pr.npx))
+    for l, sd in enumerate(st.subs):
+        acc[sd.J0:sd.J0 + sd.npy, sd.I0:sd.I0 + sd.npx] += st.u[l].reshape(sd.npy, sd.npx)
+        cnt[sd.J0:sd.J0 + sd.npy, sd.I0:sd.I0 + sd.npx] += 1.0
+    return acc / cnt
+
+
+def ddm_solve(pr: Problem, sx: int, sy: int, n_outer: int, n_wh: int, warm_start: bool = True,
+              relax: float = 0.5, cfl_frac: float = 0.5, n_t: int | None = None,
+              sign_2ik: float = -1.0, state: DDMState | None = None):
+    """n_outer sweeps from lambda^0 = 0, u^0 = 0 (or continue `state`)."""
+    st = state if state is not None else ddm_setup(pr, sx, sy, cfl_frac, n_t)
+    for _ in range(n_outer):
+        ddm_sweep(st, n_wh, warm_start, relax, sign_2ik)
+    return st

@@ -1,0 +1,168 @@
+"""Seeded synthetic inputs for the five BASELINE.json configs ("Input recipe").
+
+This module serves BOTH the CPU oracle (tests, bench cpu_baseline) and the CUDA library.
+It holds none of the method's arithmetic: it only places nodes, samples the wave speed
+c(x) and the source f(x) AT the global GLL nodes, and names the partition / solver options
+of each config.  No RNG is re-implemented on either side: the random draws happen here
+(numpy.random.default_rng(seed)) and reach both sides as plain arrays.
+
+The paper's workloads are synthetic too (constant / piecewise-constant coefficients on a
+square with uniform elements; the Y-waveguide picture of Fig. 1,
+PAPER.md:27), so nothing here stands in for a public dataset.
+"""
+from __future__ import annotations
+
+import math
+from dataclasses import dataclass, field
+
+import numpy as np
+
+# Gauss-Lobatto-Legendre points on [-1,1] in closed form (p <= 4); only used to PLACE the
+# nodes at which c and f are sampled.  The oracle and the CUDA library each compute their
+# own nodes, weights and differentiation matrices.
+_GLL_CLOSED_FORM = {
+    1: (-1.0, 1.0),
+    2: (-1.0, 0.0, 1.0),
+    3: (-1.0, -1.0 / math.sqrt(5.0), 1.0 / math.sqrt(5.0), 1.0),
+    4: (-1.0, -math.sqrt(3.0 / 7.0), 0.0, math.sqrt(3.0 / 7.0), 1.0),
+}
+
+
+def node_coords_1d(n: int, p: int, a: float = 0.0, b: float = 1.0) -> np.ndarray:
+    """The n*p+1 node abscissae of n uniform degree-p elements on [a,b]."""
+    xi = np.asarray(_GLL_CLOSED_FORM[p])
+    h = (b - a) / n
+    x = np.empty(n * p + 1)
+    for e in range(n):
+        x[e * p:e * p + p] = a + h * (e + (xi[:-1] + 1.0) / 2.0)
+    x[-1] = b
+    return x
+
+
+@dataclass
+class HzInputs:
+    """Everything hz_mesh_setup / hz_partition / hz_ddm_solve (and the oracle) need."""
+    name: str
+    nx: int
+    ny: int
+    p: int
+    x0: float
+    y0: float
+    x1: float
+    y1: float
+    omega: float
+    c_nodes: np.ndarray            # (ny*p+1, nx*p+1) float64, x fastest
+    f_re: np.ndarray               # (ny*p+1, nx*p+1) float64
+    f_im: np.ndarray | None
+    sx: int
+    sy: int
+    cfl_frac: float = 0.5
+    relax: float = 0.5
+    n_wh: int = 5
+    warm_start: bool = True
+    seed: int = 0
+    meta: dict = field(default_factory=dict)
+
+    @property
+    def npx(self):
+        return self.nx * self.p + 1
+
+    @property
+    def npy(self):
+        return self.ny * self.p + 1
+
+
+def omega_for_ppw(n: int, p: int, ppw: float, c_ref: float = 1.0, length: float = 1.0) -> float:
+    """omega such that the wavelength 2 pi c_ref / omega spans `ppw` node spacings h/p
+    (reading R18)."""
+    return 2.0 * math.pi * c_ref * p * n / (ppw * length)
+
+
+def _seg_dist(X, Y, ax, ay, bx, by):
+    dx, dy = bx - ax, by - ay
+    t = ((X - ax) * dx + (Y - ay) * dy) / (dx * dx + dy * dy)
+    t = np.clip(t, 0.0, 1.0)
+    return np.hypot(X - (ax + t * dx), Y - (ay + t * dy))
+
+
+def y_waveguide_speed(X, Y, c_in: float = 3.0, c_out: float = 1.0, width: float = 0.1):
+    """c = c_in where the distance to any of the three centre-line segments of the Y is
+    <= width/2 (closed set), else c_out (reading R16)."""
+    d = np.minimum(_seg_dist(X, Y, 0.5, 0.0, 0.5, 0.5),
+                   np.minimum(_seg_dist(X, Y, 0.5, 0.5, 0.2, 1.0),
+                              _seg_dist(X, Y, 0.5, 0.5, 0.8, 1.0)))
+    return np.where(d <= 0.5 * width, c_in, c_out)
+
+
+def random_block_speed(X, Y, rng, nb: int = 8, lo: float = 1.0, hi: float = 3.0):
+    """Piecewise-constant c on an nb x nb grid of blocks with i.i.d. U[lo,hi] values; a node
+    on a block line belongs to block min(floor(nb*x), nb-1) (reading R14)."""
+    vals = rng.uniform(lo, hi, size=(nb, nb))
+    bi = np.minimum(np.floor(nb * X).astype(int), nb - 1)
+    bj = np.minimum(np.floor(nb * Y).astype(int), nb - 1)
+    return vals[bj, bi], vals
+
+
+def draw_source_points(rng, count: int):
+    """x_s ~ U([0.15,0.85]^2), rejecting |x_s - (1/2,1/2)|_inf < 0.05 (reading R17)."""
+    pts = []
+    while len(pts) < count:
+        xs, ys = rng.uniform(0.15, 0.85, size=2)
+        if max(abs(xs - 0.5), abs(ys - 0.5)) < 0.05:
+            continue
+        pts.append((float(xs), float(ys)))
+    return pts
+
+
+def gaussian_sources(X, Y, pts, sigma: float):
+    f = np.zeros_like(X)
+    for xs, ys in pts:
+        f += np.exp(-((X - xs) ** 2 + (Y - ys) ** 2) / (2.0 * sigma ** 2))
+    return f
+
+
+def make_config(cfg: int, n: int | None = None, p: int | None = None, sub_elems: int | None = None,
+                seed: int | None = None) -> HzInputs:
+    """Config `cfg` in 1..5 of BASELINE.json.  `n` (elements per side), `p` and `sub_elems`
+    (elements per subdomain side) override the full-size values to get a SMALLER problem of
+    the same structure for the parity tests; the full-size values are the defaults."""
+    defaults = {1: (16, 2, 8, 8.0), 2: (128, 3, 8, 10.0), 3: (512, 3, 8, 10.0),
+                4: (1024, 3, 32, 10.0), 5: (2048, 3, 8, 10.0)}
+    n0, p0, s0, ppw = defaults[cfg]
+    n = n0 if n is None else n
+    p = p0 if p is None else p
+    s = s0 if sub_elems is None else sub_elems
+    if n % s:
+        raise ValueError("sub_elems must divide n")
+    seed = 1000 + cfg if seed is None else seed
+    rng = np.random.default_rng(seed)
+    x = node_coords_1d(n, p)
+    X, Y = np.meshgrid(x, x, indexing="xy")            # [J, I]: x fastest
+    h = 1.0 / n
+    omega = omega_for_ppw(n, p, ppw)
+    meta = {"ppw": ppw}
+    if cfg == 1:
+        c = np.ones_like(X)
+        pts = draw_source_points(rng, 1)
+        sigma = 0.03 * (16.0 / n)                          # = 0.03 at n = 16
+    elif cfg in (2, 4):
+        c = y_waveguide_speed(X, Y)
+        pts = draw_source_points(rng, 1)
+        sigma = 1.28 * h                                   # = 0.01 at n = 128
+    else:
+        c, vals = random_block_speed(X, Y, rng)
+        meta["block_speeds"] = vals
+        pts = draw_source_points(rng, 3)
+        sigma = 1.28 * h
+    f = gaussian_sources(X, Y, pts, sigma)
+    meta.update(sources=pts, sigma=sigma)
+    return HzInputs(name=f"cfg{cfg}_n{n}_p{p}_s{s}", nx=n, ny=n, p=p, x0=0.0, y0=0.0, x1=1.0, y1=1.0,
+                    omega=omega, c_nodes=np.ascontiguousarray(c, dtype=np.float64),
+                    f_re=np.ascontiguousarray(f, dtype=np.float64), f_im=None,
+                    sx=n // s, sy=n // s, seed=seed, meta=meta)
+
+
+def random_lambda(rng, n_sub: int, edge_nodes: int):
+    """A random complex interface vector lambda[l, side, node] (the paper's benchmark applies
+    the DDM cycle to a random input vector)."""
+    return rng.standard_normal((n_sub, 4, edge_nodes)) + 1j * rng.standard_normal((n_sub, 4, edge_nodes))
