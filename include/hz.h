@@ -1,0 +1,173 @@
+/* hz.h — C ABI of the B200-native block-level DDM / WaveHoltz Helmholtz sweep.
+ *
+ * Implements the hot path of arxiv/paper_2606_21695 ("Efficient Domain Decomposition for the
+ * Helmholtz Equation on GPUs").  Citations are PAPER.md:<line> (section / equation / algorithm);
+ * "reading Rn" refers to the list of readings in DESIGN.md.
+ *
+ * Every entry point returns an hz_status and never throws or aborts across the ABI.  Output
+ * parameters are left untouched on error.  A NULL required pointer gives HZ_EINVAL.  CUDA runtime
+ * failures give HZ_ECUDA with the runtime's message in hz_last_error().  There is no CPU fallback:
+ * without a CUDA device every compute call fails with HZ_ECUDA.
+ *
+ * Pointer kinds are stated per argument: HOST (plain host memory, copied during the call, the caller
+ * keeps ownership) or DEVICE (device memory owned by the caller, e.g. a torch tensor; must stay
+ * valid until the stream work that uses it has finished).  Everything the library allocates on
+ * the device is owned by the context and released by hz_destroy().
+ *
+ * Node numbering (all arrays): nx*ny rectangular elements of degree p on [x0,x1]x[y0,y1];
+ * global node (I,J), I in 0..nx*p, J in 0..ny*p, flat index J*(nx*p+1)+I (x fastest); nodes sit at
+ * the Gauss-Lobatto-Legendre points of each element.
+ * Sides: 0=W (I=0), 1=E (I=max), 2=S (J=0), 3=N (J=max); an edge array runs along increasing J (W,E)
+ * or increasing I (S,N) and includes both end nodes.
+ */
+#ifndef HZ_H
+#define HZ_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct hz_ctx hz_ctx; /* opaque; owns every device buffer it creates */
+
+typedef enum {
+  HZ_OK = 0,
+  HZ_EINVAL = 1,       /* bad argument (NULL, non-positive size, partition does not divide the mesh) */
+  HZ_ENOMEM = 2,       /* host or device allocation failed */
+  HZ_ECUDA = 3,        /* CUDA runtime error; see hz_last_error */
+  HZ_EUNSUPPORTED = 4, /* degree, subdomain size or variant has no compiled kernel */
+  HZ_ESTATE = 5        /* call order violated (e.g. hz_ddm_solve before hz_partition) */
+} hz_status;
+
+typedef enum { HZ_F32 = 0, HZ_F64 = 1 } hz_prec;
+
+/* Transmission operator on interfaces.  B = d/dn - i k is the only one in the paper
+ * (Section III). */
+typedef enum { HZ_TC_IMPEDANCE0 = 0 } hz_transmission;
+
+/* ---------------------------------------------------------------------------------------------
+ * hz_mesh_setup — the Helmholtz problem (eq. (1a,b)) on a uniform quad mesh with
+ * the spectral-element discretisation of PAPER.md:94-117 (Section IV, eq. (3)-(4)).
+ *
+ *   out        receives a new context.
+ *   nx, ny     elements per direction (>= 1);  [x0,x1]x[y0,y1] the domain (x1>x0, y1>y0).
+ *   p          polynomial degree, 1..4 (else HZ_EUNSUPPORTED).
+ *   c_nodes    HOST, (nx*p+1)*(ny*p+1) doubles: wave speed c(x_j) > 0 AT the global nodes (reading R14).
+ *   omega      angular frequency > 0;  k_j = omega / c_j.
+ *   f_re,f_im  HOST, same shape: source f(x_j) at the nodes.  f_im may be NULL (= 0).
+ *   bc_lambda  HOST or NULL (= 0): boundary datum lambda of eq. (1b) on the outer boundary, as
+ *              4 consecutive side blocks W,E,S,N, each 2*EB doubles (re[EB] then im[EB]) with
+ *              EB = max(nx*p+1, ny*p+1); side arrays are indexed by J (W,E) or I (S,N).
+ * ------------------------------------------------------------------------------------------- */
+hz_status hz_mesh_setup(hz_ctx **out, int nx, int ny, double x0, double y0, double x1, double y1, int p,
+                        const double *c_nodes, double omega, const double *f_re, const double *f_im,
+                        const double *bc_lambda);
+
+/* Replace the source f (HOST arrays as in hz_mesh_setup; f_im may be NULL).  After hz_partition
+ * the per-subdomain load vectors are rebuilt on the device ("Assemble b from f"). */
+hz_status hz_set_source(hz_ctx *ctx, const double *f_re, const double *f_im);
+
+/* What hz_partition chose; all values are also what the oracle must reproduce independently. */
+typedef struct {
+  int n_t;               /* time steps per period T = 2 pi / omega (reading R9) */
+  int dofs_per_sub;      /* (ex*p+1)*(ey*p+1) */
+  int edge_nodes_x;      /* ex*p+1: nodes on a S/N side */
+  int edge_nodes_y;      /* ey*p+1: nodes on a W/E side */
+  int edge_stride;       /* E = max of the two: stride of one side in lambda arrays */
+  int threads_per_block; /* block size of the sweep kernel */
+  int blocks;            /* = sx*sy subdomains = thread blocks of one sweep launch */
+  int dofs_per_thread;   /* 1, or (mx*p)*(my*p) of the register-blocked variant */
+  int tile_mx, tile_my;  /* elements per thread tile (0 for the one-DOF-per-thread variant) */
+  double dt, theta, sigma; /* dt = T/n_t; theta = tan(w dt/2)/w; sigma = 2 sin(w dt/2)/w */
+  size_t smem_bytes;       /* dynamic shared memory per block */
+  size_t workspace_bytes;  /* device bytes the context allocated for this partition */
+} hz_part_info;
+
+/* ---------------------------------------------------------------------------------------------
+ * hz_partition — non-overlapping decomposition into sx*sy rectangular subdomains of
+ * (nx/sx)*(ny/sy) elements, one thread block per subdomain, and the
+ * per-subdomain operator data of the modified leapfrog (alpha_j, beta_j).
+ *
+ *   sx, sy           subdomain grid; must divide nx, ny (else HZ_EINVAL; reading R23).
+ *   tc               transmission condition (only HZ_TC_IMPEDANCE0).
+ *   prec             arithmetic of the sweep (fp32 or fp64 build of the subdomain solve).
+ *   dofs_per_thread  1 = one DOF per thread (needs dofs_per_sub <= 1024);
+ *                    k > 1 = register-blocked variant with k = (mx*p)*(my*p) DOFs per thread
+ *                    (PAPER.md:209-217), HZ_EUNSUPPORTED if no tile of that size is compiled or fits;
+ *                    0 = choose automatically.
+ *   cfl_frac         fraction of the stable leapfrog step, in (0,1] (0.5 in all configs).
+ *   info_out         may be NULL.
+ * Re-partitioning an existing context is allowed; it discards lambda and the subdomain states.
+ * ------------------------------------------------------------------------------------------- */
+hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec prec, int dofs_per_thread,
+                       double cfl_frac, hz_part_info *info_out);
+
+typedef struct {
+  int n_outer_max;  /* sweeps to run (>= 0) */
+  int n_wh;         /* WaveHoltz iterations per sweep (>= 1; reading R10; the paper times 5) */
+  int warm_start;   /* 0: u^(0) = 0 every sweep (Algorithm 1); 1: previous u_l (reading R11) */
+  double relax;     /* rho in (0,1]; 1 = eq. (2) literally; configs use 0.5 (reading R12) */
+  double tol;       /* > 0: stop when the global relative residual <= tol (checked every check_every sweeps) */
+  int check_every;  /* residual check period in sweeps; <= 0 = never (run exactly n_outer_max) */
+  int reset_state;  /* 1: zero lambda and u_l before the first sweep; 0: continue from the current state */
+  int fused_exchange; /* 0: separate exchange kernel after every sweep; 1: the next sweep's prologue
+                         applies the exchange itself (same arithmetic, one launch per sweep) */
+} hz_solve_opts;
+
+typedef struct {
+  int n_outer_done;
+  int n_t;
+  double rel_residual;   /* last residual computed, or -1 if none was */
+  double sweep_ms_total; /* device time of all sweep launches (CUDA events on `stream`) */
+  double exch_ms_total;  /* device time of all exchange launches */
+  double total_ms;       /* device time of the whole call on `stream` */
+  double dof_timesteps;  /* sum_l N_l * n_wh * (n_t-1) * n_outer_done  (WaveHoltz DOF-timestep updates) */
+  int sweep_launches, exch_launches, other_launches; /* kernels launched by this call */
+} hz_solve_info;
+
+/* ---------------------------------------------------------------------------------------------
+ * hz_ddm_solve — the outer iteration on the interface data lambda (eq. (2) with the
+ * sign of reading R3): each sweep applies the DDM cycle of Algorithm 1 to all
+ * subdomains concurrently in ONE kernel launch, then exchanges the outgoing
+ * interface data with relaxation.
+ *
+ *   u_out   DEVICE or NULL: 2*(nx*p+1)*(ny*p+1) reals of the partition's precision, re plane then
+ *           im plane; nodes shared by several subdomains hold the mean of their copies (reading R19).
+ *   info    may be NULL.
+ *   stream  a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); 0 = default stream.
+ * The call enqueues all work on `stream` and synchronises the stream before returning (timings
+ * in `info` are then valid).
+ * ------------------------------------------------------------------------------------------- */
+hz_status hz_ddm_solve(hz_ctx *ctx, const hz_solve_opts *opts, void *u_out, hz_solve_info *info, void *stream);
+
+/* Relative residual || b - (A - i w H - w^2 M) u ||_2 / || b ||_2 of a global nodal vector on the
+ * UNPARTITIONED system (4) (the operator is the "Operator time" kernel of PAPER.md:223),
+ * accumulated in fp64.  u_dev: DEVICE, layout as u_out, of precision u_prec.  Synchronises `stream`. */
+hz_status hz_residual(hz_ctx *ctx, const void *u_dev, hz_prec u_prec, double *rel_residual, void *stream);
+
+/* Raw state for parity tests.  u_sub_dev: DEVICE or NULL, doubles [blocks][2][dofs_per_sub]
+ * (re then im, local node (I,J) at J*edge_nodes_x+I).  lambda_dev: DEVICE or NULL, doubles
+ * [blocks][4][2][edge_stride] (current lambda^n; zeros on physical sides). */
+hz_status hz_get_subdomain_state(hz_ctx *ctx, double *u_sub_dev, double *lambda_dev, void *stream);
+
+/* Overwrite the state (same layouts; either may be NULL = keep).  Used by the paper-style benchmark
+ * that applies one DDM cycle to a random interface vector. */
+hz_status hz_set_subdomain_state(hz_ctx *ctx, const double *u_sub_dev, const double *lambda_dev, void *stream);
+
+/* Message of the last failure on this context ("" if none).  Valid until the next call on ctx.
+ * Not thread-safe.  ctx == NULL returns the message of the last failed hz_mesh_setup. */
+const char *hz_last_error(const hz_ctx *ctx);
+
+/* Frees the context and all its device memory.  NULL-safe. */
+void hz_destroy(hz_ctx *ctx);
+
+/* Micro-benchmarks that establish this GPU's own CUDA-core and shared-memory ceilings (used by
+ * bench.py for the roofline denominators; no method arithmetic).  kind: 0 = FP32 FMA, 1 = FP64 FMA,
+ * 2 = shared-memory load bandwidth.  Returns TFLOP/s (kinds 0,1; 2 flops per FMA) or TB/s (kind 2). */
+hz_status hz_peak_probe(int kind, double *result, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HZ_H */

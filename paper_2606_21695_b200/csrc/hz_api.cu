@@ -1,0 +1,742 @@
+// hz_api.cu — the C-ABI entry points of include/hz.h: host-side setup (GLL tables, time-step tables,
+// partition, variant choice), the outer DDM driver on one stream, and the launches of the auxiliary
+// kernels.  No torch types; device memory of the context is cudaMalloc'd here and freed in hz_destroy.
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/hz.h"
+#include "hz_aux.cuh"
+#include "hz_internal.h"
+
+using namespace hz;
+
+namespace {
+
+std::string g_setup_error;  // message of the last failed hz_mesh_setup (no context exists then)
+
+// ------------------------------------------------------------------------------------------------
+// GLL nodes, weights and differentiation matrix, from the Legendre recurrence.
+// ------------------------------------------------------------------------------------------------
+void legendre(int n, double x, double *Pn, double *dPn) {
+  // P_n(x) and P_n'(x) by the three-term recurrence
+  double p0 = 1.0, p1 = x, d0 = 0.0, d1 = 1.0;
+  if (n == 0) { *Pn = 1.0; *dPn = 0.0; return; }
+  for (int k = 2; k <= n; ++k) {
+    const double p2 = ((2.0 * k - 1.0) * x * p1 - (k - 1.0) * p0) / k;
+    const double d2 = d0 + (2.0 * k - 1.0) * p1;
+    p0 = p1; p1 = p2; d0 = d1; d1 = d2;
+  }
+  *Pn = p1; *dPn = d1;
+}
+
+struct Gll {
+  int p;
+  double xi[kMaxP + 1], w[kMaxP + 1], D[kMaxP + 1][kMaxP + 1], K[kMaxP + 1][kMaxP + 1];
+  double lambda_p;  // largest eigenvalue of the 1-D element pencil (K_h, W_h) at h = 1 (reading R9)
+};
+
+double sym_max_eig(int n, double A[kMaxP + 1][kMaxP + 1]) {
+  // cyclic Jacobi on a small symmetric matrix
+  double a[kMaxP + 1][kMaxP + 1];
+  for (int i = 0; i < n; ++i) for (int j = 0; j < n; ++j) a[i][j] = A[i][j];
+  for (int sweep = 0; sweep < 100; ++sweep) {
+    double off = 0.0;
+    for (int i = 0; i < n; ++i) for (int j = i + 1; j < n; ++j) off += a[i][j] * a[i][j];
+    if (off < 1e-30) break;
+    for (int pi = 0; pi < n; ++pi)
+      for (int q = pi + 1; q < n; ++q) {
+        if (std::fabs(a[pi][q]) < 1e-300) continue;
+        const double th = (a[q][q] - a[pi][pi]) / (2.0 * a[pi][q]);
+        const double t = (th >= 0 ? 1.0 : -1.0) / (std::fabs(th) + std::sqrt(th * th + 1.0));
+        const double cs = 1.0 / std::sqrt(t * t + 1.0), sn = t * cs;
+        for (int k = 0; k < n; ++k) {
+          const double akp = a[k][pi], akq = a[k][q];
+          a[k][pi] = cs * akp - sn * akq; a[k][q] = sn * akp + cs * akq;
+        }
+        for (int k = 0; k < n; ++k) {
+          const double apk = a[pi][k], aqk = a[q][k];
+          a[pi][k] = cs * apk - sn * aqk; a[q][k] = sn * apk + cs * aqk;
+        }
+      }
+  }
+  double mx = a[0][0];
+  for (int i = 1; i < n; ++i) mx = std::fmax(mx, a[i][i]);
+  return mx;
+}
+
+void make_gll(int p, Gll *g) {
+  g->p = p;
+  const int n = p + 1;
+  g->xi[0] = -1.0; g->xi[p] = 1.0;
+  // interior nodes: roots of P_p'(x); Chebyshev-Gauss-Lobatto initial guess + Newton with deflation-free
+  // second derivative from the Legendre ODE: (1-x^2) P'' = 2x P' - p(p+1) P
+  for (int a = 1; a < p; ++a) {
+    double x = -std::cos(M_PI * a / p);
+    for (int it = 0; it < 50; ++it) {
+      double P, dP;
+      legendre(p, x, &P, &dP);
+      const double d2P = (2.0 * x * dP - p * (p + 1.0) * P) / (1.0 - x * x);
+      const double dx = dP / d2P;
+      x -= dx;
+      if (std::fabs(dx) < 1e-16) break;
+    }
+    g->xi[a] = x;
+  }
+  if (p % 2 == 0) g->xi[p / 2] = 0.0;
+  double Pv[kMaxP + 1];
+  for (int a = 0; a < n; ++a) {
+    double P, dP;
+    legendre(p, g->xi[a], &P, &dP);
+    Pv[a] = P;
+    g->w[a] = 2.0 / (p * (p + 1.0) * P * P);
+  }
+  // D[a][b] = l_b'(xi_a) = P_p(xi_a) / (P_p(xi_b) (xi_a - xi_b)),  D[0][0] = -p(p+1)/4 = -D[p][p]
+  for (int a = 0; a < n; ++a)
+    for (int b = 0; b < n; ++b) {
+      if (a != b) g->D[a][b] = Pv[a] / (Pv[b] * (g->xi[a] - g->xi[b]));
+      else if (a == 0) g->D[a][b] = -0.25 * p * (p + 1.0);
+      else if (a == p) g->D[a][b] = 0.25 * p * (p + 1.0);
+      else g->D[a][b] = 0.0;
+    }
+  // K = D^T W D
+  for (int a = 0; a < n; ++a)
+    for (int b = 0; b < n; ++b) {
+      double s = 0.0;
+      for (int q = 0; q < n; ++q) s += g->D[q][a] * g->w[q] * g->D[q][b];
+      g->K[a][b] = s;
+    }
+  // lambda_p = 4 * max eig(W^-1 K) = 4 * max eig(W^-1/2 K W^-1/2)
+  double S[kMaxP + 1][kMaxP + 1];
+  for (int a = 0; a < n; ++a)
+    for (int b = 0; b < n; ++b) S[a][b] = g->K[a][b] / std::sqrt(g->w[a] * g->w[b]);
+  g->lambda_p = 4.0 * sym_max_eig(n, S);
+}
+
+template <typename T>
+cudaError_t dmalloc(T **ptr, size_t n) {
+  *ptr = nullptr;
+  if (n == 0) return cudaSuccess;
+  return cudaMalloc((void **)ptr, n * sizeof(T));
+}
+
+inline int roundup(int a, int b) { return (a + b - 1) / b * b; }
+
+}  // namespace
+
+struct hz_ctx {
+  // mesh + physics
+  int nx = 0, ny = 0, p = 0, npx = 0, npy = 0, EB = 0;
+  double x0 = 0, y0 = 0, x1 = 0, y1 = 0, omega = 0, hx = 0, hy = 0, c_max = 0;
+  Gll gll;
+  double *d_c = nullptr, *d_fre = nullptr, *d_fim = nullptr, *d_bc = nullptr;
+  // partition
+  bool part = false;
+  int sx = 0, sy = 0, ex = 0, ey = 0, L = 0, E = 0, prec = 0;
+  int mx = 0, my = 0, csm = 0;
+  Layout lay{};
+  SweepLaunch launch{};
+  int n_t = 0;
+  double dt = 0, theta = 0, sigma = 0;
+  size_t ws_bytes = 0;
+  void *d_tab = nullptr, *d_gamma = nullptr, *d_alpha = nullptr, *d_bbf_re = nullptr, *d_bbf_im = nullptr;
+  void *d_usub = nullptr, *d_lam = nullptr, *d_g = nullptr, *d_k2 = nullptr, *d_bs = nullptr;
+  void *d_bandx = nullptr, *d_bandy = nullptr;
+  double *d_wxl = nullptr, *d_wyl = nullptr;
+  double *d_part = nullptr, *d_red = nullptr, *d_ures = nullptr;
+  int res_blocks = 0;
+  Elem1D<double> ex1{}, ey1{};
+  std::string err;
+};
+
+namespace {
+
+hz_status fail(hz_ctx *ctx, hz_status st, const std::string &msg) {
+  if (ctx) ctx->err = msg; else g_setup_error = msg;
+  return st;
+}
+hz_status cuda_fail(hz_ctx *ctx, cudaError_t e, const char *what) {
+  return fail(ctx, e == cudaErrorMemoryAllocation ? HZ_ENOMEM : HZ_ECUDA,
+              std::string(what) + ": " + cudaGetErrorString(e));
+}
+#define HZ_CUDA(call)                                        \
+  do {                                                       \
+    cudaError_t e_ = (call);                                 \
+    if (e_ != cudaSuccess) return cuda_fail(ctx, e_, #call); \
+  } while (0)
+
+void free_partition(hz_ctx *c) {
+  void **ptrs[] = {&c->d_tab, &c->d_gamma, &c->d_alpha, &c->d_bbf_re, &c->d_bbf_im, &c->d_usub, &c->d_lam,
+                   &c->d_g, &c->d_k2, &c->d_bs, &c->d_bandx, &c->d_bandy, (void **)&c->d_wxl, (void **)&c->d_wyl,
+                   (void **)&c->d_part, (void **)&c->d_red, (void **)&c->d_ures};
+  for (void **q : ptrs) { if (*q) cudaFree(*q); *q = nullptr; }
+  c->part = false;
+  c->ws_bytes = 0;
+}
+
+Geo make_geo(const hz_ctx *c) {
+  Geo g{};
+  g.nx = c->nx; g.ny = c->ny; g.p = c->p; g.npx = c->npx; g.npy = c->npy;
+  g.sx = c->sx; g.sy = c->sy; g.ex = c->ex; g.ey = c->ey; g.E = c->E; g.EB = c->EB;
+  g.hx = c->hx; g.hy = c->hy; g.omega = c->omega; g.theta = c->theta; g.sigma = c->sigma;
+  return g;
+}
+
+template <typename real>
+hz_status run_build(hz_ctx *ctx, int only_source, cudaStream_t st) {
+  const long long total = (long long)ctx->L * ctx->lay.lnx * ctx->lay.lny;
+  const int bs = 256;
+  const unsigned nb = (unsigned)((total + bs - 1) / bs);
+  k_build<real><<<nb, bs, 0, st>>>(make_geo(ctx), ctx->lay, ctx->d_c, ctx->d_fre, ctx->d_fim, ctx->d_bc, ctx->d_wxl,
+                                   ctx->d_wyl, (real *)ctx->d_gamma, (real *)ctx->d_alpha, (real *)ctx->d_bbf_re,
+                                   (real *)ctx->d_bbf_im, (real *)ctx->d_k2, (real *)ctx->d_bs, only_source);
+  HZ_CUDA(cudaGetLastError());
+  return HZ_OK;
+}
+
+template <typename real>
+void fill_elem1d(const Gll &g, double h, Elem1D<real> *e) {
+  const int P = g.p;
+  const double sc = 4.0 / (h * h);
+  std::memset(e, 0, sizeof(*e));
+  for (int a = 1; a < P; ++a)
+    for (int c = 0; c <= P; ++c) e->kin[a][c] = (real)(sc * g.K[a][c] / g.w[a]);
+  for (int c = 0; c <= P; ++c) {
+    e->k0[c] = (real)(sc * g.K[0][c] / (2.0 * g.w[0]));
+    e->kp[c] = (real)(sc * g.K[P][c] / (2.0 * g.w[0]));
+  }
+}
+
+// Assembled 1-D operator rows of one subdomain side for the one-DOF-per-thread kernel:
+// band[i][d] = (4/h^2) Kasm[i][i+d-P] / wasm[i], d = 0..2P (zero outside the side).
+void make_band(const Gll &g, int ne, double h, std::vector<double> *band, std::vector<double> *wasm) {
+  const int P = g.p, n = ne * P + 1, B = 2 * P + 1;
+  std::vector<double> Kasm((size_t)n * B, 0.0);
+  wasm->assign(n, 0.0);
+  for (int e = 0; e < ne; ++e)
+    for (int a = 0; a <= P; ++a) {
+      (*wasm)[e * P + a] += g.w[a];
+      for (int c = 0; c <= P; ++c) Kasm[(size_t)(e * P + a) * B + (c - a + P)] += g.K[a][c];
+    }
+  band->assign((size_t)n * B, 0.0);
+  for (int i = 0; i < n; ++i)
+    for (int d = 0; d < B; ++d) (*band)[(size_t)i * B + d] = 4.0 / (h * h) * Kasm[(size_t)i * B + d] / (*wasm)[i];
+}
+
+template <typename real>
+cudaError_t upload_as(const std::vector<double> &src, void **dst) {
+  std::vector<real> tmp(src.size());
+  for (size_t i = 0; i < src.size(); ++i) tmp[i] = (real)src[i];
+  cudaError_t e = cudaMalloc(dst, tmp.size() * sizeof(real));
+  if (e != cudaSuccess) return e;
+  return cudaMemcpy(*dst, tmp.data(), tmp.size() * sizeof(real), cudaMemcpyHostToDevice);
+}
+
+template <typename real>
+SweepArgs<real> make_args(const hz_ctx *c, const hz_solve_opts *o) {
+  SweepArgs<real> a{};
+  a.lay = c->lay;
+  a.sx = c->sx; a.sy = c->sy; a.E = c->E;
+  a.n_t = c->n_t; a.n_wh = o->n_wh; a.warm = o->warm_start;
+  a.sigma = (real)c->sigma; a.omega = (real)c->omega;
+  a.cos_h = (real)std::cos(M_PI / c->n_t); a.sin_h = (real)std::sin(M_PI / c->n_t);
+  a.two_over_nt = (real)(2.0 / c->n_t);
+  a.tab = (const Tab4<real> *)c->d_tab;
+  a.gamma = (const real *)c->d_gamma; a.alpha = (const real *)c->d_alpha;
+  a.bbf_re = (const real *)c->d_bbf_re; a.bbf_im = (const real *)c->d_bbf_im;
+  a.u_sub = (real *)c->d_usub; a.lam = (const real *)c->d_lam; a.gout = (real *)c->d_g;
+  a.k2edge = (const real *)c->d_k2; a.bs = (const real *)c->d_bs;
+  a.bandx = (const real *)c->d_bandx; a.bandy = (const real *)c->d_bandy;
+  for (int i = 0; i <= kMaxP; ++i) {
+    for (int j = 0; j <= kMaxP; ++j) { a.ex1.kin[i][j] = (real)c->ex1.kin[i][j]; a.ey1.kin[i][j] = (real)c->ey1.kin[i][j]; }
+    a.ex1.k0[i] = (real)c->ex1.k0[i]; a.ex1.kp[i] = (real)c->ex1.kp[i];
+    a.ey1.k0[i] = (real)c->ey1.k0[i]; a.ey1.kp[i] = (real)c->ey1.kp[i];
+  }
+  a.fused = 0; a.relax = (real)o->relax; a.g_prev = nullptr; a.lam_rw = nullptr;
+  return a;
+}
+
+cudaError_t launch_sweep(const hz_ctx *c, const hz_solve_opts *o, cudaStream_t st) {
+  if (c->prec == HZ_F32) {
+    SweepArgs<float> a = make_args<float>(c, o);
+    return c->lay.variant == 0 ? launch_sweep_dof_f32(a, c->p, c->launch, st)
+                               : launch_sweep_tile_f32(a, c->p, c->mx, c->my, c->csm, c->launch, st);
+  }
+  SweepArgs<double> a = make_args<double>(c, o);
+  return c->lay.variant == 0 ? launch_sweep_dof_f64(a, c->p, c->launch, st)
+                             : launch_sweep_tile_f64(a, c->p, c->mx, c->my, c->csm, c->launch, st);
+}
+
+cudaError_t launch_exchange(const hz_ctx *c, double rho, cudaStream_t st) {
+  const long long total = (long long)c->L * 8 * c->E;
+  const int bs = 256;
+  const unsigned nb = (unsigned)((total + bs - 1) / bs);
+  if (c->prec == HZ_F32)
+    k_exchange<float><<<nb, bs, 0, st>>>(c->sx, c->sy, c->E, c->lay.lnx, c->lay.lny, (float)rho, (float *)c->d_lam,
+                                         (const float *)c->d_g);
+  else
+    k_exchange<double><<<nb, bs, 0, st>>>(c->sx, c->sy, c->E, c->lay.lnx, c->lay.lny, rho, (double *)c->d_lam,
+                                          (const double *)c->d_g);
+  return cudaGetLastError();
+}
+
+// gather into `out` of type outT (precision prec_out)
+cudaError_t launch_gather(const hz_ctx *c, void *out, int prec_out, cudaStream_t st) {
+  const long long total = (long long)c->npx * c->npy;
+  const int bs = 256;
+  const unsigned nb = (unsigned)((total + bs - 1) / bs);
+  const Geo g = make_geo(c);
+  if (c->prec == HZ_F32) {
+    if (prec_out == HZ_F32) k_gather<float, float><<<nb, bs, 0, st>>>(g, c->lay, (const float *)c->d_usub, (float *)out);
+    else k_gather<float, double><<<nb, bs, 0, st>>>(g, c->lay, (const float *)c->d_usub, (double *)out);
+  } else {
+    if (prec_out == HZ_F32) k_gather<double, float><<<nb, bs, 0, st>>>(g, c->lay, (const double *)c->d_usub, (float *)out);
+    else k_gather<double, double><<<nb, bs, 0, st>>>(g, c->lay, (const double *)c->d_usub, (double *)out);
+  }
+  return cudaGetLastError();
+}
+
+hz_status residual_impl(hz_ctx *ctx, const void *u_dev, int u_prec, double *rel, cudaStream_t st) {
+  const long long total = (long long)ctx->npx * ctx->npy;
+  const int bs = 256;
+  const int nb = (int)((total + bs - 1) / bs);
+  if (!ctx->d_part || ctx->res_blocks != nb) {
+    if (ctx->d_part) cudaFree(ctx->d_part);
+    if (ctx->d_red) cudaFree(ctx->d_red);
+    ctx->d_part = nullptr; ctx->d_red = nullptr;
+    HZ_CUDA(dmalloc(&ctx->d_part, (size_t)2 * nb));
+    HZ_CUDA(dmalloc(&ctx->d_red, 2));
+    ctx->res_blocks = nb;
+  }
+  Ref1D ref{};
+  for (int a = 0; a <= ctx->p; ++a) {
+    ref.w[a] = ctx->gll.w[a];
+    for (int b = 0; b <= ctx->p; ++b) ref.K[a][b] = ctx->gll.K[a][b];
+  }
+  Geo g = make_geo(ctx);
+  if (u_prec == HZ_F32)
+    k_residual<float><<<nb, bs, 0, st>>>(g, ref, ctx->d_c, ctx->d_fre, ctx->d_fim, ctx->d_bc, (const float *)u_dev, ctx->d_part);
+  else
+    k_residual<double><<<nb, bs, 0, st>>>(g, ref, ctx->d_c, ctx->d_fre, ctx->d_fim, ctx->d_bc, (const double *)u_dev, ctx->d_part);
+  HZ_CUDA(cudaGetLastError());
+  k_reduce2<<<1, 1024, 0, st>>>(ctx->d_part, nb, ctx->d_red);
+  HZ_CUDA(cudaGetLastError());
+  double h[2];
+  HZ_CUDA(cudaMemcpyAsync(h, ctx->d_red, sizeof(h), cudaMemcpyDeviceToHost, st));
+  HZ_CUDA(cudaStreamSynchronize(st));
+  *rel = (h[1] > 0.0) ? std::sqrt(h[0] / h[1]) : std::sqrt(h[0]);
+  return HZ_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+hz_status hz_mesh_setup(hz_ctx **out, int nx, int ny, double x0, double y0, double x1, double y1, int p,
+                        const double *c_nodes, double omega, const double *f_re, const double *f_im,
+                        const double *bc_lambda) {
+  hz_ctx *ctx = nullptr;  // for the HZ_CUDA macro before the context exists
+  if (!out || !c_nodes || !f_re) return fail(nullptr, HZ_EINVAL, "hz_mesh_setup: NULL out, c_nodes or f_re");
+  if (nx < 1 || ny < 1 || !(x1 > x0) || !(y1 > y0) || !(omega > 0.0) || !std::isfinite(omega))
+    return fail(nullptr, HZ_EINVAL, "hz_mesh_setup: need nx,ny >= 1, x1 > x0, y1 > y0, omega > 0");
+  if (p < 1 || p > kMaxP) return fail(nullptr, HZ_EUNSUPPORTED, "hz_mesh_setup: degree p must be 1..4");
+  const long long nn = ((long long)nx * p + 1) * ((long long)ny * p + 1);
+  if (nn > (1ll << 31) - 1) return fail(nullptr, HZ_EUNSUPPORTED, "hz_mesh_setup: more than 2^31-1 nodes");
+  double cmax = 0.0;
+  for (long long q = 0; q < nn; ++q) {
+    if (!(c_nodes[q] > 0.0) || !std::isfinite(c_nodes[q])) return fail(nullptr, HZ_EINVAL, "hz_mesh_setup: c_nodes must be finite and > 0");
+    cmax = std::fmax(cmax, c_nodes[q]);
+  }
+  hz_ctx *c = new (std::nothrow) hz_ctx();
+  if (!c) return fail(nullptr, HZ_ENOMEM, "hz_mesh_setup: out of host memory");
+  c->nx = nx; c->ny = ny; c->p = p; c->npx = nx * p + 1; c->npy = ny * p + 1;
+  c->EB = c->npx > c->npy ? c->npx : c->npy;
+  c->x0 = x0; c->y0 = y0; c->x1 = x1; c->y1 = y1; c->omega = omega;
+  c->hx = (x1 - x0) / nx; c->hy = (y1 - y0) / ny; c->c_max = cmax;
+  make_gll(p, &c->gll);
+  cudaError_t e = cudaSuccess;
+  const size_t bytes = (size_t)nn * sizeof(double);
+  if (e == cudaSuccess) e = dmalloc(&c->d_c, (size_t)nn);
+  if (e == cudaSuccess) e = dmalloc(&c->d_fre, (size_t)nn);
+  if (e == cudaSuccess) e = cudaMemcpy(c->d_c, c_nodes, bytes, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(c->d_fre, f_re, bytes, cudaMemcpyHostToDevice);
+  if (e == cudaSuccess && f_im) {
+    e = dmalloc(&c->d_fim, (size_t)nn);
+    if (e == cudaSuccess) e = cudaMemcpy(c->d_fim, f_im, bytes, cudaMemcpyHostToDevice);
+  }
+  if (e == cudaSuccess && bc_lambda) {
+    e = dmalloc(&c->d_bc, (size_t)8 * c->EB);
+    if (e == cudaSuccess) e = cudaMemcpy(c->d_bc, bc_lambda, (size_t)8 * c->EB * sizeof(double), cudaMemcpyHostToDevice);
+  }
+  if (e != cudaSuccess) {
+    hz_status st = cuda_fail(nullptr, e, "hz_mesh_setup (device allocation / copy)");
+    hz_destroy(c);
+    return st;
+  }
+  (void)ctx;
+  *out = c;
+  return HZ_OK;
+}
+
+hz_status hz_set_source(hz_ctx *ctx, const double *f_re, const double *f_im) {
+  if (!ctx) return HZ_EINVAL;
+  if (!f_re) return fail(ctx, HZ_EINVAL, "hz_set_source: NULL f_re");
+  const size_t nn = (size_t)ctx->npx * ctx->npy;
+  if (f_im && !ctx->d_fim) {
+    if (ctx->part && (ctx->lay.variant == 1))
+      return fail(ctx, HZ_EUNSUPPORTED, "hz_set_source: complex f needs the one-DOF-per-thread variant; re-partition");
+    HZ_CUDA(dmalloc(&ctx->d_fim, nn));
+    if (ctx->part && !ctx->d_bbf_im) {
+      const size_t rs = ctx->prec == HZ_F32 ? 4 : 8;
+      HZ_CUDA(cudaMalloc(&ctx->d_bbf_im, (size_t)ctx->L * ctx->lay.NS * rs));
+      HZ_CUDA(cudaMemset(ctx->d_bbf_im, 0, (size_t)ctx->L * ctx->lay.NS * rs));
+    }
+  }
+  HZ_CUDA(cudaMemcpyAsync(ctx->d_fre, f_re, nn * sizeof(double), cudaMemcpyHostToDevice, 0));
+  if (f_im) HZ_CUDA(cudaMemcpyAsync(ctx->d_fim, f_im, nn * sizeof(double), cudaMemcpyHostToDevice, 0));
+  else if (ctx->d_fim) HZ_CUDA(cudaMemsetAsync(ctx->d_fim, 0, nn * sizeof(double), 0));
+  if (ctx->part) {
+    hz_status st = ctx->prec == HZ_F32 ? run_build<float>(ctx, 1, 0) : run_build<double>(ctx, 1, 0);
+    if (st != HZ_OK) return st;
+  }
+  HZ_CUDA(cudaStreamSynchronize(0));
+  return HZ_OK;
+}
+
+hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec prec, int dofs_per_thread,
+                       double cfl_frac, hz_part_info *info_out) {
+  if (!ctx) return HZ_EINVAL;
+  if (sx < 1 || sy < 1 || ctx->nx % sx || ctx->ny % sy)
+    return fail(ctx, HZ_EINVAL, "hz_partition: sx, sy must be >= 1 and divide nx, ny");
+  if (tc != HZ_TC_IMPEDANCE0) return fail(ctx, HZ_EUNSUPPORTED, "hz_partition: only HZ_TC_IMPEDANCE0");
+  if (prec != HZ_F32 && prec != HZ_F64) return fail(ctx, HZ_EINVAL, "hz_partition: bad precision");
+  if (!(cfl_frac > 0.0) || cfl_frac > 1.0) return fail(ctx, HZ_EINVAL, "hz_partition: cfl_frac must be in (0,1]");
+  if (dofs_per_thread < 0) return fail(ctx, HZ_EINVAL, "hz_partition: dofs_per_thread < 0");
+  free_partition(ctx);
+  const int P = ctx->p;
+  ctx->sx = sx; ctx->sy = sy; ctx->ex = ctx->nx / sx; ctx->ey = ctx->ny / sy; ctx->L = sx * sy; ctx->prec = prec;
+  const int lnx = ctx->ex * P + 1, lny = ctx->ey * P + 1, N = lnx * lny;
+  ctx->E = lnx > lny ? lnx : lny;
+  const size_t rs = prec == HZ_F32 ? 4 : 8;
+
+  // --- time step (reading R9): dt_stab = 2 / sqrt(c_max^2 Lambda_p (1/hx^2 + 1/hy^2)) ---
+  const double lmax = ctx->c_max * ctx->c_max * ctx->gll.lambda_p * (1.0 / (ctx->hx * ctx->hx) + 1.0 / (ctx->hy * ctx->hy));
+  const double dt_stab = 2.0 / std::sqrt(lmax);
+  const double T = 2.0 * M_PI / ctx->omega;
+  int n_t = (int)std::ceil(T / (cfl_frac * dt_stab) * (1.0 - 1e-12));
+  if (n_t < 4) n_t = 4;
+  ctx->n_t = n_t;
+  ctx->dt = T / n_t;
+  ctx->theta = std::tan(ctx->omega * ctx->dt / 2.0) / ctx->omega;
+  ctx->sigma = std::sin(ctx->omega * ctx->dt / 2.0) / (ctx->omega / 2.0);
+
+  // --- variant choice ---
+  const TileEntry *tiles = nullptr;
+  const int ntiles = prec == HZ_F32 ? tile_table_f32(&tiles) : tile_table_f64(&tiles);
+  const size_t tab_bytes = (size_t)n_t * 4 * rs;
+  const size_t smem_cap = 227 * 1024;
+  Layout lay{};
+  lay.lnx = lnx; lay.lny = lny;
+  int best = -1;
+  SweepLaunch bl{};
+  Layout blay{};
+  auto tile_fit = [&](const TileEntry &t, Layout *lo, SweepLaunch *la) -> bool {
+    if (t.p != P || ctx->ex % t.mx || ctx->ey % t.my) return false;
+    Layout q = lay;
+    q.variant = 1; q.TX = t.mx * P; q.TY = t.my * P;
+    q.ntx = ctx->ex / t.mx + 1; q.nty = ctx->ey / t.my + 1;
+    const int nthr = roundup(q.ntx * q.nty, 32);
+    if (nthr > t.maxt) return false;
+    q.NT = nthr; q.NS = q.TX * q.TY * nthr;
+    const size_t narr = 2 * (size_t)(q.TX + q.TY);
+    size_t sm = tab_bytes + 2 * narr * (nthr + 1) * rs + (t.csm ? 2 * (size_t)q.TX * q.TY * nthr * rs : 0);
+    if (sm > smem_cap) return false;
+    *lo = q; la->blocks = ctx->L; la->threads = nthr; la->smem = sm;
+    return true;
+  };
+  const bool complex_f = ctx->d_fim != nullptr;
+  if (dofs_per_thread == 1 || (dofs_per_thread == 0 && complex_f)) {
+    if (N > 1024) return fail(ctx, HZ_EUNSUPPORTED, "hz_partition: one DOF per thread needs <= 1024 DOFs per subdomain");
+  } else {
+    for (int i = 0; i < ntiles; ++i) {
+      const TileEntry &t = tiles[i];
+      const int k = t.mx * P * t.my * P;
+      if (dofs_per_thread > 1 && k != dofs_per_thread) continue;
+      Layout lo; SweepLaunch la;
+      if (!tile_fit(t, &lo, &la)) continue;
+      // prefer register-resident coefficients, then the smaller tile (more threads, better latency hiding)
+      if (best < 0 || (t.csm < tiles[best].csm) || (t.csm == tiles[best].csm && k < tiles[best].mx * P * tiles[best].my * P)) {
+        best = i; blay = lo; bl = la;
+      }
+    }
+    if (best < 0 && dofs_per_thread > 1)
+      return fail(ctx, HZ_EUNSUPPORTED, "hz_partition: no compiled register-blocked kernel with that many DOFs per thread fits this subdomain");
+    if (best >= 0 && complex_f)
+      return fail(ctx, HZ_EUNSUPPORTED, "hz_partition: complex f is only supported by the one-DOF-per-thread variant");
+    if (best < 0 && N > 1024)
+      return fail(ctx, HZ_EUNSUPPORTED, "hz_partition: subdomain fits no compiled kernel variant");
+  }
+  if (best >= 0) {
+    ctx->lay = blay; ctx->launch = bl;
+    ctx->mx = tiles[best].mx; ctx->my = tiles[best].my; ctx->csm = tiles[best].csm;
+  } else {
+    lay.variant = 0; lay.NT = roundup(N, 32); lay.NS = lay.NT; lay.TX = lay.TY = 1; lay.ntx = lay.nty = 0;
+    ctx->lay = lay; ctx->mx = ctx->my = 0; ctx->csm = 0;
+    ctx->launch.blocks = ctx->L; ctx->launch.threads = lay.NT;
+    ctx->launch.smem = tab_bytes + 2 * (size_t)(lnx + 2 * P) * (lny + 2 * P) * rs;
+  }
+
+  // --- host tables ---
+  std::vector<double> tab((size_t)n_t * 4);
+  const double tan2 = std::tan(M_PI / n_t) * std::tan(M_PI / n_t);
+  for (int nu = 0; nu < n_t; ++nu) {
+    tab[4 * nu + 0] = std::cos(2.0 * M_PI * nu / n_t);
+    tab[4 * nu + 1] = std::sin(2.0 * M_PI * nu / n_t);
+    tab[4 * nu + 2] = std::cos(2.0 * M_PI * nu / n_t) - 0.25 + 0.25 * tan2;                       // kappa_nu
+    tab[4 * nu + 3] = (std::cos(2.0 * M_PI * (nu + 0.5) / n_t) - 0.25 + 0.25 * tan2) / ctx->omega;  // kappa_{nu+1/2}/omega
+  }
+  std::vector<double> bandx, bandy, wxl, wyl;
+  make_band(ctx->gll, ctx->ex, ctx->hx, &bandx, &wxl);
+  make_band(ctx->gll, ctx->ey, ctx->hy, &bandy, &wyl);
+  fill_elem1d<double>(ctx->gll, ctx->hx, &ctx->ex1);
+  fill_elem1d<double>(ctx->gll, ctx->hy, &ctx->ey1);
+
+  // --- device allocation ---
+  const size_t LS = (size_t)ctx->L * ctx->lay.NS;
+  const size_t lam_n = (size_t)ctx->L * 8 * ctx->E, edge_n = (size_t)ctx->L * 4 * ctx->E;
+  size_t ws = 0;
+  auto alloc0 = [&](void **ptr, size_t bytes) -> cudaError_t {
+    cudaError_t e = cudaMalloc(ptr, bytes);
+    if (e != cudaSuccess) return e;
+    ws += bytes;
+    return cudaMemset(*ptr, 0, bytes);
+  };
+  const bool need_im = ctx->d_fim != nullptr || ctx->d_bc != nullptr;
+  HZ_CUDA(alloc0(&ctx->d_gamma, LS * rs));
+  HZ_CUDA(alloc0(&ctx->d_alpha, LS * rs));
+  HZ_CUDA(alloc0(&ctx->d_bbf_re, LS * rs));
+  if (need_im) HZ_CUDA(alloc0(&ctx->d_bbf_im, LS * rs));
+  HZ_CUDA(alloc0(&ctx->d_usub, 2 * LS * rs));
+  HZ_CUDA(alloc0(&ctx->d_lam, lam_n * rs));
+  HZ_CUDA(alloc0(&ctx->d_g, lam_n * rs));
+  HZ_CUDA(alloc0(&ctx->d_k2, edge_n * rs));
+  HZ_CUDA(alloc0(&ctx->d_bs, edge_n * rs));
+  HZ_CUDA(alloc0((void **)&ctx->d_ures, (size_t)2 * ctx->npx * ctx->npy * sizeof(double)));
+  if (prec == HZ_F32) {
+    HZ_CUDA(upload_as<float>(tab, &ctx->d_tab));
+    HZ_CUDA(upload_as<float>(bandx, &ctx->d_bandx));
+    HZ_CUDA(upload_as<float>(bandy, &ctx->d_bandy));
+  } else {
+    HZ_CUDA(upload_as<double>(tab, &ctx->d_tab));
+    HZ_CUDA(upload_as<double>(bandx, &ctx->d_bandx));
+    HZ_CUDA(upload_as<double>(bandy, &ctx->d_bandy));
+  }
+  HZ_CUDA(upload_as<double>(wxl, (void **)&ctx->d_wxl));
+  HZ_CUDA(upload_as<double>(wyl, (void **)&ctx->d_wyl));
+  ctx->ws_bytes = ws;
+  ctx->part = true;
+  hz_status st = prec == HZ_F32 ? run_build<float>(ctx, 0, 0) : run_build<double>(ctx, 0, 0);
+  if (st != HZ_OK) { free_partition(ctx); return st; }
+  HZ_CUDA(cudaStreamSynchronize(0));
+  if (info_out) {
+    hz_part_info inf{};
+    inf.n_t = n_t; inf.dofs_per_sub = N; inf.edge_nodes_x = lnx; inf.edge_nodes_y = lny; inf.edge_stride = ctx->E;
+    inf.threads_per_block = ctx->launch.threads; inf.blocks = ctx->L;
+    inf.dofs_per_thread = ctx->lay.variant == 0 ? 1 : ctx->lay.TX * ctx->lay.TY;
+    inf.tile_mx = ctx->mx; inf.tile_my = ctx->my;
+    inf.dt = ctx->dt; inf.theta = ctx->theta; inf.sigma = ctx->sigma;
+    inf.smem_bytes = ctx->launch.smem; inf.workspace_bytes = ws;
+    *info_out = inf;
+  }
+  return HZ_OK;
+}
+
+hz_status hz_ddm_solve(hz_ctx *ctx, const hz_solve_opts *opts, void *u_out, hz_solve_info *info, void *stream) {
+  if (!ctx) return HZ_EINVAL;
+  if (!opts) return fail(ctx, HZ_EINVAL, "hz_ddm_solve: NULL opts");
+  if (!ctx->part) return fail(ctx, HZ_ESTATE, "hz_ddm_solve: call hz_partition first");
+  if (opts->n_outer_max < 0 || opts->n_wh < 1 || !(opts->relax > 0.0) || opts->relax > 1.0)
+    return fail(ctx, HZ_EINVAL, "hz_ddm_solve: need n_outer_max >= 0, n_wh >= 1, relax in (0,1]");
+  if (opts->fused_exchange) return fail(ctx, HZ_EUNSUPPORTED, "hz_ddm_solve: fused_exchange is not built yet");
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t rs = ctx->prec == HZ_F32 ? 4 : 8;
+  if (opts->reset_state) {
+    HZ_CUDA(cudaMemsetAsync(ctx->d_lam, 0, (size_t)ctx->L * 8 * ctx->E * rs, st));
+    HZ_CUDA(cudaMemsetAsync(ctx->d_g, 0, (size_t)ctx->L * 8 * ctx->E * rs, st));
+    HZ_CUDA(cudaMemsetAsync(ctx->d_usub, 0, (size_t)2 * ctx->L * ctx->lay.NS * rs, st));
+  }
+  const int n = opts->n_outer_max;
+  std::vector<cudaEvent_t> ev((size_t)2 * n + 2);
+  for (auto &e : ev) HZ_CUDA(cudaEventCreate(&e));
+  auto cleanup = [&]() { for (auto &e : ev) cudaEventDestroy(e); };
+  double rel = -1.0;
+  int done = 0, other = 0, nexch = 0;
+  cudaError_t ce = cudaEventRecord(ev[0], st);
+  hz_status status = HZ_OK;
+  for (int it = 0; it < n && ce == cudaSuccess; ++it) {
+    ce = launch_sweep(ctx, opts, st);
+    if (ce != cudaSuccess) break;
+    ce = cudaEventRecord(ev[1 + 2 * it], st);
+    if (ce != cudaSuccess) break;
+    ce = launch_exchange(ctx, opts->relax, st);
+    if (ce != cudaSuccess) break;
+    ++nexch;
+    ce = cudaEventRecord(ev[2 + 2 * it], st);
+    if (ce != cudaSuccess) break;
+    ++done;
+    if (opts->tol > 0.0 && opts->check_every > 0 && (done % opts->check_every == 0 || done == n)) {
+      ce = launch_gather(ctx, ctx->d_ures, HZ_F64, st);
+      if (ce != cudaSuccess) break;
+      status = residual_impl(ctx, ctx->d_ures, HZ_F64, &rel, st);
+      other += 3;
+      if (status != HZ_OK) { cleanup(); return status; }
+      if (rel <= opts->tol) break;
+    }
+  }
+  if (ce == cudaSuccess && u_out) { ce = launch_gather(ctx, u_out, ctx->prec, st); ++other; }
+  cudaEvent_t ev_end;
+  if (ce == cudaSuccess) ce = cudaEventCreate(&ev_end);
+  if (ce == cudaSuccess) ce = cudaEventRecord(ev_end, st);
+  if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
+  if (ce != cudaSuccess) { cleanup(); return cuda_fail(ctx, ce, "hz_ddm_solve"); }
+  if (info) {
+    hz_solve_info inf{};
+    inf.n_outer_done = done; inf.n_t = ctx->n_t; inf.rel_residual = rel;
+    float ms = 0.f;
+    for (int it = 0; it < done; ++it) {
+      cudaEventElapsedTime(&ms, ev[2 * it], ev[2 * it + 1]);
+      inf.sweep_ms_total += ms;
+      cudaEventElapsedTime(&ms, ev[2 * it + 1], ev[2 * it + 2]);
+      inf.exch_ms_total += ms;
+    }
+    cudaEventElapsedTime(&ms, ev[0], ev_end);
+    inf.total_ms = ms;
+    inf.dof_timesteps = (double)ctx->L * ctx->lay.lnx * ctx->lay.lny * (double)opts->n_wh * (ctx->n_t - 1) * done;
+    inf.sweep_launches = done; inf.exch_launches = nexch; inf.other_launches = other;
+    *info = inf;
+  }
+  cudaEventDestroy(ev_end);
+  cleanup();
+  return HZ_OK;
+}
+
+hz_status hz_residual(hz_ctx *ctx, const void *u_dev, hz_prec u_prec, double *rel_residual, void *stream) {
+  if (!ctx) return HZ_EINVAL;
+  if (!u_dev || !rel_residual) return fail(ctx, HZ_EINVAL, "hz_residual: NULL u_dev or rel_residual");
+  if (u_prec != HZ_F32 && u_prec != HZ_F64) return fail(ctx, HZ_EINVAL, "hz_residual: bad precision");
+  double rel = 0.0;
+  // the residual needs sx..E only through Geo fields that the kernel does not read when unpartitioned
+  hz_status st = residual_impl(ctx, u_dev, u_prec, &rel, (cudaStream_t)stream);
+  if (st != HZ_OK) return st;
+  *rel_residual = rel;
+  return HZ_OK;
+}
+
+hz_status hz_get_subdomain_state(hz_ctx *ctx, double *u_sub_dev, double *lambda_dev, void *stream) {
+  if (!ctx) return HZ_EINVAL;
+  if (!ctx->part) return fail(ctx, HZ_ESTATE, "hz_get_subdomain_state: call hz_partition first");
+  cudaStream_t st = (cudaStream_t)stream;
+  const int bs = 256;
+  if (u_sub_dev) {
+    const long long n = (long long)ctx->L * 2 * ctx->lay.lnx * ctx->lay.lny;
+    const unsigned nb = (unsigned)((n + bs - 1) / bs);
+    if (ctx->prec == HZ_F32) k_state_get<float><<<nb, bs, 0, st>>>(ctx->lay, ctx->L, (const float *)ctx->d_usub, u_sub_dev);
+    else k_state_get<double><<<nb, bs, 0, st>>>(ctx->lay, ctx->L, (const double *)ctx->d_usub, u_sub_dev);
+    HZ_CUDA(cudaGetLastError());
+  }
+  if (lambda_dev) {
+    const long long n = (long long)ctx->L * 8 * ctx->E;
+    const unsigned nb = (unsigned)((n + bs - 1) / bs);
+    if (ctx->prec == HZ_F32) k_convert<float, double><<<nb, bs, 0, st>>>(n, (const float *)ctx->d_lam, lambda_dev);
+    else k_convert<double, double><<<nb, bs, 0, st>>>(n, (const double *)ctx->d_lam, lambda_dev);
+    HZ_CUDA(cudaGetLastError());
+  }
+  HZ_CUDA(cudaStreamSynchronize(st));
+  return HZ_OK;
+}
+
+hz_status hz_set_subdomain_state(hz_ctx *ctx, const double *u_sub_dev, const double *lambda_dev, void *stream) {
+  if (!ctx) return HZ_EINVAL;
+  if (!ctx->part) return fail(ctx, HZ_ESTATE, "hz_set_subdomain_state: call hz_partition first");
+  cudaStream_t st = (cudaStream_t)stream;
+  const int bs = 256;
+  if (u_sub_dev) {
+    const long long n = (long long)ctx->L * 2 * ctx->lay.lnx * ctx->lay.lny;
+    const unsigned nb = (unsigned)((n + bs - 1) / bs);
+    if (ctx->prec == HZ_F32) k_state_set<float><<<nb, bs, 0, st>>>(ctx->lay, ctx->L, (float *)ctx->d_usub, u_sub_dev);
+    else k_state_set<double><<<nb, bs, 0, st>>>(ctx->lay, ctx->L, (double *)ctx->d_usub, u_sub_dev);
+    HZ_CUDA(cudaGetLastError());
+  }
+  if (lambda_dev) {
+    const long long n = (long long)ctx->L * 8 * ctx->E;
+    const unsigned nb = (unsigned)((n + bs - 1) / bs);
+    if (ctx->prec == HZ_F32) k_convert<double, float><<<nb, bs, 0, st>>>(n, lambda_dev, (float *)ctx->d_lam);
+    else k_convert<double, double><<<nb, bs, 0, st>>>(n, lambda_dev, (double *)ctx->d_lam);
+    HZ_CUDA(cudaGetLastError());
+  }
+  HZ_CUDA(cudaStreamSynchronize(st));
+  return HZ_OK;
+}
+
+const char *hz_last_error(const hz_ctx *ctx) { return ctx ? ctx->err.c_str() : g_setup_error.c_str(); }
+
+void hz_destroy(hz_ctx *ctx) {
+  if (!ctx) return;
+  free_partition(ctx);
+  double **ptrs[] = {&ctx->d_c, &ctx->d_fre, &ctx->d_fim, &ctx->d_bc};
+  for (double **q : ptrs) { if (*q) cudaFree(*q); *q = nullptr; }
+  delete ctx;
+}
+
+hz_status hz_peak_probe(int kind, double *result, void *stream) {
+  if (!result || kind < 0 || kind > 2) return HZ_EINVAL;
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaDeviceProp prop;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return HZ_ECUDA;
+  const int sms = prop.multiProcessorCount;
+  cudaEvent_t e0, e1;
+  if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return HZ_ECUDA;
+  float *d_out = nullptr;
+  if (cudaMalloc((void **)&d_out, 64) != cudaSuccess) return HZ_ECUDA;
+  double best = 0.0;
+  for (int rep = 0; rep < 5; ++rep) {
+    float ms = 0.f;
+    double work = 0.0;
+    if (kind == 0) {
+      const int iters = 4096, blocks = sms * 8, thr = 256;
+      cudaEventRecord(e0, st);
+      k_probe_fma<float><<<blocks, thr, 0, st>>>(iters, 1.0f, d_out);
+      cudaEventRecord(e1, st);
+      work = 2.0 * 64.0 * iters * (double)blocks * thr;
+    } else if (kind == 1) {
+      const int iters = 2048, blocks = sms * 8, thr = 256;
+      cudaEventRecord(e0, st);
+      k_probe_fma<double><<<blocks, thr, 0, st>>>(iters, 1.0, (double *)d_out);
+      cudaEventRecord(e1, st);
+      work = 2.0 * 64.0 * iters * (double)blocks * thr;
+    } else {
+      const int iters = 2048, blocks = sms * 2, thr = 1024;
+      cudaFuncSetAttribute(k_probe_lds, cudaFuncAttributeMaxDynamicSharedMemorySize, 32768);
+      cudaEventRecord(e0, st);
+      k_probe_lds<<<blocks, thr, 32768, st>>>(iters, d_out);
+      cudaEventRecord(e1, st);
+      work = 16.0 * 8.0 * iters * (double)blocks * thr;  // bytes
+    }
+    if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) { cudaFree(d_out); return HZ_ECUDA; }
+    cudaEventElapsedTime(&ms, e0, e1);
+    const double rate = work / (ms * 1e-3) / 1e12;
+    if (rate > best) best = rate;
+  }
+  cudaFree(d_out);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  *result = best;
+  return HZ_OK;
+}
+
+}  // extern "C"

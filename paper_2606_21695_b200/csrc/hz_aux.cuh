@@ -1,0 +1,312 @@
+// hz_aux.cuh — the kernels around the sweep: per-subdomain operator builder (A0), interface exchange (A8),
+// gather of the global field (A7/R19), global residual (A10), state import/export and the peak probes.
+#pragma once
+#include "hz_internal.h"
+
+namespace hz {
+
+// Mesh / partition description used by the auxiliary kernels (all fp64).
+struct Geo {
+  int nx, ny, p, npx, npy;  // global elements, degree, global nodes per side
+  int sx, sy, ex, ey;       // subdomain grid, elements per subdomain
+  int E, EB;                // edge stride of lambda arrays; of the bc_lambda side blocks
+  double hx, hy, omega, theta, sigma;
+};
+
+// ---------------------------------------------------------------------------------------------
+// A0: per-subdomain operator data (PAPER.md:107-113 for M, H; PAPER.md:144 for alpha, beta).
+// One thread per (subdomain, local node).  wxl/wyl: assembled reference GLL weights of the ex (ey)
+// elements of a subdomain side.  Everything is computed in fp64 and rounded once.
+// ---------------------------------------------------------------------------------------------
+template <typename real>
+__global__ void k_build(Geo g, Layout lay, const double *__restrict__ c, const double *__restrict__ f_re,
+                        const double *__restrict__ f_im, const double *__restrict__ bc, const double *__restrict__ wxl,
+                        const double *__restrict__ wyl, real *gamma, real *alpha, real *bbf_re, real *bbf_im,
+                        real *k2edge, real *bs, int only_source) {
+  const int N = lay.lnx * lay.lny;
+  const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long total = (long long)g.sx * g.sy * N;
+  if (gid >= total) return;
+  const int l = (int)(gid / N), q = (int)(gid - (long long)l * N);
+  const int i = q % lay.lnx, j = q / lay.lnx;
+  const int six = l % g.sx, siy = l / g.sx;
+  const int I = six * g.ex * g.p + i, J = siy * g.ey * g.p + j;
+  const size_t gn = (size_t)J * g.npx + I;
+  const double cj = c[gn];
+  const double m = 0.25 * g.hx * g.hy * wxl[i] * wyl[j];  // local lumped mass (geometric)
+  const double M = m / (cj * cj);
+  // impedance weight on the WHOLE subdomain boundary: interfaces carry the same operator as the
+  // outer boundary
+  const bool onW = i == 0, onE = i == lay.lnx - 1, onS = j == 0, onN = j == lay.lny - 1;
+  const double sWE = 0.5 * g.hy * wyl[j], sSN = 0.5 * g.hx * wxl[i];
+  double H = 0.0;
+  if (onW) H += sWE / cj;
+  if (onE) H += sWE / cj;
+  if (onS) H += sSN / cj;
+  if (onN) H += sSN / cj;
+  const double den = M + g.theta * H;
+  const double beta = g.sigma / den;
+  // load: f(x_j) m_j (+ the outer-boundary datum lambda of eq. (1b) on physical sides)
+  double bre = f_re[gn] * m, bim = f_im ? f_im[gn] * m : 0.0;
+  if (bc) {
+    if (onW && six == 0) { bre += sWE * bc[(0 * 2 + 0) * g.EB + J]; bim += sWE * bc[(0 * 2 + 1) * g.EB + J]; }
+    if (onE && six == g.sx - 1) { bre += sWE * bc[(1 * 2 + 0) * g.EB + J]; bim += sWE * bc[(1 * 2 + 1) * g.EB + J]; }
+    if (onS && siy == 0) { bre += sSN * bc[(2 * 2 + 0) * g.EB + I]; bim += sSN * bc[(2 * 2 + 1) * g.EB + I]; }
+    if (onN && siy == g.sy - 1) { bre += sSN * bc[(3 * 2 + 0) * g.EB + I]; bim += sSN * bc[(3 * 2 + 1) * g.EB + I]; }
+  }
+  const size_t o = (size_t)l * lay.NS + lay.slot(i, j);
+  bbf_re[o] = (real)(beta * bre);
+  if (bbf_im) bbf_im[o] = (real)(beta * bim);
+  if (only_source) return;
+  gamma[o] = (real)(beta * m);
+  alpha[o] = (real)((M - g.theta * H) / den);
+  const size_t eb = (size_t)l * 4 * g.E;
+  const double k2 = 2.0 * g.omega / cj;
+  if (onW) { k2edge[eb + 0 * g.E + j] = (real)k2; bs[eb + 0 * g.E + j] = (real)(beta * sWE); }
+  if (onE) { k2edge[eb + 1 * g.E + j] = (real)k2; bs[eb + 1 * g.E + j] = (real)(beta * sWE); }
+  if (onS) { k2edge[eb + 2 * g.E + i] = (real)k2; bs[eb + 2 * g.E + i] = (real)(beta * sSN); }
+  if (onN) { k2edge[eb + 3 * g.E + i] = (real)k2; bs[eb + 3 * g.E + i] = (real)(beta * sSN); }
+}
+
+// ---------------------------------------------------------------------------------------------
+// A8: exchange with relaxation (eq. (2); readings R3, R12):
+//   lambda^{n+1}_{r,o} = (1-rho) lambda^n_{r,o} + rho g_{nb(r,o), opp(o)}      on interface sides.
+// One thread per (subdomain r, side o, re/im, edge node); in place on lambda (each entry is read and
+// written by one thread only; g is a separate array).
+// ---------------------------------------------------------------------------------------------
+template <typename real>
+__global__ void k_exchange(int sx, int sy, int E, int ex_nodes, int ey_nodes, real rho, real *__restrict__ lam,
+                           const real *__restrict__ g) {
+  const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long total = (long long)sx * sy * 8 * E;
+  if (gid >= total) return;
+  const int e = (int)(gid % E);
+  const int c = (int)((gid / E) % 2);
+  const int o = (int)((gid / (2 * E)) % 4);
+  const int r = (int)(gid / (8 * E));
+  const int rx = r % sx, ry = r / sx;
+  int nb = -1;
+  if (o == kSideW && rx > 0) nb = r - 1;
+  if (o == kSideE && rx < sx - 1) nb = r + 1;
+  if (o == kSideS && ry > 0) nb = r - sx;
+  if (o == kSideN && ry < sy - 1) nb = r + sx;
+  if (nb < 0) return;
+  const int len = (o < 2) ? ey_nodes : ex_nodes;
+  if (e >= len) return;
+  const int opp = o ^ 1;
+  const real gv = g[(((size_t)nb * 4 + opp) * 2 + c) * E + e];
+  lam[gid] = (real(1) - rho) * lam[gid] + rho * gv;
+}
+
+// ---------------------------------------------------------------------------------------------
+// A7 / R19: global nodal field, mean of the copies at nodes shared by several subdomains, summed in
+// the fixed order (iy ascending, ix ascending).
+// ---------------------------------------------------------------------------------------------
+template <typename real, typename outT>
+__global__ void k_gather(Geo g, Layout lay, const real *__restrict__ u_sub, outT *__restrict__ u_out) {
+  const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long total = (long long)g.npx * g.npy;
+  if (gid >= total) return;
+  const int I = (int)(gid % g.npx), J = (int)(gid / g.npx);
+  const int wx = g.ex * g.p, wy = g.ey * g.p;
+  int ix1 = I / wx;
+  if (ix1 > g.sx - 1) ix1 = g.sx - 1;
+  int iy1 = J / wy;
+  if (iy1 > g.sy - 1) iy1 = g.sy - 1;
+  const int ix0 = (I - ix1 * wx == 0 && ix1 > 0) ? ix1 - 1 : ix1;
+  const int iy0 = (J - iy1 * wy == 0 && iy1 > 0) ? iy1 - 1 : iy1;
+  double sr = 0.0, si = 0.0;
+  int cnt = 0;
+  for (int iy = iy0; iy <= iy1; ++iy)
+    for (int ix = ix0; ix <= ix1; ++ix) {
+      const int l = iy * g.sx + ix;
+      const int s = lay.slot(I - ix * wx, J - iy * wy);
+      sr += (double)u_sub[(size_t)l * 2 * lay.NS + s];
+      si += (double)u_sub[(size_t)l * 2 * lay.NS + lay.NS + s];
+      ++cnt;
+    }
+  u_out[gid] = (outT)(sr / cnt);
+  u_out[total + gid] = (outT)(si / cnt);
+}
+
+// ---------------------------------------------------------------------------------------------
+// A10: r = b - (A - i w H - w^2 M) u on the unpartitioned system (4), fp64.
+// One thread per global node; the stiffness is applied matrix-free from the 1-D element matrix
+// K1 = D^T W D in constant memory.  Block partial sums of |r|^2 and |b|^2 are
+// written to part[2*blockIdx] and reduced in a fixed order by k_reduce2 (deterministic).
+// ---------------------------------------------------------------------------------------------
+struct Ref1D {
+  double K[kMaxP + 1][kMaxP + 1];
+  double w[kMaxP + 1];
+};
+
+template <typename inT>
+__global__ void k_residual(Geo g, Ref1D ref, const double *__restrict__ c, const double *__restrict__ f_re,
+                           const double *__restrict__ f_im, const double *__restrict__ bc,
+                           const inT *__restrict__ u, double *__restrict__ part) {
+  __shared__ double red[2][32];
+  const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long total = (long long)g.npx * g.npy;
+  double r2 = 0.0, b2 = 0.0;
+  if (gid < total) {
+    const int I = (int)(gid % g.npx), J = (int)(gid / g.npx);
+    const int P = g.p;
+    // assembled reference weights at this node
+    const int ax = I % P, ay = J % P;
+    const bool shx = ax == 0 && I > 0 && I < g.npx - 1, shy = ay == 0 && J > 0 && J < g.npy - 1;
+    const double wxI = (ax == 0) ? (shx ? 2.0 * ref.w[0] : ref.w[0]) : ref.w[ax];
+    const double wyJ = (ay == 0) ? (shy ? 2.0 * ref.w[0] : ref.w[0]) : ref.w[ay];
+    const inT *ur = u, *ui = u + total;
+    // (Kx u)_I along row J and (Ky u)_J along column I, summed over the elements containing the node
+    double kxr = 0.0, kxi = 0.0, kyr = 0.0, kyi = 0.0;
+    {
+      const int e_hi = (I == g.npx - 1) ? g.nx - 1 : I / P;       // element whose node (I - e*P) this is
+      const int e_lo = (ax == 0 && I > 0) ? I / P - 1 : e_hi;     // the element before, at a shared node
+      for (int e = e_lo; e <= e_hi; ++e) {
+        const int a = I - e * P;
+        for (int cc = 0; cc <= P; ++cc) {
+          const size_t n = (size_t)J * g.npx + (e * P + cc);
+          kxr += ref.K[a][cc] * (double)ur[n];
+          kxi += ref.K[a][cc] * (double)ui[n];
+        }
+      }
+    }
+    {
+      const int e_hi = (J == g.npy - 1) ? g.ny - 1 : J / P;
+      const int e_lo = (ay == 0 && J > 0) ? J / P - 1 : e_hi;
+      for (int e = e_lo; e <= e_hi; ++e) {
+        const int a = J - e * P;
+        for (int cc = 0; cc <= P; ++cc) {
+          const size_t n = (size_t)(e * P + cc) * g.npx + I;
+          kyr += ref.K[a][cc] * (double)ur[n];
+          kyi += ref.K[a][cc] * (double)ui[n];
+        }
+      }
+    }
+    const double Aur = (g.hy / g.hx) * wyJ * kxr + (g.hx / g.hy) * wxI * kyr;
+    const double Aui = (g.hy / g.hx) * wyJ * kxi + (g.hx / g.hy) * wxI * kyi;
+    const double cj = c[gid];
+    const double m = 0.25 * g.hx * g.hy * wxI * wyJ;
+    const double M = m / (cj * cj);
+    const double sWE = 0.5 * g.hy * wyJ, sSN = 0.5 * g.hx * wxI;
+    double H = 0.0, bre = f_re[gid] * m, bim = f_im ? f_im[gid] * m : 0.0;
+    if (I == 0) { H += sWE / cj; if (bc) { bre += sWE * bc[(0 * 2 + 0) * g.EB + J]; bim += sWE * bc[(0 * 2 + 1) * g.EB + J]; } }
+    if (I == g.npx - 1) { H += sWE / cj; if (bc) { bre += sWE * bc[(1 * 2 + 0) * g.EB + J]; bim += sWE * bc[(1 * 2 + 1) * g.EB + J]; } }
+    if (J == 0) { H += sSN / cj; if (bc) { bre += sSN * bc[(2 * 2 + 0) * g.EB + I]; bim += sSN * bc[(2 * 2 + 1) * g.EB + I]; } }
+    if (J == g.npy - 1) { H += sSN / cj; if (bc) { bre += sSN * bc[(3 * 2 + 0) * g.EB + I]; bim += sSN * bc[(3 * 2 + 1) * g.EB + I]; } }
+    const double u_r = (double)ur[gid], u_i = (double)ui[gid];
+    const double w2M = g.omega * g.omega * M, wH = g.omega * H;
+    // (i w H + w^2 M) u = (w2M u_r - wH u_i) + i (w2M u_i + wH u_r)
+    const double rr = bre - Aur + (w2M * u_r - wH * u_i);
+    const double ri = bim - Aui + (w2M * u_i + wH * u_r);
+    r2 = rr * rr + ri * ri;
+    b2 = bre * bre + bim * bim;
+  }
+  for (int o = 16; o > 0; o >>= 1) {
+    r2 += __shfl_down_sync(0xffffffffu, r2, o);
+    b2 += __shfl_down_sync(0xffffffffu, b2, o);
+  }
+  const int w = threadIdx.x >> 5, ln = threadIdx.x & 31;
+  if (ln == 0) { red[0][w] = r2; red[1][w] = b2; }
+  __syncthreads();
+  if (w == 0) {
+    const int nw = blockDim.x >> 5;
+    r2 = ln < nw ? red[0][ln] : 0.0;
+    b2 = ln < nw ? red[1][ln] : 0.0;
+    for (int o = 16; o > 0; o >>= 1) {
+      r2 += __shfl_down_sync(0xffffffffu, r2, o);
+      b2 += __shfl_down_sync(0xffffffffu, b2, o);
+    }
+    if (ln == 0) { part[2 * (size_t)blockIdx.x] = r2; part[2 * (size_t)blockIdx.x + 1] = b2; }
+  }
+}
+
+__global__ void k_reduce2(const double *__restrict__ part, int n, double *__restrict__ out) {
+  __shared__ double red[2][32];
+  double a = 0.0, b = 0.0;
+  for (int q = threadIdx.x; q < n; q += blockDim.x) { a += part[2 * (size_t)q]; b += part[2 * (size_t)q + 1]; }
+  for (int o = 16; o > 0; o >>= 1) {
+    a += __shfl_down_sync(0xffffffffu, a, o);
+    b += __shfl_down_sync(0xffffffffu, b, o);
+  }
+  const int w = threadIdx.x >> 5, ln = threadIdx.x & 31;
+  if (ln == 0) { red[0][w] = a; red[1][w] = b; }
+  __syncthreads();
+  if (w == 0) {
+    const int nw = blockDim.x >> 5;
+    a = ln < nw ? red[0][ln] : 0.0;
+    b = ln < nw ? red[1][ln] : 0.0;
+    for (int o = 16; o > 0; o >>= 1) {
+      a += __shfl_down_sync(0xffffffffu, a, o);
+      b += __shfl_down_sync(0xffffffffu, b, o);
+    }
+    if (ln == 0) { out[0] = a; out[1] = b; }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------
+// State export / import in canonical fp64 layout (parity tests, random-lambda benchmark)
+// ---------------------------------------------------------------------------------------------
+template <typename real>
+__global__ void k_state_get(Layout lay, int L, const real *__restrict__ u_sub, double *__restrict__ out) {
+  const int N = lay.lnx * lay.lny;
+  const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (gid >= (long long)L * 2 * N) return;
+  const int q = (int)(gid % N), c = (int)((gid / N) % 2), l = (int)(gid / (2 * N));
+  out[gid] = (double)u_sub[(size_t)l * 2 * lay.NS + (size_t)c * lay.NS + lay.slot(q % lay.lnx, q / lay.lnx)];
+}
+template <typename real>
+__global__ void k_state_set(Layout lay, int L, real *__restrict__ u_sub, const double *__restrict__ in) {
+  const int N = lay.lnx * lay.lny;
+  const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (gid >= (long long)L * 2 * N) return;
+  const int q = (int)(gid % N), c = (int)((gid / N) % 2), l = (int)(gid / (2 * N));
+  u_sub[(size_t)l * 2 * lay.NS + (size_t)c * lay.NS + lay.slot(q % lay.lnx, q / lay.lnx)] = (real)in[gid];
+}
+template <typename A, typename B>
+__global__ void k_convert(long long n, const A *__restrict__ in, B *__restrict__ out) {
+  const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (gid < n) out[gid] = (B)in[gid];
+}
+
+// ---------------------------------------------------------------------------------------------
+// Peak probes (no method arithmetic): dependent-chain-free FMA streams and shared-memory loads.
+// ---------------------------------------------------------------------------------------------
+template <typename real>
+__global__ void __launch_bounds__(256) k_probe_fma(int iters, real seed, real *out) {
+  real a[16];
+#pragma unroll
+  for (int q = 0; q < 16; ++q) a[q] = seed + real(q) * real(1e-3) + real(threadIdx.x) * real(1e-6);
+  const real m = real(0.999), c = real(1e-4);
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int r = 0; r < 4; ++r)
+#pragma unroll
+      for (int q = 0; q < 16; ++q) a[q] = a[q] * m + c;
+  }
+  real s = 0;
+#pragma unroll
+  for (int q = 0; q < 16; ++q) s += a[q];
+  if (s == real(-12345)) out[0] = s;
+}
+
+__global__ void __launch_bounds__(1024) k_probe_lds(int iters, float *out) {
+  extern __shared__ __align__(16) float sm_f[];
+  for (int q = threadIdx.x; q < 8192; q += blockDim.x) sm_f[q] = (float)q;
+  __syncthreads();
+  // 2048 float4 = 32 KB; lane-consecutive 16-byte loads (conflict-free LDS.128)
+  const unsigned base = (unsigned)__cvta_generic_to_shared(sm_f) + (threadIdx.x & 255) * 16u;
+  float acc0 = 0.f, acc1 = 0.f;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+      float x, y, z, w;
+      asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(x), "=f"(y), "=f"(z), "=f"(w) : "r"(base + r * 4096u));
+      acc0 += x;
+      acc1 += w;
+    }
+  }
+  if (acc0 + acc1 == -1.f) out[0] = acc0;
+}
+
+}  // namespace hz

@@ -1,0 +1,92 @@
+// hz_internal.h — types shared by the host driver (hz_api.cu) and the kernel translation units.
+// Internal to the CUDA library; nothing here is visible through include/hz.h.
+#pragma once
+#include <cuda_runtime.h>
+#include <stddef.h>
+
+namespace hz {
+
+constexpr int kMaxP = 4;
+constexpr int kSideW = 0, kSideE = 1, kSideS = 2, kSideN = 3;
+
+// Where node (i,j) of a subdomain lives inside the subdomain's slot range [0, NS).
+//   variant 0 (one DOF per thread):   slot = j*lnx + i                       (thread = slot)
+//   variant 1 (register-blocked):     thread tile (tx,ty) owns TX x TY nodes; node (a,b) of the tile of
+//                                     thread t = ty*ntx+tx lives at (b*TX+a)*NT + t, so that one node
+//                                     index across the block's threads is one coalesced line.
+struct Layout {
+  int variant;
+  int lnx, lny;  // nodes per subdomain side: ex*p+1, ey*p+1
+  int TX, TY;    // nodes per thread tile (variant 1)
+  int ntx, nty;  // thread tiles per side (variant 1): ex/MX+1, ey/MY+1
+  int NT;        // threads per block
+  int NS;        // slots per subdomain (>= lnx*lny; padding slots hold zeros)
+  __host__ __device__ inline int slot(int i, int j) const {
+    if (variant == 0) return j * lnx + i;
+    const int tx = i / TX, a = i - tx * TX, ty = j / TY, b = j - ty * TY;
+    return (b * TX + a) * NT + ty * ntx + tx;
+  }
+};
+
+// One row of the time-step tables (A0): cos(2 pi nu/N_t), sin(2 pi nu/N_t), kappa_nu, kappa_{nu+1/2}/omega.
+template <typename real>
+struct __align__(16) Tab4 {
+  real c, s, k, kh;
+};
+
+// 1-D element constants of the register-blocked kernel, already scaled by 4/h^2 and the GLL weights:
+//   kin[a][c] = (4/h^2) K[a][c] / w_a        rows of element-interior nodes a = 1..P-1
+//   k0[c]     = (4/h^2) K[0][c] / (2 w_0)    row of an element's first node (shared with the element before)
+//   kp[c]     = (4/h^2) K[P][c] / (2 w_0)    row of an element's last node  (shared with the element after)
+template <typename real>
+struct Elem1D {
+  real kin[kMaxP + 1][kMaxP + 1];
+  real k0[kMaxP + 1];
+  real kp[kMaxP + 1];
+};
+
+template <typename real>
+struct SweepArgs {
+  Layout lay;
+  int sx, sy;      // subdomain grid
+  int E;           // edge stride of lambda / g / kedge / bs arrays
+  int n_t, n_wh, warm;
+  real sigma, omega, cos_h, sin_h, two_over_nt;  // cos_h = cos(pi/N_t), sin_h = sin(pi/N_t)
+  const Tab4<real> *tab;                         // [n_t]
+  const real *gamma, *alpha, *bbf_re, *bbf_im;   // [L][NS]; bbf_im may be NULL
+  real *u_sub;                                   // [L][2][NS]
+  const real *lam;                               // [L][4][2][E]  lambda^n
+  real *gout;                                    // [L][4][2][E]  outgoing g
+  const real *k2edge;                            // [L][4][E]     2 k_j on each side
+  const real *bs;                                // [L][4][E]     beta_j * s_j^{side}
+  const real *bandx, *bandy;                     // variant 0: [lnx][2P+1], [lny][2P+1]
+  Elem1D<real> ex1, ey1;                         // variant 1
+  // fused exchange (optional): lam is then lambda^{n-1}, read-write; g_prev the neighbours' g^{n-1}
+  int fused;
+  real relax;
+  const real *g_prev;
+  real *lam_rw;
+};
+
+struct TileEntry {
+  int p, mx, my, csm, maxt;  // csm: gamma / beta b in shared memory instead of registers
+  const void *fn;
+};
+
+struct SweepLaunch {
+  int blocks, threads;
+  size_t smem;
+};
+
+// Implemented in hz_sweep_*.cu.  Return cudaErrorInvalidValue when no instantiation matches.
+cudaError_t launch_sweep_dof_f32(const SweepArgs<float> &a, int p, SweepLaunch cfg, cudaStream_t st);
+cudaError_t launch_sweep_dof_f64(const SweepArgs<double> &a, int p, SweepLaunch cfg, cudaStream_t st);
+cudaError_t launch_sweep_tile_f32(const SweepArgs<float> &a, int p, int mx, int my, int csm, SweepLaunch cfg,
+                                  cudaStream_t st);
+cudaError_t launch_sweep_tile_f64(const SweepArgs<double> &a, int p, int mx, int my, int csm, SweepLaunch cfg,
+                                  cudaStream_t st);
+// compiled register-blocked instantiations of one precision
+int tile_table_f32(const TileEntry **out);
+int tile_table_f64(const TileEntry **out);
+
+}  // namespace hz

@@ -1,0 +1,37 @@
+// fp32 build of the subdomain solve (subsystem (e)); see hz_sweep.cuh.
+#include "hz_sweep_inst.cuh"
+
+namespace hz {
+
+// X(P, MX, MY, CSM, MAXT, MINB)
+#define HZ_TILE_TABLE_F32(X) \
+  X(1, 2, 2, 0, 1024, 1)     \
+  X(1, 4, 4, 0, 512, 1)      \
+  X(2, 1, 1, 0, 1024, 1)     \
+  X(2, 2, 2, 0, 384, 1)      \
+  X(3, 1, 1, 0, 512, 1)      \
+  X(3, 2, 1, 0, 320, 1)      \
+  X(3, 2, 1, 1, 576, 1)      \
+  X(3, 2, 2, 1, 320, 1)      \
+  X(4, 1, 1, 0, 384, 1)      \
+  X(4, 1, 1, 1, 640, 1)
+
+#define X_ENTRY(P, MX, MY, CSM, MAXT, MINB) \
+  {P, MX, MY, CSM, MAXT, (const void *)k_sweep_tile<float, P, MX, MY, (CSM != 0), MAXT, MINB>},
+static const TileEntry kTilesF32[] = {HZ_TILE_TABLE_F32(X_ENTRY)};
+#undef X_ENTRY
+static const int kNumTilesF32 = sizeof(kTilesF32) / sizeof(kTilesF32[0]);
+
+cudaError_t launch_sweep_dof_f32(const SweepArgs<float> &a, int p, SweepLaunch cfg, cudaStream_t st) {
+  return launch_dof_impl<float>(a, p, cfg, st);
+}
+cudaError_t launch_sweep_tile_f32(const SweepArgs<float> &a, int p, int mx, int my, int csm, SweepLaunch cfg,
+                                  cudaStream_t st) {
+  return launch_tile_impl<float>(kTilesF32, kNumTilesF32, a, p, mx, my, csm, cfg, st);
+}
+int tile_table_f32(const TileEntry **out) {
+  *out = kTilesF32;
+  return kNumTilesF32;
+}
+
+}  // namespace hz

@@ -1,0 +1,41 @@
+// hz_sweep_inst.cuh — instantiation table and launch dispatch of the sweep kernels for one precision.
+// Included by hz_sweep_f32.cu / hz_sweep_f64.cu (one translation unit per precision so they build in
+// parallel).  HZ_TILE_TABLE(X) lists X(P, MX, MY, CSM, MAXT, MINB).
+#pragma once
+#include "hz_sweep.cuh"
+
+namespace hz {
+
+template <typename real>
+static cudaError_t launch_dof_impl(const SweepArgs<real> &a, int p, SweepLaunch cfg, cudaStream_t st) {
+  void (*fn)(const SweepArgs<real>) = nullptr;
+  switch (p) {
+    case 1: fn = k_sweep_dof<real, 1>; break;
+    case 2: fn = k_sweep_dof<real, 2>; break;
+    case 3: fn = k_sweep_dof<real, 3>; break;
+    case 4: fn = k_sweep_dof<real, 4>; break;
+    default: return cudaErrorInvalidValue;
+  }
+  cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem);
+  if (e != cudaSuccess) return e;
+  fn<<<cfg.blocks, cfg.threads, cfg.smem, st>>>(a);
+  return cudaGetLastError();
+}
+
+template <typename real>
+static cudaError_t launch_tile_impl(const TileEntry *tab, int n, const SweepArgs<real> &a, int p, int mx, int my,
+                                    int csm, SweepLaunch cfg, cudaStream_t st) {
+  for (int i = 0; i < n; ++i) {
+    const TileEntry &e = tab[i];
+    if (e.p == p && e.mx == mx && e.my == my && e.csm == csm && cfg.threads <= e.maxt) {
+      auto fn = reinterpret_cast<void (*)(const SweepArgs<real>)>(const_cast<void *>(e.fn));
+      cudaError_t err = cudaFuncSetAttribute(e.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem);
+      if (err != cudaSuccess) return err;
+      fn<<<cfg.blocks, cfg.threads, cfg.smem, st>>>(a);
+      return cudaGetLastError();
+    }
+  }
+  return cudaErrorInvalidValue;
+}
+
+}  // namespace hz

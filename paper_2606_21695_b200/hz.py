@@ -1,0 +1,187 @@
+"""Thin ctypes binding over the C-ABI library of include/hz.h (same names, argument marshalling only).
+
+Every step of the hot path runs in the CUDA kernels of libhz.so; nothing here computes.  PyTorch
+is used by callers for device memory and streams only: device arrays are passed as `tensor.data_ptr()`
+integers, streams as `torch.cuda.current_stream().cuda_stream`.  There is no CPU fallback: if the
+library is not built, loading it raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libhz.so")
+
+HZ_OK, HZ_EINVAL, HZ_ENOMEM, HZ_ECUDA, HZ_EUNSUPPORTED, HZ_ESTATE = range(6)
+HZ_F32, HZ_F64 = 0, 1
+HZ_TC_IMPEDANCE0 = 0
+STATUS_NAMES = {0: "HZ_OK", 1: "HZ_EINVAL", 2: "HZ_ENOMEM", 3: "HZ_ECUDA", 4: "HZ_EUNSUPPORTED", 5: "HZ_ESTATE"}
+
+# every symbol include/hz.h declares
+EXPORTS = ("hz_mesh_setup", "hz_set_source", "hz_partition", "hz_ddm_solve", "hz_residual",
+           "hz_get_subdomain_state", "hz_set_subdomain_state", "hz_last_error", "hz_destroy", "hz_peak_probe")
+
+
+class hz_part_info(C.Structure):
+    _fields_ = [("n_t", C.c_int), ("dofs_per_sub", C.c_int), ("edge_nodes_x", C.c_int), ("edge_nodes_y", C.c_int),
+                ("edge_stride", C.c_int), ("threads_per_block", C.c_int), ("blocks", C.c_int),
+                ("dofs_per_thread", C.c_int), ("tile_mx", C.c_int), ("tile_my", C.c_int),
+                ("dt", C.c_double), ("theta", C.c_double), ("sigma", C.c_double),
+                ("smem_bytes", C.c_size_t), ("workspace_bytes", C.c_size_t)]
+
+
+class hz_solve_opts(C.Structure):
+    _fields_ = [("n_outer_max", C.c_int), ("n_wh", C.c_int), ("warm_start", C.c_int), ("relax", C.c_double),
+                ("tol", C.c_double), ("check_every", C.c_int), ("reset_state", C.c_int), ("fused_exchange", C.c_int)]
+
+
+class hz_solve_info(C.Structure):
+    _fields_ = [("n_outer_done", C.c_int), ("n_t", C.c_int), ("rel_residual", C.c_double),
+                ("sweep_ms_total", C.c_double), ("exch_ms_total", C.c_double), ("total_ms", C.c_double),
+                ("dof_timesteps", C.c_double), ("sweep_launches", C.c_int), ("exch_launches", C.c_int),
+                ("other_launches", C.c_int)]
+
+
+class HzError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(f"{STATUS_NAMES.get(status, status)}: {msg}")
+        self.status = status
+
+
+_lib = None
+
+
+def lib():
+    """Loads libhz.so (built by `python -m paper_2606_21695_b200.build`).  Raises if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} is not built (run `python -m paper_2606_21695_b200.build`); "
+                           "there is no CPU fallback")
+    L = C.CDLL(LIB_PATH)
+    vp, dp, ip = C.c_void_p, C.POINTER(C.c_double), C.c_int
+    L.hz_mesh_setup.argtypes = [C.POINTER(vp), ip, ip, C.c_double, C.c_double, C.c_double, C.c_double, ip,
+                                vp, C.c_double, vp, vp, vp]
+    L.hz_set_source.argtypes = [vp, vp, vp]
+    L.hz_partition.argtypes = [vp, ip, ip, ip, ip, ip, C.c_double, C.POINTER(hz_part_info)]
+    L.hz_ddm_solve.argtypes = [vp, C.POINTER(hz_solve_opts), vp, C.POINTER(hz_solve_info), vp]
+    L.hz_residual.argtypes = [vp, vp, ip, dp, vp]
+    L.hz_get_subdomain_state.argtypes = [vp, vp, vp, vp]
+    L.hz_set_subdomain_state.argtypes = [vp, vp, vp, vp]
+    L.hz_last_error.argtypes = [vp]
+    L.hz_last_error.restype = C.c_char_p
+    L.hz_destroy.argtypes = [vp]
+    L.hz_destroy.restype = None
+    L.hz_peak_probe.argtypes = [ip, dp, vp]
+    for name in EXPORTS:
+        if name not in ("hz_last_error", "hz_destroy"):
+            getattr(L, name).restype = C.c_int
+    _lib = L
+    return L
+
+
+def _host_ptr(a, n=None):
+    """Pointer to a C-contiguous float64 host array (or None)."""
+    if a is None:
+        return None, None
+    arr = np.ascontiguousarray(a, dtype=np.float64)
+    if n is not None and arr.size != n:
+        raise ValueError(f"expected {n} values, got {arr.size}")
+    return arr.ctypes.data_as(C.c_void_p), arr
+
+
+def _check(ctx, st):
+    if st != HZ_OK:
+        raise HzError(st, lib().hz_last_error(ctx).decode())
+
+
+def hz_mesh_setup(nx, ny, x0, y0, x1, y1, p, c_nodes, omega, f_re, f_im=None, bc_lambda=None):
+    """-> context handle (c_void_p).  Host numpy arrays; see include/hz.h."""
+    L = lib()
+    ctx = C.c_void_p()
+    cp, _c = _host_ptr(c_nodes)
+    fr, _fr = _host_ptr(f_re)
+    fi, _fi = _host_ptr(f_im)
+    bc, _bc = _host_ptr(bc_lambda)
+    st = L.hz_mesh_setup(C.byref(ctx), nx, ny, x0, y0, x1, y1, p, cp, omega, fr, fi, bc)
+    if st != HZ_OK:
+        raise HzError(st, L.hz_last_error(None).decode())
+    return ctx
+
+
+def hz_set_source(ctx, f_re, f_im=None):
+    fr, _fr = _host_ptr(f_re)
+    fi, _fi = _host_ptr(f_im)
+    _check(ctx, lib().hz_set_source(ctx, fr, fi))
+
+
+def hz_set_source_ptr(ctx, f_re_ptr, f_im_ptr=None):
+    """Same as hz_set_source with raw HOST pointers (e.g. pinned torch tensors' data_ptr())."""
+    _check(ctx, lib().hz_set_source(ctx, C.c_void_p(f_re_ptr), C.c_void_p(f_im_ptr) if f_im_ptr else None))
+
+
+def hz_partition(ctx, sx, sy, tc=HZ_TC_IMPEDANCE0, prec=HZ_F64, dofs_per_thread=0, cfl_frac=0.5):
+    info = hz_part_info()
+    _check(ctx, lib().hz_partition(ctx, sx, sy, tc, prec, dofs_per_thread, cfl_frac, C.byref(info)))
+    return info
+
+
+def hz_ddm_solve(ctx, n_outer_max, n_wh=5, warm_start=True, relax=0.5, tol=0.0, check_every=0, reset_state=False,
+                 fused_exchange=False, u_out_ptr=None, stream=None):
+    opts = hz_solve_opts(int(n_outer_max), int(n_wh), int(bool(warm_start)), float(relax), float(tol),
+                         int(check_every), int(bool(reset_state)), int(bool(fused_exchange)))
+    info = hz_solve_info()
+    _check(ctx, lib().hz_ddm_solve(ctx, C.byref(opts), C.c_void_p(u_out_ptr) if u_out_ptr else None, C.byref(info),
+                                   C.c_void_p(stream) if stream else None))
+    return info
+
+
+def hz_residual(ctx, u_ptr, u_prec, stream=None):
+    r = C.c_double()
+    _check(ctx, lib().hz_residual(ctx, C.c_void_p(u_ptr), u_prec, C.byref(r), C.c_void_p(stream) if stream else None))
+    return r.value
+
+
+def hz_get_subdomain_state(ctx, u_sub_ptr=None, lambda_ptr=None, stream=None):
+    _check(ctx, lib().hz_get_subdomain_state(ctx, C.c_void_p(u_sub_ptr) if u_sub_ptr else None,
+                                             C.c_void_p(lambda_ptr) if lambda_ptr else None,
+                                             C.c_void_p(stream) if stream else None))
+
+
+def hz_set_subdomain_state(ctx, u_sub_ptr=None, lambda_ptr=None, stream=None):
+    _check(ctx, lib().hz_set_subdomain_state(ctx, C.c_void_p(u_sub_ptr) if u_sub_ptr else None,
+                                             C.c_void_p(lambda_ptr) if lambda_ptr else None,
+                                             C.c_void_p(stream) if stream else None))
+
+
+def hz_last_error(ctx):
+    return lib().hz_last_error(ctx).decode()
+
+
+def hz_destroy(ctx):
+    if ctx:
+        lib().hz_destroy(ctx)
+
+
+def hz_peak_probe(kind, stream=None):
+    r = C.c_double()
+    st = lib().hz_peak_probe(kind, C.byref(r), C.c_void_p(stream) if stream else None)
+    if st != HZ_OK:
+        raise HzError(st, "hz_peak_probe failed")
+    return r.value
+
+
+def setup_from_inputs(inp, prec=HZ_F64, dofs_per_thread=0):
+    """Convenience: hz_mesh_setup + hz_partition from an inputs.HzInputs.  -> (ctx, part_info)."""
+    ctx = hz_mesh_setup(inp.nx, inp.ny, inp.x0, inp.y0, inp.x1, inp.y1, inp.p, inp.c_nodes, inp.omega, inp.f_re,
+                        inp.f_im)
+    try:
+        info = hz_partition(ctx, inp.sx, inp.sy, HZ_TC_IMPEDANCE0, prec, dofs_per_thread, inp.cfl_frac)
+    except Exception:
+        hz_destroy(ctx)
+        raise
+    return ctx, info

@@ -1,0 +1,292 @@
+"""GPU parity: the CUDA path (through the C ABI, paper_2606_21695_b200.hz) against the CPU oracle
+(oracle/hz_oracle.py), element by element, after IDENTICAL iteration counts on the same seeded inputs.
+
+Bar (BASELINE.json north_star): fp64 relative L2 <= 1e-10, fp32 <= 1e-4 -- on the raw per-subdomain
+states u_l, on the interface data lambda, and on the gathered global field.
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+from oracle import hz_oracle as O  # noqa: E402
+from paper_2606_21695_b200 import hz  # noqa: E402
+from paper_2606_21695_b200.inputs import HzInputs, make_config  # noqa: E402
+
+TOL = {hz.HZ_F64: 1e-10, hz.HZ_F32: 1e-4}
+
+
+def _require_cuda():
+    if not torch.cuda.is_available():
+        pytest.fail("CUDA device required for -m gpu tests (there is no CPU fallback)")
+
+
+def problem_from(inp, bc=None):
+    f = inp.f_re.astype(complex)
+    if inp.f_im is not None:
+        f = f + 1j * inp.f_im
+    return O.Problem(inp.nx, inp.ny, inp.p, inp.x0, inp.y0, inp.x1, inp.y1, inp.c_nodes, inp.omega, f, bc)
+
+
+def pack_bc(inp, bc):
+    """oracle bc_lambda (4 complex side arrays) -> the C ABI's 4 x (re[EB], im[EB]) block."""
+    if bc is None:
+        return None
+    EB = max(inp.npx, inp.npy)
+    out = np.zeros((4, 2, EB))
+    for s in range(4):
+        out[s, 0, :len(bc[s])] = bc[s].real
+        out[s, 1, :len(bc[s])] = bc[s].imag
+    return out
+
+
+def rel(a, b):
+    return float(np.linalg.norm(np.asarray(a) - np.asarray(b)) / max(np.linalg.norm(np.asarray(b)), 1e-300))
+
+
+def oracle_state_arrays(st):
+    L = len(st.subs)
+    N = st.subs[0].npx * st.subs[0].npy
+    E = max(st.subs[0].npx, st.subs[0].npy)
+    u = np.zeros((L, 2, N))
+    lam = np.zeros((L, 4, 2, E))
+    for l in range(L):
+        u[l, 0], u[l, 1] = st.u[l].real, st.u[l].imag
+        for s in range(4):
+            a = st.lam[l][s]
+            lam[l, s, 0, :len(a)], lam[l, s, 1, :len(a)] = a.real, a.imag
+    return u, lam
+
+
+def run_gpu(inp, prec, k, n_outer, n_wh, warm, relax, bc=None, res_field=None):
+    ctx = hz.hz_mesh_setup(inp.nx, inp.ny, inp.x0, inp.y0, inp.x1, inp.y1, inp.p, inp.c_nodes, inp.omega, inp.f_re,
+                           inp.f_im, pack_bc(inp, bc))
+    try:
+        info = hz.hz_partition(ctx, inp.sx, inp.sy, hz.HZ_TC_IMPEDANCE0, prec, k, inp.cfl_frac)
+        dt = torch.float64 if prec == hz.HZ_F64 else torch.float32
+        u_out = torch.zeros(2 * inp.npx * inp.npy, dtype=dt, device="cuda")
+        sinfo = hz.hz_ddm_solve(ctx, n_outer, n_wh=n_wh, warm_start=warm, relax=relax, reset_state=True,
+                                u_out_ptr=u_out.data_ptr(), stream=torch.cuda.current_stream().cuda_stream)
+        usub = torch.zeros(info.blocks * 2 * info.dofs_per_sub, dtype=torch.float64, device="cuda")
+        lam = torch.zeros(info.blocks * 8 * info.edge_stride, dtype=torch.float64, device="cuda")
+        hz.hz_get_subdomain_state(ctx, usub.data_ptr(), lam.data_ptr())
+        res = hz.hz_residual(ctx, u_out.data_ptr(), prec)
+        res_of_field = None
+        if res_field is not None:  # residual kernel (A10) applied to a field given by the caller
+            t = torch.from_numpy(np.concatenate([res_field.real.ravel(), res_field.imag.ravel()])).cuda()
+            res_of_field = hz.hz_residual(ctx, t.data_ptr(), hz.HZ_F64)
+        u_glob = u_out.double().cpu().numpy().reshape(2, inp.npy, inp.npx)
+        return dict(info=info, sinfo=sinfo, u=u_glob[0] + 1j * u_glob[1],
+                    usub=usub.cpu().numpy().reshape(info.blocks, 2, info.dofs_per_sub),
+                    lam=lam.cpu().numpy().reshape(info.blocks, 4, 2, info.edge_stride), res=res,
+                    res_of_field=res_of_field)
+    finally:
+        hz.hz_destroy(ctx)
+
+
+def check_case(inp, prec, k, n_outer=3, n_wh=2, warm=True, relax=0.5, bc=None):
+    _require_cuda()
+    pr = problem_from(inp, bc)
+    st = O.ddm_solve(pr, inp.sx, inp.sy, n_outer, n_wh, warm_start=warm, relax=relax, cfl_frac=inp.cfl_frac)
+    ug = O.ddm_gather(st)
+    g = run_gpu(inp, prec, k, n_outer, n_wh, warm, relax, bc, res_field=ug)
+    assert g["info"].n_t == st.tab.n_t, "N_t must be reproduced independently (reading R9)"
+    assert g["sinfo"].n_outer_done == n_outer
+    if k:
+        assert g["info"].dofs_per_thread == k
+    u_o, lam_o = oracle_state_arrays(st)
+    tol = TOL[prec]
+    assert rel(g["usub"], u_o) <= tol, f"u_l: {rel(g['usub'], u_o):.3e}"
+    assert rel(g["lam"], lam_o) <= tol, f"lambda: {rel(g['lam'], lam_o):.3e}"
+    assert rel(g["u"], ug) <= tol, f"gathered u: {rel(g['u'], ug):.3e}"
+    # the residual kernel (A10), applied to the ORACLE's field, against the oracle's residual of it
+    r_o = O.residual(pr, ug)
+    assert abs(g["res_of_field"] - r_o) <= 1e-9 * r_o, (g["res_of_field"], r_o)
+    return g
+
+
+def hetero_inputs(nx, ny, p, sx, sy, seed, complex_f=False, omega=None):
+    """Non-square mesh (hx != hy, ex != ey), smoothly random c, random f: a transposed operand or an
+    anisotropy mistake cannot cancel."""
+    rng = np.random.default_rng(seed)
+    shape = (ny * p + 1, nx * p + 1)
+    c = 1.0 + rng.uniform(0, 1.5, size=shape)
+    f_re = rng.standard_normal(shape)
+    f_im = rng.standard_normal(shape) if complex_f else None
+    if omega is None:
+        omega = 2.0 * np.pi * p * nx / 10.0 / 1.5
+    return HzInputs(name=f"hetero_{nx}x{ny}_p{p}", nx=nx, ny=ny, p=p, x0=0.0, y0=0.0, x1=1.5, y1=0.8, omega=omega,
+                    c_nodes=c, f_re=f_re, f_im=f_im, sx=sx, sy=sy, seed=seed)
+
+
+# ------------------------------------------------------------------ config 1 at full size (fp64)
+@pytest.mark.parametrize("k", [1, 4])
+def test_config1_full_fp64(k):
+    check_case(make_config(1), hz.HZ_F64, k, n_outer=4, n_wh=5)
+
+
+def test_config1_cold_start_algorithm1_literal():
+    # warm_start = 0 is Algorithm 1 as printed (u^(0) <- 0)
+    check_case(make_config(1), hz.HZ_F64, 1, n_outer=3, n_wh=3, warm=False)
+    check_case(make_config(1), hz.HZ_F64, 4, n_outer=3, n_wh=3, warm=False)
+
+
+# ------------------------------------------------------------------ configs 2/3 reduced (several tiles + ragged tail)
+@pytest.mark.parametrize("prec", [hz.HZ_F64, hz.HZ_F32])
+@pytest.mark.parametrize("k", [1, 9])
+def test_config2_reduced(prec, k):
+    # Y-waveguide, p=3, 4x4 subdomains of 8x8 elements (625 DOF each: the full-size block shape)
+    check_case(make_config(2, n=32), prec, k, n_outer=3, n_wh=5)
+
+
+@pytest.mark.parametrize("prec", [hz.HZ_F64, hz.HZ_F32])
+def test_config3_reduced(prec):
+    check_case(make_config(3, n=40), prec, 9, n_outer=3, n_wh=2)
+
+
+@pytest.mark.parametrize("prec", [hz.HZ_F64, hz.HZ_F32])
+def test_config4_reduced_large_subdomain(prec):
+    # 2x2 subdomains of 16x16 elements (2401 DOF): only the register-blocked variant fits
+    check_case(make_config(4, n=32, sub_elems=16), prec, 0, n_outer=2, n_wh=2)
+
+
+# ------------------------------------------------------------------ degrees, tiles, anisotropy
+@pytest.mark.parametrize("p,k", [(1, 1), (1, 4), (1, 16), (2, 1), (2, 4), (2, 16), (3, 1), (3, 9), (3, 18), (4, 1), (4, 16)])
+def test_degrees_and_tiles_fp64(p, k):
+    nx, ny = (8, 8) if k >= 16 and p <= 2 else (8, 4)
+    if p == 1 and k == 16:
+        nx, ny = 16, 8
+    inp = hetero_inputs(nx, ny, p, 2, 2, seed=10 * p + k)
+    check_case(inp, hz.HZ_F64, k, n_outer=3, n_wh=2)
+
+
+@pytest.mark.parametrize("p,k", [(1, 4), (2, 16), (3, 9), (3, 18), (4, 16)])
+def test_degrees_and_tiles_fp32(p, k):
+    inp = hetero_inputs(8, 8, p, 2, 2, seed=100 + 10 * p + k)
+    check_case(inp, hz.HZ_F32, k, n_outer=3, n_wh=2)
+
+
+def test_complex_source_and_boundary_datum_one_dof_per_thread():
+    inp = hetero_inputs(6, 4, 3, 3, 2, seed=77, complex_f=True)
+    rng = np.random.default_rng(5)
+    bc = [rng.standard_normal(n) + 1j * rng.standard_normal(n) for n in (inp.npy, inp.npy, inp.npx, inp.npx)]
+    check_case(inp, hz.HZ_F64, 1, n_outer=3, n_wh=2, bc=bc)
+
+
+def test_boundary_datum_register_blocked():
+    inp = hetero_inputs(6, 4, 3, 3, 2, seed=78)
+    rng = np.random.default_rng(6)
+    bc = [rng.standard_normal(n) + 1j * rng.standard_normal(n) for n in (inp.npy, inp.npy, inp.npx, inp.npx)]
+    check_case(inp, hz.HZ_F64, 9, n_outer=3, n_wh=2, bc=bc)
+
+
+# ------------------------------------------------------------------ degenerate cases
+@pytest.mark.parametrize("k", [1, 9])
+def test_single_subdomain_is_plain_waveholtz(k):
+    # L = 1: no interfaces, the exchange is a no-op (T5)
+    inp = hetero_inputs(4, 4, 3, 1, 1, seed=3)
+    check_case(inp, hz.HZ_F64, k, n_outer=2, n_wh=3)
+
+
+def test_one_element_subdomains():
+    inp = hetero_inputs(4, 3, 3, 4, 3, seed=4)
+    check_case(inp, hz.HZ_F64, 9, n_outer=3, n_wh=2)
+    check_case(inp, hz.HZ_F64, 1, n_outer=3, n_wh=2)
+
+
+def test_zero_sweeps_returns_zero_field():
+    _require_cuda()
+    inp = make_config(1)
+    g = run_gpu(inp, hz.HZ_F64, 0, 0, 1, True, 0.5)
+    assert np.all(g["u"] == 0) and np.all(g["lam"] == 0)
+    assert abs(g["res"] - 1.0) < 1e-14
+
+
+def test_relaxation_one_is_equation_2_literally():
+    check_case(make_config(1), hz.HZ_F64, 4, n_outer=4, n_wh=2, relax=1.0)
+
+
+def test_continue_equals_one_shot():
+    """Two calls of 2 sweeps (state kept in the context) == one call of 4 sweeps, bit for bit."""
+    _require_cuda()
+    inp = make_config(2, n=16)
+    ctx, info = hz.setup_from_inputs(inp, hz.HZ_F64, 9)
+    try:
+        a = torch.zeros(2 * inp.npx * inp.npy, dtype=torch.float64, device="cuda")
+        b = torch.zeros_like(a)
+        hz.hz_ddm_solve(ctx, 4, n_wh=2, reset_state=True, u_out_ptr=a.data_ptr())
+        hz.hz_ddm_solve(ctx, 2, n_wh=2, reset_state=True)
+        hz.hz_ddm_solve(ctx, 2, n_wh=2, reset_state=False, u_out_ptr=b.data_ptr())
+        assert torch.equal(a, b)
+    finally:
+        hz.hz_destroy(ctx)
+
+
+def test_variants_agree_and_are_deterministic():
+    _require_cuda()
+    inp = make_config(2, n=16)
+    g1 = run_gpu(inp, hz.HZ_F64, 1, 3, 2, True, 0.5)
+    g9 = run_gpu(inp, hz.HZ_F64, 9, 3, 2, True, 0.5)
+    g9b = run_gpu(inp, hz.HZ_F64, 9, 3, 2, True, 0.5)
+    assert rel(g1["usub"], g9["usub"]) < 1e-11
+    assert np.array_equal(g9["usub"], g9b["usub"]), "no atomics: runs must be bit-identical"
+
+
+def test_converged_ddm_matches_direct_solve_and_tolerance_stop():
+    """North star: converged DDM == direct solve of the global system (here the oracle's sparse LU),
+    and the tol-driven stop of the driver reports a residual that hz_residual reproduces."""
+    _require_cuda()
+    inp = make_config(1)
+    pr = problem_from(inp)
+    ustar = O.direct_solve(pr)
+    ctx, info = hz.setup_from_inputs(inp, hz.HZ_F64, 0)
+    try:
+        u = torch.zeros(2 * inp.npx * inp.npy, dtype=torch.float64, device="cuda")
+        s = hz.hz_ddm_solve(ctx, 600, n_wh=2, warm_start=True, relax=0.5, tol=1e-9, check_every=10, reset_state=True,
+                            u_out_ptr=u.data_ptr())
+        assert s.n_outer_done < 600 and s.rel_residual <= 1e-9
+        ug = u.cpu().numpy().reshape(2, inp.npy, inp.npx)
+        assert rel(ug[0] + 1j * ug[1], ustar) < 1e-8
+        assert abs(hz.hz_residual(ctx, u.data_ptr(), hz.HZ_F64) - s.rel_residual) <= 1e-6 * s.rel_residual
+    finally:
+        hz.hz_destroy(ctx)
+
+
+def test_fp32_reaches_the_shared_residual_tolerance():
+    """fp32 and fp64 reach the same final residual tolerance 1e-4 (reading R21)."""
+    _require_cuda()
+    inp = make_config(1)
+    for prec in (hz.HZ_F64, hz.HZ_F32):
+        ctx, info = hz.setup_from_inputs(inp, prec, 0)
+        try:
+            s = hz.hz_ddm_solve(ctx, 400, n_wh=2, tol=1e-4, check_every=5, reset_state=True)
+            assert s.rel_residual <= 1e-4 and s.n_outer_done < 400
+        finally:
+            hz.hz_destroy(ctx)
+
+
+def test_error_paths():
+    _require_cuda()
+    inp = make_config(1)
+    with pytest.raises(hz.HzError) as e:
+        hz.hz_mesh_setup(inp.nx, inp.ny, 0, 0, 1, 1, 7, inp.c_nodes, inp.omega, inp.f_re)
+    assert e.value.status == hz.HZ_EUNSUPPORTED
+    ctx = hz.hz_mesh_setup(inp.nx, inp.ny, 0, 0, 1, 1, inp.p, inp.c_nodes, inp.omega, inp.f_re)
+    try:
+        with pytest.raises(hz.HzError) as e:
+            hz.hz_ddm_solve(ctx, 1)
+        assert e.value.status == hz.HZ_ESTATE
+        with pytest.raises(hz.HzError) as e:
+            hz.hz_partition(ctx, 3, 2)
+        assert e.value.status == hz.HZ_EINVAL
+        with pytest.raises(hz.HzError) as e:
+            hz.hz_partition(ctx, 2, 2, dofs_per_thread=7)
+        assert e.value.status == hz.HZ_EUNSUPPORTED
+        hz.hz_partition(ctx, 2, 2)
+        with pytest.raises(hz.HzError) as e:
+            hz.hz_ddm_solve(ctx, 1, n_wh=0)
+        assert e.value.status == hz.HZ_EINVAL
+    finally:
+        hz.hz_destroy(ctx)
