@@ -137,7 +137,7 @@ struct hz_ctx {
   // partition
   bool part = false;
   int sx = 0, sy = 0, ex = 0, ey = 0, L = 0, E = 0, prec = 0;
-  int mx = 0, my = 0, csm = 0;
+  int mx = 0, my = 0, csm = 0, ws = 0;
   Layout lay{};
   SweepLaunch launch{};
   int n_t = 0;
@@ -264,11 +264,11 @@ cudaError_t launch_sweep(const hz_ctx *c, const hz_solve_opts *o, cudaStream_t s
   if (c->prec == HZ_F32) {
     SweepArgs<float> a = make_args<float>(c, o);
     return c->lay.variant == 0 ? launch_sweep_dof_f32(a, c->p, c->launch, st)
-                               : launch_sweep_tile_f32(a, c->p, c->mx, c->my, c->csm, c->launch, st);
+                               : launch_sweep_tile_f32(a, c->p, c->mx, c->my, c->csm, c->ws, c->launch, st);
   }
   SweepArgs<double> a = make_args<double>(c, o);
   return c->lay.variant == 0 ? launch_sweep_dof_f64(a, c->p, c->launch, st)
-                             : launch_sweep_tile_f64(a, c->p, c->mx, c->my, c->csm, c->launch, st);
+                             : launch_sweep_tile_f64(a, c->p, c->mx, c->my, c->csm, c->ws, c->launch, st);
 }
 
 cudaError_t launch_exchange(const hz_ctx *c, double rho, cudaStream_t st) {
@@ -444,16 +444,26 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
   int best = -1;
   SweepLaunch bl{};
   Layout blay{};
+  const char *env_ws = std::getenv("HZ_DISABLE_WS");  // debug knob: force the non-specialised tile kernel
+  const bool no_ws = env_ws && env_ws[0] == '1';
   auto tile_fit = [&](const TileEntry &t, Layout *lo, SweepLaunch *la) -> bool {
     if (t.p != P || ctx->ex % t.mx || ctx->ey % t.my) return false;
     Layout q = lay;
     q.variant = 1; q.TX = t.mx * P; q.TY = t.my * P;
     q.ntx = ctx->ex / t.mx + 1; q.nty = ctx->ey / t.my + 1;
-    const int nthr = roundup(q.ntx * q.nty, 32);
-    if (nthr > t.maxt) return false;
-    q.NT = nthr; q.NS = q.TX * q.TY * nthr;
+    const int ntv = roundup(q.ntx * q.nty, 32);   // virtual tile slots (stride of the per-node arrays)
+    int nthr = ntv;
+    size_t sm = 0;
     const size_t narr = 2 * (size_t)(q.TX + q.TY);
-    size_t sm = tab_bytes + 2 * narr * (nthr + 1) * rs + (t.csm ? 2 * (size_t)q.TX * q.TY * nthr * rs : 0);
+    if (t.ws) {
+      if (no_ws) return false;
+      nthr = roundup((q.ntx - 1) * (q.nty - 1), 32) + roundup(q.ntx + q.nty - 1, 32);
+      sm = tab_bytes + 2 * (size_t)(ntv + 64) * (narr + 1) * rs + (t.csm ? 2 * (size_t)q.TX * q.TY * nthr * rs : 0);
+    } else {
+      sm = tab_bytes + 2 * narr * (nthr + 1) * rs + (t.csm ? 2 * (size_t)q.TX * q.TY * nthr * rs : 0);
+    }
+    if (nthr > t.maxt) return false;
+    q.NT = ntv; q.NS = q.TX * q.TY * ntv;
     if (sm > smem_cap) return false;
     *lo = q; la->blocks = ctx->L; la->threads = nthr; la->smem = sm;
     return true;
@@ -468,8 +478,12 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
       if (dofs_per_thread > 1 && k != dofs_per_thread) continue;
       Layout lo; SweepLaunch la;
       if (!tile_fit(t, &lo, &la)) continue;
-      // prefer register-resident coefficients, then the smaller tile (more threads, better latency hiding)
-      if (best < 0 || (t.csm < tiles[best].csm) || (t.csm == tiles[best].csm && k < tiles[best].mx * P * tiles[best].my * P)) {
+      // prefer the warp-specialised kernel, then register-resident coefficients, then the smaller tile
+      // (more threads, better latency hiding)
+      const int kb = best < 0 ? 0 : tiles[best].mx * P * tiles[best].my * P;
+      const long long score = (long long)(1 - t.ws) * 1000000 + (long long)t.csm * 10000 + k;
+      const long long bscore = best < 0 ? 0 : (long long)(1 - tiles[best].ws) * 1000000 + (long long)tiles[best].csm * 10000 + kb;
+      if (best < 0 || score < bscore) {
         best = i; blay = lo; bl = la;
       }
     }
@@ -482,10 +496,10 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
   }
   if (best >= 0) {
     ctx->lay = blay; ctx->launch = bl;
-    ctx->mx = tiles[best].mx; ctx->my = tiles[best].my; ctx->csm = tiles[best].csm;
+    ctx->mx = tiles[best].mx; ctx->my = tiles[best].my; ctx->csm = tiles[best].csm; ctx->ws = tiles[best].ws;
   } else {
     lay.variant = 0; lay.NT = roundup(N, 32); lay.NS = lay.NT; lay.TX = lay.TY = 1; lay.ntx = lay.nty = 0;
-    ctx->lay = lay; ctx->mx = ctx->my = 0; ctx->csm = 0;
+    ctx->lay = lay; ctx->mx = ctx->my = 0; ctx->csm = 0; ctx->ws = 0;
     ctx->launch.blocks = ctx->L; ctx->launch.threads = lay.NT;
     ctx->launch.smem = tab_bytes + 2 * (size_t)(lnx + 2 * P) * (lny + 2 * P) * rs;
   }

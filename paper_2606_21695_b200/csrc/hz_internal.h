@@ -70,6 +70,7 @@ struct SweepArgs {
 
 struct TileEntry {
   int p, mx, my, csm, maxt;  // csm: gamma / beta b in shared memory instead of registers
+  int ws;                    // 1: warp-specialised kernel (hz_sweep_ws.cuh), needs mx == my
   const void *fn;
 };
 
@@ -81,9 +82,9 @@ struct SweepLaunch {
 // Implemented in hz_sweep_*.cu.  Return cudaErrorInvalidValue when no instantiation matches.
 cudaError_t launch_sweep_dof_f32(const SweepArgs<float> &a, int p, SweepLaunch cfg, cudaStream_t st);
 cudaError_t launch_sweep_dof_f64(const SweepArgs<double> &a, int p, SweepLaunch cfg, cudaStream_t st);
-cudaError_t launch_sweep_tile_f32(const SweepArgs<float> &a, int p, int mx, int my, int csm, SweepLaunch cfg,
+cudaError_t launch_sweep_tile_f32(const SweepArgs<float> &a, int p, int mx, int my, int csm, int ws, SweepLaunch cfg,
                                   cudaStream_t st);
-cudaError_t launch_sweep_tile_f64(const SweepArgs<double> &a, int p, int mx, int my, int csm, SweepLaunch cfg,
+cudaError_t launch_sweep_tile_f64(const SweepArgs<double> &a, int p, int mx, int my, int csm, int ws, SweepLaunch cfg,
                                   cudaStream_t st);
 // compiled register-blocked instantiations of one precision
 int tile_table_f32(const TileEntry **out);

@@ -3,6 +3,7 @@
 // parallel).  HZ_TILE_TABLE(X) lists X(P, MX, MY, CSM, MAXT, MINB).
 #pragma once
 #include "hz_sweep.cuh"
+#include "hz_sweep_ws.cuh"
 
 namespace hz {
 
@@ -24,10 +25,10 @@ static cudaError_t launch_dof_impl(const SweepArgs<real> &a, int p, SweepLaunch 
 
 template <typename real>
 static cudaError_t launch_tile_impl(const TileEntry *tab, int n, const SweepArgs<real> &a, int p, int mx, int my,
-                                    int csm, SweepLaunch cfg, cudaStream_t st) {
+                                    int csm, int ws, SweepLaunch cfg, cudaStream_t st) {
   for (int i = 0; i < n; ++i) {
     const TileEntry &e = tab[i];
-    if (e.p == p && e.mx == mx && e.my == my && e.csm == csm && cfg.threads <= e.maxt) {
+    if (e.p == p && e.mx == mx && e.my == my && e.csm == csm && e.ws == ws && cfg.threads <= e.maxt) {
       auto fn = reinterpret_cast<void (*)(const SweepArgs<real>)>(const_cast<void *>(e.fn));
       cudaError_t err = cudaFuncSetAttribute(e.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem);
       if (err != cudaSuccess) return err;

@@ -1,0 +1,432 @@
+// hz_sweep_ws.cuh — warp-specialised register-blocked sweep kernel (square thread tiles, MX = MY = M).
+//
+// Same arithmetic and the same shared-memory exchange protocol as k_sweep_tile (hz_sweep.cuh), but the
+// (ntx-1) x (nty-1) "bulk" tiles, which own full (M*P)^2 node tiles, run in their own warps, and the
+// ntx + nty - 1 ragged tiles on the far edges (last node column / last node row of the subdomain, which
+// own only one line of M*P nodes) are packed one per lane into separate "edge" warps that run a
+// line-only code path.  In k_sweep_tile the ragged tiles execute the full-tile instruction stream on
+// padding (28 % of the issue slots at 8x8 elements, p = 3); here they cost a fraction of a warp.
+//
+// Exchange records: virtual tile v = ty*ntx + tx owns record v of RS = 2(TX+TY)+1 words (odd stride:
+// conflict-free for 32- and 64-bit accesses):  PX[b] | RX[b] | PY[a] | RY[a]
+//   PX[b]  partial sum  sum_{c<P} kp_x[c] p[b][last element, c]   (what the right neighbour's first column needs)
+//   RX[b]  raw p[b][0]                                           (what the left neighbour's last element needs)
+//   PY[a], RY[a] the same along y.
+// Records NTV..NTV+31 are always zero (missing neighbours; one per bank so the access stays
+// conflict-free), records NTV+32.. are write-only scratch for idle lanes.  Two buffers (ping-pong), one
+// named barrier per time step.
+#pragma once
+#include "hz_sweep.cuh"
+
+namespace hz {
+
+__device__ __forceinline__ void bar_sync_all(int nthreads) {
+  asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory");
+}
+
+// One line of T = M*P owned nodes q[0..T-1] plus q[T] (first node of the next tile along the line):
+// S[n] (+)= (assembled 1-D operator row n) . q, using the incoming partial `pin` for node 0.
+// k: Elem1D coefficients of this direction.  d0/s0: diagonal and scale of node 0 (one-sided at the ends).
+template <typename real, int P, int M, bool ACC, typename KT>
+__device__ __forceinline__ void line_apply(const real (&q)[M * P + 1], real pin, real d0, real s0, const KT &k,
+                                           real (&S)[M * P]) {
+  {
+    real T = fmaT(d0, q[0], pin);
+#pragma unroll
+    for (int c = 1; c <= P; ++c) T = fmaT(k.k0[c], q[c], T);
+    S[0] = ACC ? fmaT(s0, T, S[0]) : s0 * T;
+  }
+#pragma unroll
+  for (int e = 0; e < M; ++e) {
+#pragma unroll
+    for (int a = 1; a < P; ++a) {
+      real T = ACC ? fmaT(k.kin[a][0], q[e * P], S[e * P + a]) : k.kin[a][0] * q[e * P];
+#pragma unroll
+      for (int c = 1; c <= P; ++c) T = fmaT(k.kin[a][c], q[e * P + c], T);
+      S[e * P + a] = T;
+    }
+    if (e > 0) {
+      real T = ACC ? fmaT(k.k0[0] + k.kp[P], q[e * P], S[e * P]) : (k.k0[0] + k.kp[P]) * q[e * P];
+#pragma unroll
+      for (int c = 0; c < P; ++c) T = fmaT(k.kp[c], q[(e - 1) * P + c], T);
+#pragma unroll
+      for (int c = 1; c <= P; ++c) T = fmaT(k.k0[c], q[e * P + c], T);
+      S[e * P] = T;
+    }
+  }
+}
+
+template <typename real, int P, int M, typename KT>
+__device__ __forceinline__ real line_partial(const real (&q)[M * P + 1], const KT &k) {
+  real s = k.kp[0] * q[(M - 1) * P];
+#pragma unroll
+  for (int c = 1; c < P; ++c) s = fmaT(k.kp[c], q[(M - 1) * P + c], s);
+  return s;
+}
+
+template <typename real, int P, int M, bool CSM, int MAXT, int MINB>
+__global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A) {
+  constexpr int T = M * P, KT = T * T;
+  constexpr int RS = 4 * T + 1;  // record stride (words of `real`)
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  Tab4<real> *tab = reinterpret_cast<Tab4<real> *>(smem_raw);
+  const int h = threadIdx.x, NTH = blockDim.x, l = blockIdx.x;
+  const int ntx = A.lay.ntx, nty = A.lay.nty, NTV = A.lay.NT, NS = A.lay.NS;
+  const int lnx = A.lay.lnx, lny = A.lay.lny;
+  const int BUFW = (NTV + 64) * RS;
+  real *xb = reinterpret_cast<real *>(tab + A.n_t);
+  real *csm = xb + 2 * BUFW;  // CSM: [2][KT][NTH] gamma | beta b_r of the bulk tiles
+  const int nbulk = (ntx - 1) * (nty - 1);
+  const int bulk_warps = (nbulk + 31) >> 5;
+  const int warp = h >> 5, lane = h & 31;
+
+  for (int q = h; q < 2 * BUFW; q += NTH) xb[q] = real(0);
+  for (int q = h; q < A.n_t; q += NTH) tab[q] = A.tab[q];
+
+  const int six = l % A.sx, siy = l / A.sx;
+  const size_t lbase = (size_t)l * 4 * 2 * A.E, ebase = (size_t)l * 4 * A.E;
+  const real sigma = A.sigma;
+
+  if (warp < bulk_warps) {
+    // ============================ bulk tiles: full T x T node tiles ============================
+    const bool act = h < nbulk;
+    const int tx = act ? h % (ntx - 1) : 0, ty = act ? h / (ntx - 1) : 0;
+    const int v = ty * ntx + tx;
+    const int rMy = act ? v : NTV + 32 + lane;
+    const int rL = (act && tx > 0) ? v - 1 : NTV + ((v - 1) & 31);
+    const int rR = act ? v + 1 : NTV + ((v + 1) & 31);
+    const int rD = (act && ty > 0) ? v - ntx : NTV + ((v - ntx) & 31);
+    const int rU = act ? v + ntx : NTV + ((v + ntx) & 31);
+    const real *pL = xb + rL * RS, *pR = xb + rR * RS, *pD = xb + rD * RS, *pU = xb + rU * RS;
+    real *pMy = xb + rMy * RS;
+    const bool hasL = tx > 0, hasD = ty > 0;
+    const real d0x = A.ex1.k0[0] + (hasL ? A.ex1.kp[P] : real(0));
+    const real d0y = A.ey1.k0[0] + (hasD ? A.ey1.kp[P] : real(0));
+    const real s0x = hasL ? real(1) : real(2), s0y = hasD ? real(1) : real(2);
+
+    real p[T][T], pd[T][T], vr[T][T], vi[T][T], ur[T][T], ui[T][T];
+    real gam[CSM ? 1 : T][CSM ? 1 : T], bbr[CSM ? 1 : T][CSM ? 1 : T];
+    real alc[T], bic[T], alr[T], bir[T];
+    const size_t base = (size_t)l * NS + v;
+#pragma unroll
+    for (int b = 0; b < T; ++b)
+#pragma unroll
+      for (int a = 0; a < T; ++a) {
+        const size_t o = base + (size_t)(b * T + a) * NTV;
+        const real g_ = act ? A.gamma[o] : real(0), r_ = act ? A.bbf_re[o] : real(0);
+        if (CSM) {
+          csm[(b * T + a) * NTH + h] = g_;
+          csm[(KT + b * T + a) * NTH + h] = r_;
+        } else {
+          gam[CSM ? 0 : b][CSM ? 0 : a] = g_;
+          bbr[CSM ? 0 : b][CSM ? 0 : a] = r_;
+        }
+        ur[b][a] = (act && A.warm) ? A.u_sub[(size_t)l * 2 * NS + (size_t)(b * T + a) * NTV + v] : real(0);
+        ui[b][a] = (act && A.warm) ? A.u_sub[(size_t)l * 2 * NS + NS + (size_t)(b * T + a) * NTV + v] : real(0);
+      }
+#pragma unroll
+    for (int b = 0; b < T; ++b) {
+      const size_t o = base + (size_t)(b * T) * NTV;
+      alc[b] = act ? A.alpha[o] : real(0);
+      bic[b] = (act && A.bbf_im) ? A.bbf_im[o] : real(0);
+    }
+#pragma unroll
+    for (int a = 0; a < T; ++a) {
+      const size_t o = base + (size_t)a * NTV;
+      alr[a] = act ? A.alpha[o] : real(0);
+      bir[a] = (act && A.bbf_im) ? A.bbf_im[o] : real(0);
+    }
+    // Assemble b from lambda^n: bulk tiles touch only the W side (tx = 0) and the S side (ty = 0)
+    const bool onW = act && tx == 0 && six > 0, onS = act && ty == 0 && siy > 0;
+    real lcr[T], lci[T], lrr[T], lri[T];
+#pragma unroll
+    for (int b = 0; b < T; ++b) { lcr[b] = 0; lci[b] = 0; lrr[b] = 0; lri[b] = 0; }
+    if (onW) {
+#pragma unroll
+      for (int b = 0; b < T; ++b) {
+        const int j = ty * T + b;
+        lcr[b] = A.lam[lbase + (kSideW * 2 + 0) * A.E + j];
+        lci[b] = A.lam[lbase + (kSideW * 2 + 1) * A.E + j];
+        const real s = A.bs[ebase + kSideW * A.E + j];
+        if (CSM) csm[(KT + b * T) * NTH + h] = fmaT(s, lcr[b], csm[(KT + b * T) * NTH + h]);
+        else bbr[CSM ? 0 : b][0] = fmaT(s, lcr[b], bbr[CSM ? 0 : b][0]);
+        bic[b] = fmaT(s, lci[b], bic[b]);
+      }
+    }
+    if (onS) {
+#pragma unroll
+      for (int a = 0; a < T; ++a) {
+        const int i = tx * T + a;
+        lrr[a] = A.lam[lbase + (kSideS * 2 + 0) * A.E + i];
+        lri[a] = A.lam[lbase + (kSideS * 2 + 1) * A.E + i];
+        const real s = A.bs[ebase + kSideS * A.E + i];
+        if (CSM) csm[(KT + a) * NTH + h] = fmaT(s, lrr[a], csm[(KT + a) * NTH + h]);
+        else bbr[0][CSM ? 0 : a] = fmaT(s, lrr[a], bbr[0][CSM ? 0 : a]);
+        if (a == 0) bic[0] = fmaT(s, lri[a], bic[0]);
+        else bir[a] = fmaT(s, lri[a], bir[a]);
+      }
+    }
+    bar_sync_all(NTH);
+
+    int cur = 0;
+    for (int m = 0; m < A.n_wh; ++m) {
+      const Tab4<real> t0 = tab[0];
+#pragma unroll
+      for (int b = 0; b < T; ++b)
+#pragma unroll
+        for (int a = 0; a < T; ++a) {
+          p[b][a] = ur[b][a];
+          pd[b][a] = A.omega * (ui[b][a] * A.cos_h - ur[b][a] * A.sin_h);
+          vr[b][a] = t0.k * p[b][a];
+          vi[b][a] = t0.kh * pd[b][a];
+        }
+#pragma unroll 1
+      for (int nu = 1; nu < A.n_t; ++nu) {
+#pragma unroll
+        for (int b = 0; b < T; ++b)
+#pragma unroll
+          for (int a = 0; a < T; ++a) p[b][a] = fmaT(sigma, pd[b][a], p[b][a]);
+        real *my = pMy + cur;
+#pragma unroll
+        for (int b = 0; b < T; ++b) {
+          real q[T + 1];
+#pragma unroll
+          for (int a = 0; a < T; ++a) q[a] = p[b][a];
+          q[T] = real(0);
+          my[b] = line_partial<real, P, M>(q, A.ex1);
+          my[T + b] = p[b][0];
+        }
+#pragma unroll
+        for (int a = 0; a < T; ++a) {
+          real q[T + 1];
+#pragma unroll
+          for (int b = 0; b < T; ++b) q[b] = p[b][a];
+          q[T] = real(0);
+          my[2 * T + a] = line_partial<real, P, M>(q, A.ey1);
+          my[3 * T + a] = p[0][a];
+        }
+        bar_sync_all(NTH);
+        const real *nL = pL + cur, *nR = pR + cur, *nD = pD + cur, *nU = pU + cur;
+        cur = BUFW - cur;
+        real S[T][T];
+#pragma unroll
+        for (int b = 0; b < T; ++b) {
+          real q[T + 1];
+#pragma unroll
+          for (int a = 0; a < T; ++a) q[a] = p[b][a];
+          q[T] = nR[T + b];
+          line_apply<real, P, M, false>(q, nL[b], d0x, s0x, A.ex1, S[b]);
+        }
+#pragma unroll
+        for (int a = 0; a < T; ++a) {
+          real q[T + 1], Sc[T];
+#pragma unroll
+          for (int b = 0; b < T; ++b) { q[b] = p[b][a]; Sc[b] = S[b][a]; }
+          q[T] = nU[3 * T + a];
+          line_apply<real, P, M, true>(q, nD[2 * T + a], d0y, s0y, A.ey1, Sc);
+#pragma unroll
+          for (int b = 0; b < T; ++b) S[b][a] = Sc[b];
+        }
+        const Tab4<real> tn = tab[nu];
+#pragma unroll
+        for (int b = 0; b < T; ++b)
+#pragma unroll
+          for (int a = 0; a < T; ++a) {
+            const real g_ = CSM ? csm[(b * T + a) * NTH + h] : gam[CSM ? 0 : b][CSM ? 0 : a];
+            const real r_ = CSM ? csm[(KT + b * T + a) * NTH + h] : bbr[CSM ? 0 : b][CSM ? 0 : a];
+            real x = fmaT(-g_, S[b][a], r_ * tn.c);
+            if (a == 0) {
+              x = fmaT(bic[b], tn.s, x);
+              pd[b][a] = fmaT(alc[b], pd[b][a], x);
+            } else if (b == 0) {
+              x = fmaT(bir[a], tn.s, x);
+              pd[b][a] = fmaT(alr[a], pd[b][a], x);
+            } else {
+              pd[b][a] += x;
+            }
+            vr[b][a] = fmaT(tn.k, p[b][a], vr[b][a]);
+            vi[b][a] = fmaT(tn.kh, pd[b][a], vi[b][a]);
+          }
+      }
+#pragma unroll
+      for (int b = 0; b < T; ++b)
+#pragma unroll
+        for (int a = 0; a < T; ++a) {
+          ur[b][a] = A.two_over_nt * vr[b][a];
+          ui[b][a] = A.two_over_nt * vi[b][a];
+        }
+    }
+    if (act) {
+#pragma unroll
+      for (int b = 0; b < T; ++b)
+#pragma unroll
+        for (int a = 0; a < T; ++a) {
+          A.u_sub[(size_t)l * 2 * NS + (size_t)(b * T + a) * NTV + v] = ur[b][a];
+          A.u_sub[(size_t)l * 2 * NS + NS + (size_t)(b * T + a) * NTV + v] = ui[b][a];
+        }
+    }
+    if (onW) {
+#pragma unroll
+      for (int b = 0; b < T; ++b) {
+        const int j = ty * T + b;
+        const real k2 = A.k2edge[ebase + kSideW * A.E + j];
+        A.gout[lbase + (kSideW * 2 + 0) * A.E + j] = fmaT(k2, ui[b][0], -lcr[b]);
+        A.gout[lbase + (kSideW * 2 + 1) * A.E + j] = fmaT(-k2, ur[b][0], -lci[b]);
+      }
+    }
+    if (onS) {
+#pragma unroll
+      for (int a = 0; a < T; ++a) {
+        const int i = tx * T + a;
+        const real k2 = A.k2edge[ebase + kSideS * A.E + i];
+        A.gout[lbase + (kSideS * 2 + 0) * A.E + i] = fmaT(k2, ui[0][a], -lrr[a]);
+        A.gout[lbase + (kSideS * 2 + 1) * A.E + i] = fmaT(-k2, ur[0][a], -lri[a]);
+      }
+    }
+  } else {
+    // ============================ edge pieces: one line of T nodes per lane ============================
+    // lane e < nty-1: right piece, virtual tile (ntx-1, e), nodes (lnx-1, e*T + n), "along" = y.
+    // lane e >= nty-1: top piece, virtual tile (e-(nty-1), nty-1), nodes (tx*T + n, lny-1), "along" = x;
+    //                  the last one (tx = ntx-1) is the corner and owns node 0 only.
+    const int e = h - 32 * bulk_warps;
+    const bool act = e < (nty - 1) + ntx;
+    const bool top = act && e >= nty - 1;
+    const int tx = !act ? 0 : (top ? e - (nty - 1) : ntx - 1);
+    const int ty = !act ? 0 : (top ? nty - 1 : e);
+    const int v = ty * ntx + tx;
+    const int ta = top ? tx : ty, nta = top ? ntx : nty;  // position / count along the line direction
+    const int sa = top ? 1 : ntx;                         // virtual-tile stride along
+    const int sc = top ? ntx : 1;                         // virtual-tile stride across
+    // record field offsets: along partial / along raw / across partial (read from the bulk tile) / across raw
+    const int oPA = top ? 0 : 2 * T, oRA = top ? T : 3 * T, oPC = top ? 2 * T : 0, oRC = top ? 3 * T : T;
+    const int rMy = act ? v : NTV + 32 + lane;
+    const bool hasP = act && ta > 0, hasN = act && ta < nta - 1;
+    const int rP = hasP ? v - sa : NTV + ((v - sa) & 31);  // previous piece along the edge
+    const int rN = hasN ? v + sa : NTV + ((v + sa) & 31);  // next piece along the edge
+    // the tile across (below a top piece / left of a right piece); the corner's is an edge piece too
+    const int rC = act ? v - sc : NTV + ((v - sc) & 31);
+    real *pMy = xb + rMy * RS;
+    const real *pP = xb + rP * RS + oPA, *pN = xb + rN * RS + oRA, *pC = xb + rC * RS + oPC;
+    Elem1D<real> ka;  // coefficients along
+#pragma unroll
+    for (int c = 0; c <= P; ++c) {
+      ka.k0[c] = top ? A.ex1.k0[c] : A.ey1.k0[c];
+      ka.kp[c] = top ? A.ex1.kp[c] : A.ey1.kp[c];
+#pragma unroll
+      for (int a = 1; a < P; ++a) ka.kin[a][c] = top ? A.ex1.kin[a][c] : A.ey1.kin[a][c];
+    }
+    const real d0a = (hasN ? ka.k0[0] : real(0)) + (hasP ? ka.kp[P] : real(0));
+    const real s0a = (hasP && hasN) ? real(1) : real(2);
+    // across: the piece sits on the last node line, only the element before it exists
+    const real d0c = top ? A.ey1.kp[P] : A.ex1.kp[P];
+    const real s0c = real(2);
+
+    real p[T], pd[T], vr[T], vi[T], ur[T], ui[T], gam[T], bbr[T], al[T], bbi[T];
+    const size_t base = (size_t)l * NS + v;
+#pragma unroll
+    for (int n = 0; n < T; ++n) {
+      const size_t o = base + (size_t)(top ? n : n * T) * NTV;  // tile node (a=n,b=0) or (a=0,b=n)
+      gam[n] = act ? A.gamma[o] : real(0);
+      bbr[n] = act ? A.bbf_re[o] : real(0);
+      al[n] = act ? A.alpha[o] : real(0);
+      bbi[n] = (act && A.bbf_im) ? A.bbf_im[o] : real(0);
+      ur[n] = (act && A.warm) ? A.u_sub[(size_t)l * 2 * NS + (o - (size_t)l * NS)] : real(0);
+      ui[n] = (act && A.warm) ? A.u_sub[(size_t)l * 2 * NS + NS + (o - (size_t)l * NS)] : real(0);
+    }
+    // interface sides: the whole piece lies on N (top) or E (right); node 0 may also lie on a second side
+    const int side1 = top ? kSideN : kSideE;
+    const bool on1 = act && (top ? siy < A.sy - 1 : six < A.sx - 1);
+    const int len1 = top ? lnx : lny;
+    int side2 = -1, idx2 = 0;
+    if (act && top && tx == 0 && six > 0) { side2 = kSideW; idx2 = lny - 1; }
+    if (act && top && tx == ntx - 1 && six < A.sx - 1) { side2 = kSideE; idx2 = lny - 1; }
+    if (act && !top && ty == 0 && siy > 0) { side2 = kSideS; idx2 = lnx - 1; }
+    real l1r[T], l1i[T], l2r = 0, l2i = 0;
+#pragma unroll
+    for (int n = 0; n < T; ++n) {
+      l1r[n] = 0; l1i[n] = 0;
+      const int idx = ta * T + n;
+      if (on1 && idx < len1) {
+        l1r[n] = A.lam[lbase + (side1 * 2 + 0) * A.E + idx];
+        l1i[n] = A.lam[lbase + (side1 * 2 + 1) * A.E + idx];
+        const real s = A.bs[ebase + side1 * A.E + idx];
+        bbr[n] = fmaT(s, l1r[n], bbr[n]);
+        bbi[n] = fmaT(s, l1i[n], bbi[n]);
+      }
+    }
+    if (side2 >= 0) {
+      l2r = A.lam[lbase + (side2 * 2 + 0) * A.E + idx2];
+      l2i = A.lam[lbase + (side2 * 2 + 1) * A.E + idx2];
+      const real s = A.bs[ebase + side2 * A.E + idx2];
+      bbr[0] = fmaT(s, l2r, bbr[0]);
+      bbi[0] = fmaT(s, l2i, bbi[0]);
+    }
+    bar_sync_all(NTH);
+
+    int cur = 0;
+    for (int m = 0; m < A.n_wh; ++m) {
+      const Tab4<real> t0 = tab[0];
+#pragma unroll
+      for (int n = 0; n < T; ++n) {
+        p[n] = ur[n];
+        pd[n] = A.omega * (ui[n] * A.cos_h - ur[n] * A.sin_h);
+        vr[n] = t0.k * p[n];
+        vi[n] = t0.kh * pd[n];
+      }
+#pragma unroll 1
+      for (int nu = 1; nu < A.n_t; ++nu) {
+        real q[T + 1];
+#pragma unroll
+        for (int n = 0; n < T; ++n) { p[n] = fmaT(sigma, pd[n], p[n]); q[n] = p[n]; }
+        q[T] = real(0);
+        real *my = pMy + cur;
+        my[oPA] = line_partial<real, P, M>(q, ka);
+        my[oRA] = p[0];
+#pragma unroll
+        for (int n = 0; n < T; ++n) my[oRC + n] = p[n];
+        bar_sync_all(NTH);
+        q[T] = pN[cur];
+        real S[T];
+        line_apply<real, P, M, false>(q, pP[cur], d0a, s0a, ka, S);
+#pragma unroll
+        for (int n = 0; n < T; ++n) S[n] = fmaT(s0c, fmaT(d0c, p[n], pC[cur + n]), S[n]);
+        cur = BUFW - cur;
+        const Tab4<real> tn = tab[nu];
+#pragma unroll
+        for (int n = 0; n < T; ++n) {
+          real x = fmaT(-gam[n], S[n], bbr[n] * tn.c);
+          x = fmaT(bbi[n], tn.s, x);
+          pd[n] = fmaT(al[n], pd[n], x);
+          vr[n] = fmaT(tn.k, p[n], vr[n]);
+          vi[n] = fmaT(tn.kh, pd[n], vi[n]);
+        }
+      }
+#pragma unroll
+      for (int n = 0; n < T; ++n) {
+        ur[n] = A.two_over_nt * vr[n];
+        ui[n] = A.two_over_nt * vi[n];
+      }
+    }
+    if (act) {
+#pragma unroll
+      for (int n = 0; n < T; ++n) {
+        const size_t o = (size_t)(top ? n : n * T) * NTV + v;
+        A.u_sub[(size_t)l * 2 * NS + o] = ur[n];
+        A.u_sub[(size_t)l * 2 * NS + NS + o] = ui[n];
+        const int idx = ta * T + n;
+        if (on1 && idx < len1) {
+          const real k2 = A.k2edge[ebase + side1 * A.E + idx];
+          A.gout[lbase + (side1 * 2 + 0) * A.E + idx] = fmaT(k2, ui[n], -l1r[n]);
+          A.gout[lbase + (side1 * 2 + 1) * A.E + idx] = fmaT(-k2, ur[n], -l1i[n]);
+        }
+      }
+      if (side2 >= 0) {
+        const real k2 = A.k2edge[ebase + side2 * A.E + idx2];
+        A.gout[lbase + (side2 * 2 + 0) * A.E + idx2] = fmaT(k2, ui[0], -l2r);
+        A.gout[lbase + (side2 * 2 + 1) * A.E + idx2] = fmaT(-k2, ur[0], -l2i);
+      }
+    }
+  }
+}
+
+}  // namespace hz
