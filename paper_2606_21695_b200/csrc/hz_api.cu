@@ -458,7 +458,9 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
     if (t.ws) {
       if (no_ws) return false;
       nthr = roundup((q.ntx - 1) * (q.nty - 1), 32) + roundup(q.ntx + q.nty - 1, 32);
-      sm = tab_bytes + 2 * (size_t)(ntv + 64) * (narr + 1) * rs + (t.csm ? 2 * (size_t)q.TX * q.TY * nthr * rs : 0);
+      const int nbulk = (q.ntx - 1) * (q.nty - 1), nedge = q.ntx + q.nty - 1;
+      const size_t nrec = (size_t)roundup(nbulk + q.ntx, 32) + 64 + roundup(nedge, 32);
+      sm = tab_bytes + 2 * nrec * (narr + 1) * rs + (t.csm ? 2 * (size_t)q.TX * q.TY * nthr * rs : 0);
     } else {
       sm = tab_bytes + 2 * narr * (nthr + 1) * rs + (t.csm ? 2 * (size_t)q.TX * q.TY * nthr * rs : 0);
     }

@@ -7,14 +7,18 @@
 // line-only code path.  In k_sweep_tile the ragged tiles execute the full-tile instruction stream on
 // padding (28 % of the issue slots at 8x8 elements, p = 3); here they cost a fraction of a warp.
 //
-// Exchange records: virtual tile v = ty*ntx + tx owns record v of RS = 2(TX+TY)+1 words (odd stride:
-// conflict-free for 32- and 64-bit accesses):  PX[b] | RX[b] | PY[a] | RY[a]
+// Exchange records of RS = 2(TX+TY)+1 words (odd stride: lane-consecutive records are conflict-free for
+// 32- and 64-bit accesses):  PX[b] | RX[b] | PY[a] | RY[a].  Bulk thread h owns record h; what it reads is
+// ALWAYS record h-1 / h+1 / h-w / h+w (w = ntx-1 bulk tiles per row) or a zero record of the same bank, so
+// every bulk access is conflict-free.  To make that true at the far edges, a right edge piece publishes its
+// raw values into the RX fields of record (ty+1)*w (the first bulk tile of the next row, whose own RX has no
+// reader and is redirected to scratch) and a top piece into the RY fields of record nbulk+tx.
 //   PX[b]  partial sum  sum_{c<P} kp_x[c] p[b][last element, c]   (what the right neighbour's first column needs)
 //   RX[b]  raw p[b][0]                                           (what the left neighbour's last element needs)
 //   PY[a], RY[a] the same along y.
-// Records NTV..NTV+31 are always zero (missing neighbours; one per bank so the access stays
-// conflict-free), records NTV+32.. are write-only scratch for idle lanes.  Two buffers (ping-pong), one
-// named barrier per time step.
+// Records NB..NB+31 (NB = roundup32(nbulk+ntx)) are always zero (missing neighbours), NB+32..NB+63 are
+// write-only scratch, NB+64.. are the edge pieces' own records (along-the-edge exchange).  Two buffers
+// (ping-pong), one named barrier per time step.
 #pragma once
 #include "hz_sweep.cuh"
 
@@ -73,11 +77,12 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
   const int h = threadIdx.x, NTH = blockDim.x, l = blockIdx.x;
   const int ntx = A.lay.ntx, nty = A.lay.nty, NTV = A.lay.NT, NS = A.lay.NS;
   const int lnx = A.lay.lnx, lny = A.lay.lny;
-  const int BUFW = (NTV + 64) * RS;
+  const int w = ntx - 1, nbulk = (ntx - 1) * (nty - 1), nedge = ntx + nty - 1;
+  const int bulk_warps = (nbulk + 31) >> 5;
+  const int NB = (nbulk + ntx + 31) & ~31, ZR = NB, SCR = NB + 32, EB = NB + 64;
+  const int BUFW = (NB + 64 + ((nedge + 31) & ~31)) * RS;
   real *xb = reinterpret_cast<real *>(tab + A.n_t);
   real *csm = xb + 2 * BUFW;  // CSM: [2][KT][NTH] gamma | beta b_r of the bulk tiles
-  const int nbulk = (ntx - 1) * (nty - 1);
-  const int bulk_warps = (nbulk + 31) >> 5;
   const int warp = h >> 5, lane = h & 31;
 
   for (int q = h; q < 2 * BUFW; q += NTH) xb[q] = real(0);
@@ -92,13 +97,14 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
     const bool act = h < nbulk;
     const int tx = act ? h % (ntx - 1) : 0, ty = act ? h / (ntx - 1) : 0;
     const int v = ty * ntx + tx;
-    const int rMy = act ? v : NTV + 32 + lane;
-    const int rL = (act && tx > 0) ? v - 1 : NTV + ((v - 1) & 31);
-    const int rR = act ? v + 1 : NTV + ((v + 1) & 31);
-    const int rD = (act && ty > 0) ? v - ntx : NTV + ((v - ntx) & 31);
-    const int rU = act ? v + ntx : NTV + ((v + ntx) & 31);
+    const int rMy = act ? h : SCR + lane;
+    const int rL = (act && tx > 0) ? h - 1 : ZR + ((h - 1) & 31);
+    const int rR = act ? h + 1 : ZR + ((h + 1) & 31);
+    const int rD = (act && ty > 0) ? h - w : ZR + ((h - w) & 31);
+    const int rU = act ? h + w : ZR + ((h + w) & 31);
     const real *pL = xb + rL * RS, *pR = xb + rR * RS, *pD = xb + rD * RS, *pU = xb + rU * RS;
     real *pMy = xb + rMy * RS;
+    real *pMyRX = xb + ((act && tx > 0) ? h : SCR + lane) * RS + T;  // RX of a tx = 0 tile has no reader
     const bool hasL = tx > 0, hasD = ty > 0;
     const real d0x = A.ex1.k0[0] + (hasL ? A.ex1.kp[P] : real(0));
     const real d0y = A.ey1.k0[0] + (hasD ? A.ey1.kp[P] : real(0));
@@ -186,7 +192,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
         for (int b = 0; b < T; ++b)
 #pragma unroll
           for (int a = 0; a < T; ++a) p[b][a] = fmaT(sigma, pd[b][a], p[b][a]);
-        real *my = pMy + cur;
+        real *my = pMy + cur, *myRX = pMyRX + cur;
 #pragma unroll
         for (int b = 0; b < T; ++b) {
           real q[T + 1];
@@ -194,7 +200,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
           for (int a = 0; a < T; ++a) q[a] = p[b][a];
           q[T] = real(0);
           my[b] = line_partial<real, P, M>(q, A.ex1);
-          my[T + b] = p[b][0];
+          myRX[b] = p[b][0];
         }
 #pragma unroll
         for (int a = 0; a < T; ++a) {
@@ -299,14 +305,23 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
     const int sc = top ? ntx : 1;                         // virtual-tile stride across
     // record field offsets: along partial / along raw / across partial (read from the bulk tile) / across raw
     const int oPA = top ? 0 : 2 * T, oRA = top ? T : 3 * T, oPC = top ? 2 * T : 0, oRC = top ? 3 * T : T;
-    const int rMy = act ? v : NTV + 32 + lane;
     const bool hasP = act && ta > 0, hasN = act && ta < nta - 1;
-    const int rP = hasP ? v - sa : NTV + ((v - sa) & 31);  // previous piece along the edge
-    const int rN = hasN ? v + sa : NTV + ((v + sa) & 31);  // next piece along the edge
-    // the tile across (below a top piece / left of a right piece); the corner's is an edge piece too
-    const int rC = act ? v - sc : NTV + ((v - sc) & 31);
-    real *pMy = xb + rMy * RS;
-    const real *pP = xb + rP * RS + oPA, *pN = xb + rN * RS + oRA, *pC = xb + rC * RS + oPC;
+    // own record (along-the-edge exchange): EB + e
+    real *pOwn = xb + (act ? EB + e : SCR + lane) * RS;
+    // where the raw values go that the bulk tile across reads: right piece -> RX of record (ty+1)*w,
+    // top piece -> RY of record nbulk + tx
+    real *pRaw = xb + (!act ? SCR + lane : (top ? nbulk + tx : (ty + 1) * w)) * RS + oRC;
+    // previous / next piece along the edge.  The last right piece's "next" is the corner, whose raw value
+    // sits in RY[0] of record nbulk + w.
+    const int rP = hasP ? EB + e - 1 : ZR + ((e - 1) & 31);
+    const real *pP = xb + rP * RS + oPA;
+    const real *pN = !hasN ? xb + (ZR + ((e + 1) & 31)) * RS
+                           : ((!top && ty == nty - 2) ? xb + (nbulk + w) * RS + 3 * T : xb + (EB + e + 1) * RS + oRA);
+    // the partial sums from the tile across: bulk tile below / left; for the corner the last right piece's
+    // along partial (field PY[0] of its own record; the fields after it stay zero)
+    const real *pC = !act ? xb + (ZR + lane) * RS
+                          : (top ? (tx < w ? xb + ((nty - 2) * w + tx) * RS + 2 * T : xb + (EB + nty - 2) * RS + 2 * T)
+                                 : xb + (ty * w + w - 1) * RS);
     Elem1D<real> ka;  // coefficients along
 #pragma unroll
     for (int c = 0; c <= P; ++c) {
@@ -379,11 +394,11 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
 #pragma unroll
         for (int n = 0; n < T; ++n) { p[n] = fmaT(sigma, pd[n], p[n]); q[n] = p[n]; }
         q[T] = real(0);
-        real *my = pMy + cur;
+        real *my = pOwn + cur, *raw = pRaw + cur;
         my[oPA] = line_partial<real, P, M>(q, ka);
         my[oRA] = p[0];
 #pragma unroll
-        for (int n = 0; n < T; ++n) my[oRC + n] = p[n];
+        for (int n = 0; n < T; ++n) raw[n] = p[n];
         bar_sync_all(NTH);
         q[T] = pN[cur];
         real S[T];
