@@ -137,7 +137,7 @@ struct hz_ctx {
   // partition
   bool part = false;
   int sx = 0, sy = 0, ex = 0, ey = 0, L = 0, E = 0, prec = 0;
-  int mx = 0, my = 0, csm = 0, ws = 0;
+  int mx = 0, my = 0, csm = 0, ws = 0, entry = -1;
   Layout lay{};
   SweepLaunch launch{};
   int n_t = 0;
@@ -264,11 +264,11 @@ cudaError_t launch_sweep(const hz_ctx *c, const hz_solve_opts *o, cudaStream_t s
   if (c->prec == HZ_F32) {
     SweepArgs<float> a = make_args<float>(c, o);
     return c->lay.variant == 0 ? launch_sweep_dof_f32(a, c->p, c->launch, st)
-                               : launch_sweep_tile_f32(a, c->p, c->mx, c->my, c->csm, c->ws, c->launch, st);
+                               : launch_sweep_tile_f32(a, c->entry, c->launch, st);
   }
   SweepArgs<double> a = make_args<double>(c, o);
   return c->lay.variant == 0 ? launch_sweep_dof_f64(a, c->p, c->launch, st)
-                             : launch_sweep_tile_f64(a, c->p, c->mx, c->my, c->csm, c->ws, c->launch, st);
+                             : launch_sweep_tile_f64(a, c->entry, c->launch, st);
 }
 
 cudaError_t launch_exchange(const hz_ctx *c, double rho, cudaStream_t st) {
@@ -444,8 +444,12 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
   int best = -1;
   SweepLaunch bl{};
   Layout blay{};
+  int sm_count = 148, dev = 0;
+  if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev);
   const char *env_ws = std::getenv("HZ_DISABLE_WS");  // debug knob: force the non-specialised tile kernel
   const bool no_ws = env_ws && env_ws[0] == '1';
+  const char *env_rc = std::getenv("HZ_NO_REGCAP");  // debug knob: never pick a register-capped instantiation
+  const bool no_regcap = env_rc && env_rc[0] == '1';
   auto tile_fit = [&](const TileEntry &t, Layout *lo, SweepLaunch *la) -> bool {
     if (t.p != P || ctx->ex % t.mx || ctx->ey % t.my) return false;
     Layout q = lay;
@@ -481,10 +485,14 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
       Layout lo; SweepLaunch la;
       if (!tile_fit(t, &lo, &la)) continue;
       // prefer the warp-specialised kernel, then register-resident coefficients, then the smaller tile
-      // (more threads, better latency hiding)
-      const int kb = best < 0 ? 0 : tiles[best].mx * P * tiles[best].my * P;
-      const long long score = (long long)(1 - t.ws) * 1000000 + (long long)t.csm * 10000 + k;
-      const long long bscore = best < 0 ? 0 : (long long)(1 - tiles[best].ws) * 1000000 + (long long)tiles[best].csm * 10000 + kb;
+      // (more threads, better latency hiding); among otherwise equal instantiations take the
+      // register-capped one (higher occupancy, a few spills) only when the grid can fill that occupancy
+      if (t.minb > 1 && ((long long)ctx->L < (long long)sm_count * t.minb || no_regcap)) continue;
+      auto score_of = [&](const TileEntry &q) {
+        return (long long)(1 - q.ws) * 100000000 + (long long)q.csm * 1000000 + (long long)q.mx * P * q.my * P * 100 - q.minb;
+      };
+      const long long score = score_of(t);
+      const long long bscore = best < 0 ? 0 : score_of(tiles[best]);
       if (best < 0 || score < bscore) {
         best = i; blay = lo; bl = la;
       }
@@ -499,6 +507,7 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
   if (best >= 0) {
     ctx->lay = blay; ctx->launch = bl;
     ctx->mx = tiles[best].mx; ctx->my = tiles[best].my; ctx->csm = tiles[best].csm; ctx->ws = tiles[best].ws;
+    ctx->entry = best;
   } else {
     lay.variant = 0; lay.NT = roundup(N, 32); lay.NS = lay.NT; lay.TX = lay.TY = 1; lay.ntx = lay.nty = 0;
     ctx->lay = lay; ctx->mx = ctx->my = 0; ctx->csm = 0; ctx->ws = 0;

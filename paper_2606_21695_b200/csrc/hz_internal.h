@@ -71,6 +71,7 @@ struct SweepArgs {
 struct TileEntry {
   int p, mx, my, csm, maxt;  // csm: gamma / beta b in shared memory instead of registers
   int ws;                    // 1: warp-specialised kernel (hz_sweep_ws.cuh), needs mx == my
+  int minb;                  // __launch_bounds__ min blocks per SM (register cap = 64K / (minb * maxt))
   const void *fn;
 };
 
@@ -82,10 +83,8 @@ struct SweepLaunch {
 // Implemented in hz_sweep_*.cu.  Return cudaErrorInvalidValue when no instantiation matches.
 cudaError_t launch_sweep_dof_f32(const SweepArgs<float> &a, int p, SweepLaunch cfg, cudaStream_t st);
 cudaError_t launch_sweep_dof_f64(const SweepArgs<double> &a, int p, SweepLaunch cfg, cudaStream_t st);
-cudaError_t launch_sweep_tile_f32(const SweepArgs<float> &a, int p, int mx, int my, int csm, int ws, SweepLaunch cfg,
-                                  cudaStream_t st);
-cudaError_t launch_sweep_tile_f64(const SweepArgs<double> &a, int p, int mx, int my, int csm, int ws, SweepLaunch cfg,
-                                  cudaStream_t st);
+cudaError_t launch_sweep_tile_f32(const SweepArgs<float> &a, int entry, SweepLaunch cfg, cudaStream_t st);
+cudaError_t launch_sweep_tile_f64(const SweepArgs<double> &a, int entry, SweepLaunch cfg, cudaStream_t st);
 // compiled register-blocked instantiations of one precision
 int tile_table_f32(const TileEntry **out);
 int tile_table_f64(const TileEntry **out);

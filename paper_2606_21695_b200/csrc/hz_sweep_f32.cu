@@ -27,9 +27,9 @@ namespace hz {
   W(4, 1, 0, 384, 1)
 
 #define X_ENTRY(P, MX, MY, CSM, MAXT, MINB) \
-  {P, MX, MY, CSM, MAXT, 0, (const void *)k_sweep_tile<float, P, MX, MY, (CSM != 0), MAXT, MINB>},
+  {P, MX, MY, CSM, MAXT, 0, MINB, (const void *)k_sweep_tile<float, P, MX, MY, (CSM != 0), MAXT, MINB>},
 #define W_ENTRY(P, M, CSM, MAXT, MINB) \
-  {P, M, M, CSM, MAXT, 1, (const void *)k_sweep_ws<float, P, M, (CSM != 0), MAXT, MINB>},
+  {P, M, M, CSM, MAXT, 1, MINB, (const void *)k_sweep_ws<float, P, M, (CSM != 0), MAXT, MINB>},
 static const TileEntry kTilesF32[] = {HZ_WS_TABLE_F32(W_ENTRY) HZ_TILE_TABLE_F32(X_ENTRY)};
 #undef X_ENTRY
 #undef W_ENTRY
@@ -38,9 +38,8 @@ static const int kNumTilesF32 = sizeof(kTilesF32) / sizeof(kTilesF32[0]);
 cudaError_t launch_sweep_dof_f32(const SweepArgs<float> &a, int p, SweepLaunch cfg, cudaStream_t st) {
   return launch_dof_impl<float>(a, p, cfg, st);
 }
-cudaError_t launch_sweep_tile_f32(const SweepArgs<float> &a, int p, int mx, int my, int csm, int ws, SweepLaunch cfg,
-                                  cudaStream_t st) {
-  return launch_tile_impl<float>(kTilesF32, kNumTilesF32, a, p, mx, my, csm, ws, cfg, st);
+cudaError_t launch_sweep_tile_f32(const SweepArgs<float> &a, int entry, SweepLaunch cfg, cudaStream_t st) {
+  return launch_tile_impl<float>(kTilesF32, kNumTilesF32, a, entry, cfg, st);
 }
 int tile_table_f32(const TileEntry **out) {
   *out = kTilesF32;

@@ -20,15 +20,16 @@ namespace hz {
   W(1, 4, 0, 256, 1)       \
   W(2, 1, 0, 512, 1)       \
   W(2, 2, 1, 320, 1)       \
+  W(3, 1, 0, 128, 3)       \
   W(3, 1, 0, 128, 1)       \
   W(3, 1, 0, 320, 1)       \
   W(3, 1, 1, 512, 1)       \
   W(4, 1, 1, 320, 1)
 
 #define X_ENTRY(P, MX, MY, CSM, MAXT, MINB) \
-  {P, MX, MY, CSM, MAXT, 0, (const void *)k_sweep_tile<double, P, MX, MY, (CSM != 0), MAXT, MINB>},
+  {P, MX, MY, CSM, MAXT, 0, MINB, (const void *)k_sweep_tile<double, P, MX, MY, (CSM != 0), MAXT, MINB>},
 #define W_ENTRY(P, M, CSM, MAXT, MINB) \
-  {P, M, M, CSM, MAXT, 1, (const void *)k_sweep_ws<double, P, M, (CSM != 0), MAXT, MINB>},
+  {P, M, M, CSM, MAXT, 1, MINB, (const void *)k_sweep_ws<double, P, M, (CSM != 0), MAXT, MINB>},
 static const TileEntry kTilesF64[] = {HZ_WS_TABLE_F64(W_ENTRY) HZ_TILE_TABLE_F64(X_ENTRY)};
 #undef X_ENTRY
 #undef W_ENTRY
@@ -37,9 +38,8 @@ static const int kNumTilesF64 = sizeof(kTilesF64) / sizeof(kTilesF64[0]);
 cudaError_t launch_sweep_dof_f64(const SweepArgs<double> &a, int p, SweepLaunch cfg, cudaStream_t st) {
   return launch_dof_impl<double>(a, p, cfg, st);
 }
-cudaError_t launch_sweep_tile_f64(const SweepArgs<double> &a, int p, int mx, int my, int csm, int ws, SweepLaunch cfg,
-                                  cudaStream_t st) {
-  return launch_tile_impl<double>(kTilesF64, kNumTilesF64, a, p, mx, my, csm, ws, cfg, st);
+cudaError_t launch_sweep_tile_f64(const SweepArgs<double> &a, int entry, SweepLaunch cfg, cudaStream_t st) {
+  return launch_tile_impl<double>(kTilesF64, kNumTilesF64, a, entry, cfg, st);
 }
 int tile_table_f64(const TileEntry **out) {
   *out = kTilesF64;

@@ -24,19 +24,15 @@ static cudaError_t launch_dof_impl(const SweepArgs<real> &a, int p, SweepLaunch 
 }
 
 template <typename real>
-static cudaError_t launch_tile_impl(const TileEntry *tab, int n, const SweepArgs<real> &a, int p, int mx, int my,
-                                    int csm, int ws, SweepLaunch cfg, cudaStream_t st) {
-  for (int i = 0; i < n; ++i) {
-    const TileEntry &e = tab[i];
-    if (e.p == p && e.mx == mx && e.my == my && e.csm == csm && e.ws == ws && cfg.threads <= e.maxt) {
-      auto fn = reinterpret_cast<void (*)(const SweepArgs<real>)>(const_cast<void *>(e.fn));
-      cudaError_t err = cudaFuncSetAttribute(e.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem);
-      if (err != cudaSuccess) return err;
-      fn<<<cfg.blocks, cfg.threads, cfg.smem, st>>>(a);
-      return cudaGetLastError();
-    }
-  }
-  return cudaErrorInvalidValue;
+static cudaError_t launch_tile_impl(const TileEntry *tab, int n, const SweepArgs<real> &a, int entry, SweepLaunch cfg,
+                                    cudaStream_t st) {
+  if (entry < 0 || entry >= n || cfg.threads > tab[entry].maxt) return cudaErrorInvalidValue;
+  const TileEntry &e = tab[entry];
+  auto fn = reinterpret_cast<void (*)(const SweepArgs<real>)>(const_cast<void *>(e.fn));
+  cudaError_t err = cudaFuncSetAttribute(e.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem);
+  if (err != cudaSuccess) return err;
+  fn<<<cfg.blocks, cfg.threads, cfg.smem, st>>>(a);
+  return cudaGetLastError();
 }
 
 }  // namespace hz

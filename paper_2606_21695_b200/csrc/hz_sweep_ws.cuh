@@ -60,6 +60,48 @@ __device__ __forceinline__ void line_apply(const real (&q)[M * P + 1], real pin,
   }
 }
 
+// Own-only part of one tile line (no neighbour data): S[n] (+)= terms over q[0..T-1] for n >= 1; returns the
+// unscaled own part of node 0.
+template <typename real, int P, int M, bool ACC, typename KT>
+__device__ __forceinline__ real line_own(const real (&q)[M * P + 1], real d0, const KT &k, real (&S)[M * P]) {
+  constexpr int T = M * P;
+  real t0 = d0 * q[0];
+#pragma unroll
+  for (int c = 1; c <= P; ++c)
+    if (c < T) t0 = fmaT(k.k0[c], q[c], t0);
+#pragma unroll
+  for (int e = 0; e < M; ++e) {
+#pragma unroll
+    for (int a = 1; a < P; ++a) {
+      real t = ACC ? fmaT(k.kin[a][0], q[e * P], S[e * P + a]) : k.kin[a][0] * q[e * P];
+#pragma unroll
+      for (int c = 1; c <= P; ++c)
+        if (e * P + c < T) t = fmaT(k.kin[a][c], q[e * P + c], t);
+      S[e * P + a] = t;
+    }
+    if (e > 0) {
+      real t = ACC ? fmaT(k.k0[0] + k.kp[P], q[e * P], S[e * P]) : (k.k0[0] + k.kp[P]) * q[e * P];
+#pragma unroll
+      for (int c = 0; c < P; ++c) t = fmaT(k.kp[c], q[(e - 1) * P + c], t);
+#pragma unroll
+      for (int c = 1; c <= P; ++c)
+        if (e * P + c < T) t = fmaT(k.k0[c], q[e * P + c], t);
+      S[e * P] = t;
+    }
+  }
+  return t0;
+}
+// Neighbour part: qT = first node of the next tile along the line, pin = partial sum from the previous tile.
+template <typename real, int P, int M, bool ACC0, typename KT>
+__device__ __forceinline__ void line_finish(real qT, real pin, real s0, real t0, const KT &k, real (&S)[M * P]) {
+#pragma unroll
+  for (int a = 1; a < P; ++a) S[(M - 1) * P + a] = fmaT(k.kin[a][P], qT, S[(M - 1) * P + a]);
+  if (M == 1) t0 = fmaT(k.k0[P], qT, t0);
+  else S[(M - 1) * P] = fmaT(k.k0[P], qT, S[(M - 1) * P]);
+  t0 += pin;
+  S[0] = ACC0 ? fmaT(s0, t0, S[0]) : s0 * t0;
+}
+
 template <typename real, int P, int M, typename KT>
 __device__ __forceinline__ real line_partial(const real (&q)[M * P + 1], const KT &k) {
   real s = k.kp[0] * q[(M - 1) * P];
@@ -144,32 +186,30 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
     }
     // Assemble b from lambda^n: bulk tiles touch only the W side (tx = 0) and the S side (ty = 0)
     const bool onW = act && tx == 0 && six > 0, onS = act && ty == 0 && siy > 0;
-    real lcr[T], lci[T], lrr[T], lri[T];
-#pragma unroll
-    for (int b = 0; b < T; ++b) { lcr[b] = 0; lci[b] = 0; lrr[b] = 0; lri[b] = 0; }
+    // (lambda^n is re-read from global memory in the epilogue instead of being held in registers)
     if (onW) {
 #pragma unroll
       for (int b = 0; b < T; ++b) {
         const int j = ty * T + b;
-        lcr[b] = A.lam[lbase + (kSideW * 2 + 0) * A.E + j];
-        lci[b] = A.lam[lbase + (kSideW * 2 + 1) * A.E + j];
+        const real lr_ = A.lam[lbase + (kSideW * 2 + 0) * A.E + j];
+        const real li_ = A.lam[lbase + (kSideW * 2 + 1) * A.E + j];
         const real s = A.bs[ebase + kSideW * A.E + j];
-        if (CSM) csm[(KT + b * T) * NTH + h] = fmaT(s, lcr[b], csm[(KT + b * T) * NTH + h]);
-        else bbr[CSM ? 0 : b][0] = fmaT(s, lcr[b], bbr[CSM ? 0 : b][0]);
-        bic[b] = fmaT(s, lci[b], bic[b]);
+        if (CSM) csm[(KT + b * T) * NTH + h] = fmaT(s, lr_, csm[(KT + b * T) * NTH + h]);
+        else bbr[CSM ? 0 : b][0] = fmaT(s, lr_, bbr[CSM ? 0 : b][0]);
+        bic[b] = fmaT(s, li_, bic[b]);
       }
     }
     if (onS) {
 #pragma unroll
       for (int a = 0; a < T; ++a) {
         const int i = tx * T + a;
-        lrr[a] = A.lam[lbase + (kSideS * 2 + 0) * A.E + i];
-        lri[a] = A.lam[lbase + (kSideS * 2 + 1) * A.E + i];
+        const real lr_ = A.lam[lbase + (kSideS * 2 + 0) * A.E + i];
+        const real li_ = A.lam[lbase + (kSideS * 2 + 1) * A.E + i];
         const real s = A.bs[ebase + kSideS * A.E + i];
-        if (CSM) csm[(KT + a) * NTH + h] = fmaT(s, lrr[a], csm[(KT + a) * NTH + h]);
-        else bbr[0][CSM ? 0 : a] = fmaT(s, lrr[a], bbr[0][CSM ? 0 : a]);
-        if (a == 0) bic[0] = fmaT(s, lri[a], bic[0]);
-        else bir[a] = fmaT(s, lri[a], bir[a]);
+        if (CSM) csm[(KT + a) * NTH + h] = fmaT(s, lr_, csm[(KT + a) * NTH + h]);
+        else bbr[0][CSM ? 0 : a] = fmaT(s, lr_, bbr[0][CSM ? 0 : a]);
+        if (a == 0) bic[0] = fmaT(s, li_, bic[0]);
+        else bir[a] = fmaT(s, li_, bir[a]);
       }
     }
     bar_sync_all(NTH);
@@ -212,28 +252,53 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
           my[3 * T + a] = p[0][a];
         }
         bar_sync_all(NTH);
+        // issue the neighbour loads first, then do the part of the step that needs none of them
         const real *nL = pL + cur, *nR = pR + cur, *nD = pD + cur, *nU = pU + cur;
         cur = BUFW - cur;
-        real S[T][T];
+        real qR[T], piL[T], qU[T], piD[T];
+#pragma unroll
+        for (int b = 0; b < T; ++b) { qR[b] = nR[T + b]; piL[b] = nL[b]; }
+#pragma unroll
+        for (int a = 0; a < T; ++a) { qU[a] = nU[3 * T + a]; piD[a] = nD[2 * T + a]; }
+        const Tab4<real> tn = tab[nu];
+        real S[T][T], X0[T], Y0[T];
 #pragma unroll
         for (int b = 0; b < T; ++b) {
           real q[T + 1];
 #pragma unroll
           for (int a = 0; a < T; ++a) q[a] = p[b][a];
-          q[T] = nR[T + b];
-          line_apply<real, P, M, false>(q, nL[b], d0x, s0x, A.ex1, S[b]);
+          q[T] = real(0);
+          X0[b] = line_own<real, P, M, false>(q, d0x, A.ex1, S[b]);
         }
 #pragma unroll
         for (int a = 0; a < T; ++a) {
           real q[T + 1], Sc[T];
 #pragma unroll
           for (int b = 0; b < T; ++b) { q[b] = p[b][a]; Sc[b] = S[b][a]; }
-          q[T] = nU[3 * T + a];
-          line_apply<real, P, M, true>(q, nD[2 * T + a], d0y, s0y, A.ey1, Sc);
+          q[T] = real(0);
+          if (a == 0) Y0[a] = line_own<real, P, M, false>(q, d0y, A.ey1, Sc);
+          else Y0[a] = line_own<real, P, M, true>(q, d0y, A.ey1, Sc);
+#pragma unroll
+          for (int b = 1; b < T; ++b) S[b][a] = Sc[b];
+        }
+#pragma unroll
+        for (int b = 0; b < T; ++b)
+#pragma unroll
+          for (int a = 0; a < T; ++a) vr[b][a] = fmaT(tn.k, p[b][a], vr[b][a]);
+#pragma unroll
+        for (int b = 0; b < T; ++b) {
+          if (b == 0) line_finish<real, P, M, false>(qR[b], piL[b], s0x, X0[b], A.ex1, S[b]);
+          else line_finish<real, P, M, true>(qR[b], piL[b], s0x, X0[b], A.ex1, S[b]);
+        }
+#pragma unroll
+        for (int a = 0; a < T; ++a) {
+          real Sc[T];
+#pragma unroll
+          for (int b = 0; b < T; ++b) Sc[b] = S[b][a];
+          line_finish<real, P, M, true>(qU[a], piD[a], s0y, Y0[a], A.ey1, Sc);
 #pragma unroll
           for (int b = 0; b < T; ++b) S[b][a] = Sc[b];
         }
-        const Tab4<real> tn = tab[nu];
 #pragma unroll
         for (int b = 0; b < T; ++b)
 #pragma unroll
@@ -250,7 +315,6 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
             } else {
               pd[b][a] += x;
             }
-            vr[b][a] = fmaT(tn.k, p[b][a], vr[b][a]);
             vi[b][a] = fmaT(tn.kh, pd[b][a], vi[b][a]);
           }
       }
@@ -276,8 +340,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
       for (int b = 0; b < T; ++b) {
         const int j = ty * T + b;
         const real k2 = A.k2edge[ebase + kSideW * A.E + j];
-        A.gout[lbase + (kSideW * 2 + 0) * A.E + j] = fmaT(k2, ui[b][0], -lcr[b]);
-        A.gout[lbase + (kSideW * 2 + 1) * A.E + j] = fmaT(-k2, ur[b][0], -lci[b]);
+        A.gout[lbase + (kSideW * 2 + 0) * A.E + j] = fmaT(k2, ui[b][0], -A.lam[lbase + (kSideW * 2 + 0) * A.E + j]);
+        A.gout[lbase + (kSideW * 2 + 1) * A.E + j] = fmaT(-k2, ur[b][0], -A.lam[lbase + (kSideW * 2 + 1) * A.E + j]);
       }
     }
     if (onS) {
@@ -285,8 +349,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
       for (int a = 0; a < T; ++a) {
         const int i = tx * T + a;
         const real k2 = A.k2edge[ebase + kSideS * A.E + i];
-        A.gout[lbase + (kSideS * 2 + 0) * A.E + i] = fmaT(k2, ui[0][a], -lrr[a]);
-        A.gout[lbase + (kSideS * 2 + 1) * A.E + i] = fmaT(-k2, ur[0][a], -lri[a]);
+        A.gout[lbase + (kSideS * 2 + 0) * A.E + i] = fmaT(k2, ui[0][a], -A.lam[lbase + (kSideS * 2 + 0) * A.E + i]);
+        A.gout[lbase + (kSideS * 2 + 1) * A.E + i] = fmaT(-k2, ur[0][a], -A.lam[lbase + (kSideS * 2 + 1) * A.E + i]);
       }
     }
   } else {
@@ -356,22 +420,20 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
     if (act && top && tx == 0 && six > 0) { side2 = kSideW; idx2 = lny - 1; }
     if (act && top && tx == ntx - 1 && six < A.sx - 1) { side2 = kSideE; idx2 = lny - 1; }
     if (act && !top && ty == 0 && siy > 0) { side2 = kSideS; idx2 = lnx - 1; }
-    real l1r[T], l1i[T], l2r = 0, l2i = 0;
 #pragma unroll
     for (int n = 0; n < T; ++n) {
-      l1r[n] = 0; l1i[n] = 0;
       const int idx = ta * T + n;
       if (on1 && idx < len1) {
-        l1r[n] = A.lam[lbase + (side1 * 2 + 0) * A.E + idx];
-        l1i[n] = A.lam[lbase + (side1 * 2 + 1) * A.E + idx];
+        const real lr_ = A.lam[lbase + (side1 * 2 + 0) * A.E + idx];
+        const real li_ = A.lam[lbase + (side1 * 2 + 1) * A.E + idx];
         const real s = A.bs[ebase + side1 * A.E + idx];
-        bbr[n] = fmaT(s, l1r[n], bbr[n]);
-        bbi[n] = fmaT(s, l1i[n], bbi[n]);
+        bbr[n] = fmaT(s, lr_, bbr[n]);
+        bbi[n] = fmaT(s, li_, bbi[n]);
       }
     }
     if (side2 >= 0) {
-      l2r = A.lam[lbase + (side2 * 2 + 0) * A.E + idx2];
-      l2i = A.lam[lbase + (side2 * 2 + 1) * A.E + idx2];
+      const real l2r = A.lam[lbase + (side2 * 2 + 0) * A.E + idx2];
+      const real l2i = A.lam[lbase + (side2 * 2 + 1) * A.E + idx2];
       const real s = A.bs[ebase + side2 * A.E + idx2];
       bbr[0] = fmaT(s, l2r, bbr[0]);
       bbi[0] = fmaT(s, l2i, bbi[0]);
@@ -400,19 +462,25 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
 #pragma unroll
         for (int n = 0; n < T; ++n) raw[n] = p[n];
         bar_sync_all(NTH);
-        q[T] = pN[cur];
-        real S[T];
-        line_apply<real, P, M, false>(q, pP[cur], d0a, s0a, ka, S);
+        const real qN = pN[cur], piP = pP[cur];
+        real piC[T];
 #pragma unroll
-        for (int n = 0; n < T; ++n) S[n] = fmaT(s0c, fmaT(d0c, p[n], pC[cur + n]), S[n]);
+        for (int n = 0; n < T; ++n) piC[n] = pC[cur + n];
         cur = BUFW - cur;
         const Tab4<real> tn = tab[nu];
+        real S[T];
+        const real a0 = line_own<real, P, M, false>(q, d0a, ka, S);
+        real cown[T];
+#pragma unroll
+        for (int n = 0; n < T; ++n) { cown[n] = d0c * p[n]; vr[n] = fmaT(tn.k, p[n], vr[n]); }
+        line_finish<real, P, M, false>(qN, piP, s0a, a0, ka, S);
+#pragma unroll
+        for (int n = 0; n < T; ++n) S[n] = fmaT(s0c, cown[n] + piC[n], S[n]);
 #pragma unroll
         for (int n = 0; n < T; ++n) {
           real x = fmaT(-gam[n], S[n], bbr[n] * tn.c);
           x = fmaT(bbi[n], tn.s, x);
           pd[n] = fmaT(al[n], pd[n], x);
-          vr[n] = fmaT(tn.k, p[n], vr[n]);
           vi[n] = fmaT(tn.kh, pd[n], vi[n]);
         }
       }
@@ -431,14 +499,14 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
         const int idx = ta * T + n;
         if (on1 && idx < len1) {
           const real k2 = A.k2edge[ebase + side1 * A.E + idx];
-          A.gout[lbase + (side1 * 2 + 0) * A.E + idx] = fmaT(k2, ui[n], -l1r[n]);
-          A.gout[lbase + (side1 * 2 + 1) * A.E + idx] = fmaT(-k2, ur[n], -l1i[n]);
+          A.gout[lbase + (side1 * 2 + 0) * A.E + idx] = fmaT(k2, ui[n], -A.lam[lbase + (side1 * 2 + 0) * A.E + idx]);
+          A.gout[lbase + (side1 * 2 + 1) * A.E + idx] = fmaT(-k2, ur[n], -A.lam[lbase + (side1 * 2 + 1) * A.E + idx]);
         }
       }
       if (side2 >= 0) {
         const real k2 = A.k2edge[ebase + side2 * A.E + idx2];
-        A.gout[lbase + (side2 * 2 + 0) * A.E + idx2] = fmaT(k2, ui[0], -l2r);
-        A.gout[lbase + (side2 * 2 + 1) * A.E + idx2] = fmaT(-k2, ur[0], -l2i);
+        A.gout[lbase + (side2 * 2 + 0) * A.E + idx2] = fmaT(k2, ui[0], -A.lam[lbase + (side2 * 2 + 0) * A.E + idx2]);
+        A.gout[lbase + (side2 * 2 + 1) * A.E + idx2] = fmaT(-k2, ur[0], -A.lam[lbase + (side2 * 2 + 1) * A.E + idx2]);
       }
     }
   }
