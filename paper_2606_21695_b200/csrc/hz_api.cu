@@ -150,6 +150,9 @@ struct hz_ctx {
   double *d_part = nullptr, *d_red = nullptr, *d_ures = nullptr;
   int res_blocks = 0;
   Elem1D<double> ex1{}, ey1{};
+  std::vector<double> h_tab;  // host copy of the time-step table (kernel-parameter form of the ws kernel)
+  TabC<float> tc32{};
+  TabC<double> tc64{};
   std::string err;
 };
 
@@ -264,11 +267,11 @@ cudaError_t launch_sweep(const hz_ctx *c, const hz_solve_opts *o, cudaStream_t s
   if (c->prec == HZ_F32) {
     SweepArgs<float> a = make_args<float>(c, o);
     return c->lay.variant == 0 ? launch_sweep_dof_f32(a, c->p, c->launch, st)
-                               : launch_sweep_tile_f32(a, c->entry, c->launch, st);
+                               : launch_sweep_tile_f32(a, &c->tc32, c->entry, c->launch, st);
   }
   SweepArgs<double> a = make_args<double>(c, o);
   return c->lay.variant == 0 ? launch_sweep_dof_f64(a, c->p, c->launch, st)
-                             : launch_sweep_tile_f64(a, c->entry, c->launch, st);
+                             : launch_sweep_tile_f64(a, &c->tc64, c->entry, c->launch, st);
 }
 
 cudaError_t launch_exchange(const hz_ctx *c, double rho, cudaStream_t st) {
@@ -460,11 +463,11 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
     size_t sm = 0;
     const size_t narr = 2 * (size_t)(q.TX + q.TY);
     if (t.ws) {
-      if (no_ws) return false;
+      if (no_ws || n_t > kTabCMax) return false;
       nthr = roundup((q.ntx - 1) * (q.nty - 1), 32) + roundup(q.ntx + q.nty - 1, 32);
       const int nbulk = (q.ntx - 1) * (q.nty - 1), nedge = q.ntx + q.nty - 1;
       const size_t nrec = (size_t)roundup(nbulk + q.ntx, 32) + 64 + roundup(nedge, 32);
-      sm = tab_bytes + 2 * nrec * (narr + 1) * rs + (t.csm ? 2 * (size_t)q.TX * q.TY * nthr * rs : 0);
+      sm = 2 * nrec * (narr + 1) * rs + (t.csm ? 2 * (size_t)q.TX * q.TY * nthr * rs : 0);
     } else {
       sm = tab_bytes + 2 * narr * (nthr + 1) * rs + (t.csm ? 2 * (size_t)q.TX * q.TY * nthr * rs : 0);
     }
@@ -523,6 +526,10 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
     tab[4 * nu + 1] = std::sin(2.0 * M_PI * nu / n_t);
     tab[4 * nu + 2] = std::cos(2.0 * M_PI * nu / n_t) - 0.25 + 0.25 * tan2;                       // kappa_nu
     tab[4 * nu + 3] = (std::cos(2.0 * M_PI * (nu + 0.5) / n_t) - 0.25 + 0.25 * tan2) / ctx->omega;  // kappa_{nu+1/2}/omega
+  }
+  for (int nu = 0; nu < n_t && nu < kTabCMax; ++nu) {
+    ctx->tc32.t[nu] = Tab4<float>{(float)tab[4 * nu], (float)tab[4 * nu + 1], (float)tab[4 * nu + 2], (float)tab[4 * nu + 3]};
+    ctx->tc64.t[nu] = Tab4<double>{tab[4 * nu], tab[4 * nu + 1], tab[4 * nu + 2], tab[4 * nu + 3]};
   }
   std::vector<double> bandx, bandy, wxl, wyl;
   make_band(ctx->gll, ctx->ex, ctx->hx, &bandx, &wxl);

@@ -34,6 +34,15 @@ struct __align__(16) Tab4 {
   real c, s, k, kh;
 };
 
+// The whole time-step table as a by-value kernel parameter (constant bank): the step index is warp-uniform, so
+// the kernel reads a row with uniform loads into uniform registers and the FMAs that use it keep a free
+// vector-register read port.  Used by the warp-specialised kernel when n_t <= kTabCMax.
+constexpr int kTabCMax = 256;
+template <typename real>
+struct TabC {
+  Tab4<real> t[kTabCMax];
+};
+
 // 1-D element constants of the register-blocked kernel, already scaled by 4/h^2 and the GLL weights:
 //   kin[a][c] = (4/h^2) K[a][c] / w_a        rows of element-interior nodes a = 1..P-1
 //   k0[c]     = (4/h^2) K[0][c] / (2 w_0)    row of an element's first node (shared with the element before)
@@ -83,8 +92,10 @@ struct SweepLaunch {
 // Implemented in hz_sweep_*.cu.  Return cudaErrorInvalidValue when no instantiation matches.
 cudaError_t launch_sweep_dof_f32(const SweepArgs<float> &a, int p, SweepLaunch cfg, cudaStream_t st);
 cudaError_t launch_sweep_dof_f64(const SweepArgs<double> &a, int p, SweepLaunch cfg, cudaStream_t st);
-cudaError_t launch_sweep_tile_f32(const SweepArgs<float> &a, int entry, SweepLaunch cfg, cudaStream_t st);
-cudaError_t launch_sweep_tile_f64(const SweepArgs<double> &a, int entry, SweepLaunch cfg, cudaStream_t st);
+cudaError_t launch_sweep_tile_f32(const SweepArgs<float> &a, const TabC<float> *tc, int entry, SweepLaunch cfg,
+                                  cudaStream_t st);
+cudaError_t launch_sweep_tile_f64(const SweepArgs<double> &a, const TabC<double> *tc, int entry, SweepLaunch cfg,
+                                  cudaStream_t st);
 // compiled register-blocked instantiations of one precision
 int tile_table_f32(const TileEntry **out);
 int tile_table_f64(const TileEntry **out);

@@ -38,8 +38,9 @@ static const int kNumTilesF32 = sizeof(kTilesF32) / sizeof(kTilesF32[0]);
 cudaError_t launch_sweep_dof_f32(const SweepArgs<float> &a, int p, SweepLaunch cfg, cudaStream_t st) {
   return launch_dof_impl<float>(a, p, cfg, st);
 }
-cudaError_t launch_sweep_tile_f32(const SweepArgs<float> &a, int entry, SweepLaunch cfg, cudaStream_t st) {
-  return launch_tile_impl<float>(kTilesF32, kNumTilesF32, a, entry, cfg, st);
+cudaError_t launch_sweep_tile_f32(const SweepArgs<float> &a, const TabC<float> *tc, int entry, SweepLaunch cfg,
+                                  cudaStream_t st) {
+  return launch_tile_impl<float>(kTilesF32, kNumTilesF32, a, tc, entry, cfg, st);
 }
 int tile_table_f32(const TileEntry **out) {
   *out = kTilesF32;

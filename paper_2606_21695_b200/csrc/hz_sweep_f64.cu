@@ -38,8 +38,9 @@ static const int kNumTilesF64 = sizeof(kTilesF64) / sizeof(kTilesF64[0]);
 cudaError_t launch_sweep_dof_f64(const SweepArgs<double> &a, int p, SweepLaunch cfg, cudaStream_t st) {
   return launch_dof_impl<double>(a, p, cfg, st);
 }
-cudaError_t launch_sweep_tile_f64(const SweepArgs<double> &a, int entry, SweepLaunch cfg, cudaStream_t st) {
-  return launch_tile_impl<double>(kTilesF64, kNumTilesF64, a, entry, cfg, st);
+cudaError_t launch_sweep_tile_f64(const SweepArgs<double> &a, const TabC<double> *tc, int entry, SweepLaunch cfg,
+                                  cudaStream_t st) {
+  return launch_tile_impl<double>(kTilesF64, kNumTilesF64, a, tc, entry, cfg, st);
 }
 int tile_table_f64(const TileEntry **out) {
   *out = kTilesF64;

@@ -24,14 +24,20 @@ static cudaError_t launch_dof_impl(const SweepArgs<real> &a, int p, SweepLaunch 
 }
 
 template <typename real>
-static cudaError_t launch_tile_impl(const TileEntry *tab, int n, const SweepArgs<real> &a, int entry, SweepLaunch cfg,
-                                    cudaStream_t st) {
+static cudaError_t launch_tile_impl(const TileEntry *tab, int n, const SweepArgs<real> &a, const TabC<real> *tc, int entry,
+                                    SweepLaunch cfg, cudaStream_t st) {
   if (entry < 0 || entry >= n || cfg.threads > tab[entry].maxt) return cudaErrorInvalidValue;
   const TileEntry &e = tab[entry];
-  auto fn = reinterpret_cast<void (*)(const SweepArgs<real>)>(const_cast<void *>(e.fn));
   cudaError_t err = cudaFuncSetAttribute(e.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem);
   if (err != cudaSuccess) return err;
-  fn<<<cfg.blocks, cfg.threads, cfg.smem, st>>>(a);
+  if (e.ws) {
+    if (!tc) return cudaErrorInvalidValue;
+    auto fn = reinterpret_cast<void (*)(const SweepArgs<real>, const TabC<real>)>(const_cast<void *>(e.fn));
+    fn<<<cfg.blocks, cfg.threads, cfg.smem, st>>>(a, *tc);
+  } else {
+    auto fn = reinterpret_cast<void (*)(const SweepArgs<real>)>(const_cast<void *>(e.fn));
+    fn<<<cfg.blocks, cfg.threads, cfg.smem, st>>>(a);
+  }
   return cudaGetLastError();
 }
 

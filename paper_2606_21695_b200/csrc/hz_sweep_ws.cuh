@@ -111,11 +111,10 @@ __device__ __forceinline__ real line_partial(const real (&q)[M * P + 1], const K
 }
 
 template <typename real, int P, int M, bool CSM, int MAXT, int MINB>
-__global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A) {
+__global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A, const __grid_constant__ TabC<real> TC) {
   constexpr int T = M * P, KT = T * T;
   constexpr int RS = 4 * T + 1;  // record stride (words of `real`)
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  Tab4<real> *tab = reinterpret_cast<Tab4<real> *>(smem_raw);
   const int h = threadIdx.x, NTH = blockDim.x, l = blockIdx.x;
   const int ntx = A.lay.ntx, nty = A.lay.nty, NTV = A.lay.NT, NS = A.lay.NS;
   const int lnx = A.lay.lnx, lny = A.lay.lny;
@@ -123,12 +122,11 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
   const int bulk_warps = (nbulk + 31) >> 5;
   const int NB = (nbulk + ntx + 31) & ~31, ZR = NB, SCR = NB + 32, EB = NB + 64;
   const int BUFW = (NB + 64 + ((nedge + 31) & ~31)) * RS;
-  real *xb = reinterpret_cast<real *>(tab + A.n_t);
+  real *xb = reinterpret_cast<real *>(smem_raw);
   real *csm = xb + 2 * BUFW;  // CSM: [2][KT][NTH] gamma | beta b_r of the bulk tiles
   const int warp = h >> 5, lane = h & 31;
 
   for (int q = h; q < 2 * BUFW; q += NTH) xb[q] = real(0);
-  for (int q = h; q < A.n_t; q += NTH) tab[q] = A.tab[q];
 
   const int six = l % A.sx, siy = l / A.sx;
   const size_t lbase = (size_t)l * 4 * 2 * A.E, ebase = (size_t)l * 4 * A.E;
@@ -216,7 +214,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
 
     int cur = 0;
     for (int m = 0; m < A.n_wh; ++m) {
-      const Tab4<real> t0 = tab[0];
+      const Tab4<real> t0 = TC.t[0];
 #pragma unroll
       for (int b = 0; b < T; ++b)
 #pragma unroll
@@ -260,7 +258,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
         for (int b = 0; b < T; ++b) { qR[b] = nR[T + b]; piL[b] = nL[b]; }
 #pragma unroll
         for (int a = 0; a < T; ++a) { qU[a] = nU[3 * T + a]; piD[a] = nD[2 * T + a]; }
-        const Tab4<real> tn = tab[nu];
+        const Tab4<real> tn = TC.t[nu];
         real S[T][T], X0[T], Y0[T];
 #pragma unroll
         for (int b = 0; b < T; ++b) {
@@ -305,15 +303,14 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
           for (int a = 0; a < T; ++a) {
             const real g_ = CSM ? csm[(b * T + a) * NTH + h] : gam[CSM ? 0 : b][CSM ? 0 : a];
             const real r_ = CSM ? csm[(KT + b * T + a) * NTH + h] : bbr[CSM ? 0 : b][CSM ? 0 : a];
-            real x = fmaT(-g_, S[b][a], r_ * tn.c);
             if (a == 0) {
-              x = fmaT(bic[b], tn.s, x);
+              const real x = fmaT(bic[b], tn.s, fmaT(-g_, S[b][a], r_ * tn.c));
               pd[b][a] = fmaT(alc[b], pd[b][a], x);
             } else if (b == 0) {
-              x = fmaT(bir[a], tn.s, x);
+              const real x = fmaT(bir[a], tn.s, fmaT(-g_, S[b][a], r_ * tn.c));
               pd[b][a] = fmaT(alr[a], pd[b][a], x);
-            } else {
-              pd[b][a] += x;
+            } else {  // interior of the subdomain: alpha = 1, Im b = 0
+              pd[b][a] = fmaT(r_, tn.c, fmaT(-g_, S[b][a], pd[b][a]));
             }
             vi[b][a] = fmaT(tn.kh, pd[b][a], vi[b][a]);
           }
@@ -442,7 +439,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
 
     int cur = 0;
     for (int m = 0; m < A.n_wh; ++m) {
-      const Tab4<real> t0 = tab[0];
+      const Tab4<real> t0 = TC.t[0];
 #pragma unroll
       for (int n = 0; n < T; ++n) {
         p[n] = ur[n];
@@ -467,7 +464,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
 #pragma unroll
         for (int n = 0; n < T; ++n) piC[n] = pC[cur + n];
         cur = BUFW - cur;
-        const Tab4<real> tn = tab[nu];
+        const Tab4<real> tn = TC.t[nu];
         real S[T];
         const real a0 = line_own<real, P, M, false>(q, d0a, ka, S);
         real cown[T];
