@@ -7,8 +7,8 @@
 // line-only code path.  In k_sweep_tile the ragged tiles execute the full-tile instruction stream on
 // padding (28 % of the issue slots at 8x8 elements, p = 3); here they cost a fraction of a warp.
 //
-// Exchange records of RS = 2(TX+TY)+1 words (odd stride: lane-consecutive records are conflict-free for
-// 32- and 64-bit accesses):  PX[b] | RX[b] | PY[a] | RY[a].  Bulk thread h owns record h; what it reads is
+// Exchange records of four 16-byte-aligned chunks PX[b] | RX[b] | PY[a] | RY[a] plus 16 bytes of padding (an odd
+// number of 16-byte units: lane-consecutive records are conflict-free for the 128-bit accesses used).  Bulk thread h owns record h; what it reads is
 // ALWAYS record h-1 / h+1 / h-w / h+w (w = ntx-1 bulk tiles per row) or a zero record of the same bank, so
 // every bulk access is conflict-free.  To make that true at the far edges, a right edge piece publishes its
 // raw values into the RX fields of record (ty+1)*w (the first bulk tile of the next row, whose own RX has no
@@ -102,6 +102,50 @@ __device__ __forceinline__ void line_finish(real qT, real pin, real s0, real t0,
   S[0] = ACC0 ? fmaT(s0, t0, S[0]) : s0 * t0;
 }
 
+// Vectorised access to one record chunk of N values (16-byte aligned, padded to a multiple of 16 bytes).
+template <int N>
+__device__ __forceinline__ void st_chunk(float *dst, const float (&v)[N]) {
+#pragma unroll
+  for (int i = 0; i < (N + 3) / 4; ++i) {
+    float4 x;
+    x.x = v[4 * i];
+    x.y = 4 * i + 1 < N ? v[4 * i + 1 < N ? 4 * i + 1 : 0] : 0.f;
+    x.z = 4 * i + 2 < N ? v[4 * i + 2 < N ? 4 * i + 2 : 0] : 0.f;
+    x.w = 4 * i + 3 < N ? v[4 * i + 3 < N ? 4 * i + 3 : 0] : 0.f;
+    reinterpret_cast<float4 *>(dst)[i] = x;
+  }
+}
+template <int N>
+__device__ __forceinline__ void ld_chunk(const float *src, float (&v)[N]) {
+#pragma unroll
+  for (int i = 0; i < (N + 3) / 4; ++i) {
+    const float4 x = reinterpret_cast<const float4 *>(src)[i];
+    v[4 * i] = x.x;
+    if (4 * i + 1 < N) v[4 * i + 1 < N ? 4 * i + 1 : 0] = x.y;
+    if (4 * i + 2 < N) v[4 * i + 2 < N ? 4 * i + 2 : 0] = x.z;
+    if (4 * i + 3 < N) v[4 * i + 3 < N ? 4 * i + 3 : 0] = x.w;
+  }
+}
+template <int N>
+__device__ __forceinline__ void st_chunk(double *dst, const double (&v)[N]) {
+#pragma unroll
+  for (int i = 0; i < (N + 1) / 2; ++i) {
+    double2 x;
+    x.x = v[2 * i];
+    x.y = 2 * i + 1 < N ? v[2 * i + 1 < N ? 2 * i + 1 : 0] : 0.0;
+    reinterpret_cast<double2 *>(dst)[i] = x;
+  }
+}
+template <int N>
+__device__ __forceinline__ void ld_chunk(const double *src, double (&v)[N]) {
+#pragma unroll
+  for (int i = 0; i < (N + 1) / 2; ++i) {
+    const double2 x = reinterpret_cast<const double2 *>(src)[i];
+    v[2 * i] = x.x;
+    if (2 * i + 1 < N) v[2 * i + 1 < N ? 2 * i + 1 : 0] = x.y;
+  }
+}
+
 template <typename real, int P, int M, typename KT>
 __device__ __forceinline__ real line_partial(const real (&q)[M * P + 1], const KT &k) {
   real s = k.kp[0] * q[(M - 1) * P];
@@ -113,7 +157,11 @@ __device__ __forceinline__ real line_partial(const real (&q)[M * P + 1], const K
 template <typename real, int P, int M, bool CSM, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A, const __grid_constant__ TabC<real> TC) {
   constexpr int T = M * P, KT = T * T;
-  constexpr int RS = 4 * T + 1;  // record stride (words of `real`)
+  // record = 4 chunks PX | RX | PY | RY of CH values each (T padded to 16 bytes) + 16 bytes of padding, so the
+  // stride is an odd number of 16-byte units: lane-consecutive records are conflict-free for 128-bit accesses
+  constexpr int V16 = 16 / (int)sizeof(real);
+  constexpr int CH = (T + V16 - 1) / V16 * V16;
+  constexpr int RS = 4 * CH + V16;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int h = threadIdx.x, NTH = blockDim.x, l = blockIdx.x;
   const int ntx = A.lay.ntx, nty = A.lay.nty, NTV = A.lay.NT, NS = A.lay.NS;
@@ -144,7 +192,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
     const int rU = act ? h + w : ZR + ((h + w) & 31);
     const real *pL = xb + rL * RS, *pR = xb + rR * RS, *pD = xb + rD * RS, *pU = xb + rU * RS;
     real *pMy = xb + rMy * RS;
-    real *pMyRX = xb + ((act && tx > 0) ? h : SCR + lane) * RS + T;  // RX of a tx = 0 tile has no reader
+    real *pMyRX = xb + ((act && tx > 0) ? h : SCR + lane) * RS + CH;  // RX of a tx = 0 tile has no reader
     const bool hasL = tx > 0, hasD = ty > 0;
     const real d0x = A.ex1.k0[0] + (hasL ? A.ex1.kp[P] : real(0));
     const real d0y = A.ey1.k0[0] + (hasD ? A.ey1.kp[P] : real(0));
@@ -231,33 +279,40 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
 #pragma unroll
           for (int a = 0; a < T; ++a) p[b][a] = fmaT(sigma, pd[b][a], p[b][a]);
         real *my = pMy + cur, *myRX = pMyRX + cur;
+        {
+          real oPX[T], oRX[T], oPY[T], oRY[T];
 #pragma unroll
-        for (int b = 0; b < T; ++b) {
-          real q[T + 1];
+          for (int b = 0; b < T; ++b) {
+            real q[T + 1];
 #pragma unroll
-          for (int a = 0; a < T; ++a) q[a] = p[b][a];
-          q[T] = real(0);
-          my[b] = line_partial<real, P, M>(q, A.ex1);
-          myRX[b] = p[b][0];
-        }
+            for (int a = 0; a < T; ++a) q[a] = p[b][a];
+            q[T] = real(0);
+            oPX[b] = line_partial<real, P, M>(q, A.ex1);
+            oRX[b] = p[b][0];
+          }
 #pragma unroll
-        for (int a = 0; a < T; ++a) {
-          real q[T + 1];
+          for (int a = 0; a < T; ++a) {
+            real q[T + 1];
 #pragma unroll
-          for (int b = 0; b < T; ++b) q[b] = p[b][a];
-          q[T] = real(0);
-          my[2 * T + a] = line_partial<real, P, M>(q, A.ey1);
-          my[3 * T + a] = p[0][a];
+            for (int b = 0; b < T; ++b) q[b] = p[b][a];
+            q[T] = real(0);
+            oPY[a] = line_partial<real, P, M>(q, A.ey1);
+            oRY[a] = p[0][a];
+          }
+          st_chunk<T>(my, oPX);
+          st_chunk<T>(myRX, oRX);
+          st_chunk<T>(my + 2 * CH, oPY);
+          st_chunk<T>(my + 3 * CH, oRY);
         }
         bar_sync_all(NTH);
         // issue the neighbour loads first, then do the part of the step that needs none of them
         const real *nL = pL + cur, *nR = pR + cur, *nD = pD + cur, *nU = pU + cur;
         cur = BUFW - cur;
         real qR[T], piL[T], qU[T], piD[T];
-#pragma unroll
-        for (int b = 0; b < T; ++b) { qR[b] = nR[T + b]; piL[b] = nL[b]; }
-#pragma unroll
-        for (int a = 0; a < T; ++a) { qU[a] = nU[3 * T + a]; piD[a] = nD[2 * T + a]; }
+        ld_chunk<T>(nL, piL);
+        ld_chunk<T>(nR + CH, qR);
+        ld_chunk<T>(nD + 2 * CH, piD);
+        ld_chunk<T>(nU + 3 * CH, qU);
         const Tab4<real> tn = TC.t[nu];
         real S[T][T], X0[T], Y0[T];
 #pragma unroll
@@ -365,7 +420,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
     const int sa = top ? 1 : ntx;                         // virtual-tile stride along
     const int sc = top ? ntx : 1;                         // virtual-tile stride across
     // record field offsets: along partial / along raw / across partial (read from the bulk tile) / across raw
-    const int oPA = top ? 0 : 2 * T, oRA = top ? T : 3 * T, oPC = top ? 2 * T : 0, oRC = top ? 3 * T : T;
+    const int oPA = top ? 0 : 2 * CH, oRA = top ? CH : 3 * CH, oPC = top ? 2 * CH : 0, oRC = top ? 3 * CH : CH;
     const bool hasP = act && ta > 0, hasN = act && ta < nta - 1;
     // own record (along-the-edge exchange): EB + e
     real *pOwn = xb + (act ? EB + e : SCR + lane) * RS;
@@ -377,11 +432,11 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
     const int rP = hasP ? EB + e - 1 : ZR + ((e - 1) & 31);
     const real *pP = xb + rP * RS + oPA;
     const real *pN = !hasN ? xb + (ZR + ((e + 1) & 31)) * RS
-                           : ((!top && ty == nty - 2) ? xb + (nbulk + w) * RS + 3 * T : xb + (EB + e + 1) * RS + oRA);
+                           : ((!top && ty == nty - 2) ? xb + (nbulk + w) * RS + 3 * CH : xb + (EB + e + 1) * RS + oRA);
     // the partial sums from the tile across: bulk tile below / left; for the corner the last right piece's
     // along partial (field PY[0] of its own record; the fields after it stay zero)
     const real *pC = !act ? xb + (ZR + lane) * RS
-                          : (top ? (tx < w ? xb + ((nty - 2) * w + tx) * RS + 2 * T : xb + (EB + nty - 2) * RS + 2 * T)
+                          : (top ? (tx < w ? xb + ((nty - 2) * w + tx) * RS + 2 * CH : xb + (EB + nty - 2) * RS + 2 * CH)
                                  : xb + (ty * w + w - 1) * RS);
     Elem1D<real> ka;  // coefficients along
 #pragma unroll
@@ -456,13 +511,11 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
         real *my = pOwn + cur, *raw = pRaw + cur;
         my[oPA] = line_partial<real, P, M>(q, ka);
         my[oRA] = p[0];
-#pragma unroll
-        for (int n = 0; n < T; ++n) raw[n] = p[n];
+        st_chunk<T>(raw, p);
         bar_sync_all(NTH);
         const real qN = pN[cur], piP = pP[cur];
         real piC[T];
-#pragma unroll
-        for (int n = 0; n < T; ++n) piC[n] = pC[cur + n];
+        ld_chunk<T>(pC + cur, piC);
         cur = BUFW - cur;
         const Tab4<real> tn = TC.t[nu];
         real S[T];
