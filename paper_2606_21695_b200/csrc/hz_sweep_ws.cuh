@@ -7,18 +7,14 @@
 // line-only code path.  In k_sweep_tile the ragged tiles execute the full-tile instruction stream on
 // padding (28 % of the issue slots at 8x8 elements, p = 3); here they cost a fraction of a warp.
 //
-// Exchange records of four 16-byte-aligned chunks PX[b] | RX[b] | PY[a] | RY[a] plus 16 bytes of padding (an odd
-// number of 16-byte units: lane-consecutive records are conflict-free for the 128-bit accesses used).  Bulk thread h owns record h; what it reads is
-// ALWAYS record h-1 / h+1 / h-w / h+w (w = ntx-1 bulk tiles per row) or a zero record of the same bank, so
-// every bulk access is conflict-free.  To make that true at the far edges, a right edge piece publishes its
-// raw values into the RX fields of record (ty+1)*w (the first bulk tile of the next row, whose own RX has no
-// reader and is redirected to scratch) and a top piece into the RY fields of record nbulk+tx.
+// Exchange records: virtual tile v = ty*ntx + tx owns record v = four 16-byte-aligned chunks PX[b] | RX[b] |
+// PY[a] | RY[a] plus 16 bytes of padding (an odd number of 16-byte units, so 8 lane-consecutive records are
+// conflict-free for the 128-bit accesses used: one LDS.128 / STS.128 per chunk).
 //   PX[b]  partial sum  sum_{c<P} kp_x[c] p[b][last element, c]   (what the right neighbour's first column needs)
 //   RX[b]  raw p[b][0]                                           (what the left neighbour's last element needs)
-//   PY[a], RY[a] the same along y.
-// Records NB..NB+31 (NB = roundup32(nbulk+ntx)) are always zero (missing neighbours), NB+32..NB+63 are
-// write-only scratch, NB+64.. are the edge pieces' own records (along-the-edge exchange).  Two buffers
-// (ping-pong), one named barrier per time step.
+//   PY[a], RY[a] the same along y.  An edge piece uses element 0 of the chunks of its "along" direction.
+// Records NTV..NTV+31 are always zero (missing neighbours, same bank group as the record they stand in for),
+// NTV+32..NTV+63 are write-only scratch for idle lanes.  Two buffers (ping-pong), one named barrier per step.
 #pragma once
 #include "hz_sweep.cuh"
 
@@ -168,8 +164,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
   const int lnx = A.lay.lnx, lny = A.lay.lny;
   const int w = ntx - 1, nbulk = (ntx - 1) * (nty - 1), nedge = ntx + nty - 1;
   const int bulk_warps = (nbulk + 31) >> 5;
-  const int NB = (nbulk + ntx + 31) & ~31, ZR = NB, SCR = NB + 32, EB = NB + 64;
-  const int BUFW = (NB + 64 + ((nedge + 31) & ~31)) * RS;
+  const int ZR = NTV, SCR = NTV + 32;  // zero records, scratch records
+  const int BUFW = (NTV + 64) * RS;
   real *xb = reinterpret_cast<real *>(smem_raw);
   real *csm = xb + 2 * BUFW;  // CSM: [2][KT][NTH] gamma | beta b_r of the bulk tiles
   const int warp = h >> 5, lane = h & 31;
@@ -185,14 +181,14 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
     const bool act = h < nbulk;
     const int tx = act ? h % (ntx - 1) : 0, ty = act ? h / (ntx - 1) : 0;
     const int v = ty * ntx + tx;
-    const int rMy = act ? h : SCR + lane;
-    const int rL = (act && tx > 0) ? h - 1 : ZR + ((h - 1) & 31);
-    const int rR = act ? h + 1 : ZR + ((h + 1) & 31);
-    const int rD = (act && ty > 0) ? h - w : ZR + ((h - w) & 31);
-    const int rU = act ? h + w : ZR + ((h + w) & 31);
+    const int rMy = act ? v : SCR + lane;
+    const int rL = (act && tx > 0) ? v - 1 : ZR + ((v - 1) & 31);
+    const int rR = act ? v + 1 : ZR + ((v + 1) & 31);
+    const int rD = (act && ty > 0) ? v - ntx : ZR + ((v - ntx) & 31);
+    const int rU = act ? v + ntx : ZR + ((v + ntx) & 31);
     const real *pL = xb + rL * RS, *pR = xb + rR * RS, *pD = xb + rD * RS, *pU = xb + rU * RS;
     real *pMy = xb + rMy * RS;
-    real *pMyRX = xb + ((act && tx > 0) ? h : SCR + lane) * RS + CH;  // RX of a tx = 0 tile has no reader
+    real *pMyRX = pMy + CH;
     const bool hasL = tx > 0, hasD = ty > 0;
     const real d0x = A.ex1.k0[0] + (hasL ? A.ex1.kp[P] : real(0));
     const real d0y = A.ey1.k0[0] + (hasD ? A.ey1.kp[P] : real(0));
@@ -422,22 +418,16 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
     // record field offsets: along partial / along raw / across partial (read from the bulk tile) / across raw
     const int oPA = top ? 0 : 2 * CH, oRA = top ? CH : 3 * CH, oPC = top ? 2 * CH : 0, oRC = top ? 3 * CH : CH;
     const bool hasP = act && ta > 0, hasN = act && ta < nta - 1;
-    // own record (along-the-edge exchange): EB + e
-    real *pOwn = xb + (act ? EB + e : SCR + lane) * RS;
-    // where the raw values go that the bulk tile across reads: right piece -> RX of record (ty+1)*w,
-    // top piece -> RY of record nbulk + tx
-    real *pRaw = xb + (!act ? SCR + lane : (top ? nbulk + tx : (ty + 1) * w)) * RS + oRC;
-    // previous / next piece along the edge.  The last right piece's "next" is the corner, whose raw value
-    // sits in RY[0] of record nbulk + w.
-    const int rP = hasP ? EB + e - 1 : ZR + ((e - 1) & 31);
-    const real *pP = xb + rP * RS + oPA;
-    const real *pN = !hasN ? xb + (ZR + ((e + 1) & 31)) * RS
-                           : ((!top && ty == nty - 2) ? xb + (nbulk + w) * RS + 3 * CH : xb + (EB + e + 1) * RS + oRA);
-    // the partial sums from the tile across: bulk tile below / left; for the corner the last right piece's
-    // along partial (field PY[0] of its own record; the fields after it stay zero)
-    const real *pC = !act ? xb + (ZR + lane) * RS
-                          : (top ? (tx < w ? xb + ((nty - 2) * w + tx) * RS + 2 * CH : xb + (EB + nty - 2) * RS + 2 * CH)
-                                 : xb + (ty * w + w - 1) * RS);
+    // own record: virtual tile v (everything an edge piece publishes goes there)
+    real *pOwn = xb + (act ? v : SCR + lane) * RS;
+    real *pRaw = pOwn + oRC;
+    // previous / next piece along the edge (the corner is the "next" of the last right piece and of the last
+    // top piece; its raw value sits in element 0 of both its RX and RY chunks)
+    const real *pP = xb + (hasP ? v - sa : ZR + ((v - sa) & 31)) * RS + oPA;
+    const real *pN = xb + (hasN ? v + sa : ZR + ((v + sa) & 31)) * RS + oRA;
+    // the partial sums from the tile across: bulk tile below / left; for the corner the last right piece, whose
+    // along partial is element 0 of its PY chunk (the elements after it stay zero)
+    const real *pC = xb + (act ? v - sc : ZR + lane) * RS + oPC;
     Elem1D<real> ka;  // coefficients along
 #pragma unroll
     for (int c = 0; c <= P; ++c) {
