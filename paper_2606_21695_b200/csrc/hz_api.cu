@@ -468,7 +468,7 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
       const int nbulk = (q.ntx - 1) * (q.nty - 1), nedge = q.ntx + q.nty - 1;
       const size_t nrec = (size_t)ntv + 64;
       const size_t v16 = 16 / rs, chx = ((size_t)q.TX + v16 - 1) / v16 * v16;  // chunk length (square tiles)
-      sm = 2 * nrec * (4 * chx + v16) * rs + (t.csm ? 2 * (size_t)q.TX * q.TY * nthr * rs : 0);
+      sm = 2 * (nrec * (4 * chx + v16) + 2 * (size_t)roundup(nedge, 32)) * rs + (t.csm ? 2 * (size_t)q.TX * q.TY * nthr * rs : 0);
     } else {
       sm = tab_bytes + 2 * narr * (nthr + 1) * rs + (t.csm ? 2 * (size_t)q.TX * q.TY * nthr * rs : 0);
     }

@@ -165,7 +165,9 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
   const int w = ntx - 1, nbulk = (ntx - 1) * (nty - 1), nedge = ntx + nty - 1;
   const int bulk_warps = (nbulk + 31) >> 5;
   const int ZR = NTV, SCR = NTV + 32;  // zero records, scratch records
-  const int BUFW = (NTV + 64) * RS;
+  const int NE32 = (nedge + 31) & ~31;
+  const int EAO = (NTV + 64) * RS;     // per buffer, after the records: PA[NE32] | RA[NE32], the edge pieces'
+  const int BUFW = EAO + 2 * NE32;     // along-the-edge partial sums and raw values, indexed by edge lane
   real *xb = reinterpret_cast<real *>(smem_raw);
   real *csm = xb + 2 * BUFW;  // CSM: [2][KT][NTH] gamma | beta b_r of the bulk tiles
   const int warp = h >> 5, lane = h & 31;
@@ -181,7 +183,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
     const bool act = h < nbulk;
     const int tx = act ? h % (ntx - 1) : 0, ty = act ? h / (ntx - 1) : 0;
     const int v = ty * ntx + tx;
-    const int rMy = act ? v : SCR + lane;
+    const int rMy = act ? v : SCR;
     const int rL = (act && tx > 0) ? v - 1 : ZR + ((v - 1) & 31);
     const int rR = act ? v + 1 : ZR + ((v + 1) & 31);
     const int rD = (act && ty > 0) ? v - ntx : ZR + ((v - ntx) & 31);
@@ -418,16 +420,17 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
     // record field offsets: along partial / along raw / across partial (read from the bulk tile) / across raw
     const int oPA = top ? 0 : 2 * CH, oRA = top ? CH : 3 * CH, oPC = top ? 2 * CH : 0, oRC = top ? 3 * CH : CH;
     const bool hasP = act && ta > 0, hasN = act && ta < nta - 1;
-    // own record: virtual tile v (everything an edge piece publishes goes there)
-    real *pOwn = xb + (act ? v : SCR + lane) * RS;
-    real *pRaw = pOwn + oRC;
-    // previous / next piece along the edge (the corner is the "next" of the last right piece and of the last
-    // top piece; its raw value sits in element 0 of both its RX and RY chunks)
-    const real *pP = xb + (hasP ? v - sa : ZR + ((v - sa) & 31)) * RS + oPA;
-    const real *pN = xb + (hasN ? v + sa : ZR + ((v + sa) & 31)) * RS + oRA;
-    // the partial sums from the tile across: bulk tile below / left; for the corner the last right piece, whose
-    // along partial is element 0 of its PY chunk (the elements after it stay zero)
-    const real *pC = xb + (act ? v - sc : ZR + lane) * RS + oPC;
+    // raw values for the bulk tile across: own record (virtual tile v), chunk RX (right piece) / RY (top piece)
+    real *pRaw = xb + (act ? v : SCR) * RS + oRC;
+    // along-the-edge exchange through the compact arrays PA[e], RA[e] (conflict-free).  The last right piece's
+    // partial sum has one reader, the corner, which reads it as a chunk: it goes to element 0 of that piece's
+    // own PY chunk (whose other elements stay zero).
+    real *pPAout = !act ? xb + SCR * RS : ((!top && ty == nty - 2) ? xb + v * RS + 2 * CH : xb + EAO + e);
+    real *pRAout = !act ? xb + SCR * RS + 1 : xb + EAO + NE32 + e;
+    const real *pP = hasP ? xb + EAO + e - 1 : xb + ZR * RS;
+    const real *pN = hasN ? xb + EAO + NE32 + ((!top && ty == nty - 2) ? nedge - 1 : e + 1) : xb + ZR * RS;
+    // the partial sums from the tile across: bulk tile below / left; for the corner the last right piece
+    const real *pC = xb + (act ? v - sc : ZR) * RS + oPC;
     Elem1D<real> ka;  // coefficients along
 #pragma unroll
     for (int c = 0; c <= P; ++c) {
@@ -498,9 +501,9 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
 #pragma unroll
         for (int n = 0; n < T; ++n) { p[n] = fmaT(sigma, pd[n], p[n]); q[n] = p[n]; }
         q[T] = real(0);
-        real *my = pOwn + cur, *raw = pRaw + cur;
-        my[oPA] = line_partial<real, P, M>(q, ka);
-        my[oRA] = p[0];
+        real *raw = pRaw + cur;
+        pPAout[cur] = line_partial<real, P, M>(q, ka);
+        pRAout[cur] = p[0];
         st_chunk<T>(raw, p);
         bar_sync_all(NTH);
         const real qN = pN[cur], piP = pP[cur];
