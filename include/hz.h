@@ -111,15 +111,16 @@ typedef struct {
   double tol;       /* > 0: stop when the global relative residual <= tol (checked every check_every sweeps) */
   int check_every;  /* residual check period in sweeps; <= 0 = never (run exactly n_outer_max) */
   int reset_state;  /* 1: zero lambda and u_l before the first sweep; 0: continue from the current state */
-  int fused_exchange; /* 0: separate exchange kernel after every sweep; 1: the next sweep's prologue
-                         applies the exchange itself (same arithmetic, one launch per sweep) */
+  int use_graph;    /* 1: the {sweep, exchange} pairs between two residual checks are captured once into a CUDA
+                       graph and replayed (removes the per-launch overhead that dominates tiny configs); the
+                       per-kernel timings of hz_solve_info are then not measured (-1), total_ms still is */
 } hz_solve_opts;
 
 typedef struct {
   int n_outer_done;
   int n_t;
   double rel_residual;   /* last residual computed, or -1 if none was */
-  double sweep_ms_total; /* device time of all sweep launches (CUDA events on `stream`) */
+  double sweep_ms_total; /* device time of all sweep launches (CUDA events on `stream`); -1 with use_graph */
   double exch_ms_total;  /* device time of all exchange launches */
   double total_ms;       /* device time of the whole call on `stream` */
   double dof_timesteps;  /* sum_l N_l * n_wh * (n_t-1) * n_outer_done  (WaveHoltz DOF-timestep updates) */

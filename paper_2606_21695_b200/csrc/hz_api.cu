@@ -150,6 +150,11 @@ struct hz_ctx {
   double *d_part = nullptr, *d_red = nullptr, *d_ures = nullptr;
   int res_blocks = 0;
   Elem1D<double> ex1{}, ey1{};
+  // cached CUDA graph of `g_chunk` {sweep, exchange} pairs (use_graph)
+  cudaGraphExec_t g_exec = nullptr;
+  cudaStream_t cap_stream = nullptr;  // capture happens on this private stream (the legacy default stream cannot capture)
+  int g_chunk = 0, g_nwh = 0, g_warm = 0;
+  double g_relax = 0;
   std::vector<double> h_tab;  // host copy of the time-step table (kernel-parameter form of the ws kernel)
   TabC<float> tc32{};
   TabC<double> tc64{};
@@ -173,6 +178,7 @@ hz_status cuda_fail(hz_ctx *ctx, cudaError_t e, const char *what) {
   } while (0)
 
 void free_partition(hz_ctx *c) {
+  if (c->g_exec) { cudaGraphExecDestroy(c->g_exec); c->g_exec = nullptr; }
   void **ptrs[] = {&c->d_tab, &c->d_gamma, &c->d_alpha, &c->d_bbf_re, &c->d_bbf_im, &c->d_usub, &c->d_lam,
                    &c->d_g, &c->d_k2, &c->d_bs, &c->d_bandx, &c->d_bandy, (void **)&c->d_wxl, (void **)&c->d_wyl,
                    (void **)&c->d_part, (void **)&c->d_red, (void **)&c->d_ures};
@@ -594,7 +600,6 @@ hz_status hz_ddm_solve(hz_ctx *ctx, const hz_solve_opts *opts, void *u_out, hz_s
   if (!ctx->part) return fail(ctx, HZ_ESTATE, "hz_ddm_solve: call hz_partition first");
   if (opts->n_outer_max < 0 || opts->n_wh < 1 || !(opts->relax > 0.0) || opts->relax > 1.0)
     return fail(ctx, HZ_EINVAL, "hz_ddm_solve: need n_outer_max >= 0, n_wh >= 1, relax in (0,1]");
-  if (opts->fused_exchange) return fail(ctx, HZ_EUNSUPPORTED, "hz_ddm_solve: fused_exchange is not built yet");
   cudaStream_t st = (cudaStream_t)stream;
   const size_t rs = ctx->prec == HZ_F32 ? 4 : 8;
   if (opts->reset_state) {
@@ -603,31 +608,81 @@ hz_status hz_ddm_solve(hz_ctx *ctx, const hz_solve_opts *opts, void *u_out, hz_s
     HZ_CUDA(cudaMemsetAsync(ctx->d_usub, 0, (size_t)2 * ctx->L * ctx->lay.NS * rs, st));
   }
   const int n = opts->n_outer_max;
-  std::vector<cudaEvent_t> ev((size_t)2 * n + 2);
+  const bool checking = opts->tol > 0.0 && opts->check_every > 0;
+  const bool graph = opts->use_graph && n > 1;
+  std::vector<cudaEvent_t> ev(graph ? (size_t)1 : (size_t)2 * n + 2);
   for (auto &e : ev) HZ_CUDA(cudaEventCreate(&e));
   auto cleanup = [&]() { for (auto &e : ev) cudaEventDestroy(e); };
   double rel = -1.0;
   int done = 0, other = 0, nexch = 0;
-  cudaError_t ce = cudaEventRecord(ev[0], st);
+  cudaError_t ce = cudaSuccess;
   hz_status status = HZ_OK;
-  for (int it = 0; it < n && ce == cudaSuccess; ++it) {
-    ce = launch_sweep(ctx, opts, st);
-    if (ce != cudaSuccess) break;
-    ce = cudaEventRecord(ev[1 + 2 * it], st);
-    if (ce != cudaSuccess) break;
-    ce = launch_exchange(ctx, opts->relax, st);
-    if (ce != cudaSuccess) break;
-    ++nexch;
-    ce = cudaEventRecord(ev[2 + 2 * it], st);
-    if (ce != cudaSuccess) break;
-    ++done;
-    if (opts->tol > 0.0 && opts->check_every > 0 && (done % opts->check_every == 0 || done == n)) {
-      ce = launch_gather(ctx, ctx->d_ures, HZ_F64, st);
+  auto check = [&]() -> int {  // 1 = converged, 0 = go on, -1 = error (status / ce set)
+    ce = launch_gather(ctx, ctx->d_ures, HZ_F64, st);
+    if (ce != cudaSuccess) return -1;
+    status = residual_impl(ctx, ctx->d_ures, HZ_F64, &rel, st);
+    other += 3;
+    if (status != HZ_OK) return -1;
+    return rel <= opts->tol ? 1 : 0;
+  };
+  if (graph) {
+    int chunk = checking ? opts->check_every : 64;
+    if (chunk > n) chunk = n;
+    if (!ctx->g_exec || ctx->g_chunk != chunk || ctx->g_nwh != opts->n_wh || ctx->g_warm != opts->warm_start ||
+        ctx->g_relax != opts->relax) {
+      if (ctx->g_exec) { cudaGraphExecDestroy(ctx->g_exec); ctx->g_exec = nullptr; }
+      cudaGraph_t gr = nullptr;
+      if (!ctx->cap_stream) ce = cudaStreamCreateWithFlags(&ctx->cap_stream, cudaStreamNonBlocking);
+      if (ce != cudaSuccess) { cleanup(); return cuda_fail(ctx, ce, "hz_ddm_solve (capture stream)"); }
+      ce = cudaStreamBeginCapture(ctx->cap_stream, cudaStreamCaptureModeThreadLocal);
+      for (int it = 0; it < chunk && ce == cudaSuccess; ++it) {
+        ce = launch_sweep(ctx, opts, ctx->cap_stream);
+        if (ce == cudaSuccess) ce = launch_exchange(ctx, opts->relax, ctx->cap_stream);
+      }
+      cudaError_t ce2 = cudaStreamEndCapture(ctx->cap_stream, &gr);
+      if (ce == cudaSuccess) ce = ce2;
+      if (ce == cudaSuccess) ce = cudaGraphInstantiate(&ctx->g_exec, gr, 0);
+      if (gr) cudaGraphDestroy(gr);
+      if (ce != cudaSuccess) { cleanup(); return cuda_fail(ctx, ce, "hz_ddm_solve (graph capture)"); }
+      ctx->g_chunk = chunk; ctx->g_nwh = opts->n_wh; ctx->g_warm = opts->warm_start; ctx->g_relax = opts->relax;
+    }
+    ce = cudaEventRecord(ev[0], st);
+    while (done < n && ce == cudaSuccess) {
+      const int m = n - done < chunk ? n - done : chunk;
+      if (m == chunk) {
+        ce = cudaGraphLaunch(ctx->g_exec, st);
+      } else {
+        for (int it = 0; it < m && ce == cudaSuccess; ++it) {
+          ce = launch_sweep(ctx, opts, st);
+          if (ce == cudaSuccess) ce = launch_exchange(ctx, opts->relax, st);
+        }
+      }
       if (ce != cudaSuccess) break;
-      status = residual_impl(ctx, ctx->d_ures, HZ_F64, &rel, st);
-      other += 3;
-      if (status != HZ_OK) { cleanup(); return status; }
-      if (rel <= opts->tol) break;
+      done += m; nexch += m;
+      if (checking) {
+        const int c = check();
+        if (c < 0) { if (status != HZ_OK) { cleanup(); return status; } break; }
+        if (c > 0) break;
+      }
+    }
+  } else {
+    ce = cudaEventRecord(ev[0], st);
+    for (int it = 0; it < n && ce == cudaSuccess; ++it) {
+      ce = launch_sweep(ctx, opts, st);
+      if (ce != cudaSuccess) break;
+      ce = cudaEventRecord(ev[1 + 2 * it], st);
+      if (ce != cudaSuccess) break;
+      ce = launch_exchange(ctx, opts->relax, st);
+      if (ce != cudaSuccess) break;
+      ++nexch;
+      ce = cudaEventRecord(ev[2 + 2 * it], st);
+      if (ce != cudaSuccess) break;
+      ++done;
+      if (checking && (done % opts->check_every == 0 || done == n)) {
+        const int c = check();
+        if (c < 0) { if (status != HZ_OK) { cleanup(); return status; } break; }
+        if (c > 0) break;
+      }
     }
   }
   if (ce == cudaSuccess && u_out) { ce = launch_gather(ctx, u_out, ctx->prec, st); ++other; }
@@ -640,11 +695,16 @@ hz_status hz_ddm_solve(hz_ctx *ctx, const hz_solve_opts *opts, void *u_out, hz_s
     hz_solve_info inf{};
     inf.n_outer_done = done; inf.n_t = ctx->n_t; inf.rel_residual = rel;
     float ms = 0.f;
-    for (int it = 0; it < done; ++it) {
-      cudaEventElapsedTime(&ms, ev[2 * it], ev[2 * it + 1]);
-      inf.sweep_ms_total += ms;
-      cudaEventElapsedTime(&ms, ev[2 * it + 1], ev[2 * it + 2]);
-      inf.exch_ms_total += ms;
+    if (graph) {
+      inf.sweep_ms_total = -1.0;
+      inf.exch_ms_total = -1.0;
+    } else {
+      for (int it = 0; it < done; ++it) {
+        cudaEventElapsedTime(&ms, ev[2 * it], ev[2 * it + 1]);
+        inf.sweep_ms_total += ms;
+        cudaEventElapsedTime(&ms, ev[2 * it + 1], ev[2 * it + 2]);
+        inf.exch_ms_total += ms;
+      }
     }
     cudaEventElapsedTime(&ms, ev[0], ev_end);
     inf.total_ms = ms;
@@ -720,6 +780,7 @@ const char *hz_last_error(const hz_ctx *ctx) { return ctx ? ctx->err.c_str() : g
 void hz_destroy(hz_ctx *ctx) {
   if (!ctx) return;
   free_partition(ctx);
+  if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
   double **ptrs[] = {&ctx->d_c, &ctx->d_fre, &ctx->d_fim, &ctx->d_bc};
   for (double **q : ptrs) { if (*q) cudaFree(*q); *q = nullptr; }
   delete ctx;

@@ -35,7 +35,7 @@ class hz_part_info(C.Structure):
 
 class hz_solve_opts(C.Structure):
     _fields_ = [("n_outer_max", C.c_int), ("n_wh", C.c_int), ("warm_start", C.c_int), ("relax", C.c_double),
-                ("tol", C.c_double), ("check_every", C.c_int), ("reset_state", C.c_int), ("fused_exchange", C.c_int)]
+                ("tol", C.c_double), ("check_every", C.c_int), ("reset_state", C.c_int), ("use_graph", C.c_int)]
 
 
 class hz_solve_info(C.Structure):
@@ -131,9 +131,9 @@ def hz_partition(ctx, sx, sy, tc=HZ_TC_IMPEDANCE0, prec=HZ_F64, dofs_per_thread=
 
 
 def hz_ddm_solve(ctx, n_outer_max, n_wh=5, warm_start=True, relax=0.5, tol=0.0, check_every=0, reset_state=False,
-                 fused_exchange=False, u_out_ptr=None, stream=None):
+                 use_graph=False, u_out_ptr=None, stream=None):
     opts = hz_solve_opts(int(n_outer_max), int(n_wh), int(bool(warm_start)), float(relax), float(tol),
-                         int(check_every), int(bool(reset_state)), int(bool(fused_exchange)))
+                         int(check_every), int(bool(reset_state)), int(bool(use_graph)))
     info = hz_solve_info()
     _check(ctx, lib().hz_ddm_solve(ctx, C.byref(opts), C.c_void_p(u_out_ptr) if u_out_ptr else None, C.byref(info),
                                    C.c_void_p(stream) if stream else None))

@@ -290,3 +290,21 @@ def test_error_paths():
         assert e.value.status == hz.HZ_EINVAL
     finally:
         hz.hz_destroy(ctx)
+
+
+def test_graph_replay_is_bit_identical_to_plain_launches():
+    """use_graph = 1 replays the captured {sweep, exchange} pairs: same kernels, same arguments."""
+    _require_cuda()
+    inp = make_config(2, n=16)
+    ctx, info = hz.setup_from_inputs(inp, hz.HZ_F64, 0)
+    try:
+        a = torch.zeros(2 * inp.npx * inp.npy, dtype=torch.float64, device="cuda")
+        b = torch.zeros_like(a)
+        sa = hz.hz_ddm_solve(ctx, 23, n_wh=2, reset_state=True, u_out_ptr=a.data_ptr())
+        sb = hz.hz_ddm_solve(ctx, 23, n_wh=2, reset_state=True, use_graph=True, tol=1e-30, check_every=5,
+                             u_out_ptr=b.data_ptr())
+        assert sa.n_outer_done == sb.n_outer_done == 23
+        assert torch.equal(a, b)
+        assert sb.sweep_ms_total == -1.0 and sb.total_ms > 0
+    finally:
+        hz.hz_destroy(ctx)
