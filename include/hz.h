@@ -77,7 +77,7 @@ typedef struct {
   int edge_stride;       /* E = max of the two: stride of one side in lambda arrays */
   int threads_per_block; /* block size of the sweep kernel */
   int blocks;            /* = sx*sy subdomains = thread blocks of one sweep launch */
-  int dofs_per_thread;   /* 1, or (mx*p)*(my*p) of the register-blocked variant */
+  int dofs_per_thread;   /* 1, or (mx*p)*(my*p) of the register-blocked variant, or -1 (streamed) */
   int tile_mx, tile_my;  /* elements per thread tile (0 for the one-DOF-per-thread variant) */
   double dt, theta, sigma; /* dt = T/n_t; theta = tan(w dt/2)/w; sigma = 2 sin(w dt/2)/w */
   size_t smem_bytes;       /* dynamic shared memory per block */
@@ -95,7 +95,10 @@ typedef struct {
  *   dofs_per_thread  1 = one DOF per thread (needs dofs_per_sub <= 1024);
  *                    k > 1 = register-blocked variant with k = (mx*p)*(my*p) DOFs per thread
  *                    (PAPER.md:209-217), HZ_EUNSUPPORTED if no tile of that size is compiled or fits;
- *                    0 = choose automatically.
+ *                    0 = choose automatically (falls back to the streamed variant when the subdomain's
+ *                    state does not fit one SM's registers + shared memory);
+ *                    -1 = streamed variant: state in an L2-resident global scratch (PAPER.md:209-217's
+ *                    pGlobal idea), any subdomain size, slow.
  *   cfl_frac         fraction of the stable leapfrog step, in (0,1] (0.5 in all configs).
  *   info_out         may be NULL.
  * Re-partitioning an existing context is allowed; it discards lambda and the subdomain states.

@@ -145,7 +145,7 @@ struct hz_ctx {
   size_t ws_bytes = 0;
   void *d_tab = nullptr, *d_gamma = nullptr, *d_alpha = nullptr, *d_bbf_re = nullptr, *d_bbf_im = nullptr;
   void *d_usub = nullptr, *d_lam = nullptr, *d_g = nullptr, *d_k2 = nullptr, *d_bs = nullptr;
-  void *d_bandx = nullptr, *d_bandy = nullptr;
+  void *d_bandx = nullptr, *d_bandy = nullptr, *d_scr = nullptr;
   double *d_wxl = nullptr, *d_wyl = nullptr;
   double *d_part = nullptr, *d_red = nullptr, *d_ures = nullptr;
   int res_blocks = 0;
@@ -180,7 +180,7 @@ hz_status cuda_fail(hz_ctx *ctx, cudaError_t e, const char *what) {
 void free_partition(hz_ctx *c) {
   if (c->g_exec) { cudaGraphExecDestroy(c->g_exec); c->g_exec = nullptr; }
   void **ptrs[] = {&c->d_tab, &c->d_gamma, &c->d_alpha, &c->d_bbf_re, &c->d_bbf_im, &c->d_usub, &c->d_lam,
-                   &c->d_g, &c->d_k2, &c->d_bs, &c->d_bandx, &c->d_bandy, (void **)&c->d_wxl, (void **)&c->d_wyl,
+                   &c->d_g, &c->d_k2, &c->d_bs, &c->d_bandx, &c->d_bandy, &c->d_scr, (void **)&c->d_wxl, (void **)&c->d_wyl,
                    (void **)&c->d_part, (void **)&c->d_red, (void **)&c->d_ures};
   for (void **q : ptrs) { if (*q) cudaFree(*q); *q = nullptr; }
   c->part = false;
@@ -272,10 +272,12 @@ SweepArgs<real> make_args(const hz_ctx *c, const hz_solve_opts *o) {
 cudaError_t launch_sweep(const hz_ctx *c, const hz_solve_opts *o, cudaStream_t st) {
   if (c->prec == HZ_F32) {
     SweepArgs<float> a = make_args<float>(c, o);
+    if (c->lay.variant == 2) return launch_sweep_stream_f32(a, (float *)c->d_scr, c->p, c->launch, st);
     return c->lay.variant == 0 ? launch_sweep_dof_f32(a, c->p, c->launch, st)
                                : launch_sweep_tile_f32(a, &c->tc32, c->entry, c->launch, st);
   }
   SweepArgs<double> a = make_args<double>(c, o);
+  if (c->lay.variant == 2) return launch_sweep_stream_f64(a, (double *)c->d_scr, c->p, c->launch, st);
   return c->lay.variant == 0 ? launch_sweep_dof_f64(a, c->p, c->launch, st)
                              : launch_sweep_tile_f64(a, &c->tc64, c->entry, c->launch, st);
 }
@@ -424,7 +426,7 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
   if (tc != HZ_TC_IMPEDANCE0) return fail(ctx, HZ_EUNSUPPORTED, "hz_partition: only HZ_TC_IMPEDANCE0");
   if (prec != HZ_F32 && prec != HZ_F64) return fail(ctx, HZ_EINVAL, "hz_partition: bad precision");
   if (!(cfl_frac > 0.0) || cfl_frac > 1.0) return fail(ctx, HZ_EINVAL, "hz_partition: cfl_frac must be in (0,1]");
-  if (dofs_per_thread < 0) return fail(ctx, HZ_EINVAL, "hz_partition: dofs_per_thread < 0");
+  if (dofs_per_thread < -1) return fail(ctx, HZ_EINVAL, "hz_partition: dofs_per_thread < -1");
   free_partition(ctx);
   const int P = ctx->p;
   ctx->sx = sx; ctx->sy = sy; ctx->ex = ctx->nx / sx; ctx->ey = ctx->ny / sy; ctx->L = sx * sy; ctx->prec = prec;
@@ -485,8 +487,13 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
     return true;
   };
   const bool complex_f = ctx->d_fim != nullptr;
-  if (dofs_per_thread == 1 || (dofs_per_thread == 0 && complex_f)) {
-    if (N > 1024) return fail(ctx, HZ_EUNSUPPORTED, "hz_partition: one DOF per thread needs <= 1024 DOFs per subdomain");
+  bool streamed = dofs_per_thread == -1;
+  if (streamed) {
+  } else if (dofs_per_thread == 1 || (dofs_per_thread == 0 && complex_f)) {
+    if (N > 1024) {
+      if (dofs_per_thread == 1) return fail(ctx, HZ_EUNSUPPORTED, "hz_partition: one DOF per thread needs <= 1024 DOFs per subdomain");
+      streamed = true;
+    }
   } else {
     for (int i = 0; i < ntiles; ++i) {
       const TileEntry &t = tiles[i];
@@ -499,7 +506,10 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
       // register-capped one (higher occupancy, a few spills) only when the grid can fill that occupancy
       if (t.minb > 1 && ((long long)ctx->L < (long long)sm_count * t.minb || no_regcap)) continue;
       auto score_of = [&](const TileEntry &q) {
-        return (long long)(1 - q.ws) * 100000000 + (long long)q.csm * 1000000 + (long long)q.mx * P * q.my * P * 100 - q.minb;
+        const long long k_ = (long long)q.mx * P * q.my * P;
+        // register-resident coefficients first; there the warp-specialised kernel wins, with shared-memory
+        // coefficients (large subdomains, one block per SM) the smaller tile does
+        return (long long)q.csm * 100000000 + (q.csm ? k_ * 100 + (1 - q.ws) : (long long)(1 - q.ws) * 1000000 + k_ * 100) - q.minb;
       };
       const long long score = score_of(t);
       const long long bscore = best < 0 ? 0 : score_of(tiles[best]);
@@ -511,13 +521,17 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
       return fail(ctx, HZ_EUNSUPPORTED, "hz_partition: no compiled register-blocked kernel with that many DOFs per thread fits this subdomain");
     if (best >= 0 && complex_f)
       return fail(ctx, HZ_EUNSUPPORTED, "hz_partition: complex f is only supported by the one-DOF-per-thread variant");
-    if (best < 0 && N > 1024)
-      return fail(ctx, HZ_EUNSUPPORTED, "hz_partition: subdomain fits no compiled kernel variant");
+    if (best < 0 && N > 1024) streamed = true;  // state does not fit on chip: streamed fallback
   }
   if (best >= 0) {
     ctx->lay = blay; ctx->launch = bl;
     ctx->mx = tiles[best].mx; ctx->my = tiles[best].my; ctx->csm = tiles[best].csm; ctx->ws = tiles[best].ws;
     ctx->entry = best;
+  } else if (streamed) {
+    lay.variant = 2; lay.NT = N < 1024 ? roundup(N, 32) : 1024; lay.NS = roundup(N, 32); lay.TX = lay.TY = 1;
+    lay.ntx = lay.nty = 0;
+    ctx->lay = lay; ctx->mx = ctx->my = 0; ctx->csm = 0; ctx->ws = 0;
+    ctx->launch.blocks = ctx->L; ctx->launch.threads = lay.NT; ctx->launch.smem = 0;
   } else {
     lay.variant = 0; lay.NT = roundup(N, 32); lay.NS = lay.NT; lay.TX = lay.TY = 1; lay.ntx = lay.nty = 0;
     ctx->lay = lay; ctx->mx = ctx->my = 0; ctx->csm = 0; ctx->ws = 0;
@@ -560,6 +574,7 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
   HZ_CUDA(alloc0(&ctx->d_bbf_re, LS * rs));
   if (need_im) HZ_CUDA(alloc0(&ctx->d_bbf_im, LS * rs));
   HZ_CUDA(alloc0(&ctx->d_usub, 2 * LS * rs));
+  if (ctx->lay.variant == 2) HZ_CUDA(alloc0(&ctx->d_scr, 7 * LS * rs));
   HZ_CUDA(alloc0(&ctx->d_lam, lam_n * rs));
   HZ_CUDA(alloc0(&ctx->d_g, lam_n * rs));
   HZ_CUDA(alloc0(&ctx->d_k2, edge_n * rs));
@@ -585,7 +600,7 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
     hz_part_info inf{};
     inf.n_t = n_t; inf.dofs_per_sub = N; inf.edge_nodes_x = lnx; inf.edge_nodes_y = lny; inf.edge_stride = ctx->E;
     inf.threads_per_block = ctx->launch.threads; inf.blocks = ctx->L;
-    inf.dofs_per_thread = ctx->lay.variant == 0 ? 1 : ctx->lay.TX * ctx->lay.TY;
+    inf.dofs_per_thread = ctx->lay.variant == 0 ? 1 : (ctx->lay.variant == 2 ? -1 : ctx->lay.TX * ctx->lay.TY);
     inf.tile_mx = ctx->mx; inf.tile_my = ctx->my;
     inf.dt = ctx->dt; inf.theta = ctx->theta; inf.sigma = ctx->sigma;
     inf.smem_bytes = ctx->launch.smem; inf.workspace_bytes = ws;

@@ -11,6 +11,7 @@ constexpr int kSideW = 0, kSideE = 1, kSideS = 2, kSideN = 3;
 
 // Where node (i,j) of a subdomain lives inside the subdomain's slot range [0, NS).
 //   variant 0 (one DOF per thread):   slot = j*lnx + i                       (thread = slot)
+//   variant 2 (streamed fallback):    slot = j*lnx + i
 //   variant 1 (register-blocked):     thread tile (tx,ty) owns TX x TY nodes; node (a,b) of the tile of
 //                                     thread t = ty*ntx+tx lives at (b*TX+a)*NT + t, so that one node
 //                                     index across the block's threads is one coalesced line.
@@ -22,7 +23,7 @@ struct Layout {
   int NT;        // threads per block
   int NS;        // slots per subdomain (>= lnx*lny; padding slots hold zeros)
   __host__ __device__ inline int slot(int i, int j) const {
-    if (variant == 0) return j * lnx + i;
+    if (variant != 1) return j * lnx + i;
     const int tx = i / TX, a = i - tx * TX, ty = j / TY, b = j - ty * TY;
     return (b * TX + a) * NT + ty * ntx + tx;
   }
@@ -96,6 +97,8 @@ cudaError_t launch_sweep_tile_f32(const SweepArgs<float> &a, const TabC<float> *
                                   cudaStream_t st);
 cudaError_t launch_sweep_tile_f64(const SweepArgs<double> &a, const TabC<double> *tc, int entry, SweepLaunch cfg,
                                   cudaStream_t st);
+cudaError_t launch_sweep_stream_f32(const SweepArgs<float> &a, float *scr, int p, SweepLaunch cfg, cudaStream_t st);
+cudaError_t launch_sweep_stream_f64(const SweepArgs<double> &a, double *scr, int p, SweepLaunch cfg, cudaStream_t st);
 // compiled register-blocked instantiations of one precision
 int tile_table_f32(const TileEntry **out);
 int tile_table_f64(const TileEntry **out);

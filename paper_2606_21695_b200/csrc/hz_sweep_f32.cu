@@ -43,6 +43,9 @@ cudaError_t launch_sweep_tile_f32(const SweepArgs<float> &a, const TabC<float> *
                                   cudaStream_t st) {
   return launch_tile_impl<float>(kTilesF32, kNumTilesF32, a, tc, entry, cfg, st);
 }
+cudaError_t launch_sweep_stream_f32(const SweepArgs<float> &a, float *scr, int p, SweepLaunch cfg, cudaStream_t st) {
+  return launch_stream_impl<float>(a, scr, p, cfg, st);
+}
 int tile_table_f32(const TileEntry **out) {
   *out = kTilesF32;
   return kNumTilesF32;

@@ -42,6 +42,9 @@ cudaError_t launch_sweep_tile_f64(const SweepArgs<double> &a, const TabC<double>
                                   cudaStream_t st) {
   return launch_tile_impl<double>(kTilesF64, kNumTilesF64, a, tc, entry, cfg, st);
 }
+cudaError_t launch_sweep_stream_f64(const SweepArgs<double> &a, double *scr, int p, SweepLaunch cfg, cudaStream_t st) {
+  return launch_stream_impl<double>(a, scr, p, cfg, st);
+}
 int tile_table_f64(const TileEntry **out) {
   *out = kTilesF64;
   return kNumTilesF64;

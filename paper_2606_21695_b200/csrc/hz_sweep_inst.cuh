@@ -3,6 +3,7 @@
 // parallel).  HZ_TILE_TABLE(X) lists X(P, MX, MY, CSM, MAXT, MINB).
 #pragma once
 #include "hz_sweep.cuh"
+#include "hz_sweep_stream.cuh"
 #include "hz_sweep_ws.cuh"
 
 namespace hz {
@@ -20,6 +21,18 @@ static cudaError_t launch_dof_impl(const SweepArgs<real> &a, int p, SweepLaunch 
   cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem);
   if (e != cudaSuccess) return e;
   fn<<<cfg.blocks, cfg.threads, cfg.smem, st>>>(a);
+  return cudaGetLastError();
+}
+
+template <typename real>
+static cudaError_t launch_stream_impl(const SweepArgs<real> &a, real *scr, int p, SweepLaunch cfg, cudaStream_t st) {
+  switch (p) {
+    case 1: k_sweep_stream<real, 1><<<cfg.blocks, cfg.threads, 0, st>>>(a, scr); break;
+    case 2: k_sweep_stream<real, 2><<<cfg.blocks, cfg.threads, 0, st>>>(a, scr); break;
+    case 3: k_sweep_stream<real, 3><<<cfg.blocks, cfg.threads, 0, st>>>(a, scr); break;
+    case 4: k_sweep_stream<real, 4><<<cfg.blocks, cfg.threads, 0, st>>>(a, scr); break;
+    default: return cudaErrorInvalidValue;
+  }
   return cudaGetLastError();
 }
 

@@ -37,7 +37,7 @@ def oracle_two_sweeps_on(st, l, n_wh, relax):
 
 
 @pytest.mark.parametrize("cfg,prec,n_wh", [(2, hz.HZ_F64, 5), (2, hz.HZ_F32, 5), (3, hz.HZ_F32, 5), (3, hz.HZ_F64, 2),
-                                           (4, hz.HZ_F32, 1)])
+                                           (4, hz.HZ_F32, 1), (4, hz.HZ_F64, 1)])
 def test_full_size_sampled_subdomains(cfg, prec, n_wh):
     if not torch.cuda.is_available():
         pytest.fail("CUDA device required")

@@ -308,3 +308,20 @@ def test_graph_replay_is_bit_identical_to_plain_launches():
         assert sb.sweep_ms_total == -1.0 and sb.total_ms > 0
     finally:
         hz.hz_destroy(ctx)
+
+
+@pytest.mark.parametrize("prec", [hz.HZ_F64, hz.HZ_F32])
+def test_streamed_fallback_variant(prec):
+    """dofs_per_thread = -1: state in global scratch (the variant that covers subdomains too large for one SM)."""
+    inp = hetero_inputs(6, 4, 3, 3, 2, seed=91, complex_f=True)
+    rng = np.random.default_rng(8)
+    bc = [rng.standard_normal(n) + 1j * rng.standard_normal(n) for n in (inp.npy, inp.npy, inp.npx, inp.npx)]
+    g = check_case(inp, prec, -1, n_outer=3, n_wh=2, bc=bc)
+    check_case(make_config(2, n=32), prec, -1, n_outer=2, n_wh=2)
+    check_case(make_config(1), prec, -1, n_outer=3, n_wh=3, warm=False)
+
+
+def test_auto_falls_back_to_streamed_when_state_does_not_fit():
+    # 2x2 subdomains of 32x32 elements, p=3, fp64: 9409 DOF x 6 values x 8 B = 452 KB > one SM (config-4 block shape)
+    g = check_case(make_config(4, n=64, sub_elems=32), hz.HZ_F64, 0, n_outer=2, n_wh=1)
+    assert g["info"].dofs_per_thread == -1
