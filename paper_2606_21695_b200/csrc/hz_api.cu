@@ -507,9 +507,13 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
       if (t.minb > 1 && ((long long)ctx->L < (long long)sm_count * t.minb || no_regcap)) continue;
       auto score_of = [&](const TileEntry &q) {
         const long long k_ = (long long)q.mx * P * q.my * P;
-        // register-resident coefficients first; there the warp-specialised kernel wins, with shared-memory
-        // coefficients (large subdomains, one block per SM) the smaller tile does
-        return (long long)q.csm * 100000000 + (q.csm ? k_ * 100 + (1 - q.ws) : (long long)(1 - q.ws) * 1000000 + k_ * 100) - q.minb;
+        // register-resident coefficients first; there the warp-specialised kernel wins and tiles of 9..16 DOFs
+        // per thread are the sweet spot (smaller tiles exchange too much, larger ones leave too few warps);
+        // with shared-memory coefficients (large subdomains, one block per SM) the smaller tile wins
+        const long long nbulk_ = (long long)(ctx->ex / q.mx) * (ctx->ey / q.my);
+        // ... provided the subdomain still has two warps of full tiles; otherwise the smaller tile
+        const long long dk = nbulk_ < 64 ? 100 + k_ : (k_ < 9 ? 9 - k_ : (k_ > 16 ? k_ - 16 : 0));
+        return (long long)q.csm * 100000000 + (q.csm ? k_ * 100 + (1 - q.ws) : (long long)(1 - q.ws) * 1000000 + dk * 1000 + k_) * 10 - q.minb;
       };
       const long long score = score_of(t);
       const long long bscore = best < 0 ? 0 : score_of(tiles[best]);

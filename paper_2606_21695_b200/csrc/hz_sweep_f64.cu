@@ -19,6 +19,7 @@ namespace hz {
   W(1, 2, 0, 1024, 1)      \
   W(1, 4, 0, 256, 1)       \
   W(2, 1, 0, 512, 1)       \
+  W(2, 2, 0, 128, 1)       \
   W(2, 2, 1, 320, 1)       \
   W(3, 1, 0, 128, 3)       \
   W(3, 1, 0, 128, 1)       \
