@@ -19,6 +19,9 @@ What is pinned (tests/test_oracle_pins.py; none of the pins re-types a formula b
   ddm_*()                    converged DDM == dense direct solve <=1e-8,
                              L=1 DDM == WaveHoltz on the whole domain, hand-sized 2x1 case,
                              wrong sign of eq. (2) diverges (reading R3)
+  ddm_gmres()                (tests/test_oracle_gmres_pins.py) iterate == least-squares minimiser over an
+                             explicitly built Krylov basis (numpy lstsq, tiny case), converged == dense direct
+                             solve, monotone residuals, sweep map affine / real-linear
 Nothing here is "parity unpinned".
 
 Conventions
@@ -438,3 +441,99 @@ def ddm_solve(pr: Problem, sx: int, sy: int, n_outer: int, n_wh: int, warm_start
     for _ in range(n_outer):
         ddm_sweep(st, n_wh, warm_start, relax, sign_2ik)
     return st
+
+
+# --------------------------------------------------------------------------------------
+# F2  Krylov acceleration of the outer iteration (the fixed-point iteration on
+#     lambda "can be accelerated with a Krylov space method")
+# --------------------------------------------------------------------------------------
+# One warm-started sweep is an affine map x -> F(x) = T x + c of the joint state
+# x = (lambda on all interface sides, u_l of all subdomains); its fixed point is the DDM fixed
+# point (u_l = exact subdomain solutions, lambda consistent), i.e. the global discrete solution.
+# T is only REAL-linear (WaveHoltz takes real parts), so x is packed as a real
+# vector (real parts, then imaginary parts) with the Euclidean inner product.
+# Restarted GMRES(m) on (I - T) x = c: Arnoldi with modified Gram-Schmidt, least-squares problem
+# by Givens rotations (Saad & Schultz 1986, in its textbook form).  Each Arnoldi step costs one sweep.
+def ddm_pack(st: DDMState) -> np.ndarray:
+    parts = []
+    for l, sd in enumerate(st.subs):
+        for side in range(4):
+            if sd.neighbour[side] >= 0:
+                parts.append(st.lam[l][side])
+    parts += st.u
+    z = np.concatenate(parts)
+    return np.concatenate([z.real, z.imag])
+
+
+def ddm_unpack(st: DDMState, x: np.ndarray) -> None:
+    h = len(x) // 2
+    z = x[:h] + 1j * x[h:]
+    o = 0
+    for l, sd in enumerate(st.subs):
+        for side in range(4):
+            if sd.neighbour[side] >= 0:
+                n = len(st.lam[l][side])
+                st.lam[l][side] = z[o:o + n].copy()
+                o += n
+    for l in range(len(st.subs)):
+        n = len(st.u[l])
+        st.u[l] = z[o:o + n].copy()
+        o += n
+
+
+def ddm_gmres(pr: Problem, sx: int, sy: int, n_wh: int, relax: float, restart: int, n_steps: int,
+              cfl_frac: float = 0.5, tol: float = 0.0):
+    """Runs `n_steps` Arnoldi steps in total (restarting every `restart` steps) of GMRES on
+    (I - T) x = c from x = 0 and leaves the final iterate in the returned state.
+    Returns (state, history) with history[k] = relative LINEAR residual ||c - (I-T)x_k|| / ||c||
+    after k steps, as estimated by the Givens recurrence.  Stops early when that drops to `tol`."""
+    st = ddm_setup(pr, sx, sy, cfl_frac)
+
+    def F(x):
+        ddm_unpack(st, x)
+        ddm_sweep(st, n_wh, True, relax)
+        return ddm_pack(st)
+
+    x = np.zeros_like(ddm_pack(st))
+    c = F(x)
+    cnorm = float(np.linalg.norm(c))
+    hist = [1.0]
+    done = 0
+    while done < n_steps and cnorm > 0:
+        r = c - (x - (F(x) - c)) if done > 0 else c.copy()
+        beta = float(np.linalg.norm(r))
+        m = min(restart, n_steps - done)
+        V = [r / beta]
+        H = np.zeros((m + 1, m))
+        cs, sn = np.zeros(m), np.zeros(m)
+        g = np.zeros(m + 1)
+        g[0] = beta
+        k = 0
+        for j in range(m):
+            w = V[j] - (F(V[j]) - c)                       # (I - T) v_j
+            for i in range(j + 1):                          # modified Gram-Schmidt
+                H[i, j] = float(V[i] @ w)
+                w = w - H[i, j] * V[i]
+            H[j + 1, j] = float(np.linalg.norm(w))
+            V.append(w / H[j + 1, j])
+            for i in range(j):                              # previous rotations on the new column
+                t = cs[i] * H[i, j] + sn[i] * H[i + 1, j]
+                H[i + 1, j] = -sn[i] * H[i, j] + cs[i] * H[i + 1, j]
+                H[i, j] = t
+            d = math.hypot(H[j, j], H[j + 1, j])
+            cs[j], sn[j] = H[j, j] / d, H[j + 1, j] / d
+            H[j, j], H[j + 1, j] = d, 0.0
+            g[j + 1] = -sn[j] * g[j]
+            g[j] = cs[j] * g[j]
+            k = j + 1
+            done += 1
+            hist.append(abs(g[j + 1]) / cnorm)
+            if tol > 0 and hist[-1] <= tol:
+                break
+        y = np.linalg.solve(np.triu(H[:k, :k]), g[:k])
+        for i in range(k):
+            x = x + y[i] * V[i]
+        if tol > 0 and hist[-1] <= tol:
+            break
+    ddm_unpack(st, x)
+    return st, hist
