@@ -351,6 +351,21 @@ def run_extras(hz, torch, args, flush, stream):
             hz.hz_destroy(ctx)
         except Exception as e:
             out[key] = {"error": str(e)}
+    # the same with the Krylov-accelerated outer iteration (hz_ddm_solve_gmres, restarted GMRES(50) on (lambda, u))
+    for cfg, pr, tol in ((2, "f32", 1e-4), (2, "f64", 1e-4)):
+        key = f"config{cfg}_{pr}_time_to_solution_gmres"
+        try:
+            inp = make_config(cfg)
+            ctx, pinfo = hz.setup_from_inputs(inp, hz.HZ_F32 if pr == "f32" else hz.HZ_F64, 0)
+            hz.hz_ddm_solve_gmres(ctx, 5, n_wh=2, restart=50, stream=stream)                      # allocation, warm-up
+            t0 = time.perf_counter()
+            s = hz.hz_ddm_solve_gmres(ctx, 3000, n_wh=2, relax=0.5, restart=50, tol=tol, reset_state=True, stream=stream)
+            out[key] = {"tol": tol, "sweeps": s.sweeps_done, "cycles": s.cycles, "rel_residual": s.rel_residual,
+                        "device_ms": s.total_ms, "wall_ms": (time.perf_counter() - t0) * 1e3, "n_wh": 2, "relax": 0.5,
+                        "restart": 50}
+            hz.hz_destroy(ctx)
+        except Exception as e:
+            out[key] = {"error": str(e)}
     return out
 
 

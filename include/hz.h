@@ -145,6 +145,39 @@ typedef struct {
  * ------------------------------------------------------------------------------------------- */
 hz_status hz_ddm_solve(hz_ctx *ctx, const hz_solve_opts *opts, void *u_out, hz_solve_info *info, void *stream);
 
+/* ---------------------------------------------------------------------------------------------
+ * hz_ddm_solve_gmres — Krylov acceleration of the outer iteration (the fixed-point iteration on
+ * lambda "can be accelerated with a Krylov space method").  One warm-started sweep (sweep kernel + exchange
+ * kernel, exactly as in hz_ddm_solve) is an affine, real-linear map x -> T x + c of the joint state
+ * x = (lambda, u_l); restarted GMRES(restart) solves (I - T) x = c, one sweep per Arnoldi step (classical
+ * Gram-Schmidt applied twice, Givens rotations on the host).  The fixed point is the DDM fixed point.
+ * ------------------------------------------------------------------------------------------- */
+typedef struct {
+  int n_wh;        /* WaveHoltz iterations per sweep (>= 1) */
+  double relax;    /* rho in (0,1] of the exchange */
+  int restart;     /* Krylov vectors per cycle (>= 1) */
+  int max_steps;   /* Arnoldi steps (= sweeps, besides one per cycle start) to run at most */
+  double lin_tol;  /* > 0: stop when the relative linear residual ||c - (I-T)x|| / ||c|| <= lin_tol */
+  double tol;      /* > 0: stop when the global Helmholtz residual (hz_residual) <= tol.  It is evaluated at the end of
+                      a cycle; a cycle is ended early once the linear residual estimate reaches tol/2 (a target
+                      that is tightened whenever the true residual is still above tol) */
+  int reset_state; /* 1: start from x = 0; 0: start from the context's current (lambda, u_l) */
+  double *lin_history; /* HOST or NULL: receives the relative linear residual after each Arnoldi step */
+  int history_len;     /* capacity of lin_history */
+} hz_gmres_opts;
+
+typedef struct {
+  int steps_done;      /* Arnoldi steps */
+  int sweeps_done;     /* sweep launches (steps + one per cycle start + one for c) */
+  int cycles;
+  double lin_residual; /* last relative linear residual estimate */
+  double rel_residual; /* global Helmholtz residual of the final iterate (always computed) */
+  double total_ms;     /* device time of the call */
+  size_t krylov_bytes; /* device memory held by the Krylov basis */
+} hz_gmres_info;
+
+hz_status hz_ddm_solve_gmres(hz_ctx *ctx, const hz_gmres_opts *opts, void *u_out, hz_gmres_info *info, void *stream);
+
 /* Relative residual || b - (A - i w H - w^2 M) u ||_2 / || b ||_2 of a global nodal vector on the
  * UNPARTITIONED system (4) (the operator is the "Operator time" kernel of PAPER.md:223),
  * accumulated in fp64.  u_dev: DEVICE, layout as u_out, of precision u_prec.  Synchronises `stream`. */

@@ -151,6 +151,11 @@ struct hz_ctx {
   int res_blocks = 0;
   Elem1D<double> ex1{}, ey1{};
   // cached CUDA graph of `g_chunk` {sweep, exchange} pairs (use_graph)
+  // Krylov workspace of hz_ddm_solve_gmres: kry_vecs vectors of n_state reals; partial sums of the dots
+  void *d_kry = nullptr;
+  double *d_kpart = nullptr;
+  int kry_vecs = 0;
+  long long n_state = 0;
   cudaGraphExec_t g_exec = nullptr;
   cudaStream_t cap_stream = nullptr;  // capture happens on this private stream (the legacy default stream cannot capture)
   int g_chunk = 0, g_nwh = 0, g_warm = 0;
@@ -178,8 +183,11 @@ hz_status cuda_fail(hz_ctx *ctx, cudaError_t e, const char *what) {
   } while (0)
 
 void free_partition(hz_ctx *c) {
+  c->d_usub = nullptr;  // lives inside the d_lam allocation (joint state lambda | u_l)
+  if (c->d_kry) { cudaFree(c->d_kry); c->d_kry = nullptr; c->kry_vecs = 0; }
+  if (c->d_kpart) { cudaFree(c->d_kpart); c->d_kpart = nullptr; }
   if (c->g_exec) { cudaGraphExecDestroy(c->g_exec); c->g_exec = nullptr; }
-  void **ptrs[] = {&c->d_tab, &c->d_gamma, &c->d_alpha, &c->d_bbf_re, &c->d_bbf_im, &c->d_usub, &c->d_lam,
+  void **ptrs[] = {&c->d_tab, &c->d_gamma, &c->d_alpha, &c->d_bbf_re, &c->d_bbf_im, &c->d_lam,
                    &c->d_g, &c->d_k2, &c->d_bs, &c->d_bandx, &c->d_bandy, &c->d_scr, (void **)&c->d_wxl, (void **)&c->d_wyl,
                    (void **)&c->d_part, (void **)&c->d_red, (void **)&c->d_ures};
   for (void **q : ptrs) { if (*q) cudaFree(*q); *q = nullptr; }
@@ -577,9 +585,10 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
   HZ_CUDA(alloc0(&ctx->d_alpha, LS * rs));
   HZ_CUDA(alloc0(&ctx->d_bbf_re, LS * rs));
   if (need_im) HZ_CUDA(alloc0(&ctx->d_bbf_im, LS * rs));
-  HZ_CUDA(alloc0(&ctx->d_usub, 2 * LS * rs));
   if (ctx->lay.variant == 2) HZ_CUDA(alloc0(&ctx->d_scr, 7 * LS * rs));
-  HZ_CUDA(alloc0(&ctx->d_lam, lam_n * rs));
+  HZ_CUDA(alloc0(&ctx->d_lam, (lam_n + 2 * LS) * rs));  // joint state: lambda | u_l, one flat array
+  ctx->d_usub = (char *)ctx->d_lam + lam_n * rs;
+  ctx->n_state = (long long)(lam_n + 2 * LS);
   HZ_CUDA(alloc0(&ctx->d_g, lam_n * rs));
   HZ_CUDA(alloc0(&ctx->d_k2, edge_n * rs));
   HZ_CUDA(alloc0(&ctx->d_bs, edge_n * rs));
@@ -735,6 +744,189 @@ hz_status hz_ddm_solve(hz_ctx *ctx, const hz_solve_opts *opts, void *u_out, hz_s
   cleanup();
   return HZ_OK;
 }
+
+}  // extern "C"
+
+namespace {
+
+template <typename real>
+hz_status gmres_impl(hz_ctx *ctx, const hz_gmres_opts *o, void *u_out, hz_gmres_info *info, cudaStream_t st) {
+  const long long n = ctx->n_state;
+  const int m = o->restart;
+  const int nvec = m + 3;  // V_0..V_m, c, x
+  const size_t rs = sizeof(real);
+  const int bs = 256, nblk = 592;  // 4 blocks per SM on 148 SMs
+  if (!ctx->d_kry || ctx->kry_vecs < nvec) {
+    if (ctx->d_kry) cudaFree(ctx->d_kry);
+    if (ctx->d_kpart) cudaFree(ctx->d_kpart);
+    ctx->d_kry = nullptr; ctx->d_kpart = nullptr; ctx->kry_vecs = 0;
+    HZ_CUDA(cudaMalloc(&ctx->d_kry, (size_t)nvec * n * rs));
+    HZ_CUDA(cudaMalloc((void **)&ctx->d_kpart, ((size_t)(m + 2) * nblk + 2 * (m + 2)) * sizeof(double)));
+    ctx->kry_vecs = nvec;
+  }
+  real *V = (real *)ctx->d_kry, *cvec = V + (size_t)(m + 1) * n, *x = cvec + n, *state = (real *)ctx->d_lam;
+  double *part = ctx->d_kpart, *dres = part + (size_t)(m + 2) * nblk, *dcoef = dres + (m + 2);
+  hz_solve_opts so{};
+  so.n_wh = o->n_wh; so.warm_start = 1; so.relax = o->relax;
+  int sweeps = 0;
+  auto sweep = [&]() -> cudaError_t {
+    cudaError_t e = launch_sweep(ctx, &so, st);
+    if (e == cudaSuccess) e = launch_exchange(ctx, o->relax, st);
+    ++sweeps;
+    return e;
+  };
+  std::vector<double> hbuf(m + 2);
+  // h[0..nv) = V_i . w  (i < nv), synchronous
+  auto dots = [&](const real *Vb, int nv, const real *w, double *h) -> cudaError_t {
+    k_dots<real><<<dim3(nblk, nv), bs, 0, st>>>(n, Vb, n, w, part);
+    k_reduce_rows<<<nv, 256, 0, st>>>(part, nblk, dres);
+    cudaError_t e = cudaMemcpyAsync(h, dres, nv * sizeof(double), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    return e;
+  };
+  auto axpys = [&](real *w, const real *Vb, int nv, const double *coef) -> cudaError_t {
+    cudaError_t e = cudaMemcpyAsync(dcoef, coef, nv * sizeof(double), cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) return e;
+    k_axpys<real><<<nblk, bs, 0, st>>>(n, w, Vb, n, nv, dcoef);
+    return cudaGetLastError();
+  };
+  cudaEvent_t e0, e1;
+  HZ_CUDA(cudaEventCreate(&e0));
+  HZ_CUDA(cudaEventCreate(&e1));
+  HZ_CUDA(cudaEventRecord(e0, st));
+  // x0 and c = F(0)
+  if (o->reset_state) HZ_CUDA(cudaMemsetAsync(x, 0, n * rs, st));
+  else HZ_CUDA(cudaMemcpyAsync(x, state, n * rs, cudaMemcpyDeviceToDevice, st));
+  HZ_CUDA(cudaMemsetAsync(state, 0, n * rs, st));
+  HZ_CUDA(cudaMemsetAsync(ctx->d_g, 0, (size_t)ctx->L * 8 * ctx->E * rs, st));
+  HZ_CUDA(sweep());
+  HZ_CUDA(cudaMemcpyAsync(cvec, state, n * rs, cudaMemcpyDeviceToDevice, st));
+  double cc = 0.0;
+  HZ_CUDA(dots(cvec, 1, cvec, &cc));
+  const double cnorm = std::sqrt(cc);
+  int steps = 0, cycles = 0;
+  double lin = 1.0, rel = -1.0;
+  bool x_is_zero = o->reset_state != 0;
+  std::vector<double> H((size_t)(m + 1) * m), cs(m), sn(m), g(m + 1), y(m), h2(m + 2);
+  bool finished = cnorm == 0.0;
+  // linear-residual target that ends a cycle when a Helmholtz tolerance is given; tightened whenever the true
+  // residual (checked at the end of the cycle) turns out to be above the tolerance
+  double lin_target = 0.5 * o->tol;
+  while (!finished && steps < o->max_steps) {
+    // r = F(x) - x  (= c for x = 0)
+    if (x_is_zero) {
+      HZ_CUDA(cudaMemcpyAsync(V, cvec, n * rs, cudaMemcpyDeviceToDevice, st));
+    } else {
+      HZ_CUDA(cudaMemcpyAsync(state, x, n * rs, cudaMemcpyDeviceToDevice, st));
+      HZ_CUDA(sweep());
+      k_lincomb<real><<<nblk, bs, 0, st>>>(n, V, 1.0, state, -1.0, x, 0.0, nullptr);
+      HZ_CUDA(cudaGetLastError());
+    }
+    double bb = 0.0;
+    HZ_CUDA(dots(V, 1, V, &bb));
+    const double beta = std::sqrt(bb);
+    if (beta == 0.0) break;
+    k_lincomb<real><<<nblk, bs, 0, st>>>(n, V, 1.0 / beta, V, 0.0, V, 0.0, nullptr);
+    HZ_CUDA(cudaGetLastError());
+    std::fill(g.begin(), g.end(), 0.0);
+    g[0] = beta;
+    const int mc = m < o->max_steps - steps ? m : o->max_steps - steps;
+    int k = 0;
+    for (int j = 0; j < mc; ++j) {
+      real *vj = V + (size_t)j * n, *w = V + (size_t)(j + 1) * n;
+      // w = (I - T) v_j = v_j - (F(v_j) - c)
+      HZ_CUDA(cudaMemcpyAsync(state, vj, n * rs, cudaMemcpyDeviceToDevice, st));
+      HZ_CUDA(sweep());
+      k_lincomb<real><<<nblk, bs, 0, st>>>(n, w, 1.0, vj, -1.0, state, 1.0, cvec);
+      HZ_CUDA(cudaGetLastError());
+      // classical Gram-Schmidt, twice
+      double *hc = &H[(size_t)j * (m + 1)];  // column j, rows 0..j+1
+      HZ_CUDA(dots(V, j + 1, w, hbuf.data()));
+      for (int i = 0; i <= j; ++i) { hc[i] = hbuf[i]; h2[i] = -hbuf[i]; }
+      HZ_CUDA(axpys(w, V, j + 1, h2.data()));
+      HZ_CUDA(dots(V, j + 1, w, hbuf.data()));
+      for (int i = 0; i <= j; ++i) { hc[i] += hbuf[i]; h2[i] = -hbuf[i]; }
+      HZ_CUDA(axpys(w, V, j + 1, h2.data()));
+      double ww = 0.0;
+      HZ_CUDA(dots(w, 1, w, &ww));
+      hc[j + 1] = std::sqrt(ww);
+      if (hc[j + 1] > 0.0) {
+        k_lincomb<real><<<nblk, bs, 0, st>>>(n, w, 1.0 / hc[j + 1], w, 0.0, w, 0.0, nullptr);
+        HZ_CUDA(cudaGetLastError());
+      }
+      for (int i = 0; i < j; ++i) {  // previous Givens rotations on the new column
+        const double t = cs[i] * hc[i] + sn[i] * hc[i + 1];
+        hc[i + 1] = -sn[i] * hc[i] + cs[i] * hc[i + 1];
+        hc[i] = t;
+      }
+      const double d = std::hypot(hc[j], hc[j + 1]);
+      cs[j] = hc[j] / d; sn[j] = hc[j + 1] / d;
+      hc[j] = d; hc[j + 1] = 0.0;
+      g[j + 1] = -sn[j] * g[j];
+      g[j] = cs[j] * g[j];
+      k = j + 1;
+      ++steps;
+      lin = std::fabs(g[j + 1]) / cnorm;
+      if (o->lin_history && steps <= o->history_len) o->lin_history[steps - 1] = lin;
+      if ((o->lin_tol > 0.0 && lin <= o->lin_tol) || (o->tol > 0.0 && lin <= lin_target)) break;
+    }
+    // y = R^-1 g (back substitution), x += V y
+    for (int i = k - 1; i >= 0; --i) {
+      double sacc = g[i];
+      for (int q = i + 1; q < k; ++q) sacc -= H[(size_t)q * (m + 1) + i] * y[q];
+      y[i] = sacc / H[(size_t)i * (m + 1) + i];
+    }
+    HZ_CUDA(axpys(x, V, k, y.data()));
+    x_is_zero = false;
+    ++cycles;
+    if (o->lin_tol > 0.0 && lin <= o->lin_tol) finished = true;
+    if (o->tol > 0.0 && lin <= lin_target) {
+      HZ_CUDA(cudaMemcpyAsync(state, x, n * rs, cudaMemcpyDeviceToDevice, st));
+      HZ_CUDA(launch_gather(ctx, ctx->d_ures, HZ_F64, st));
+      hz_status s2 = residual_impl(ctx, ctx->d_ures, HZ_F64, &rel, st);
+      if (s2 != HZ_OK) return s2;
+      if (rel <= o->tol) finished = true;
+      else lin_target *= std::fmin(0.5, 0.5 * o->tol / rel);
+    }
+  }
+  // leave the iterate in the context's state, report its Helmholtz residual
+  HZ_CUDA(cudaMemcpyAsync(state, x, n * rs, cudaMemcpyDeviceToDevice, st));
+  HZ_CUDA(launch_gather(ctx, ctx->d_ures, HZ_F64, st));
+  {
+    hz_status s2 = residual_impl(ctx, ctx->d_ures, HZ_F64, &rel, st);
+    if (s2 != HZ_OK) return s2;
+  }
+  if (u_out) HZ_CUDA(launch_gather(ctx, u_out, ctx->prec, st));
+  HZ_CUDA(cudaEventRecord(e1, st));
+  HZ_CUDA(cudaStreamSynchronize(st));
+  float ms = 0.f;
+  cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  if (info) {
+    hz_gmres_info inf{};
+    inf.steps_done = steps; inf.sweeps_done = sweeps; inf.cycles = cycles; inf.lin_residual = lin;
+    inf.rel_residual = rel; inf.total_ms = ms; inf.krylov_bytes = (size_t)nvec * n * rs;
+    *info = inf;
+  }
+  return HZ_OK;
+}
+
+}  // namespace
+
+extern "C" hz_status hz_ddm_solve_gmres(hz_ctx *ctx, const hz_gmres_opts *opts, void *u_out, hz_gmres_info *info,
+                                        void *stream) {
+  if (!ctx) return HZ_EINVAL;
+  if (!opts) return fail(ctx, HZ_EINVAL, "hz_ddm_solve_gmres: NULL opts");
+  if (!ctx->part) return fail(ctx, HZ_ESTATE, "hz_ddm_solve_gmres: call hz_partition first");
+  if (opts->n_wh < 1 || !(opts->relax > 0.0) || opts->relax > 1.0 || opts->restart < 1 || opts->restart > 1000 ||
+      opts->max_steps < 0 || (opts->lin_history && opts->history_len < 0))
+    return fail(ctx, HZ_EINVAL, "hz_ddm_solve_gmres: need n_wh >= 1, relax in (0,1], 1 <= restart <= 1000, max_steps >= 0");
+  cudaStream_t st = (cudaStream_t)stream;
+  return ctx->prec == HZ_F32 ? gmres_impl<float>(ctx, opts, u_out, info, st) : gmres_impl<double>(ctx, opts, u_out, info, st);
+}
+
+extern "C" {
 
 hz_status hz_residual(hz_ctx *ctx, const void *u_dev, hz_prec u_prec, double *rel_residual, void *stream) {
   if (!ctx) return HZ_EINVAL;

@@ -310,3 +310,70 @@ __global__ void __launch_bounds__(1024) k_probe_lds(int iters, float *out) {
 }
 
 }  // namespace hz
+
+namespace hz {
+
+// ---------------------------------------------------------------------------------------------
+// Vector kernels of the Krylov-accelerated outer iteration.  The joint
+// state x = (lambda | u_l) is one flat array of `real`; Krylov vectors V_i are rows of a [nv][n] array.
+// Inner products are accumulated in fp64 and reduced in a fixed order (deterministic).
+// ---------------------------------------------------------------------------------------------
+template <typename real>
+__global__ void k_dots(long long n, const real *__restrict__ V, long long ld, const real *__restrict__ w,
+                       double *__restrict__ part) {
+  // grid (nblk, nv): block (bx, i) -> partial sum of V_i . w over its grid-stride slice
+  __shared__ double red[32];
+  const real *v = V + (size_t)blockIdx.y * ld;
+  double s = 0.0;
+  for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (long long)gridDim.x * blockDim.x)
+    s += (double)v[e] * (double)w[e];
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+  const int wp = threadIdx.x >> 5, ln = threadIdx.x & 31;
+  if (ln == 0) red[wp] = s;
+  __syncthreads();
+  if (wp == 0) {
+    s = ln < (blockDim.x >> 5) ? red[ln] : 0.0;
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+    if (ln == 0) part[(size_t)blockIdx.y * gridDim.x + blockIdx.x] = s;
+  }
+}
+
+__global__ void k_reduce_rows(const double *__restrict__ part, int nblk, double *__restrict__ out) {
+  // one block per row: out[row] = sum of part[row][0..nblk)
+  __shared__ double red[32];
+  double s = 0.0;
+  for (int q = threadIdx.x; q < nblk; q += blockDim.x) s += part[(size_t)blockIdx.x * nblk + q];
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+  const int wp = threadIdx.x >> 5, ln = threadIdx.x & 31;
+  if (ln == 0) red[wp] = s;
+  __syncthreads();
+  if (wp == 0) {
+    s = ln < (blockDim.x >> 5) ? red[ln] : 0.0;
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_down_sync(0xffffffffu, s, o);
+    if (ln == 0) out[blockIdx.x] = s;
+  }
+}
+
+// w[e] += sum_i coef[i] V_i[e]   (coef on the device, already signed)
+template <typename real>
+__global__ void k_axpys(long long n, real *__restrict__ w, const real *__restrict__ V, long long ld, int nv,
+                        const double *__restrict__ coef) {
+  for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (long long)gridDim.x * blockDim.x) {
+    double s = (double)w[e];
+    for (int i = 0; i < nv; ++i) s += coef[i] * (double)V[(size_t)i * ld + e];
+    w[e] = (real)s;
+  }
+}
+
+// out = a*x + b*y + c*z  (z may be NULL)
+template <typename real>
+__global__ void k_lincomb(long long n, real *__restrict__ out, double a, const real *__restrict__ x, double b,
+                          const real *__restrict__ y, double c, const real *__restrict__ z) {
+  for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (long long)gridDim.x * blockDim.x) {
+    double s = a * (double)x[e] + b * (double)y[e];
+    if (z) s += c * (double)z[e];
+    out[e] = (real)s;
+  }
+}
+
+}  // namespace hz

@@ -21,7 +21,7 @@ HZ_TC_IMPEDANCE0 = 0
 STATUS_NAMES = {0: "HZ_OK", 1: "HZ_EINVAL", 2: "HZ_ENOMEM", 3: "HZ_ECUDA", 4: "HZ_EUNSUPPORTED", 5: "HZ_ESTATE"}
 
 # every symbol include/hz.h declares
-EXPORTS = ("hz_mesh_setup", "hz_set_source", "hz_partition", "hz_ddm_solve", "hz_residual",
+EXPORTS = ("hz_mesh_setup", "hz_set_source", "hz_partition", "hz_ddm_solve", "hz_ddm_solve_gmres", "hz_residual",
            "hz_get_subdomain_state", "hz_set_subdomain_state", "hz_last_error", "hz_destroy", "hz_peak_probe")
 
 
@@ -43,6 +43,17 @@ class hz_solve_info(C.Structure):
                 ("sweep_ms_total", C.c_double), ("exch_ms_total", C.c_double), ("total_ms", C.c_double),
                 ("dof_timesteps", C.c_double), ("sweep_launches", C.c_int), ("exch_launches", C.c_int),
                 ("other_launches", C.c_int)]
+
+
+class hz_gmres_opts(C.Structure):
+    _fields_ = [("n_wh", C.c_int), ("relax", C.c_double), ("restart", C.c_int), ("max_steps", C.c_int),
+                ("lin_tol", C.c_double), ("tol", C.c_double), ("reset_state", C.c_int),
+                ("lin_history", C.POINTER(C.c_double)), ("history_len", C.c_int)]
+
+
+class hz_gmres_info(C.Structure):
+    _fields_ = [("steps_done", C.c_int), ("sweeps_done", C.c_int), ("cycles", C.c_int), ("lin_residual", C.c_double),
+                ("rel_residual", C.c_double), ("total_ms", C.c_double), ("krylov_bytes", C.c_size_t)]
 
 
 class HzError(RuntimeError):
@@ -69,6 +80,7 @@ def lib():
     L.hz_set_source.argtypes = [vp, vp, vp]
     L.hz_partition.argtypes = [vp, ip, ip, ip, ip, ip, C.c_double, C.POINTER(hz_part_info)]
     L.hz_ddm_solve.argtypes = [vp, C.POINTER(hz_solve_opts), vp, C.POINTER(hz_solve_info), vp]
+    L.hz_ddm_solve_gmres.argtypes = [vp, C.POINTER(hz_gmres_opts), vp, C.POINTER(hz_gmres_info), vp]
     L.hz_residual.argtypes = [vp, vp, ip, dp, vp]
     L.hz_get_subdomain_state.argtypes = [vp, vp, vp, vp]
     L.hz_set_subdomain_state.argtypes = [vp, vp, vp, vp]
@@ -137,6 +149,20 @@ def hz_ddm_solve(ctx, n_outer_max, n_wh=5, warm_start=True, relax=0.5, tol=0.0, 
     info = hz_solve_info()
     _check(ctx, lib().hz_ddm_solve(ctx, C.byref(opts), C.c_void_p(u_out_ptr) if u_out_ptr else None, C.byref(info),
                                    C.c_void_p(stream) if stream else None))
+    return info
+
+
+def hz_ddm_solve_gmres(ctx, max_steps, n_wh=2, relax=0.5, restart=50, lin_tol=0.0, tol=0.0, reset_state=True,
+                       u_out_ptr=None, stream=None, want_history=False):
+    """-> hz_gmres_info (and the per-step relative linear residuals if want_history)."""
+    hist = (C.c_double * max(1, int(max_steps)))() if want_history else None
+    opts = hz_gmres_opts(int(n_wh), float(relax), int(restart), int(max_steps), float(lin_tol), float(tol),
+                         int(bool(reset_state)), hist if want_history else None, int(max_steps) if want_history else 0)
+    info = hz_gmres_info()
+    _check(ctx, lib().hz_ddm_solve_gmres(ctx, C.byref(opts), C.c_void_p(u_out_ptr) if u_out_ptr else None,
+                                         C.byref(info), C.c_void_p(stream) if stream else None))
+    if want_history:
+        return info, [hist[i] for i in range(info.steps_done)]
     return info
 
 
