@@ -486,7 +486,14 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
       const size_t v16 = 16 / rs, chx = ((size_t)q.TX + v16 - 1) / v16 * v16;  // chunk length (square tiles)
       sm = 2 * (nrec * (4 * chx + v16) + 2 * (size_t)roundup(nedge, 32)) * rs + (t.csm ? 2 * (size_t)q.TX * q.TY * nthr * rs : 0);
     } else {
-      sm = tab_bytes + 2 * narr * (nthr + 1) * rs + (t.csm ? 2 * (size_t)q.TX * q.TY * nthr * rs : 0);
+      if (n_t > kTabCMax) return false;
+      const size_t v16 = 16 / rs;
+      const size_t chx = ((size_t)q.TX + v16 - 1) / v16 * v16, chy = ((size_t)q.TY + v16 - 1) / v16 * v16;
+      size_t rsw = 2 * chx + 2 * chy;                       // record stride, odd number of 16-byte units
+      if ((rsw / v16) % 2 == 0) rsw += v16;
+      size_t cst = (2 * (size_t)q.TX * q.TY + v16 - 1) / v16 * v16;  // CSM strip per thread
+      if ((cst / v16) % 2 == 0) cst += v16;
+      sm = 2 * (size_t)(nthr + 33) * rsw * rs + (t.csm ? (size_t)nthr * cst * rs : 0);
     }
     if (nthr > t.maxt) return false;
     q.NT = ntv; q.NS = q.TX * q.TY * ntv;

@@ -4,6 +4,7 @@
 #pragma once
 #include "hz_sweep.cuh"
 #include "hz_sweep_stream.cuh"
+#include "hz_sweep_tile.cuh"
 #include "hz_sweep_ws.cuh"
 
 namespace hz {
@@ -43,14 +44,9 @@ static cudaError_t launch_tile_impl(const TileEntry *tab, int n, const SweepArgs
   const TileEntry &e = tab[entry];
   cudaError_t err = cudaFuncSetAttribute(e.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem);
   if (err != cudaSuccess) return err;
-  if (e.ws) {
-    if (!tc) return cudaErrorInvalidValue;
-    auto fn = reinterpret_cast<void (*)(const SweepArgs<real>, const TabC<real>)>(const_cast<void *>(e.fn));
-    fn<<<cfg.blocks, cfg.threads, cfg.smem, st>>>(a, *tc);
-  } else {
-    auto fn = reinterpret_cast<void (*)(const SweepArgs<real>)>(const_cast<void *>(e.fn));
-    fn<<<cfg.blocks, cfg.threads, cfg.smem, st>>>(a);
-  }
+  if (!tc) return cudaErrorInvalidValue;
+  auto fn = reinterpret_cast<void (*)(const SweepArgs<real>, const TabC<real>)>(const_cast<void *>(e.fn));
+  fn<<<cfg.blocks, cfg.threads, cfg.smem, st>>>(a, *tc);
   return cudaGetLastError();
 }
 
