@@ -22,6 +22,9 @@ What is pinned (tests/test_oracle_pins.py; none of the pins re-types a formula b
   ddm_gmres()                (tests/test_oracle_gmres_pins.py) iterate == least-squares minimiser over an
                              explicitly built Krylov basis (numpy lstsq, tiny case), converged == dense direct
                              solve, monotone residuals, sweep map affine / real-linear
+  minres()/block_system()    (tests/test_oracle_minres_pins.py) symmetry/indefiniteness of (5), iterate == residual
+                             minimiser over an explicit Krylov basis, recurrence residual == true residual,
+                             converged == dense direct solve, agreement with scipy.sparse.linalg.minres
 Nothing here is "parity unpinned".
 
 Conventions
@@ -537,3 +540,98 @@ def ddm_gmres(pr: Problem, sx: int, sy: int, n_wh: int, relax: float, restart: i
             break
     ddm_unpack(st, x)
     return st, hist
+
+
+# --------------------------------------------------------------------------------------
+# F1  MINRES as the subdomain solver: the paper's comparator (eq. (5), 123, 271-277)
+# --------------------------------------------------------------------------------------
+def block_system(A, M, H, b, omega):
+    """The real symmetric indefinite 2N x 2N form (5) of (4):
+        [[A - w^2 M, w H], [w H, w^2 M - A]] [Re u; Im u] = [Re b; -Im b]."""
+    D = sp.diags(omega ** 2 * M)
+    Hm = sp.diags(omega * H)
+    K = sp.bmat([[A - D, Hm], [Hm, D - A]]).tocsr()
+    rhs = np.concatenate([np.real(b), -np.imag(b)])
+    return K, rhs
+
+
+def minres(K, rhs, x0=None, tol=1e-12, max_iters=10000, history=None):
+    """MINRES of Paige & Saunders (1975) in its textbook Lanczos / Givens form, no preconditioner, for the
+    symmetric indefinite system K x = rhs ("five vectors and two inner products per iteration",
+    PAPER.md:123, 275).  Stops when the recurrence's residual norm |eta| <= tol * ||rhs|| (the relative
+    residual the paper iterates to: 1e-6 in single, 1e-12 in double precision).
+    Returns (x, iterations)."""
+    n = len(rhs)
+    x = np.zeros(n) if x0 is None else np.array(x0, dtype=float)
+    bnorm = float(np.linalg.norm(rhs))
+    v = rhs - K @ x
+    gamma = float(np.linalg.norm(v))            # gamma_1
+    if history is not None:
+        history.append(gamma / bnorm if bnorm > 0 else 0.0)
+    if bnorm == 0.0 or gamma <= tol * bnorm:
+        return x, 0
+    eta = gamma
+    v_old = np.zeros(n)
+    w_old, w = np.zeros(n), np.zeros(n)         # w_{j-1}, w_j
+    s_old, s, c_old, c = 0.0, 0.0, 1.0, 1.0
+    it = 0
+    for it in range(1, max_iters + 1):
+        v = v / gamma
+        Kv = K @ v
+        delta = float(v @ Kv)
+        v_new = Kv - delta * v - gamma * v_old
+        gamma_new = float(np.linalg.norm(v_new))
+        a0 = c * delta - c_old * s * gamma
+        a1 = math.hypot(a0, gamma_new)
+        a2 = s * delta + c_old * c * gamma
+        a3 = s_old * gamma
+        c_new, s_new = a0 / a1, gamma_new / a1
+        w_new = (v - a3 * w_old - a2 * w) / a1
+        x = x + c_new * eta * w_new
+        eta = -s_new * eta
+        if history is not None:
+            history.append(abs(eta) / bnorm)
+        v_old, v, gamma = v, v_new, gamma_new
+        w_old, w = w, w_new
+        s_old, s, c_old, c = s, s_new, c, c_new
+        if abs(eta) <= tol * bnorm or gamma == 0.0:
+            break
+    return x, it
+
+
+def ddm_cycle_minres(st: DDMState, l: int, tol: float, max_iters: int, warm_start: bool):
+    """The DDM cycle of Algorithm 1 with MINRES on (5) in place of the WaveHoltz loop.
+    Returns (u_l, g, iterations)."""
+    sd = st.subs[l]
+    b = sd.bf.copy()
+    for side in range(4):
+        if sd.neighbour[side] >= 0:
+            b[sd.edge_idx[side]] += sd.s[side] * st.lam[l][side]
+    K, rhs = block_system(sd.A, sd.M, sd.H, b, st.pr.omega)
+    x0 = np.concatenate([st.u[l].real, st.u[l].imag]) if warm_start else None
+    x, its = minres(K, rhs, x0, tol, max_iters)
+    n = len(b)
+    u = x[:n] + 1j * x[n:]
+    g = [None] * 4
+    for side in range(4):
+        if sd.neighbour[side] >= 0:
+            g[side] = -st.lam[l][side] - 2j * sd.k_edge[side] * u[sd.edge_idx[side]]
+    return u, g, its
+
+
+def ddm_sweep_minres(st: DDMState, tol: float, max_iters: int, warm_start: bool, relax: float):
+    """One outer iteration with MINRES subdomain solves; returns the iteration counts."""
+    L = len(st.subs)
+    new_u, gs, its = [None] * L, [None] * L, [0] * L
+    for l in range(L):
+        new_u[l], gs[l], its[l] = ddm_cycle_minres(st, l, tol, max_iters, warm_start)
+    new_lam = [[a.copy() for a in st.lam[l]] for l in range(L)]
+    for l in range(L):
+        for side in range(4):
+            r = st.subs[l].neighbour[side]
+            if r >= 0:
+                o = OPPOSITE[side]
+                new_lam[r][o] = (1.0 - relax) * st.lam[r][o] + relax * gs[l][side]
+    st.lam, st.u = new_lam, new_u
+    st.n_sweeps += 1
+    return its
