@@ -178,6 +178,34 @@ typedef struct {
 
 hz_status hz_ddm_solve_gmres(hz_ctx *ctx, const hz_gmres_opts *opts, void *u_out, hz_gmres_info *info, void *stream);
 
+/* ---------------------------------------------------------------------------------------------
+ * hz_minres_cycle — the paper's comparator: one DDM cycle on every subdomain (one thread
+ * block per subdomain, one launch) with unpreconditioned MINRES on the real symmetric block system (5)
+ * as the subdomain solver instead of WaveHoltz.  Assembles b from f and the current lambda^n,
+ * iterates until the recurrence's relative residual <= tol (the paper: 1e-6 in single, 1e-12 in double precision) or
+ * max_iters, stores u_l and the outgoing interface data, then (relax > 0) runs the exchange kernel.
+ * Needs the one-DOF-per-thread partition (hz_partition(..., dofs_per_thread = 1)), else HZ_EUNSUPPORTED.
+ * max_iters = 0 with warm_start = 1 only evaluates the subdomain residuals of the current u_l.
+ *   iters_out  HOST or NULL: `blocks` ints, MINRES iterations of each subdomain.
+ *   res_out    HOST or NULL: `blocks` doubles, true relative residual ||rhs - K x|| / ||rhs|| of each subdomain.
+ * ------------------------------------------------------------------------------------------- */
+typedef struct {
+  double tol;
+  int max_iters;
+  int warm_start;  /* 0: x0 = 0; 1: x0 = current u_l */
+  double relax;    /* > 0: run the exchange with this rho afterwards; 0: leave lambda untouched */
+} hz_minres_opts;
+
+typedef struct {
+  int iters_max;
+  double iters_mean;
+  double res_max;    /* largest true relative subdomain residual */
+  double kernel_ms;  /* device time of the MINRES kernel */
+} hz_minres_info;
+
+hz_status hz_minres_cycle(hz_ctx *ctx, const hz_minres_opts *opts, int *iters_out, double *res_out,
+                          hz_minres_info *info, void *stream);
+
 /* Relative residual || b - (A - i w H - w^2 M) u ||_2 / || b ||_2 of a global nodal vector on the
  * UNPARTITIONED system (4) (the operator is the "Operator time" kernel of PAPER.md:223),
  * accumulated in fp64.  u_dev: DEVICE, layout as u_out, of precision u_prec.  Synchronises `stream`. */

@@ -12,6 +12,7 @@
 #include "../../include/hz.h"
 #include "hz_aux.cuh"
 #include "hz_internal.h"
+#include "hz_minres.cuh"
 
 using namespace hz;
 
@@ -151,6 +152,10 @@ struct hz_ctx {
   int res_blocks = 0;
   Elem1D<double> ex1{}, ey1{};
   // cached CUDA graph of `g_chunk` {sweep, exchange} pairs (use_graph)
+  // operator data of the MINRES comparator (built on first use): m | w2M | wH | bf_re | bf_im [L][NS], sedge [L][4][E]
+  void *d_mr = nullptr;
+  int *d_mr_iters = nullptr;
+  double *d_mr_res = nullptr;
   // Krylov workspace of hz_ddm_solve_gmres: kry_vecs vectors of n_state reals; partial sums of the dots
   void *d_kry = nullptr;
   double *d_kpart = nullptr;
@@ -184,6 +189,9 @@ hz_status cuda_fail(hz_ctx *ctx, cudaError_t e, const char *what) {
 
 void free_partition(hz_ctx *c) {
   c->d_usub = nullptr;  // lives inside the d_lam allocation (joint state lambda | u_l)
+  if (c->d_mr) { cudaFree(c->d_mr); c->d_mr = nullptr; }
+  if (c->d_mr_iters) { cudaFree(c->d_mr_iters); c->d_mr_iters = nullptr; }
+  if (c->d_mr_res) { cudaFree(c->d_mr_res); c->d_mr_res = nullptr; }
   if (c->d_kry) { cudaFree(c->d_kry); c->d_kry = nullptr; c->kry_vecs = 0; }
   if (c->d_kpart) { cudaFree(c->d_kpart); c->d_kpart = nullptr; }
   if (c->g_exec) { cudaGraphExecDestroy(c->g_exec); c->g_exec = nullptr; }
@@ -920,6 +928,92 @@ hz_status gmres_impl(hz_ctx *ctx, const hz_gmres_opts *o, void *u_out, hz_gmres_
 }
 
 }  // namespace
+
+namespace {
+
+inline cudaError_t launch_minres(const MinresArgs<float> &a, int p, SweepLaunch c, cudaStream_t st) { return launch_minres_f32(a, p, c, st); }
+inline cudaError_t launch_minres(const MinresArgs<double> &a, int p, SweepLaunch c, cudaStream_t st) { return launch_minres_f64(a, p, c, st); }
+
+template <typename real>
+hz_status minres_impl(hz_ctx *ctx, const hz_minres_opts *o, int *iters_out, double *res_out, hz_minres_info *info,
+                      cudaStream_t st) {
+  const size_t LS = (size_t)ctx->L * ctx->lay.NS, EN = (size_t)ctx->L * 4 * ctx->E;
+  if (!ctx->d_mr) {
+    HZ_CUDA(cudaMalloc(&ctx->d_mr, (5 * LS + EN) * sizeof(real)));
+    HZ_CUDA(cudaMemset(ctx->d_mr, 0, (5 * LS + EN) * sizeof(real)));
+    HZ_CUDA(cudaMalloc((void **)&ctx->d_mr_iters, ctx->L * sizeof(int)));
+    HZ_CUDA(cudaMalloc((void **)&ctx->d_mr_res, ctx->L * sizeof(double)));
+  }
+  real *base = (real *)ctx->d_mr;
+  real *mloc = base, *w2M = base + LS, *wH = base + 2 * LS, *bfr = base + 3 * LS, *bfi = base + 4 * LS, *sedge = base + 5 * LS;
+  {  // (re)build: the source may have changed through hz_set_source
+    const long long total = (long long)ctx->L * ctx->lay.lnx * ctx->lay.lny;
+    k_build_minres<real><<<(unsigned)((total + 255) / 256), 256, 0, st>>>(make_geo(ctx), ctx->lay, ctx->d_c, ctx->d_fre,
+                                                                         ctx->d_fim, ctx->d_bc, ctx->d_wxl, ctx->d_wyl,
+                                                                         mloc, w2M, wH, bfr, bfi, sedge);
+    HZ_CUDA(cudaGetLastError());
+  }
+  MinresArgs<real> a{};
+  a.lay = ctx->lay; a.sx = ctx->sx; a.sy = ctx->sy; a.E = ctx->E;
+  a.warm = o->warm_start; a.max_iters = o->max_iters; a.tol = (real)o->tol;
+  a.mloc = mloc; a.w2M = w2M; a.wH = wH; a.bf_re = bfr;
+  a.bf_im = (ctx->d_fim || ctx->d_bc) ? bfi : nullptr;
+  a.sedge = sedge;
+  a.bandx = (const real *)ctx->d_bandx; a.bandy = (const real *)ctx->d_bandy;
+  a.u_sub = (real *)ctx->d_usub; a.lam = (const real *)ctx->d_lam; a.gout = (real *)ctx->d_g;
+  a.k2edge = (const real *)ctx->d_k2;
+  a.iters = ctx->d_mr_iters; a.res = ctx->d_mr_res;
+  SweepLaunch cfg = ctx->launch;
+  const int P = ctx->p;
+  cfg.smem = 72 * sizeof(double) + 2 * (size_t)(ctx->lay.lnx + 2 * P) * (ctx->lay.lny + 2 * P) * sizeof(real);
+  cudaEvent_t e0, e1;
+  HZ_CUDA(cudaEventCreate(&e0));
+  HZ_CUDA(cudaEventCreate(&e1));
+  HZ_CUDA(cudaEventRecord(e0, st));
+  HZ_CUDA(launch_minres(a, P, cfg, st));
+  HZ_CUDA(cudaEventRecord(e1, st));
+  if (o->relax > 0.0) HZ_CUDA(launch_exchange(ctx, o->relax, st));
+  std::vector<int> hi(ctx->L);
+  std::vector<double> hr(ctx->L);
+  HZ_CUDA(cudaMemcpyAsync(hi.data(), ctx->d_mr_iters, ctx->L * sizeof(int), cudaMemcpyDeviceToHost, st));
+  HZ_CUDA(cudaMemcpyAsync(hr.data(), ctx->d_mr_res, ctx->L * sizeof(double), cudaMemcpyDeviceToHost, st));
+  HZ_CUDA(cudaStreamSynchronize(st));
+  float ms = 0.f;
+  cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  if (iters_out) std::memcpy(iters_out, hi.data(), ctx->L * sizeof(int));
+  if (res_out) std::memcpy(res_out, hr.data(), ctx->L * sizeof(double));
+  if (info) {
+    hz_minres_info inf{};
+    double sum = 0.0;
+    for (int l = 0; l < ctx->L; ++l) {
+      if (hi[l] > inf.iters_max) inf.iters_max = hi[l];
+      sum += hi[l];
+      if (hr[l] > inf.res_max) inf.res_max = hr[l];
+    }
+    inf.iters_mean = sum / ctx->L;
+    inf.kernel_ms = ms;
+    *info = inf;
+  }
+  return HZ_OK;
+}
+
+}  // namespace
+
+extern "C" hz_status hz_minres_cycle(hz_ctx *ctx, const hz_minres_opts *opts, int *iters_out, double *res_out,
+                                     hz_minres_info *info, void *stream) {
+  if (!ctx) return HZ_EINVAL;
+  if (!opts) return fail(ctx, HZ_EINVAL, "hz_minres_cycle: NULL opts");
+  if (!ctx->part) return fail(ctx, HZ_ESTATE, "hz_minres_cycle: call hz_partition first");
+  if (ctx->lay.variant != 0)
+    return fail(ctx, HZ_EUNSUPPORTED, "hz_minres_cycle: needs the one-DOF-per-thread partition (dofs_per_thread = 1)");
+  if (!(opts->tol >= 0.0) || opts->max_iters < 0 || opts->relax < 0.0 || opts->relax > 1.0)
+    return fail(ctx, HZ_EINVAL, "hz_minres_cycle: need tol >= 0, max_iters >= 0, relax in [0,1]");
+  cudaStream_t st = (cudaStream_t)stream;
+  return ctx->prec == HZ_F32 ? minres_impl<float>(ctx, opts, iters_out, res_out, info, st)
+                             : minres_impl<double>(ctx, opts, iters_out, res_out, info, st);
+}
 
 extern "C" hz_status hz_ddm_solve_gmres(hz_ctx *ctx, const hz_gmres_opts *opts, void *u_out, hz_gmres_info *info,
                                         void *stream) {

@@ -69,6 +69,52 @@ __global__ void k_build(Geo g, Layout lay, const double *__restrict__ c, const d
 }
 
 // ---------------------------------------------------------------------------------------------
+// Operator data of the MINRES comparator (block system (5)), natural slot layout:
+// m_j, w^2 M_j, w H_j, the load f m (+ outer-boundary datum) and the geometric edge weights s_j^{side}.
+// ---------------------------------------------------------------------------------------------
+template <typename real>
+__global__ void k_build_minres(Geo g, Layout lay, const double *__restrict__ c, const double *__restrict__ f_re,
+                               const double *__restrict__ f_im, const double *__restrict__ bc,
+                               const double *__restrict__ wxl, const double *__restrict__ wyl, real *mloc, real *w2M,
+                               real *wH, real *bf_re, real *bf_im, real *sedge) {
+  const int N = lay.lnx * lay.lny;
+  const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (gid >= (long long)g.sx * g.sy * N) return;
+  const int l = (int)(gid / N), q = (int)(gid - (long long)l * N);
+  const int i = q % lay.lnx, j = q / lay.lnx;
+  const int six = l % g.sx, siy = l / g.sx;
+  const int I = six * g.ex * g.p + i, J = siy * g.ey * g.p + j;
+  const size_t gn = (size_t)J * g.npx + I;
+  const double cj = c[gn];
+  const double m = 0.25 * g.hx * g.hy * wxl[i] * wyl[j];
+  const bool onW = i == 0, onE = i == lay.lnx - 1, onS = j == 0, onN = j == lay.lny - 1;
+  const double sWE = 0.5 * g.hy * wyl[j], sSN = 0.5 * g.hx * wxl[i];
+  double H = 0.0;
+  if (onW) H += sWE / cj;
+  if (onE) H += sWE / cj;
+  if (onS) H += sSN / cj;
+  if (onN) H += sSN / cj;
+  double bre = f_re[gn] * m, bim = f_im ? f_im[gn] * m : 0.0;
+  if (bc) {
+    if (onW && six == 0) { bre += sWE * bc[(0 * 2 + 0) * g.EB + J]; bim += sWE * bc[(0 * 2 + 1) * g.EB + J]; }
+    if (onE && six == g.sx - 1) { bre += sWE * bc[(1 * 2 + 0) * g.EB + J]; bim += sWE * bc[(1 * 2 + 1) * g.EB + J]; }
+    if (onS && siy == 0) { bre += sSN * bc[(2 * 2 + 0) * g.EB + I]; bim += sSN * bc[(2 * 2 + 1) * g.EB + I]; }
+    if (onN && siy == g.sy - 1) { bre += sSN * bc[(3 * 2 + 0) * g.EB + I]; bim += sSN * bc[(3 * 2 + 1) * g.EB + I]; }
+  }
+  const size_t o = (size_t)l * lay.NS + q;
+  mloc[o] = (real)m;
+  w2M[o] = (real)(g.omega * g.omega * m / (cj * cj));
+  wH[o] = (real)(g.omega * H);
+  bf_re[o] = (real)bre;
+  if (bf_im) bf_im[o] = (real)bim;
+  const size_t eb = (size_t)l * 4 * g.E;
+  if (onW) sedge[eb + 0 * g.E + j] = (real)sWE;
+  if (onE) sedge[eb + 1 * g.E + j] = (real)sWE;
+  if (onS) sedge[eb + 2 * g.E + i] = (real)sSN;
+  if (onN) sedge[eb + 3 * g.E + i] = (real)sSN;
+}
+
+// ---------------------------------------------------------------------------------------------
 // A8: exchange with relaxation (eq. (2); readings R3, R12):
 //   lambda^{n+1}_{r,o} = (1-rho) lambda^n_{r,o} + rho g_{nb(r,o), opp(o)}      on interface sides.
 // One thread per (subdomain r, side o, re/im, edge node); in place on lambda (each entry is read and

@@ -99,6 +99,10 @@ cudaError_t launch_sweep_tile_f64(const SweepArgs<double> &a, const TabC<double>
                                   cudaStream_t st);
 cudaError_t launch_sweep_stream_f32(const SweepArgs<float> &a, float *scr, int p, SweepLaunch cfg, cudaStream_t st);
 cudaError_t launch_sweep_stream_f64(const SweepArgs<double> &a, double *scr, int p, SweepLaunch cfg, cudaStream_t st);
+template <typename real>
+struct MinresArgs;
+cudaError_t launch_minres_f32(const MinresArgs<float> &a, int p, SweepLaunch cfg, cudaStream_t st);
+cudaError_t launch_minres_f64(const MinresArgs<double> &a, int p, SweepLaunch cfg, cudaStream_t st);
 // compiled register-blocked instantiations of one precision
 int tile_table_f32(const TileEntry **out);
 int tile_table_f64(const TileEntry **out);

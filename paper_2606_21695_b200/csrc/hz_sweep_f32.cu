@@ -46,6 +46,9 @@ cudaError_t launch_sweep_tile_f32(const SweepArgs<float> &a, const TabC<float> *
 cudaError_t launch_sweep_stream_f32(const SweepArgs<float> &a, float *scr, int p, SweepLaunch cfg, cudaStream_t st) {
   return launch_stream_impl<float>(a, scr, p, cfg, st);
 }
+cudaError_t launch_minres_f32(const MinresArgs<float> &a, int p, SweepLaunch cfg, cudaStream_t st) {
+  return launch_minres_impl<float>(a, p, cfg, st);
+}
 int tile_table_f32(const TileEntry **out) {
   *out = kTilesF32;
   return kNumTilesF32;

@@ -46,6 +46,9 @@ cudaError_t launch_sweep_tile_f64(const SweepArgs<double> &a, const TabC<double>
 cudaError_t launch_sweep_stream_f64(const SweepArgs<double> &a, double *scr, int p, SweepLaunch cfg, cudaStream_t st) {
   return launch_stream_impl<double>(a, scr, p, cfg, st);
 }
+cudaError_t launch_minres_f64(const MinresArgs<double> &a, int p, SweepLaunch cfg, cudaStream_t st) {
+  return launch_minres_impl<double>(a, p, cfg, st);
+}
 int tile_table_f64(const TileEntry **out) {
   *out = kTilesF64;
   return kNumTilesF64;

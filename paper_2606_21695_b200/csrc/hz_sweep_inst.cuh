@@ -2,6 +2,7 @@
 // Included by hz_sweep_f32.cu / hz_sweep_f64.cu (one translation unit per precision so they build in
 // parallel).  HZ_TILE_TABLE(X) lists X(P, MX, MY, CSM, MAXT, MINB).
 #pragma once
+#include "hz_minres.cuh"
 #include "hz_sweep.cuh"
 #include "hz_sweep_stream.cuh"
 #include "hz_sweep_tile.cuh"
@@ -17,6 +18,22 @@ static cudaError_t launch_dof_impl(const SweepArgs<real> &a, int p, SweepLaunch 
     case 2: fn = k_sweep_dof<real, 2>; break;
     case 3: fn = k_sweep_dof<real, 3>; break;
     case 4: fn = k_sweep_dof<real, 4>; break;
+    default: return cudaErrorInvalidValue;
+  }
+  cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem);
+  if (e != cudaSuccess) return e;
+  fn<<<cfg.blocks, cfg.threads, cfg.smem, st>>>(a);
+  return cudaGetLastError();
+}
+
+template <typename real>
+static cudaError_t launch_minres_impl(const MinresArgs<real> &a, int p, SweepLaunch cfg, cudaStream_t st) {
+  void (*fn)(const MinresArgs<real>) = nullptr;
+  switch (p) {
+    case 1: fn = k_minres_dof<real, 1>; break;
+    case 2: fn = k_minres_dof<real, 2>; break;
+    case 3: fn = k_minres_dof<real, 3>; break;
+    case 4: fn = k_minres_dof<real, 4>; break;
     default: return cudaErrorInvalidValue;
   }
   cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem);

@@ -21,7 +21,7 @@ HZ_TC_IMPEDANCE0 = 0
 STATUS_NAMES = {0: "HZ_OK", 1: "HZ_EINVAL", 2: "HZ_ENOMEM", 3: "HZ_ECUDA", 4: "HZ_EUNSUPPORTED", 5: "HZ_ESTATE"}
 
 # every symbol include/hz.h declares
-EXPORTS = ("hz_mesh_setup", "hz_set_source", "hz_partition", "hz_ddm_solve", "hz_ddm_solve_gmres", "hz_residual",
+EXPORTS = ("hz_mesh_setup", "hz_set_source", "hz_partition", "hz_ddm_solve", "hz_ddm_solve_gmres", "hz_minres_cycle", "hz_residual",
            "hz_get_subdomain_state", "hz_set_subdomain_state", "hz_last_error", "hz_destroy", "hz_peak_probe")
 
 
@@ -56,6 +56,14 @@ class hz_gmres_info(C.Structure):
                 ("rel_residual", C.c_double), ("total_ms", C.c_double), ("krylov_bytes", C.c_size_t)]
 
 
+class hz_minres_opts(C.Structure):
+    _fields_ = [("tol", C.c_double), ("max_iters", C.c_int), ("warm_start", C.c_int), ("relax", C.c_double)]
+
+
+class hz_minres_info(C.Structure):
+    _fields_ = [("iters_max", C.c_int), ("iters_mean", C.c_double), ("res_max", C.c_double), ("kernel_ms", C.c_double)]
+
+
 class HzError(RuntimeError):
     def __init__(self, status, msg):
         super().__init__(f"{STATUS_NAMES.get(status, status)}: {msg}")
@@ -81,6 +89,7 @@ def lib():
     L.hz_partition.argtypes = [vp, ip, ip, ip, ip, ip, C.c_double, C.POINTER(hz_part_info)]
     L.hz_ddm_solve.argtypes = [vp, C.POINTER(hz_solve_opts), vp, C.POINTER(hz_solve_info), vp]
     L.hz_ddm_solve_gmres.argtypes = [vp, C.POINTER(hz_gmres_opts), vp, C.POINTER(hz_gmres_info), vp]
+    L.hz_minres_cycle.argtypes = [vp, C.POINTER(hz_minres_opts), vp, vp, C.POINTER(hz_minres_info), vp]
     L.hz_residual.argtypes = [vp, vp, ip, dp, vp]
     L.hz_get_subdomain_state.argtypes = [vp, vp, vp, vp]
     L.hz_set_subdomain_state.argtypes = [vp, vp, vp, vp]
@@ -164,6 +173,17 @@ def hz_ddm_solve_gmres(ctx, max_steps, n_wh=2, relax=0.5, restart=50, lin_tol=0.
     if want_history:
         return info, [hist[i] for i in range(info.steps_done)]
     return info
+
+
+def hz_minres_cycle(ctx, blocks, tol, max_iters, warm_start=False, relax=0.0, stream=None):
+    """-> (hz_minres_info, iterations per subdomain, true relative residual per subdomain)"""
+    opts = hz_minres_opts(float(tol), int(max_iters), int(bool(warm_start)), float(relax))
+    info = hz_minres_info()
+    iters = np.zeros(blocks, dtype=np.int32)
+    res = np.zeros(blocks, dtype=np.float64)
+    _check(ctx, lib().hz_minres_cycle(ctx, C.byref(opts), iters.ctypes.data_as(C.c_void_p), res.ctypes.data_as(C.c_void_p),
+                                      C.byref(info), C.c_void_p(stream) if stream else None))
+    return info, iters, res
 
 
 def hz_residual(ctx, u_ptr, u_prec, stream=None):
