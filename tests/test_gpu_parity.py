@@ -325,3 +325,12 @@ def test_auto_falls_back_to_streamed_when_state_does_not_fit():
     # 2x2 subdomains of 32x32 elements, p=3, fp64: 9409 DOF x 6 values x 8 B = 452 KB > one SM (config-4 block shape)
     g = check_case(make_config(4, n=64, sub_elems=32), hz.HZ_F64, 0, n_outer=2, n_wh=1)
     assert g["info"].dofs_per_thread == -1
+
+
+def test_more_than_256_time_steps_uses_the_shared_memory_table():
+    """The register-blocked kernels take the time-step table as a kernel parameter (<= 256 rows); a finer CFL
+    fraction must fall back to a variant that keeps the table in shared / global memory, with the same result."""
+    inp = make_config(2, n=16)
+    inp.cfl_frac = 0.2
+    g = check_case(inp, hz.HZ_F64, 0, n_outer=2, n_wh=1)
+    assert g["info"].n_t > 256 and g["info"].dofs_per_thread == 1
