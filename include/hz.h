@@ -227,9 +227,8 @@ const char *hz_last_error(const hz_ctx *ctx);
 /* Frees the context and all its device memory.  NULL-safe. */
 void hz_destroy(hz_ctx *ctx);
 
-/* Micro-benchmarks that establish this GPU's own CUDA-core and shared-memory ceilings (used by
- * bench.py for the roofline denominators; no method arithmetic).  kind: 0 = FP32 FMA, 1 = FP64 FMA,
- * 2 = shared-memory load bandwidth.  Returns TFLOP/s (kinds 0,1; 2 flops per FMA) or TB/s (kind 2). */
+/* Micro-benchmark that establishes this GPU's own CUDA-core FMA ceiling (used by bench.py beside the derived
+ * roofline denominator; no method arithmetic).  kind: 0 = FP32 FMA, 1 = FP64 FMA.  Returns TFLOP/s (2 flops per FMA). */
 hz_status hz_peak_probe(int kind, double *result, void *stream);
 
 #ifdef __cplusplus

@@ -1099,7 +1099,7 @@ void hz_destroy(hz_ctx *ctx) {
 }
 
 hz_status hz_peak_probe(int kind, double *result, void *stream) {
-  if (!result || kind < 0 || kind > 2) return HZ_EINVAL;
+  if (!result || kind < 0 || kind > 1) return HZ_EINVAL;
   cudaStream_t st = (cudaStream_t)stream;
   cudaDeviceProp prop;
   int dev = 0;
@@ -1119,19 +1119,12 @@ hz_status hz_peak_probe(int kind, double *result, void *stream) {
       k_probe_fma<float><<<blocks, thr, 0, st>>>(iters, 1.0f, d_out);
       cudaEventRecord(e1, st);
       work = 2.0 * 64.0 * iters * (double)blocks * thr;
-    } else if (kind == 1) {
+    } else {
       const int iters = 2048, blocks = sms * 8, thr = 256;
       cudaEventRecord(e0, st);
       k_probe_fma<double><<<blocks, thr, 0, st>>>(iters, 1.0, (double *)d_out);
       cudaEventRecord(e1, st);
       work = 2.0 * 64.0 * iters * (double)blocks * thr;
-    } else {
-      const int iters = 2048, blocks = sms * 2, thr = 1024;
-      cudaFuncSetAttribute(k_probe_lds, cudaFuncAttributeMaxDynamicSharedMemorySize, 32768);
-      cudaEventRecord(e0, st);
-      k_probe_lds<<<blocks, thr, 32768, st>>>(iters, d_out);
-      cudaEventRecord(e1, st);
-      work = 16.0 * 8.0 * iters * (double)blocks * thr;  // bytes
     }
     if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) { cudaFree(d_out); return HZ_ECUDA; }
     cudaEventElapsedTime(&ms, e0, e1);

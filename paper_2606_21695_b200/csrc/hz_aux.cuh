@@ -316,7 +316,7 @@ __global__ void k_convert(long long n, const A *__restrict__ in, B *__restrict__
 }
 
 // ---------------------------------------------------------------------------------------------
-// Peak probes (no method arithmetic): dependent-chain-free FMA streams and shared-memory loads.
+// Peak probe (no method arithmetic): independent FMA streams.
 // ---------------------------------------------------------------------------------------------
 template <typename real>
 __global__ void __launch_bounds__(256) k_probe_fma(int iters, real seed, real *out) {
@@ -334,25 +334,6 @@ __global__ void __launch_bounds__(256) k_probe_fma(int iters, real seed, real *o
 #pragma unroll
   for (int q = 0; q < 16; ++q) s += a[q];
   if (s == real(-12345)) out[0] = s;
-}
-
-__global__ void __launch_bounds__(1024) k_probe_lds(int iters, float *out) {
-  extern __shared__ __align__(16) float sm_f[];
-  for (int q = threadIdx.x; q < 8192; q += blockDim.x) sm_f[q] = (float)q;
-  __syncthreads();
-  // 2048 float4 = 32 KB; lane-consecutive 16-byte loads (conflict-free LDS.128)
-  const unsigned base = (unsigned)__cvta_generic_to_shared(sm_f) + (threadIdx.x & 255) * 16u;
-  float acc0 = 0.f, acc1 = 0.f;
-  for (int it = 0; it < iters; ++it) {
-#pragma unroll
-    for (int r = 0; r < 8; ++r) {
-      float x, y, z, w;
-      asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(x), "=f"(y), "=f"(z), "=f"(w) : "r"(base + r * 4096u));
-      acc0 += x;
-      acc1 += w;
-    }
-  }
-  if (acc0 + acc1 == -1.f) out[0] = acc0;
 }
 
 }  // namespace hz
