@@ -22,6 +22,7 @@ namespace hz {
   W(1, 4, 0, 512, 1)       \
   W(2, 1, 0, 1024, 1)      \
   W(2, 2, 0, 384, 1)       \
+  W(3, 1, 0, 128, 5)       \
   W(3, 1, 0, 256, 1)       \
   W(3, 1, 0, 512, 1)       \
   W(3, 2, 1, 320, 1)       \
