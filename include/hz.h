@@ -79,6 +79,8 @@ typedef struct {
   int blocks;            /* = sx*sy subdomains = thread blocks of one sweep launch */
   int dofs_per_thread;   /* 1, or (mx*p)*(my*p) of the register-blocked variant, or -1 (streamed) */
   int tile_mx, tile_my;  /* elements per thread tile (0 for the one-DOF-per-thread variant) */
+  int cluster_size;      /* thread blocks (CTAs of one cluster, on as many SMs) per subdomain; 1 unless the state of
+                            a subdomain needs the registers of several SMs (hz_sweep_cl.cuh) */
   double dt, theta, sigma; /* dt = T/n_t; theta = tan(w dt/2)/w; sigma = 2 sin(w dt/2)/w */
   size_t smem_bytes;       /* dynamic shared memory per block */
   size_t workspace_bytes;  /* device bytes the context allocated for this partition */

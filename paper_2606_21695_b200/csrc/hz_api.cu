@@ -138,7 +138,7 @@ struct hz_ctx {
   // partition
   bool part = false;
   int sx = 0, sy = 0, ex = 0, ey = 0, L = 0, E = 0, prec = 0;
-  int mx = 0, my = 0, csm = 0, ws = 0, entry = -1;
+  int mx = 0, my = 0, csm = 0, ws = 0, cl = 1, entry = -1;
   Layout lay{};
   SweepLaunch launch{};
   int n_t = 0;
@@ -475,10 +475,15 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
   if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev);
   const char *env_ws = std::getenv("HZ_DISABLE_WS");  // debug knob: force the non-specialised tile kernel
   const bool no_ws = env_ws && env_ws[0] == '1';
+  const char *env_cl = std::getenv("HZ_DISABLE_CLUSTER");  // debug knob: never pick a cluster kernel
+  const bool no_cl = env_cl && env_cl[0] == '1';
+  const char *env_fc = std::getenv("HZ_FORCE_CLUSTER");  // debug knob: only cluster kernels of this size compete
+  const int force_cl = env_fc ? std::atoi(env_fc) : 0;
   const char *env_rc = std::getenv("HZ_NO_REGCAP");  // debug knob: never pick a register-capped instantiation
   const bool no_regcap = env_rc && env_rc[0] == '1';
   auto tile_fit = [&](const TileEntry &t, Layout *lo, SweepLaunch *la) -> bool {
     if (t.p != P || ctx->ex % t.mx || ctx->ey % t.my) return false;
+    if (force_cl > 1 && t.cl != force_cl) return false;
     Layout q = lay;
     q.variant = 1; q.TX = t.mx * P; q.TY = t.my * P;
     q.ntx = ctx->ex / t.mx + 1; q.nty = ctx->ey / t.my + 1;
@@ -486,7 +491,16 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
     int nthr = ntv;
     size_t sm = 0;
     const size_t narr = 2 * (size_t)(q.TX + q.TY);
-    if (t.ws) {
+    if (t.cl > 1) {
+      if (no_cl || n_t > kTabCMax || q.ntx < t.cl) return false;
+      const int wmax = (q.ntx + t.cl - 1) / t.cl;
+      nthr = roundup(wmax * q.nty, 32);
+      const size_t v16 = 16 / rs;
+      const size_t chx = ((size_t)q.TX + v16 - 1) / v16 * v16, chy = ((size_t)q.TY + v16 - 1) / v16 * v16;
+      size_t rsw = 2 * chx + 2 * chy;
+      if ((rsw / v16) % 2 == 0) rsw += v16;
+      sm = 2 * (size_t)(nthr + 33) * rsw * rs + 2 * (size_t)(2 * q.nty) * chy * rs + 16;  // records, halo slots, 2 mbarriers
+    } else if (t.ws) {
       if (no_ws || n_t > kTabCMax) return false;
       nthr = roundup((q.ntx - 1) * (q.nty - 1), 32) + roundup(q.ntx + q.nty - 1, 32);
       const int nbulk = (q.ntx - 1) * (q.nty - 1), nedge = q.ntx + q.nty - 1;
@@ -506,7 +520,7 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
     if (nthr > t.maxt) return false;
     q.NT = ntv; q.NS = q.TX * q.TY * ntv;
     if (sm > smem_cap) return false;
-    *lo = q; la->blocks = ctx->L; la->threads = nthr; la->smem = sm;
+    *lo = q; la->blocks = ctx->L * t.cl; la->threads = nthr; la->smem = sm;
     return true;
   };
   const bool complex_f = ctx->d_fim != nullptr;
@@ -536,7 +550,12 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
         const long long nbulk_ = (long long)(ctx->ex / q.mx) * (ctx->ey / q.my);
         // ... provided the subdomain still has two warps of full tiles; otherwise the smaller tile
         const long long dk = nbulk_ < 64 ? 100 + k_ : (k_ < 9 ? 9 - k_ : (k_ > 16 ? k_ - 16 : 0));
-        return (long long)q.csm * 100000000 + (q.csm ? k_ * 100 + (1 - q.ws) : (long long)(1 - q.ws) * 1000000 + dk * 1000 + k_) * 10 - q.minb;
+        // tiers: (0) one CTA, everything in registers; (1) one CTA, warp-specialised, coefficients in shared memory,
+        // tiles of at most 16 DOFs; (2) clusters, smallest first; (3) the remaining shared-memory-coefficient kernels
+        // (measured order on configs 4 and 5, profiles/r01_config_sweep.md)
+        if (q.cl > 1) return 200000000LL + q.cl * 1000 + k_;
+        if (q.csm) return ((q.ws && k_ <= 16) ? 100000000LL : 300000000LL) + k_ * 100 + (1 - q.ws);
+        return ((long long)(1 - q.ws) * 1000000 + dk * 1000 + k_) * 10 - q.minb;
       };
       const long long score = score_of(t);
       const long long bscore = best < 0 ? 0 : score_of(tiles[best]);
@@ -553,11 +572,12 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
   if (best >= 0) {
     ctx->lay = blay; ctx->launch = bl;
     ctx->mx = tiles[best].mx; ctx->my = tiles[best].my; ctx->csm = tiles[best].csm; ctx->ws = tiles[best].ws;
+    ctx->cl = tiles[best].cl;
     ctx->entry = best;
   } else if (streamed) {
     lay.variant = 2; lay.NT = N < 1024 ? roundup(N, 32) : 1024; lay.NS = roundup(N, 32); lay.TX = lay.TY = 1;
     lay.ntx = lay.nty = 0;
-    ctx->lay = lay; ctx->mx = ctx->my = 0; ctx->csm = 0; ctx->ws = 0;
+    ctx->lay = lay; ctx->mx = ctx->my = 0; ctx->csm = 0; ctx->ws = 0; ctx->cl = 1;
     ctx->launch.blocks = ctx->L; ctx->launch.threads = lay.NT; ctx->launch.smem = 0;
   } else {
     lay.variant = 0; lay.NT = roundup(N, 32); lay.NS = lay.NT; lay.TX = lay.TY = 1; lay.ntx = lay.nty = 0;
@@ -629,7 +649,7 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
     inf.n_t = n_t; inf.dofs_per_sub = N; inf.edge_nodes_x = lnx; inf.edge_nodes_y = lny; inf.edge_stride = ctx->E;
     inf.threads_per_block = ctx->launch.threads; inf.blocks = ctx->L;
     inf.dofs_per_thread = ctx->lay.variant == 0 ? 1 : (ctx->lay.variant == 2 ? -1 : ctx->lay.TX * ctx->lay.TY);
-    inf.tile_mx = ctx->mx; inf.tile_my = ctx->my;
+    inf.tile_mx = ctx->mx; inf.tile_my = ctx->my; inf.cluster_size = ctx->lay.variant == 1 ? ctx->cl : 1;
     inf.dt = ctx->dt; inf.theta = ctx->theta; inf.sigma = ctx->sigma;
     inf.smem_bytes = ctx->launch.smem; inf.workspace_bytes = ws;
     *info_out = inf;

@@ -82,6 +82,7 @@ struct TileEntry {
   int p, mx, my, csm, maxt;  // csm: gamma / beta b in shared memory instead of registers
   int ws;                    // 1: warp-specialised kernel (hz_sweep_ws.cuh), needs mx == my
   int minb;                  // __launch_bounds__ min blocks per SM (register cap = 64K / (minb * maxt))
+  int cl;                    // > 1: thread-block-cluster kernel (hz_sweep_cl.cuh), CTAs per subdomain
   const void *fn;
 };
 

@@ -28,11 +28,25 @@ namespace hz {
   W(3, 2, 1, 320, 1)       \
   W(4, 1, 0, 384, 1)
 
+// C(P, MX, MY, CL, MAXT, MINB): cluster of CL CTAs per subdomain, coefficients in registers
+#define HZ_CL_TABLE_F32(C) \
+  C(3, 1, 1, 2, 576, 1)    \
+  C(3, 1, 1, 4, 320, 2)    \
+  C(3, 1, 1, 8, 192, 3)    \
+  C(3, 1, 1, 8, 640, 1)    \
+  C(2, 2, 2, 2, 384, 1)    \
+  C(2, 2, 2, 4, 384, 1)    \
+  C(4, 1, 1, 2, 384, 1)    \
+  C(4, 1, 1, 4, 384, 1)
+
 #define X_ENTRY(P, MX, MY, CSM, MAXT, MINB) \
-  {P, MX, MY, CSM, MAXT, 0, MINB, (const void *)k_sweep_tile<float, P, MX, MY, (CSM != 0), MAXT, MINB>},
+  {P, MX, MY, CSM, MAXT, 0, MINB, 1, (const void *)k_sweep_tile<float, P, MX, MY, (CSM != 0), MAXT, MINB>},
 #define W_ENTRY(P, M, CSM, MAXT, MINB) \
-  {P, M, M, CSM, MAXT, 1, MINB, (const void *)k_sweep_ws<float, P, M, (CSM != 0), MAXT, MINB>},
-static const TileEntry kTilesF32[] = {HZ_WS_TABLE_F32(W_ENTRY) HZ_TILE_TABLE_F32(X_ENTRY)};
+  {P, M, M, CSM, MAXT, 1, MINB, 1, (const void *)k_sweep_ws<float, P, M, (CSM != 0), MAXT, MINB>},
+#define C_ENTRY(P, MX, MY, CL, MAXT, MINB) \
+  {P, MX, MY, 0, MAXT, 0, MINB, CL, (const void *)k_sweep_cl<float, P, MX, MY, CL, MAXT, MINB>},
+static const TileEntry kTilesF32[] = {HZ_WS_TABLE_F32(W_ENTRY) HZ_TILE_TABLE_F32(X_ENTRY) HZ_CL_TABLE_F32(C_ENTRY)};
+#undef C_ENTRY
 #undef X_ENTRY
 #undef W_ENTRY
 static const int kNumTilesF32 = sizeof(kTilesF32) / sizeof(kTilesF32[0]);

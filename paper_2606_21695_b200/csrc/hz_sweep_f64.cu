@@ -27,11 +27,26 @@ namespace hz {
   W(3, 1, 1, 512, 1)       \
   W(4, 1, 1, 320, 1)
 
+// C(P, MX, MY, CL, MAXT, MINB): cluster of CL CTAs per subdomain, coefficients in registers
+#define HZ_CL_TABLE_F64(C) \
+  C(3, 1, 1, 2, 320, 1)    \
+  C(3, 1, 1, 4, 320, 1)    \
+  C(3, 1, 1, 8, 192, 2)    \
+  C(3, 1, 1, 8, 320, 1)    \
+  C(2, 1, 1, 2, 512, 1)    \
+  C(2, 1, 1, 4, 512, 1)    \
+  C(1, 2, 2, 2, 1024, 1)   \
+  C(4, 1, 1, 4, 128, 1)    \
+  C(4, 1, 1, 8, 128, 1)
+
 #define X_ENTRY(P, MX, MY, CSM, MAXT, MINB) \
-  {P, MX, MY, CSM, MAXT, 0, MINB, (const void *)k_sweep_tile<double, P, MX, MY, (CSM != 0), MAXT, MINB>},
+  {P, MX, MY, CSM, MAXT, 0, MINB, 1, (const void *)k_sweep_tile<double, P, MX, MY, (CSM != 0), MAXT, MINB>},
 #define W_ENTRY(P, M, CSM, MAXT, MINB) \
-  {P, M, M, CSM, MAXT, 1, MINB, (const void *)k_sweep_ws<double, P, M, (CSM != 0), MAXT, MINB>},
-static const TileEntry kTilesF64[] = {HZ_WS_TABLE_F64(W_ENTRY) HZ_TILE_TABLE_F64(X_ENTRY)};
+  {P, M, M, CSM, MAXT, 1, MINB, 1, (const void *)k_sweep_ws<double, P, M, (CSM != 0), MAXT, MINB>},
+#define C_ENTRY(P, MX, MY, CL, MAXT, MINB) \
+  {P, MX, MY, 0, MAXT, 0, MINB, CL, (const void *)k_sweep_cl<double, P, MX, MY, CL, MAXT, MINB>},
+static const TileEntry kTilesF64[] = {HZ_WS_TABLE_F64(W_ENTRY) HZ_TILE_TABLE_F64(X_ENTRY) HZ_CL_TABLE_F64(C_ENTRY)};
+#undef C_ENTRY
 #undef X_ENTRY
 #undef W_ENTRY
 static const int kNumTilesF64 = sizeof(kTilesF64) / sizeof(kTilesF64[0]);

@@ -5,6 +5,7 @@
 #include "hz_minres.cuh"
 #include "hz_sweep.cuh"
 #include "hz_sweep_stream.cuh"
+#include "hz_sweep_cl.cuh"
 #include "hz_sweep_tile.cuh"
 #include "hz_sweep_ws.cuh"
 
@@ -63,6 +64,21 @@ static cudaError_t launch_tile_impl(const TileEntry *tab, int n, const SweepArgs
   if (err != cudaSuccess) return err;
   if (!tc) return cudaErrorInvalidValue;
   auto fn = reinterpret_cast<void (*)(const SweepArgs<real>, const TabC<real>)>(const_cast<void *>(e.fn));
+  if (e.cl > 1) {  // one cluster of e.cl CTAs per subdomain
+    cudaLaunchConfig_t lc = {};
+    lc.gridDim = dim3(cfg.blocks, 1, 1);
+    lc.blockDim = dim3(cfg.threads, 1, 1);
+    lc.dynamicSmemBytes = cfg.smem;
+    lc.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeClusterDimension;
+    at[0].val.clusterDim.x = e.cl;
+    at[0].val.clusterDim.y = 1;
+    at[0].val.clusterDim.z = 1;
+    lc.attrs = at;
+    lc.numAttrs = 1;
+    return cudaLaunchKernelEx(&lc, fn, a, *tc);
+  }
   fn<<<cfg.blocks, cfg.threads, cfg.smem, st>>>(a, *tc);
   return cudaGetLastError();
 }

@@ -28,7 +28,7 @@ EXPORTS = ("hz_mesh_setup", "hz_set_source", "hz_partition", "hz_ddm_solve", "hz
 class hz_part_info(C.Structure):
     _fields_ = [("n_t", C.c_int), ("dofs_per_sub", C.c_int), ("edge_nodes_x", C.c_int), ("edge_nodes_y", C.c_int),
                 ("edge_stride", C.c_int), ("threads_per_block", C.c_int), ("blocks", C.c_int),
-                ("dofs_per_thread", C.c_int), ("tile_mx", C.c_int), ("tile_my", C.c_int),
+                ("dofs_per_thread", C.c_int), ("tile_mx", C.c_int), ("tile_my", C.c_int), ("cluster_size", C.c_int),
                 ("dt", C.c_double), ("theta", C.c_double), ("sigma", C.c_double),
                 ("smem_bytes", C.c_size_t), ("workspace_bytes", C.c_size_t)]
 
