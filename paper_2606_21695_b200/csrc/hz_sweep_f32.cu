@@ -37,7 +37,8 @@ namespace hz {
   C(2, 2, 2, 2, 384, 1)    \
   C(2, 2, 2, 4, 384, 1)    \
   C(4, 1, 1, 2, 384, 1)    \
-  C(4, 1, 1, 4, 384, 1)
+  C(4, 1, 1, 4, 384, 1)    \
+  C(4, 1, 1, 16, 352, 1)
 
 #define X_ENTRY(P, MX, MY, CSM, MAXT, MINB) \
   {P, MX, MY, CSM, MAXT, 0, MINB, 1, (const void *)k_sweep_tile<float, P, MX, MY, (CSM != 0), MAXT, MINB>},

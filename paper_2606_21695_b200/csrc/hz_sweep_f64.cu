@@ -37,7 +37,11 @@ namespace hz {
   C(2, 1, 1, 4, 512, 1)    \
   C(1, 2, 2, 2, 1024, 1)   \
   C(4, 1, 1, 4, 128, 1)    \
-  C(4, 1, 1, 8, 128, 1)
+  C(4, 1, 1, 8, 128, 1)    \
+  C(4, 1, 1, 8, 192, 1)    \
+  C(2, 2, 2, 8, 192, 1)    \
+  C(2, 1, 1, 8, 608, 1)    \
+  C(3, 1, 1, 16, 352, 1)
 
 #define X_ENTRY(P, MX, MY, CSM, MAXT, MINB) \
   {P, MX, MY, CSM, MAXT, 0, MINB, 1, (const void *)k_sweep_tile<double, P, MX, MY, (CSM != 0), MAXT, MINB>},

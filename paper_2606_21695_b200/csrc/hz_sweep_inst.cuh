@@ -65,6 +65,10 @@ static cudaError_t launch_tile_impl(const TileEntry *tab, int n, const SweepArgs
   if (!tc) return cudaErrorInvalidValue;
   auto fn = reinterpret_cast<void (*)(const SweepArgs<real>, const TabC<real>)>(const_cast<void *>(e.fn));
   if (e.cl > 1) {  // one cluster of e.cl CTAs per subdomain
+    if (e.cl > 8) {  // beyond the portable cluster size
+      err = cudaFuncSetAttribute(e.fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+      if (err != cudaSuccess) return err;
+    }
     cudaLaunchConfig_t lc = {};
     lc.gridDim = dim3(cfg.blocks, 1, 1);
     lc.blockDim = dim3(cfg.threads, 1, 1);

@@ -26,7 +26,7 @@ def run(cfg, prec, k, n=None, p=None, s=None, nwh=5, reps=3):
     try:
         ctx, info = hz.setup_from_inputs(inp, prec, k)
     except hz.HzError as e:
-        print(f"{name} {k or 'auto'} | — | — | — | — | — | — | {e.args[0].split(':', 1)[0]} |", flush=True)
+        print(f"{name} {k or 'auto'} | — | — | — | — | — | — | — | {e.args[0].split(':', 1)[0]} |", flush=True)
         return
     try:
         hz.hz_ddm_solve(ctx, 1, n_wh=nwh, reset_state=True)
@@ -34,7 +34,7 @@ def run(cfg, prec, k, n=None, p=None, s=None, nwh=5, reps=3):
         rate = r.dof_timesteps / (r.sweep_ms_total * 1e-3)
         fl = 2 * (2 * (inp.p + 2) + 5)
         peak = SMS * (128 if prec == hz.HZ_F32 else 64) * 2 * CLK
-        print(f"{name} {info.dofs_per_thread} | {info.dofs_per_sub} | {info.blocks} | {info.threads_per_block} | "
+        print(f"{name} {info.dofs_per_thread} | {info.cluster_size} | {info.dofs_per_sub} | {info.blocks} | {info.threads_per_block} | "
               f"{info.smem_bytes} | {r.sweep_ms_total / reps:.3f} | {rate:.3e} | {rate * fl / peak:.3f} |", flush=True)
     finally:
         hz.hz_destroy(ctx)
@@ -45,8 +45,8 @@ def main():
     ap.add_argument("which", choices=["cfg2", "cfg3", "cfg4", "cfg5"])
     ap.add_argument("--scale", type=int, default=4)
     a = ap.parse_args()
-    print("| cfg | n | p | sub side | prec | DOF/thread | DOF/sub | blocks | threads | smem B | sweep ms | DOF-steps/s | frac of FMA peak |")
-    print("|---|---|---|---|---|---|---|---|---|---|---|---|---|")
+    print("| cfg | n | p | sub side | prec | DOF/thread | CTAs/sub | DOF/sub | blocks | threads | smem B | sweep ms | DOF-steps/s | frac of FMA peak |")
+    print("|---|---|---|---|---|---|---|---|---|---|---|---|---|---|")
     if a.which in ("cfg2", "cfg3"):
         for prec in (hz.HZ_F32, hz.HZ_F64):
             for k in (1, 9):
