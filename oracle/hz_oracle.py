@@ -7,7 +7,7 @@ Only `tests/`, `__graft_entry__.smoke()` and `bench.py`'s `cpu_baseline` /
 generator with `paper_2606_21695_b200/` (the CUDA path) and never imports it.
 
 Citations are "PAPER.md:<line> (section / equation)".  Where the paper is silent,
-garbled or inconsistent the reading is the one listed in DESIGN.md ("Readings", R1..R23).
+garbled or inconsistent the reading is the one listed in DESIGN.md ("Readings", R1..R24).
 
 What is pinned (tests/test_oracle_pins.py; none of the pins re-types a formula below):
   gll()                      sum(w)=2, D exact on polynomials, symmetry, Lambda_1=4, Lambda_2=24
@@ -25,6 +25,11 @@ What is pinned (tests/test_oracle_pins.py; none of the pins re-types a formula b
   minres()/block_system()    (tests/test_oracle_minres_pins.py) symmetry/indefiniteness of (5), iterate == residual
                              minimiser over an explicit Krylov basis, recurrence residual == true residual,
                              converged == dense direct solve, agreement with scipy.sparse.linalg.minres
+  quad_geometry()/element_stiffness_quad()/region_operators_quads()/choose_nt_quads()
+                             (tests/test_oracle_quads_pins.py) rectangles reduce to the pinned rectangular operators,
+                             patch test (A x linear = 0 inside), exact area / first moment / side lengths, the
+                             N_t bound really bounds lmax(M^-1 A), plane wave recovered at high order on a
+                             distorted mesh, converged DDM == direct solve on a distorted mesh
 Nothing here is "parity unpinned".
 
 Conventions
@@ -121,6 +126,8 @@ class Problem:
     omega: float
     f: np.ndarray                # (ny*p+1, nx*p+1) complex source AT the nodes
     bc_lambda: list | None = None  # 4 complex edge arrays (W,E,S,N) or None (=0)
+    vx: np.ndarray | None = None   # F3: (ny+1, nx+1) vertex coordinates of straight-sided convex quads on a
+    vy: np.ndarray | None = None   #     logically rectangular mesh; when given, x0..y1 are ignored
 
     @property
     def hx(self):
@@ -197,7 +204,10 @@ def edge_index(npx, npy, side):
 def assemble_global(pr: Problem):
     """Returns A (sparse real), M (diag, real), H (diag, real; outer boundary only), b (complex)
     of  (A - i w H - w^2 M) u = b,  PAPER.md:105-111."""
-    A, m, s = _region_operators(pr.p, pr.nx, pr.ny, pr.hx, pr.hy)
+    if pr.vx is not None:
+        A, m, s = region_operators_quads(pr.p, pr.vx, pr.vy)
+    else:
+        A, m, s = _region_operators(pr.p, pr.nx, pr.ny, pr.hx, pr.hy)
     c = np.asarray(pr.c_nodes, dtype=float).reshape(-1)
     M = m.reshape(-1) / c ** 2
     H = np.zeros_like(M)
@@ -340,17 +350,25 @@ def ddm_setup(pr: Problem, sx: int, sy: int, cfl_frac: float = 0.5, n_t: int | N
     if pr.nx % sx or pr.ny % sy:
         raise ValueError("subdomain grid must divide the element grid (reading R23)")
     ex, ey = pr.nx // sx, pr.ny // sy
-    A, m, s = _region_operators(pr.p, ex, ey, pr.hx, pr.hy)
+    quads = pr.vx is not None
+    if not quads:
+        A, m, s = _region_operators(pr.p, ex, ey, pr.hx, pr.hy)
     npx, npy = ex * pr.p + 1, ey * pr.p + 1
     c = np.asarray(pr.c_nodes, dtype=float)
     f = np.asarray(pr.f, dtype=complex)
     if n_t is None:
-        n_t = choose_nt(pr.p, pr.hx, pr.hy, float(c.max()), pr.omega, cfl_frac)
+        if quads:
+            n_t = choose_nt_quads(pr.p, pr.vx, pr.vy, c, pr.omega, cfl_frac)
+        else:
+            n_t = choose_nt(pr.p, pr.hx, pr.hy, float(c.max()), pr.omega, cfl_frac)
     tab = wh_tables(n_t, pr.omega)
     subs = []
     for iy in range(sy):
         for ix in range(sx):
             I0, J0 = ix * ex * pr.p, iy * ey * pr.p
+            if quads:   # F3: the subdomain's own elements, from its block of the vertex arrays
+                A, m, s = region_operators_quads(pr.p, pr.vx[iy * ey:(iy + 1) * ey + 1, ix * ex:(ix + 1) * ex + 1],
+                                                 pr.vy[iy * ey:(iy + 1) * ey + 1, ix * ex:(ix + 1) * ex + 1])
             cl = c[J0:J0 + npy, I0:I0 + npx].reshape(-1)
             fl = f[J0:J0 + npy, I0:I0 + npx].reshape(-1)
             M = m.reshape(-1) / cl ** 2
@@ -635,3 +653,124 @@ def ddm_sweep_minres(st: DDMState, tol: float, max_iters: int, warm_start: bool,
     st.lam, st.u = new_lam, new_u
     st.n_sweeps += 1
     return its
+
+
+# --------------------------------------------------------------------------------------
+# F3  General straight-sided convex quadrilaterals ("quadrilateral ... elements",
+#     gradient through D, "geometric factors" at the quadrature points, then D^T;
+#     SURVEY.md section 8(f) F3).  The mesh is logically rectangular: element (fx,fy) has the vertices
+#     (vx,vy)[fy:fy+2, fx:fx+2]; each element is the bilinear image of the reference square [-1,1]^2.
+#     Pins: tests/test_oracle_quads_pins.py (rectangles reduce to _region_operators, patch test,
+#     exact area / first moment / side lengths, plane-wave convergence on a distorted mesh,
+#     converged DDM == direct solve on a distorted mesh).
+# --------------------------------------------------------------------------------------
+def quad_geometry(p: int, X4, Y4):
+    """Element map x(xi,eta) = sum_k N_k(xi,eta) x_k with the bilinear N_k; X4[b][a] is the vertex at
+    (xi,eta) = (2a-1, 2b-1).  Returns, at the (p+1)^2 GLL points [b,a] (eta index first):
+    x, y, detJ and the three geometric factors of  grad u . grad v detJ = (u_xi,u_eta) g (v_xi,v_eta)^T,
+    g = detJ J^-1 J^-T  (J = d(x,y)/d(xi,eta)):  gxx = (x_eta^2+y_eta^2)/detJ,
+    gxy = -(x_xi x_eta + y_xi y_eta)/detJ, gyy = (x_xi^2+y_xi^2)/detJ."""
+    xi, _, _ = gll(p)
+    X4, Y4 = np.asarray(X4, dtype=float), np.asarray(Y4, dtype=float)
+    XI, ETA = np.meshgrid(xi, xi)                       # [b,a]: XI varies along a
+    N00, N10 = (1 - XI) * (1 - ETA) / 4, (1 + XI) * (1 - ETA) / 4
+    N01, N11 = (1 - XI) * (1 + ETA) / 4, (1 + XI) * (1 + ETA) / 4
+    x = N00 * X4[0, 0] + N10 * X4[0, 1] + N01 * X4[1, 0] + N11 * X4[1, 1]
+    y = N00 * Y4[0, 0] + N10 * Y4[0, 1] + N01 * Y4[1, 0] + N11 * Y4[1, 1]
+    x_xi = ((1 - ETA) * (X4[0, 1] - X4[0, 0]) + (1 + ETA) * (X4[1, 1] - X4[1, 0])) / 4
+    y_xi = ((1 - ETA) * (Y4[0, 1] - Y4[0, 0]) + (1 + ETA) * (Y4[1, 1] - Y4[1, 0])) / 4
+    x_eta = ((1 - XI) * (X4[1, 0] - X4[0, 0]) + (1 + XI) * (X4[1, 1] - X4[0, 1])) / 4
+    y_eta = ((1 - XI) * (Y4[1, 0] - Y4[0, 0]) + (1 + XI) * (Y4[1, 1] - Y4[0, 1])) / 4
+    det = x_xi * y_eta - x_eta * y_xi
+    if np.any(det <= 0):
+        raise ValueError("element is not convex / not positively oriented")
+    gxx = (x_eta ** 2 + y_eta ** 2) / det
+    gxy = -(x_xi * x_eta + y_xi * y_eta) / det
+    gyy = (x_xi ** 2 + y_xi ** 2) / det
+    return x, y, det, gxx, gxy, gyy
+
+
+def element_stiffness_quad(p: int, X4, Y4):
+    """A_e[i,j] = sum_q w_q (grad phi_j . grad phi_i detJ)(q), local node (a,b) -> b*(p+1)+a, written
+    as D^T (geometric factors) D."""
+    _, w, D = gll(p)
+    _, _, _, gxx, gxy, gyy = quad_geometry(p, X4, Y4)
+    I = np.eye(p + 1)
+    Dxi, Deta = np.kron(I, D), np.kron(D, I)            # d/dxi acts on a, d/deta on b
+    W2 = np.outer(w, w)                                 # [b,a]
+    Gxx, Gxy, Gyy = (np.diag((W2 * g).reshape(-1)) for g in (gxx, gxy, gyy))
+    return Dxi.T @ Gxx @ Dxi + Dxi.T @ Gxy @ Deta + Deta.T @ Gxy @ Dxi + Deta.T @ Gyy @ Deta
+
+
+def region_operators_quads(p: int, VX, VY):
+    """Stiffness A (sparse), geometric lumped mass m[j,i] = sum_e w_a w_b detJ and geometric edge weights
+    s[side] = sum_e w_a |edge_e|/2 of the region whose (ey+1) x (ex+1) vertices are VX, VY — the general-geometry
+    counterpart of _region_operators."""
+    VX, VY = np.asarray(VX, dtype=float), np.asarray(VY, dtype=float)
+    ey, ex = VX.shape[0] - 1, VX.shape[1] - 1
+    _, w, _ = gll(p)
+    npx, npy = ex * p + 1, ey * p + 1
+    rows, cols, vals = [], [], []
+    m = np.zeros((npy, npx))
+    la = np.arange(p + 1)
+    for fy in range(ey):
+        for fx in range(ex):
+            X4, Y4 = VX[fy:fy + 2, fx:fx + 2], VY[fy:fy + 2, fx:fx + 2]
+            Ae = element_stiffness_quad(p, X4, Y4)
+            det = quad_geometry(p, X4, Y4)[2]
+            gi = ((fy * p + la)[:, None] * npx + (fx * p + la)[None, :]).reshape(-1)
+            rows.append(np.repeat(gi, (p + 1) ** 2))
+            cols.append(np.tile(gi, (p + 1) ** 2))
+            vals.append(Ae.reshape(-1))
+            m[fy * p:fy * p + p + 1, fx * p:fx * p + p + 1] += np.outer(w, w) * det
+    A = sp.csr_matrix((np.concatenate(vals), (np.concatenate(rows), np.concatenate(cols))),
+                      shape=(npx * npy, npx * npy))
+    A.sum_duplicates()
+
+    def side_weights(PX, PY):                           # polyline of vertices -> assembled w_a * |edge|/2
+        out = np.zeros((len(PX) - 1) * p + 1)
+        for e in range(len(PX) - 1):
+            half = 0.5 * math.hypot(PX[e + 1] - PX[e], PY[e + 1] - PY[e])
+            out[e * p:e * p + p + 1] += half * w
+        return out
+    s = [side_weights(VX[:, 0], VY[:, 0]), side_weights(VX[:, -1], VY[:, -1]),
+         side_weights(VX[0, :], VY[0, :]), side_weights(VX[-1, :], VY[-1, :])]
+    return A, m, s
+
+
+def node_coords_quads(p: int, VX, VY):
+    """(npy, npx) coordinates of the global GLL nodes of the mapped mesh."""
+    VX, VY = np.asarray(VX, dtype=float), np.asarray(VY, dtype=float)
+    ey, ex = VX.shape[0] - 1, VX.shape[1] - 1
+    X = np.zeros((ey * p + 1, ex * p + 1))
+    Y = np.zeros_like(X)
+    for fy in range(ey):
+        for fx in range(ex):
+            x, y = quad_geometry(p, VX[fy:fy + 2, fx:fx + 2], VY[fy:fy + 2, fx:fx + 2])[:2]
+            X[fy * p:fy * p + p + 1, fx * p:fx * p + p + 1] = x
+            Y[fy * p:fy * p + p + 1, fx * p:fx * p + p + 1] = y
+    return X, Y
+
+
+def choose_nt_quads(p, VX, VY, c_nodes, omega, cfl_frac):
+    """N_t for general quads (reading R24, the element-wise form of R9).  lmax(M^-1 A) <= max_e lmax(M_e^-1 A_e)
+    (A and M are sums of element matrices), and on one element, with Lhat = Lambda_p / 4 the largest
+    eigenvalue of the reference pencil (K, W) on [-1,1]:
+        u^T A_e u <= sum_q w_q [(gxx+|gxy|) u_xi^2 + (gyy+|gxy|) u_eta^2] <= Lhat (Gx + Gy) sum_q w_q u_q^2,
+        u^T M_e u >= mu sum_q w_q u_q^2,   Gx = max_q (gxx+|gxy|), Gy = max_q (gyy+|gxy|), mu = min_q detJ/c^2,
+    so lmax <= max_e Lhat (Gx+Gy)/mu.  On hx-by-hy rectangles this is c_max^2 Lambda_p (1/hx^2+1/hy^2): choose_nt."""
+    VX, VY = np.asarray(VX, dtype=float), np.asarray(VY, dtype=float)
+    ey, ex = VX.shape[0] - 1, VX.shape[1] - 1
+    c = np.asarray(c_nodes, dtype=float)
+    lhat = lambda_p(p) / 4.0
+    lmax = 0.0
+    for fy in range(ey):
+        for fx in range(ex):
+            _, _, det, gxx, gxy, gyy = quad_geometry(p, VX[fy:fy + 2, fx:fx + 2], VY[fy:fy + 2, fx:fx + 2])
+            ce = c[fy * p:fy * p + p + 1, fx * p:fx * p + p + 1]
+            Gx, Gy = np.max(gxx + np.abs(gxy)), np.max(gyy + np.abs(gxy))
+            mu = np.min(det / ce ** 2)
+            lmax = max(lmax, lhat * (Gx + Gy) / mu)
+    dt_stab = 2.0 / math.sqrt(lmax)
+    T = 2.0 * math.pi / omega
+    return max(4, int(math.ceil(T / (cfl_frac * dt_stab) * (1.0 - 1e-12))))

@@ -62,6 +62,8 @@ class HzInputs:
     warm_start: bool = True
     seed: int = 0
     meta: dict = field(default_factory=dict)
+    vx: np.ndarray | None = None   # general quads (F3): (ny+1, nx+1) vertex coordinates; None = uniform rectangles
+    vy: np.ndarray | None = None
 
     @property
     def npx(self):
@@ -121,11 +123,42 @@ def gaussian_sources(X, Y, pts, sigma: float):
     return f
 
 
+def distorted_vertices(nx: int, ny: int, rng, amp: float, x0=0.0, y0=0.0, x1=1.0, y1=1.0):
+    """Vertices of a logically rectangular mesh of straight-sided convex quads: the uniform grid with every
+    INTERIOR vertex moved by amp * (hx, hy) * U(-1,1)^2 (amp <= 0.25 keeps all elements convex); the boundary
+    vertices stay, so the domain is still the rectangle."""
+    gx, gy = np.linspace(x0, x1, nx + 1), np.linspace(y0, y1, ny + 1)
+    VX, VY = np.meshgrid(gx, gy, indexing="xy")
+    VX, VY = VX.copy(), VY.copy()
+    hx, hy = (x1 - x0) / nx, (y1 - y0) / ny
+    VX[1:-1, 1:-1] += amp * hx * rng.uniform(-1, 1, size=(ny - 1, nx - 1))
+    VY[1:-1, 1:-1] += amp * hy * rng.uniform(-1, 1, size=(ny - 1, nx - 1))
+    return VX, VY
+
+
+def mapped_node_coords(p: int, VX: np.ndarray, VY: np.ndarray):
+    """(npy, npx) positions of the GLL nodes of the bilinearly mapped elements (node placement only)."""
+    xi = np.asarray(_GLL_CLOSED_FORM[p])
+    ny, nx = VX.shape[0] - 1, VX.shape[1] - 1
+    XI, ETA = np.meshgrid(xi, xi, indexing="xy")
+    X = np.zeros((ny * p + 1, nx * p + 1))
+    Y = np.zeros_like(X)
+    for fy in range(ny):
+        for fx in range(nx):
+            for Z, V in ((X, VX), (Y, VY)):
+                Z[fy * p:fy * p + p + 1, fx * p:fx * p + p + 1] = (
+                    (1 - XI) * (1 - ETA) * V[fy, fx] + (1 + XI) * (1 - ETA) * V[fy, fx + 1]
+                    + (1 - XI) * (1 + ETA) * V[fy + 1, fx] + (1 + XI) * (1 + ETA) * V[fy + 1, fx + 1]) / 4.0
+    return X, Y
+
+
 def make_config(cfg: int, n: int | None = None, p: int | None = None, sub_elems: int | None = None,
-                seed: int | None = None) -> HzInputs:
+                seed: int | None = None, distort: float = 0.0) -> HzInputs:
     """Config `cfg` in 1..5 of BASELINE.json.  `n` (elements per side), `p` and `sub_elems`
     (elements per subdomain side) override the full-size values to get a SMALLER problem of
-    the same structure for the parity tests; the full-size values are the defaults."""
+    the same structure for the parity tests; the full-size values are the defaults.
+    `distort` > 0: the same config on general convex quads: interior vertices moved by
+    distort * h * U(-1,1), c and f sampled at the mapped nodes."""
     defaults = {1: (16, 2, 8, 8.0), 2: (128, 3, 8, 10.0), 3: (512, 3, 8, 10.0),
                 4: (1024, 3, 32, 10.0), 5: (2048, 3, 8, 10.0)}
     n0, p0, s0, ppw = defaults[cfg]
@@ -141,6 +174,11 @@ def make_config(cfg: int, n: int | None = None, p: int | None = None, sub_elems:
     h = 1.0 / n
     omega = omega_for_ppw(n, p, ppw)
     meta = {"ppw": ppw}
+    VX = VY = None
+    if distort > 0.0:
+        VX, VY = distorted_vertices(n, n, np.random.default_rng(seed + 7919), distort)
+        X, Y = mapped_node_coords(p, VX, VY)
+        meta["distort"] = distort
     if cfg == 1:
         c = np.ones_like(X)
         pts = draw_source_points(rng, 1)
@@ -156,10 +194,11 @@ def make_config(cfg: int, n: int | None = None, p: int | None = None, sub_elems:
         sigma = 1.28 * h
     f = gaussian_sources(X, Y, pts, sigma)
     meta.update(sources=pts, sigma=sigma)
-    return HzInputs(name=f"cfg{cfg}_n{n}_p{p}_s{s}", nx=n, ny=n, p=p, x0=0.0, y0=0.0, x1=1.0, y1=1.0,
+    return HzInputs(name=f"cfg{cfg}_n{n}_p{p}_s{s}" + ("_quads" if VX is not None else ""), nx=n, ny=n, p=p,
+                    x0=0.0, y0=0.0, x1=1.0, y1=1.0,
                     omega=omega, c_nodes=np.ascontiguousarray(c, dtype=np.float64),
                     f_re=np.ascontiguousarray(f, dtype=np.float64), f_im=None,
-                    sx=n // s, sy=n // s, seed=seed, meta=meta)
+                    sx=n // s, sy=n // s, seed=seed, meta=meta, vx=VX, vy=VY)
 
 
 def random_lambda(rng, n_sub: int, edge_nodes: int):
