@@ -43,11 +43,14 @@ def parse_args():
     ap.add_argument("--k", type=int, default=0, help="DOFs per thread (0 = auto, 1 = one DOF per thread)")
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--no-extras", action="store_true", help="skip the secondary measurements")
+    ap.add_argument("--distort", type=float, default=0.0,
+                    help="> 0: the same config on general convex quads (interior vertices moved by distort*h; SURVEY F3)")
     return ap.parse_args()
 
 
 def workload_name(inp, prec):
-    return (f"config{inp.name[3]}: {inp.nx}x{inp.ny} quads p={inp.p}, {inp.sx}x{inp.sy} subdomains of "
+    geo = f"general convex quads (vertices distorted by {inp.meta['distort']} h)" if inp.vx is not None else "uniform quads"
+    return (f"config{inp.name[3]}: {inp.nx}x{inp.ny} {geo} p={inp.p}, {inp.sx}x{inp.sy} subdomains of "
             f"{inp.nx // inp.sx}x{inp.ny // inp.sy} elements, {prec}, n_wh={N_WH}, warm start, relax 0.5")
 
 
@@ -61,9 +64,20 @@ class OracleSample:
     def __init__(self, inp):
         from oracle import hz_oracle as O
         self.O = O
-        pr = O.Problem(inp.nx, inp.ny, inp.p, inp.x0, inp.y0, inp.x1, inp.y1, inp.c_nodes, inp.omega,
-                       inp.f_re.astype(complex))
-        self.st = O.ddm_setup(pr, inp.sx, inp.sy, inp.cfl_frac)
+        if inp.vx is not None and inp.sx * inp.sy > 16:
+            # general quads: the oracle assembles every element matrix in Python, so the sample is set up on the
+            # lower-left 4x4 subdomains of the mesh only (same elements, same block shape, same N_t rule per element)
+            ex, ey, p = inp.nx // inp.sx, inp.ny // inp.sy, inp.p
+            sx, sy = min(4, inp.sx), min(4, inp.sy)
+            nx, ny = sx * ex, sy * ey
+            pr = O.Problem(nx, ny, p, 0, 0, 1, 1, inp.c_nodes[:ny * p + 1, :nx * p + 1], inp.omega,
+                           inp.f_re[:ny * p + 1, :nx * p + 1].astype(complex), vx=inp.vx[:ny + 1, :nx + 1],
+                           vy=inp.vy[:ny + 1, :nx + 1])
+            self.st = O.ddm_setup(pr, sx, sy, inp.cfl_frac)   # N_t is that of the cropped mesh (fewer elements in the max)
+        else:
+            pr = O.Problem(inp.nx, inp.ny, inp.p, inp.x0, inp.y0, inp.x1, inp.y1, inp.c_nodes, inp.omega,
+                           inp.f_re.astype(complex), vx=inp.vx, vy=inp.vy)
+            self.st = O.ddm_setup(pr, inp.sx, inp.sy, inp.cfl_frac)
         self.n_sub = len(self.st.subs)
         self.dofs = self.st.subs[0].npx * self.st.subs[0].npy
         self.n_t = self.st.tab.n_t
@@ -84,7 +98,7 @@ def run_reference(args):
     if rank != 0:
         return
     from paper_2606_21695_b200.inputs import make_config
-    inp = make_config(args.config, n=args.n)
+    inp = make_config(args.config, n=args.n, distort=args.distort)
     smp = OracleSample(inp)
     t, _ = smp.run(1)
     per_step = max(1, min(smp.n_sub, int(1.0 / max(t, 1e-4))))   # about 1 s of oracle work per step
@@ -157,9 +171,25 @@ class ClockSampler:
 # ---------------------------------------------------------------------------------------------------
 # the CUDA arm
 # ---------------------------------------------------------------------------------------------------
-def flops_per_dof_step(p):
-    """Necessary FMAs of the assembled line-stencil formulation: 2(p+2) for A p + 5 updates."""
+def flops_per_dof_step(p, quads=False):
+    """Necessary FMAs of the assembled line-stencil formulation: 2(p+2) for A p + 5 updates.
+    General quads: (p+1)^2 points per element x (2(p+1) gradient + 4 geometric factors + 2(p+1) D^T) over the
+    p^2 DOFs an element adds, + 5 updates."""
+    if quads:
+        return 2.0 * ((p + 1) ** 2 * (4 * (p + 1) + 4) / float(p * p) + 5)
     return 2.0 * (2 * (p + 2) + 5)
+
+
+def kernel_name(pinfo, quads=False):
+    if quads:
+        return "k_sweep_quad"
+    if pinfo.cluster_size > 1:
+        return "k_sweep_cl"
+    if pinfo.dofs_per_thread == 1:
+        return "k_sweep_dof"
+    if pinfo.dofs_per_thread == -1:
+        return "k_sweep_stream"
+    return "k_sweep_ws" if pinfo.tile_mx == pinfo.tile_my and not os.environ.get("HZ_DISABLE_WS") else "k_sweep_tile"
 
 
 def job_value(units_this_rank, ms_this_rank, world, device):
@@ -213,7 +243,8 @@ def run_b200(args):
 
     prec = hz.HZ_F32 if args.prec == "f32" else hz.HZ_F64
     tdt = torch.float32 if prec == hz.HZ_F32 else torch.float64
-    inp = make_config(args.config, n=args.n)
+    inp = make_config(args.config, n=args.n, distort=args.distort)
+    quads = inp.vx is not None
     ctx, pinfo = hz.setup_from_inputs(inp, prec, args.k)
     stream = torch.cuda.current_stream().cuda_stream
     flush = torch.zeros(64 * 1024 * 1024, dtype=torch.float32, device="cuda")   # 256 MB > 126 MB L2
@@ -263,7 +294,7 @@ def run_b200(args):
     # ---- roofline of the dominant kernel (the sweep), live numbers ----
     sweep_ms = float(sum(swp)) / args.steps
     units_per_launch = units / args.steps
-    fl = flops_per_dof_step(inp.p)
+    fl = flops_per_dof_step(inp.p, quads)
     sm_max = (clocks or {}).get("sm_max_mhz") or 1965.0
     lanes = FP32_LANES if prec == hz.HZ_F32 else FP32_LANES // 2
     peak_tf = SMS * lanes * 2 * sm_max * 1e6 / 1e12
@@ -272,13 +303,13 @@ def run_b200(args):
     tpath = os.path.join(ROOT, "profiles", "sweep_traffic.json")
     if os.path.exists(tpath):
         with open(tpath) as fh:
-            traffic = json.load(fh).get(f"config{args.config}_{args.prec}")
+            traffic = json.load(fh).get(f"config{args.config}_{args.prec}" + ("_quads" if quads else ""))
     try:
         probe_tf = hz.hz_peak_probe(0 if prec == hz.HZ_F32 else 1, stream)
     except Exception:
         probe_tf = None
     roofline = {"bound": "alu", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved_tf / peak_tf,
-                "traffic": traffic, "kernel": "k_sweep_tile" if pinfo.dofs_per_thread > 1 else "k_sweep_dof",
+                "traffic": traffic, "kernel": kernel_name(pinfo, quads),
                 "peak_source": f"derived: {SMS} SMs x {lanes} FMA lanes x 2 x {sm_max:.0f} MHz (guide unit counts, "
                                "nvidia-smi max clock); MEASURED_PEAKS.json has no CUDA-core entry",
                 "peak_measured_fma_probe": probe_tf, "frac_of_probe": (achieved_tf / probe_tf) if probe_tf else None,

@@ -64,6 +64,24 @@ hz_status hz_mesh_setup(hz_ctx **out, int nx, int ny, double x0, double y0, doub
                         const double *c_nodes, double omega, const double *f_re, const double *f_im,
                         const double *bc_lambda);
 
+/* ---------------------------------------------------------------------------------------------
+ * hz_mesh_setup_quads — the same problem on a logically rectangular mesh of GENERAL straight-sided convex
+ * quadrilaterals ("quadrilateral ... elements"; gradient through D, geometric
+ * factors at the quadrature points, D^T).  Element (gx,gy) is the bilinear image of
+ * the reference square with the vertices (vx,vy)[gy..gy+1][gx..gx+1].
+ *
+ *   vx, vy     HOST, (ny+1)*(nx+1) doubles each, row-major (x index fastest): vertex coordinates.  Every element
+ *              must be convex and counter-clockwise (detJ > 0 at all its GLL points), else HZ_EINVAL.
+ *   c_nodes, f_re, f_im, bc_lambda, omega, p   as in hz_mesh_setup, sampled at the MAPPED GLL nodes.
+ * hz_partition on such a context has one kernel variant (one thread per element, the element's (p+1)^2 nodes in
+ * registers; pass dofs_per_thread = 0; at most 1024 elements per subdomain) and takes N_t from the element-wise
+ * bound of reading R24; hz_minres_cycle returns HZ_EUNSUPPORTED.  Everything else (hz_ddm_solve,
+ * hz_ddm_solve_gmres, hz_residual, state get/set) works as on a uniform mesh.
+ * ------------------------------------------------------------------------------------------- */
+hz_status hz_mesh_setup_quads(hz_ctx **out, int nx, int ny, int p, const double *vx, const double *vy,
+                              const double *c_nodes, double omega, const double *f_re, const double *f_im,
+                              const double *bc_lambda);
+
 /* Replace the source f (HOST arrays as in hz_mesh_setup; f_im may be NULL).  After hz_partition
  * the per-subdomain load vectors are rebuilt on the device ("Assemble b from f"). */
 hz_status hz_set_source(hz_ctx *ctx, const double *f_re, const double *f_im);
@@ -77,7 +95,8 @@ typedef struct {
   int edge_stride;       /* E = max of the two: stride of one side in lambda arrays */
   int threads_per_block; /* block size of the sweep kernel */
   int blocks;            /* = sx*sy subdomains = thread blocks of one sweep launch */
-  int dofs_per_thread;   /* 1, or (mx*p)*(my*p) of the register-blocked variant, or -1 (streamed) */
+  int dofs_per_thread;   /* 1, or (mx*p)*(my*p) of the register-blocked variant, or -1 (streamed); general quads:
+                            (p+1)^2 = the nodes of one element, shared ones replicated */
   int tile_mx, tile_my;  /* elements per thread tile (0 for the one-DOF-per-thread variant) */
   int cluster_size;      /* thread blocks (CTAs of one cluster, on as many SMs) per subdomain; 1 unless the state of
                             a subdomain needs the registers of several SMs (hz_sweep_cl.cuh) */

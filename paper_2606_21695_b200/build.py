@@ -15,7 +15,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhz.so")
-SOURCES = ["hz_api.cu", "hz_sweep_f32.cu", "hz_sweep_f64.cu"]
+SOURCES = ["hz_api.cu", "hz_sweep_f32.cu", "hz_sweep_f64.cu", "hz_sweep_quad.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "--fmad=true"]
 

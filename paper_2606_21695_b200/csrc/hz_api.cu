@@ -13,6 +13,7 @@
 #include "hz_aux.cuh"
 #include "hz_internal.h"
 #include "hz_minres.cuh"
+#include "hz_quad.cuh"
 
 using namespace hz;
 
@@ -135,6 +136,13 @@ struct hz_ctx {
   double x0 = 0, y0 = 0, x1 = 0, y1 = 0, omega = 0, hx = 0, hy = 0, c_max = 0;
   Gll gll;
   double *d_c = nullptr, *d_fre = nullptr, *d_fim = nullptr, *d_bc = nullptr;
+  // general quadrilaterals (hz_mesh_setup_quads): vertex coordinates, the element-wise bound on lmax(M^-1 A)
+  // (reading R24), the reference data and, per partition, the geometric factors of every quadrature point
+  bool general = false;
+  double *d_vx = nullptr, *d_vy = nullptr;
+  double lmax_quads = 0;
+  RefQ refq{};
+  void *d_G = nullptr;
   // partition
   bool part = false;
   int sx = 0, sy = 0, ex = 0, ey = 0, L = 0, E = 0, prec = 0;
@@ -195,6 +203,7 @@ void free_partition(hz_ctx *c) {
   if (c->d_kry) { cudaFree(c->d_kry); c->d_kry = nullptr; c->kry_vecs = 0; }
   if (c->d_kpart) { cudaFree(c->d_kpart); c->d_kpart = nullptr; }
   if (c->g_exec) { cudaGraphExecDestroy(c->g_exec); c->g_exec = nullptr; }
+  if (c->d_G) { cudaFree(c->d_G); c->d_G = nullptr; }
   void **ptrs[] = {&c->d_tab, &c->d_gamma, &c->d_alpha, &c->d_bbf_re, &c->d_bbf_im, &c->d_lam,
                    &c->d_g, &c->d_k2, &c->d_bs, &c->d_bandx, &c->d_bandy, &c->d_scr, (void **)&c->d_wxl, (void **)&c->d_wyl,
                    (void **)&c->d_part, (void **)&c->d_red, (void **)&c->d_ures};
@@ -216,6 +225,21 @@ hz_status run_build(hz_ctx *ctx, int only_source, cudaStream_t st) {
   const long long total = (long long)ctx->L * ctx->lay.lnx * ctx->lay.lny;
   const int bs = 256;
   const unsigned nb = (unsigned)((total + bs - 1) / bs);
+  if (ctx->general) {
+    k_build_quad<real><<<nb, bs, 0, st>>>(make_geo(ctx), ctx->lay, ctx->refq, ctx->d_vx, ctx->d_vy, ctx->d_c, ctx->d_fre,
+                                          ctx->d_fim, ctx->d_bc, (real *)ctx->d_gamma, (real *)ctx->d_alpha,
+                                          (real *)ctx->d_bbf_re, (real *)ctx->d_bbf_im, (real *)ctx->d_k2,
+                                          (real *)ctx->d_bs, only_source);
+    HZ_CUDA(cudaGetLastError());
+    if (!only_source) {
+      const int NQ = (ctx->p + 1) * (ctx->p + 1);
+      const long long tq = (long long)ctx->L * ctx->ex * ctx->ey * NQ;
+      k_build_quad_metric<real><<<(unsigned)((tq + bs - 1) / bs), bs, 0, st>>>(make_geo(ctx), ctx->refq, ctx->d_vx, ctx->d_vy,
+                                                                               ctx->launch.threads, (real *)ctx->d_G);
+      HZ_CUDA(cudaGetLastError());
+    }
+    return HZ_OK;
+  }
   k_build<real><<<nb, bs, 0, st>>>(make_geo(ctx), ctx->lay, ctx->d_c, ctx->d_fre, ctx->d_fim, ctx->d_bc, ctx->d_wxl,
                                    ctx->d_wyl, (real *)ctx->d_gamma, (real *)ctx->d_alpha, (real *)ctx->d_bbf_re,
                                    (real *)ctx->d_bbf_im, (real *)ctx->d_k2, (real *)ctx->d_bs, only_source);
@@ -285,7 +309,22 @@ SweepArgs<real> make_args(const hz_ctx *c, const hz_solve_opts *o) {
   return a;
 }
 
+template <typename real>
+QuadArgs<real> make_quad_args(const hz_ctx *c) {
+  QuadArgs<real> q{};
+  q.G = (const real *)c->d_G;
+  q.nep = c->launch.threads;
+  for (int a = 0; a <= c->p; ++a)
+    for (int b = 0; b <= c->p; ++b) q.D[a][b] = (real)c->gll.D[a][b];
+  return q;
+}
+
 cudaError_t launch_sweep(const hz_ctx *c, const hz_solve_opts *o, cudaStream_t st) {
+  if (c->lay.variant == 3) {
+    if (c->prec == HZ_F32)
+      return launch_sweep_quad_f32(make_args<float>(c, o), make_quad_args<float>(c), &c->tc32, c->p, c->launch, st);
+    return launch_sweep_quad_f64(make_args<double>(c, o), make_quad_args<double>(c), &c->tc64, c->p, c->launch, st);
+  }
   if (c->prec == HZ_F32) {
     SweepArgs<float> a = make_args<float>(c, o);
     if (c->lay.variant == 2) return launch_sweep_stream_f32(a, (float *)c->d_scr, c->p, c->launch, st);
@@ -345,7 +384,14 @@ hz_status residual_impl(hz_ctx *ctx, const void *u_dev, int u_prec, double *rel,
     for (int b = 0; b <= ctx->p; ++b) ref.K[a][b] = ctx->gll.K[a][b];
   }
   Geo g = make_geo(ctx);
-  if (u_prec == HZ_F32)
+  if (ctx->general) {
+    if (u_prec == HZ_F32)
+      k_residual_quad<float><<<nb, bs, 0, st>>>(g, ctx->refq, ctx->d_vx, ctx->d_vy, ctx->d_c, ctx->d_fre, ctx->d_fim,
+                                                ctx->d_bc, (const float *)u_dev, ctx->d_part);
+    else
+      k_residual_quad<double><<<nb, bs, 0, st>>>(g, ctx->refq, ctx->d_vx, ctx->d_vy, ctx->d_c, ctx->d_fre, ctx->d_fim,
+                                                 ctx->d_bc, (const double *)u_dev, ctx->d_part);
+  } else if (u_prec == HZ_F32)
     k_residual<float><<<nb, bs, 0, st>>>(g, ref, ctx->d_c, ctx->d_fre, ctx->d_fim, ctx->d_bc, (const float *)u_dev, ctx->d_part);
   else
     k_residual<double><<<nb, bs, 0, st>>>(g, ref, ctx->d_c, ctx->d_fre, ctx->d_fim, ctx->d_bc, (const double *)u_dev, ctx->d_part);
@@ -409,6 +455,59 @@ hz_status hz_mesh_setup(hz_ctx **out, int nx, int ny, double x0, double y0, doub
   return HZ_OK;
 }
 
+hz_status hz_mesh_setup_quads(hz_ctx **out, int nx, int ny, int p, const double *vx, const double *vy,
+                              const double *c_nodes, double omega, const double *f_re, const double *f_im,
+                              const double *bc_lambda) {
+  if (!vx || !vy) return fail(nullptr, HZ_EINVAL, "hz_mesh_setup_quads: NULL vertex arrays");
+  if (nx < 1 || ny < 1 || p < 1 || p > kMaxP || !out || !c_nodes)
+    return hz_mesh_setup(out, nx, ny, 0.0, 0.0, 1.0, 1.0, p, c_nodes, omega, f_re, f_im, bc_lambda);  // its messages
+  // element-wise bound on lmax(M^-1 A) (reading R24):  Lhat (Gx + Gy) / mu  with  Lhat = Lambda_p / 4,
+  // Gx = max_q (gxx + |gxy|), Gy = max_q (gyy + |gxy|), mu = min_q detJ / c^2 over the element's GLL points
+  Gll gl;
+  make_gll(p, &gl);
+  const int npx = nx * p + 1;
+  double lmax = 0.0;
+  for (int gy = 0; gy < ny; ++gy)
+    for (int gx = 0; gx < nx; ++gx) {
+      double X[4], Y[4];
+      quad_vertices(vx, vy, nx, gx, gy, X, Y);
+      double Gx = 0.0, Gy = 0.0, mu = INFINITY;
+      for (int b = 0; b <= p; ++b)
+        for (int a = 0; a <= p; ++a) {
+          const QuadPt q = quad_point(X, Y, gl.xi[a], gl.xi[b]);
+          if (!(q.det > 0.0) || !std::isfinite(q.det))
+            return fail(nullptr, HZ_EINVAL, "hz_mesh_setup_quads: an element is not convex / not counter-clockwise");
+          const double cc = c_nodes[(size_t)(gy * p + b) * npx + gx * p + a];
+          Gx = std::fmax(Gx, q.gxx + std::fabs(q.gxy));
+          Gy = std::fmax(Gy, q.gyy + std::fabs(q.gxy));
+          mu = std::fmin(mu, q.det / (cc * cc));
+        }
+      lmax = std::fmax(lmax, 0.25 * gl.lambda_p * (Gx + Gy) / mu);
+    }
+  hz_ctx *c = nullptr;
+  // hx = hy = 1 in the rectangular fields: unused by the general-geometry kernels
+  hz_status stt = hz_mesh_setup(&c, nx, ny, 0.0, 0.0, (double)nx, (double)ny, p, c_nodes, omega, f_re, f_im, bc_lambda);
+  if (stt != HZ_OK) return stt;
+  c->general = true;
+  c->lmax_quads = lmax;
+  for (int a = 0; a <= p; ++a) {
+    c->refq.xi[a] = gl.xi[a]; c->refq.w[a] = gl.w[a];
+    for (int b = 0; b <= p; ++b) c->refq.D[a][b] = gl.D[a][b];
+  }
+  const size_t nv = (size_t)(nx + 1) * (ny + 1);
+  cudaError_t e = dmalloc(&c->d_vx, nv);
+  if (e == cudaSuccess) e = dmalloc(&c->d_vy, nv);
+  if (e == cudaSuccess) e = cudaMemcpy(c->d_vx, vx, nv * sizeof(double), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(c->d_vy, vy, nv * sizeof(double), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) {
+    hz_status st2 = cuda_fail(nullptr, e, "hz_mesh_setup_quads (device allocation / copy)");
+    hz_destroy(c);
+    return st2;
+  }
+  *out = c;
+  return HZ_OK;
+}
+
 hz_status hz_set_source(hz_ctx *ctx, const double *f_re, const double *f_im) {
   if (!ctx) return HZ_EINVAL;
   if (!f_re) return fail(ctx, HZ_EINVAL, "hz_set_source: NULL f_re");
@@ -451,7 +550,8 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
   const size_t rs = prec == HZ_F32 ? 4 : 8;
 
   // --- time step (reading R9): dt_stab = 2 / sqrt(c_max^2 Lambda_p (1/hx^2 + 1/hy^2)) ---
-  const double lmax = ctx->c_max * ctx->c_max * ctx->gll.lambda_p * (1.0 / (ctx->hx * ctx->hx) + 1.0 / (ctx->hy * ctx->hy));
+  const double lmax = ctx->general ? ctx->lmax_quads  // reading R24: element-wise form of the same bound
+                                   : ctx->c_max * ctx->c_max * ctx->gll.lambda_p * (1.0 / (ctx->hx * ctx->hx) + 1.0 / (ctx->hy * ctx->hy));
   const double dt_stab = 2.0 / std::sqrt(lmax);
   const double T = 2.0 * M_PI / ctx->omega;
   int n_t = (int)std::ceil(T / (cfl_frac * dt_stab) * (1.0 - 1e-12));
@@ -525,7 +625,26 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
   };
   const bool complex_f = ctx->d_fim != nullptr;
   bool streamed = dofs_per_thread == -1;
-  if (streamed) {
+  bool quad = false;
+  if (ctx->general) {  // one thread per element, the element's nodes in registers (hz_sweep_quad.cuh)
+    if (dofs_per_thread != 0)
+      return fail(ctx, HZ_EUNSUPPORTED, "hz_partition: general quadrilaterals have one variant; pass dofs_per_thread = 0");
+    const int ne = ctx->ex * ctx->ey;
+    if (ne > 1024) return fail(ctx, HZ_EUNSUPPORTED, "hz_partition: general quadrilaterals need <= 1024 elements per subdomain");
+    const int n1 = P + 1, v16 = (int)(16 / rs);
+    const int ch = roundup(n1, v16);
+    int rsw = 4 * ch;
+    if ((rsw / v16) % 2 == 0) rsw += v16;
+    int cst = n1 * (4 * n1 + roundup(3 * n1, v16));
+    if ((cst / v16) % 2 == 0) cst += v16;
+    const int nthr = roundup(ne, 32);
+    const size_t sm = (2 * (size_t)(nthr + 33) * rsw + (size_t)nthr * cst) * rs;
+    if (sm > smem_cap) return fail(ctx, HZ_EUNSUPPORTED, "hz_partition: general quadrilaterals: the subdomain does not fit the shared memory of one SM");
+    lay.variant = 3; lay.TX = lay.TY = P; lay.ntx = ctx->ex; lay.nty = ctx->ey; lay.NT = nthr; lay.NS = roundup(N, 32);
+    ctx->lay = lay; ctx->mx = ctx->my = 1; ctx->csm = 1; ctx->ws = 0; ctx->cl = 1;
+    ctx->launch.blocks = ctx->L; ctx->launch.threads = nthr; ctx->launch.smem = sm;
+    quad = true;
+  } else if (streamed) {
   } else if (dofs_per_thread == 1 || (dofs_per_thread == 0 && complex_f)) {
     if (N > 1024) {
       if (dofs_per_thread == 1) return fail(ctx, HZ_EUNSUPPORTED, "hz_partition: one DOF per thread needs <= 1024 DOFs per subdomain");
@@ -569,7 +688,8 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
       return fail(ctx, HZ_EUNSUPPORTED, "hz_partition: complex f is only supported by the one-DOF-per-thread variant");
     if (best < 0 && N > 1024) streamed = true;  // state does not fit on chip: streamed fallback
   }
-  if (best >= 0) {
+  if (quad) {
+  } else if (best >= 0) {
     ctx->lay = blay; ctx->launch = bl;
     ctx->mx = tiles[best].mx; ctx->my = tiles[best].my; ctx->csm = tiles[best].csm; ctx->ws = tiles[best].ws;
     ctx->cl = tiles[best].cl;
@@ -621,6 +741,7 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
   HZ_CUDA(alloc0(&ctx->d_bbf_re, LS * rs));
   if (need_im) HZ_CUDA(alloc0(&ctx->d_bbf_im, LS * rs));
   if (ctx->lay.variant == 2) HZ_CUDA(alloc0(&ctx->d_scr, 7 * LS * rs));
+  if (ctx->lay.variant == 3) HZ_CUDA(alloc0(&ctx->d_G, (size_t)ctx->L * 3 * (P + 1) * (P + 1) * ctx->launch.threads * rs));
   HZ_CUDA(alloc0(&ctx->d_lam, (lam_n + 2 * LS) * rs));  // joint state: lambda | u_l, one flat array
   ctx->d_usub = (char *)ctx->d_lam + lam_n * rs;
   ctx->n_state = (long long)(lam_n + 2 * LS);
@@ -649,6 +770,7 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
     inf.n_t = n_t; inf.dofs_per_sub = N; inf.edge_nodes_x = lnx; inf.edge_nodes_y = lny; inf.edge_stride = ctx->E;
     inf.threads_per_block = ctx->launch.threads; inf.blocks = ctx->L;
     inf.dofs_per_thread = ctx->lay.variant == 0 ? 1 : (ctx->lay.variant == 2 ? -1 : ctx->lay.TX * ctx->lay.TY);
+    if (ctx->lay.variant == 3) inf.dofs_per_thread = (P + 1) * (P + 1);  // incl. the replicated shared nodes
     inf.tile_mx = ctx->mx; inf.tile_my = ctx->my; inf.cluster_size = ctx->lay.variant == 1 ? ctx->cl : 1;
     inf.dt = ctx->dt; inf.theta = ctx->theta; inf.sigma = ctx->sigma;
     inf.smem_bytes = ctx->launch.smem; inf.workspace_bytes = ws;
@@ -1113,7 +1235,7 @@ void hz_destroy(hz_ctx *ctx) {
   if (!ctx) return;
   free_partition(ctx);
   if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
-  double **ptrs[] = {&ctx->d_c, &ctx->d_fre, &ctx->d_fim, &ctx->d_bc};
+  double **ptrs[] = {&ctx->d_c, &ctx->d_fre, &ctx->d_fim, &ctx->d_bc, &ctx->d_vx, &ctx->d_vy};
   for (double **q : ptrs) { if (*q) cudaFree(*q); *q = nullptr; }
   delete ctx;
 }

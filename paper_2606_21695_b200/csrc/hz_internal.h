@@ -12,6 +12,7 @@ constexpr int kSideW = 0, kSideE = 1, kSideS = 2, kSideN = 3;
 // Where node (i,j) of a subdomain lives inside the subdomain's slot range [0, NS).
 //   variant 0 (one DOF per thread):   slot = j*lnx + i                       (thread = slot)
 //   variant 2 (streamed fallback):    slot = j*lnx + i
+//   variant 3 (general quads):        slot = j*lnx + i; ntx, nty = elements per subdomain side (one thread each)
 //   variant 1 (register-blocked):     thread tile (tx,ty) owns TX x TY nodes; node (a,b) of the tile of
 //                                     thread t = ty*ntx+tx lives at (b*TX+a)*NT + t, so that one node
 //                                     index across the block's threads is one coalesced line.
@@ -78,6 +79,14 @@ struct SweepArgs {
   real *lam_rw;
 };
 
+// Extra arguments of the general-quadrilateral sweep kernel (hz_sweep_quad.cuh)
+template <typename real>
+struct QuadArgs {
+  const real *G;                 // [L][3 (P+1)^2][nep]: w_a w_b {gxx, gxy, gyy} of every quadrature point
+  int nep;                       // element stride of G (threads per block)
+  real D[kMaxP + 1][kMaxP + 1];  // D[a][c] = l_c'(xi_a)
+};
+
 struct TileEntry {
   int p, mx, my, csm, maxt;  // csm: gamma / beta b in shared memory instead of registers
   int ws;                    // 1: warp-specialised kernel (hz_sweep_ws.cuh), needs mx == my
@@ -100,6 +109,10 @@ cudaError_t launch_sweep_tile_f64(const SweepArgs<double> &a, const TabC<double>
                                   cudaStream_t st);
 cudaError_t launch_sweep_stream_f32(const SweepArgs<float> &a, float *scr, int p, SweepLaunch cfg, cudaStream_t st);
 cudaError_t launch_sweep_stream_f64(const SweepArgs<double> &a, double *scr, int p, SweepLaunch cfg, cudaStream_t st);
+cudaError_t launch_sweep_quad_f32(const SweepArgs<float> &a, const QuadArgs<float> &q, const TabC<float> *tc, int p,
+                                  SweepLaunch cfg, cudaStream_t st);
+cudaError_t launch_sweep_quad_f64(const SweepArgs<double> &a, const QuadArgs<double> &q, const TabC<double> *tc, int p,
+                                  SweepLaunch cfg, cudaStream_t st);
 template <typename real>
 struct MinresArgs;
 cudaError_t launch_minres_f32(const MinresArgs<float> &a, int p, SweepLaunch cfg, cudaStream_t st);

@@ -21,7 +21,7 @@ HZ_TC_IMPEDANCE0 = 0
 STATUS_NAMES = {0: "HZ_OK", 1: "HZ_EINVAL", 2: "HZ_ENOMEM", 3: "HZ_ECUDA", 4: "HZ_EUNSUPPORTED", 5: "HZ_ESTATE"}
 
 # every symbol include/hz.h declares
-EXPORTS = ("hz_mesh_setup", "hz_set_source", "hz_partition", "hz_ddm_solve", "hz_ddm_solve_gmres", "hz_minres_cycle", "hz_residual",
+EXPORTS = ("hz_mesh_setup", "hz_mesh_setup_quads", "hz_set_source", "hz_partition", "hz_ddm_solve", "hz_ddm_solve_gmres", "hz_minres_cycle", "hz_residual",
            "hz_get_subdomain_state", "hz_set_subdomain_state", "hz_last_error", "hz_destroy", "hz_peak_probe")
 
 
@@ -85,6 +85,7 @@ def lib():
     vp, dp, ip = C.c_void_p, C.POINTER(C.c_double), C.c_int
     L.hz_mesh_setup.argtypes = [C.POINTER(vp), ip, ip, C.c_double, C.c_double, C.c_double, C.c_double, ip,
                                 vp, C.c_double, vp, vp, vp]
+    L.hz_mesh_setup_quads.argtypes = [C.POINTER(vp), ip, ip, ip, vp, vp, vp, C.c_double, vp, vp, vp]
     L.hz_set_source.argtypes = [vp, vp, vp]
     L.hz_partition.argtypes = [vp, ip, ip, ip, ip, ip, C.c_double, C.POINTER(hz_part_info)]
     L.hz_ddm_solve.argtypes = [vp, C.POINTER(hz_solve_opts), vp, C.POINTER(hz_solve_info), vp]
@@ -129,6 +130,22 @@ def hz_mesh_setup(nx, ny, x0, y0, x1, y1, p, c_nodes, omega, f_re, f_im=None, bc
     fi, _fi = _host_ptr(f_im)
     bc, _bc = _host_ptr(bc_lambda)
     st = L.hz_mesh_setup(C.byref(ctx), nx, ny, x0, y0, x1, y1, p, cp, omega, fr, fi, bc)
+    if st != HZ_OK:
+        raise HzError(st, L.hz_last_error(None).decode())
+    return ctx
+
+
+def hz_mesh_setup_quads(nx, ny, p, vx, vy, c_nodes, omega, f_re, f_im=None, bc_lambda=None):
+    """General straight-sided convex quads: vx, vy are (ny+1, nx+1) vertex arrays.  -> context handle."""
+    L = lib()
+    ctx = C.c_void_p()
+    xp, _x = _host_ptr(vx)
+    yp, _y = _host_ptr(vy)
+    cp, _c = _host_ptr(c_nodes)
+    fr, _fr = _host_ptr(f_re)
+    fi, _fi = _host_ptr(f_im)
+    bc, _bc = _host_ptr(bc_lambda)
+    st = L.hz_mesh_setup_quads(C.byref(ctx), nx, ny, p, xp, yp, cp, omega, fr, fi, bc)
     if st != HZ_OK:
         raise HzError(st, L.hz_last_error(None).decode())
     return ctx
@@ -223,8 +240,11 @@ def hz_peak_probe(kind, stream=None):
 
 def setup_from_inputs(inp, prec=HZ_F64, dofs_per_thread=0):
     """Convenience: hz_mesh_setup + hz_partition from an inputs.HzInputs.  -> (ctx, part_info)."""
-    ctx = hz_mesh_setup(inp.nx, inp.ny, inp.x0, inp.y0, inp.x1, inp.y1, inp.p, inp.c_nodes, inp.omega, inp.f_re,
-                        inp.f_im)
+    if getattr(inp, "vx", None) is not None:
+        ctx = hz_mesh_setup_quads(inp.nx, inp.ny, inp.p, inp.vx, inp.vy, inp.c_nodes, inp.omega, inp.f_re, inp.f_im)
+    else:
+        ctx = hz_mesh_setup(inp.nx, inp.ny, inp.x0, inp.y0, inp.x1, inp.y1, inp.p, inp.c_nodes, inp.omega, inp.f_re,
+                            inp.f_im)
     try:
         info = hz_partition(ctx, inp.sx, inp.sy, HZ_TC_IMPEDANCE0, prec, dofs_per_thread, inp.cfl_frac)
     except Exception:

@@ -20,8 +20,8 @@ from .inputs import make_config
 SMS, CLK = 148, 1.965e9
 
 
-def run(cfg, prec, k, n=None, p=None, s=None, nwh=5, reps=3):
-    inp = make_config(cfg, n=n, p=p, sub_elems=s)
+def run(cfg, prec, k, n=None, p=None, s=None, nwh=5, reps=3, distort=0.0):
+    inp = make_config(cfg, n=n, p=p, sub_elems=s, distort=distort)
     name = f"| {cfg} | {inp.nx} | {inp.p} | {inp.nx // inp.sx} | {'f32' if prec == hz.HZ_F32 else 'f64'} |"
     try:
         ctx, info = hz.setup_from_inputs(inp, prec, k)
@@ -33,6 +33,8 @@ def run(cfg, prec, k, n=None, p=None, s=None, nwh=5, reps=3):
         r = hz.hz_ddm_solve(ctx, reps, n_wh=nwh)
         rate = r.dof_timesteps / (r.sweep_ms_total * 1e-3)
         fl = 2 * (2 * (inp.p + 2) + 5)
+        if distort > 0:   # general quads: (p+1)^2 (4(p+1)+4) FMAs per element over p^2 DOFs, + 5 updates
+            fl = 2 * ((inp.p + 1) ** 2 * (4 * (inp.p + 1) + 4) / inp.p ** 2 + 5)
         peak = SMS * (128 if prec == hz.HZ_F32 else 64) * 2 * CLK
         print(f"{name} {info.dofs_per_thread} | {info.cluster_size} | {info.dofs_per_sub} | {info.blocks} | {info.threads_per_block} | "
               f"{info.smem_bytes} | {r.sweep_ms_total / reps:.3f} | {rate:.3e} | {rate * fl / peak:.3f} |", flush=True)
@@ -42,7 +44,7 @@ def run(cfg, prec, k, n=None, p=None, s=None, nwh=5, reps=3):
 
 def main():
     ap = argparse.ArgumentParser()
-    ap.add_argument("which", choices=["cfg2", "cfg3", "cfg4", "cfg5"])
+    ap.add_argument("which", choices=["cfg2", "cfg3", "cfg4", "cfg5", "quads"])
     ap.add_argument("--scale", type=int, default=4)
     a = ap.parse_args()
     print("| cfg | n | p | sub side | prec | DOF/thread | CTAs/sub | DOF/sub | blocks | threads | smem B | sweep ms | DOF-steps/s | frac of FMA peak |")
@@ -51,6 +53,14 @@ def main():
         for prec in (hz.HZ_F32, hz.HZ_F64):
             for k in (1, 9):
                 run(int(a.which[3]), prec, k)
+    elif a.which == "quads":   # general convex quads (distorted meshes): configs 2, 3 and a degree x side sweep
+        for prec in (hz.HZ_F32, hz.HZ_F64):
+            run(2, prec, 0, distort=0.2)
+            run(3, prec, 0, distort=0.2)
+        for p in (1, 2, 3, 4):
+            for s in (4, 8, 16):
+                for prec in (hz.HZ_F32, hz.HZ_F64):
+                    run(5, prec, 0, n=(6144 // p) // a.scale // s * s, p=p, s=s, reps=2, distort=0.2)
     elif a.which == "cfg4":
         for prec in (hz.HZ_F32, hz.HZ_F64):
             for k in (0, 18, 36):

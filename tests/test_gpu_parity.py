@@ -27,7 +27,8 @@ def problem_from(inp, bc=None):
     f = inp.f_re.astype(complex)
     if inp.f_im is not None:
         f = f + 1j * inp.f_im
-    return O.Problem(inp.nx, inp.ny, inp.p, inp.x0, inp.y0, inp.x1, inp.y1, inp.c_nodes, inp.omega, f, bc)
+    return O.Problem(inp.nx, inp.ny, inp.p, inp.x0, inp.y0, inp.x1, inp.y1, inp.c_nodes, inp.omega, f, bc,
+                     vx=getattr(inp, "vx", None), vy=getattr(inp, "vy", None))
 
 
 def pack_bc(inp, bc):
@@ -61,8 +62,12 @@ def oracle_state_arrays(st):
 
 
 def run_gpu(inp, prec, k, n_outer, n_wh, warm, relax, bc=None, res_field=None):
-    ctx = hz.hz_mesh_setup(inp.nx, inp.ny, inp.x0, inp.y0, inp.x1, inp.y1, inp.p, inp.c_nodes, inp.omega, inp.f_re,
-                           inp.f_im, pack_bc(inp, bc))
+    if getattr(inp, "vx", None) is not None:
+        ctx = hz.hz_mesh_setup_quads(inp.nx, inp.ny, inp.p, inp.vx, inp.vy, inp.c_nodes, inp.omega, inp.f_re,
+                                     inp.f_im, pack_bc(inp, bc))
+    else:
+        ctx = hz.hz_mesh_setup(inp.nx, inp.ny, inp.x0, inp.y0, inp.x1, inp.y1, inp.p, inp.c_nodes, inp.omega,
+                               inp.f_re, inp.f_im, pack_bc(inp, bc))
     try:
         info = hz.hz_partition(ctx, inp.sx, inp.sy, hz.HZ_TC_IMPEDANCE0, prec, k, inp.cfl_frac)
         dt = torch.float64 if prec == hz.HZ_F64 else torch.float32
