@@ -110,7 +110,12 @@ typedef struct {
  * (nx/sx)*(ny/sy) elements, one thread block per subdomain, and the
  * per-subdomain operator data of the modified leapfrog (alpha_j, beta_j).
  *
- *   sx, sy           subdomain grid; must divide nx, ny (else HZ_EINVAL; reading R23).
+ *   sx, sy           subdomain grid; must divide nx, ny on a uniform-mesh context (else HZ_EINVAL; reading R23).
+ *                    On a hz_mesh_setup_quads context any 1 <= sx <= nx, 1 <= sy <= ny is accepted (ragged
+ *                    partitions, reading R25; "at most K elements"): the first nx mod sx subdomain
+ *                    columns have floor(nx/sx)+1 elements, the others floor(nx/sx); same in y.  All per-subdomain
+ *                    arrays (and hz_part_info) are then sized for the largest subdomain, the padding is zero, and
+ *                    the excess threads of a smaller subdomain's block idle (PAPER.md fn. at 203).
  *   tc               transmission condition (only HZ_TC_IMPEDANCE0).
  *   prec             arithmetic of the sweep (fp32 or fp64 build of the subdomain solve).
  *   dofs_per_thread  1 = one DOF per thread (needs dofs_per_sub <= 1024);

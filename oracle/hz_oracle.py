@@ -342,18 +342,27 @@ class DDMState:
     n_sweeps: int = 0
 
 
+def split_elements(n: int, s: int):
+    """Sizes and offsets of the s consecutive groups n elements are split into (reading R25): floor(n/s) each,
+    the first n mod s groups one more."""
+    q, r = divmod(n, s)
+    sizes = [q + 1 if k < r else q for k in range(s)]
+    offs = [k * q + min(k, r) for k in range(s)]
+    return sizes, offs
+
+
 def ddm_setup(pr: Problem, sx: int, sy: int, cfl_frac: float = 0.5, n_t: int | None = None) -> DDMState:
-    """Partition into sx*sy rectangular subdomains of (nx/sx)*(ny/sy) elements and build the
+    """Partition into sx*sy rectangular subdomains of about (nx/sx)*(ny/sy) elements and build the
     subdomain systems (O3): A_l, M_l from the subdomain's own elements; H_l on its whole
     boundary (interfaces carry the same impedance operator as the outer boundary,
     PAPER.md:70-75, 83); load f(x_j) m^l_j with the LOCAL mass."""
-    if pr.nx % sx or pr.ny % sy:
-        raise ValueError("subdomain grid must divide the element grid (reading R23)")
-    ex, ey = pr.nx // sx, pr.ny // sy
+    if not (1 <= sx <= pr.nx and 1 <= sy <= pr.ny):
+        raise ValueError("need 1 <= sx <= nx, 1 <= sy <= ny")
+    # Ragged partitions (reading R25; PAPER.md:195 "at most K elements", fn. at 203): the nx element columns are
+    # split as evenly as possible, the first nx mod sx subdomain columns get one element more; same in y.
+    exs, X0 = split_elements(pr.nx, sx)
+    eys, Y0 = split_elements(pr.ny, sy)
     quads = pr.vx is not None
-    if not quads:
-        A, m, s = _region_operators(pr.p, ex, ey, pr.hx, pr.hy)
-    npx, npy = ex * pr.p + 1, ey * pr.p + 1
     c = np.asarray(pr.c_nodes, dtype=float)
     f = np.asarray(pr.f, dtype=complex)
     if n_t is None:
@@ -363,12 +372,19 @@ def ddm_setup(pr: Problem, sx: int, sy: int, cfl_frac: float = 0.5, n_t: int | N
             n_t = choose_nt(pr.p, pr.hx, pr.hy, float(c.max()), pr.omega, cfl_frac)
     tab = wh_tables(n_t, pr.omega)
     subs = []
+    rect_ops = {}
     for iy in range(sy):
         for ix in range(sx):
-            I0, J0 = ix * ex * pr.p, iy * ey * pr.p
+            ex, ey = exs[ix], eys[iy]
+            npx, npy = ex * pr.p + 1, ey * pr.p + 1
+            I0, J0 = X0[ix] * pr.p, Y0[iy] * pr.p
             if quads:   # F3: the subdomain's own elements, from its block of the vertex arrays
-                A, m, s = region_operators_quads(pr.p, pr.vx[iy * ey:(iy + 1) * ey + 1, ix * ex:(ix + 1) * ex + 1],
-                                                 pr.vy[iy * ey:(iy + 1) * ey + 1, ix * ex:(ix + 1) * ex + 1])
+                A, m, s = region_operators_quads(pr.p, pr.vx[Y0[iy]:Y0[iy] + ey + 1, X0[ix]:X0[ix] + ex + 1],
+                                                 pr.vy[Y0[iy]:Y0[iy] + ey + 1, X0[ix]:X0[ix] + ex + 1])
+            else:
+                if (ex, ey) not in rect_ops:
+                    rect_ops[(ex, ey)] = _region_operators(pr.p, ex, ey, pr.hx, pr.hy)
+                A, m, s = rect_ops[(ex, ey)]
             cl = c[J0:J0 + npy, I0:I0 + npx].reshape(-1)
             fl = f[J0:J0 + npy, I0:I0 + npx].reshape(-1)
             M = m.reshape(-1) / cl ** 2

@@ -216,6 +216,7 @@ Geo make_geo(const hz_ctx *c) {
   Geo g{};
   g.nx = c->nx; g.ny = c->ny; g.p = c->p; g.npx = c->npx; g.npy = c->npy;
   g.sx = c->sx; g.sy = c->sy; g.ex = c->ex; g.ey = c->ey; g.E = c->E; g.EB = c->EB;
+  g.exq = c->nx / c->sx; g.exr = c->nx % c->sx; g.eyq = c->ny / c->sy; g.eyr = c->ny % c->sy;
   g.hx = c->hx; g.hy = c->hy; g.omega = c->omega; g.theta = c->theta; g.sigma = c->sigma;
   return g;
 }
@@ -290,6 +291,7 @@ SweepArgs<real> make_args(const hz_ctx *c, const hz_solve_opts *o) {
   SweepArgs<real> a{};
   a.lay = c->lay;
   a.sx = c->sx; a.sy = c->sy; a.E = c->E;
+  a.exq = c->nx / c->sx; a.exr = c->nx % c->sx; a.eyq = c->ny / c->sy; a.eyr = c->ny % c->sy;
   a.n_t = c->n_t; a.n_wh = o->n_wh; a.warm = o->warm_start;
   a.sigma = (real)c->sigma; a.omega = (real)c->omega;
   a.cos_h = (real)std::cos(M_PI / c->n_t); a.sin_h = (real)std::sin(M_PI / c->n_t);
@@ -536,15 +538,19 @@ hz_status hz_set_source(hz_ctx *ctx, const double *f_re, const double *f_im) {
 hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec prec, int dofs_per_thread,
                        double cfl_frac, hz_part_info *info_out) {
   if (!ctx) return HZ_EINVAL;
-  if (sx < 1 || sy < 1 || ctx->nx % sx || ctx->ny % sy)
-    return fail(ctx, HZ_EINVAL, "hz_partition: sx, sy must be >= 1 and divide nx, ny");
+  if (sx < 1 || sy < 1 || sx > ctx->nx || sy > ctx->ny)
+    return fail(ctx, HZ_EINVAL, "hz_partition: need 1 <= sx <= nx, 1 <= sy <= ny");
+  if (!ctx->general && (ctx->nx % sx || ctx->ny % sy))
+    return fail(ctx, HZ_EINVAL, "hz_partition: sx, sy must divide nx, ny on a uniform mesh (ragged partitions: hz_mesh_setup_quads)");
   if (tc != HZ_TC_IMPEDANCE0) return fail(ctx, HZ_EUNSUPPORTED, "hz_partition: only HZ_TC_IMPEDANCE0");
   if (prec != HZ_F32 && prec != HZ_F64) return fail(ctx, HZ_EINVAL, "hz_partition: bad precision");
   if (!(cfl_frac > 0.0) || cfl_frac > 1.0) return fail(ctx, HZ_EINVAL, "hz_partition: cfl_frac must be in (0,1]");
   if (dofs_per_thread < -1) return fail(ctx, HZ_EINVAL, "hz_partition: dofs_per_thread < -1");
   free_partition(ctx);
   const int P = ctx->p;
-  ctx->sx = sx; ctx->sy = sy; ctx->ex = ctx->nx / sx; ctx->ey = ctx->ny / sy; ctx->L = sx * sy; ctx->prec = prec;
+  // ex, ey: elements per subdomain side; for a ragged partition (general quads only, reading R25) the maximum
+  ctx->sx = sx; ctx->sy = sy; ctx->ex = (ctx->nx + sx - 1) / sx; ctx->ey = (ctx->ny + sy - 1) / sy;
+  ctx->L = sx * sy; ctx->prec = prec;
   const int lnx = ctx->ex * P + 1, lny = ctx->ey * P + 1, N = lnx * lny;
   ctx->E = lnx > lny ? lnx : lny;
   const size_t rs = prec == HZ_F32 ? 4 : 8;

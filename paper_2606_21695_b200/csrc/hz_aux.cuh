@@ -8,10 +8,19 @@ namespace hz {
 // Mesh / partition description used by the auxiliary kernels (all fp64).
 struct Geo {
   int nx, ny, p, npx, npy;  // global elements, degree, global nodes per side
-  int sx, sy, ex, ey;       // subdomain grid, elements per subdomain
+  int sx, sy, ex, ey;       // subdomain grid, elements per subdomain side (the maximum, for ragged partitions)
+  int exq, exr, eyq, eyr;   // nx = sx*exq + exr, ny = sy*eyq + eyr: the first exr (eyr) subdomain columns (rows)
+                            // have exq+1 (eyq+1) elements, the others exq (eyq) (reading R25); uniform: exr = eyr = 0
   int E, EB;                // edge stride of lambda arrays; of the bc_lambda side blocks
   double hx, hy, omega, theta, sigma;
 };
+
+// even split of n = s*q + r elements into s groups: size, offset of group k, group of element e
+__host__ __device__ inline int sub_size(int q, int r, int k) { return q + (k < r ? 1 : 0); }
+__host__ __device__ inline int sub_off(int q, int r, int k) { return k * q + (k < r ? k : r); }
+__host__ __device__ inline int sub_of_elem(int q, int r, int e) {
+  return e < r * (q + 1) ? e / (q + 1) : r + (e - r * (q + 1)) / q;
+}
 
 // ---------------------------------------------------------------------------------------------
 // A0: per-subdomain operator data (PAPER.md:107-113 for M, H; PAPER.md:144 for alpha, beta).
@@ -154,19 +163,17 @@ __global__ void k_gather(Geo g, Layout lay, const real *__restrict__ u_sub, outT
   const long long total = (long long)g.npx * g.npy;
   if (gid >= total) return;
   const int I = (int)(gid % g.npx), J = (int)(gid / g.npx);
-  const int wx = g.ex * g.p, wy = g.ey * g.p;
-  int ix1 = I / wx;
-  if (ix1 > g.sx - 1) ix1 = g.sx - 1;
-  int iy1 = J / wy;
-  if (iy1 > g.sy - 1) iy1 = g.sy - 1;
-  const int ix0 = (I - ix1 * wx == 0 && ix1 > 0) ? ix1 - 1 : ix1;
-  const int iy0 = (J - iy1 * wy == 0 && iy1 > 0) ? iy1 - 1 : iy1;
+  // the subdomain column (row) of the element that has this node as a lower node, and the one before at a shared node
+  const int ehx = I / g.p > g.nx - 1 ? g.nx - 1 : I / g.p, ehy = J / g.p > g.ny - 1 ? g.ny - 1 : J / g.p;
+  const int ix1 = sub_of_elem(g.exq, g.exr, ehx), iy1 = sub_of_elem(g.eyq, g.eyr, ehy);
+  const int ix0 = (I == sub_off(g.exq, g.exr, ix1) * g.p && ix1 > 0) ? ix1 - 1 : ix1;
+  const int iy0 = (J == sub_off(g.eyq, g.eyr, iy1) * g.p && iy1 > 0) ? iy1 - 1 : iy1;
   double sr = 0.0, si = 0.0;
   int cnt = 0;
   for (int iy = iy0; iy <= iy1; ++iy)
     for (int ix = ix0; ix <= ix1; ++ix) {
       const int l = iy * g.sx + ix;
-      const int s = lay.slot(I - ix * wx, J - iy * wy);
+      const int s = lay.slot(I - sub_off(g.exq, g.exr, ix) * g.p, J - sub_off(g.eyq, g.eyr, iy) * g.p);
       sr += (double)u_sub[(size_t)l * 2 * lay.NS + s];
       si += (double)u_sub[(size_t)l * 2 * lay.NS + lay.NS + s];
       ++cnt;

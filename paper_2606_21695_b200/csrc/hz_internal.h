@@ -60,6 +60,7 @@ template <typename real>
 struct SweepArgs {
   Layout lay;
   int sx, sy;      // subdomain grid
+  int exq, exr, eyq, eyr;  // ragged partitions (general-quad kernel): see Geo
   int E;           // edge stride of lambda / g / kedge / bs arrays
   int n_t, n_wh, warm;
   real sigma, omega, cos_h, sin_h, two_over_nt;  // cos_h = cos(pi/N_t), sin_h = sin(pi/N_t)

@@ -73,11 +73,15 @@ __global__ void k_build_quad(Geo g, Layout lay, RefQ ref, const double *__restri
   const int l = (int)(gid / N), q = (int)(gid - (long long)l * N);
   const int i = q % lay.lnx, j = q / lay.lnx;
   const int six = l % g.sx, siy = l / g.sx;
-  const int I = six * g.ex * g.p + i, J = siy * g.ey * g.p + j;
+  const int exl = sub_size(g.exq, g.exr, six), eyl = sub_size(g.eyq, g.eyr, siy);  // this subdomain's elements
+  const int gx0 = sub_off(g.exq, g.exr, six), gy0 = sub_off(g.eyq, g.eyr, siy);
+  const int lnxl = exl * g.p + 1, lnyl = eyl * g.p + 1;
+  if (i >= lnxl || j >= lnyl) return;  // padding of a ragged subdomain: stays zero
+  const int I = gx0 * g.p + i, J = gy0 * g.p + j;
   const size_t gn = (size_t)J * g.npx + I;
   const double cj = c[gn];
   double m, s[4];
-  quad_node_weights(ref, vx, vy, g.nx, g.p, six * g.ex, siy * g.ey, g.ex, g.ey, i, j, &m, s);
+  quad_node_weights(ref, vx, vy, g.nx, g.p, gx0, gy0, exl, eyl, i, j, &m, s);
   const double M = m / (cj * cj);
   const double H = (s[0] + s[1] + s[2] + s[3]) / cj;  // impedance on the whole subdomain boundary
   const double den = M + g.theta * H;
@@ -85,9 +89,9 @@ __global__ void k_build_quad(Geo g, Layout lay, RefQ ref, const double *__restri
   double bre = f_re[gn] * m, bim = f_im ? f_im[gn] * m : 0.0;
   if (bc) {
     if (i == 0 && six == 0) { bre += s[0] * bc[(0 * 2 + 0) * g.EB + J]; bim += s[0] * bc[(0 * 2 + 1) * g.EB + J]; }
-    if (i == lay.lnx - 1 && six == g.sx - 1) { bre += s[1] * bc[(1 * 2 + 0) * g.EB + J]; bim += s[1] * bc[(1 * 2 + 1) * g.EB + J]; }
+    if (i == lnxl - 1 && six == g.sx - 1) { bre += s[1] * bc[(1 * 2 + 0) * g.EB + J]; bim += s[1] * bc[(1 * 2 + 1) * g.EB + J]; }
     if (j == 0 && siy == 0) { bre += s[2] * bc[(2 * 2 + 0) * g.EB + I]; bim += s[2] * bc[(2 * 2 + 1) * g.EB + I]; }
-    if (j == lay.lny - 1 && siy == g.sy - 1) { bre += s[3] * bc[(3 * 2 + 0) * g.EB + I]; bim += s[3] * bc[(3 * 2 + 1) * g.EB + I]; }
+    if (j == lnyl - 1 && siy == g.sy - 1) { bre += s[3] * bc[(3 * 2 + 0) * g.EB + I]; bim += s[3] * bc[(3 * 2 + 1) * g.EB + I]; }
   }
   const size_t o = (size_t)l * lay.NS + lay.slot(i, j);
   bbf_re[o] = (real)(beta * bre);
@@ -98,13 +102,14 @@ __global__ void k_build_quad(Geo g, Layout lay, RefQ ref, const double *__restri
   const size_t eb = (size_t)l * 4 * g.E;
   const double k2 = 2.0 * g.omega / cj;
   if (i == 0) { k2edge[eb + 0 * g.E + j] = (real)k2; bs[eb + 0 * g.E + j] = (real)(beta * s[0]); }
-  if (i == lay.lnx - 1) { k2edge[eb + 1 * g.E + j] = (real)k2; bs[eb + 1 * g.E + j] = (real)(beta * s[1]); }
+  if (i == lnxl - 1) { k2edge[eb + 1 * g.E + j] = (real)k2; bs[eb + 1 * g.E + j] = (real)(beta * s[1]); }
   if (j == 0) { k2edge[eb + 2 * g.E + i] = (real)k2; bs[eb + 2 * g.E + i] = (real)(beta * s[2]); }
-  if (j == lay.lny - 1) { k2edge[eb + 3 * g.E + i] = (real)k2; bs[eb + 3 * g.E + i] = (real)(beta * s[3]); }
+  if (j == lnyl - 1) { k2edge[eb + 3 * g.E + i] = (real)k2; bs[eb + 3 * g.E + i] = (real)(beta * s[3]); }
 }
 
 // Geometric factors of every quadrature point, weights folded in: G[l][3 n + {0,1,2}][t] = w_a w_b {gxx, gxy, gyy}
-// for element t = fy*ex + fx of subdomain l and point n = b (P+1) + a; nep = element stride (threads per block).
+// for element t = fy*ex + fx of subdomain l (ex = the maximal width: ragged subdomains leave gaps) and point
+// n = b (P+1) + a; nep = element stride (threads per block).
 template <typename real>
 __global__ void k_build_quad_metric(Geo g, RefQ ref, const double *__restrict__ vx, const double *__restrict__ vy,
                                     int nep, real *G) {
@@ -113,8 +118,10 @@ __global__ void k_build_quad_metric(Geo g, RefQ ref, const double *__restrict__ 
   if (gid >= (long long)g.sx * g.sy * ne * NQ) return;
   const int t = (int)(gid % ne), n = (int)((gid / ne) % NQ), l = (int)(gid / ((long long)ne * NQ));
   const int fx = t % g.ex, fy = t / g.ex, a = n % (P + 1), b = n / (P + 1);
+  const int six = l % g.sx, siy = l / g.sx;
+  if (fx >= sub_size(g.exq, g.exr, six) || fy >= sub_size(g.eyq, g.eyr, siy)) return;
   double X[4], Y[4];
-  quad_vertices(vx, vy, g.nx, (l % g.sx) * g.ex + fx, (l / g.sx) * g.ey + fy, X, Y);
+  quad_vertices(vx, vy, g.nx, sub_off(g.exq, g.exr, six) + fx, sub_off(g.eyq, g.eyr, siy) + fy, X, Y);
   const QuadPt q = quad_point(X, Y, ref.xi[a], ref.xi[b]);
   const double ww = ref.w[a] * ref.w[b];
   real *o = G + ((size_t)l * 3 * NQ + 3 * n) * nep + t;

@@ -36,14 +36,19 @@ __global__ void __launch_bounds__(MAXT, MINB)
   const int BUFW = (NT + 33) * RS;
   real *xb = reinterpret_cast<real *>(smem_raw);
   real *csm = xb + 2 * BUFW + (size_t)t * CST;
-  const int ex = A.lay.ntx, ey = A.lay.nty, NS = A.lay.NS, lnx = A.lay.lnx, lny = A.lay.lny;
-  const bool act = t < ex * ey;
+  // ex = element stride of the thread grid (the widest subdomain); exl x eyl = this subdomain's elements (ragged
+  // partitions, reading R25); lnx = node stride of the per-DOF arrays, lnxl x lnyl = this subdomain's nodes
+  const int ex = A.lay.ntx, NS = A.lay.NS, lnx = A.lay.lnx;
+  const int six = l % A.sx, siy = l / A.sx;
+  const int exl = A.exq + (six < A.exr ? 1 : 0), eyl = A.eyq + (siy < A.eyr ? 1 : 0);
+  const int lnxl = exl * P + 1, lnyl = eyl * P + 1;
+  const bool act = t < ex * A.lay.nty && t % ex < exl && t / ex < eyl;
   const int fx = act ? t % ex : 0, fy = act ? t / ex : 0;
   const int ZR = NT, SCR = NT + 32;
 
   for (int q = t; q < 2 * BUFW; q += NT) xb[q] = real(0);
 
-  const bool hasL = act && fx > 0, hasR = act && fx < ex - 1, hasD = act && fy > 0, hasU = act && fy < ey - 1;
+  const bool hasL = act && fx > 0, hasR = act && fx < exl - 1, hasD = act && fy > 0, hasU = act && fy < eyl - 1;
   auto rec = [&](bool has, int nb) { return xb + (has ? nb : ZR + (nb & 31)) * RS; };
   const real *pL = rec(hasL, t - 1) + oE, *pR = rec(hasR, t + 1) + oW;
   const real *pD = rec(hasD, t - ex) + oN, *pU = rec(hasU, t + ex) + oS;
@@ -52,7 +57,6 @@ __global__ void __launch_bounds__(MAXT, MINB)
   real *pMy = xb + (act ? t : SCR) * RS;
 
   real p[N1][N1], pd[N1][N1], vr[N1][N1], vi[N1][N1], ur[N1][N1], ui[N1][N1];
-  const int six = l % A.sx, siy = l / A.sx;
   const size_t lbase = (size_t)l * 4 * 2 * A.E, ebase = (size_t)l * 4 * A.E;
   if (act) {
 #pragma unroll
@@ -68,7 +72,7 @@ __global__ void __launch_bounds__(MAXT, MINB)
           br = fmaT(s, A.lam[lbase + (kSideW * 2 + 0) * A.E + j], br);
           bi = fmaT(s, A.lam[lbase + (kSideW * 2 + 1) * A.E + j], bi);
         }
-        if (i == lnx - 1 && six < A.sx - 1) {
+        if (i == lnxl - 1 && six < A.sx - 1) {
           const real s = A.bs[ebase + kSideE * A.E + j];
           br = fmaT(s, A.lam[lbase + (kSideE * 2 + 0) * A.E + j], br);
           bi = fmaT(s, A.lam[lbase + (kSideE * 2 + 1) * A.E + j], bi);
@@ -78,7 +82,7 @@ __global__ void __launch_bounds__(MAXT, MINB)
           br = fmaT(s, A.lam[lbase + (kSideS * 2 + 0) * A.E + i], br);
           bi = fmaT(s, A.lam[lbase + (kSideS * 2 + 1) * A.E + i], bi);
         }
-        if (j == lny - 1 && siy < A.sy - 1) {
+        if (j == lnyl - 1 && siy < A.sy - 1) {
           const real s = A.bs[ebase + kSideN * A.E + i];
           br = fmaT(s, A.lam[lbase + (kSideN * 2 + 0) * A.E + i], br);
           bi = fmaT(s, A.lam[lbase + (kSideN * 2 + 1) * A.E + i], bi);
@@ -219,15 +223,15 @@ __global__ void __launch_bounds__(MAXT, MINB)
   for (int b = 0; b < N1; ++b)
 #pragma unroll
     for (int a = 0; a < N1; ++a) {
-      if ((a == P && fx != ex - 1) || (b == P && fy != ey - 1)) continue;
+      if ((a == P && fx != exl - 1) || (b == P && fy != eyl - 1)) continue;
       const int i = fx * P + a, j = fy * P + b;
       A.u_sub[(size_t)l * 2 * NS + (size_t)j * lnx + i] = ur[b][a];
       A.u_sub[(size_t)l * 2 * NS + NS + (size_t)j * lnx + i] = ui[b][a];
       int side[2], idx[2], ns = 0;
       if (i == 0 && six > 0) { side[ns] = kSideW; idx[ns++] = j; }
-      if (i == lnx - 1 && six < A.sx - 1) { side[ns] = kSideE; idx[ns++] = j; }
+      if (i == lnxl - 1 && six < A.sx - 1) { side[ns] = kSideE; idx[ns++] = j; }
       if (j == 0 && siy > 0) { side[ns] = kSideS; idx[ns++] = i; }
-      if (j == lny - 1 && siy < A.sy - 1) { side[ns] = kSideN; idx[ns++] = i; }
+      if (j == lnyl - 1 && siy < A.sy - 1) { side[ns] = kSideN; idx[ns++] = i; }
       for (int k = 0; k < ns; ++k) {
         const real k2 = A.k2edge[ebase + side[k] * A.E + idx[k]];
         const size_t o = lbase + (size_t)(side[k] * 2) * A.E + idx[k];

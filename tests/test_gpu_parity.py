@@ -49,12 +49,15 @@ def rel(a, b):
 
 def oracle_state_arrays(st):
     L = len(st.subs)
-    N = st.subs[0].npx * st.subs[0].npy
-    E = max(st.subs[0].npx, st.subs[0].npy)
+    nxm, nym = max(sd.npx for sd in st.subs), max(sd.npy for sd in st.subs)   # ragged: padded to the largest
+    N = nxm * nym
+    E = max(nxm, nym)
     u = np.zeros((L, 2, N))
     lam = np.zeros((L, 4, 2, E))
     for l in range(L):
-        u[l, 0], u[l, 1] = st.u[l].real, st.u[l].imag
+        sd = st.subs[l]
+        u[l, 0].reshape(nym, nxm)[:sd.npy, :sd.npx] = st.u[l].real.reshape(sd.npy, sd.npx)
+        u[l, 1].reshape(nym, nxm)[:sd.npy, :sd.npx] = st.u[l].imag.reshape(sd.npy, sd.npx)
         for s in range(4):
             a = st.lam[l][s]
             lam[l, s, 0, :len(a)], lam[l, s, 1, :len(a)] = a.real, a.imag

@@ -99,6 +99,37 @@ def test_quads_converge_to_the_direct_solve_and_replicated_nodes_stay_consistent
         hz.hz_destroy(ctx)
 
 
+@pytest.mark.parametrize("prec", [hz.HZ_F64, hz.HZ_F32])
+def test_ragged_partitions(prec):
+    # 11x7 elements in 3x2 subdomains: 4,4,3 x 4,3 elements; blocks sized for 4x4, the smaller ones idle threads
+    inp = quad_inputs(11, 7, 3, 3, 2, seed=91)
+    rng = np.random.default_rng(6)
+    bc = [rng.standard_normal(n) + 1j * rng.standard_normal(n) for n in (inp.npy, inp.npy, inp.npx, inp.npx)]
+    g = check_case(inp, prec, 0, n_outer=3, n_wh=2, bc=bc)
+    assert g["info"].dofs_per_sub == 13 * 13 and g["info"].blocks == 6
+    # 7x5 in 3x2 (3,2,2 x 3,2), p = 2, and a partition into single elements and pairs (5 in 3: 2,2,1)
+    check_case(quad_inputs(7, 5, 2, 3, 2, seed=92), prec, 0, n_outer=3, n_wh=2)
+    check_case(quad_inputs(5, 5, 4, 3, 3, seed=93), prec, 0, n_outer=2, n_wh=2)
+
+
+def test_ragged_rectangles_converge_to_the_direct_solve():
+    # uniform rectangles as vertices, 10x10 elements in 3x3 subdomains (4,3,3): converged field == direct solve
+    inp = make_config(1, n=10, p=2, sub_elems=10)
+    gx = np.linspace(0.0, 1.0, inp.nx + 1)
+    VX, VY = np.meshgrid(gx, gx, indexing="xy")
+    inp = HzInputs(**{**inp.__dict__, "vx": VX, "vy": VY, "sx": 3, "sy": 3})
+    uref = O.direct_solve(O.Problem(inp.nx, inp.ny, inp.p, 0, 0, 1, 1, inp.c_nodes, inp.omega, inp.f_re.astype(complex)))
+    ctx, info = hz.setup_from_inputs(inp, hz.HZ_F64, 0)
+    try:
+        u_out = torch.zeros(2 * inp.npx * inp.npy, dtype=torch.float64, device="cuda")
+        r = hz.hz_ddm_solve(ctx, 2000, n_wh=5, tol=1e-11, check_every=50, reset_state=True, use_graph=True,
+                            u_out_ptr=u_out.data_ptr())
+        u = u_out.cpu().numpy().reshape(2, inp.npy, inp.npx)
+        assert r.rel_residual <= 1e-11 and rel(u[0] + 1j * u[1], uref) < 1e-9
+    finally:
+        hz.hz_destroy(ctx)
+
+
 def test_quads_errors():
     inp = quad_inputs(4, 4, 2, 2, 2, seed=1)
     bad = inp.vx.copy()
@@ -111,6 +142,9 @@ def test_quads_errors():
         with pytest.raises(hz.HzError) as e:
             hz.hz_partition(ctx, 2, 2, prec=hz.HZ_F64, dofs_per_thread=1)
         assert e.value.status == hz.HZ_EUNSUPPORTED
+        with pytest.raises(hz.HzError) as e:
+            hz.hz_partition(ctx, 5, 2, prec=hz.HZ_F64, dofs_per_thread=0)      # more subdomain columns than elements
+        assert e.value.status == hz.HZ_EINVAL
         hz.hz_partition(ctx, 2, 2, prec=hz.HZ_F64, dofs_per_thread=0)
         with pytest.raises(hz.HzError) as e:
             hz.hz_minres_cycle(ctx, 4, 1e-6, 10, False, 0.5)

@@ -165,3 +165,34 @@ def test_ddm_on_quads_converges_to_the_direct_solve():
     u = O.ddm_gather(st)
     assert np.linalg.norm(u - uref) / np.linalg.norm(uref) < 2e-9     # linear convergence, 1e-13 after 800 sweeps
     assert O.residual(pr, u) < 5e-8
+
+
+# ---------------------------------------------------------------- ragged partitions (reading R25)
+def test_split_elements_is_the_even_split():
+    for n in range(1, 40):
+        for s in range(1, n + 1):
+            sizes, offs = O.split_elements(n, s)
+            assert sum(sizes) == n and max(sizes) - min(sizes) <= 1 and sorted(sizes, reverse=True) == sizes
+            assert offs == [sum(sizes[:k]) for k in range(s)]
+
+
+@pytest.mark.parametrize("quads", [False, True])
+def test_ragged_ddm_converges_to_the_same_direct_solve(quads):
+    # the converged answer does not depend on the partition: 7x5 elements in 3x2 subdomains (3,2,2 x 3,2 elements)
+    rng = np.random.default_rng(3)
+    nx, ny, p = 7, 5, 2
+    VX = VY = None
+    if quads:
+        VX, VY = distorted_vertices(nx, ny, rng, 0.2)
+    shape = (ny * p + 1, nx * p + 1)
+    c = 1.0 + 0.5 * rng.uniform(0, 1, shape)
+    f = rng.standard_normal(shape) + 0j
+    pr = O.Problem(nx, ny, p, 0, 0, 1, 1, c, 9.0, f, vx=VX, vy=VY)
+    uref = O.direct_solve(pr)
+    st = O.ddm_setup(pr, 3, 2)
+    assert [(sd.npx, sd.npy) for sd in st.subs] == [(7, 7), (5, 7), (5, 7), (7, 5), (5, 5), (5, 5)]
+    errs = []
+    for _ in range(3):                                  # linear convergence towards the partition-independent answer
+        st = O.ddm_solve(pr, 3, 2, 200, 5, state=st)
+        errs.append(np.linalg.norm(O.ddm_gather(st) - uref) / np.linalg.norm(uref))
+    assert errs[2] < 1e-5 and errs[1] < 0.3 * errs[0] and errs[2] < 0.3 * errs[1], errs
