@@ -1,0 +1,129 @@
+"""Pins of the 3-D oracle (oracle/hz_oracle3d.py) against what the mathematics fixes.  CPU only."""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import hz_oracle as O2
+from oracle import hz_oracle3d as O
+
+
+def box_problem(n, p, omega, c=None, f=None, bc=None, box=(0, 0, 0, 1, 1, 1)):
+    nx, ny, nz = n if isinstance(n, tuple) else (n, n, n)
+    shape = (nz * p + 1, ny * p + 1, nx * p + 1)
+    c = np.ones(shape) if c is None else c
+    f = np.zeros(shape, dtype=complex) if f is None else f
+    return O.Problem3D(nx, ny, nz, p, box, c, omega, f, bc)
+
+
+@pytest.mark.parametrize("p", [1, 2, 3])
+def test_measure_symmetry_kernel_and_exact_energy(p):
+    ex, ey, ez, hx, hy, hz = 3, 2, 2, 0.4, 0.25, 0.35
+    A, m, s = O.region_operators(p, ex, ey, ez, hx, hy, hz)
+    Lx, Ly, Lz = ex * hx, ey * hy, ez * hz
+    assert abs(m.sum() - Lx * Ly * Lz) < 1e-13
+    for face, area in zip(range(6), (Ly * Lz, Ly * Lz, Lx * Lz, Lx * Lz, Lx * Ly, Lx * Ly)):
+        assert abs(s[face].sum() - area) < 1e-13
+    assert abs(A - A.T).max() < 1e-13
+    assert np.abs(A @ np.ones(A.shape[0])).max() < 1e-12
+    if p >= 2:
+        # u = x y z + x^2/2 - z:  grad = (yz + x, xz, xy - 1);  |grad|^2 has degree <= 2 per variable <= 2p-1: GLL exact
+        pr = box_problem((ex, ey, ez), p, 1.0, box=(0, 0, 0, Lx, Ly, Lz))
+        x, y, z = pr.node_coords()
+        Z, Y, X = np.meshgrid(z, y, x, indexing="ij")
+        u = (X * Y * Z + 0.5 * X ** 2 - Z).reshape(-1)
+        gx, gw = np.polynomial.legendre.leggauss(6)
+        def q1(L):
+            return 0.5 * L * (gx + 1), 0.5 * L * gw
+        (xa, wa), (ya, wb), (za, wc) = q1(Lx), q1(Ly), q1(Lz)
+        ZZ, YY, XX = np.meshgrid(za, ya, xa, indexing="ij")
+        W3 = wc[:, None, None] * wb[None, :, None] * wa[None, None, :]
+        exact = np.sum(W3 * ((YY * ZZ + XX) ** 2 + (XX * ZZ) ** 2 + (XX * YY - 1) ** 2))
+        assert abs(u @ (A @ u) - exact) < 1e-11 * exact
+
+
+@pytest.mark.parametrize("p", [1, 2, 3])
+def test_z_independent_field_sees_the_2d_operators(p):
+    ex, ey, ez, hx, hy, hz = 3, 2, 2, 0.4, 0.25, 0.35
+    A3, m3, _ = O.region_operators(p, ex, ey, ez, hx, hy, hz)
+    A2, m2, _ = O2._region_operators(p, ex, ey, hx, hy)
+    _, wz = O.assembled_1d(p, ez, hz)
+    u2 = np.random.default_rng(p).standard_normal(A2.shape[0])
+    u3 = np.tile(u2, len(wz))
+    assert np.allclose(A3 @ u3, np.kron(wz, A2 @ u2), atol=1e-12)
+    assert np.allclose(m3.reshape(len(wz), -1), np.outer(wz, m2.reshape(-1)), rtol=1e-13)
+
+
+@pytest.mark.parametrize("p", [1, 2, 3])
+def test_nt_bound_bounds_the_spectrum(p):
+    ex, ey, ez, hx, hy, hz = 2, 2, 1, 0.3, 0.2, 0.25
+    A, m, _ = O.region_operators(p, ex, ey, ez, hx, hy, hz)
+    M = m.reshape(-1)
+    lmax = np.max(np.linalg.eigvalsh(A.toarray() / np.sqrt(np.outer(M, M))))
+    omega = 20.0
+    nt = O.choose_nt(p, hx, hy, hz, 1.0, omega, 1.0)
+    dt = 2 * math.pi / omega / nt
+    assert 1.0 < dt * dt * lmax <= 4.0
+
+
+def planewave_error(p, n):
+    omega = 2 * math.pi * p * 4 / 10          # 10 points per wavelength at n = 4
+    d = np.array([0.6, 0.48, 0.64])           # unit vector
+    pr0 = box_problem(n, p, omega)
+    x, y, z = pr0.node_coords()
+    Z, Y, X = np.meshgrid(z, y, x, indexing="ij")
+    uex = np.exp(1j * omega * (d[0] * X + d[1] * Y + d[2] * Z))
+    normals = [(-1, 0, 0), (1, 0, 0), (0, -1, 0), (0, 1, 0), (0, 0, -1), (0, 0, 1)]
+    faces = [uex[:, :, 0], uex[:, :, -1], uex[:, 0, :], uex[:, -1, :], uex[0, :, :], uex[-1, :, :]]
+    lam = [1j * omega * (np.dot(d, nn) - 1.0) * e for nn, e in zip(normals, faces)]
+    pr = box_problem(n, p, omega, bc=lam)
+    u = O.direct_solve(pr)
+    return np.linalg.norm(u - uex) / np.linalg.norm(uex), pr, u
+
+
+def test_plane_wave_recovered_at_high_order():
+    e4, _, _ = planewave_error(2, 4)
+    e8, pr, u = planewave_error(2, 8)
+    assert e4 / e8 > 8 and e8 < 2e-3, (e4, e8)
+    assert O.residual(pr, u) < 1e-12
+
+
+def test_direct_solution_is_the_waveholtz_fixed_point_and_iteration_converges():
+    rng = np.random.default_rng(0)
+    p, n = 2, 2
+    shape = (n * p + 1,) * 3
+    c = 1.0 + 0.5 * rng.uniform(0, 1, shape)
+    f = rng.standard_normal(shape) + 1j * rng.standard_normal(shape)
+    pr = box_problem(n, p, 7.0, c=c, f=f)
+    A, M, H, b = O.assemble_global(pr)
+    ustar = O.direct_solve(pr).reshape(-1)
+    hx, hy, hz = pr.h
+    tab = O2.wh_tables(O.choose_nt(p, hx, hy, hz, float(c.max()), pr.omega, 0.5), pr.omega)
+    assert np.linalg.norm(O2.waveholtz_iteration(A, M, H, b, ustar, pr.omega, tab) - ustar) < 1e-11 * np.linalg.norm(ustar)
+    u = np.zeros_like(ustar)
+    for _ in range(60):
+        u = O2.waveholtz_iteration(A, M, H, b, u, pr.omega, tab)
+    assert np.linalg.norm(u - ustar) < 1e-6 * np.linalg.norm(ustar)
+
+
+def test_ddm_converges_to_the_direct_solve_and_single_subdomain_is_plain_waveholtz():
+    rng = np.random.default_rng(1)
+    p, n = 2, 4
+    shape = (n * p + 1,) * 3
+    c = 1.0 + 0.5 * rng.uniform(0, 1, shape)
+    f = rng.standard_normal(shape) + 0j
+    pr = box_problem(n, p, 6.0, c=c, f=f)
+    uref = O.direct_solve(pr)
+    st = O.ddm_setup(pr, 2, 2, 2)
+    errs = []
+    for _ in range(3):
+        st = O.ddm_solve(pr, 2, 2, 2, 100, 5, state=st)
+        errs.append(np.linalg.norm(O.ddm_gather(st) - uref) / np.linalg.norm(uref))
+    assert errs[2] < 1e-4 and errs[1] < 0.3 * errs[0] and errs[2] < 0.3 * errs[1], errs
+    # L = 1: one sweep is n_wh WaveHoltz iterations on the whole box
+    st1 = O.ddm_solve(pr, 1, 1, 1, 1, 3)
+    A, M, H, b = O.assemble_global(pr)
+    u = np.zeros(A.shape[0], dtype=complex)
+    for _ in range(3):
+        u = O2.waveholtz_iteration(A, M, H, b, u, pr.omega, st1.tab)
+    assert np.allclose(st1.u[0], u, rtol=0, atol=1e-14 * np.abs(u).max())
