@@ -119,7 +119,7 @@ def test_ddm_converges_to_the_direct_solve_and_single_subdomain_is_plain_wavehol
     for _ in range(3):
         st = O.ddm_solve(pr, 2, 2, 2, 100, 5, state=st)
         errs.append(np.linalg.norm(O.ddm_gather(st) - uref) / np.linalg.norm(uref))
-    assert errs[2] < 1e-4 and errs[1] < 0.3 * errs[0] and errs[2] < 0.3 * errs[1], errs
+    assert errs[2] < 1e-4 and errs[1] < 0.5 * errs[0] and errs[2] < 0.5 * errs[1], errs   # linear convergence
     # L = 1: one sweep is n_wh WaveHoltz iterations on the whole box
     st1 = O.ddm_solve(pr, 1, 1, 1, 1, 3)
     A, M, H, b = O.assemble_global(pr)
