@@ -274,7 +274,7 @@ __global__ void k_residual(Geo g, Ref1D ref, const double *__restrict__ c, const
   }
 }
 
-__global__ void k_reduce2(const double *__restrict__ part, int n, double *__restrict__ out) {
+static __global__ void k_reduce2(const double *__restrict__ part, int n, double *__restrict__ out) {
   __shared__ double red[2][32];
   double a = 0.0, b = 0.0;
   for (int q = threadIdx.x; q < n; q += blockDim.x) { a += part[2 * (size_t)q]; b += part[2 * (size_t)q + 1]; }
@@ -372,7 +372,7 @@ __global__ void k_dots(long long n, const real *__restrict__ V, long long ld, co
   }
 }
 
-__global__ void k_reduce_rows(const double *__restrict__ part, int nblk, double *__restrict__ out) {
+static __global__ void k_reduce_rows(const double *__restrict__ part, int nblk, double *__restrict__ out) {
   // one block per row: out[row] = sum of part[row][0..nblk)
   __shared__ double red[32];
   double s = 0.0;

@@ -205,3 +205,51 @@ def random_lambda(rng, n_sub: int, edge_nodes: int):
     """A random complex interface vector lambda[l, side, node] (the paper's benchmark applies
     the DDM cycle to a random input vector)."""
     return rng.standard_normal((n_sub, 4, edge_nodes)) + 1j * rng.standard_normal((n_sub, 4, edge_nodes))
+
+
+# ---------------------------------------------------------------------------------------------------------
+# 3-D hexahedral variant (SURVEY.md 8(f) F4; PAPER.md:263-269: uniform elements on a box, constant or blockwise
+# coefficients, random input)
+# ---------------------------------------------------------------------------------------------------------
+@dataclass
+class Hz3Inputs:
+    name: str
+    nx: int
+    ny: int
+    nz: int
+    p: int
+    box: tuple
+    omega: float
+    c_nodes: np.ndarray            # (npz, npy, npx)
+    f_re: np.ndarray
+    f_im: np.ndarray | None
+    sx: int
+    sy: int
+    sz: int
+    cfl_frac: float = 0.5
+    seed: int = 0
+
+    @property
+    def shape(self):
+        return self.nz * self.p + 1, self.ny * self.p + 1, self.nx * self.p + 1
+
+
+def make_config_3d(n, p: int, sub_elems, seed: int = 3000, ppw: float = 8.0, random_c: bool = True,
+                   box=(0.0, 0.0, 0.0, 1.0, 1.0, 1.0)) -> Hz3Inputs:
+    """n (int or 3-tuple) elements per side of a box, subdomains of sub_elems (int or 3-tuple) elements per side;
+    omega for `ppw` node spacings per wavelength; nodal c ~ 1 + U(0,1) (or 1); Gaussian source at a random point."""
+    nx, ny, nz = (n, n, n) if isinstance(n, int) else n
+    ex, ey, ez = (sub_elems,) * 3 if isinstance(sub_elems, int) else sub_elems
+    if nx % ex or ny % ey or nz % ez:
+        raise ValueError("sub_elems must divide n")
+    rng = np.random.default_rng(seed)
+    xs = [node_coords_1d(m, p, box[d], box[d + 3]) for d, m in enumerate((nx, ny, nz))]
+    Z, Y, X = np.meshgrid(xs[2], xs[1], xs[0], indexing="ij")
+    c = 1.0 + rng.uniform(0, 1, size=X.shape) if random_c else np.ones_like(X)
+    omega = omega_for_ppw(nx, p, ppw, length=box[3] - box[0])
+    x0 = np.array([rng.uniform(box[d] + 0.25 * (box[d + 3] - box[d]), box[d] + 0.75 * (box[d + 3] - box[d])) for d in range(3)])
+    sig = 1.5 * (box[3] - box[0]) / nx
+    f = np.exp(-((X - x0[0]) ** 2 + (Y - x0[1]) ** 2 + (Z - x0[2]) ** 2) / (2 * sig ** 2))
+    return Hz3Inputs(name=f"box_{nx}x{ny}x{nz}_p{p}_s{ex}x{ey}x{ez}", nx=nx, ny=ny, nz=nz, p=p, box=tuple(box),
+                     omega=omega, c_nodes=np.ascontiguousarray(c), f_re=np.ascontiguousarray(f), f_im=None,
+                     sx=nx // ex, sy=ny // ey, sz=nz // ez, seed=seed)

@@ -1,0 +1,42 @@
+"""Throughput of the 3-D sweep kernel over the block shapes of PAPER.md:265 (run under gpurun):
+
+    python -m paper_2606_21695_b200.sweep3d
+
+DOF-steps/s of the sweep kernel alone (CUDA events inside hz3_ddm_solve), n_wh = 5, warm start; frac = rate x
+2(3(2p+1)+5) / FMA peak: the (2p+1)-wide band rows of the three directions + 5 updates per DOF-step, as executed by
+the one-node-per-thread kernel."""
+from __future__ import annotations
+
+from . import hz, hz3
+from .inputs import make_config_3d
+
+SMS, CLK = 148, 1.965e9
+
+
+def run(n, p, s, prec):
+    inp = make_config_3d(n, p, s)
+    ctx = hz3.hz3_mesh_setup(inp.nx, inp.ny, inp.nz, inp.box, inp.p, inp.c_nodes, inp.omega, inp.f_re)
+    try:
+        info = hz3.hz3_partition(ctx, inp.sx, inp.sy, inp.sz, prec)
+        hz3.hz3_ddm_solve(ctx, 1, n_wh=5, reset_state=True)
+        r = hz3.hz3_ddm_solve(ctx, 3, n_wh=5)
+        rate = r.dof_timesteps / (r.sweep_ms_total * 1e-3)
+        fl = 2 * (3 * (2 * p + 1) + 5)
+        peak = SMS * (128 if prec == hz.HZ_F32 else 64) * 2 * CLK
+        print(f"| {inp.nx}^3 | {p} | {s}^3 | {'f32' if prec == hz.HZ_F32 else 'f64'} | {info.dofs_per_sub} | {info.blocks} | "
+              f"{info.threads_per_block} | {info.smem_bytes} | {info.n_t} | {r.sweep_ms_total / 3:.3f} | {rate:.3e} | "
+              f"{rate * fl / peak:.3f} |", flush=True)
+    finally:
+        hz3.hz3_destroy(ctx)
+
+
+def main():
+    print("| mesh | p | elements per subdomain | prec | DOF/sub | blocks | threads | smem B | N_t | sweep ms | DOF-steps/s | frac of FMA peak |")
+    print("|---|---|---|---|---|---|---|---|---|---|---|---|")
+    for n, p, s in ((128, 1, 8), (128, 1, 4), (64, 2, 4), (64, 2, 2), (48, 3, 3), (48, 3, 2), (32, 4, 2), (32, 4, 1)):
+        for prec in (hz.HZ_F32, hz.HZ_F64):
+            run(n, p, s, prec)
+
+
+if __name__ == "__main__":
+    main()

@@ -31,6 +31,25 @@ def test_library_exports_every_declared_symbol(libpath):
     assert set(hz.EXPORTS) == declared
 
 
+def test_library_exports_every_symbol_of_the_3d_header(libpath, tmp_path):
+    hdr = open(os.path.join(ROOT, "include", "hz3.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(hz3_[a-z_0-9]+)\s*\(", hdr))
+    lib = ctypes.CDLL(libpath)
+    for name in sorted(declared):
+        assert hasattr(lib, name), f"{name} declared in hz3.h but not exported"
+    from paper_2606_21695_b200 import hz3
+    assert set(hz3.EXPORTS) == declared
+    src = tmp_path / "sz3.c"
+    src.write_text('#include <stdio.h>\n#include "hz3.h"\nint main(void){printf("%zu %zu %zu\\n", sizeof(hz3_part_info),'
+                   ' sizeof(hz3_solve_opts), sizeof(hz3_solve_info));return 0;}\n')
+    exe = tmp_path / "sz3"
+    subprocess.check_call(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)])
+    a, b, c = map(int, subprocess.check_output([str(exe)]).split())
+    assert (a, b, c) == (ctypes.sizeof(hz3.hz3_part_info), ctypes.sizeof(hz3.hz3_solve_opts),
+                         ctypes.sizeof(hz3.hz3_solve_info))
+
+
 def test_ctypes_structs_match_header_sizes(libpath, tmp_path):
     """Compile a tiny C program against include/hz.h and compare sizeof() with the ctypes mirrors."""
     from paper_2606_21695_b200 import hz
