@@ -69,6 +69,11 @@ hz_status hz3_ddm_solve(hz3_ctx *ctx, const hz3_solve_opts *opts, void *u_out, h
  * u_dev: DEVICE, 2*npx*npy*npz values of precision `prec`. */
 hz_status hz3_residual(hz3_ctx *ctx, const void *u_dev, hz_prec prec, double *rel, void *stream);
 
+/* The paper's "operator time" normaliser ("the time it takes to evaluate the Helmholtz operator
+ * A - i w H - w^2 M on the entire domain"): `reps` back-to-back evaluations of the global operator (the kernel of
+ * hz3_residual, fp64) on u_dev (DEVICE, 2*npx*npy*npz doubles); *ms_per_eval = CUDA-event time / reps. */
+hz_status hz3_operator_time(hz3_ctx *ctx, const double *u_dev, int reps, double *ms_per_eval, void *stream);
+
 /* Raw per-subdomain state in fp64 (parity tests): u_sub DEVICE [L][2][N] (N = dofs_per_sub, node (i,j,k) at
  * (k*lny+j)*lnx+i), lam DEVICE [L][6][2][F]; either may be NULL. */
 hz_status hz3_get_subdomain_state(hz3_ctx *ctx, double *u_sub, double *lam);

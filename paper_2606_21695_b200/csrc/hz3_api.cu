@@ -339,6 +339,40 @@ hz_status hz3_residual(hz3_ctx *ctx, const void *u_dev, hz_prec prec, double *re
   return HZ_OK;
 }
 
+hz_status hz3_operator_time(hz3_ctx *ctx, const double *u_dev, int reps, double *ms_per_eval, void *stream) {
+  if (!ctx) return HZ_EINVAL;
+  if (!u_dev || !ms_per_eval || reps < 1) return fail3(ctx, HZ_EINVAL, "hz3_operator_time: NULL argument or reps < 1");
+  cudaStream_t st = (cudaStream_t)stream;
+  const Geo3 &g = ctx->g;
+  const long long total = (long long)g.npx * g.npy * g.npz;
+  const int nb = (int)((total + 255) / 256);
+  if (!ctx->d_part) {
+    HZ3_CUDA(cudaMalloc((void **)&ctx->d_part, (size_t)2 * nb * sizeof(double)));
+    HZ3_CUDA(cudaMalloc((void **)&ctx->d_red, 2 * sizeof(double)));
+  }
+  Ref1D ref{};
+  for (int a = 0; a <= g.p; ++a) {
+    ref.w[a] = ctx->gll.w[a];
+    for (int b = 0; b <= g.p; ++b) ref.K[a][b] = ctx->gll.K[a][b];
+  }
+  cudaEvent_t e0, e1;
+  HZ3_CUDA(cudaEventCreate(&e0));
+  HZ3_CUDA(cudaEventCreate(&e1));
+  k3_residual<double><<<nb, 256, 0, st>>>(g, ref, ctx->d_c, ctx->d_fre, ctx->d_fim, ctx->d_bc, u_dev, const_cast<double *>(u_dev), ctx->d_part);
+  cudaEventRecord(e0, st);
+  for (int r = 0; r < reps; ++r)
+    k3_residual<double><<<nb, 256, 0, st>>>(g, ref, ctx->d_c, ctx->d_fre, ctx->d_fim, ctx->d_bc, u_dev, const_cast<double *>(u_dev), ctx->d_part);
+  cudaEventRecord(e1, st);
+  cudaError_t ce = cudaStreamSynchronize(st);
+  float ms = 0.f;
+  if (ce == cudaSuccess) ce = cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  if (ce != cudaSuccess) return cuda_fail3(ctx, ce, "hz3_operator_time");
+  *ms_per_eval = ms / reps;
+  return HZ_OK;
+}
+
 hz_status hz3_get_subdomain_state(hz3_ctx *ctx, double *u_sub, double *lam) {
   if (!ctx) return HZ_EINVAL;
   if (!ctx->part) return fail3(ctx, HZ_ESTATE, "hz3_get_subdomain_state: call hz3_partition first");

@@ -7,7 +7,7 @@ import numpy as np
 
 from .hz import HZ_F32, HZ_F64, HZ_OK, HzError, _host_ptr, lib
 
-EXPORTS = ("hz3_mesh_setup", "hz3_partition", "hz3_ddm_solve", "hz3_residual", "hz3_get_subdomain_state",
+EXPORTS = ("hz3_mesh_setup", "hz3_partition", "hz3_ddm_solve", "hz3_residual", "hz3_operator_time", "hz3_get_subdomain_state",
            "hz3_last_error", "hz3_destroy")
 
 
@@ -40,6 +40,7 @@ def lib3():
         L.hz3_partition.argtypes = [vp, ip, ip, ip, ip, C.c_double, C.POINTER(hz3_part_info)]
         L.hz3_ddm_solve.argtypes = [vp, C.POINTER(hz3_solve_opts), vp, C.POINTER(hz3_solve_info), vp]
         L.hz3_residual.argtypes = [vp, vp, ip, C.POINTER(C.c_double), vp]
+        L.hz3_operator_time.argtypes = [vp, vp, ip, C.POINTER(C.c_double), vp]
         L.hz3_get_subdomain_state.argtypes = [vp, vp, vp]
         L.hz3_last_error.argtypes = [vp]
         L.hz3_last_error.restype = C.c_char_p
@@ -86,6 +87,13 @@ def hz3_residual(ctx, u_ptr, prec, stream=None):
     rel = C.c_double()
     _check(ctx, lib3().hz3_residual(ctx, C.c_void_p(u_ptr), prec, C.byref(rel), C.c_void_p(stream) if stream else None))
     return rel.value
+
+
+def hz3_operator_time(ctx, u_ptr, reps=20, stream=None):
+    """ms per evaluation of the global Helmholtz operator (fp64) on the device field at u_ptr."""
+    ms = C.c_double()
+    _check(ctx, lib3().hz3_operator_time(ctx, C.c_void_p(u_ptr), int(reps), C.byref(ms), C.c_void_p(stream) if stream else None))
+    return ms.value
 
 
 def hz3_get_subdomain_state(ctx, u_sub_ptr, lam_ptr):
