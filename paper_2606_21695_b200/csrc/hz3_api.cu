@@ -86,13 +86,20 @@ Sweep3Args<real> make_args3(const hz3_ctx *c, const hz3_solve_opts *o) {
 template <typename real>
 cudaError_t launch_sweep3(const hz3_ctx *c, const hz3_solve_opts *o, const TabC<real> &tc, cudaStream_t st) {
   void (*fn)(const Sweep3Args<real>, const TabC<real>) = nullptr;
+  // register cap by block size (the node's 3(2P+1) band coefficients live in registers)
+  const int sel = c->threads <= 256 ? 0 : (c->threads <= 512 ? 1 : 2);
+#define HZ3_CASE(P_)                                                                                            \
+  case P_:                                                                                                      \
+    fn = sel == 0 ? k3_sweep_dof<real, P_, 256> : (sel == 1 ? k3_sweep_dof<real, P_, 512> : k3_sweep_dof<real, P_, 1024>); \
+    break;
   switch (c->g.p) {
-    case 1: fn = k3_sweep_dof<real, 1>; break;
-    case 2: fn = k3_sweep_dof<real, 2>; break;
-    case 3: fn = k3_sweep_dof<real, 3>; break;
-    case 4: fn = k3_sweep_dof<real, 4>; break;
+    HZ3_CASE(1)
+    HZ3_CASE(2)
+    HZ3_CASE(3)
+    HZ3_CASE(4)
     default: return cudaErrorInvalidValue;
   }
+#undef HZ3_CASE
   cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem);
   if (e != cudaSuccess) return e;
   fn<<<c->L, c->threads, c->smem, st>>>(make_args3<real>(c, o), tc);
@@ -175,7 +182,7 @@ hz_status hz3_partition(hz3_ctx *ctx, int sx, int sy, int sz, hz_prec prec, doub
   g.theta = std::tan(g.omega * ctx->dt / 2.0) / g.omega;
   g.sigma = std::sin(g.omega * ctx->dt / 2.0) / (g.omega / 2.0);
   ctx->threads = g.NS;
-  ctx->smem = 2 * (size_t)(g.lnx + 2 * P) * (g.lny + 2 * P) * (g.lnz + 2 * P) * rs;
+  ctx->smem = 2 * (size_t)((N + 2 * P * (g.lnx * g.lny + g.lnx + 1) + 3) / 4 * 4) * rs;  // see k3_sweep_dof
   if (ctx->smem > 227 * 1024) return fail3(ctx, HZ_EUNSUPPORTED, "hz3_partition: subdomain volume exceeds shared memory");
   std::vector<double> tab((size_t)n_t * 4);
   const double tan2 = std::tan(M_PI / n_t) * std::tan(M_PI / n_t);

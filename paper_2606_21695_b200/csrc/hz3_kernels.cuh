@@ -108,22 +108,26 @@ __global__ void k3_build(Geo3 g, const double *__restrict__ c, const double *__r
 
 // ---------------------------------------------------------------------------------------------
 // The sweep: Algorithm 1 on every subdomain, one thread block per subdomain, one thread per
-// node.  p lives in two shared-memory volumes (ping-pong, zero halo of width P so the band rows need no bounds
-// checks); pdot, v_r, v_i, the coefficients and the node's three band rows stay in registers; one barrier per step.
+// node.  p lives in two shared-memory volumes (ping-pong); pdot, v_r, v_i, the coefficients and the node's three
+// band rows stay in registers; one barrier per step.  The volume is stored CONTIGUOUSLY (node t at word t, no halo
+// inside): a band row has zeros where it would leave the subdomain, so what such a read returns (a finite value of
+// another line, or the zero margin of P planes + P rows + P words before and after the volume) does not matter, and
+// consecutive lanes read consecutive words in all three directions — no bank conflicts.
 // ---------------------------------------------------------------------------------------------
-template <typename real, int P>
-__global__ void __launch_bounds__(1024) k3_sweep_dof(const Sweep3Args<real> A, const __grid_constant__ TabC<real> TC) {
+template <typename real, int P, int MAXT>
+__global__ void __launch_bounds__(MAXT) k3_sweep_dof(const Sweep3Args<real> A, const __grid_constant__ TabC<real> TC) {
   constexpr int B = 2 * P + 1;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   real *vol = reinterpret_cast<real *>(smem_raw);
   const Geo3 &g = A.g;
   const int t = threadIdx.x, l = blockIdx.x;
   const int N = g.lnx * g.lny * g.lnz;
-  const int SX = g.lnx + 2 * P, SXY = SX * (g.lny + 2 * P), VOL = SXY * (g.lnz + 2 * P);
+  const int SX = g.lnx, SXY = g.lnx * g.lny, MARG = P * (SXY + SX + 1);
+  const int VOL = (N + 2 * MARG + 3) / 4 * 4;
   for (int q = t; q < 2 * VOL; q += blockDim.x) vol[q] = real(0);
   const bool act = t < N;
   const int i = act ? t % g.lnx : 0, j = act ? (t / g.lnx) % g.lny : 0, k = act ? t / (g.lnx * g.lny) : 0;
-  const int pos = (k + P) * SXY + (j + P) * SX + (i + P);
+  const int pos = MARG + (act ? t : 0);
   real bx[B], by[B], bz[B];
 #pragma unroll
   for (int d = 0; d < B; ++d) {
