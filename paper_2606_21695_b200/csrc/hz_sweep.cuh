@@ -4,8 +4,11 @@
 // device-wide synchronisation.
 //
 // This file: k_sweep_dof, one DOF per thread (PAPER.md:191-207 re-designed).  p^nu lives in a ping-pong
-// shared-memory plane with a halo; each thread applies its own row of the assembled 1-D operators (2(2P+1)
-// shared loads, one shared store and ONE __syncthreads per time step; no atomics).  The register-blocked
+// shared-memory plane; each thread applies its own row of the assembled 1-D operators (2(2P+1)
+// shared loads, one shared store and ONE __syncthreads per time step; no atomics).  The plane is stored
+// contiguously (node t at word t): a band row is zero where it would leave the subdomain, so such a read may
+// return any finite value (the neighbouring line, or the zero margin of P rows + P words around the plane) and
+// consecutive lanes read consecutive words in both directions: no halo, no bounds checks, no bank conflicts.  The register-blocked
 // variants are in hz_sweep_tile.cuh (rectangular tiles, uniform code) and hz_sweep_ws.cuh (square tiles,
 // warp-specialised), the streamed fallback in hz_sweep_stream.cuh.
 // On the uniform rectangular elements of all configs the stiffness is  A = (hy/hx) Wy (x) Kx + (hx/hy) Ky (x) Wx
@@ -26,14 +29,15 @@ __global__ void __launch_bounds__(1024, 1) k_sweep_dof(const SweepArgs<real> A) 
   extern __shared__ __align__(16) unsigned char smem_raw[];
   Tab4<real> *tab = reinterpret_cast<Tab4<real> *>(smem_raw);
   const int lnx = A.lay.lnx, lny = A.lay.lny, N = lnx * lny, NS = A.lay.NS;
-  const int W = lnx + 2 * P, H = lny + 2 * P;
+  const int W = lnx, MARG = P * (lnx + 1);
+  const int PL = (N + 2 * MARG + 3) / 4 * 4;  // <= (lnx + 2P)(lny + 2P), the size the host reserves per plane
   real *pb0 = reinterpret_cast<real *>(tab + A.n_t);
-  real *pb1 = pb0 + W * H;
+  real *pb1 = pb0 + PL;
   const int t = threadIdx.x, NT = blockDim.x, l = blockIdx.x;
   const bool act = t < N;
   const int i = act ? t % lnx : 0, j = act ? t / lnx : 0;
 
-  for (int q = t; q < 2 * W * H; q += NT) pb0[q] = real(0);
+  for (int q = t; q < 2 * PL; q += NT) pb0[q] = real(0);
   for (int q = t; q < A.n_t; q += NT) tab[q] = A.tab[q];
 
   real cx[B], cy[B];
@@ -72,7 +76,7 @@ __global__ void __launch_bounds__(1024, 1) k_sweep_dof(const SweepArgs<real> A) 
   }
   __syncthreads();
 
-  const int center = (j + P) * W + (i + P);
+  const int center = MARG + (act ? t : 0);
   const real sigma = A.sigma;
   int par = 0;
   for (int m = 0; m < A.n_wh; ++m) {
