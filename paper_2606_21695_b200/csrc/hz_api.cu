@@ -531,7 +531,7 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
     int cst = n1 * (4 * n1 + roundup(3 * n1, v16));
     if ((cst / v16) % 2 == 0) cst += v16;
     const int nthr = roundup(ne, 32);
-    const size_t sm = (2 * (size_t)(nthr + 33) * rsw + (size_t)nthr * cst) * rs;
+    const size_t sm = (2 * (size_t)(nthr + 2) * rsw + (size_t)nthr * cst) * rs;
     if (sm > smem_cap) return fail(ctx, HZ_EUNSUPPORTED, "hz_partition: general quadrilaterals: the subdomain does not fit the shared memory of one SM");
     lay.variant = 3; lay.TX = lay.TY = P; lay.ntx = ctx->ex; lay.nty = ctx->ey; lay.NT = nthr; lay.NS = roundup(N, 32);
     ctx->lay = lay; ctx->mx = ctx->my = 1; ctx->csm = 1; ctx->ws = 0; ctx->cl = 1;

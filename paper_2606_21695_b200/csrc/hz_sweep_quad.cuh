@@ -33,7 +33,7 @@ __global__ void __launch_bounds__(MAXT, MINB)
   constexpr int oW = 0, oE = CH, oS = 2 * CH, oN = 3 * CH;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int t = threadIdx.x, NT = blockDim.x, l = blockIdx.x;
-  const int BUFW = (NT + 33) * RS;
+  const int BUFW = (NT + 2) * RS;  // + one all-zero record (missing neighbours; a broadcast read) + one scratch record
   real *xb = reinterpret_cast<real *>(smem_raw);
   real *csm = xb + 2 * BUFW + (size_t)t * CST;
   // ex = element stride of the thread grid (the widest subdomain); exl x eyl = this subdomain's elements (ragged
@@ -44,12 +44,12 @@ __global__ void __launch_bounds__(MAXT, MINB)
   const int lnxl = exl * P + 1, lnyl = eyl * P + 1;
   const bool act = t < ex * A.lay.nty && t % ex < exl && t / ex < eyl;
   const int fx = act ? t % ex : 0, fy = act ? t / ex : 0;
-  const int ZR = NT, SCR = NT + 32;
+  const int ZR = NT, SCR = NT + 1;
 
   for (int q = t; q < 2 * BUFW; q += NT) xb[q] = real(0);
 
   const bool hasL = act && fx > 0, hasR = act && fx < exl - 1, hasD = act && fy > 0, hasU = act && fy < eyl - 1;
-  auto rec = [&](bool has, int nb) { return xb + (has ? nb : ZR + (nb & 31)) * RS; };
+  auto rec = [&](bool has, int nb) { return xb + (has ? nb : ZR) * RS; };
   const real *pL = rec(hasL, t - 1) + oE, *pR = rec(hasR, t + 1) + oW;
   const real *pD = rec(hasD, t - ex) + oN, *pU = rec(hasU, t + ex) + oS;
   const real *pDL = rec(hasD && hasL, t - ex - 1) + oE + P, *pDR = rec(hasD && hasR, t - ex + 1) + oW + P;
