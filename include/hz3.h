@@ -3,8 +3,9 @@
  *
  * Same method as include/hz.h on a uniform mesh of nx*ny*nz hexahedra of degree p on a box: spectral elements with
  * GLL quadrature, sx*sy*sz box subdomains with the impedance transmission condition on all six
- * faces, one thread block per subdomain and one thread per subdomain node (at most
- * 1024 nodes per subdomain), WaveHoltz as the subdomain solver (Algorithm 1).
+ * faces, one thread block per subdomain and one thread per subdomain node or per column of nodes
+ * (at most 1024 nodes per subdomain), WaveHoltz as the subdomain solver (Algorithm 1,
+ * PAPER.md:160-183).
  *
  * Plain pointers, no torch types.  HOST = host memory read during the call; DEVICE = device memory owned by the caller.
  * Node (I,J,K) of the global mesh has the flat index (K*npy + J)*npx + I (npx = nx*p+1, ...).  Faces are ordered
@@ -35,7 +36,8 @@ typedef struct {
   int dofs_per_sub;      /* lnx*lny*lnz */
   int lnx, lny, lnz;     /* nodes per subdomain side */
   int face_stride;       /* F = max(lny*lnz, lnx*lnz, lnx*lny): stride of one face in lambda arrays */
-  int threads_per_block; /* dofs_per_sub rounded up to a warp */
+  int threads_per_block; /* nodes (one-node-per-thread kernel) or (i,j) node columns (column kernel), rounded to a warp */
+  int nodes_per_thread;  /* 1, or lnz: one thread per node column along z with its nodes in registers */
   int blocks;            /* sx*sy*sz */
   double dt, theta, sigma;
   size_t smem_bytes, workspace_bytes;

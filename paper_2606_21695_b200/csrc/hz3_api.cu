@@ -1,6 +1,7 @@
 // hz3_api.cu — C-ABI entry points of include/hz3.h: the 3-D hexahedral variant.
 // Host-side setup (GLL tables, time-step tables, partition) and the outer driver on one stream.
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -24,8 +25,10 @@ struct hz3_ctx {
   void *d_usub = nullptr, *d_lam = nullptr, *d_g = nullptr, *d_k2 = nullptr, *d_bs = nullptr;
   void *d_bx = nullptr, *d_by = nullptr, *d_bz = nullptr;
   double *d_wx = nullptr, *d_wy = nullptr, *d_wz = nullptr, *d_part = nullptr, *d_red = nullptr, *d_u64 = nullptr;
-  int threads = 0;
+  int threads = 0, colz = 0;  // colz > 0: column kernel with colz nodes per thread
   size_t smem = 0, ws_bytes = 0;
+  BandZ<float> bz32{};
+  BandZ<double> bz64{};
   TabC<float> tc32{};
   TabC<double> tc64{};
   std::string err;
@@ -106,6 +109,38 @@ cudaError_t launch_sweep3(const hz3_ctx *c, const hz3_solve_opts *o, const TabC<
   return cudaGetLastError();
 }
 
+// compiled (P, LNZ) pairs of the column kernel: LNZ = ez*P + 1 for the block shapes of PAPER.md:265
+bool col_supported(int P, int lnz) {
+  switch (P) {
+    case 1: return lnz == 3 || lnz == 5 || lnz == 9;
+    case 2: return lnz == 5 || lnz == 9;
+    case 3: return lnz == 4 || lnz == 7 || lnz == 10;
+    case 4: return lnz == 5 || lnz == 9;
+    default: return false;
+  }
+}
+
+template <typename real>
+cudaError_t launch_sweep3_col(const hz3_ctx *c, const hz3_solve_opts *o, const BandZ<real> &bz, const TabC<real> &tc,
+                              cudaStream_t st) {
+  void (*fn)(const Sweep3Args<real>, const BandZ<real>, const TabC<real>) = nullptr;
+  const int key = c->g.p * 100 + c->colz;
+#define HZ3_COL(P_, Z_) \
+  case P_ * 100 + Z_: fn = k3_sweep_col<real, P_, Z_, 128>; break;
+  switch (key) {
+    HZ3_COL(1, 3) HZ3_COL(1, 5) HZ3_COL(1, 9)
+    HZ3_COL(2, 5) HZ3_COL(2, 9)
+    HZ3_COL(3, 4) HZ3_COL(3, 7) HZ3_COL(3, 10)
+    HZ3_COL(4, 5) HZ3_COL(4, 9)
+    default: return cudaErrorInvalidValue;
+  }
+#undef HZ3_COL
+  cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)c->smem);
+  if (e != cudaSuccess) return e;
+  fn<<<c->L, c->threads, c->smem, st>>>(make_args3<real>(c, o), bz, tc);
+  return cudaGetLastError();
+}
+
 }  // namespace
 
 extern "C" {
@@ -182,6 +217,12 @@ hz_status hz3_partition(hz3_ctx *ctx, int sx, int sy, int sz, hz_prec prec, doub
   g.theta = std::tan(g.omega * ctx->dt / 2.0) / g.omega;
   g.sigma = std::sin(g.omega * ctx->dt / 2.0) / (g.omega / 2.0);
   ctx->threads = g.NS;
+  ctx->colz = 0;
+  const char *env_col = std::getenv("HZ3_DISABLE_COL");  // debug knob: always the one-node-per-thread kernel
+  if (!(env_col && env_col[0] == '1') && col_supported(P, g.lnz) && g.lnx * g.lny <= 128) {
+    ctx->colz = g.lnz;
+    ctx->threads = roundup3(g.lnx * g.lny, 32);
+  }
   ctx->smem = 2 * (size_t)((N + 2 * P * (g.lnx * g.lny + g.lnx + 1) + 3) / 4 * 4) * rs;  // see k3_sweep_dof
   if (ctx->smem > 227 * 1024) return fail3(ctx, HZ_EUNSUPPORTED, "hz3_partition: subdomain volume exceeds shared memory");
   std::vector<double> tab((size_t)n_t * 4);
@@ -200,6 +241,12 @@ hz_status hz3_partition(hz3_ctx *ctx, int sx, int sy, int sz, hz_prec prec, doub
   make_band(ctx->gll, g.ex, g.hx, &bx, &wx);
   make_band(ctx->gll, g.ey, g.hy, &by, &wy);
   make_band(ctx->gll, g.ez, g.hz, &bz, &wz);
+  if (ctx->colz)
+    for (int k = 0; k < g.lnz; ++k)
+      for (int d = 0; d < 2 * P + 1; ++d) {
+        ctx->bz32.z[k][d] = (float)bz[(size_t)k * (2 * P + 1) + d];
+        ctx->bz64.z[k][d] = bz[(size_t)k * (2 * P + 1) + d];
+      }
   const size_t LS = (size_t)ctx->L * g.NS, lam_n = (size_t)ctx->L * 12 * g.F, face_n = (size_t)ctx->L * 6 * g.F;
   size_t ws = 0;
   auto alloc0 = [&](void **ptr, size_t bytes) -> cudaError_t {
@@ -244,7 +291,7 @@ hz_status hz3_partition(hz3_ctx *ctx, int sx, int sy, int sz, hz_prec prec, doub
   if (info) {
     hz3_part_info inf{};
     inf.n_t = n_t; inf.dofs_per_sub = N; inf.lnx = g.lnx; inf.lny = g.lny; inf.lnz = g.lnz; inf.face_stride = g.F;
-    inf.threads_per_block = ctx->threads; inf.blocks = ctx->L;
+    inf.threads_per_block = ctx->threads; inf.blocks = ctx->L; inf.nodes_per_thread = ctx->colz ? ctx->colz : 1;
     inf.dt = ctx->dt; inf.theta = g.theta; inf.sigma = g.sigma;
     inf.smem_bytes = ctx->smem; inf.workspace_bytes = ws;
     *info = inf;
@@ -275,8 +322,13 @@ hz_status hz3_ddm_solve(hz3_ctx *ctx, const hz3_solve_opts *opts, void *u_out, h
   const unsigned nbx = (unsigned)((lam_n + 255) / 256);
   for (int it = 0; it < n && ce == cudaSuccess; ++it) {
     ce = cudaEventRecord(ev[2 * it], st);
-    if (ce == cudaSuccess)
-      ce = ctx->prec == HZ_F32 ? launch_sweep3<float>(ctx, opts, ctx->tc32, st) : launch_sweep3<double>(ctx, opts, ctx->tc64, st);
+    if (ce == cudaSuccess) {
+      if (ctx->colz)
+        ce = ctx->prec == HZ_F32 ? launch_sweep3_col<float>(ctx, opts, ctx->bz32, ctx->tc32, st)
+                                 : launch_sweep3_col<double>(ctx, opts, ctx->bz64, ctx->tc64, st);
+      else
+        ce = ctx->prec == HZ_F32 ? launch_sweep3<float>(ctx, opts, ctx->tc32, st) : launch_sweep3<double>(ctx, opts, ctx->tc64, st);
+    }
     if (ce == cudaSuccess) ce = cudaEventRecord(ev[2 * it + 1], st);
     if (ce != cudaSuccess) break;
     if (ctx->prec == HZ_F32) k3_exchange<float><<<nbx, 256, 0, st>>>(g, (float)opts->relax, (float *)ctx->d_lam, (const float *)ctx->d_g);

@@ -196,6 +196,121 @@ __global__ void __launch_bounds__(MAXT) k3_sweep_dof(const Sweep3Args<real> A, c
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// Column variant: one thread per (i,j) node COLUMN, its LNZ nodes along z in registers (state and coefficients).
+// The z part of the operator is then register-only, with the band coefficients of the z direction as compile-time
+// offsets into a by-value kernel parameter (constant bank operands); x and y parts read the shared volume as in
+// k3_sweep_dof.  One third fewer shared loads per DOF and LNZ times fewer threads per barrier.
+// ---------------------------------------------------------------------------------------------
+constexpr int kColMaxZ = 10;
+template <typename real>
+struct BandZ {
+  real z[kColMaxZ][2 * kMaxP + 1];  // z[k][d] = band row of z-node k (zero outside the subdomain)
+};
+
+template <typename real, int P, int LNZ, int MAXT>
+__global__ void __launch_bounds__(MAXT) k3_sweep_col(const Sweep3Args<real> A, const __grid_constant__ BandZ<real> BZ,
+                                                     const __grid_constant__ TabC<real> TC) {
+  constexpr int B = 2 * P + 1;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  real *vol = reinterpret_cast<real *>(smem_raw);
+  const Geo3 &g = A.g;
+  const int t = threadIdx.x, l = blockIdx.x;
+  const int SX = g.lnx, SXY = g.lnx * g.lny, N = SXY * LNZ, MARG = P * (SXY + SX + 1);
+  const int VOL = (N + 2 * MARG + 3) / 4 * 4;
+  for (int q = t; q < 2 * VOL; q += blockDim.x) vol[q] = real(0);
+  const bool act = t < SXY;
+  const int i = act ? t % g.lnx : 0, j = act ? t / g.lnx : 0;
+  const int pos = MARG + (act ? t : 0);
+  real bx[B], by[B];
+#pragma unroll
+  for (int d = 0; d < B; ++d) {
+    bx[d] = act ? A.bandx[i * B + d] : real(0);
+    by[d] = act ? A.bandy[j * B + d] : real(0);
+  }
+  real gam[LNZ], alp[LNZ], br[LNZ], bi[LNZ], ur[LNZ], ui[LNZ];
+#pragma unroll
+  for (int k = 0; k < LNZ; ++k) {
+    gam[k] = alp[k] = br[k] = bi[k] = ur[k] = ui[k] = real(0);
+    if (act) {
+      const size_t o = (size_t)l * g.NS + (size_t)k * SXY + t;
+      gam[k] = A.gamma[o]; alp[k] = A.alpha[o]; br[k] = A.bbf_re[o];
+      bi[k] = A.bbf_im ? A.bbf_im[o] : real(0);
+      for (int f = 0; f < 6; ++f)  // b from lambda^n on the interface faces (R13)
+        if (on_face(g, f, i, j, k) && face_neighbour(g, l, f) >= 0) {
+          const int e = face_node(g, f, i, j, k);
+          const real s = A.bs[((size_t)l * 6 + f) * g.F + e];
+          br[k] = fmaT(s, A.lam[((size_t)(l * 6 + f) * 2 + 0) * g.F + e], br[k]);
+          bi[k] = fmaT(s, A.lam[((size_t)(l * 6 + f) * 2 + 1) * g.F + e], bi[k]);
+        }
+      if (A.warm) {
+        ur[k] = A.u_sub[(size_t)l * 2 * g.NS + (size_t)k * SXY + t];
+        ui[k] = A.u_sub[(size_t)l * 2 * g.NS + g.NS + (size_t)k * SXY + t];
+      }
+    }
+  }
+  __syncthreads();
+  int cur = 0;
+  real p[LNZ], pd[LNZ], vr[LNZ], vi[LNZ];
+  for (int m = 0; m < A.n_wh; ++m) {
+    const Tab4<real> t0 = A.n_t <= kTabCMax ? TC.t[0] : A.tab[0];
+#pragma unroll
+    for (int k = 0; k < LNZ; ++k) {  // PAPER.md:168-170; readings R2, R8
+      p[k] = ur[k];
+      pd[k] = A.omega * (ui[k] * A.cos_h - ur[k] * A.sin_h);
+      vr[k] = t0.k * p[k];
+      vi[k] = t0.kh * pd[k];
+    }
+#pragma unroll 1
+    for (int nu = 1; nu < A.n_t; ++nu) {
+      const Tab4<real> tn = A.n_t <= kTabCMax ? TC.t[nu] : A.tab[nu];
+      real *buf = vol + cur + pos;
+#pragma unroll
+      for (int k = 0; k < LNZ; ++k) {
+        p[k] = fmaT(A.sigma, pd[k], p[k]);
+        if (act) buf[k * SXY] = p[k];
+      }
+      __syncthreads();
+#pragma unroll
+      for (int k = 0; k < LNZ; ++k) {
+        const real *c = buf + k * SXY;
+        real Sx = real(0), Sy = real(0), Sz = real(0);
+#pragma unroll
+        for (int d = 0; d < B; ++d) {
+          Sx = fmaT(bx[d], c[d - P], Sx);
+          Sy = fmaT(by[d], c[(d - P) * SX], Sy);
+          if (k + d - P >= 0 && k + d - P < LNZ) Sz = fmaT(BZ.z[k][d], p[k + d - P < 0 ? 0 : (k + d - P >= LNZ ? 0 : k + d - P)], Sz);
+        }
+        const real S = (Sx + Sy) + Sz;
+        const real x = fmaT(bi[k], tn.s, fmaT(-gam[k], S, br[k] * tn.c));
+        pd[k] = fmaT(alp[k], pd[k], x);
+        vr[k] = fmaT(tn.k, p[k], vr[k]);
+        vi[k] = fmaT(tn.kh, pd[k], vi[k]);
+      }
+      cur = VOL - cur;
+    }
+#pragma unroll
+    for (int k = 0; k < LNZ; ++k) {  // eq. (7) prefactor (reading R4)
+      ur[k] = A.two_over_nt * vr[k];
+      ui[k] = A.two_over_nt * vi[k];
+    }
+  }
+  if (!act) return;
+#pragma unroll
+  for (int k = 0; k < LNZ; ++k) {
+    A.u_sub[(size_t)l * 2 * g.NS + (size_t)k * SXY + t] = ur[k];
+    A.u_sub[(size_t)l * 2 * g.NS + g.NS + (size_t)k * SXY + t] = ui[k];
+    for (int f = 0; f < 6; ++f)  // g = -lambda^n - 2 i k u (eq. (2), sign per reading R3)
+      if (on_face(g, f, i, j, k) && face_neighbour(g, l, f) >= 0) {
+        const int e = face_node(g, f, i, j, k);
+        const real k2 = A.k2face[((size_t)l * 6 + f) * g.F + e];
+        const size_t a = ((size_t)(l * 6 + f) * 2) * g.F + e;
+        A.gout[a] = fmaT(k2, ui[k], -A.lam[a]);
+        A.gout[a + g.F] = fmaT(-k2, ur[k], -A.lam[a + g.F]);
+      }
+  }
+}
+
 // A8 in 3-D: lambda^{n+1}_{r,o} = (1-rho) lambda^n_{r,o} + rho g_{nb(r,o), opp(o)}; one thread per lambda entry.
 template <typename real>
 __global__ void k3_exchange(Geo3 g, real rho, real *__restrict__ lam, const real *__restrict__ gg) {

@@ -13,7 +13,7 @@ EXPORTS = ("hz3_mesh_setup", "hz3_partition", "hz3_ddm_solve", "hz3_residual", "
 
 class hz3_part_info(C.Structure):
     _fields_ = [("n_t", C.c_int), ("dofs_per_sub", C.c_int), ("lnx", C.c_int), ("lny", C.c_int), ("lnz", C.c_int),
-                ("face_stride", C.c_int), ("threads_per_block", C.c_int), ("blocks", C.c_int),
+                ("face_stride", C.c_int), ("threads_per_block", C.c_int), ("nodes_per_thread", C.c_int), ("blocks", C.c_int),
                 ("dt", C.c_double), ("theta", C.c_double), ("sigma", C.c_double),
                 ("smem_bytes", C.c_size_t), ("workspace_bytes", C.c_size_t)]
 

@@ -83,9 +83,19 @@ def check_case(inp, prec, n_outer=2, n_wh=2, warm=True, relax=0.5, bc=None):
 
 @pytest.mark.parametrize("prec", [hz.HZ_F64, hz.HZ_F32])
 @pytest.mark.parametrize("p,n,s", [(1, 8, 4), (2, 4, 2), (3, 4, 2), (4, 2, 1)])
-def test_cube_all_degrees(prec, p, n, s):
+@pytest.mark.parametrize("col", [True, False])
+def test_cube_all_degrees(prec, p, n, s, col, monkeypatch):
+    # col: one thread per node column along z (k3_sweep_col); else one thread per node (k3_sweep_dof)
+    monkeypatch.setenv("HZ3_DISABLE_COL", "0" if col else "1")
     info = check_case(make_config_3d(n, p, s, seed=3000 + p), prec, n_outer=3, n_wh=2)
     assert info.dofs_per_sub == (s * p + 1) ** 3 and info.blocks == (n // s) ** 3
+    assert info.nodes_per_thread == (s * p + 1 if col else 1)
+
+
+def test_column_kernel_falls_back_when_the_column_length_is_not_compiled():
+    # 3 elements of degree 2 along z: lnz = 7 is not an instantiated column length for p = 2 -> one node per thread
+    info = check_case(make_config_3d((2, 2, 3), 2, (2, 2, 3), seed=8), hz.HZ_F64, n_outer=2, n_wh=2)
+    assert info.nodes_per_thread == 1
 
 
 def test_anisotropic_box_boundary_data_complex_source_cold_start():
