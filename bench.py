@@ -397,6 +397,36 @@ def run_extras(hz, torch, args, flush, stream):
             hz.hz_destroy(ctx)
         except Exception as e:
             out[key] = {"error": str(e)}
+    # the rows SURVEY.md 8(f) marks "next": general convex quads (F3) and 3-D hexahedra (F4), sweep kernel only
+    try:
+        inp = make_config(3, n=args.n, distort=0.2)
+        ctx, pinfo = hz.setup_from_inputs(inp, hz.HZ_F32, 0)
+        hz.hz_ddm_solve(ctx, 2, n_wh=N_WH, reset_state=True, stream=stream)
+        tot, swp, exc, _, units = time_sweeps(hz, torch, ctx, 3, 1, flush, stream)
+        rate = units / (sum(swp) * 1e-3)
+        out["config3_general_quads_f32"] = {
+            "dof_steps_per_s_sweep_kernel": rate, "sweep_ms": sum(swp) / 3, "n_t": pinfo.n_t, "kernel": "k_sweep_quad",
+            "frac_of_derived_peak": rate * flops_per_dof_step(inp.p, True) / (SMS * FP32_LANES * 2 * 1965e6)}
+        hz.hz_destroy(ctx)
+    except Exception as e:
+        out["config3_general_quads_f32"] = {"error": str(e)}
+    try:
+        from paper_2606_21695_b200 import hz3
+        from paper_2606_21695_b200.inputs import make_config_3d
+        for name, n, p, s in (("hex_128cubed_p1_sub8", 128, 1, 8), ("hex_48cubed_p3_sub3", 48, 3, 3)):
+            i3 = make_config_3d(n, p, s)
+            c3 = hz3.hz3_mesh_setup(i3.nx, i3.ny, i3.nz, i3.box, i3.p, i3.c_nodes, i3.omega, i3.f_re)
+            try:
+                info3 = hz3.hz3_partition(c3, i3.sx, i3.sy, i3.sz, hz.HZ_F32)
+                hz3.hz3_ddm_solve(c3, 1, n_wh=N_WH, reset_state=True, stream=stream)
+                r = hz3.hz3_ddm_solve(c3, 3, n_wh=N_WH, stream=stream)
+                out[name + "_f32"] = {"dof_steps_per_s_sweep_kernel": r.dof_timesteps / (r.sweep_ms_total * 1e-3),
+                                      "sweep_ms": r.sweep_ms_total / 3, "n_t": info3.n_t,
+                                      "nodes_per_thread": info3.nodes_per_thread, "blocks": info3.blocks}
+            finally:
+                hz3.hz3_destroy(c3)
+    except Exception as e:
+        out["hex_3d"] = {"error": str(e)}
     return out
 
 

@@ -143,12 +143,13 @@ def mapped_node_coords(p: int, VX: np.ndarray, VY: np.ndarray):
     XI, ETA = np.meshgrid(xi, xi, indexing="xy")
     X = np.zeros((ny * p + 1, nx * p + 1))
     Y = np.zeros_like(X)
-    for fy in range(ny):
-        for fx in range(nx):
+    for b in range(p + 1):          # local node (a,b) of every element at once
+        for a in range(p + 1):
+            n00, n10 = (1 - xi[a]) * (1 - xi[b]) / 4.0, (1 + xi[a]) * (1 - xi[b]) / 4.0
+            n01, n11 = (1 - xi[a]) * (1 + xi[b]) / 4.0, (1 + xi[a]) * (1 + xi[b]) / 4.0
             for Z, V in ((X, VX), (Y, VY)):
-                Z[fy * p:fy * p + p + 1, fx * p:fx * p + p + 1] = (
-                    (1 - XI) * (1 - ETA) * V[fy, fx] + (1 + XI) * (1 - ETA) * V[fy, fx + 1]
-                    + (1 - XI) * (1 + ETA) * V[fy + 1, fx] + (1 + XI) * (1 + ETA) * V[fy + 1, fx + 1]) / 4.0
+                Z[b:b + (ny - 1) * p + 1:p, a:a + (nx - 1) * p + 1:p] = (
+                    n00 * V[:-1, :-1] + n10 * V[:-1, 1:] + n01 * V[1:, :-1] + n11 * V[1:, 1:])
     return X, Y
 
 
