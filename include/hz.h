@@ -172,6 +172,31 @@ typedef struct {
 hz_status hz_ddm_solve(hz_ctx *ctx, const hz_solve_opts *opts, void *u_out, hz_solve_info *info, void *stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * hz_ddm_solve_sources — a stream of right-hand sides on one mesh and partition, end to end from HOST to HOST:
+ * for s = 0..n_src-1: copy source f_s to the device, rebuild the load ("Assemble b from f"), run
+ * opts->n_outer_max {sweep, exchange} pairs (continuing from the current lambda / u_l unless opts->reset_state),
+ * gather the field and copy it to u_host[s].  The copies run on two private streams with double-buffered staging, so
+ * the upload of source s+1 and the download of field s-1 overlap the sweeps of source s; the results are bit-identical
+ * to hz_set_source + hz_ddm_solve + a device-to-host copy, source by source.
+ *
+ *   f_re_host  n_src HOST pointers, (nx*p+1)*(ny*p+1) doubles each (pinned memory for the copies to overlap);
+ *              real sources only (HZ_EUNSUPPORTED if the context has an imaginary source).
+ *   u_host     n_src HOST pointers, 2*(nx*p+1)*(ny*p+1) values of the PARTITION's precision each (re, then im).
+ *   opts       n_outer_max (>= 1), n_wh, warm_start, relax, reset_state are used; no tolerance check.
+ *   info       optional; total_ms = CUDA-event time from the first upload to the last download.
+ * On return all copies have completed and the context holds the last source.
+ * ------------------------------------------------------------------------------------------- */
+typedef struct {
+  int sources_done;
+  double total_ms;
+  double dof_timesteps;        /* all sources together */
+  int launches;                /* kernels launched (build + sweeps + exchanges + gather per source) */
+  double h2d_bytes, d2h_bytes; /* copied in total */
+} hz_sources_info;
+hz_status hz_ddm_solve_sources(hz_ctx *ctx, const hz_solve_opts *opts, int n_src, const double *const *f_re_host,
+                               void *const *u_host, hz_sources_info *info, void *stream);
+
+/* ---------------------------------------------------------------------------------------------
  * hz_ddm_solve_gmres — Krylov acceleration of the outer iteration (the fixed-point iteration on
  * lambda "can be accelerated with a Krylov space method").  One warm-started sweep (sweep kernel + exchange
  * kernel, exactly as in hz_ddm_solve) is an affine, real-linear map x -> T x + c of the joint state

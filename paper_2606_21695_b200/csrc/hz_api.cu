@@ -74,6 +74,12 @@ struct hz_ctx {
   long long n_state = 0;
   cudaGraphExec_t g_exec = nullptr;
   cudaStream_t cap_stream = nullptr;  // capture happens on this private stream (the legacy default stream cannot capture)
+  // hz_ddm_solve_sources: copy-in / copy-out streams, double-buffered staging and the events that order them
+  cudaStream_t s_in = nullptr, s_out = nullptr;
+  double *d_fstage[2] = {nullptr, nullptr};
+  void *d_ubuf[2] = {nullptr, nullptr};
+  cudaEvent_t ev_up[2] = {nullptr, nullptr}, ev_build[2] = {nullptr, nullptr}, ev_gather[2] = {nullptr, nullptr},
+              ev_down[2] = {nullptr, nullptr};
   int g_chunk = 0, g_nwh = 0, g_warm = 0;
   double g_relax = 0;
   std::vector<double> h_tab;  // host copy of the time-step table (kernel-parameter form of the ws kernel)
@@ -125,12 +131,13 @@ Geo make_geo(const hz_ctx *c) {
 }
 
 template <typename real>
-hz_status run_build(hz_ctx *ctx, int only_source, cudaStream_t st) {
+hz_status run_build(hz_ctx *ctx, int only_source, cudaStream_t st, const double *f_re = nullptr) {
+  if (!f_re) f_re = ctx->d_fre;  // hz_ddm_solve_sources builds from its staging buffers
   const long long total = (long long)ctx->L * ctx->lay.lnx * ctx->lay.lny;
   const int bs = 256;
   const unsigned nb = (unsigned)((total + bs - 1) / bs);
   if (ctx->general) {
-    k_build_quad<real><<<nb, bs, 0, st>>>(make_geo(ctx), ctx->lay, ctx->refq, ctx->d_vx, ctx->d_vy, ctx->d_c, ctx->d_fre,
+    k_build_quad<real><<<nb, bs, 0, st>>>(make_geo(ctx), ctx->lay, ctx->refq, ctx->d_vx, ctx->d_vy, ctx->d_c, f_re,
                                           ctx->d_fim, ctx->d_bc, (real *)ctx->d_gamma, (real *)ctx->d_alpha,
                                           (real *)ctx->d_bbf_re, (real *)ctx->d_bbf_im, (real *)ctx->d_k2,
                                           (real *)ctx->d_bs, only_source);
@@ -144,7 +151,7 @@ hz_status run_build(hz_ctx *ctx, int only_source, cudaStream_t st) {
     }
     return HZ_OK;
   }
-  k_build<real><<<nb, bs, 0, st>>>(make_geo(ctx), ctx->lay, ctx->d_c, ctx->d_fre, ctx->d_fim, ctx->d_bc, ctx->d_wxl,
+  k_build<real><<<nb, bs, 0, st>>>(make_geo(ctx), ctx->lay, ctx->d_c, f_re, ctx->d_fim, ctx->d_bc, ctx->d_wxl,
                                    ctx->d_wyl, (real *)ctx->d_gamma, (real *)ctx->d_alpha, (real *)ctx->d_bbf_re,
                                    (real *)ctx->d_bbf_im, (real *)ctx->d_k2, (real *)ctx->d_bs, only_source);
   HZ_CUDA(cudaGetLastError());
@@ -795,6 +802,96 @@ hz_status hz_ddm_solve(hz_ctx *ctx, const hz_solve_opts *opts, void *u_out, hz_s
   return HZ_OK;
 }
 
+hz_status hz_ddm_solve_sources(hz_ctx *ctx, const hz_solve_opts *opts, int n_src, const double *const *f_re_host,
+                               void *const *u_host, hz_sources_info *info, void *stream) {
+  if (!ctx) return HZ_EINVAL;
+  if (!opts || !f_re_host || !u_host || n_src < 1) return fail(ctx, HZ_EINVAL, "hz_ddm_solve_sources: NULL argument or n_src < 1");
+  if (!ctx->part) return fail(ctx, HZ_ESTATE, "hz_ddm_solve_sources: call hz_partition first");
+  if (opts->n_outer_max < 1 || opts->n_wh < 1 || !(opts->relax > 0.0) || opts->relax > 1.0)
+    return fail(ctx, HZ_EINVAL, "hz_ddm_solve_sources: need n_outer_max >= 1, n_wh >= 1, relax in (0,1]");
+  if (ctx->d_fim) return fail(ctx, HZ_EUNSUPPORTED, "hz_ddm_solve_sources: real sources only (the context has an imaginary part)");
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t rs = ctx->prec == HZ_F32 ? 4 : 8;
+  const size_t nn = (size_t)ctx->npx * ctx->npy;
+  if (!ctx->s_in) {
+    HZ_CUDA(cudaStreamCreateWithFlags(&ctx->s_in, cudaStreamNonBlocking));
+    HZ_CUDA(cudaStreamCreateWithFlags(&ctx->s_out, cudaStreamNonBlocking));
+    for (int b = 0; b < 2; ++b) {
+      HZ_CUDA(cudaMalloc((void **)&ctx->d_fstage[b], nn * sizeof(double)));
+      HZ_CUDA(cudaEventCreateWithFlags(&ctx->ev_up[b], cudaEventDisableTiming));
+      HZ_CUDA(cudaEventCreateWithFlags(&ctx->ev_build[b], cudaEventDisableTiming));
+      HZ_CUDA(cudaEventCreateWithFlags(&ctx->ev_gather[b], cudaEventDisableTiming));
+      HZ_CUDA(cudaEventCreateWithFlags(&ctx->ev_down[b], cudaEventDisableTiming));
+    }
+  }
+  for (int b = 0; b < 2; ++b) {  // the gathered field has the partition's precision, which may have changed
+    if (ctx->d_ubuf[b]) cudaFree(ctx->d_ubuf[b]);
+    ctx->d_ubuf[b] = nullptr;
+    HZ_CUDA(cudaMalloc(&ctx->d_ubuf[b], 2 * nn * rs));
+  }
+  cudaEvent_t e0, e1;
+  HZ_CUDA(cudaEventCreate(&e0));
+  HZ_CUDA(cudaEventCreate(&e1));
+  cudaError_t ce = cudaEventRecord(e0, st);
+  if (ce == cudaSuccess) ce = cudaStreamWaitEvent(ctx->s_in, e0, 0);
+  int launches = 0;
+  for (int s = 0; s < n_src && ce == cudaSuccess; ++s) {
+    const int b = s & 1;
+    if (!f_re_host[s] || !u_host[s]) { ce = cudaErrorInvalidValue; break; }
+    // copy-in stream: source s into staging buffer b, once the build of source s-2 has consumed it
+    if (s >= 2) ce = cudaStreamWaitEvent(ctx->s_in, ctx->ev_build[b], 0);
+    if (ce == cudaSuccess) ce = cudaMemcpyAsync(ctx->d_fstage[b], f_re_host[s], nn * sizeof(double), cudaMemcpyHostToDevice, ctx->s_in);
+    if (ce == cudaSuccess) ce = cudaEventRecord(ctx->ev_up[b], ctx->s_in);
+    // compute stream: rebuild beta*b from the staged source, sweeps, gather
+    if (ce == cudaSuccess) ce = cudaStreamWaitEvent(st, ctx->ev_up[b], 0);
+    if (ce != cudaSuccess) break;
+    hz_status bst = ctx->prec == HZ_F32 ? run_build<float>(ctx, 1, st, ctx->d_fstage[b]) : run_build<double>(ctx, 1, st, ctx->d_fstage[b]);
+    if (bst != HZ_OK) { cudaEventDestroy(e0); cudaEventDestroy(e1); return bst; }
+    ce = cudaEventRecord(ctx->ev_build[b], st);
+    ++launches;
+    if (ce == cudaSuccess && opts->reset_state) {
+      ce = cudaMemsetAsync(ctx->d_lam, 0, (size_t)ctx->n_state * rs, st);
+      if (ce == cudaSuccess) ce = cudaMemsetAsync(ctx->d_g, 0, (size_t)ctx->L * 8 * ctx->E * rs, st);
+    }
+    for (int it = 0; it < opts->n_outer_max && ce == cudaSuccess; ++it) {
+      ce = launch_sweep(ctx, opts, st);
+      if (ce == cudaSuccess) ce = launch_exchange(ctx, opts->relax, st);
+      launches += 2;
+    }
+    if (ce == cudaSuccess && s >= 2) ce = cudaStreamWaitEvent(st, ctx->ev_down[b], 0);  // field buffer b is free again
+    if (ce == cudaSuccess) ce = launch_gather(ctx, ctx->d_ubuf[b], ctx->prec, st);
+    ++launches;
+    if (ce == cudaSuccess) ce = cudaEventRecord(ctx->ev_gather[b], st);
+    // copy-out stream: field s to the host
+    if (ce == cudaSuccess) ce = cudaStreamWaitEvent(ctx->s_out, ctx->ev_gather[b], 0);
+    if (ce == cudaSuccess) ce = cudaMemcpyAsync(u_host[s], ctx->d_ubuf[b], 2 * nn * rs, cudaMemcpyDeviceToHost, ctx->s_out);
+    if (ce == cudaSuccess) ce = cudaEventRecord(ctx->ev_down[b], ctx->s_out);
+  }
+  // the context keeps the last source (hz_residual and later hz_ddm_solve calls see it)
+  if (ce == cudaSuccess) ce = cudaMemcpyAsync(ctx->d_fre, ctx->d_fstage[(n_src - 1) & 1], nn * sizeof(double), cudaMemcpyDeviceToDevice, st);
+  if (ce == cudaSuccess) ce = cudaStreamWaitEvent(st, ctx->ev_down[(n_src - 1) & 1], 0);
+  if (ce == cudaSuccess && n_src >= 2) ce = cudaStreamWaitEvent(st, ctx->ev_down[n_src & 1], 0);
+  if (ce == cudaSuccess) ce = cudaEventRecord(e1, st);
+  if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
+  float ms = 0.f;
+  if (ce == cudaSuccess) ce = cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  if (ce != cudaSuccess) {
+    cudaStreamSynchronize(ctx->s_in); cudaStreamSynchronize(ctx->s_out); cudaStreamSynchronize(st);
+    return cuda_fail(ctx, ce, "hz_ddm_solve_sources");
+  }
+  if (info) {
+    info->sources_done = n_src;
+    info->total_ms = ms;
+    info->dof_timesteps = (double)ctx->L * ctx->lay.lnx * ctx->lay.lny * (double)opts->n_wh * (ctx->n_t - 1) * opts->n_outer_max * n_src;
+    info->launches = launches;
+    info->h2d_bytes = (double)n_src * nn * sizeof(double);
+    info->d2h_bytes = (double)n_src * 2 * nn * rs;
+  }
+  return HZ_OK;
+}
+
 }  // extern "C"
 
 namespace {
@@ -1128,6 +1225,14 @@ void hz_destroy(hz_ctx *ctx) {
   if (!ctx) return;
   free_partition(ctx);
   if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
+  if (ctx->s_in) cudaStreamDestroy(ctx->s_in);
+  if (ctx->s_out) cudaStreamDestroy(ctx->s_out);
+  for (int b = 0; b < 2; ++b) {
+    if (ctx->d_fstage[b]) cudaFree(ctx->d_fstage[b]);
+    if (ctx->d_ubuf[b]) cudaFree(ctx->d_ubuf[b]);
+    for (cudaEvent_t e : {ctx->ev_up[b], ctx->ev_build[b], ctx->ev_gather[b], ctx->ev_down[b]})
+      if (e) cudaEventDestroy(e);
+  }
   double **ptrs[] = {&ctx->d_c, &ctx->d_fre, &ctx->d_fim, &ctx->d_bc, &ctx->d_vx, &ctx->d_vy};
   for (double **q : ptrs) { if (*q) cudaFree(*q); *q = nullptr; }
   delete ctx;

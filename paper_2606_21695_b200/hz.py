@@ -21,7 +21,7 @@ HZ_TC_IMPEDANCE0 = 0
 STATUS_NAMES = {0: "HZ_OK", 1: "HZ_EINVAL", 2: "HZ_ENOMEM", 3: "HZ_ECUDA", 4: "HZ_EUNSUPPORTED", 5: "HZ_ESTATE"}
 
 # every symbol include/hz.h declares
-EXPORTS = ("hz_mesh_setup", "hz_mesh_setup_quads", "hz_set_source", "hz_partition", "hz_ddm_solve", "hz_ddm_solve_gmres", "hz_minres_cycle", "hz_residual",
+EXPORTS = ("hz_mesh_setup", "hz_mesh_setup_quads", "hz_set_source", "hz_partition", "hz_ddm_solve", "hz_ddm_solve_sources", "hz_ddm_solve_gmres", "hz_minres_cycle", "hz_residual",
            "hz_get_subdomain_state", "hz_set_subdomain_state", "hz_last_error", "hz_destroy", "hz_peak_probe")
 
 
@@ -36,6 +36,11 @@ class hz_part_info(C.Structure):
 class hz_solve_opts(C.Structure):
     _fields_ = [("n_outer_max", C.c_int), ("n_wh", C.c_int), ("warm_start", C.c_int), ("relax", C.c_double),
                 ("tol", C.c_double), ("check_every", C.c_int), ("reset_state", C.c_int), ("use_graph", C.c_int)]
+
+
+class hz_sources_info(C.Structure):
+    _fields_ = [("sources_done", C.c_int), ("total_ms", C.c_double), ("dof_timesteps", C.c_double),
+                ("launches", C.c_int), ("h2d_bytes", C.c_double), ("d2h_bytes", C.c_double)]
 
 
 class hz_solve_info(C.Structure):
@@ -89,6 +94,8 @@ def lib():
     L.hz_set_source.argtypes = [vp, vp, vp]
     L.hz_partition.argtypes = [vp, ip, ip, ip, ip, ip, C.c_double, C.POINTER(hz_part_info)]
     L.hz_ddm_solve.argtypes = [vp, C.POINTER(hz_solve_opts), vp, C.POINTER(hz_solve_info), vp]
+    L.hz_ddm_solve_sources.argtypes = [vp, C.POINTER(hz_solve_opts), ip, C.POINTER(vp), C.POINTER(vp),
+                                       C.POINTER(hz_sources_info), vp]
     L.hz_ddm_solve_gmres.argtypes = [vp, C.POINTER(hz_gmres_opts), vp, C.POINTER(hz_gmres_info), vp]
     L.hz_minres_cycle.argtypes = [vp, C.POINTER(hz_minres_opts), vp, vp, C.POINTER(hz_minres_info), vp]
     L.hz_residual.argtypes = [vp, vp, ip, dp, vp]
@@ -175,6 +182,21 @@ def hz_ddm_solve(ctx, n_outer_max, n_wh=5, warm_start=True, relax=0.5, tol=0.0, 
     info = hz_solve_info()
     _check(ctx, lib().hz_ddm_solve(ctx, C.byref(opts), C.c_void_p(u_out_ptr) if u_out_ptr else None, C.byref(info),
                                    C.c_void_p(stream) if stream else None))
+    return info
+
+
+def hz_ddm_solve_sources(ctx, f_host_ptrs, u_host_ptrs, n_outer=1, n_wh=5, warm_start=True, relax=0.5,
+                         reset_state=False, stream=None):
+    """A stream of sources, host to host, copies overlapped with the sweeps (include/hz.h).  f_host_ptrs /
+    u_host_ptrs: raw HOST pointers (e.g. pinned torch tensors' data_ptr()).  -> hz_sources_info"""
+    n = len(f_host_ptrs)
+    assert n == len(u_host_ptrs) and n >= 1
+    fa = (C.c_void_p * n)(*[C.c_void_p(int(q)) for q in f_host_ptrs])
+    ua = (C.c_void_p * n)(*[C.c_void_p(int(q)) for q in u_host_ptrs])
+    opts = hz_solve_opts(int(n_outer), int(n_wh), int(bool(warm_start)), float(relax), 0.0, 0, int(bool(reset_state)), 0)
+    info = hz_sources_info()
+    _check(ctx, lib().hz_ddm_solve_sources(ctx, C.byref(opts), n, fa, ua, C.byref(info),
+                                           C.c_void_p(stream) if stream else None))
     return info
 
 
