@@ -151,3 +151,30 @@ def test_quads_errors():
         assert e.value.status == hz.HZ_EUNSUPPORTED
     finally:
         hz.hz_destroy(ctx)
+
+
+def test_sources_stream_and_set_source_on_a_quad_context():
+    # hz_set_source rebuilds the load with the general-geometry mass; hz_ddm_solve_sources does the same from its
+    # staging buffers: both against the oracle with the new source
+    inp = quad_inputs(8, 6, 2, 2, 2, seed=55)
+    rng = np.random.default_rng(2)
+    f2 = rng.standard_normal(inp.f_re.shape)
+    inp2 = HzInputs(**{**inp.__dict__, "f_re": f2})
+    st = O.ddm_solve(problem_from(inp2), inp.sx, inp.sy, 2, 2)
+    ref = O.ddm_gather(st)
+    nn = inp.npx * inp.npy
+    ctx, info = hz.setup_from_inputs(inp, hz.HZ_F64, 0)           # set up with the OLD source
+    try:
+        u = torch.zeros(2 * nn, dtype=torch.float64, device="cuda")
+        hz.hz_set_source(ctx, f2)
+        hz.hz_ddm_solve(ctx, 2, n_wh=2, reset_state=True, u_out_ptr=u.data_ptr())
+        a = u.cpu().numpy().reshape(2, inp.npy, inp.npx)
+        assert rel(a[0] + 1j * a[1], ref) <= 1e-10
+        f_pin = [torch.from_numpy(np.ascontiguousarray(f)).pin_memory() for f in (inp.f_re, f2)]
+        u_pin = [torch.empty(2 * nn, dtype=torch.float64).pin_memory() for _ in range(2)]
+        hz.hz_ddm_solve_sources(ctx, [t.data_ptr() for t in f_pin], [t.data_ptr() for t in u_pin], n_outer=2, n_wh=2,
+                                reset_state=True)
+        b = u_pin[1].numpy().reshape(2, inp.npy, inp.npx)
+        assert rel(b[0] + 1j * b[1], ref) <= 1e-10
+    finally:
+        hz.hz_destroy(ctx)
