@@ -53,10 +53,15 @@ typedef struct {
   int warm_start;  /* 0: u^(0) = 0 (Algorithm 1 as printed); 1: previous u_l (reading R11) */
   double relax;    /* rho in (0,1] (reading R12) */
   int reset_state; /* 1: lambda = 0, u_l = 0 first */
+  double tol;      /* > 0 with check_every > 0: stop when the global relative residual (hz3_residual of the gathered
+                      field, fp64) is <= tol; the check runs outside the sweep, every check_every sweeps */
+  int check_every;
 } hz3_solve_opts;
 
 typedef struct {
   int n_outer_done, n_t;
+  double rel_residual;                  /* last residual check, or -1 */
+  double total_ms;                      /* CUDA-event time of the whole call */
   double sweep_ms_total, exch_ms_total; /* CUDA-event times of the sweep / exchange kernels */
   double dof_timesteps;                 /* sweeps * blocks * dofs_per_sub * n_wh * (n_t - 1) */
   int launches;

@@ -141,6 +141,38 @@ cudaError_t launch_sweep3_col(const hz3_ctx *c, const hz3_solve_opts *o, const B
   return cudaGetLastError();
 }
 
+hz_status residual3_impl(hz3_ctx *ctx, const void *u_dev, int prec, double *rel, cudaStream_t st) {
+  const Geo3 &g = ctx->g;
+  const long long total = (long long)g.npx * g.npy * g.npz;
+  const int nb = (int)((total + 255) / 256);
+  if (!ctx->d_part) {
+    HZ3_CUDA(cudaMalloc((void **)&ctx->d_part, (size_t)2 * nb * sizeof(double)));
+    HZ3_CUDA(cudaMalloc((void **)&ctx->d_red, 2 * sizeof(double)));
+  }
+  const double *u64 = (const double *)u_dev;
+  if (prec == HZ_F32) {
+    if (!ctx->d_u64) HZ3_CUDA(cudaMalloc((void **)&ctx->d_u64, (size_t)2 * total * sizeof(double)));
+    k3_to_f64<float><<<(unsigned)((2 * total + 255) / 256), 256, 0, st>>>((const float *)u_dev, ctx->d_u64, 2 * total);
+    HZ3_CUDA(cudaGetLastError());
+    u64 = ctx->d_u64;
+  }
+  Ref1D ref{};
+  for (int a = 0; a <= g.p; ++a) {
+    ref.w[a] = ctx->gll.w[a];
+    for (int b = 0; b <= g.p; ++b) ref.K[a][b] = ctx->gll.K[a][b];
+  }
+  k3_residual<double><<<nb, 256, 0, st>>>(g, ref, ctx->d_c, ctx->d_fre, ctx->d_fim, ctx->d_bc, u64, const_cast<double *>(u64),
+                                          ctx->d_part);
+  HZ3_CUDA(cudaGetLastError());
+  k_reduce2<<<1, 1024, 0, st>>>(ctx->d_part, nb, ctx->d_red);
+  HZ3_CUDA(cudaGetLastError());
+  double h[2];
+  HZ3_CUDA(cudaMemcpyAsync(h, ctx->d_red, sizeof(h), cudaMemcpyDeviceToHost, st));
+  HZ3_CUDA(cudaStreamSynchronize(st));
+  *rel = h[1] > 0.0 ? std::sqrt(h[0] / h[1]) : std::sqrt(h[0]);
+  return HZ_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -315,11 +347,18 @@ hz_status hz3_ddm_solve(hz3_ctx *ctx, const hz3_solve_opts *opts, void *u_out, h
     HZ3_CUDA(cudaMemsetAsync(ctx->d_usub, 0, (size_t)2 * ctx->L * g.NS * rs, st));
   }
   const int n = opts->n_outer;
-  std::vector<cudaEvent_t> ev((size_t)2 * n + 1);
+  const bool checking = opts->tol > 0.0 && opts->check_every > 0;
+  const long long total = (long long)g.npx * g.npy * g.npz;
+  const unsigned nbg = (unsigned)((total + 255) / 256);
+  if (checking && !ctx->d_u64) HZ3_CUDA(cudaMalloc((void **)&ctx->d_u64, (size_t)2 * total * sizeof(double)));
+  std::vector<cudaEvent_t> ev((size_t)2 * n + 2);
   for (auto &e : ev) HZ3_CUDA(cudaEventCreate(&e));
   auto cleanup = [&]() { for (auto &e : ev) cudaEventDestroy(e); };
   cudaError_t ce = cudaSuccess;
   const unsigned nbx = (unsigned)((lam_n + 255) / 256);
+  int done = 0, launches = 0;
+  double rel = -1.0;
+  ce = cudaEventRecord(ev[2 * n + 1], st);  // start of the call
   for (int it = 0; it < n && ce == cudaSuccess; ++it) {
     ce = cudaEventRecord(ev[2 * it], st);
     if (ce == cudaSuccess) {
@@ -334,30 +373,49 @@ hz_status hz3_ddm_solve(hz3_ctx *ctx, const hz3_solve_opts *opts, void *u_out, h
     if (ctx->prec == HZ_F32) k3_exchange<float><<<nbx, 256, 0, st>>>(g, (float)opts->relax, (float *)ctx->d_lam, (const float *)ctx->d_g);
     else k3_exchange<double><<<nbx, 256, 0, st>>>(g, opts->relax, (double *)ctx->d_lam, (const double *)ctx->d_g);
     ce = cudaGetLastError();
+    if (ce != cudaSuccess) break;
+    ++done; launches += 2;
+    if (checking && (done % opts->check_every == 0 || done == n)) {  // the only reduction, outside the sweep
+      if (ctx->prec == HZ_F32) k3_gather<float, double><<<nbg, 256, 0, st>>>(g, (const float *)ctx->d_usub, ctx->d_u64);
+      else k3_gather<double, double><<<nbg, 256, 0, st>>>(g, (const double *)ctx->d_usub, ctx->d_u64);
+      ce = cudaGetLastError();
+      if (ce != cudaSuccess) break;
+      hz_status rs_ = residual3_impl(ctx, ctx->d_u64, HZ_F64, &rel, st);
+      launches += 3;
+      if (rs_ != HZ_OK) { cleanup(); return rs_; }
+      if (rel <= opts->tol) break;
+    }
   }
   if (ce == cudaSuccess) ce = cudaEventRecord(ev[2 * n], st);
-  int launches = 2 * n;
   if (ce == cudaSuccess && u_out) {
-    const long long total = (long long)g.npx * g.npy * g.npz;
-    const unsigned nb = (unsigned)((total + 255) / 256);
-    if (ctx->prec == HZ_F32) k3_gather<float, float><<<nb, 256, 0, st>>>(g, (const float *)ctx->d_usub, (float *)u_out);
-    else k3_gather<double, double><<<nb, 256, 0, st>>>(g, (const double *)ctx->d_usub, (double *)u_out);
+    if (ctx->prec == HZ_F32) k3_gather<float, float><<<nbg, 256, 0, st>>>(g, (const float *)ctx->d_usub, (float *)u_out);
+    else k3_gather<double, double><<<nbg, 256, 0, st>>>(g, (const double *)ctx->d_usub, (double *)u_out);
     ce = cudaGetLastError();
     ++launches;
   }
+  cudaEvent_t ev_end = nullptr;
+  if (ce == cudaSuccess) ce = cudaEventCreate(&ev_end);
+  if (ce == cudaSuccess) ce = cudaEventRecord(ev_end, st);
   if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
-  if (ce != cudaSuccess) { cleanup(); return cuda_fail3(ctx, ce, "hz3_ddm_solve"); }
+  if (ce != cudaSuccess) { cleanup(); if (ev_end) cudaEventDestroy(ev_end); return cuda_fail3(ctx, ce, "hz3_ddm_solve"); }
   double sw = 0.0, ex = 0.0;
-  for (int it = 0; it < n; ++it) {
+  for (int it = 0; it < done; ++it) {
     float a = 0.f, b = 0.f;
     cudaEventElapsedTime(&a, ev[2 * it], ev[2 * it + 1]);
-    cudaEventElapsedTime(&b, ev[2 * it + 1], ev[2 * it + 2]);
-    sw += a; ex += b;
+    sw += a;
+    if (!checking) {  // with residual checks in between, the exchange has no closing event of its own
+      cudaEventElapsedTime(&b, ev[2 * it + 1], it + 1 < done ? ev[2 * it + 2] : ev[2 * n]);
+      ex += b;
+    }
   }
+  float tot = 0.f;
+  cudaEventElapsedTime(&tot, ev[2 * n + 1], ev_end);
+  cudaEventDestroy(ev_end);
   cleanup();
   if (info) {
-    info->n_outer_done = n; info->n_t = ctx->n_t; info->sweep_ms_total = sw; info->exch_ms_total = ex;
-    info->dof_timesteps = (double)n * ctx->L * (double)(g.lnx * g.lny * g.lnz) * opts->n_wh * (ctx->n_t - 1);
+    info->n_outer_done = done; info->n_t = ctx->n_t; info->rel_residual = rel; info->total_ms = tot;
+    info->sweep_ms_total = sw; info->exch_ms_total = checking ? -1.0 : ex;
+    info->dof_timesteps = (double)done * ctx->L * (double)(g.lnx * g.lny * g.lnz) * opts->n_wh * (ctx->n_t - 1);
     info->launches = launches;
   }
   return HZ_OK;
@@ -366,36 +424,7 @@ hz_status hz3_ddm_solve(hz3_ctx *ctx, const hz3_solve_opts *opts, void *u_out, h
 hz_status hz3_residual(hz3_ctx *ctx, const void *u_dev, hz_prec prec, double *rel, void *stream) {
   if (!ctx) return HZ_EINVAL;
   if (!u_dev || !rel) return fail3(ctx, HZ_EINVAL, "hz3_residual: NULL u_dev or rel");
-  cudaStream_t st = (cudaStream_t)stream;
-  const Geo3 &g = ctx->g;
-  const long long total = (long long)g.npx * g.npy * g.npz;
-  const int nb = (int)((total + 255) / 256);
-  if (!ctx->d_part) {
-    HZ3_CUDA(cudaMalloc((void **)&ctx->d_part, (size_t)2 * nb * sizeof(double)));
-    HZ3_CUDA(cudaMalloc((void **)&ctx->d_red, 2 * sizeof(double)));
-  }
-  const double *u64 = (const double *)u_dev;
-  if (prec == HZ_F32) {
-    if (!ctx->d_u64) HZ3_CUDA(cudaMalloc((void **)&ctx->d_u64, (size_t)2 * total * sizeof(double)));
-    k3_to_f64<float><<<(unsigned)((2 * total + 255) / 256), 256, 0, st>>>((const float *)u_dev, ctx->d_u64, 2 * total);
-    HZ3_CUDA(cudaGetLastError());
-    u64 = ctx->d_u64;
-  }
-  Ref1D ref{};
-  for (int a = 0; a <= g.p; ++a) {
-    ref.w[a] = ctx->gll.w[a];
-    for (int b = 0; b <= g.p; ++b) ref.K[a][b] = ctx->gll.K[a][b];
-  }
-  k3_residual<double><<<nb, 256, 0, st>>>(g, ref, ctx->d_c, ctx->d_fre, ctx->d_fim, ctx->d_bc, u64, const_cast<double *>(u64),
-                                          ctx->d_part);
-  HZ3_CUDA(cudaGetLastError());
-  k_reduce2<<<1, 1024, 0, st>>>(ctx->d_part, nb, ctx->d_red);
-  HZ3_CUDA(cudaGetLastError());
-  double h[2];
-  HZ3_CUDA(cudaMemcpyAsync(h, ctx->d_red, sizeof(h), cudaMemcpyDeviceToHost, st));
-  HZ3_CUDA(cudaStreamSynchronize(st));
-  *rel = h[1] > 0.0 ? std::sqrt(h[0] / h[1]) : std::sqrt(h[0]);
-  return HZ_OK;
+  return residual3_impl(ctx, u_dev, prec, rel, (cudaStream_t)stream);
 }
 
 hz_status hz3_operator_time(hz3_ctx *ctx, const double *u_dev, int reps, double *ms_per_eval, void *stream) {

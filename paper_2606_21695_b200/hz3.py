@@ -20,11 +20,12 @@ class hz3_part_info(C.Structure):
 
 class hz3_solve_opts(C.Structure):
     _fields_ = [("n_outer", C.c_int), ("n_wh", C.c_int), ("warm_start", C.c_int), ("relax", C.c_double),
-                ("reset_state", C.c_int)]
+                ("reset_state", C.c_int), ("tol", C.c_double), ("check_every", C.c_int)]
 
 
 class hz3_solve_info(C.Structure):
-    _fields_ = [("n_outer_done", C.c_int), ("n_t", C.c_int), ("sweep_ms_total", C.c_double),
+    _fields_ = [("n_outer_done", C.c_int), ("n_t", C.c_int), ("rel_residual", C.c_double), ("total_ms", C.c_double),
+                ("sweep_ms_total", C.c_double),
                 ("exch_ms_total", C.c_double), ("dof_timesteps", C.c_double), ("launches", C.c_int)]
 
 
@@ -75,8 +76,10 @@ def hz3_partition(ctx, sx, sy, sz, prec=HZ_F64, cfl_frac=0.5):
     return info
 
 
-def hz3_ddm_solve(ctx, n_outer, n_wh=5, warm_start=True, relax=0.5, reset_state=False, u_out_ptr=None, stream=None):
-    opts = hz3_solve_opts(int(n_outer), int(n_wh), int(bool(warm_start)), float(relax), int(bool(reset_state)))
+def hz3_ddm_solve(ctx, n_outer, n_wh=5, warm_start=True, relax=0.5, reset_state=False, u_out_ptr=None, stream=None,
+                  tol=0.0, check_every=0):
+    opts = hz3_solve_opts(int(n_outer), int(n_wh), int(bool(warm_start)), float(relax), int(bool(reset_state)),
+                          float(tol), int(check_every))
     info = hz3_solve_info()
     _check(ctx, lib3().hz3_ddm_solve(ctx, C.byref(opts), C.c_void_p(u_out_ptr) if u_out_ptr else None, C.byref(info),
                                      C.c_void_p(stream) if stream else None))
