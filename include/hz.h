@@ -171,6 +171,12 @@ typedef struct {
  * ------------------------------------------------------------------------------------------- */
 hz_status hz_ddm_solve(hz_ctx *ctx, const hz_solve_opts *opts, void *u_out, hz_solve_info *info, void *stream);
 
+/* The paper's "operator time" normaliser (the DDM cycle is compared "to the time it takes to evaluate
+ * the Helmholtz operator A - i w H - w^2 M on the entire domain"): `reps` back-to-back evaluations of the global
+ * operator (the kernel of hz_residual, fp64) on u_dev (DEVICE, 2*(nx*p+1)*(ny*p+1) doubles);
+ * *ms_per_eval = CUDA-event time / reps. */
+hz_status hz_operator_time(hz_ctx *ctx, const double *u_dev, int reps, double *ms_per_eval, void *stream);
+
 /* ---------------------------------------------------------------------------------------------
  * hz_ddm_solve_sources — a stream of right-hand sides on one mesh and partition, end to end from HOST to HOST:
  * for s = 0..n_src-1: copy source f_s to the device, rebuild the load ("Assemble b from f"), run

@@ -802,6 +802,42 @@ hz_status hz_ddm_solve(hz_ctx *ctx, const hz_solve_opts *opts, void *u_out, hz_s
   return HZ_OK;
 }
 
+hz_status hz_operator_time(hz_ctx *ctx, const double *u_dev, int reps, double *ms_per_eval, void *stream) {
+  if (!ctx) return HZ_EINVAL;
+  if (!u_dev || !ms_per_eval || reps < 1) return fail(ctx, HZ_EINVAL, "hz_operator_time: NULL argument or reps < 1");
+  cudaStream_t st = (cudaStream_t)stream;
+  double rel = 0.0;
+  hz_status s0 = residual_impl(ctx, u_dev, HZ_F64, &rel, st);  // allocates the partial-sum buffers, warm-up
+  if (s0 != HZ_OK) return s0;
+  const long long total = (long long)ctx->npx * ctx->npy;
+  const int bs = 256, nb = (int)((total + bs - 1) / bs);
+  Ref1D ref{};
+  for (int a = 0; a <= ctx->p; ++a) {
+    ref.w[a] = ctx->gll.w[a];
+    for (int b = 0; b <= ctx->p; ++b) ref.K[a][b] = ctx->gll.K[a][b];
+  }
+  const Geo g = make_geo(ctx);
+  cudaEvent_t e0, e1;
+  HZ_CUDA(cudaEventCreate(&e0));
+  HZ_CUDA(cudaEventCreate(&e1));
+  cudaEventRecord(e0, st);
+  for (int r = 0; r < reps; ++r) {
+    if (ctx->general)
+      k_residual_quad<double><<<nb, bs, 0, st>>>(g, ctx->refq, ctx->d_vx, ctx->d_vy, ctx->d_c, ctx->d_fre, ctx->d_fim, ctx->d_bc, u_dev, ctx->d_part);
+    else
+      k_residual<double><<<nb, bs, 0, st>>>(g, ref, ctx->d_c, ctx->d_fre, ctx->d_fim, ctx->d_bc, u_dev, ctx->d_part);
+  }
+  cudaEventRecord(e1, st);
+  cudaError_t ce = cudaStreamSynchronize(st);
+  float ms = 0.f;
+  if (ce == cudaSuccess) ce = cudaEventElapsedTime(&ms, e0, e1);
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  if (ce != cudaSuccess) return cuda_fail(ctx, ce, "hz_operator_time");
+  *ms_per_eval = ms / reps;
+  return HZ_OK;
+}
+
 hz_status hz_ddm_solve_sources(hz_ctx *ctx, const hz_solve_opts *opts, int n_src, const double *const *f_re_host,
                                void *const *u_host, hz_sources_info *info, void *stream) {
   if (!ctx) return HZ_EINVAL;

@@ -21,7 +21,7 @@ HZ_TC_IMPEDANCE0 = 0
 STATUS_NAMES = {0: "HZ_OK", 1: "HZ_EINVAL", 2: "HZ_ENOMEM", 3: "HZ_ECUDA", 4: "HZ_EUNSUPPORTED", 5: "HZ_ESTATE"}
 
 # every symbol include/hz.h declares
-EXPORTS = ("hz_mesh_setup", "hz_mesh_setup_quads", "hz_set_source", "hz_partition", "hz_ddm_solve", "hz_ddm_solve_sources", "hz_ddm_solve_gmres", "hz_minres_cycle", "hz_residual",
+EXPORTS = ("hz_mesh_setup", "hz_mesh_setup_quads", "hz_set_source", "hz_partition", "hz_ddm_solve", "hz_operator_time", "hz_ddm_solve_sources", "hz_ddm_solve_gmres", "hz_minres_cycle", "hz_residual",
            "hz_get_subdomain_state", "hz_set_subdomain_state", "hz_last_error", "hz_destroy", "hz_peak_probe")
 
 
@@ -94,6 +94,7 @@ def lib():
     L.hz_set_source.argtypes = [vp, vp, vp]
     L.hz_partition.argtypes = [vp, ip, ip, ip, ip, ip, C.c_double, C.POINTER(hz_part_info)]
     L.hz_ddm_solve.argtypes = [vp, C.POINTER(hz_solve_opts), vp, C.POINTER(hz_solve_info), vp]
+    L.hz_operator_time.argtypes = [vp, vp, ip, C.POINTER(C.c_double), vp]
     L.hz_ddm_solve_sources.argtypes = [vp, C.POINTER(hz_solve_opts), ip, C.POINTER(vp), C.POINTER(vp),
                                        C.POINTER(hz_sources_info), vp]
     L.hz_ddm_solve_gmres.argtypes = [vp, C.POINTER(hz_gmres_opts), vp, C.POINTER(hz_gmres_info), vp]
@@ -183,6 +184,13 @@ def hz_ddm_solve(ctx, n_outer_max, n_wh=5, warm_start=True, relax=0.5, tol=0.0, 
     _check(ctx, lib().hz_ddm_solve(ctx, C.byref(opts), C.c_void_p(u_out_ptr) if u_out_ptr else None, C.byref(info),
                                    C.c_void_p(stream) if stream else None))
     return info
+
+
+def hz_operator_time(ctx, u_ptr, reps=20, stream=None):
+    """ms per evaluation of the global Helmholtz operator (fp64) on the device field at u_ptr (the paper's normaliser)."""
+    ms = C.c_double()
+    _check(ctx, lib().hz_operator_time(ctx, C.c_void_p(u_ptr), int(reps), C.byref(ms), C.c_void_p(stream) if stream else None))
+    return ms.value
 
 
 def hz_ddm_solve_sources(ctx, f_host_ptrs, u_host_ptrs, n_outer=1, n_wh=5, warm_start=True, relax=0.5,

@@ -14,6 +14,9 @@ from __future__ import annotations
 
 import argparse
 
+import numpy as np
+import torch
+
 from . import hz
 from .inputs import make_config
 
@@ -26,7 +29,7 @@ def run(cfg, prec, k, n=None, p=None, s=None, nwh=5, reps=3, distort=0.0):
     try:
         ctx, info = hz.setup_from_inputs(inp, prec, k)
     except hz.HzError as e:
-        print(f"{name} {k or 'auto'} | — | — | — | — | — | — | — | {e.args[0].split(':', 1)[0]} |", flush=True)
+        print(f"{name} {k or 'auto'} | — | — | — | — | — | — | — | — | — | {e.args[0].split(':', 1)[0]} |", flush=True)
         return
     try:
         hz.hz_ddm_solve(ctx, 1, n_wh=nwh, reset_state=True)
@@ -36,8 +39,12 @@ def run(cfg, prec, k, n=None, p=None, s=None, nwh=5, reps=3, distort=0.0):
         if distort > 0:   # general quads: (p+1)^2 (4(p+1)+4) FMAs per element over p^2 DOFs, + 5 updates
             fl = 2 * ((inp.p + 1) ** 2 * (4 * (inp.p + 1) + 4) / inp.p ** 2 + 5)
         peak = SMS * (128 if prec == hz.HZ_F32 else 64) * 2 * CLK
+        # the paper's normaliser: one evaluation of the global operator (fp64) on a random vector
+        v = torch.from_numpy(np.random.default_rng(1).standard_normal(2 * inp.npx * inp.npy)).cuda()
+        op_ms = hz.hz_operator_time(ctx, v.data_ptr(), 20)
         print(f"{name} {info.dofs_per_thread} | {info.cluster_size} | {info.dofs_per_sub} | {info.blocks} | {info.threads_per_block} | "
-              f"{info.smem_bytes} | {r.sweep_ms_total / reps:.3f} | {rate:.3e} | {rate * fl / peak:.3f} |", flush=True)
+              f"{info.smem_bytes} | {r.sweep_ms_total / reps:.3f} | {rate:.3e} | {rate * fl / peak:.3f} | {op_ms:.4f} | "
+              f"{r.sweep_ms_total / reps / op_ms:.1f} |", flush=True)
     finally:
         hz.hz_destroy(ctx)
 
@@ -47,8 +54,8 @@ def main():
     ap.add_argument("which", choices=["cfg2", "cfg3", "cfg4", "cfg5", "quads"])
     ap.add_argument("--scale", type=int, default=4)
     a = ap.parse_args()
-    print("| cfg | n | p | sub side | prec | DOF/thread | CTAs/sub | DOF/sub | blocks | threads | smem B | sweep ms | DOF-steps/s | frac of FMA peak |")
-    print("|---|---|---|---|---|---|---|---|---|---|---|---|---|---|")
+    print("| cfg | n | p | sub side | prec | DOF/thread | CTAs/sub | DOF/sub | blocks | threads | smem B | sweep ms | DOF-steps/s | frac of FMA peak | operator ms (fp64) | DDM cycle / operator |")
+    print("|---|---|---|---|---|---|---|---|---|---|---|---|---|---|---|---|")
     if a.which in ("cfg2", "cfg3"):
         for prec in (hz.HZ_F32, hz.HZ_F64):
             for k in (1, 9):
