@@ -201,6 +201,13 @@ SweepArgs<real> make_args(const hz_ctx *c, const hz_solve_opts *o) {
     a.ex1.k0[i] = (real)c->ex1.k0[i]; a.ex1.kp[i] = (real)c->ex1.kp[i];
     a.ey1.k0[i] = (real)c->ey1.k0[i]; a.ey1.kp[i] = (real)c->ey1.kp[i];
   }
+  // warp-role order of k_sweep_ws: a 3-warp block (2 bulk + 1 edge) puts its edge warp in the middle, so that the bulk
+  // warps of the blocks resident on an SM (consecutive hardware warp slots, slot mod 4 = sub-partition) spread evenly
+  // over the 4 schedulers (measured: config 2 fp32 0.147 -> 0.111 ms per sweep, config 3 fp32 1.273 -> 1.241 ms)
+  {
+    const char *env_wo = std::getenv("HZ_WARP_ORDER");  // debug knob
+    a.worder = env_wo ? std::atoi(env_wo) : ((c->ws && c->launch.threads == 96) ? 1 : 0);
+  }
   a.fused = 0; a.relax = (real)o->relax; a.g_prev = nullptr; a.lam_rw = nullptr;
   return a;
 }

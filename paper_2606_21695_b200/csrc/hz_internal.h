@@ -75,6 +75,7 @@ struct SweepArgs {
   Elem1D<real> ex1, ey1;                         // variant 1
   // fused exchange (optional): lam is then lambda^{n-1}, read-write; g_prev the neighbours' g^{n-1}
   int fused;
+  int worder;  // warp-role order of the warp-specialised kernel (hz_sweep_ws.cuh): 0 bulk warps first, 1 / 2 see there
   real relax;
   const real *g_prev;
   real *lam_rw;

@@ -116,7 +116,6 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_cl(const SweepArgs<real> A
   const real *pR = remR ? halo + (nty + ty) * CHY : xb + (hasR ? t + 1 : ZR + ((t + 1) & 31)) * RS + oRX;
   const real *pD = xb + (hasD ? t - wloc : ZR + ((t - wloc) & 31)) * RS + oPY;
   const real *pU = xb + (hasU ? t + wloc : ZR + ((t + wloc) & 31)) * RS + oRY;
-  const int strL = remL ? HS : BUFW, strR = remR ? HS : BUFW;  // distance between the two buffers of that source
   // where this tile pushes for the CTA across the cut: its PX chunk to the right CTA's haloL[ty], its RX chunk to the
   // left CTA's haloR[ty]; and that CTA's mbarriers
   const unsigned hbase = (unsigned)__cvta_generic_to_shared(halo), RB = (unsigned)sizeof(real);
@@ -254,14 +253,18 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_cl(const SweepArgs<real> A
       }
       if (t == 0) mbar_arm(mbar0 + 8u * bsel, tx_bytes);
       __syncthreads();
-      if (bsel) { mbar_wait_parity(mbar0 + 8u, ph1); ph1 ^= 1u; }
-      else { mbar_wait_parity(mbar0, ph0); ph0 ^= 1u; }
-      // neighbour loads first, then the part of the step that needs none of them
+      // neighbour loads from this CTA's own records first, then the part of the step that needs none of them; the
+      // tiles on a strip boundary fetch their halo chunk (pushed by the adjacent CTA) only after that part, so the
+      // DSMEM latency of the push hides behind it and no other thread ever waits on the mbarrier
       real qR[TY], piL[TY], qU[TX], piD[TX];
-      ld_chunk<TY>(pL + bsel * strL, piL);
-      ld_chunk<TY>(pR + bsel * strR, qR);
+      if (!remL) ld_chunk<TY>(pL + cur, piL);
+      if (!remR) ld_chunk<TY>(pR + cur, qR);
       ld_chunk<TX>(pD + cur, piD);
       ld_chunk<TX>(pU + cur, qU);
+      const unsigned mb_now = mbar0 + 8u * bsel, ph_now = bsel ? ph1 : ph0;
+      const int hsel = bsel * HS;
+      if (bsel) ph1 ^= 1u;
+      else ph0 ^= 1u;
       cur = BUFW - cur;
       bsel ^= 1;
       const Tab4<real> tn = TC.t[nu];
@@ -289,6 +292,11 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_cl(const SweepArgs<real> A
       for (int b = 0; b < TY; ++b)
 #pragma unroll
         for (int a = 0; a < TX; ++a) vr[b][a] = fmaT(tn.k, p[b][a], vr[b][a]);
+      if (remL || remR) {
+        mbar_wait_parity(mb_now, ph_now);
+        if (remL) ld_chunk<TY>(pL + hsel, piL);
+        if (remR) ld_chunk<TY>(pR + hsel, qR);
+      }
 #pragma unroll
       for (int b = 0; b < TY; ++b) {
         if (b == 0) line_finish<real, P, MX, false>(qR[b], piL[b], s0x, X0[b], A.ex1, S[b]);

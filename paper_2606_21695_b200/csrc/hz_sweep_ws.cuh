@@ -29,7 +29,17 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
   constexpr int CH = (T + V16 - 1) / V16 * V16;
   constexpr int RS = 4 * CH + V16;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  const int h = threadIdx.x, NTH = blockDim.x, l = blockIdx.x;
+  const int NTH = blockDim.x, l = blockIdx.x;
+  // Warp-role order.  Roles are a function of the VIRTUAL thread index h; worder permutes the physical warps
+  // so that the bulk warps of consecutive blocks spread evenly over the 4 SM sub-partitions (hardware warp slot
+  // mod 4): 1 = the first edge warp sits at physical warp 1, 2 = at physical warp 0.
+  int wv_ = threadIdx.x >> 5;
+  {
+    const int nw_ = NTH >> 5;
+    if (A.worder == 1 && nw_ >= 3) wv_ = (wv_ == 1) ? nw_ - 1 : (wv_ == nw_ - 1 ? 1 : wv_);
+    else if (A.worder == 2) wv_ = (wv_ == 0) ? nw_ - 1 : wv_ - 1;
+  }
+  const int h = (wv_ << 5) | (threadIdx.x & 31);
   const int ntx = A.lay.ntx, nty = A.lay.nty, NTV = A.lay.NT, NS = A.lay.NS;
   const int lnx = A.lay.lnx, lny = A.lay.lny;
   const int w = ntx - 1, nbulk = (ntx - 1) * (nty - 1), nedge = ntx + nty - 1;
