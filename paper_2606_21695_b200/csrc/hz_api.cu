@@ -493,6 +493,7 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
     if (force_cl > 1 && t.cl != force_cl) return false;
     Layout q = lay;
     q.variant = 1; q.TX = t.mx * P; q.TY = t.my * P;
+    q.cm = t.cl > 1 ? 1 : 0;
     q.ntx = ctx->ex / t.mx + 1; q.nty = ctx->ey / t.my + 1;
     const int ntv = roundup(q.ntx * q.nty, 32);   // virtual tile slots (stride of the per-node arrays)
     int nthr = ntv;

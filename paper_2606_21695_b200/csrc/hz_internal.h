@@ -23,10 +23,12 @@ struct Layout {
   int ntx, nty;  // thread tiles per side (variant 1): ex/MX+1, ey/MY+1
   int NT;        // threads per block
   int NS;        // slots per subdomain (>= lnx*lny; padding slots hold zeros)
+  int cm;        // variant 1: 1 = virtual tiles numbered column by column, t = tx*nty+ty (cluster kernel: a column
+                 // strip of the tile grid is then a contiguous range of t)
   __host__ __device__ inline int slot(int i, int j) const {
     if (variant != 1) return j * lnx + i;
     const int tx = i / TX, a = i - tx * TX, ty = j / TY, b = j - ty * TY;
-    return (b * TX + a) * NT + ty * ntx + tx;
+    return (b * TX + a) * NT + (cm ? tx * nty + ty : ty * ntx + tx);
   }
 };
 

@@ -97,9 +97,18 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_cl(const SweepArgs<real> A
   const int c0 = rk * wq + (rk < wrem ? rk : wrem), wloc = wq + (rk < wrem ? 1 : 0);
   const int wleft = wq + (rk - 1 < wrem ? 1 : 0), wright = wq + (rk + 1 < wrem ? 1 : 0);
   const bool act = t < wloc * nty;
-  const int txl = act ? t % wloc : 0, ty = act ? t / wloc : 0;
+  // threads number the strip's tiles column by column: the tiles on a strip boundary (first / last column) then sit
+  // in the first / last two warps, and only those warps ever wait for the adjacent CTA's pushes
+  // ... and those columns come LAST in thread order (position q of column c below): the arbiter favours the
+  // highest warp index, and the boundary warps are the critical path of a step (they start it late, after the wait,
+  // and their pushes release the adjacent CTA)
+  const int ord = (CL == 1 || wloc < 2) ? 0 : (rk == 0 ? 0 : (rk == CL - 1 ? 1 : 2));  // 0 natural, 1 reversed, 2 column 0 moved to wloc-2
+  auto pos_of = [&](int c) { return ord == 0 ? c : (ord == 1 ? wloc - 1 - c : (c == 0 ? wloc - 2 : (c == wloc - 1 ? c : c - 1))); };
+  auto col_of = [&](int q) { return ord == 0 ? q : (ord == 1 ? wloc - 1 - q : (q == wloc - 2 ? 0 : (q == wloc - 1 ? q : q + 1))); };
+  const int txl = act ? col_of(t / nty) : 0, ty = act ? t % nty : 0;
+  const int tLn = pos_of(txl > 0 ? txl - 1 : 0) * nty + ty, tRn = pos_of(txl < wloc - 1 ? txl + 1 : txl) * nty + ty;  // records of the x neighbours
   const int tx = c0 + txl;
-  const int v = ty * ntx + tx;  // virtual tile index = slot in the per-node global arrays
+  const int v = tx * nty + ty;  // virtual tile index = slot in the per-node global arrays (Layout::cm = 1)
   const int ZR = NT, SCR = NT + 32;
 
   for (int q = t; q < 2 * BUFW + 2 * HS; q += NT) xb[q] = real(0);
@@ -112,10 +121,12 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_cl(const SweepArgs<real> A
   const bool hasL = act && tx > 0, hasR = act && tx < ntx - 1, hasD = act && ty > 0, hasU = act && ty < nty - 1;
   // neighbour records: own CTA's records, a halo slot fed by the adjacent CTA (strip boundary), or a zero record
   const bool remL = hasL && txl == 0, remR = hasR && txl == wloc - 1;
-  const real *pL = remL ? halo + ty * CHY : xb + (hasL ? t - 1 : ZR + ((t - 1) & 31)) * RS + oPX;
-  const real *pR = remR ? halo + (nty + ty) * CHY : xb + (hasR ? t + 1 : ZR + ((t + 1) & 31)) * RS + oRX;
-  const real *pD = xb + (hasD ? t - wloc : ZR + ((t - wloc) & 31)) * RS + oPY;
-  const real *pU = xb + (hasU ? t + wloc : ZR + ((t + wloc) & 31)) * RS + oRY;
+  const real *pL = remL ? halo + ty * CHY : xb + (hasL ? tLn : ZR + ((t - nty) & 31)) * RS + oPX;
+  const real *pR = remR ? halo + (nty + ty) * CHY : xb + (hasR ? tRn : ZR + ((t + nty) & 31)) * RS + oRX;
+  const real *pD = xb + (hasD ? t - 1 : ZR + ((t - 1) & 31)) * RS + oPY;
+  const real *pU = xb + (hasU ? t + 1 : ZR + ((t + 1) & 31)) * RS + oRY;
+  const bool wwait = __any_sync(0xffffffffu, remL || remR);  // warp-uniform: this warp reads a halo slot
+  const int strL = remL ? HS : BUFW, strR = remR ? HS : BUFW;  // distance between the two buffers of that source
   // where this tile pushes for the CTA across the cut: its PX chunk to the right CTA's haloL[ty], its RX chunk to the
   // left CTA's haloR[ty]; and that CTA's mbarriers
   const unsigned hbase = (unsigned)__cvta_generic_to_shared(halo), RB = (unsigned)sizeof(real);
@@ -253,18 +264,15 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_cl(const SweepArgs<real> A
       }
       if (t == 0) mbar_arm(mbar0 + 8u * bsel, tx_bytes);
       __syncthreads();
-      // neighbour loads from this CTA's own records first, then the part of the step that needs none of them; the
-      // tiles on a strip boundary fetch their halo chunk (pushed by the adjacent CTA) only after that part, so the
-      // DSMEM latency of the push hides behind it and no other thread ever waits on the mbarrier
-      real qR[TY], piL[TY], qU[TX], piD[TX];
-      if (!remL) ld_chunk<TY>(pL + cur, piL);
-      if (!remR) ld_chunk<TY>(pR + cur, qR);
-      ld_chunk<TX>(pD + cur, piD);
-      ld_chunk<TX>(pU + cur, qU);
-      const unsigned mb_now = mbar0 + 8u * bsel, ph_now = bsel ? ph1 : ph0;
-      const int hsel = bsel * HS;
+      if (wwait) mbar_wait_parity(mbar0 + 8u * bsel, bsel ? ph1 : ph0);
       if (bsel) ph1 ^= 1u;
       else ph0 ^= 1u;
+      // neighbour loads first, then the part of the step that needs none of them
+      real qR[TY], piL[TY], qU[TX], piD[TX];
+      ld_chunk<TY>(pL + bsel * strL, piL);
+      ld_chunk<TY>(pR + bsel * strR, qR);
+      ld_chunk<TX>(pD + cur, piD);
+      ld_chunk<TX>(pU + cur, qU);
       cur = BUFW - cur;
       bsel ^= 1;
       const Tab4<real> tn = TC.t[nu];
@@ -292,11 +300,6 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_cl(const SweepArgs<real> A
       for (int b = 0; b < TY; ++b)
 #pragma unroll
         for (int a = 0; a < TX; ++a) vr[b][a] = fmaT(tn.k, p[b][a], vr[b][a]);
-      if (remL || remR) {
-        mbar_wait_parity(mb_now, ph_now);
-        if (remL) ld_chunk<TY>(pL + hsel, piL);
-        if (remR) ld_chunk<TY>(pR + hsel, qR);
-      }
 #pragma unroll
       for (int b = 0; b < TY; ++b) {
         if (b == 0) line_finish<real, P, MX, false>(qR[b], piL[b], s0x, X0[b], A.ex1, S[b]);
