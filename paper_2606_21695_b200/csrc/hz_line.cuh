@@ -13,6 +13,30 @@ __device__ __forceinline__ float fmaT<float>(float a, float b, float c) { return
 template <>
 __device__ __forceinline__ double fmaT<double>(double a, double b, double c) { return fma(a, b, c); }
 
+// Two fp32 values in one aligned register pair, operated on by the packed sm_100 instruction FFMA2 (one issue slot
+// for two IEEE round-to-nearest FMAs, each half bit-identical to the scalar FFMA).  mk2 / un2 are register
+// renamings; mk2(x, x) becomes a broadcast operand of the instruction (no copy).
+struct f2 {
+  unsigned long long v;
+};
+__device__ __forceinline__ f2 mk2(float lo, float hi) {
+  f2 r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r.v) : "f"(lo), "f"(hi));
+  return r;
+}
+__device__ __forceinline__ void un2(f2 a, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(a.v)); }
+template <>
+__device__ __forceinline__ f2 fmaT<f2>(f2 a, f2 b, f2 c) {
+  f2 r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r.v) : "l"(a.v), "l"(b.v), "l"(c.v));
+  return r;
+}
+__device__ __forceinline__ f2 operator*(f2 a, f2 b) {
+  f2 r;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v));
+  return r;
+}
+
 __device__ __forceinline__ void bar_sync_all(int nthreads) {
   asm volatile("bar.sync 1, %0;" ::"r"(nthreads) : "memory");
 }

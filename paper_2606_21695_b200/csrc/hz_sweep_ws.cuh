@@ -16,13 +16,26 @@
 // Records NTV..NTV+31 are always zero (missing neighbours, same bank group as the record they stand in for),
 // NTV+32..NTV+63 are write-only scratch for idle lanes.  Two buffers (ping-pong), one named barrier per step.
 #pragma once
+#include <type_traits>
 #include "hz_line.cuh"
+
+#ifndef HZ_WS_PACK
+#define HZ_WS_PACK 1
+#endif
 
 namespace hz {
 
 template <typename real, int P, int M, bool CSM, int MAXT, int MINB>
 __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A, const __grid_constant__ TabC<real> TC) {
   constexpr int T = M * P, KT = T * T;
+  // fp32, register-capped instantiation (MINB > 1: the one hz_partition picks when the grid fills the GPU, i.e. the
+  // issue-bound case): the element-wise updates p += sigma p-dot, v_r += kappa p, v_i += kappa' p-dot of the node
+  // columns (2j, 2j+1) of a bulk tile run as packed pairs (FFMA2: one issue slot, two round-to-nearest FMAs, each
+  // half bit-identical to the scalar FFMA); an odd last column stays scalar.  Measured: config 3
+  // 1.279 -> 1.259 ms per sweep; on the latency-bound config 2 (256 blocks) packing is 6 % slower, and packing the
+  // y-direction lines or the p-dot update as well is slower everywhere, hence this scope.
+  constexpr bool PK = HZ_WS_PACK && std::is_same<real, float>::value && !CSM && MINB > 1 && T >= 2;
+  constexpr int NP = PK ? T / 2 : 0;
   // record = 4 chunks PX | RX | PY | RY of CH values each (T padded to 16 bytes) + 16 bytes of padding, so the
   // stride is an odd number of 16-byte units: lane-consecutive records are conflict-free for 128-bit accesses
   constexpr int V16 = 16 / (int)sizeof(real);
@@ -153,9 +166,18 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
 #pragma unroll 1
       for (int nu = 1; nu < A.n_t; ++nu) {
 #pragma unroll
-        for (int b = 0; b < T; ++b)
+        for (int b = 0; b < T; ++b) {
+          if constexpr (PK) {
 #pragma unroll
-          for (int a = 0; a < T; ++a) p[b][a] = fmaT(sigma, pd[b][a], p[b][a]);
+            for (int j = 0; j < NP; ++j) {
+              const int a = 2 * j;
+              un2(fmaT(mk2(sigma, sigma), mk2(pd[b][a], pd[b][a + 1]), mk2(p[b][a], p[b][a + 1])), p[b][a], p[b][a + 1]);
+            }
+          }
+#pragma unroll
+          for (int a = 0; a < T; ++a)
+            if (a >= 2 * NP) p[b][a] = fmaT(sigma, pd[b][a], p[b][a]);
+        }
         real *my = pMy + cur, *myRX = pMyRX + cur;
         {
           real oPX[T], oRX[T], oPY[T], oRY[T];
@@ -213,9 +235,18 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
           for (int b = 1; b < T; ++b) S[b][a] = Sc[b];
         }
 #pragma unroll
-        for (int b = 0; b < T; ++b)
+        for (int b = 0; b < T; ++b) {
+          if constexpr (PK) {
 #pragma unroll
-          for (int a = 0; a < T; ++a) vr[b][a] = fmaT(tn.k, p[b][a], vr[b][a]);
+            for (int j = 0; j < NP; ++j) {
+              const int a = 2 * j;
+              un2(fmaT(mk2(tn.k, tn.k), mk2(p[b][a], p[b][a + 1]), mk2(vr[b][a], vr[b][a + 1])), vr[b][a], vr[b][a + 1]);
+            }
+          }
+#pragma unroll
+          for (int a = 0; a < T; ++a)
+            if (a >= 2 * NP) vr[b][a] = fmaT(tn.k, p[b][a], vr[b][a]);
+        }
 #pragma unroll
         for (int b = 0; b < T; ++b) {
           if (b == 0) line_finish<real, P, M, false>(qR[b], piL[b], s0x, X0[b], A.ex1, S[b]);
@@ -245,8 +276,17 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
             } else {  // interior of the subdomain: alpha = 1, Im b = 0
               pd[b][a] = fmaT(r_, tn.c, fmaT(-g_, S[b][a], pd[b][a]));
             }
-            vi[b][a] = fmaT(tn.kh, pd[b][a], vi[b][a]);
+            if (a >= 2 * NP) vi[b][a] = fmaT(tn.kh, pd[b][a], vi[b][a]);
           }
+        if constexpr (PK) {
+#pragma unroll
+          for (int b = 0; b < T; ++b)
+#pragma unroll
+            for (int j = 0; j < NP; ++j) {
+              const int a = 2 * j;
+              un2(fmaT(mk2(tn.kh, tn.kh), mk2(pd[b][a], pd[b][a + 1]), mk2(vi[b][a], vi[b][a + 1])), vi[b][a], vi[b][a + 1]);
+            }
+        }
       }
 #pragma unroll
       for (int b = 0; b < T; ++b)
