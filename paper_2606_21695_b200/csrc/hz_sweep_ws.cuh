@@ -36,6 +36,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
   // y-direction lines or the p-dot update as well is slower everywhere, hence this scope.
   constexpr bool PK = HZ_WS_PACK && std::is_same<real, float>::value && !CSM && MINB > 1 && T >= 2;
   constexpr int NP = PK ? T / 2 : 0;
+  constexpr bool PRE = MINB > 1;  // own-only work before the barrier (see the time loop)
   // record = 4 chunks PX | RX | PY | RY of CH values each (T padded to 16 bytes) + 16 bytes of padding, so the
   // stride is an odd number of 16-byte units: lane-consecutive records are conflict-free for 128-bit accesses
   constexpr int V16 = 16 / (int)sizeof(real);
@@ -204,17 +205,14 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
           st_chunk<T>(my + 2 * CH, oPY);
           st_chunk<T>(my + 3 * CH, oRY);
         }
-        bar_sync_all(NTH);
-        // issue the neighbour loads first, then do the part of the step that needs none of them
-        const real *nL = pL + cur, *nR = pR + cur, *nD = pD + cur, *nU = pU + cur;
-        cur = BUFW - cur;
-        real qR[T], piL[T], qU[T], piD[T];
-        ld_chunk<T>(nL, piL);
-        ld_chunk<T>(nR + CH, qR);
-        ld_chunk<T>(nD + 2 * CH, piD);
-        ld_chunk<T>(nU + 3 * CH, qU);
         const Tab4<real> tn = TC.t[nu];
         real S[T][T], X0[T], Y0[T];
+        // the part of the step that needs no neighbour data (own terms of the line operators, v_r update).  PRE: run it
+        // before the barrier, so that the skew between the warps of a block is absorbed by work instead of by waiting
+        // (grid-filling instantiations: config 3 fp32 1.257 -> 1.224 ms, fp64 2.498 -> 2.415 ms); otherwise after the
+        // neighbour loads are issued, where it covers their latency (config 2, one bulk warp per scheduler: 0.114 ms
+        // against 0.124 ms with PRE)
+        auto own_part = [&]() {
 #pragma unroll
         for (int b = 0; b < T; ++b) {
           real q[T + 1];
@@ -247,6 +245,18 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
           for (int a = 0; a < T; ++a)
             if (a >= 2 * NP) vr[b][a] = fmaT(tn.k, p[b][a], vr[b][a]);
         }
+        };
+        if constexpr (PRE) own_part();
+        bar_sync_all(NTH);
+        // issue the neighbour loads first, then do the part of the step that needs none of them
+        const real *nL = pL + cur, *nR = pR + cur, *nD = pD + cur, *nU = pU + cur;
+        cur = BUFW - cur;
+        real qR[T], piL[T], qU[T], piD[T];
+        ld_chunk<T>(nL, piL);
+        ld_chunk<T>(nR + CH, qR);
+        ld_chunk<T>(nD + 2 * CH, piD);
+        ld_chunk<T>(nU + 3 * CH, qU);
+        if constexpr (!PRE) own_part();
 #pragma unroll
         for (int b = 0; b < T; ++b) {
           if (b == 0) line_finish<real, P, M, false>(qR[b], piL[b], s0x, X0[b], A.ex1, S[b]);
