@@ -22,6 +22,9 @@ What is pinned (tests/test_oracle_pins.py; none of the pins re-types a formula b
   ddm_gmres()                (tests/test_oracle_gmres_pins.py) iterate == least-squares minimiser over an
                              explicitly built Krylov basis (numpy lstsq, tiny case), converged == dense direct
                              solve, monotone residuals, sweep map affine / real-linear
+  ddm_mixed_cycle()/_solve() (tests/test_oracle_mixed_pins.py) without rounding a cycle == m plain sweeps (exact
+                             identity), with the correction stored in float32 it still converges to the dense direct
+                             solve <= 1e-8 where the plain iteration with a float32 state stalls above it
   minres()/block_system()    (tests/test_oracle_minres_pins.py) symmetry/indefiniteness of (5), iterate == residual
                              minimiser over an explicit Krylov basis, recurrence residual == true residual,
                              converged == dense direct solve, agreement with scipy.sparse.linalg.minres
@@ -477,6 +480,62 @@ def ddm_solve(pr: Problem, sx: int, sy: int, n_outer: int, n_wh: int, warm_start
     st = state if state is not None else ddm_setup(pr, sx, sy, cfl_frac, n_t)
     for _ in range(n_outer):
         ddm_sweep(st, n_wh, warm_start, relax, sign_2ik)
+    return st
+
+
+# --------------------------------------------------------------------------------------
+# R27  Mixed-precision outer iteration ("Since the DDM is a preconditioner, we can gain
+#      significant speedups simply by evaluating the preconditioner in a lower precision")
+# --------------------------------------------------------------------------------------
+# One warm-started sweep is an affine map F(X) = T X + c of the joint state X = (lambda, u_l) (see F2 below);
+# T is the same sweep with the load removed (f = 0, boundary datum = 0).  Defect correction in that state
+# space, X kept in fp64:
+#     D        = F(X) - X                          one sweep at full precision
+#     delta_1  = lo(D)
+#     delta_k+1 = lo(T delta_k + D),  k = 1..m-1   m-1 homogeneous sweeps whose state is stored at LOW precision
+#     X       <- X + delta_m
+# Without rounding (lo = identity) delta_m = sum_{j<m} T^j D and X + delta_m = F^m(X) exactly: the cycle IS m
+# plain sweeps.  With rounding the low-precision sweeps only ever see the correction, so their rounding error
+# is relative to |delta|, not to |X|, and the fixed point is still that of the full-precision map (D = 0).
+def _state_copy(st: DDMState):
+    return [[a.copy() for a in sides] for sides in st.lam], [a.copy() for a in st.u]
+
+
+def _state_round(st: DDMState, lo_dtype) -> None:
+    if lo_dtype is None:
+        return
+    st.lam = [[a.astype(lo_dtype).astype(complex) for a in sides] for sides in st.lam]
+    st.u = [a.astype(lo_dtype).astype(complex) for a in st.u]
+
+
+def ddm_mixed_cycle(st: DDMState, st_h: DDMState, m_inner: int, n_wh: int, relax: float, lo_dtype=np.complex64):
+    """One defect-correction cycle on `st` (state X, load f).  `st_h` is a DDMState of the SAME problem with
+    f = 0 and no boundary datum (the homogeneous sweep T); its state is scratch."""
+    lam0, u0 = _state_copy(st)
+    ddm_sweep(st, n_wh, True, relax)                                   # F(X), full precision
+    Dl = [[a - b for a, b in zip(sa, sb)] for sa, sb in zip(st.lam, lam0)]
+    Du = [a - b for a, b in zip(st.u, u0)]
+    st_h.lam, st_h.u = [[a.copy() for a in sides] for sides in Dl], [a.copy() for a in Du]
+    _state_round(st_h, lo_dtype)                                       # delta_1 = lo(D)
+    for _ in range(m_inner - 1):
+        ddm_sweep(st_h, n_wh, True, relax)                             # T delta_k
+        st_h.lam = [[a + d for a, d in zip(sa, sd)] for sa, sd in zip(st_h.lam, Dl)]
+        st_h.u = [a + d for a, d in zip(st_h.u, Du)]
+        _state_round(st_h, lo_dtype)
+    st.lam = [[a + d for a, d in zip(sa, sd)] for sa, sd in zip(lam0, st_h.lam)]
+    st.u = [a + d for a, d in zip(u0, st_h.u)]
+    return st
+
+
+def ddm_mixed_solve(pr: Problem, sx: int, sy: int, n_cycles: int, m_inner: int, n_wh: int, relax: float = 0.5,
+                    cfl_frac: float = 0.5, lo_dtype=np.complex64):
+    """n_cycles defect-correction cycles from X = 0.  Returns the fp64 state."""
+    st = ddm_setup(pr, sx, sy, cfl_frac)
+    pr0 = Problem(pr.nx, pr.ny, pr.p, pr.x0, pr.y0, pr.x1, pr.y1, pr.c_nodes, pr.omega,
+                  np.zeros_like(pr.f), None, vx=pr.vx, vy=pr.vy)
+    st_h = ddm_setup(pr0, sx, sy, cfl_frac, n_t=st.tab.n_t)
+    for _ in range(n_cycles):
+        ddm_mixed_cycle(st, st_h, m_inner, n_wh, relax, lo_dtype)
     return st
 
 
