@@ -94,12 +94,13 @@ typedef struct {
   int edge_nodes_y;      /* ey*p+1: nodes on a W/E side */
   int edge_stride;       /* E = max of the two: stride of one side in lambda arrays */
   int threads_per_block; /* block size of the sweep kernel */
-  int blocks;            /* = sx*sy subdomains = thread blocks of one sweep launch */
+  int blocks;            /* = sx*sy subdomains */
   int dofs_per_thread;   /* 1, or (mx*p)*(my*p) of the register-blocked variant, or -1 (streamed); general quads:
                             (p+1)^2 = the nodes of one element, shared ones replicated */
   int tile_mx, tile_my;  /* elements per thread tile (0 for the one-DOF-per-thread variant) */
   int cluster_size;      /* thread blocks (CTAs of one cluster, on as many SMs) per subdomain; 1 unless the state of
                             a subdomain needs the registers of several SMs (hz_sweep_cl.cuh) */
+  int subs_per_block;    /* subdomains per thread block; 1 except for the packed small-subdomain kernel */
   double dt, theta, sigma; /* dt = T/n_t; theta = tan(w dt/2)/w; sigma = 2 sin(w dt/2)/w */
   size_t smem_bytes;       /* dynamic shared memory per block */
   size_t workspace_bytes;  /* device bytes the context allocated for this partition */
@@ -131,6 +132,23 @@ typedef struct {
  * ------------------------------------------------------------------------------------------- */
 hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec prec, int dofs_per_thread,
                        double cfl_frac, hz_part_info *info_out);
+
+/* hz_partition with explicit control of the variant choice (the (P, B, T) sweep of block layouts).
+ * All fields zero (or flags == NULL) is hz_partition.  Used to time and to parity-test one particular launch shape,
+ * e.g. the launch shape of a full-size config on a reduced mesh. */
+typedef struct {
+  int cluster;       /* 0: automatic; -1: never a thread-block-cluster kernel (streamed fallback instead);
+                        c > 1: only cluster kernels with exactly c CTAs per subdomain compete */
+  int no_warp_spec;  /* 1: never the warp-specialised kernel (the uniform register-blocked kernel instead) */
+  int no_reg_cap;    /* 1: never a register-capped (higher-occupancy) instantiation */
+  int grid_blocks;   /* > 0: choose the variant as if the partition had this many subdomains (the register-capped
+                        instantiations are only picked when the grid fills the GPU) */
+  int warp_order;    /* 0: automatic; 1, 2, 3: warp-role order 0, 1, 2 of the warp-specialised kernel */
+  int pack;          /* 0: automatic; g >= 1: g subdomains per thread block (small-subdomain kernel), HZ_EUNSUPPORTED
+                        if no such instantiation fits */
+} hz_part_flags;
+hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec prec, int dofs_per_thread,
+                          double cfl_frac, const hz_part_flags *flags, hz_part_info *info_out);
 
 typedef struct {
   int n_outer_max;  /* sweeps to run (>= 0) */
@@ -236,6 +254,41 @@ typedef struct {
 hz_status hz_ddm_solve_gmres(hz_ctx *ctx, const hz_gmres_opts *opts, void *u_out, hz_gmres_info *info, void *stream);
 
 /* ---------------------------------------------------------------------------------------------
+ * hz_ddm_solve_mixed — the fp32 path to the fp64 path's residual tolerance ("Since the DDM is a
+ * preconditioner, we can gain significant speedups simply by evaluating the preconditioner in a lower precision";
+ * reading R27).  Defect correction in the DDM state space X = (lambda, u_l), X held in fp64 by `hi`:
+ *     D = F(X) - X                              one fp64 sweep + exchange on `hi` (F = the warm-started sweep map)
+ *     delta_1 = D,  delta_{k+1} = T delta_k + D  m_inner - 1 fp32 sweeps + exchanges on `lo` with the load removed
+ *     X <- X + delta_m
+ * Without rounding a cycle is exactly m_inner plain sweeps; the fp32 sweeps only ever see the correction, so the
+ * iteration converges to the fixed point of the fp64 map at the fp64 rate, at close to fp32 cost.
+ *
+ *   lo, hi   two contexts of the SAME mesh, source and subdomain grid (else HZ_EINVAL), partitioned with
+ *            HZ_F32 and HZ_F64 respectively (else HZ_ESTATE); uniform-mesh contexts with a real source.
+ *            `hi` holds X (continue / reset as in hz_ddm_solve); the state of `lo` is scratch.
+ *   u_out    DEVICE or NULL: 2*(nx*p+1)*(ny*p+1) DOUBLES, the gathered fp64 field.
+ * The global residual (hz_residual of the gathered X, fp64) is checked after every check_every cycles.
+ * ------------------------------------------------------------------------------------------- */
+typedef struct {
+  int n_cycles_max; /* defect-correction cycles (>= 0); one cycle advances the iteration by m_inner sweeps */
+  int m_inner;      /* >= 1 */
+  int n_wh;         /* WaveHoltz iterations per sweep */
+  double relax;     /* rho in (0,1] */
+  double tol;       /* > 0: stop when the global relative residual <= tol */
+  int check_every;  /* in cycles; <= 0 = never */
+  int reset_state;  /* 1: X = 0 first */
+} hz_mixed_opts;
+typedef struct {
+  int cycles_done;
+  int sweeps_lo, sweeps_hi; /* fp32 / fp64 sweep launches */
+  double rel_residual;      /* last residual computed, or -1 */
+  double total_ms;          /* device time of the call */
+  double dof_timesteps;     /* of all sweeps, both precisions */
+} hz_mixed_info;
+hz_status hz_ddm_solve_mixed(hz_ctx *lo, hz_ctx *hi, const hz_mixed_opts *opts, double *u_out, hz_mixed_info *info,
+                             void *stream);
+
+/* ---------------------------------------------------------------------------------------------
  * hz_minres_cycle — the paper's comparator: one DDM cycle on every subdomain (one thread
  * block per subdomain, one launch) with unpreconditioned MINRES on the real symmetric block system (5)
  * as the subdomain solver instead of WaveHoltz.  Assembles b from f and the current lambda^n,
@@ -283,10 +336,6 @@ const char *hz_last_error(const hz_ctx *ctx);
 
 /* Frees the context and all its device memory.  NULL-safe. */
 void hz_destroy(hz_ctx *ctx);
-
-/* Micro-benchmark that establishes this GPU's own CUDA-core FMA ceiling (used by bench.py beside the derived
- * roofline denominator; no method arithmetic).  kind: 0 = FP32 FMA, 1 = FP64 FMA.  Returns TFLOP/s (2 flops per FMA). */
-hz_status hz_peak_probe(int kind, double *result, void *stream);
 
 #ifdef __cplusplus
 }

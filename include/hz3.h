@@ -43,9 +43,12 @@ typedef struct {
   size_t smem_bytes, workspace_bytes;
 } hz3_part_info;
 
-/* sx*sy*sz subdomains (must divide nx, ny, nz: HZ_EINVAL otherwise), one thread block each, one node per thread
- * (HZ_EUNSUPPORTED if a subdomain has more than 1024 nodes).  prec: arithmetic of the sweep. */
-hz_status hz3_partition(hz3_ctx *ctx, int sx, int sy, int sz, hz_prec prec, double cfl_frac, hz3_part_info *info);
+/* sx*sy*sz subdomains (must divide nx, ny, nz: HZ_EINVAL otherwise), one thread block each
+ * (HZ_EUNSUPPORTED if a subdomain has more than 1024 nodes).  prec: arithmetic of the sweep.
+ * nodes_per_thread: 0 = automatic (one thread per node column along z where that column length is compiled, else one
+ * node per thread); 1 = one node per thread (PAPER.md:191-207 in three dimensions); other values HZ_EINVAL. */
+hz_status hz3_partition(hz3_ctx *ctx, int sx, int sy, int sz, hz_prec prec, double cfl_frac, int nodes_per_thread,
+                        hz3_part_info *info);
 
 typedef struct {
   int n_outer;     /* sweeps (each followed by the exchange with relaxation) */

@@ -15,9 +15,10 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhz.so")
+PROBE_LIB = os.path.join(HERE, "libhz_probe.so")   # bench-only FMA-peak micro-benchmark (csrc/hz_probe.cu), not the product ABI
 SOURCES = ["hz_api.cu", "hz_sweep_f32.cu", "hz_sweep_f64.cu", "hz_sweep_quad.cu", "hz3_api.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-Xcompiler", "-fPIC", "--fmad=true"]
+              "-Xcompiler", "-fPIC", "--fmad=true"] + os.environ.get("HZ_NVCC_FLAGS", "").split()   # like CXXFLAGS
 
 
 def _nvcc() -> str:
@@ -55,8 +56,13 @@ def build(force: bool = False, verbose: bool = False) -> str:
             sys.stderr.write(r.stderr)
         return obj
 
-    with ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
-        objs = list(ex.map(compile_one, SOURCES))
+    with ThreadPoolExecutor(max_workers=len(SOURCES) + 1) as ex:
+        objs = list(ex.map(compile_one, SOURCES + ["hz_probe.cu"]))
+    probe_obj = objs.pop()
+    r = subprocess.run([nvcc, "-shared", "-o", PROBE_LIB, probe_obj, "-gencode", "arch=compute_100a,code=sm_100a", "-lcudart"],
+                       capture_output=True, text=True)
+    if r.returncode != 0:
+        raise RuntimeError(f"link failed:\n{r.stdout}\n{r.stderr}")
     cmd = [nvcc, "-shared", "-o", LIB, *objs, "-gencode", "arch=compute_100a,code=sm_100a", "-lcudart"]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:

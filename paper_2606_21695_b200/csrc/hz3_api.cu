@@ -223,7 +223,8 @@ hz_status hz3_mesh_setup(hz3_ctx **out, int nx, int ny, int nz, const double *bo
   return HZ_OK;
 }
 
-hz_status hz3_partition(hz3_ctx *ctx, int sx, int sy, int sz, hz_prec prec, double cfl_frac, hz3_part_info *info) {
+hz_status hz3_partition(hz3_ctx *ctx, int sx, int sy, int sz, hz_prec prec, double cfl_frac, int nodes_per_thread,
+                        hz3_part_info *info) {
   if (!ctx) return HZ_EINVAL;
   Geo3 &g = ctx->g;
   if (sx < 1 || sy < 1 || sz < 1 || g.nx % sx || g.ny % sy || g.nz % sz)
@@ -250,8 +251,7 @@ hz_status hz3_partition(hz3_ctx *ctx, int sx, int sy, int sz, hz_prec prec, doub
   g.sigma = std::sin(g.omega * ctx->dt / 2.0) / (g.omega / 2.0);
   ctx->threads = g.NS;
   ctx->colz = 0;
-  const char *env_col = std::getenv("HZ3_DISABLE_COL");  // debug knob: always the one-node-per-thread kernel
-  if (!(env_col && env_col[0] == '1') && col_supported(P, g.lnz) && g.lnx * g.lny <= 128) {
+  if (nodes_per_thread != 1 && col_supported(P, g.lnz) && g.lnx * g.lny <= 128) {
     ctx->colz = g.lnz;
     ctx->threads = roundup3(g.lnx * g.lny, 32);
   }

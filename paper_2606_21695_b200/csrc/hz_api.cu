@@ -31,6 +31,11 @@ cudaError_t dmalloc(T **ptr, size_t n) {
 
 inline int roundup(int a, int b) { return (a + b - 1) / b * b; }
 
+struct EventGuard {  // a CUDA event released on scope exit
+  cudaEvent_t e = nullptr;
+  ~EventGuard() { if (e) cudaEventDestroy(e); }
+};
+
 }  // namespace
 
 struct hz_ctx {
@@ -52,12 +57,16 @@ struct hz_ctx {
   int mx = 0, my = 0, csm = 0, ws = 0, cl = 1, entry = -1;
   Layout lay{};
   SweepLaunch launch{};
+  hz_part_flags flags{};  // variant-choice controls of the last hz_partition_ex
+  int worder = 0;         // warp-role order of the warp-specialised kernel
   int n_t = 0;
   double dt = 0, theta = 0, sigma = 0;
   size_t ws_bytes = 0;
   void *d_tab = nullptr, *d_gamma = nullptr, *d_alpha = nullptr, *d_bbf_re = nullptr, *d_bbf_im = nullptr;
   void *d_usub = nullptr, *d_lam = nullptr, *d_g = nullptr, *d_k2 = nullptr, *d_bs = nullptr;
   void *d_bandx = nullptr, *d_bandy = nullptr, *d_scr = nullptr;
+  void *d_bbf_zero = nullptr;  // all-zero load of the homogeneous sweep (hz_ddm_solve_mixed), allocated on first use
+  void *d_mix = nullptr;       // hz_ddm_solve_mixed: hi context: X_old (n_state doubles); lo context: D (n_state floats)
   double *d_wxl = nullptr, *d_wyl = nullptr;
   double *d_part = nullptr, *d_red = nullptr, *d_ures = nullptr;
   int res_blocks = 0;
@@ -78,6 +87,7 @@ struct hz_ctx {
   cudaStream_t s_in = nullptr, s_out = nullptr;
   double *d_fstage[2] = {nullptr, nullptr};
   void *d_ubuf[2] = {nullptr, nullptr};
+  size_t ubuf_bytes = 0;
   cudaEvent_t ev_up[2] = {nullptr, nullptr}, ev_build[2] = {nullptr, nullptr}, ev_gather[2] = {nullptr, nullptr},
               ev_down[2] = {nullptr, nullptr};
   int g_chunk = 0, g_nwh = 0, g_warm = 0;
@@ -113,7 +123,7 @@ void free_partition(hz_ctx *c) {
   if (c->d_kpart) { cudaFree(c->d_kpart); c->d_kpart = nullptr; }
   if (c->g_exec) { cudaGraphExecDestroy(c->g_exec); c->g_exec = nullptr; }
   if (c->d_G) { cudaFree(c->d_G); c->d_G = nullptr; }
-  void **ptrs[] = {&c->d_tab, &c->d_gamma, &c->d_alpha, &c->d_bbf_re, &c->d_bbf_im, &c->d_lam,
+  void **ptrs[] = {&c->d_tab, &c->d_gamma, &c->d_alpha, &c->d_bbf_re, &c->d_bbf_im, &c->d_lam, &c->d_bbf_zero, &c->d_mix,
                    &c->d_g, &c->d_k2, &c->d_bs, &c->d_bandx, &c->d_bandy, &c->d_scr, (void **)&c->d_wxl, (void **)&c->d_wyl,
                    (void **)&c->d_part, (void **)&c->d_red, (void **)&c->d_ures};
   for (void **q : ptrs) { if (*q) cudaFree(*q); *q = nullptr; }
@@ -181,7 +191,7 @@ cudaError_t upload_as(const std::vector<double> &src, void **dst) {
 }
 
 template <typename real>
-SweepArgs<real> make_args(const hz_ctx *c, const hz_solve_opts *o) {
+SweepArgs<real> make_args(const hz_ctx *c, const hz_solve_opts *o, bool homog = false) {
   SweepArgs<real> a{};
   a.lay = c->lay;
   a.sx = c->sx; a.sy = c->sy; a.E = c->E;
@@ -193,6 +203,7 @@ SweepArgs<real> make_args(const hz_ctx *c, const hz_solve_opts *o) {
   a.tab = (const Tab4<real> *)c->d_tab;
   a.gamma = (const real *)c->d_gamma; a.alpha = (const real *)c->d_alpha;
   a.bbf_re = (const real *)c->d_bbf_re; a.bbf_im = (const real *)c->d_bbf_im;
+  if (homog) { a.bbf_re = (const real *)c->d_bbf_zero; a.bbf_im = nullptr; }  // the sweep with the load removed
   a.u_sub = (real *)c->d_usub; a.lam = (const real *)c->d_lam; a.gout = (real *)c->d_g;
   a.k2edge = (const real *)c->d_k2; a.bs = (const real *)c->d_bs;
   a.bandx = (const real *)c->d_bandx; a.bandy = (const real *)c->d_bandy;
@@ -201,13 +212,7 @@ SweepArgs<real> make_args(const hz_ctx *c, const hz_solve_opts *o) {
     a.ex1.k0[i] = (real)c->ex1.k0[i]; a.ex1.kp[i] = (real)c->ex1.kp[i];
     a.ey1.k0[i] = (real)c->ey1.k0[i]; a.ey1.kp[i] = (real)c->ey1.kp[i];
   }
-  // warp-role order of k_sweep_ws: a 3-warp block (2 bulk + 1 edge) puts its edge warp in the middle, so that the bulk
-  // warps of the blocks resident on an SM (consecutive hardware warp slots, slot mod 4 = sub-partition) spread evenly
-  // over the 4 schedulers (measured: config 2 fp32 0.147 -> 0.111 ms per sweep, config 3 fp32 1.273 -> 1.241 ms)
-  {
-    const char *env_wo = std::getenv("HZ_WARP_ORDER");  // debug knob
-    a.worder = env_wo ? std::atoi(env_wo) : ((c->ws && c->launch.threads == 96) ? 1 : 0);
-  }
+  a.worder = c->worder;
   a.fused = 0; a.relax = (real)o->relax; a.g_prev = nullptr; a.lam_rw = nullptr;
   return a;
 }
@@ -222,19 +227,19 @@ QuadArgs<real> make_quad_args(const hz_ctx *c) {
   return q;
 }
 
-cudaError_t launch_sweep(const hz_ctx *c, const hz_solve_opts *o, cudaStream_t st) {
+cudaError_t launch_sweep(const hz_ctx *c, const hz_solve_opts *o, cudaStream_t st, bool homog = false) {
   if (c->lay.variant == 3) {
     if (c->prec == HZ_F32)
-      return launch_sweep_quad_f32(make_args<float>(c, o), make_quad_args<float>(c), &c->tc32, c->p, c->launch, st);
-    return launch_sweep_quad_f64(make_args<double>(c, o), make_quad_args<double>(c), &c->tc64, c->p, c->launch, st);
+      return launch_sweep_quad_f32(make_args<float>(c, o, homog), make_quad_args<float>(c), &c->tc32, c->p, c->launch, st);
+    return launch_sweep_quad_f64(make_args<double>(c, o, homog), make_quad_args<double>(c), &c->tc64, c->p, c->launch, st);
   }
   if (c->prec == HZ_F32) {
-    SweepArgs<float> a = make_args<float>(c, o);
+    SweepArgs<float> a = make_args<float>(c, o, homog);
     if (c->lay.variant == 2) return launch_sweep_stream_f32(a, (float *)c->d_scr, c->p, c->launch, st);
     return c->lay.variant == 0 ? launch_sweep_dof_f32(a, c->p, c->launch, st)
                                : launch_sweep_tile_f32(a, &c->tc32, c->entry, c->launch, st);
   }
-  SweepArgs<double> a = make_args<double>(c, o);
+  SweepArgs<double> a = make_args<double>(c, o, homog);
   if (c->lay.variant == 2) return launch_sweep_stream_f64(a, (double *)c->d_scr, c->p, c->launch, st);
   return c->lay.variant == 0 ? launch_sweep_dof_f64(a, c->p, c->launch, st)
                              : launch_sweep_tile_f64(a, &c->tc64, c->entry, c->launch, st);
@@ -306,6 +311,30 @@ hz_status residual_impl(hz_ctx *ctx, const void *u_dev, int u_prec, double *rel,
   HZ_CUDA(cudaStreamSynchronize(st));
   *rel = (h[1] > 0.0) ? std::sqrt(h[0] / h[1]) : std::sqrt(h[0]);
   return HZ_OK;
+}
+
+// Can the device co-schedule one cluster of t.cl CTAs of this shape at all?  (cudaOccupancyMaxActiveClusters; an
+// unschedulable cluster would otherwise only surface as a launch error.)  Errors count as "no".
+bool cluster_schedulable(const TileEntry &t, const SweepLaunch &la) {
+  if (cudaFuncSetAttribute(t.fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)la.smem) != cudaSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  if (t.cl > 8 && cudaFuncSetAttribute(t.fn, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  cudaLaunchConfig_t lc = {};
+  lc.gridDim = dim3(la.blocks, 1, 1);
+  lc.blockDim = dim3(la.threads, 1, 1);
+  lc.dynamicSmemBytes = la.smem;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = t.cl; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  lc.attrs = at; lc.numAttrs = 1;
+  int n = 0;
+  if (cudaOccupancyMaxActiveClusters(&n, t.fn, &lc) != cudaSuccess) { cudaGetLastError(); return false; }
+  return n > 0;
 }
 
 }  // namespace
@@ -419,6 +448,8 @@ hz_status hz_set_source(hz_ctx *ctx, const double *f_re, const double *f_im) {
     if (ctx->part && (ctx->lay.variant == 1))
       return fail(ctx, HZ_EUNSUPPORTED, "hz_set_source: complex f needs the one-DOF-per-thread variant; re-partition");
     HZ_CUDA(dmalloc(&ctx->d_fim, nn));
+    // the cached CUDA graph captured kernels whose arguments hold bbf_im == NULL: it must not be replayed
+    if (ctx->g_exec) { cudaGraphExecDestroy(ctx->g_exec); ctx->g_exec = nullptr; ctx->g_chunk = 0; }
     if (ctx->part && !ctx->d_bbf_im) {
       const size_t rs = ctx->prec == HZ_F32 ? 4 : 8;
       HZ_CUDA(cudaMalloc(&ctx->d_bbf_im, (size_t)ctx->L * ctx->lay.NS * rs));
@@ -438,7 +469,16 @@ hz_status hz_set_source(hz_ctx *ctx, const double *f_re, const double *f_im) {
 
 hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec prec, int dofs_per_thread,
                        double cfl_frac, hz_part_info *info_out) {
+  return hz_partition_ex(ctx, sx, sy, tc, prec, dofs_per_thread, cfl_frac, nullptr, info_out);
+}
+
+hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec prec, int dofs_per_thread,
+                          double cfl_frac, const hz_part_flags *flags, hz_part_info *info_out) {
   if (!ctx) return HZ_EINVAL;
+  hz_part_flags fl{};
+  if (flags) fl = *flags;
+  if (fl.cluster < -1 || fl.cluster == 1 || fl.grid_blocks < 0 || fl.warp_order < 0 || fl.warp_order > 3 || fl.pack < 0)
+    return fail(ctx, HZ_EINVAL, "hz_partition_ex: bad flags");
   if (sx < 1 || sy < 1 || sx > ctx->nx || sy > ctx->ny)
     return fail(ctx, HZ_EINVAL, "hz_partition: need 1 <= sx <= nx, 1 <= sy <= ny");
   if (!ctx->general && (ctx->nx % sx || ctx->ny % sy))
@@ -448,6 +488,8 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
   if (!(cfl_frac > 0.0) || cfl_frac > 1.0) return fail(ctx, HZ_EINVAL, "hz_partition: cfl_frac must be in (0,1]");
   if (dofs_per_thread < -1) return fail(ctx, HZ_EINVAL, "hz_partition: dofs_per_thread < -1");
   free_partition(ctx);
+  ctx->flags = fl;
+  ctx->worder = 0;
   const int P = ctx->p;
   // ex, ey: elements per subdomain side; for a ragged partition (general quads only, reading R25) the maximum
   ctx->sx = sx; ctx->sy = sy; ctx->ex = (ctx->nx + sx - 1) / sx; ctx->ey = (ctx->ny + sy - 1) / sy;
@@ -480,14 +522,9 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
   Layout blay{};
   int sm_count = 148, dev = 0;
   if (cudaGetDevice(&dev) == cudaSuccess) cudaDeviceGetAttribute(&sm_count, cudaDevAttrMultiProcessorCount, dev);
-  const char *env_ws = std::getenv("HZ_DISABLE_WS");  // debug knob: force the non-specialised tile kernel
-  const bool no_ws = env_ws && env_ws[0] == '1';
-  const char *env_cl = std::getenv("HZ_DISABLE_CLUSTER");  // debug knob: never pick a cluster kernel
-  const bool no_cl = env_cl && env_cl[0] == '1';
-  const char *env_fc = std::getenv("HZ_FORCE_CLUSTER");  // debug knob: only cluster kernels of this size compete
-  const int force_cl = env_fc ? std::atoi(env_fc) : 0;
-  const char *env_rc = std::getenv("HZ_NO_REGCAP");  // debug knob: never pick a register-capped instantiation
-  const bool no_regcap = env_rc && env_rc[0] == '1';
+  const bool no_ws = fl.no_warp_spec != 0, no_cl = fl.cluster == -1, no_regcap = fl.no_reg_cap != 0;
+  const int force_cl = fl.cluster > 1 ? fl.cluster : 0;
+  const long long Lsel = fl.grid_blocks > 0 ? fl.grid_blocks : (long long)sx * sy;  // grid size the choice assumes
   auto tile_fit = [&](const TileEntry &t, Layout *lo, SweepLaunch *la) -> bool {
     if (t.p != P || ctx->ex % t.mx || ctx->ey % t.my) return false;
     if (force_cl > 1 && t.cl != force_cl) return false;
@@ -529,6 +566,7 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
     q.NT = ntv; q.NS = q.TX * q.TY * ntv;
     if (sm > smem_cap) return false;
     *lo = q; la->blocks = ctx->L * t.cl; la->threads = nthr; la->smem = sm;
+    if (t.cl > 1 && !cluster_schedulable(t, *la)) return false;  // e.g. a GPC that cannot co-schedule t.cl such CTAs
     return true;
   };
   const bool complex_f = ctx->d_fim != nullptr;
@@ -568,7 +606,7 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
       // prefer the warp-specialised kernel, then register-resident coefficients, then the smaller tile
       // (more threads, better latency hiding); among otherwise equal instantiations take the
       // register-capped one (higher occupancy, a few spills) only when the grid can fill that occupancy
-      if (t.minb > 1 && ((long long)ctx->L < (long long)sm_count * t.minb || no_regcap)) continue;
+      if (t.minb > 1 && (Lsel < (long long)sm_count * t.minb || no_regcap)) continue;
       auto score_of = [&](const TileEntry &q) {
         const long long k_ = (long long)q.mx * P * q.my * P;
         // register-resident coefficients first; there the warp-specialised kernel wins and tiles of 9..16 DOFs
@@ -602,6 +640,10 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
     ctx->mx = tiles[best].mx; ctx->my = tiles[best].my; ctx->csm = tiles[best].csm; ctx->ws = tiles[best].ws;
     ctx->cl = tiles[best].cl;
     ctx->entry = best;
+    // warp-role order of k_sweep_ws: a 3-warp block (2 bulk + 1 edge) puts its edge warp in the middle, so that the bulk
+    // warps of the blocks resident on an SM (consecutive hardware warp slots, slot mod 4 = sub-partition) spread evenly
+    // over the 4 schedulers (measured: config 2 fp32 0.147 -> 0.111 ms per sweep, config 3 fp32 1.273 -> 1.241 ms)
+    ctx->worder = fl.warp_order > 0 ? fl.warp_order - 1 : ((ctx->ws && bl.threads == 96) ? 1 : 0);
   } else if (streamed) {
     lay.variant = 2; lay.NT = N < 1024 ? roundup(N, 32) : 1024; lay.NS = roundup(N, 32); lay.TX = lay.TY = 1;
     lay.ntx = lay.nty = 0;
@@ -680,6 +722,7 @@ hz_status hz_partition(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_prec 
     inf.dofs_per_thread = ctx->lay.variant == 0 ? 1 : (ctx->lay.variant == 2 ? -1 : ctx->lay.TX * ctx->lay.TY);
     if (ctx->lay.variant == 3) inf.dofs_per_thread = (P + 1) * (P + 1);  // incl. the replicated shared nodes
     inf.tile_mx = ctx->mx; inf.tile_my = ctx->my; inf.cluster_size = ctx->lay.variant == 1 ? ctx->cl : 1;
+    inf.subs_per_block = 1;
     inf.dt = ctx->dt; inf.theta = ctx->theta; inf.sigma = ctx->sigma;
     inf.smem_bytes = ctx->launch.smem; inf.workspace_bytes = ws;
     *info_out = inf;
@@ -703,7 +746,10 @@ hz_status hz_ddm_solve(hz_ctx *ctx, const hz_solve_opts *opts, void *u_out, hz_s
   const int n = opts->n_outer_max;
   const bool checking = opts->tol > 0.0 && opts->check_every > 0;
   const bool graph = opts->use_graph && n > 1;
-  std::vector<cudaEvent_t> ev(graph ? (size_t)1 : (size_t)2 * n + 2);
+  // plain launches: three events per sweep (before the sweep, between sweep and exchange, after the exchange), so
+  // that the residual checks between two sweeps are not billed to the sweep; [3n] = start of the call
+  std::vector<cudaEvent_t> ev(graph ? (size_t)1 : (size_t)3 * n + 1);
+  const size_t ev_start = graph ? 0 : (size_t)3 * n;
   for (auto &e : ev) HZ_CUDA(cudaEventCreate(&e));
   auto cleanup = [&]() { for (auto &e : ev) cudaEventDestroy(e); };
   double rel = -1.0;
@@ -739,7 +785,7 @@ hz_status hz_ddm_solve(hz_ctx *ctx, const hz_solve_opts *opts, void *u_out, hz_s
       if (ce != cudaSuccess) { cleanup(); return cuda_fail(ctx, ce, "hz_ddm_solve (graph capture)"); }
       ctx->g_chunk = chunk; ctx->g_nwh = opts->n_wh; ctx->g_warm = opts->warm_start; ctx->g_relax = opts->relax;
     }
-    ce = cudaEventRecord(ev[0], st);
+    ce = cudaEventRecord(ev[ev_start], st);
     while (done < n && ce == cudaSuccess) {
       const int m = n - done < chunk ? n - done : chunk;
       if (m == chunk) {
@@ -759,16 +805,18 @@ hz_status hz_ddm_solve(hz_ctx *ctx, const hz_solve_opts *opts, void *u_out, hz_s
       }
     }
   } else {
-    ce = cudaEventRecord(ev[0], st);
+    ce = cudaEventRecord(ev[ev_start], st);
     for (int it = 0; it < n && ce == cudaSuccess; ++it) {
+      ce = cudaEventRecord(ev[3 * it], st);
+      if (ce != cudaSuccess) break;
       ce = launch_sweep(ctx, opts, st);
       if (ce != cudaSuccess) break;
-      ce = cudaEventRecord(ev[1 + 2 * it], st);
+      ce = cudaEventRecord(ev[3 * it + 1], st);
       if (ce != cudaSuccess) break;
       ce = launch_exchange(ctx, opts->relax, st);
       if (ce != cudaSuccess) break;
       ++nexch;
-      ce = cudaEventRecord(ev[2 + 2 * it], st);
+      ce = cudaEventRecord(ev[3 * it + 2], st);
       if (ce != cudaSuccess) break;
       ++done;
       if (checking && (done % opts->check_every == 0 || done == n)) {
@@ -793,13 +841,13 @@ hz_status hz_ddm_solve(hz_ctx *ctx, const hz_solve_opts *opts, void *u_out, hz_s
       inf.exch_ms_total = -1.0;
     } else {
       for (int it = 0; it < done; ++it) {
-        cudaEventElapsedTime(&ms, ev[2 * it], ev[2 * it + 1]);
+        cudaEventElapsedTime(&ms, ev[3 * it], ev[3 * it + 1]);
         inf.sweep_ms_total += ms;
-        cudaEventElapsedTime(&ms, ev[2 * it + 1], ev[2 * it + 2]);
+        cudaEventElapsedTime(&ms, ev[3 * it + 1], ev[3 * it + 2]);
         inf.exch_ms_total += ms;
       }
     }
-    cudaEventElapsedTime(&ms, ev[0], ev_end);
+    cudaEventElapsedTime(&ms, ev[ev_start], ev_end);
     inf.total_ms = ms;
     inf.dof_timesteps = (double)ctx->L * ctx->lay.lnx * ctx->lay.lny * (double)opts->n_wh * (ctx->n_t - 1) * done;
     inf.sweep_launches = done; inf.exch_launches = nexch; inf.other_launches = other;
@@ -868,10 +916,13 @@ hz_status hz_ddm_solve_sources(hz_ctx *ctx, const hz_solve_opts *opts, int n_src
       HZ_CUDA(cudaEventCreateWithFlags(&ctx->ev_down[b], cudaEventDisableTiming));
     }
   }
-  for (int b = 0; b < 2; ++b) {  // the gathered field has the partition's precision, which may have changed
-    if (ctx->d_ubuf[b]) cudaFree(ctx->d_ubuf[b]);
-    ctx->d_ubuf[b] = nullptr;
-    HZ_CUDA(cudaMalloc(&ctx->d_ubuf[b], 2 * nn * rs));
+  if (ctx->ubuf_bytes != 2 * nn * rs) {  // the gathered field has the partition's precision, which may have changed
+    for (int b = 0; b < 2; ++b) {
+      if (ctx->d_ubuf[b]) cudaFree(ctx->d_ubuf[b]);
+      ctx->d_ubuf[b] = nullptr;
+      HZ_CUDA(cudaMalloc(&ctx->d_ubuf[b], 2 * nn * rs));
+    }
+    ctx->ubuf_bytes = 2 * nn * rs;
   }
   cudaEvent_t e0, e1;
   HZ_CUDA(cudaEventCreate(&e0));
@@ -890,7 +941,11 @@ hz_status hz_ddm_solve_sources(hz_ctx *ctx, const hz_solve_opts *opts, int n_src
     if (ce == cudaSuccess) ce = cudaStreamWaitEvent(st, ctx->ev_up[b], 0);
     if (ce != cudaSuccess) break;
     hz_status bst = ctx->prec == HZ_F32 ? run_build<float>(ctx, 1, st, ctx->d_fstage[b]) : run_build<double>(ctx, 1, st, ctx->d_fstage[b]);
-    if (bst != HZ_OK) { cudaEventDestroy(e0); cudaEventDestroy(e1); return bst; }
+    if (bst != HZ_OK) {
+      cudaStreamSynchronize(ctx->s_in); cudaStreamSynchronize(ctx->s_out); cudaStreamSynchronize(st);
+      cudaEventDestroy(e0); cudaEventDestroy(e1);
+      return bst;
+    }
     ce = cudaEventRecord(ctx->ev_build[b], st);
     ++launches;
     if (ce == cudaSuccess && opts->reset_state) {
@@ -981,10 +1036,10 @@ hz_status gmres_impl(hz_ctx *ctx, const hz_gmres_opts *o, void *u_out, hz_gmres_
     k_axpys<real><<<nblk, bs, 0, st>>>(n, w, Vb, n, nv, dcoef);
     return cudaGetLastError();
   };
-  cudaEvent_t e0, e1;
-  HZ_CUDA(cudaEventCreate(&e0));
-  HZ_CUDA(cudaEventCreate(&e1));
-  HZ_CUDA(cudaEventRecord(e0, st));
+  EventGuard e0, e1;  // destroyed on every return path
+  HZ_CUDA(cudaEventCreate(&e0.e));
+  HZ_CUDA(cudaEventCreate(&e1.e));
+  HZ_CUDA(cudaEventRecord(e0.e, st));
   // x0 and c = F(0)
   if (o->reset_state) HZ_CUDA(cudaMemsetAsync(x, 0, n * rs, st));
   else HZ_CUDA(cudaMemcpyAsync(x, state, n * rs, cudaMemcpyDeviceToDevice, st));
@@ -1088,12 +1143,10 @@ hz_status gmres_impl(hz_ctx *ctx, const hz_gmres_opts *o, void *u_out, hz_gmres_
     if (s2 != HZ_OK) return s2;
   }
   if (u_out) HZ_CUDA(launch_gather(ctx, u_out, ctx->prec, st));
-  HZ_CUDA(cudaEventRecord(e1, st));
+  HZ_CUDA(cudaEventRecord(e1.e, st));
   HZ_CUDA(cudaStreamSynchronize(st));
   float ms = 0.f;
-  cudaEventElapsedTime(&ms, e0, e1);
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
+  cudaEventElapsedTime(&ms, e0.e, e1.e);
   if (info) {
     hz_gmres_info inf{};
     inf.steps_done = steps; inf.sweeps_done = sweeps; inf.cycles = cycles; inf.lin_residual = lin;
@@ -1176,6 +1229,94 @@ hz_status minres_impl(hz_ctx *ctx, const hz_minres_opts *o, int *iters_out, doub
 }
 
 }  // namespace
+
+// ---------------------------------------------------------------------------------------------------------------
+// hz_ddm_solve_mixed: defect correction in the DDM state space, X in fp64 on `hi`, corrections in fp32 on `lo`
+// (reading R27; oracle: ddm_mixed_cycle)
+// ---------------------------------------------------------------------------------------------------------------
+extern "C" hz_status hz_ddm_solve_mixed(hz_ctx *lo, hz_ctx *hi, const hz_mixed_opts *opts, double *u_out,
+                                        hz_mixed_info *info, void *stream) {
+  if (!lo || !hi) return HZ_EINVAL;
+  hz_ctx *ctx = hi;  // error messages and the HZ_CUDA macro report on `hi`
+  if (!opts) return fail(ctx, HZ_EINVAL, "hz_ddm_solve_mixed: NULL opts");
+  if (!lo->part || !hi->part) return fail(ctx, HZ_ESTATE, "hz_ddm_solve_mixed: call hz_partition on both contexts first");
+  if (lo->prec != HZ_F32 || hi->prec != HZ_F64)
+    return fail(ctx, HZ_ESTATE, "hz_ddm_solve_mixed: `lo` must be partitioned with HZ_F32 and `hi` with HZ_F64");
+  if (lo->general || hi->general || lo->d_fim || hi->d_fim)
+    return fail(ctx, HZ_EUNSUPPORTED, "hz_ddm_solve_mixed: uniform-mesh contexts with a real source only");
+  if (lo->nx != hi->nx || lo->ny != hi->ny || lo->p != hi->p || lo->sx != hi->sx || lo->sy != hi->sy || lo->n_t != hi->n_t ||
+      lo->x0 != hi->x0 || lo->x1 != hi->x1 || lo->y0 != hi->y0 || lo->y1 != hi->y1 || lo->omega != hi->omega)
+    return fail(ctx, HZ_EINVAL, "hz_ddm_solve_mixed: the two contexts differ in mesh, frequency, partition or N_t");
+  if (opts->n_cycles_max < 0 || opts->m_inner < 1 || opts->n_wh < 1 || !(opts->relax > 0.0) || opts->relax > 1.0)
+    return fail(ctx, HZ_EINVAL, "hz_ddm_solve_mixed: need n_cycles_max >= 0, m_inner >= 1, n_wh >= 1, relax in (0,1]");
+  cudaStream_t st = (cudaStream_t)stream;
+  const long long nlam = (long long)hi->L * 8 * hi->E;
+  const long long ncan = nlam + (long long)hi->L * 2 * hi->lay.lnx * hi->lay.lny;  // canonical elements of the state
+  if (!hi->d_mix) HZ_CUDA(cudaMalloc(&hi->d_mix, (size_t)hi->n_state * sizeof(double)));
+  if (!lo->d_mix) {
+    HZ_CUDA(cudaMalloc(&lo->d_mix, (size_t)lo->n_state * sizeof(float)));
+    HZ_CUDA(cudaMemsetAsync(lo->d_mix, 0, (size_t)lo->n_state * sizeof(float), st));  // padding slots stay zero
+  }
+  if (!lo->d_bbf_zero) {
+    HZ_CUDA(cudaMalloc(&lo->d_bbf_zero, (size_t)lo->L * lo->lay.NS * sizeof(float)));
+    HZ_CUDA(cudaMemsetAsync(lo->d_bbf_zero, 0, (size_t)lo->L * lo->lay.NS * sizeof(float), st));
+  }
+  double *Xold = (double *)hi->d_mix, *Sh = (double *)hi->d_lam;
+  float *Dl = (float *)lo->d_mix, *Sl = (float *)lo->d_lam;
+  if (opts->reset_state) {
+    HZ_CUDA(cudaMemsetAsync(hi->d_lam, 0, (size_t)hi->n_state * sizeof(double), st));
+    HZ_CUDA(cudaMemsetAsync(hi->d_g, 0, (size_t)nlam * sizeof(double), st));
+  }
+  HZ_CUDA(cudaMemsetAsync(lo->d_lam, 0, (size_t)lo->n_state * sizeof(float), st));
+  hz_solve_opts so{};
+  so.n_wh = opts->n_wh; so.warm_start = 1; so.relax = opts->relax;
+  EventGuard e0, e1;
+  HZ_CUDA(cudaEventCreate(&e0.e));
+  HZ_CUDA(cudaEventCreate(&e1.e));
+  HZ_CUDA(cudaEventRecord(e0.e, st));
+  const bool checking = opts->tol > 0.0 && opts->check_every > 0;
+  const unsigned nbc = (unsigned)((ncan + 255) / 256);
+  int cycles = 0, nlo = 0, nhi = 0;
+  double rel = -1.0;
+  for (int cy = 0; cy < opts->n_cycles_max; ++cy) {
+    if (opts->m_inner > 1) HZ_CUDA(cudaMemcpyAsync(Xold, Sh, (size_t)hi->n_state * sizeof(double), cudaMemcpyDeviceToDevice, st));
+    HZ_CUDA(launch_sweep(hi, &so, st));                // F(X) at full precision
+    HZ_CUDA(launch_exchange(hi, opts->relax, st));
+    ++nhi;
+    if (opts->m_inner > 1) {
+      k_mixed_defect<<<nbc, 256, 0, st>>>(ncan, nlam, hi->lay, lo->lay, Sh, Xold, Sl, Dl);
+      HZ_CUDA(cudaGetLastError());
+      for (int k = 1; k < opts->m_inner; ++k) {        // delta_{k+1} = T delta_k + D
+        HZ_CUDA(launch_sweep(lo, &so, st, /*homog=*/true));
+        HZ_CUDA(launch_exchange(lo, opts->relax, st));
+        k_add_f32<<<1184, 256, 0, st>>>(lo->n_state, Sl, Dl);
+        HZ_CUDA(cudaGetLastError());
+        ++nlo;
+      }
+      k_mixed_update<<<nbc, 256, 0, st>>>(ncan, nlam, hi->lay, lo->lay, Sh, Xold, Sl);
+      HZ_CUDA(cudaGetLastError());
+    }
+    ++cycles;
+    if (checking && (cycles % opts->check_every == 0 || cycles == opts->n_cycles_max)) {
+      HZ_CUDA(launch_gather(hi, hi->d_ures, HZ_F64, st));
+      hz_status s2 = residual_impl(hi, hi->d_ures, HZ_F64, &rel, st);
+      if (s2 != HZ_OK) return s2;
+      if (rel <= opts->tol) break;
+    }
+  }
+  if (u_out) HZ_CUDA(launch_gather(hi, u_out, HZ_F64, st));
+  HZ_CUDA(cudaEventRecord(e1.e, st));
+  HZ_CUDA(cudaStreamSynchronize(st));
+  if (info) {
+    hz_mixed_info inf{};
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0.e, e1.e);
+    inf.cycles_done = cycles; inf.sweeps_lo = nlo; inf.sweeps_hi = nhi; inf.rel_residual = rel; inf.total_ms = ms;
+    inf.dof_timesteps = (double)hi->L * hi->lay.lnx * hi->lay.lny * (double)opts->n_wh * (hi->n_t - 1) * (double)(nlo + nhi);
+    *info = inf;
+  }
+  return HZ_OK;
+}
 
 extern "C" hz_status hz_minres_cycle(hz_ctx *ctx, const hz_minres_opts *opts, int *iters_out, double *res_out,
                                      hz_minres_info *info, void *stream) {
@@ -1280,46 +1421,6 @@ void hz_destroy(hz_ctx *ctx) {
   double **ptrs[] = {&ctx->d_c, &ctx->d_fre, &ctx->d_fim, &ctx->d_bc, &ctx->d_vx, &ctx->d_vy};
   for (double **q : ptrs) { if (*q) cudaFree(*q); *q = nullptr; }
   delete ctx;
-}
-
-hz_status hz_peak_probe(int kind, double *result, void *stream) {
-  if (!result || kind < 0 || kind > 1) return HZ_EINVAL;
-  cudaStream_t st = (cudaStream_t)stream;
-  cudaDeviceProp prop;
-  int dev = 0;
-  if (cudaGetDevice(&dev) != cudaSuccess || cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return HZ_ECUDA;
-  const int sms = prop.multiProcessorCount;
-  cudaEvent_t e0, e1;
-  if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return HZ_ECUDA;
-  float *d_out = nullptr;
-  if (cudaMalloc((void **)&d_out, 64) != cudaSuccess) return HZ_ECUDA;
-  double best = 0.0;
-  for (int rep = 0; rep < 5; ++rep) {
-    float ms = 0.f;
-    double work = 0.0;
-    if (kind == 0) {
-      const int iters = 4096, blocks = sms * 8, thr = 256;
-      cudaEventRecord(e0, st);
-      k_probe_fma<float><<<blocks, thr, 0, st>>>(iters, 1.0f, d_out);
-      cudaEventRecord(e1, st);
-      work = 2.0 * 64.0 * iters * (double)blocks * thr;
-    } else {
-      const int iters = 2048, blocks = sms * 8, thr = 256;
-      cudaEventRecord(e0, st);
-      k_probe_fma<double><<<blocks, thr, 0, st>>>(iters, 1.0, (double *)d_out);
-      cudaEventRecord(e1, st);
-      work = 2.0 * 64.0 * iters * (double)blocks * thr;
-    }
-    if (cudaStreamSynchronize(st) != cudaSuccess || cudaGetLastError() != cudaSuccess) { cudaFree(d_out); return HZ_ECUDA; }
-    cudaEventElapsedTime(&ms, e0, e1);
-    const double rate = work / (ms * 1e-3) / 1e12;
-    if (rate > best) best = rate;
-  }
-  cudaFree(d_out);
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
-  *result = best;
-  return HZ_OK;
 }
 
 }  // extern "C"

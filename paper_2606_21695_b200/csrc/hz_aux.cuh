@@ -323,24 +323,44 @@ __global__ void k_convert(long long n, const A *__restrict__ in, B *__restrict__
 }
 
 // ---------------------------------------------------------------------------------------------
-// Peak probe (no method arithmetic): independent FMA streams.
+// State transfer of the mixed-precision defect correction (hz_ddm_solve_mixed; reading R27).
+// The joint state (lambda | u_l) of the fp64 context `hi` and of the fp32 context `lo` share the lambda layout
+// [L][4][2][E] but not the node slot map (each precision picks its own thread tile).  One thread per canonical
+// element: q < nlam is a lambda entry, q >= nlam is (l, re/im, node).
+//   k_mixed_defect :  D = hi_new - hi_old (fp64)  ->  lo_state = lo_D = (float) D          (delta_1 = D)
+//   k_mixed_update :  hi_state = hi_old + (double) lo_state                                  (X <- X + delta_m)
 // ---------------------------------------------------------------------------------------------
-template <typename real>
-__global__ void __launch_bounds__(256) k_probe_fma(int iters, real seed, real *out) {
-  real a[16];
-#pragma unroll
-  for (int q = 0; q < 16; ++q) a[q] = seed + real(q) * real(1e-3) + real(threadIdx.x) * real(1e-6);
-  const real m = real(0.999), c = real(1e-4);
-  for (int it = 0; it < iters; ++it) {
-#pragma unroll
-    for (int r = 0; r < 4; ++r)
-#pragma unroll
-      for (int q = 0; q < 16; ++q) a[q] = a[q] * m + c;
-  }
-  real s = 0;
-#pragma unroll
-  for (int q = 0; q < 16; ++q) s += a[q];
-  if (s == real(-12345)) out[0] = s;
+__device__ __forceinline__ void mixed_index(long long q, long long nlam, Layout lh, Layout ll, size_t *ih, size_t *il) {
+  if (q < nlam) { *ih = (size_t)q; *il = (size_t)q; return; }
+  const long long r = q - nlam;
+  const int N = lh.lnx * lh.lny;
+  const int node = (int)(r % N), c = (int)((r / N) % 2);
+  const long long l = r / (2 * N);
+  const int i = node % lh.lnx, j = node / lh.lnx;
+  *ih = (size_t)nlam + (size_t)l * 2 * lh.NS + (size_t)c * lh.NS + lh.slot(i, j);
+  *il = (size_t)nlam + (size_t)l * 2 * ll.NS + (size_t)c * ll.NS + ll.slot(i, j);
+}
+static __global__ void k_mixed_defect(long long total, long long nlam, Layout lh, Layout ll, const double *__restrict__ hi_new,
+                                      const double *__restrict__ hi_old, float *__restrict__ lo_state, float *__restrict__ lo_D) {
+  const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= total) return;
+  size_t ih, il;
+  mixed_index(q, nlam, lh, ll, &ih, &il);
+  const float d = (float)(hi_new[ih] - hi_old[ih]);
+  lo_state[il] = d;
+  lo_D[il] = d;
+}
+static __global__ void k_mixed_update(long long total, long long nlam, Layout lh, Layout ll, double *__restrict__ hi_state,
+                                      const double *__restrict__ hi_old, const float *__restrict__ lo_state) {
+  const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (q >= total) return;
+  size_t ih, il;
+  mixed_index(q, nlam, lh, ll, &ih, &il);
+  hi_state[ih] = hi_old[ih] + (double)lo_state[il];
+}
+// x += y over the whole flat state
+static __global__ void k_add_f32(long long n, float *__restrict__ x, const float *__restrict__ y) {
+  for (long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x; e < n; e += (long long)gridDim.x * blockDim.x) x[e] += y[e];
 }
 
 }  // namespace hz

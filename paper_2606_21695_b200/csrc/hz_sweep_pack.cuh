@@ -1,0 +1,401 @@
+// hz_sweep_pack.cuh — SEVERAL SMALL SUBDOMAINS PER THREAD BLOCK (config 5: 25 .. 289-DOF subdomains, PAPER.md:231,
+// the B = 256, T = 1 corner of the paper's sweep; "several subdomains per warp/block needed").
+//
+// A 25-DOF subdomain is 1 full thread tile + 3 edge pieces at p = 1: one block per subdomain leaves most lanes of its
+// two warps idle and pays the block's fixed costs 2.4 million times.  Here a block holds G subdomains: the full
+// tiles of ALL of them fill the "bulk" warps (lane h -> subdomain h / NB, tile h % NB), the one-line edge pieces of
+// all of them fill the "edge" warps, so the roles stay warp-uniform as in k_sweep_ws (hz_sweep_ws.cuh) and the
+// lanes are dense.  Same arithmetic, same exchange-record protocol, same association of every sum as k_sweep_ws
+// (bit-identical results); what changes is the indexing: every subdomain has its own compact slice of shared
+// memory (ntx*nty records + one zero record + the along-the-edge arrays) and the per-node global arrays use the
+// unrounded tile count as their stride (Layout::NT = ntx*nty), so a 25-DOF subdomain occupies 36 slots, not 128.
+// One named barrier per time step for the whole block: all subdomains share N_t and run in lockstep.
+#pragma once
+#include "hz_line.cuh"
+
+namespace hz {
+
+template <typename real, int P, int M, int MAXT>
+__global__ void __launch_bounds__(MAXT, 1) k_sweep_pack(const SweepArgs<real> A, const __grid_constant__ TabC<real> TC) {
+  constexpr int T = M * P;
+  constexpr int V16 = 16 / (int)sizeof(real);
+  constexpr int CH = (T + V16 - 1) / V16 * V16;
+  constexpr int RS = 4 * CH + V16;  // record: PX | RX | PY | RY + 16 bytes (odd number of 16-byte units)
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int NTH = blockDim.x, h = threadIdx.x, G = A.pack;
+  const int ntx = A.lay.ntx, nty = A.lay.nty, NTV = A.lay.NT, NS = A.lay.NS;
+  const int lnx = A.lay.lnx, lny = A.lay.lny;
+  const int NB = (ntx - 1) * (nty - 1), NE = ntx + nty - 1;
+  const int bulkW = (G * NB + 31) & ~31;         // lanes of the bulk warps
+  const int NEP = (NE + V16 - 1) / V16 * V16;
+  const int ZR = NTV;                            // the zero record of a slice
+  const int EAO = (NTV + 1) * RS;                // in a slice, after the records: PA[NEP] | RA[NEP]
+  const int SW = EAO + 2 * NEP;                  // words per subdomain slice
+  const int BUFW = G * SW + RS;                  // per buffer: G slices + one scratch record for idle lanes
+  real *xb = reinterpret_cast<real *>(smem_raw);
+  const int SCRo = G * SW;                       // offset of the scratch record
+
+  for (int q = h; q < 2 * BUFW; q += NTH) xb[q] = real(0);
+  const real sigma = A.sigma;
+
+  if (h < bulkW) {
+    // ============================ bulk tiles: full T x T node tiles ============================
+    const int g = h / NB, t = h - g * NB;
+    const int l = blockIdx.x * G + g;
+    const bool act = h < G * NB && l < A.L;
+    const int tx = act ? t % (ntx - 1) : 0, ty = act ? t / (ntx - 1) : 0;
+    const int v = ty * ntx + tx;
+    real *sl = xb + (act ? g : 0) * SW;          // this subdomain's slice (buffer 0)
+    real *pMy = act ? sl + v * RS : xb + SCRo;
+    const real *pL = sl + ((act && tx > 0) ? v - 1 : ZR) * RS, *pR = sl + (act ? v + 1 : ZR) * RS;
+    const real *pD = sl + ((act && ty > 0) ? v - ntx : ZR) * RS, *pU = sl + (act ? v + ntx : ZR) * RS;
+    real *pMyRX = pMy + CH;
+    const bool hasL = tx > 0, hasD = ty > 0;
+    const real d0x = A.ex1.k0[0] + (hasL ? A.ex1.kp[P] : real(0));
+    const real d0y = A.ey1.k0[0] + (hasD ? A.ey1.kp[P] : real(0));
+    const real s0x = hasL ? real(1) : real(2), s0y = hasD ? real(1) : real(2);
+    const int lc = act ? l : 0;
+    const int six = lc % A.sx, siy = lc / A.sx;
+    const size_t lbase = (size_t)lc * 4 * 2 * A.E, ebase = (size_t)lc * 4 * A.E;
+
+    real p[T][T], pd[T][T], vr[T][T], vi[T][T], ur[T][T], ui[T][T], gam[T][T], bbr[T][T];
+    real alc[T], bic[T], alr[T], bir[T];
+    const size_t base = (size_t)lc * NS + v;
+#pragma unroll
+    for (int b = 0; b < T; ++b)
+#pragma unroll
+      for (int a = 0; a < T; ++a) {
+        const size_t o = base + (size_t)(b * T + a) * NTV;
+        gam[b][a] = act ? A.gamma[o] : real(0);
+        bbr[b][a] = act ? A.bbf_re[o] : real(0);
+        ur[b][a] = (act && A.warm) ? A.u_sub[(size_t)lc * 2 * NS + (size_t)(b * T + a) * NTV + v] : real(0);
+        ui[b][a] = (act && A.warm) ? A.u_sub[(size_t)lc * 2 * NS + NS + (size_t)(b * T + a) * NTV + v] : real(0);
+      }
+#pragma unroll
+    for (int b = 0; b < T; ++b) {
+      const size_t o = base + (size_t)(b * T) * NTV;
+      alc[b] = act ? A.alpha[o] : real(0);
+      bic[b] = (act && A.bbf_im) ? A.bbf_im[o] : real(0);
+    }
+#pragma unroll
+    for (int a = 0; a < T; ++a) {
+      const size_t o = base + (size_t)a * NTV;
+      alr[a] = act ? A.alpha[o] : real(0);
+      bir[a] = (act && A.bbf_im) ? A.bbf_im[o] : real(0);
+    }
+    // Assemble b from lambda^n: bulk tiles touch only the W side (tx = 0) and the S side (ty = 0)
+    const bool onW = act && tx == 0 && six > 0, onS = act && ty == 0 && siy > 0;
+    if (onW) {
+#pragma unroll
+      for (int b = 0; b < T; ++b) {
+        const int j = ty * T + b;
+        const real s = A.bs[ebase + kSideW * A.E + j];
+        bbr[b][0] = fmaT(s, A.lam[lbase + (kSideW * 2 + 0) * A.E + j], bbr[b][0]);
+        bic[b] = fmaT(s, A.lam[lbase + (kSideW * 2 + 1) * A.E + j], bic[b]);
+      }
+    }
+    if (onS) {
+#pragma unroll
+      for (int a = 0; a < T; ++a) {
+        const int i = tx * T + a;
+        const real s = A.bs[ebase + kSideS * A.E + i];
+        const real li_ = A.lam[lbase + (kSideS * 2 + 1) * A.E + i];
+        bbr[0][a] = fmaT(s, A.lam[lbase + (kSideS * 2 + 0) * A.E + i], bbr[0][a]);
+        if (a == 0) bic[0] = fmaT(s, li_, bic[0]);
+        else bir[a] = fmaT(s, li_, bir[a]);
+      }
+    }
+    bar_sync_all(NTH);
+
+    int cur = 0;
+    for (int m = 0; m < A.n_wh; ++m) {
+      const Tab4<real> t0 = TC.t[0];
+#pragma unroll
+      for (int b = 0; b < T; ++b)
+#pragma unroll
+        for (int a = 0; a < T; ++a) {  // WaveHoltz init (readings R2, R8)
+          p[b][a] = ur[b][a];
+          pd[b][a] = A.omega * (ui[b][a] * A.cos_h - ur[b][a] * A.sin_h);
+          vr[b][a] = t0.k * p[b][a];
+          vi[b][a] = t0.kh * pd[b][a];
+        }
+#pragma unroll 1
+      for (int nu = 1; nu < A.n_t; ++nu) {
+#pragma unroll
+        for (int b = 0; b < T; ++b)
+#pragma unroll
+          for (int a = 0; a < T; ++a) p[b][a] = fmaT(sigma, pd[b][a], p[b][a]);
+        {
+          real *my = pMy + cur;
+          real oPX[T], oRX[T], oPY[T], oRY[T];
+#pragma unroll
+          for (int b = 0; b < T; ++b) {
+            real q[T + 1];
+#pragma unroll
+            for (int a = 0; a < T; ++a) q[a] = p[b][a];
+            q[T] = real(0);
+            oPX[b] = line_partial<real, P, M>(q, A.ex1);
+            oRX[b] = p[b][0];
+          }
+#pragma unroll
+          for (int a = 0; a < T; ++a) {
+            real q[T + 1];
+#pragma unroll
+            for (int b = 0; b < T; ++b) q[b] = p[b][a];
+            q[T] = real(0);
+            oPY[a] = line_partial<real, P, M>(q, A.ey1);
+            oRY[a] = p[0][a];
+          }
+          st_chunk<T>(my, oPX);
+          st_chunk<T>(my + CH, oRX);
+          st_chunk<T>(my + 2 * CH, oPY);
+          st_chunk<T>(my + 3 * CH, oRY);
+        }
+        bar_sync_all(NTH);
+        real qR[T], piL[T], qU[T], piD[T];
+        ld_chunk<T>(pL + cur, piL);
+        ld_chunk<T>(pR + cur + CH, qR);
+        ld_chunk<T>(pD + cur + 2 * CH, piD);
+        ld_chunk<T>(pU + cur + 3 * CH, qU);
+        cur = BUFW - cur;
+        const Tab4<real> tn = TC.t[nu];
+        real S[T][T], X0[T], Y0[T];
+#pragma unroll
+        for (int b = 0; b < T; ++b) {
+          real q[T + 1];
+#pragma unroll
+          for (int a = 0; a < T; ++a) q[a] = p[b][a];
+          q[T] = real(0);
+          X0[b] = line_own<real, P, M, false>(q, d0x, A.ex1, S[b]);
+        }
+#pragma unroll
+        for (int a = 0; a < T; ++a) {
+          real q[T + 1], Sc[T];
+#pragma unroll
+          for (int b = 0; b < T; ++b) { q[b] = p[b][a]; Sc[b] = S[b][a]; }
+          q[T] = real(0);
+          if (a == 0) Y0[a] = line_own<real, P, M, false>(q, d0y, A.ey1, Sc);
+          else Y0[a] = line_own<real, P, M, true>(q, d0y, A.ey1, Sc);
+#pragma unroll
+          for (int b = 1; b < T; ++b) S[b][a] = Sc[b];
+        }
+#pragma unroll
+        for (int b = 0; b < T; ++b)
+#pragma unroll
+          for (int a = 0; a < T; ++a) vr[b][a] = fmaT(tn.k, p[b][a], vr[b][a]);
+#pragma unroll
+        for (int b = 0; b < T; ++b) {
+          if (b == 0) line_finish<real, P, M, false>(qR[b], piL[b], s0x, X0[b], A.ex1, S[b]);
+          else line_finish<real, P, M, true>(qR[b], piL[b], s0x, X0[b], A.ex1, S[b]);
+        }
+#pragma unroll
+        for (int a = 0; a < T; ++a) {
+          real Sc[T];
+#pragma unroll
+          for (int b = 0; b < T; ++b) Sc[b] = S[b][a];
+          line_finish<real, P, M, true>(qU[a], piD[a], s0y, Y0[a], A.ey1, Sc);
+#pragma unroll
+          for (int b = 0; b < T; ++b) S[b][a] = Sc[b];
+        }
+#pragma unroll
+        for (int b = 0; b < T; ++b)
+#pragma unroll
+          for (int a = 0; a < T; ++a) {
+            const real g_ = gam[b][a], r_ = bbr[b][a];
+            if (a == 0) {
+              const real x = fmaT(bic[b], tn.s, fmaT(-g_, S[b][a], r_ * tn.c));
+              pd[b][a] = fmaT(alc[b], pd[b][a], x);
+            } else if (b == 0) {
+              const real x = fmaT(bir[a], tn.s, fmaT(-g_, S[b][a], r_ * tn.c));
+              pd[b][a] = fmaT(alr[a], pd[b][a], x);
+            } else {  // interior of the subdomain: alpha = 1, Im b = 0
+              pd[b][a] = fmaT(r_, tn.c, fmaT(-g_, S[b][a], pd[b][a]));
+            }
+            vi[b][a] = fmaT(tn.kh, pd[b][a], vi[b][a]);
+          }
+      }
+#pragma unroll
+      for (int b = 0; b < T; ++b)
+#pragma unroll
+        for (int a = 0; a < T; ++a) {  // eq. (7) prefactor (reading R4)
+          ur[b][a] = A.two_over_nt * vr[b][a];
+          ui[b][a] = A.two_over_nt * vi[b][a];
+        }
+    }
+    if (act) {
+#pragma unroll
+      for (int b = 0; b < T; ++b)
+#pragma unroll
+        for (int a = 0; a < T; ++a) {
+          A.u_sub[(size_t)l * 2 * NS + (size_t)(b * T + a) * NTV + v] = ur[b][a];
+          A.u_sub[(size_t)l * 2 * NS + NS + (size_t)(b * T + a) * NTV + v] = ui[b][a];
+        }
+    }
+    if (onW) {
+#pragma unroll
+      for (int b = 0; b < T; ++b) {
+        const int j = ty * T + b;
+        const real k2 = A.k2edge[ebase + kSideW * A.E + j];
+        A.gout[lbase + (kSideW * 2 + 0) * A.E + j] = fmaT(k2, ui[b][0], -A.lam[lbase + (kSideW * 2 + 0) * A.E + j]);
+        A.gout[lbase + (kSideW * 2 + 1) * A.E + j] = fmaT(-k2, ur[b][0], -A.lam[lbase + (kSideW * 2 + 1) * A.E + j]);
+      }
+    }
+    if (onS) {
+#pragma unroll
+      for (int a = 0; a < T; ++a) {
+        const int i = tx * T + a;
+        const real k2 = A.k2edge[ebase + kSideS * A.E + i];
+        A.gout[lbase + (kSideS * 2 + 0) * A.E + i] = fmaT(k2, ui[0][a], -A.lam[lbase + (kSideS * 2 + 0) * A.E + i]);
+        A.gout[lbase + (kSideS * 2 + 1) * A.E + i] = fmaT(-k2, ur[0][a], -A.lam[lbase + (kSideS * 2 + 1) * A.E + i]);
+      }
+    }
+  } else {
+    // ============================ edge pieces: one line of T nodes per lane ============================
+    // piece e < nty-1: right piece, virtual tile (ntx-1, e), nodes (lnx-1, e*T + n), "along" = y.
+    // piece e >= nty-1: top piece, virtual tile (e-(nty-1), nty-1), nodes (tx*T + n, lny-1), "along" = x;
+    //                   the last one (tx = ntx-1) is the corner and owns node 0 only.
+    const int eh = h - bulkW;
+    const int g = eh / NE, e = eh - g * NE;
+    const int l = blockIdx.x * G + g;
+    const bool act = eh < G * NE && l < A.L;
+    const bool top = act && e >= nty - 1;
+    const int tx = !act ? 0 : (top ? e - (nty - 1) : ntx - 1);
+    const int ty = !act ? 0 : (top ? nty - 1 : e);
+    const int v = ty * ntx + tx;
+    const int ta = top ? tx : ty, nta = top ? ntx : nty;  // position / count along the line direction
+    const int sc = top ? ntx : 1;                         // virtual-tile stride across
+    const int oRC = top ? 3 * CH : CH, oPC = top ? 2 * CH : 0;
+    const bool hasP = act && ta > 0, hasN = act && ta < nta - 1;
+    real *sl = xb + (act ? g : 0) * SW;
+    real *scr = xb + SCRo;
+    real *pRaw = act ? sl + v * RS + oRC : scr;
+    // along-the-edge exchange through the compact arrays PA[e], RA[e].  The last right piece's partial sum has one
+    // reader, the corner, which reads it as a chunk: it goes to element 0 of that piece's own PY chunk.
+    real *pPAout = !act ? scr : ((!top && ty == nty - 2) ? sl + v * RS + 2 * CH : sl + EAO + e);
+    real *pRAout = !act ? scr + 1 : sl + EAO + NEP + e;
+    const real *pP = hasP ? sl + EAO + e - 1 : sl + ZR * RS;
+    const real *pN = hasN ? sl + EAO + NEP + ((!top && ty == nty - 2) ? NE - 1 : e + 1) : sl + ZR * RS;
+    const real *pC = sl + (act ? v - sc : ZR) * RS + oPC;
+    Elem1D<real> ka;  // coefficients along
+#pragma unroll
+    for (int c = 0; c <= P; ++c) {
+      ka.k0[c] = top ? A.ex1.k0[c] : A.ey1.k0[c];
+      ka.kp[c] = top ? A.ex1.kp[c] : A.ey1.kp[c];
+#pragma unroll
+      for (int a = 1; a < P; ++a) ka.kin[a][c] = top ? A.ex1.kin[a][c] : A.ey1.kin[a][c];
+    }
+    const real d0a = (hasN ? ka.k0[0] : real(0)) + (hasP ? ka.kp[P] : real(0));
+    const real s0a = (hasP && hasN) ? real(1) : real(2);
+    const real d0c = top ? A.ey1.kp[P] : A.ex1.kp[P];
+    const real s0c = real(2);
+    const int lc = act ? l : 0;
+    const int six = lc % A.sx, siy = lc / A.sx;
+    const size_t lbase = (size_t)lc * 4 * 2 * A.E, ebase = (size_t)lc * 4 * A.E;
+
+    real p[T], pd[T], vr[T], vi[T], ur[T], ui[T], gam[T], bbr[T], al[T], bbi[T];
+    const size_t base = (size_t)lc * NS + v;
+#pragma unroll
+    for (int n = 0; n < T; ++n) {
+      const size_t o = base + (size_t)(top ? n : n * T) * NTV;  // tile node (a=n,b=0) or (a=0,b=n)
+      gam[n] = act ? A.gamma[o] : real(0);
+      bbr[n] = act ? A.bbf_re[o] : real(0);
+      al[n] = act ? A.alpha[o] : real(0);
+      bbi[n] = (act && A.bbf_im) ? A.bbf_im[o] : real(0);
+      ur[n] = (act && A.warm) ? A.u_sub[(size_t)lc * 2 * NS + (o - (size_t)lc * NS)] : real(0);
+      ui[n] = (act && A.warm) ? A.u_sub[(size_t)lc * 2 * NS + NS + (o - (size_t)lc * NS)] : real(0);
+    }
+    const int side1 = top ? kSideN : kSideE;
+    const bool on1 = act && (top ? siy < A.sy - 1 : six < A.sx - 1);
+    const int len1 = top ? lnx : lny;
+    int side2 = -1, idx2 = 0;
+    if (act && top && tx == 0 && six > 0) { side2 = kSideW; idx2 = lny - 1; }
+    if (act && top && tx == ntx - 1 && six < A.sx - 1) { side2 = kSideE; idx2 = lny - 1; }
+    if (act && !top && ty == 0 && siy > 0) { side2 = kSideS; idx2 = lnx - 1; }
+#pragma unroll
+    for (int n = 0; n < T; ++n) {
+      const int idx = ta * T + n;
+      if (on1 && idx < len1) {
+        const real s = A.bs[ebase + side1 * A.E + idx];
+        bbr[n] = fmaT(s, A.lam[lbase + (side1 * 2 + 0) * A.E + idx], bbr[n]);
+        bbi[n] = fmaT(s, A.lam[lbase + (side1 * 2 + 1) * A.E + idx], bbi[n]);
+      }
+    }
+    if (side2 >= 0) {
+      const real s = A.bs[ebase + side2 * A.E + idx2];
+      bbr[0] = fmaT(s, A.lam[lbase + (side2 * 2 + 0) * A.E + idx2], bbr[0]);
+      bbi[0] = fmaT(s, A.lam[lbase + (side2 * 2 + 1) * A.E + idx2], bbi[0]);
+    }
+    bar_sync_all(NTH);
+
+    int cur = 0;
+    for (int m = 0; m < A.n_wh; ++m) {
+      const Tab4<real> t0 = TC.t[0];
+#pragma unroll
+      for (int n = 0; n < T; ++n) {
+        p[n] = ur[n];
+        pd[n] = A.omega * (ui[n] * A.cos_h - ur[n] * A.sin_h);
+        vr[n] = t0.k * p[n];
+        vi[n] = t0.kh * pd[n];
+      }
+#pragma unroll 1
+      for (int nu = 1; nu < A.n_t; ++nu) {
+        real q[T + 1];
+#pragma unroll
+        for (int n = 0; n < T; ++n) { p[n] = fmaT(sigma, pd[n], p[n]); q[n] = p[n]; }
+        q[T] = real(0);
+        pPAout[cur] = line_partial<real, P, M>(q, ka);
+        pRAout[cur] = p[0];
+        st_chunk<T>(pRaw + cur, p);
+        bar_sync_all(NTH);
+        const real qN = pN[cur], piP = pP[cur];
+        real piC[T];
+        ld_chunk<T>(pC + cur, piC);
+        cur = BUFW - cur;
+        const Tab4<real> tn = TC.t[nu];
+        real S[T];
+        const real a0 = line_own<real, P, M, false>(q, d0a, ka, S);
+        real cown[T];
+#pragma unroll
+        for (int n = 0; n < T; ++n) { cown[n] = d0c * p[n]; vr[n] = fmaT(tn.k, p[n], vr[n]); }
+        line_finish<real, P, M, false>(qN, piP, s0a, a0, ka, S);
+#pragma unroll
+        for (int n = 0; n < T; ++n) S[n] = fmaT(s0c, cown[n] + piC[n], S[n]);
+#pragma unroll
+        for (int n = 0; n < T; ++n) {
+          real x = fmaT(-gam[n], S[n], bbr[n] * tn.c);
+          x = fmaT(bbi[n], tn.s, x);
+          pd[n] = fmaT(al[n], pd[n], x);
+          vi[n] = fmaT(tn.kh, pd[n], vi[n]);
+        }
+      }
+#pragma unroll
+      for (int n = 0; n < T; ++n) {
+        ur[n] = A.two_over_nt * vr[n];
+        ui[n] = A.two_over_nt * vi[n];
+      }
+    }
+    if (act) {
+#pragma unroll
+      for (int n = 0; n < T; ++n) {
+        const size_t o = (size_t)(top ? n : n * T) * NTV + v;
+        const int idx = ta * T + n;
+        if (idx < len1) {   // (the corner piece owns node 0 only)
+          A.u_sub[(size_t)l * 2 * NS + o] = ur[n];
+          A.u_sub[(size_t)l * 2 * NS + NS + o] = ui[n];
+        }
+        if (on1 && idx < len1) {
+          const real k2 = A.k2edge[ebase + side1 * A.E + idx];
+          A.gout[lbase + (side1 * 2 + 0) * A.E + idx] = fmaT(k2, ui[n], -A.lam[lbase + (side1 * 2 + 0) * A.E + idx]);
+          A.gout[lbase + (side1 * 2 + 1) * A.E + idx] = fmaT(-k2, ur[n], -A.lam[lbase + (side1 * 2 + 1) * A.E + idx]);
+        }
+      }
+      if (side2 >= 0) {
+        const real k2 = A.k2edge[ebase + side2 * A.E + idx2];
+        A.gout[lbase + (side2 * 2 + 0) * A.E + idx2] = fmaT(k2, ui[0], -A.lam[lbase + (side2 * 2 + 0) * A.E + idx2]);
+        A.gout[lbase + (side2 * 2 + 1) * A.E + idx2] = fmaT(-k2, ur[0], -A.lam[lbase + (side2 * 2 + 1) * A.E + idx2]);
+      }
+    }
+  }
+}
+
+}  // namespace hz

@@ -21,16 +21,32 @@ HZ_TC_IMPEDANCE0 = 0
 STATUS_NAMES = {0: "HZ_OK", 1: "HZ_EINVAL", 2: "HZ_ENOMEM", 3: "HZ_ECUDA", 4: "HZ_EUNSUPPORTED", 5: "HZ_ESTATE"}
 
 # every symbol include/hz.h declares
-EXPORTS = ("hz_mesh_setup", "hz_mesh_setup_quads", "hz_set_source", "hz_partition", "hz_ddm_solve", "hz_operator_time", "hz_ddm_solve_sources", "hz_ddm_solve_gmres", "hz_minres_cycle", "hz_residual",
-           "hz_get_subdomain_state", "hz_set_subdomain_state", "hz_last_error", "hz_destroy", "hz_peak_probe")
+EXPORTS = ("hz_mesh_setup", "hz_mesh_setup_quads", "hz_set_source", "hz_partition", "hz_partition_ex", "hz_ddm_solve",
+           "hz_operator_time", "hz_ddm_solve_sources", "hz_ddm_solve_gmres", "hz_ddm_solve_mixed", "hz_minres_cycle",
+           "hz_residual", "hz_get_subdomain_state", "hz_set_subdomain_state", "hz_last_error", "hz_destroy")
 
 
 class hz_part_info(C.Structure):
     _fields_ = [("n_t", C.c_int), ("dofs_per_sub", C.c_int), ("edge_nodes_x", C.c_int), ("edge_nodes_y", C.c_int),
                 ("edge_stride", C.c_int), ("threads_per_block", C.c_int), ("blocks", C.c_int),
                 ("dofs_per_thread", C.c_int), ("tile_mx", C.c_int), ("tile_my", C.c_int), ("cluster_size", C.c_int),
-                ("dt", C.c_double), ("theta", C.c_double), ("sigma", C.c_double),
+                ("subs_per_block", C.c_int), ("dt", C.c_double), ("theta", C.c_double), ("sigma", C.c_double),
                 ("smem_bytes", C.c_size_t), ("workspace_bytes", C.c_size_t)]
+
+
+class hz_part_flags(C.Structure):
+    _fields_ = [("cluster", C.c_int), ("no_warp_spec", C.c_int), ("no_reg_cap", C.c_int), ("grid_blocks", C.c_int),
+                ("warp_order", C.c_int), ("pack", C.c_int)]
+
+
+class hz_mixed_opts(C.Structure):
+    _fields_ = [("n_cycles_max", C.c_int), ("m_inner", C.c_int), ("n_wh", C.c_int), ("relax", C.c_double),
+                ("tol", C.c_double), ("check_every", C.c_int), ("reset_state", C.c_int)]
+
+
+class hz_mixed_info(C.Structure):
+    _fields_ = [("cycles_done", C.c_int), ("sweeps_lo", C.c_int), ("sweeps_hi", C.c_int), ("rel_residual", C.c_double),
+                ("total_ms", C.c_double), ("dof_timesteps", C.c_double)]
 
 
 class hz_solve_opts(C.Structure):
@@ -93,6 +109,8 @@ def lib():
     L.hz_mesh_setup_quads.argtypes = [C.POINTER(vp), ip, ip, ip, vp, vp, vp, C.c_double, vp, vp, vp]
     L.hz_set_source.argtypes = [vp, vp, vp]
     L.hz_partition.argtypes = [vp, ip, ip, ip, ip, ip, C.c_double, C.POINTER(hz_part_info)]
+    L.hz_partition_ex.argtypes = [vp, ip, ip, ip, ip, ip, C.c_double, C.POINTER(hz_part_flags), C.POINTER(hz_part_info)]
+    L.hz_ddm_solve_mixed.argtypes = [vp, vp, C.POINTER(hz_mixed_opts), vp, C.POINTER(hz_mixed_info), vp]
     L.hz_ddm_solve.argtypes = [vp, C.POINTER(hz_solve_opts), vp, C.POINTER(hz_solve_info), vp]
     L.hz_operator_time.argtypes = [vp, vp, ip, C.POINTER(C.c_double), vp]
     L.hz_ddm_solve_sources.argtypes = [vp, C.POINTER(hz_solve_opts), ip, C.POINTER(vp), C.POINTER(vp),
@@ -106,7 +124,6 @@ def lib():
     L.hz_last_error.restype = C.c_char_p
     L.hz_destroy.argtypes = [vp]
     L.hz_destroy.restype = None
-    L.hz_peak_probe.argtypes = [ip, dp, vp]
     for name in EXPORTS:
         if name not in ("hz_last_error", "hz_destroy"):
             getattr(L, name).restype = C.c_int
@@ -173,6 +190,27 @@ def hz_set_source_ptr(ctx, f_re_ptr, f_im_ptr=None):
 def hz_partition(ctx, sx, sy, tc=HZ_TC_IMPEDANCE0, prec=HZ_F64, dofs_per_thread=0, cfl_frac=0.5):
     info = hz_part_info()
     _check(ctx, lib().hz_partition(ctx, sx, sy, tc, prec, dofs_per_thread, cfl_frac, C.byref(info)))
+    return info
+
+
+def hz_partition_ex(ctx, sx, sy, tc=HZ_TC_IMPEDANCE0, prec=HZ_F64, dofs_per_thread=0, cfl_frac=0.5, cluster=0,
+                    no_warp_spec=False, no_reg_cap=False, grid_blocks=0, warp_order=0, pack=0):
+    """hz_partition with the explicit variant-choice controls of include/hz.h::hz_part_flags."""
+    info = hz_part_info()
+    fl = hz_part_flags(int(cluster), int(bool(no_warp_spec)), int(bool(no_reg_cap)), int(grid_blocks), int(warp_order),
+                       int(pack))
+    _check(ctx, lib().hz_partition_ex(ctx, sx, sy, tc, prec, dofs_per_thread, cfl_frac, C.byref(fl), C.byref(info)))
+    return info
+
+
+def hz_ddm_solve_mixed(lo, hi, n_cycles_max, m_inner, n_wh=2, relax=0.5, tol=0.0, check_every=0, reset_state=False,
+                       u_out_ptr=None, stream=None):
+    """fp32 sweeps on the correction, fp64 state on `hi` (include/hz.h).  -> hz_mixed_info"""
+    opts = hz_mixed_opts(int(n_cycles_max), int(m_inner), int(n_wh), float(relax), float(tol), int(check_every),
+                         int(bool(reset_state)))
+    info = hz_mixed_info()
+    _check(hi, lib().hz_ddm_solve_mixed(lo, hi, C.byref(opts), C.c_void_p(u_out_ptr) if u_out_ptr else None,
+                                        C.byref(info), C.c_void_p(stream) if stream else None))
     return info
 
 
@@ -260,23 +298,15 @@ def hz_destroy(ctx):
         lib().hz_destroy(ctx)
 
 
-def hz_peak_probe(kind, stream=None):
-    r = C.c_double()
-    st = lib().hz_peak_probe(kind, C.byref(r), C.c_void_p(stream) if stream else None)
-    if st != HZ_OK:
-        raise HzError(st, "hz_peak_probe failed")
-    return r.value
-
-
-def setup_from_inputs(inp, prec=HZ_F64, dofs_per_thread=0):
-    """Convenience: hz_mesh_setup + hz_partition from an inputs.HzInputs.  -> (ctx, part_info)."""
+def setup_from_inputs(inp, prec=HZ_F64, dofs_per_thread=0, **flags):
+    """Convenience: hz_mesh_setup + hz_partition(_ex) from an inputs.HzInputs.  -> (ctx, part_info)."""
     if getattr(inp, "vx", None) is not None:
         ctx = hz_mesh_setup_quads(inp.nx, inp.ny, inp.p, inp.vx, inp.vy, inp.c_nodes, inp.omega, inp.f_re, inp.f_im)
     else:
         ctx = hz_mesh_setup(inp.nx, inp.ny, inp.x0, inp.y0, inp.x1, inp.y1, inp.p, inp.c_nodes, inp.omega, inp.f_re,
                             inp.f_im)
     try:
-        info = hz_partition(ctx, inp.sx, inp.sy, HZ_TC_IMPEDANCE0, prec, dofs_per_thread, inp.cfl_frac)
+        info = hz_partition_ex(ctx, inp.sx, inp.sy, HZ_TC_IMPEDANCE0, prec, dofs_per_thread, inp.cfl_frac, **flags)
     except Exception:
         hz_destroy(ctx)
         raise

@@ -38,7 +38,7 @@ def lib3():
     if not _ready:
         vp, ip = C.c_void_p, C.c_int
         L.hz3_mesh_setup.argtypes = [C.POINTER(vp), ip, ip, ip, vp, ip, vp, C.c_double, vp, vp, vp]
-        L.hz3_partition.argtypes = [vp, ip, ip, ip, ip, C.c_double, C.POINTER(hz3_part_info)]
+        L.hz3_partition.argtypes = [vp, ip, ip, ip, ip, C.c_double, ip, C.POINTER(hz3_part_info)]
         L.hz3_ddm_solve.argtypes = [vp, C.POINTER(hz3_solve_opts), vp, C.POINTER(hz3_solve_info), vp]
         L.hz3_residual.argtypes = [vp, vp, ip, C.POINTER(C.c_double), vp]
         L.hz3_operator_time.argtypes = [vp, vp, ip, C.POINTER(C.c_double), vp]
@@ -70,9 +70,9 @@ def hz3_mesh_setup(nx, ny, nz, box, p, c_nodes, omega, f_re, f_im=None, bc_lambd
     return ctx
 
 
-def hz3_partition(ctx, sx, sy, sz, prec=HZ_F64, cfl_frac=0.5):
+def hz3_partition(ctx, sx, sy, sz, prec=HZ_F64, cfl_frac=0.5, nodes_per_thread=0):
     info = hz3_part_info()
-    _check(ctx, lib3().hz3_partition(ctx, sx, sy, sz, prec, cfl_frac, C.byref(info)))
+    _check(ctx, lib3().hz3_partition(ctx, sx, sy, sz, prec, cfl_frac, int(nodes_per_thread), C.byref(info)))
     return info
 
 

@@ -37,7 +37,7 @@ def pack_bc(inp, bc):
     return out
 
 
-def check_case(inp, prec, n_outer=2, n_wh=2, warm=True, relax=0.5, bc=None):
+def check_case(inp, prec, n_outer=2, n_wh=2, warm=True, relax=0.5, bc=None, nodes_per_thread=0):
     assert torch.cuda.is_available(), "CUDA device required (there is no CPU fallback)"
     pr = problem_from(inp, bc)
     st = O.ddm_setup(pr, inp.sx, inp.sy, inp.sz, inp.cfl_frac)
@@ -47,7 +47,7 @@ def check_case(inp, prec, n_outer=2, n_wh=2, warm=True, relax=0.5, bc=None):
     ctx = hz3.hz3_mesh_setup(inp.nx, inp.ny, inp.nz, inp.box, inp.p, inp.c_nodes, inp.omega, inp.f_re, inp.f_im,
                              pack_bc(inp, bc))
     try:
-        info = hz3.hz3_partition(ctx, inp.sx, inp.sy, inp.sz, prec, inp.cfl_frac)
+        info = hz3.hz3_partition(ctx, inp.sx, inp.sy, inp.sz, prec, inp.cfl_frac, nodes_per_thread)
         assert info.n_t == st.tab.n_t, "N_t must be reproduced independently"
         dt = torch.float64 if prec == hz.HZ_F64 else torch.float32
         nn = int(np.prod(inp.shape))
@@ -84,10 +84,9 @@ def check_case(inp, prec, n_outer=2, n_wh=2, warm=True, relax=0.5, bc=None):
 @pytest.mark.parametrize("prec", [hz.HZ_F64, hz.HZ_F32])
 @pytest.mark.parametrize("p,n,s", [(1, 8, 4), (2, 4, 2), (3, 4, 2), (4, 2, 1)])
 @pytest.mark.parametrize("col", [True, False])
-def test_cube_all_degrees(prec, p, n, s, col, monkeypatch):
+def test_cube_all_degrees(prec, p, n, s, col):
     # col: one thread per node column along z (k3_sweep_col); else one thread per node (k3_sweep_dof)
-    monkeypatch.setenv("HZ3_DISABLE_COL", "0" if col else "1")
-    info = check_case(make_config_3d(n, p, s, seed=3000 + p), prec, n_outer=3, n_wh=2)
+    info = check_case(make_config_3d(n, p, s, seed=3000 + p), prec, n_outer=3, n_wh=2, nodes_per_thread=0 if col else 1)
     assert info.dofs_per_sub == (s * p + 1) ** 3 and info.blocks == (n // s) ** 3
     assert info.nodes_per_thread == (s * p + 1 if col else 1)
 

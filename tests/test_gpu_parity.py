@@ -64,7 +64,7 @@ def oracle_state_arrays(st):
     return u, lam
 
 
-def run_gpu(inp, prec, k, n_outer, n_wh, warm, relax, bc=None, res_field=None):
+def run_gpu(inp, prec, k, n_outer, n_wh, warm, relax, bc=None, res_field=None, flags=None):
     if getattr(inp, "vx", None) is not None:
         ctx = hz.hz_mesh_setup_quads(inp.nx, inp.ny, inp.p, inp.vx, inp.vy, inp.c_nodes, inp.omega, inp.f_re,
                                      inp.f_im, pack_bc(inp, bc))
@@ -72,7 +72,7 @@ def run_gpu(inp, prec, k, n_outer, n_wh, warm, relax, bc=None, res_field=None):
         ctx = hz.hz_mesh_setup(inp.nx, inp.ny, inp.x0, inp.y0, inp.x1, inp.y1, inp.p, inp.c_nodes, inp.omega,
                                inp.f_re, inp.f_im, pack_bc(inp, bc))
     try:
-        info = hz.hz_partition(ctx, inp.sx, inp.sy, hz.HZ_TC_IMPEDANCE0, prec, k, inp.cfl_frac)
+        info = hz.hz_partition_ex(ctx, inp.sx, inp.sy, hz.HZ_TC_IMPEDANCE0, prec, k, inp.cfl_frac, **(flags or {}))
         dt = torch.float64 if prec == hz.HZ_F64 else torch.float32
         u_out = torch.zeros(2 * inp.npx * inp.npy, dtype=dt, device="cuda")
         sinfo = hz.hz_ddm_solve(ctx, n_outer, n_wh=n_wh, warm_start=warm, relax=relax, reset_state=True,
@@ -94,12 +94,12 @@ def run_gpu(inp, prec, k, n_outer, n_wh, warm, relax, bc=None, res_field=None):
         hz.hz_destroy(ctx)
 
 
-def check_case(inp, prec, k, n_outer=3, n_wh=2, warm=True, relax=0.5, bc=None):
+def check_case(inp, prec, k, n_outer=3, n_wh=2, warm=True, relax=0.5, bc=None, flags=None):
     _require_cuda()
     pr = problem_from(inp, bc)
     st = O.ddm_solve(pr, inp.sx, inp.sy, n_outer, n_wh, warm_start=warm, relax=relax, cfl_frac=inp.cfl_frac)
     ug = O.ddm_gather(st)
-    g = run_gpu(inp, prec, k, n_outer, n_wh, warm, relax, bc, res_field=ug)
+    g = run_gpu(inp, prec, k, n_outer, n_wh, warm, relax, bc, res_field=ug, flags=flags)
     assert g["info"].n_t == st.tab.n_t, "N_t must be reproduced independently (reading R9)"
     assert g["sinfo"].n_outer_done == n_outer
     if k:
@@ -335,10 +335,9 @@ def test_auto_uses_a_cluster_when_one_sm_cannot_hold_the_state():
     assert g["info"].cluster_size > 1 and g["info"].dofs_per_thread == 9
 
 
-def test_auto_falls_back_to_streamed_when_no_on_chip_variant_fits(monkeypatch):
+def test_auto_falls_back_to_streamed_when_no_on_chip_variant_fits():
     # the same blocks with the cluster kernels switched off (as on a device without clusters): streamed fallback
-    monkeypatch.setenv("HZ_DISABLE_CLUSTER", "1")
-    g = check_case(make_config(4, n=64, sub_elems=32), hz.HZ_F64, 0, n_outer=2, n_wh=1)
+    g = check_case(make_config(4, n=64, sub_elems=32), hz.HZ_F64, 0, n_outer=2, n_wh=1, flags=dict(cluster=-1))
     assert g["info"].dofs_per_thread == -1 and g["info"].cluster_size == 1
 
 
@@ -352,19 +351,18 @@ def test_more_than_256_time_steps_uses_the_shared_memory_table():
 
 
 @pytest.mark.parametrize("prec,cl", [(hz.HZ_F64, 2), (hz.HZ_F64, 4), (hz.HZ_F32, 2), (hz.HZ_F32, 8), (hz.HZ_F64, 16)])
-def test_cluster_kernel_matches_the_oracle(prec, cl, monkeypatch):
+def test_cluster_kernel_matches_the_oracle(prec, cl):
     """Thread-block-cluster variant (hz_sweep_cl.cuh): the subdomain's tile grid is cut into column strips, one CTA
     each, with the strip-boundary chunks pushed through DSMEM.  Forced here on small subdomains (the automatic choice
     only uses it when one SM cannot hold the state)."""
-    monkeypatch.setenv("HZ_FORCE_CLUSTER", str(cl))
-    g = check_case(make_config(2, n=32, sub_elems=16 if cl >= 8 else None), prec, 9, n_outer=3, n_wh=2)
+    g = check_case(make_config(2, n=32, sub_elems=16 if cl >= 8 else None), prec, 9, n_outer=3, n_wh=2, flags=dict(cluster=cl))
     assert g["info"].cluster_size == cl
     if cl >= 8:      # 16 (beyond the portable size: opt-in attribute) and 8 need at least that many tile columns
         return
     inp = hetero_inputs(12, 4, 3, 2, 2, seed=55)      # 6x2-element subdomains: strips of unequal width
     rng = np.random.default_rng(12)
     bc = [rng.standard_normal(n) + 1j * rng.standard_normal(n) for n in (inp.npy, inp.npy, inp.npx, inp.npx)]
-    g = check_case(inp, prec, 9, n_outer=3, n_wh=2, warm=False, bc=bc)
+    g = check_case(inp, prec, 9, n_outer=3, n_wh=2, warm=False, bc=bc, flags=dict(cluster=cl))
     assert g["info"].cluster_size == cl
 
 
@@ -397,3 +395,62 @@ def test_stream_of_sources_matches_the_sequential_calls_bit_for_bit():
                 assert torch.equal(u_dev.cpu(), got), "pipelined and sequential paths must agree bit for bit"
         finally:
             hz.hz_destroy(ctx)
+
+
+@pytest.mark.parametrize("prec,cl", [(hz.HZ_F32, 2), (hz.HZ_F32, 4), (hz.HZ_F32, 8), (hz.HZ_F64, 2), (hz.HZ_F64, 4),
+                                     (hz.HZ_F64, 8), (hz.HZ_F64, 16)])      # every p = 3 cluster size that is compiled
+def test_cluster_halo_protocol_stress(prec, cl):
+    """compute-sanitizer is closed on this GPU pool, so the two-slot halo protocol of hz_sweep_cl.cuh (st.async pushes
+    into the adjacent CTA's shared memory, mbarrier transaction counts, no cluster barrier in the time loop) is
+    stressed instead: many time steps with strips of UNEQUAL width (17 tile columns over cl CTAs; some strips are a
+    single column at cl = 16), 20 repeats that must be bit-identical (a race shows as run-to-run noise), and the
+    result must agree with the single-CTA kernel's to rounding (its edge pieces associate their sums differently)."""
+    _require_cuda()
+    inp = make_config(2, n=32, sub_elems=16)
+    nn = inp.npx * inp.npy
+    dt = torch.float64 if prec == hz.HZ_F64 else torch.float32
+
+    def run(flags, reps):
+        ctx, info = hz.setup_from_inputs(inp, prec, 9, **flags)
+        try:
+            outs = []
+            for _ in range(reps):
+                u = torch.zeros(2 * nn, dtype=dt, device="cuda")
+                hz.hz_ddm_solve(ctx, 6, n_wh=4, relax=0.5, reset_state=True, u_out_ptr=u.data_ptr())
+                outs.append(u)
+            return info, outs
+        finally:
+            hz.hz_destroy(ctx)
+
+    info, outs = run(dict(cluster=cl, grid_blocks=4096), 20)   # grid_blocks: the register-capped instantiations compete too
+    assert info.cluster_size == cl
+    for u in outs[1:]:
+        assert torch.equal(u, outs[0]), "cluster kernel is not deterministic: halo race"
+    info1, ref = run(dict(cluster=-1), 1)
+    assert info1.cluster_size == 1 and info1.dofs_per_thread == 9
+    d = float((outs[0].double() - ref[0].double()).norm() / ref[0].double().norm())
+    assert d <= (1e-12 if prec == hz.HZ_F64 else 3e-5), d
+
+
+def test_graph_is_rebuilt_when_a_complex_source_arrives():
+    """A cached CUDA graph holds the kernel arguments of its capture; hz_set_source with a first imaginary part
+    allocates the Im b array, so the graph must be re-captured (it used to replay bbf_im = NULL and drop Im f)."""
+    _require_cuda()
+    inp = make_config(2, n=16)
+    rng = np.random.default_rng(21)
+    f_im = rng.standard_normal(inp.f_re.shape)
+    ctx, info = hz.setup_from_inputs(inp, hz.HZ_F64, 1)
+    try:
+        a = torch.zeros(2 * inp.npx * inp.npy, dtype=torch.float64, device="cuda")
+        b = torch.zeros_like(a)
+        hz.hz_ddm_solve(ctx, 8, n_wh=2, reset_state=True, use_graph=True, u_out_ptr=a.data_ptr())     # graph cached
+        hz.hz_set_source(ctx, inp.f_re, f_im)
+        hz.hz_ddm_solve(ctx, 8, n_wh=2, reset_state=True, use_graph=True, u_out_ptr=a.data_ptr())
+        hz.hz_ddm_solve(ctx, 8, n_wh=2, reset_state=True, use_graph=False, u_out_ptr=b.data_ptr())
+        assert torch.equal(a, b)
+        inp2 = HzInputs(**{**inp.__dict__, "f_im": f_im})
+        st = O.ddm_solve(problem_from(inp2), inp.sx, inp.sy, 8, 2, True, 0.5, inp.cfl_frac)
+        ug = a.cpu().numpy().reshape(2, inp.npy, inp.npx)
+        assert rel(ug[0] + 1j * ug[1], O.ddm_gather(st)) <= 1e-10
+    finally:
+        hz.hz_destroy(ctx)

@@ -54,12 +54,14 @@ def test_ctypes_structs_match_header_sizes(libpath, tmp_path):
     """Compile a tiny C program against include/hz.h and compare sizeof() with the ctypes mirrors."""
     from paper_2606_21695_b200 import hz
     src = tmp_path / "sz.c"
-    src.write_text('#include <stdio.h>\n#include "hz.h"\nint main(void){printf("%zu %zu %zu\\n", sizeof(hz_part_info),'
-                   ' sizeof(hz_solve_opts), sizeof(hz_solve_info));return 0;}\n')
+    names = ["hz_part_info", "hz_part_flags", "hz_solve_opts", "hz_solve_info", "hz_sources_info", "hz_gmres_opts",
+             "hz_gmres_info", "hz_mixed_opts", "hz_mixed_info", "hz_minres_opts", "hz_minres_info"]
+    body = "".join(f'printf("%zu\\n", sizeof({n}));' for n in names)
+    src.write_text('#include <stdio.h>\n#include "hz.h"\nint main(void){' + body + 'return 0;}\n')
     exe = tmp_path / "sz"
     subprocess.check_call(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)])
-    a, b, c = map(int, subprocess.check_output([str(exe)]).split())
-    assert (a, b, c) == (ctypes.sizeof(hz.hz_part_info), ctypes.sizeof(hz.hz_solve_opts), ctypes.sizeof(hz.hz_solve_info))
+    sizes = list(map(int, subprocess.check_output([str(exe)]).split()))
+    assert sizes == [ctypes.sizeof(getattr(hz, n)) for n in names]
 
 
 def test_argument_errors_need_no_gpu(libpath):
