@@ -416,6 +416,7 @@ def run_b200(args):
                    "copies on private streams overlap the sweeps; wall clock around the one C-ABI call",
            "sequential_value": seq_value, "sequential_steps": seq_steps,
            "sequential_what": "hz_set_source(host f) + hz_ddm_solve(1 sweep, u_out) + D2H of u, one after the other"}
+    u_elem = u_pins[0].element_size()
     del f_pins, u_pins, u_dev
 
     if rank != 0:
@@ -438,9 +439,10 @@ def run_b200(args):
     except Exception:
         probe_tf = None
     op_ms = None
-    try:   # the paper's normaliser: one evaluation of the global Helmholtz operator on a random vector
-        v = torch.randn(2 * nn, dtype=torch.float64, device="cuda")
-        op_ms = hz.hz_operator_time(ctx, v.data_ptr(), 10, stream)
+    try:   # the paper's normaliser: one evaluation of the global Helmholtz operator on a random vector,
+           # in the arithmetic of the cycle
+        v = torch.randn(2 * nn, dtype=tdt, device="cuda")
+        op_ms = hz.hz_operator_time(ctx, v.data_ptr(), prec, 10, stream)
         del v
     except Exception:
         pass
@@ -455,7 +457,10 @@ def run_b200(args):
                 "peak_measured_fma_probe": probe_tf, "frac_of_probe": (achieved_tf / probe_tf) if probe_tf else None,
                 "flops_per_dof_step": fl, "dof_steps_per_launch": units_per_launch, "sweep_kernel_ms": sweep_ms,
                 "exchange_kernel_ms": float(sum(exc)) / args.steps,
-                "operator_ms_fp64": op_ms, "ddm_cycle_over_operator": (sweep_ms / op_ms) if op_ms else None}
+                "operator_ms": op_ms, "operator_gb_per_s": (nn * 5 * u_elem / (op_ms * 1e-3) / 1e9) if op_ms else None,
+                "operator_what": "one evaluation y = (A - i w H - w^2 M) x of the global operator in the cycle's own "
+                                 "precision; bytes = x (2 words) + w^2/c^2 (1) + y (2) per node",
+                "ddm_cycle_over_operator": (sweep_ms / op_ms) if op_ms else None}
     hz.hz_destroy(ctx)
 
     extras = {}
@@ -555,11 +560,11 @@ def paper_style_cycle(hz, torch, stream, flush, n=512, p=3, s=8, prec_name="f32"
             hz.hz_set_subdomain_state(ctx, None, lam0.data_ptr(), stream=stream)
             flush.add_(1.0)
             ms.append(hz.hz_ddm_solve(ctx, 1, n_wh=N_WH, warm_start=False, stream=stream).sweep_ms_total)
-        v = torch.randn(2 * inp.npx * inp.npy, dtype=torch.float64, device="cuda")
-        op = hz.hz_operator_time(ctx, v.data_ptr(), 20, stream)
+        v = torch.randn(2 * inp.npx * inp.npy, dtype=torch.float32 if prec_name == "f32" else torch.float64, device="cuda")
+        op = hz.hz_operator_time(ctx, v.data_ptr(), prec, 20, stream)
         cyc = min(ms[1:])
         return {"mesh": f"{n}x{n}, p={p}, c=1, {info.blocks} subdomains of {s}x{s} elements, {prec_name}", "n_t": info.n_t,
-                "ddm_cycle_ms": cyc, "operator_ms_fp64": op, "cycle_over_operator": cyc / op,
+                "ddm_cycle_ms": cyc, "operator_ms": op, "cycle_over_operator": cyc / op,
                 "mdof_per_s_per_cycle": info.blocks * info.dofs_per_sub / (cyc * 1e-3) / 1e6}
     finally:
         hz.hz_destroy(ctx)
@@ -720,9 +725,14 @@ def run_tables(args):
         except hz.HzError as e:
             print(f"{head} {k or 'auto'} | — | — | — | — | — | — | — | — | — | {str(e).split(':', 1)[0]} |", flush=True)
             return
-        ctx, _ = hz.setup_from_inputs(inp, hz.HZ_F64, 1 if r["dofs_per_sub"] <= 1024 else -1)
-        v = torch.from_numpy(np.random.default_rng(1).standard_normal(2 * inp.npx * inp.npy)).cuda()
-        op_ms = hz.hz_operator_time(ctx, v.data_ptr(), 20, stream)
+        if inp.vx is not None:
+            ctx = hz.hz_mesh_setup_quads(inp.nx, inp.ny, inp.p, inp.vx, inp.vy, inp.c_nodes, inp.omega, inp.f_re)
+            opp = hz.HZ_F64                       # general quads: the fp64 residual kernel is the operator kernel
+        else:
+            ctx = hz.hz_mesh_setup(inp.nx, inp.ny, inp.x0, inp.y0, inp.x1, inp.y1, inp.p, inp.c_nodes, inp.omega, inp.f_re)
+            opp = hz.HZ_F32 if pr == "f32" else hz.HZ_F64
+        v = torch.randn(2 * inp.npx * inp.npy, dtype=torch.float32 if opp == hz.HZ_F32 else torch.float64, device="cuda")
+        op_ms = hz.hz_operator_time(ctx, v.data_ptr(), opp, 20, stream)
         hz.hz_destroy(ctx)
         print(f"{head} {r['kernel']} | {r['dofs_per_thread']} | {r['cluster_size']} | {r['subs_per_block']} | {r['dofs_per_sub']} | "
               f"{r['blocks']} | {r['threads_per_block']} | {r['smem_bytes']} | {r['sweep_ms']:.3f} | "
@@ -731,7 +741,7 @@ def run_tables(args):
 
     if which in ("cfg2", "cfg3", "cfg4", "cfg5", "quads"):
         print("| cfg | n | p | sub side | prec | kernel | DOF/thread | CTAs/sub | subs/block | DOF/sub | blocks | threads | smem B | "
-              "sweep ms | DOF-steps/s | frac of FMA peak | operator ms (fp64) | DDM cycle / operator |")
+              "sweep ms | DOF-steps/s | frac of FMA peak | operator ms (same precision) | DDM cycle / operator |")
         print("|" + "---|" * 18)
     if which in ("cfg2", "cfg3"):
         for pr in ("f32", "f64"):

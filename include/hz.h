@@ -190,10 +190,14 @@ typedef struct {
 hz_status hz_ddm_solve(hz_ctx *ctx, const hz_solve_opts *opts, void *u_out, hz_solve_info *info, void *stream);
 
 /* The paper's "operator time" normaliser (the DDM cycle is compared "to the time it takes to evaluate
- * the Helmholtz operator A - i w H - w^2 M on the entire domain"): `reps` back-to-back evaluations of the global
- * operator (the kernel of hz_residual, fp64) on u_dev (DEVICE, 2*(nx*p+1)*(ny*p+1) doubles);
- * *ms_per_eval = CUDA-event time / reps. */
-hz_status hz_operator_time(hz_ctx *ctx, const double *u_dev, int reps, double *ms_per_eval, void *stream);
+ * the Helmholtz operator A - i w H - w^2 M on the entire domain"): `reps` back-to-back evaluations y = (A - i w H -
+ * w^2 M) u of the global operator in the arithmetic `prec` (that of the DDM cycle it normalises).
+ *   u_dev  DEVICE, 2*(nx*p+1)*(ny*p+1) values of precision prec (re plane, im plane).
+ *   y_dev  DEVICE or NULL: receives y (same layout and precision); NULL = a vector owned by the context.
+ *   *ms_per_eval = CUDA-event time / reps.
+ * General-quadrilateral contexts: HZ_F64 and y_dev = NULL only (the residual kernel is timed). */
+hz_status hz_operator_time(hz_ctx *ctx, const void *u_dev, hz_prec prec, int reps, void *y_dev, double *ms_per_eval,
+                           void *stream);
 
 /* ---------------------------------------------------------------------------------------------
  * hz_ddm_solve_sources — a stream of right-hand sides on one mesh and partition, end to end from HOST to HOST:
@@ -294,7 +298,9 @@ hz_status hz_ddm_solve_mixed(hz_ctx *lo, hz_ctx *hi, const hz_mixed_opts *opts, 
  * as the subdomain solver instead of WaveHoltz.  Assembles b from f and the current lambda^n,
  * iterates until the recurrence's relative residual <= tol (the paper: 1e-6 in single, 1e-12 in double precision) or
  * max_iters, stores u_l and the outgoing interface data, then (relax > 0) runs the exchange kernel.
- * Needs the one-DOF-per-thread partition (hz_partition(..., dofs_per_thread = 1)), else HZ_EUNSUPPORTED.
+ * Runs in the layout of the partition: one DOF per thread (hz_partition(..., dofs_per_thread = 1)), or register-blocked
+ * with the WaveHoltz kernels' square thread tiles of at most 16 DOFs (k = 4, 9, 16; one thread block per subdomain
+ * even where the WaveHoltz sweep packs several or uses a cluster: those give HZ_EUNSUPPORTED, like larger tiles).
  * max_iters = 0 with warm_start = 1 only evaluates the subdomain residuals of the current u_l.
  *   iters_out  HOST or NULL: `blocks` ints, MINRES iterations of each subdomain.
  *   res_out    HOST or NULL: `blocks` doubles, true relative residual ||rhs - K x|| / ||rhs|| of each subdomain.

@@ -54,7 +54,7 @@ struct hz_ctx {
   // partition
   bool part = false;
   int sx = 0, sy = 0, ex = 0, ey = 0, L = 0, E = 0, prec = 0;
-  int mx = 0, my = 0, csm = 0, ws = 0, cl = 1, entry = -1;
+  int mx = 0, my = 0, csm = 0, ws = 0, cl = 1, entry = -1, pack = 1;
   Layout lay{};
   SweepLaunch launch{};
   hz_part_flags flags{};  // variant-choice controls of the last hz_partition_ex
@@ -69,6 +69,8 @@ struct hz_ctx {
   void *d_mix = nullptr;       // hz_ddm_solve_mixed: hi context: X_old (n_state doubles); lo context: D (n_state floats)
   double *d_wxl = nullptr, *d_wyl = nullptr;
   double *d_part = nullptr, *d_red = nullptr, *d_ures = nullptr;
+  void *d_opk2 = nullptr, *d_opy = nullptr;  // hz_operator_time: w^2/c^2 and the output vector, in precision op_prec
+  int op_prec = -1;
   int res_blocks = 0;
   Elem1D<double> ex1{}, ey1{};
   // cached CUDA graph of `g_chunk` {sweep, exchange} pairs (use_graph)
@@ -214,6 +216,7 @@ SweepArgs<real> make_args(const hz_ctx *c, const hz_solve_opts *o, bool homog = 
   }
   a.worder = c->worder;
   a.fused = 0; a.relax = (real)o->relax; a.g_prev = nullptr; a.lam_rw = nullptr;
+  a.pack = c->pack; a.L = c->L;
   return a;
 }
 
@@ -274,10 +277,36 @@ cudaError_t launch_gather(const hz_ctx *c, void *out, int prec_out, cudaStream_t
   return cudaGetLastError();
 }
 
+// launches k_helm<inT, acc, P, MODE> on the whole mesh (hz_aux.cuh)
+template <typename inT, typename acc, int MODE>
+cudaError_t launch_helm(hz_ctx *ctx, const acc *k2, const void *u_dev, double *part, acc *y, cudaStream_t st) {
+  Ref1D ref{};
+  for (int a = 0; a <= ctx->p; ++a) {
+    ref.w[a] = ctx->gll.w[a];
+    for (int b = 0; b <= ctx->p; ++b) ref.K[a][b] = ctx->gll.K[a][b];
+  }
+  const Geo g = make_geo(ctx);
+  const dim3 grid((ctx->nx + 1 + kHelmBX - 1) / kHelmBX, (ctx->ny + 1 + kHelmBY - 1) / kHelmBY), block(kHelmBX, kHelmBY);
+  const size_t sm = helm_smem(ctx->p, sizeof(acc));
+  void (*fn)(Geo, Ref1D, const double *, const acc *, const double *, const double *, const double *, const inT *, double *, acc *) = nullptr;
+  switch (ctx->p) {
+    case 1: fn = k_helm<inT, acc, 1, MODE>; break;
+    case 2: fn = k_helm<inT, acc, 2, MODE>; break;
+    case 3: fn = k_helm<inT, acc, 3, MODE>; break;
+    case 4: fn = k_helm<inT, acc, 4, MODE>; break;
+    default: return cudaErrorInvalidValue;
+  }
+  cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+  if (e != cudaSuccess) return e;
+  fn<<<grid, block, sm, st>>>(g, ref, ctx->d_c, k2, ctx->d_fre, ctx->d_fim, ctx->d_bc, (const inT *)u_dev, part, y);
+  return cudaGetLastError();
+}
+
 hz_status residual_impl(hz_ctx *ctx, const void *u_dev, int u_prec, double *rel, cudaStream_t st) {
   const long long total = (long long)ctx->npx * ctx->npy;
   const int bs = 256;
-  const int nb = (int)((total + bs - 1) / bs);
+  const int nb = ctx->general ? (int)((total + bs - 1) / bs)
+                              : ((ctx->nx + 1 + kHelmBX - 1) / kHelmBX) * ((ctx->ny + 1 + kHelmBY - 1) / kHelmBY);
   if (!ctx->d_part || ctx->res_blocks != nb) {
     if (ctx->d_part) cudaFree(ctx->d_part);
     if (ctx->d_red) cudaFree(ctx->d_red);
@@ -286,24 +315,20 @@ hz_status residual_impl(hz_ctx *ctx, const void *u_dev, int u_prec, double *rel,
     HZ_CUDA(dmalloc(&ctx->d_red, 2));
     ctx->res_blocks = nb;
   }
-  Ref1D ref{};
-  for (int a = 0; a <= ctx->p; ++a) {
-    ref.w[a] = ctx->gll.w[a];
-    for (int b = 0; b <= ctx->p; ++b) ref.K[a][b] = ctx->gll.K[a][b];
-  }
-  Geo g = make_geo(ctx);
   if (ctx->general) {
+    Geo g = make_geo(ctx);
     if (u_prec == HZ_F32)
       k_residual_quad<float><<<nb, bs, 0, st>>>(g, ctx->refq, ctx->d_vx, ctx->d_vy, ctx->d_c, ctx->d_fre, ctx->d_fim,
                                                 ctx->d_bc, (const float *)u_dev, ctx->d_part);
     else
       k_residual_quad<double><<<nb, bs, 0, st>>>(g, ctx->refq, ctx->d_vx, ctx->d_vy, ctx->d_c, ctx->d_fre, ctx->d_fim,
                                                  ctx->d_bc, (const double *)u_dev, ctx->d_part);
-  } else if (u_prec == HZ_F32)
-    k_residual<float><<<nb, bs, 0, st>>>(g, ref, ctx->d_c, ctx->d_fre, ctx->d_fim, ctx->d_bc, (const float *)u_dev, ctx->d_part);
-  else
-    k_residual<double><<<nb, bs, 0, st>>>(g, ref, ctx->d_c, ctx->d_fre, ctx->d_fim, ctx->d_bc, (const double *)u_dev, ctx->d_part);
-  HZ_CUDA(cudaGetLastError());
+    HZ_CUDA(cudaGetLastError());
+  } else if (u_prec == HZ_F32) {
+    HZ_CUDA((launch_helm<float, double, 0>(ctx, nullptr, u_dev, ctx->d_part, nullptr, st)));
+  } else {
+    HZ_CUDA((launch_helm<double, double, 0>(ctx, nullptr, u_dev, ctx->d_part, nullptr, st)));
+  }
   k_reduce2<<<1, 1024, 0, st>>>(ctx->d_part, nb, ctx->d_red);
   HZ_CUDA(cudaGetLastError());
   double h[2];
@@ -490,6 +515,7 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
   free_partition(ctx);
   ctx->flags = fl;
   ctx->worder = 0;
+  ctx->pack = 1;
   const int P = ctx->p;
   // ex, ey: elements per subdomain side; for a ragged partition (general quads only, reading R25) the maximum
   ctx->sx = sx; ctx->sy = sy; ctx->ex = (ctx->nx + sx - 1) / sx; ctx->ey = (ctx->ny + sy - 1) / sy;
@@ -517,7 +543,7 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
   const size_t smem_cap = 227 * 1024;
   Layout lay{};
   lay.lnx = lnx; lay.lny = lny;
-  int best = -1;
+  int best = -1, bpack = 1;
   SweepLaunch bl{};
   Layout blay{};
   int sm_count = 148, dev = 0;
@@ -525,18 +551,37 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
   const bool no_ws = fl.no_warp_spec != 0, no_cl = fl.cluster == -1, no_regcap = fl.no_reg_cap != 0;
   const int force_cl = fl.cluster > 1 ? fl.cluster : 0;
   const long long Lsel = fl.grid_blocks > 0 ? fl.grid_blocks : (long long)sx * sy;  // grid size the choice assumes
-  auto tile_fit = [&](const TileEntry &t, Layout *lo, SweepLaunch *la) -> bool {
+  auto tile_fit = [&](const TileEntry &t, Layout *lo, SweepLaunch *la, int *gsel) -> bool {
     if (t.p != P || ctx->ex % t.mx || ctx->ey % t.my) return false;
     if (force_cl > 1 && t.cl != force_cl) return false;
+    if (fl.pack > 1 && !t.pk) return false;
     Layout q = lay;
     q.variant = 1; q.TX = t.mx * P; q.TY = t.my * P;
     q.cm = t.cl > 1 ? 1 : 0;
     q.ntx = ctx->ex / t.mx + 1; q.nty = ctx->ey / t.my + 1;
     const int ntv = roundup(q.ntx * q.nty, 32);   // virtual tile slots (stride of the per-node arrays)
-    int nthr = ntv;
+    int nthr = ntv, ntv_pack = 0;
     size_t sm = 0;
     const size_t narr = 2 * (size_t)(q.TX + q.TY);
-    if (t.cl > 1) {
+    int G = 1;
+    if (t.pk) {
+      // several small subdomains per block: G*NB bulk lanes fill whole warps (hz_sweep_pack.cuh)
+      const int NB = (q.ntx - 1) * (q.nty - 1), NE = q.ntx + q.nty - 1;
+      if (n_t > kTabCMax || NB > 16 || fl.pack == 1) return false;
+      auto gcd = [](int a, int b) { while (b) { const int r = a % b; a = b; b = r; } return a; };
+      G = fl.pack > 1 ? fl.pack : 32 / gcd(32, NB);
+      // a small grid keeps its parallelism: at least two blocks per SM before subdomains share a block
+      while (fl.pack <= 1 && G > 1 && (Lsel + G - 1) / G < 2LL * sm_count) G /= 2;
+      const size_t v16 = 16 / rs, chx = ((size_t)q.TX + v16 - 1) / v16 * v16, rsw = 4 * chx + v16;
+      const size_t nep = ((size_t)NE + v16 - 1) / v16 * v16;
+      for (;; G /= 2) {
+        nthr = roundup(G * NB, 32) + roundup(G * NE, 32);
+        sm = 2 * ((size_t)G * ((size_t)(q.ntx * q.nty + 1) * rsw + 2 * nep) + rsw) * rs;
+        if ((nthr <= t.maxt && sm <= smem_cap) || G == 1 || fl.pack > 1) break;
+      }
+      if (G < 2) return false;
+      ntv_pack = q.ntx * q.nty;
+    } else if (t.cl > 1) {
       if (no_cl || n_t > kTabCMax || q.ntx < t.cl) return false;
       const int wmax = (q.ntx + t.cl - 1) / t.cl;
       nthr = roundup(wmax * q.nty, 32);
@@ -563,9 +608,10 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
       sm = 2 * (size_t)(nthr + 33) * rsw * rs + (t.csm ? (size_t)nthr * cst * rs : 0);
     }
     if (nthr > t.maxt) return false;
-    q.NT = ntv; q.NS = q.TX * q.TY * ntv;
+    q.NT = t.pk ? ntv_pack : ntv; q.NS = q.TX * q.TY * q.NT;
     if (sm > smem_cap) return false;
-    *lo = q; la->blocks = ctx->L * t.cl; la->threads = nthr; la->smem = sm;
+    *lo = q; la->blocks = t.pk ? (ctx->L + G - 1) / G : ctx->L * t.cl; la->threads = nthr; la->smem = sm;
+    if (gsel) *gsel = G;
     if (t.cl > 1 && !cluster_schedulable(t, *la)) return false;  // e.g. a GPC that cannot co-schedule t.cl such CTAs
     return true;
   };
@@ -602,7 +648,8 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
       const int k = t.mx * P * t.my * P;
       if (dofs_per_thread > 1 && k != dofs_per_thread) continue;
       Layout lo; SweepLaunch la;
-      if (!tile_fit(t, &lo, &la)) continue;
+      int gsel = 1;
+      if (!tile_fit(t, &lo, &la, &gsel)) continue;
       // prefer the warp-specialised kernel, then register-resident coefficients, then the smaller tile
       // (more threads, better latency hiding); among otherwise equal instantiations take the
       // register-capped one (higher occupancy, a few spills) only when the grid can fill that occupancy
@@ -618,6 +665,8 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
         // tiers: (0) one CTA, everything in registers; (1) one CTA, warp-specialised, coefficients in shared memory,
         // tiles of at most 16 DOFs; (2) clusters, smallest first; (3) the remaining shared-memory-coefficient kernels
         // (measured order on configs 4 and 5, profiles/r01_config_sweep.md)
+        // (-1) several small subdomains per block, whenever a subdomain has at most 16 full tiles; largest tile <= 16 DOFs
+        if (q.pk) return -1000000000LL + (k_ <= 16 ? 16 - k_ : k_);
         if (q.cl > 1) return 200000000LL + q.cl * 1000 + k_;
         if (q.csm) return ((q.ws && k_ <= 16) ? 100000000LL : 300000000LL) + k_ * 100 + (1 - q.ws);
         return ((long long)(1 - q.ws) * 1000000 + dk * 1000 + k_) * 10 - q.minb;
@@ -625,7 +674,7 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
       const long long score = score_of(t);
       const long long bscore = best < 0 ? 0 : score_of(tiles[best]);
       if (best < 0 || score < bscore) {
-        best = i; blay = lo; bl = la;
+        best = i; blay = lo; bl = la; bpack = gsel;
       }
     }
     if (best < 0 && dofs_per_thread > 1)
@@ -639,6 +688,7 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
     ctx->lay = blay; ctx->launch = bl;
     ctx->mx = tiles[best].mx; ctx->my = tiles[best].my; ctx->csm = tiles[best].csm; ctx->ws = tiles[best].ws;
     ctx->cl = tiles[best].cl;
+    ctx->pack = tiles[best].pk ? bpack : 1;
     ctx->entry = best;
     // warp-role order of k_sweep_ws: a 3-warp block (2 bulk + 1 edge) puts its edge warp in the middle, so that the bulk
     // warps of the blocks resident on an SM (consecutive hardware warp slots, slot mod 4 = sub-partition) spread evenly
@@ -722,7 +772,7 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
     inf.dofs_per_thread = ctx->lay.variant == 0 ? 1 : (ctx->lay.variant == 2 ? -1 : ctx->lay.TX * ctx->lay.TY);
     if (ctx->lay.variant == 3) inf.dofs_per_thread = (P + 1) * (P + 1);  // incl. the replicated shared nodes
     inf.tile_mx = ctx->mx; inf.tile_my = ctx->my; inf.cluster_size = ctx->lay.variant == 1 ? ctx->cl : 1;
-    inf.subs_per_block = 1;
+    inf.subs_per_block = ctx->lay.variant == 1 ? ctx->pack : 1;
     inf.dt = ctx->dt; inf.theta = ctx->theta; inf.sigma = ctx->sigma;
     inf.smem_bytes = ctx->launch.smem; inf.workspace_bytes = ws;
     *info_out = inf;
@@ -858,38 +908,54 @@ hz_status hz_ddm_solve(hz_ctx *ctx, const hz_solve_opts *opts, void *u_out, hz_s
   return HZ_OK;
 }
 
-hz_status hz_operator_time(hz_ctx *ctx, const double *u_dev, int reps, double *ms_per_eval, void *stream) {
+hz_status hz_operator_time(hz_ctx *ctx, const void *u_dev, hz_prec prec, int reps, void *y_dev, double *ms_per_eval,
+                           void *stream) {
   if (!ctx) return HZ_EINVAL;
   if (!u_dev || !ms_per_eval || reps < 1) return fail(ctx, HZ_EINVAL, "hz_operator_time: NULL argument or reps < 1");
+  if (prec != HZ_F32 && prec != HZ_F64) return fail(ctx, HZ_EINVAL, "hz_operator_time: bad precision");
   cudaStream_t st = (cudaStream_t)stream;
-  double rel = 0.0;
-  hz_status s0 = residual_impl(ctx, u_dev, HZ_F64, &rel, st);  // allocates the partial-sum buffers, warm-up
-  if (s0 != HZ_OK) return s0;
-  const long long total = (long long)ctx->npx * ctx->npy;
-  const int bs = 256, nb = (int)((total + bs - 1) / bs);
-  Ref1D ref{};
-  for (int a = 0; a <= ctx->p; ++a) {
-    ref.w[a] = ctx->gll.w[a];
-    for (int b = 0; b <= ctx->p; ++b) ref.K[a][b] = ctx->gll.K[a][b];
+  const size_t nn = (size_t)ctx->npx * ctx->npy, rs = prec == HZ_F32 ? 4 : 8;
+  EventGuard e0, e1;
+  HZ_CUDA(cudaEventCreate(&e0.e));
+  HZ_CUDA(cudaEventCreate(&e1.e));
+  if (ctx->general) {  // general quads: the fp64 residual kernel is the operator kernel (no separate output pass)
+    if (prec != HZ_F64 || y_dev) return fail(ctx, HZ_EUNSUPPORTED, "hz_operator_time: general quadrilaterals: HZ_F64 only, no output vector");
+    double rel = 0.0;
+    hz_status s0 = residual_impl(ctx, u_dev, HZ_F64, &rel, st);  // allocates the partial-sum buffers, warm-up
+    if (s0 != HZ_OK) return s0;
+    const int bs = 256, nb = (int)((nn + bs - 1) / bs);
+    const Geo g = make_geo(ctx);
+    HZ_CUDA(cudaEventRecord(e0.e, st));
+    for (int r = 0; r < reps; ++r)
+      k_residual_quad<double><<<nb, bs, 0, st>>>(g, ctx->refq, ctx->d_vx, ctx->d_vy, ctx->d_c, ctx->d_fre, ctx->d_fim, ctx->d_bc,
+                                                 (const double *)u_dev, ctx->d_part);
+  } else {
+    // w^2 / c^2 in the operator's precision and the output vector y, owned by the context
+    if (!ctx->d_opk2 || ctx->op_prec != (int)prec) {
+      if (ctx->d_opk2) cudaFree(ctx->d_opk2);
+      if (ctx->d_opy) cudaFree(ctx->d_opy);
+      ctx->d_opk2 = ctx->d_opy = nullptr;
+      HZ_CUDA(cudaMalloc(&ctx->d_opk2, nn * rs));
+      HZ_CUDA(cudaMalloc(&ctx->d_opy, 2 * nn * rs));
+      ctx->op_prec = (int)prec;
+      const unsigned nbk = (unsigned)((nn + 255) / 256);
+      if (prec == HZ_F32) k_helm_k2<float><<<nbk, 256, 0, st>>>((long long)nn, ctx->omega, ctx->d_c, (float *)ctx->d_opk2);
+      else k_helm_k2<double><<<nbk, 256, 0, st>>>((long long)nn, ctx->omega, ctx->d_c, (double *)ctx->d_opk2);
+      HZ_CUDA(cudaGetLastError());
+    }
+    void *yv = y_dev ? y_dev : ctx->d_opy;
+    auto once = [&]() -> cudaError_t {
+      if (prec == HZ_F32) return launch_helm<float, float, 1>(ctx, (const float *)ctx->d_opk2, u_dev, nullptr, (float *)yv, st);
+      return launch_helm<double, double, 1>(ctx, (const double *)ctx->d_opk2, u_dev, nullptr, (double *)yv, st);
+    };
+    HZ_CUDA(once());  // warm-up
+    HZ_CUDA(cudaEventRecord(e0.e, st));
+    for (int r = 0; r < reps; ++r) HZ_CUDA(once());
   }
-  const Geo g = make_geo(ctx);
-  cudaEvent_t e0, e1;
-  HZ_CUDA(cudaEventCreate(&e0));
-  HZ_CUDA(cudaEventCreate(&e1));
-  cudaEventRecord(e0, st);
-  for (int r = 0; r < reps; ++r) {
-    if (ctx->general)
-      k_residual_quad<double><<<nb, bs, 0, st>>>(g, ctx->refq, ctx->d_vx, ctx->d_vy, ctx->d_c, ctx->d_fre, ctx->d_fim, ctx->d_bc, u_dev, ctx->d_part);
-    else
-      k_residual<double><<<nb, bs, 0, st>>>(g, ref, ctx->d_c, ctx->d_fre, ctx->d_fim, ctx->d_bc, u_dev, ctx->d_part);
-  }
-  cudaEventRecord(e1, st);
-  cudaError_t ce = cudaStreamSynchronize(st);
+  HZ_CUDA(cudaEventRecord(e1.e, st));
+  HZ_CUDA(cudaStreamSynchronize(st));
   float ms = 0.f;
-  if (ce == cudaSuccess) ce = cudaEventElapsedTime(&ms, e0, e1);
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
-  if (ce != cudaSuccess) return cuda_fail(ctx, ce, "hz_operator_time");
+  HZ_CUDA(cudaEventElapsedTime(&ms, e0.e, e1.e));
   *ms_per_eval = ms / reps;
   return HZ_OK;
 }
@@ -1162,6 +1228,10 @@ namespace {
 
 inline cudaError_t launch_minres(const MinresArgs<float> &a, int p, SweepLaunch c, cudaStream_t st) { return launch_minres_f32(a, p, c, st); }
 inline cudaError_t launch_minres(const MinresArgs<double> &a, int p, SweepLaunch c, cudaStream_t st) { return launch_minres_f64(a, p, c, st); }
+inline cudaError_t launch_minres_tile(const MinresArgs<float> &a, const Elem1D<float> &x, const Elem1D<float> &y, int p, int m,
+                                      SweepLaunch c, cudaStream_t st) { return launch_minres_tile_f32(a, x, y, p, m, c, st); }
+inline cudaError_t launch_minres_tile(const MinresArgs<double> &a, const Elem1D<double> &x, const Elem1D<double> &y, int p, int m,
+                                      SweepLaunch c, cudaStream_t st) { return launch_minres_tile_f64(a, x, y, p, m, c, st); }
 
 template <typename real>
 hz_status minres_impl(hz_ctx *ctx, const hz_minres_opts *o, int *iters_out, double *res_out, hz_minres_info *info,
@@ -1194,12 +1264,28 @@ hz_status minres_impl(hz_ctx *ctx, const hz_minres_opts *o, int *iters_out, doub
   a.iters = ctx->d_mr_iters; a.res = ctx->d_mr_res;
   SweepLaunch cfg = ctx->launch;
   const int P = ctx->p;
-  cfg.smem = 72 * sizeof(double) + 2 * (size_t)(ctx->lay.lnx + 2 * P) * (ctx->lay.lny + 2 * P) * sizeof(real);
+  const bool tiled = ctx->lay.variant == 1;
+  Elem1D<real> ex1{}, ey1{};
+  if (tiled) {   // the register-blocked layout of the WaveHoltz kernels: one thread per tile, one subdomain per block
+    const int v16 = 16 / (int)sizeof(real), T = ctx->lay.TX;
+    const int rsw = 4 * ((T + v16 - 1) / v16 * v16) + v16;
+    cfg.blocks = ctx->L;
+    cfg.threads = roundup(ctx->lay.ntx * ctx->lay.nty, 32);
+    cfg.smem = 72 * sizeof(double) + 2 * (size_t)(cfg.threads + 2) * rsw * sizeof(real);
+    for (int i = 0; i <= kMaxP; ++i) {
+      for (int j = 0; j <= kMaxP; ++j) { ex1.kin[i][j] = (real)ctx->ex1.kin[i][j]; ey1.kin[i][j] = (real)ctx->ey1.kin[i][j]; }
+      ex1.k0[i] = (real)ctx->ex1.k0[i]; ex1.kp[i] = (real)ctx->ex1.kp[i];
+      ey1.k0[i] = (real)ctx->ey1.k0[i]; ey1.kp[i] = (real)ctx->ey1.kp[i];
+    }
+  } else {
+    cfg.smem = 72 * sizeof(double) + 2 * (size_t)(ctx->lay.lnx + 2 * P) * (ctx->lay.lny + 2 * P) * sizeof(real);
+  }
   cudaEvent_t e0, e1;
   HZ_CUDA(cudaEventCreate(&e0));
   HZ_CUDA(cudaEventCreate(&e1));
   HZ_CUDA(cudaEventRecord(e0, st));
-  HZ_CUDA(launch_minres(a, P, cfg, st));
+  if (tiled) HZ_CUDA(launch_minres_tile(a, ex1, ey1, P, ctx->mx, cfg, st));
+  else HZ_CUDA(launch_minres(a, P, cfg, st));
   HZ_CUDA(cudaEventRecord(e1, st));
   if (o->relax > 0.0) HZ_CUDA(launch_exchange(ctx, o->relax, st));
   std::vector<int> hi(ctx->L);
@@ -1323,8 +1409,11 @@ extern "C" hz_status hz_minres_cycle(hz_ctx *ctx, const hz_minres_opts *opts, in
   if (!ctx) return HZ_EINVAL;
   if (!opts) return fail(ctx, HZ_EINVAL, "hz_minres_cycle: NULL opts");
   if (!ctx->part) return fail(ctx, HZ_ESTATE, "hz_minres_cycle: call hz_partition first");
-  if (ctx->lay.variant != 0)
-    return fail(ctx, HZ_EUNSUPPORTED, "hz_minres_cycle: needs the one-DOF-per-thread partition (dofs_per_thread = 1)");
+  const bool tile_ok = ctx->lay.variant == 1 && ctx->cl == 1 && ctx->mx == ctx->my && ctx->lay.TX * ctx->lay.TY <= 16 &&
+                       ctx->lay.ntx * ctx->lay.nty <= 256 && !(ctx->p == 1 && ctx->mx == 1);
+  if (ctx->lay.variant != 0 && !tile_ok)
+    return fail(ctx, HZ_EUNSUPPORTED, "hz_minres_cycle: needs the one-DOF-per-thread partition or a register-blocked one with "
+                                      "square tiles of at most 16 DOFs and at most 256 tiles per subdomain");
   if (!(opts->tol >= 0.0) || opts->max_iters < 0 || opts->relax < 0.0 || opts->relax > 1.0)
     return fail(ctx, HZ_EINVAL, "hz_minres_cycle: need tol >= 0, max_iters >= 0, relax in [0,1]");
   cudaStream_t st = (cudaStream_t)stream;
@@ -1418,6 +1507,8 @@ void hz_destroy(hz_ctx *ctx) {
     for (cudaEvent_t e : {ctx->ev_up[b], ctx->ev_build[b], ctx->ev_gather[b], ctx->ev_down[b]})
       if (e) cudaEventDestroy(e);
   }
+  if (ctx->d_opk2) cudaFree(ctx->d_opk2);
+  if (ctx->d_opy) cudaFree(ctx->d_opy);
   double **ptrs[] = {&ctx->d_c, &ctx->d_fre, &ctx->d_fim, &ctx->d_bc, &ctx->d_vx, &ctx->d_vy};
   for (double **q : ptrs) { if (*q) cudaFree(*q); *q = nullptr; }
   delete ctx;

@@ -110,7 +110,7 @@ __global__ void k_build_minres(Geo g, Layout lay, const double *__restrict__ c, 
     if (onS && siy == 0) { bre += sSN * bc[(2 * 2 + 0) * g.EB + I]; bim += sSN * bc[(2 * 2 + 1) * g.EB + I]; }
     if (onN && siy == g.sy - 1) { bre += sSN * bc[(3 * 2 + 0) * g.EB + I]; bim += sSN * bc[(3 * 2 + 1) * g.EB + I]; }
   }
-  const size_t o = (size_t)l * lay.NS + q;
+  const size_t o = (size_t)l * lay.NS + lay.slot(i, j);
   mloc[o] = (real)m;
   w2M[o] = (real)(g.omega * g.omega * m / (cj * cj));
   wH[o] = (real)(g.omega * H);
@@ -193,85 +193,151 @@ struct Ref1D {
   double w[kMaxP + 1];
 };
 
-template <typename inT>
-__global__ void k_residual(Geo g, Ref1D ref, const double *__restrict__ c, const double *__restrict__ f_re,
-                           const double *__restrict__ f_im, const double *__restrict__ bc,
-                           const inT *__restrict__ u, double *__restrict__ part) {
-  __shared__ double red[2][32];
-  const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+// Launch shape of k_helm: a block of HB_X x HB_Y threads, one thread per ELEMENT (its P x P lower-left nodes, as in the
+// sweep kernels; the phantom elements nx / ny own the last node column / row), and its shared-memory patch.
+constexpr int kHelmBX = 32, kHelmBY = 8;
+inline size_t helm_smem(int P, size_t elem) { return 2 * (size_t)((kHelmBX + 1) * P + 1) * ((kHelmBY + 1) * P + 1) * elem; }
+
+// MODE 0: residual of (4): block partial sums of |b - (A - i w H - w^2 M) u|^2 and |b|^2 -> part (hz_residual)
+// MODE 1: operator evaluation y = (A - i w H - w^2 M) u written to y (re | im planes) -- the paper's "operator time"
+//         kernel, in the arithmetic `acc` of the DDM cycle it normalises
+// u: re | im planes of type inT.  k2: w^2 / c^2 per node in `acc` precision (MODE 1) or NULL (then c, fp64, is read).
+// The block stages the u patch ((32+1)P+1) x ((8+1)P+1) through shared memory with coalesced row loads; every thread
+// then applies the two 1-D element operators to its P x P nodes from shared memory (3P^2 + 2P reads per plane for P^2
+// nodes instead of 2(2P+1) P^2), compile-time P, coefficients in the constant bank.
+template <typename inT, typename acc, int P, int MODE>
+__global__ void __launch_bounds__(kHelmBX *kHelmBY) k_helm(Geo g, Ref1D ref, const double *__restrict__ c,
+                                                            const acc *__restrict__ k2, const double *__restrict__ f_re,
+                                                            const double *__restrict__ f_im, const double *__restrict__ bc,
+                                                            const inT *__restrict__ u, double *__restrict__ part,
+                                                            acc *__restrict__ y) {
+  constexpr int PW = (kHelmBX + 1) * P + 1, PH = (kHelmBY + 1) * P + 1;
+  extern __shared__ __align__(16) unsigned char helm_raw[];
+  acc *sr = reinterpret_cast<acc *>(helm_raw), *si = sr + PW * PH;
+  const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * kHelmBX + tx;
+  const int ex = blockIdx.x * kHelmBX + tx, ey = blockIdx.y * kHelmBY + ty;
+  const int I0 = blockIdx.x * kHelmBX * P - P, J0 = blockIdx.y * kHelmBY * P - P;  // patch origin
   const long long total = (long long)g.npx * g.npy;
-  double r2 = 0.0, b2 = 0.0;
-  if (gid < total) {
-    const int I = (int)(gid % g.npx), J = (int)(gid / g.npx);
-    const int P = g.p;
-    // assembled reference weights at this node
-    const int ax = I % P, ay = J % P;
-    const bool shx = ax == 0 && I > 0 && I < g.npx - 1, shy = ay == 0 && J > 0 && J < g.npy - 1;
-    const double wxI = (ax == 0) ? (shx ? 2.0 * ref.w[0] : ref.w[0]) : ref.w[ax];
-    const double wyJ = (ay == 0) ? (shy ? 2.0 * ref.w[0] : ref.w[0]) : ref.w[ay];
-    const inT *ur = u, *ui = u + total;
-    // (Kx u)_I along row J and (Ky u)_J along column I, summed over the elements containing the node
-    double kxr = 0.0, kxi = 0.0, kyr = 0.0, kyi = 0.0;
-    {
-      const int e_hi = (I == g.npx - 1) ? g.nx - 1 : I / P;       // element whose node (I - e*P) this is
-      const int e_lo = (ax == 0 && I > 0) ? I / P - 1 : e_hi;     // the element before, at a shared node
-      for (int e = e_lo; e <= e_hi; ++e) {
-        const int a = I - e * P;
-        for (int cc = 0; cc <= P; ++cc) {
-          const size_t n = (size_t)J * g.npx + (e * P + cc);
-          kxr += ref.K[a][cc] * (double)ur[n];
-          kxi += ref.K[a][cc] * (double)ui[n];
-        }
-      }
-    }
-    {
-      const int e_hi = (J == g.npy - 1) ? g.ny - 1 : J / P;
-      const int e_lo = (ay == 0 && J > 0) ? J / P - 1 : e_hi;
-      for (int e = e_lo; e <= e_hi; ++e) {
-        const int a = J - e * P;
-        for (int cc = 0; cc <= P; ++cc) {
-          const size_t n = (size_t)(e * P + cc) * g.npx + I;
-          kyr += ref.K[a][cc] * (double)ur[n];
-          kyi += ref.K[a][cc] * (double)ui[n];
-        }
-      }
-    }
-    const double Aur = (g.hy / g.hx) * wyJ * kxr + (g.hx / g.hy) * wxI * kyr;
-    const double Aui = (g.hy / g.hx) * wyJ * kxi + (g.hx / g.hy) * wxI * kyi;
-    const double cj = c[gid];
-    const double m = 0.25 * g.hx * g.hy * wxI * wyJ;
-    const double M = m / (cj * cj);
-    const double sWE = 0.5 * g.hy * wyJ, sSN = 0.5 * g.hx * wxI;
-    double H = 0.0, bre = f_re[gid] * m, bim = f_im ? f_im[gid] * m : 0.0;
-    if (I == 0) { H += sWE / cj; if (bc) { bre += sWE * bc[(0 * 2 + 0) * g.EB + J]; bim += sWE * bc[(0 * 2 + 1) * g.EB + J]; } }
-    if (I == g.npx - 1) { H += sWE / cj; if (bc) { bre += sWE * bc[(1 * 2 + 0) * g.EB + J]; bim += sWE * bc[(1 * 2 + 1) * g.EB + J]; } }
-    if (J == 0) { H += sSN / cj; if (bc) { bre += sSN * bc[(2 * 2 + 0) * g.EB + I]; bim += sSN * bc[(2 * 2 + 1) * g.EB + I]; } }
-    if (J == g.npy - 1) { H += sSN / cj; if (bc) { bre += sSN * bc[(3 * 2 + 0) * g.EB + I]; bim += sSN * bc[(3 * 2 + 1) * g.EB + I]; } }
-    const double u_r = (double)ur[gid], u_i = (double)ui[gid];
-    const double w2M = g.omega * g.omega * M, wH = g.omega * H;
-    // (i w H + w^2 M) u = (w2M u_r - wH u_i) + i (w2M u_i + wH u_r)
-    const double rr = bre - Aur + (w2M * u_r - wH * u_i);
-    const double ri = bim - Aui + (w2M * u_i + wH * u_r);
-    r2 = rr * rr + ri * ri;
-    b2 = bre * bre + bim * bim;
+  for (int q = tid; q < PW * PH; q += kHelmBX * kHelmBY) {
+    const int px = q % PW, py = q / PW;
+    const int I = I0 + px, J = J0 + py;
+    const bool in = I >= 0 && I < g.npx && J >= 0 && J < g.npy;
+    const size_t n = (size_t)(in ? J : 0) * g.npx + (in ? I : 0);
+    sr[q] = in ? (acc)u[n] : acc(0);
+    si[q] = in ? (acc)u[total + n] : acc(0);
   }
-  for (int o = 16; o > 0; o >>= 1) {
-    r2 += __shfl_down_sync(0xffffffffu, r2, o);
-    b2 += __shfl_down_sync(0xffffffffu, b2, o);
-  }
-  const int w = threadIdx.x >> 5, ln = threadIdx.x & 31;
-  if (ln == 0) { red[0][w] = r2; red[1][w] = b2; }
   __syncthreads();
-  if (w == 0) {
-    const int nw = blockDim.x >> 5;
-    r2 = ln < nw ? red[0][ln] : 0.0;
-    b2 = ln < nw ? red[1][ln] : 0.0;
+  double r2 = 0.0, b2 = 0.0;
+  if (ex <= g.nx && ey <= g.ny) {
+    const bool hasL = ex > 0, hasR = ex < g.nx, hasD = ey > 0, hasU = ey < g.ny;
+    const acc ax_ = (acc)(g.hy / g.hx), ay_ = (acc)(g.hx / g.hy);
+    const acc mh = (acc)(0.25 * g.hx * g.hy);
+    // patch coordinates of the tile's first node
+    const int bx = (tx + 1) * P, by = (ty + 1) * P;
+#pragma unroll
+    for (int b = 0; b < P; ++b) {
+      if (b > 0 && !hasU) break;
+      const acc wy = b == 0 ? (acc)((hasD ? ref.w[P] : 0.0) + (hasU ? ref.w[0] : 0.0)) : (acc)ref.w[b];
+#pragma unroll
+      for (int a = 0; a < P; ++a) {
+        if (a > 0 && !hasR) break;
+        const acc wx = a == 0 ? (acc)((hasL ? ref.w[P] : 0.0) + (hasR ? ref.w[0] : 0.0)) : (acc)ref.w[a];
+        const acc *rr = sr + (by + b) * PW + bx, *ri = si + (by + b) * PW + bx;   // row of this node, at the tile's x origin
+        const acc *cr = sr + by * PW + bx + a, *ci = si + by * PW + bx + a;       // column of this node, at the tile's y origin
+        acc kxr = 0, kxi = 0, kyr = 0, kyi = 0;
+        if (a == 0) {   // node shared by the element on the left (its row P) and this one (row 0), where they exist
+#pragma unroll
+          for (int cc = 0; cc <= P; ++cc) {
+            const acc kl = hasL ? (acc)ref.K[P][cc] : acc(0), kr = hasR ? (acc)ref.K[0][cc] : acc(0);
+            kxr += kl * rr[cc - P] + kr * rr[cc];
+            kxi += kl * ri[cc - P] + kr * ri[cc];
+          }
+        } else {
+#pragma unroll
+          for (int cc = 0; cc <= P; ++cc) {
+            kxr += (acc)ref.K[a][cc] * rr[cc];
+            kxi += (acc)ref.K[a][cc] * ri[cc];
+          }
+        }
+        if (b == 0) {
+#pragma unroll
+          for (int cc = 0; cc <= P; ++cc) {
+            const acc kd = hasD ? (acc)ref.K[P][cc] : acc(0), ku = hasU ? (acc)ref.K[0][cc] : acc(0);
+            kyr += kd * cr[(cc - P) * PW] + ku * cr[cc * PW];
+            kyi += kd * ci[(cc - P) * PW] + ku * ci[cc * PW];
+          }
+        } else {
+#pragma unroll
+          for (int cc = 0; cc <= P; ++cc) {
+            kyr += (acc)ref.K[b][cc] * cr[cc * PW];
+            kyi += (acc)ref.K[b][cc] * ci[cc * PW];
+          }
+        }
+        const int I = ex * P + a, J = ey * P + b;
+        const size_t n = (size_t)J * g.npx + I;
+        const acc u_r = rr[a], u_i = ri[a];
+        const acc Aur = ax_ * wy * kxr + ay_ * wx * kyr, Aui = ax_ * wy * kxi + ay_ * wx * kyi;
+        const acc m = mh * wx * wy;
+        acc kk;   // w^2 / c^2
+        double cj = 0.0;
+        if (k2) kk = k2[n];
+        else { cj = c[n]; kk = (acc)(g.omega * g.omega / (cj * cj)); }
+        const bool onb = I == 0 || I == g.npx - 1 || J == 0 || J == g.npy - 1;
+        acc wH = 0;
+        double bre = 0.0, bim = 0.0;
+        if (MODE == 0) { bre = f_re[n] * (double)m; bim = f_im ? f_im[n] * (double)m : 0.0; }
+        if (onb) {   // impedance term and datum of eq. (1b) on the outer boundary only
+          if (k2) cj = c[n];
+          const double sWE = 0.5 * g.hy * (double)wy, sSN = 0.5 * g.hx * (double)wx;
+          double H = 0.0;
+          if (I == 0) { H += sWE / cj; if (MODE == 0 && bc) { bre += sWE * bc[(0 * 2 + 0) * g.EB + J]; bim += sWE * bc[(0 * 2 + 1) * g.EB + J]; } }
+          if (I == g.npx - 1) { H += sWE / cj; if (MODE == 0 && bc) { bre += sWE * bc[(1 * 2 + 0) * g.EB + J]; bim += sWE * bc[(1 * 2 + 1) * g.EB + J]; } }
+          if (J == 0) { H += sSN / cj; if (MODE == 0 && bc) { bre += sSN * bc[(2 * 2 + 0) * g.EB + I]; bim += sSN * bc[(2 * 2 + 1) * g.EB + I]; } }
+          if (J == g.npy - 1) { H += sSN / cj; if (MODE == 0 && bc) { bre += sSN * bc[(3 * 2 + 0) * g.EB + I]; bim += sSN * bc[(3 * 2 + 1) * g.EB + I]; } }
+          wH = (acc)(g.omega * H);
+        }
+        // (A - i w H - w^2 M) u = (A u_r - w2M u_r + wH u_i) + i (A u_i - w2M u_i - wH u_r)
+        const acc w2M = kk * m;
+        const acc yr = Aur - w2M * u_r + wH * u_i, yi = Aui - w2M * u_i - wH * u_r;
+        if (MODE == 1) {
+          y[n] = yr;
+          y[total + n] = yi;
+        } else {
+          const double rr_ = bre - (double)yr, ri_ = bim - (double)yi;
+          r2 += rr_ * rr_ + ri_ * ri_;
+          b2 += bre * bre + bim * bim;
+        }
+      }
+    }
+  }
+  if (MODE == 0) {
+    __shared__ double red[2][32];
     for (int o = 16; o > 0; o >>= 1) {
       r2 += __shfl_down_sync(0xffffffffu, r2, o);
       b2 += __shfl_down_sync(0xffffffffu, b2, o);
     }
-    if (ln == 0) { part[2 * (size_t)blockIdx.x] = r2; part[2 * (size_t)blockIdx.x + 1] = b2; }
+    const int w = tid >> 5, ln = tid & 31;
+    if (ln == 0) { red[0][w] = r2; red[1][w] = b2; }
+    __syncthreads();
+    if (w == 0) {
+      constexpr int nw = kHelmBX * kHelmBY / 32;
+      r2 = ln < nw ? red[0][ln] : 0.0;
+      b2 = ln < nw ? red[1][ln] : 0.0;
+      for (int o = 16; o > 0; o >>= 1) {
+        r2 += __shfl_down_sync(0xffffffffu, r2, o);
+        b2 += __shfl_down_sync(0xffffffffu, b2, o);
+      }
+      const size_t bid = (size_t)blockIdx.y * gridDim.x + blockIdx.x;
+      if (ln == 0) { part[2 * bid] = r2; part[2 * bid + 1] = b2; }
+    }
   }
+}
+
+// k2[n] = w^2 / c_n^2 in the operator's precision (built once per context and precision)
+template <typename acc>
+__global__ void k_helm_k2(long long n, double omega, const double *__restrict__ c, acc *__restrict__ k2) {
+  const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (q < n) k2[q] = (acc)(omega * omega / (c[q] * c[q]));
 }
 
 static __global__ void k_reduce2(const double *__restrict__ part, int n, double *__restrict__ out) {

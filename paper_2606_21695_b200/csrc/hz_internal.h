@@ -81,6 +81,8 @@ struct SweepArgs {
   real relax;
   const real *g_prev;
   real *lam_rw;
+  int pack;  // packed small-subdomain kernel (hz_sweep_pack.cuh): subdomains per thread block
+  int L;     // number of subdomains
 };
 
 // Extra arguments of the general-quadrilateral sweep kernel (hz_sweep_quad.cuh)
@@ -97,6 +99,7 @@ struct TileEntry {
   int minb;                  // __launch_bounds__ min blocks per SM (register cap = 64K / (minb * maxt))
   int cl;                    // > 1: thread-block-cluster kernel (hz_sweep_cl.cuh), CTAs per subdomain
   const void *fn;
+  int pk;                    // 1: packed small-subdomain kernel (hz_sweep_pack.cuh), several subdomains per block
 };
 
 struct SweepLaunch {
@@ -121,6 +124,11 @@ template <typename real>
 struct MinresArgs;
 cudaError_t launch_minres_f32(const MinresArgs<float> &a, int p, SweepLaunch cfg, cudaStream_t st);
 cudaError_t launch_minres_f64(const MinresArgs<double> &a, int p, SweepLaunch cfg, cudaStream_t st);
+// register-blocked MINRES (square tiles of m x m elements); cudaErrorInvalidValue when (p, m) is not compiled
+cudaError_t launch_minres_tile_f32(const MinresArgs<float> &a, const Elem1D<float> &ex1, const Elem1D<float> &ey1, int p, int m,
+                                   SweepLaunch cfg, cudaStream_t st);
+cudaError_t launch_minres_tile_f64(const MinresArgs<double> &a, const Elem1D<double> &ex1, const Elem1D<double> &ey1, int p, int m,
+                                   SweepLaunch cfg, cudaStream_t st);
 // compiled register-blocked instantiations of one precision
 int tile_table_f32(const TileEntry **out);
 int tile_table_f64(const TileEntry **out);

@@ -31,6 +31,10 @@ namespace hz {
 // C(P, MX, MY, CL, MAXT, MINB): cluster of CL CTAs per subdomain, coefficients in registers
 #define HZ_CL_TABLE_F32(C) \
   C(3, 1, 1, 2, 576, 1)    \
+  C(3, 2, 1, 2, 320, 1)    \
+  C(3, 2, 1, 4, 192, 1)    \
+  C(3, 2, 1, 4, 192, 2)    \
+  C(3, 1, 2, 2, 320, 1)    \
   C(3, 1, 1, 4, 320, 2)    \
   C(3, 1, 1, 8, 192, 3)    \
   C(3, 1, 1, 8, 640, 1)    \
@@ -40,13 +44,24 @@ namespace hz {
   C(4, 1, 1, 4, 384, 1)    \
   C(4, 1, 1, 16, 352, 1)
 
+// K(P, M, MAXT): several small subdomains per block (hz_sweep_pack.cuh), square tiles
+#define HZ_PK_TABLE_F32(K) \
+  K(1, 4, 128)             \
+  K(1, 2, 128)             \
+  K(2, 2, 128)             \
+  K(2, 1, 128)             \
+  K(3, 1, 128)             \
+  K(4, 1, 128)
+
 #define X_ENTRY(P, MX, MY, CSM, MAXT, MINB) \
   {P, MX, MY, CSM, MAXT, 0, MINB, 1, (const void *)k_sweep_tile<float, P, MX, MY, (CSM != 0), MAXT, MINB>},
 #define W_ENTRY(P, M, CSM, MAXT, MINB) \
   {P, M, M, CSM, MAXT, 1, MINB, 1, (const void *)k_sweep_ws<float, P, M, (CSM != 0), MAXT, MINB>},
 #define C_ENTRY(P, MX, MY, CL, MAXT, MINB) \
   {P, MX, MY, 0, MAXT, 0, MINB, CL, (const void *)k_sweep_cl<float, P, MX, MY, CL, MAXT, MINB>},
-static const TileEntry kTilesF32[] = {HZ_WS_TABLE_F32(W_ENTRY) HZ_TILE_TABLE_F32(X_ENTRY) HZ_CL_TABLE_F32(C_ENTRY)};
+#define K_ENTRY(P, M, MAXT) {P, M, M, 0, MAXT, 1, 1, 1, (const void *)k_sweep_pack<float, P, M, MAXT>, 1},
+static const TileEntry kTilesF32[] = {HZ_WS_TABLE_F32(W_ENTRY) HZ_TILE_TABLE_F32(X_ENTRY) HZ_CL_TABLE_F32(C_ENTRY) HZ_PK_TABLE_F32(K_ENTRY)};
+#undef K_ENTRY
 #undef C_ENTRY
 #undef X_ENTRY
 #undef W_ENTRY
@@ -64,6 +79,10 @@ cudaError_t launch_sweep_stream_f32(const SweepArgs<float> &a, float *scr, int p
 }
 cudaError_t launch_minres_f32(const MinresArgs<float> &a, int p, SweepLaunch cfg, cudaStream_t st) {
   return launch_minres_impl<float>(a, p, cfg, st);
+}
+cudaError_t launch_minres_tile_f32(const MinresArgs<float> &a, const Elem1D<float> &ex1, const Elem1D<float> &ey1, int p, int m,
+                                   SweepLaunch cfg, cudaStream_t st) {
+  return launch_minres_tile_impl<float>(a, ex1, ey1, p, m, cfg, st);
 }
 int tile_table_f32(const TileEntry **out) {
   *out = kTilesF32;

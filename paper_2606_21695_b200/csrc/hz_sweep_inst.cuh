@@ -6,6 +6,7 @@
 #include "hz_sweep.cuh"
 #include "hz_sweep_stream.cuh"
 #include "hz_sweep_cl.cuh"
+#include "hz_sweep_pack.cuh"
 #include "hz_sweep_tile.cuh"
 #include "hz_sweep_ws.cuh"
 
@@ -40,6 +41,26 @@ static cudaError_t launch_minres_impl(const MinresArgs<real> &a, int p, SweepLau
   cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem);
   if (e != cudaSuccess) return e;
   fn<<<cfg.blocks, cfg.threads, cfg.smem, st>>>(a);
+  return cudaGetLastError();
+}
+
+template <typename real>
+static cudaError_t launch_minres_tile_impl(const MinresArgs<real> &a, const Elem1D<real> &ex1, const Elem1D<real> &ey1, int p, int m,
+                                           SweepLaunch cfg, cudaStream_t st) {
+  void (*fn)(const MinresArgs<real>, const Elem1D<real>, const Elem1D<real>) = nullptr;
+  const int key = p * 10 + m;
+  switch (key) {
+    case 12: fn = k_minres_tile<real, 1, 2>; break;
+    case 14: fn = k_minres_tile<real, 1, 4>; break;
+    case 21: fn = k_minres_tile<real, 2, 1>; break;
+    case 22: fn = k_minres_tile<real, 2, 2>; break;
+    case 31: fn = k_minres_tile<real, 3, 1>; break;
+    case 41: fn = k_minres_tile<real, 4, 1>; break;
+    default: return cudaErrorInvalidValue;
+  }
+  cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cfg.smem);
+  if (e != cudaSuccess) return e;
+  fn<<<cfg.blocks, cfg.threads, cfg.smem, st>>>(a, ex1, ey1);
   return cudaGetLastError();
 }
 

@@ -112,7 +112,7 @@ def lib():
     L.hz_partition_ex.argtypes = [vp, ip, ip, ip, ip, ip, C.c_double, C.POINTER(hz_part_flags), C.POINTER(hz_part_info)]
     L.hz_ddm_solve_mixed.argtypes = [vp, vp, C.POINTER(hz_mixed_opts), vp, C.POINTER(hz_mixed_info), vp]
     L.hz_ddm_solve.argtypes = [vp, C.POINTER(hz_solve_opts), vp, C.POINTER(hz_solve_info), vp]
-    L.hz_operator_time.argtypes = [vp, vp, ip, C.POINTER(C.c_double), vp]
+    L.hz_operator_time.argtypes = [vp, vp, ip, ip, vp, C.POINTER(C.c_double), vp]
     L.hz_ddm_solve_sources.argtypes = [vp, C.POINTER(hz_solve_opts), ip, C.POINTER(vp), C.POINTER(vp),
                                        C.POINTER(hz_sources_info), vp]
     L.hz_ddm_solve_gmres.argtypes = [vp, C.POINTER(hz_gmres_opts), vp, C.POINTER(hz_gmres_info), vp]
@@ -224,10 +224,12 @@ def hz_ddm_solve(ctx, n_outer_max, n_wh=5, warm_start=True, relax=0.5, tol=0.0, 
     return info
 
 
-def hz_operator_time(ctx, u_ptr, reps=20, stream=None):
-    """ms per evaluation of the global Helmholtz operator (fp64) on the device field at u_ptr (the paper's normaliser)."""
+def hz_operator_time(ctx, u_ptr, prec=HZ_F64, reps=20, stream=None, y_ptr=None):
+    """ms per evaluation y = (A - i w H - w^2 M) u of the global Helmholtz operator in precision `prec` on the device
+    field at u_ptr (the paper's normaliser); y goes to y_ptr if given."""
     ms = C.c_double()
-    _check(ctx, lib().hz_operator_time(ctx, C.c_void_p(u_ptr), int(reps), C.byref(ms), C.c_void_p(stream) if stream else None))
+    _check(ctx, lib().hz_operator_time(ctx, C.c_void_p(u_ptr), int(prec), int(reps), C.c_void_p(y_ptr) if y_ptr else None,
+                                       C.byref(ms), C.c_void_p(stream) if stream else None))
     return ms.value
 
 

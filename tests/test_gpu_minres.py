@@ -21,8 +21,9 @@ def gpu_state(ctx, info):
             lam.cpu().numpy().reshape(info.blocks, 4, 2, info.edge_stride))
 
 
+@pytest.mark.parametrize("k", [1, 9])
 @pytest.mark.parametrize("fixed_iters", [True, False])
-def test_minres_cycles_match_the_oracle_fp64(fixed_iters):
+def test_minres_cycles_match_the_oracle_fp64(fixed_iters, k):
     """Two outer iterations (so that lambda != 0 and the warm start are exercised).  With a fixed iteration
     count the iterates must agree; run to tolerance, the iteration counts must agree as well."""
     if not torch.cuda.is_available():
@@ -37,7 +38,9 @@ def test_minres_cycles_match_the_oracle_fp64(fixed_iters):
     ctx = hz.hz_mesh_setup(inp.nx, inp.ny, inp.x0, inp.y0, inp.x1, inp.y1, inp.p, inp.c_nodes, inp.omega, inp.f_re,
                            inp.f_im, pack_bc(inp, bc))
     try:
-        info = hz.hz_partition(ctx, inp.sx, inp.sy, prec=hz.HZ_F64, dofs_per_thread=1)
+        # k = 1: one DOF per thread; k = 9: the register-blocked layout of the WaveHoltz kernels (k_minres_tile)
+        info = hz.hz_partition_ex(ctx, inp.sx, inp.sy, prec=hz.HZ_F64, dofs_per_thread=k, pack=1)
+        assert info.dofs_per_thread == k
         hz.hz_ddm_solve(ctx, 0, reset_state=True)
         its_g = []
         for warm in (False, True):
@@ -57,14 +60,51 @@ def test_minres_cycles_match_the_oracle_fp64(fixed_iters):
         assert rel(usub, u_o) <= 1e-8 and rel(lam, lam_o) <= 1e-8, (rel(usub, u_o), rel(lam, lam_o))
 
 
-def test_minres_fp32_reaches_the_papers_single_precision_tolerance():
+@pytest.mark.parametrize("p,k,prec,iters,tol", [(1, 4, hz.HZ_F64, 25, 1e-10), (1, 16, hz.HZ_F64, 25, 1e-10),
+                                                (2, 4, hz.HZ_F64, 25, 1e-10), (2, 16, hz.HZ_F64, 25, 1e-10),
+                                                (3, 9, hz.HZ_F64, 25, 1e-10), (4, 16, hz.HZ_F64, 25, 1e-10),
+                                                (3, 1, hz.HZ_F64, 25, 1e-10),
+                                                (3, 1, hz.HZ_F32, 15, 1e-4), (3, 9, hz.HZ_F32, 15, 1e-4),
+                                                (1, 16, hz.HZ_F32, 15, 1e-4), (4, 16, hz.HZ_F32, 15, 1e-4)])
+def test_minres_first_iterates_in_every_layout(p, k, prec, iters, tol):
+    """The first N MINRES iterates (before the Lanczos recurrence has had time to amplify the different summation
+    orders of the block reductions) at north_star's bars, 1e-10 in fp64 and 1e-4 in fp32, in the one-DOF-per-thread
+    layout and in every register-blocked tile the comparator is compiled for; ragged tile rows / columns included."""
+    if not torch.cuda.is_available():
+        pytest.fail("CUDA device required")
+    inp = hetero_inputs(8, 8, p, 2, 2, seed=500 + 10 * p + k)
+    pr = problem_from(inp)
+    st = O.ddm_setup(pr, inp.sx, inp.sy, inp.cfl_frac)
+    rng = np.random.default_rng(3)
+    for l in range(len(st.subs)):           # a non-trivial interface vector on both sides
+        st.lam[l] = [rng.standard_normal(len(a)) + 1j * rng.standard_normal(len(a)) if st.subs[l].neighbour[s] >= 0 else a
+                     for s, a in enumerate(st.lam[l])]
+    u0, lam0 = oracle_state_arrays(st)
+    O.ddm_sweep_minres(st, 0.0, iters, False, 0.5)
+    ctx = hz.hz_mesh_setup(inp.nx, inp.ny, inp.x0, inp.y0, inp.x1, inp.y1, inp.p, inp.c_nodes, inp.omega, inp.f_re)
+    try:
+        info = hz.hz_partition_ex(ctx, inp.sx, inp.sy, prec=prec, dofs_per_thread=k, pack=1)
+        assert info.dofs_per_thread == k
+        hz.hz_ddm_solve(ctx, 0, reset_state=True)
+        hz.hz_set_subdomain_state(ctx, None, torch.from_numpy(lam0).cuda().data_ptr())
+        mi, it_g, res = hz.hz_minres_cycle(ctx, info.blocks, 0.0, iters, warm_start=False, relax=0.5)
+        assert list(it_g) == [iters] * info.blocks
+        usub, lam = gpu_state(ctx, info)
+    finally:
+        hz.hz_destroy(ctx)
+    u_o, lam_o = oracle_state_arrays(st)
+    assert rel(usub, u_o) <= tol and rel(lam, lam_o) <= tol, (rel(usub, u_o), rel(lam, lam_o))
+
+
+@pytest.mark.parametrize("k", [1, 9])
+def test_minres_fp32_reaches_the_papers_single_precision_tolerance(k):
     if not torch.cuda.is_available():
         pytest.fail("CUDA device required")
     inp = make_config(2, n=32)
     pr = problem_from(inp)
     st = O.ddm_setup(pr, inp.sx, inp.sy, inp.cfl_frac)
     O.ddm_sweep_minres(st, 1e-12, 20000, False, 0.5)
-    ctx, info = hz.setup_from_inputs(inp, hz.HZ_F32, 1)
+    ctx, info = hz.setup_from_inputs(inp, hz.HZ_F32, k)
     try:
         hz.hz_ddm_solve(ctx, 0, reset_state=True)
         mi, iters, res = hz.hz_minres_cycle(ctx, info.blocks, 1e-6, 20000, relax=0.5)

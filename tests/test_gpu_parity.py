@@ -454,3 +454,31 @@ def test_graph_is_rebuilt_when_a_complex_source_arrives():
         assert rel(ug[0] + 1j * ug[1], O.ddm_gather(st)) <= 1e-10
     finally:
         hz.hz_destroy(ctx)
+
+
+@pytest.mark.parametrize("prec", [hz.HZ_F64, hz.HZ_F32])
+@pytest.mark.parametrize("p,nx,ny", [(1, 37, 9), (2, 33, 11), (3, 35, 10), (4, 34, 9)])
+def test_global_operator_kernel_matches_the_assembled_matrix(p, nx, ny, prec):
+    """hz_operator_time's kernel (the paper's "operator" of PAPER.md:223; the residual kernel's other mode): y =
+    (A - i w H - w^2 M) u on a random complex vector against the oracle's assembled sparse matrix.  The mesh spans
+    several 32x8-element blocks of the kernel with ragged tails in both directions."""
+    _require_cuda()
+    inp = hetero_inputs(nx, ny, p, 1, 1, seed=300 + p)
+    pr = problem_from(inp)
+    A, M, H, b = O.assemble_global(pr)
+    Z = O.helmholtz_matrix(A, M, H, pr.omega)
+    rng = np.random.default_rng(17)
+    nn = inp.npx * inp.npy
+    u = rng.standard_normal(nn) + 1j * rng.standard_normal(nn)
+    y_o = Z @ u
+    dt = torch.float64 if prec == hz.HZ_F64 else torch.float32
+    ctx = hz.hz_mesh_setup(inp.nx, inp.ny, inp.x0, inp.y0, inp.x1, inp.y1, inp.p, inp.c_nodes, inp.omega, inp.f_re)
+    try:
+        ud = torch.from_numpy(np.concatenate([u.real, u.imag])).to(dt).cuda()
+        yd = torch.zeros(2 * nn, dtype=dt, device="cuda")
+        ms = hz.hz_operator_time(ctx, ud.data_ptr(), prec, 2, y_ptr=yd.data_ptr())
+        assert ms > 0
+        y = yd.double().cpu().numpy()
+        assert rel(y[:nn] + 1j * y[nn:], y_o) <= (1e-13 if prec == hz.HZ_F64 else 2e-6)
+    finally:
+        hz.hz_destroy(ctx)
