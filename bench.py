@@ -683,6 +683,26 @@ def run_extras(hz, torch, args, flush, stream, sampler):
     # the rows SURVEY.md 8(f) marks "next": general convex quads (F3) and 3-D hexahedra (F4), sweep kernel only
     leg("config3_general_quads_f32", lambda: sweep_rate(hz, make_config(3, distort=0.2), "f32", 0, flush, stream, 3, 1))
 
+    def quad_prologue():
+        """Share of the general-quad sweep that is NOT the time loop (staging of the per-element geometric factors and
+        coefficients into shared memory with plain loads, b assembly, epilogue): sweep time is linear in n_wh; the
+        intercept of the fit through n_wh = 1 and 5 is the prologue + epilogue (north_star (b): TMA / cp.async staging
+        would only attack this share)."""
+        ctx, pinfo = hz.setup_from_inputs(make_config(3, distort=0.2), hz.HZ_F32, 0)
+        try:
+            hz.hz_ddm_solve(ctx, 1, n_wh=N_WH, reset_state=True, stream=stream)
+            t = {}
+            for nwh in (1, 5):
+                hz.hz_ddm_solve(ctx, 1, n_wh=nwh, stream=stream)
+                t[nwh] = min(hz.hz_ddm_solve(ctx, 1, n_wh=nwh, stream=stream).sweep_ms_total for _ in range(3))
+            per_it = (t[5] - t[1]) / 4.0
+            fixed = t[1] - per_it
+            return {"sweep_ms_n_wh_1": t[1], "sweep_ms_n_wh_5": t[5], "ms_per_waveholtz_iteration": per_it,
+                    "prologue_plus_epilogue_ms": fixed, "share_of_a_5_iteration_sweep": fixed / t[5]}
+        finally:
+            hz.hz_destroy(ctx)
+    leg("general_quads_prologue_share_f32", quad_prologue)
+
     def hexes():
         from paper_2606_21695_b200 import hz3
         from paper_2606_21695_b200.inputs import make_config_3d

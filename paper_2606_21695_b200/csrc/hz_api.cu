@@ -137,7 +137,9 @@ Geo make_geo(const hz_ctx *c) {
   Geo g{};
   g.nx = c->nx; g.ny = c->ny; g.p = c->p; g.npx = c->npx; g.npy = c->npy;
   g.sx = c->sx; g.sy = c->sy; g.ex = c->ex; g.ey = c->ey; g.E = c->E; g.EB = c->EB;
-  g.exq = c->nx / c->sx; g.exr = c->nx % c->sx; g.eyq = c->ny / c->sy; g.eyr = c->ny % c->sy;
+  if (c->sx > 0 && c->sy > 0) {  // (an unpartitioned context: the global kernels do not read these)
+    g.exq = c->nx / c->sx; g.exr = c->nx % c->sx; g.eyq = c->ny / c->sy; g.eyr = c->ny % c->sy;
+  }
   g.hx = c->hx; g.hy = c->hy; g.omega = c->omega; g.theta = c->theta; g.sigma = c->sigma;
   return g;
 }
@@ -565,20 +567,39 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
     const size_t narr = 2 * (size_t)(q.TX + q.TY);
     int G = 1;
     if (t.pk) {
-      // several small subdomains per block: G*NB bulk lanes fill whole warps (hz_sweep_pack.cuh)
+      // G subdomains per block: the G*NB full tiles fill whole bulk warps (hz_sweep_pack.cuh)
       const int NB = (q.ntx - 1) * (q.nty - 1), NE = q.ntx + q.nty - 1;
-      if (n_t > kTabCMax || NB > 16 || fl.pack == 1) return false;
+      if (n_t > kTabCMax) return false;
+      if (NB > 16 || fl.pack == 1) return false;   // packing only pays below one warp of full tiles
       auto gcd = [](int a, int b) { while (b) { const int r = a % b; a = b; b = r; } return a; };
-      G = fl.pack > 1 ? fl.pack : 32 / gcd(32, NB);
-      // a small grid keeps its parallelism: at least two blocks per SM before subdomains share a block
-      while (fl.pack <= 1 && G > 1 && (Lsel + G - 1) / G < 2LL * sm_count) G /= 2;
-      const size_t v16 = 16 / rs, chx = ((size_t)q.TX + v16 - 1) / v16 * v16, rsw = 4 * chx + v16;
+      const size_t v16 = 16 / rs;
+      const size_t chx = ((size_t)q.TX + v16 - 1) / v16 * v16, chy = ((size_t)q.TY + v16 - 1) / v16 * v16;
+      const size_t rsw = 2 * chx + 2 * chy + v16;  // square tiles: 4 chunks + 16 bytes
       const size_t nep = ((size_t)NE + v16 - 1) / v16 * v16;
-      for (;; G /= 2) {
-        nthr = roundup(G * NB, 32) + roundup(G * NE, 32);
-        sm = 2 * ((size_t)G * ((size_t)(q.ntx * q.nty + 1) * rsw + 2 * nep) + rsw) * rs;
-        if ((nthr <= t.maxt && sm <= smem_cap) || G == 1 || fl.pack > 1) break;
+      auto shape = [&](int g, int *thr, size_t *smb) {
+        *thr = roundup(g * NB, 32) + roundup(g * NE, 32);
+        *smb = 2 * ((size_t)g * ((size_t)(q.ntx * q.nty + 1) * rsw + 2 * nep) + rsw) * rs;
+      };
+      if (fl.pack > 1) {
+        G = fl.pack;
+      } else {
+        G = 32 / gcd(32, NB);                        // smallest G that fills the bulk warps ...
+        // ... and for 16-tile subdomains four bulk warps (measured on config 5, profiles/r02_config_sweep.md: p = 4,
+        // side 4: 8.75 -> 6.77 ms from G = 2 to 8; 4-tile subdomains are faster with one bulk warp than with two)
+        if (NB == 16) G = 8;
+        for (;; G /= 2) {
+          int t2; size_t s2;
+          shape(G, &t2, &s2);
+          if ((t2 <= t.maxt && s2 <= smem_cap) || G == 1) break;
+        }
+        // a small grid keeps its parallelism: at least two blocks per SM before subdomains share a block
+        while (G > 1 && (Lsel + G - 1) / G < 2LL * sm_count) G /= 2;
+        for (;; G /= 2) {
+          shape(G, &nthr, &sm);
+          if ((nthr <= t.maxt && sm <= smem_cap) || G == 1) break;
+        }
       }
+      shape(G, &nthr, &sm);
       if (G < 2) return false;
       ntv_pack = q.ntx * q.nty;
     } else if (t.cl > 1) {
@@ -666,7 +687,8 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
         // tiles of at most 16 DOFs; (2) clusters, smallest first; (3) the remaining shared-memory-coefficient kernels
         // (measured order on configs 4 and 5, profiles/r01_config_sweep.md)
         // (-1) several small subdomains per block, whenever a subdomain has at most 16 full tiles; largest tile <= 16 DOFs
-        if (q.pk) return -1000000000LL + (k_ <= 16 ? 16 - k_ : k_);
+        // fp32: the largest tile; fp64 (16-DOF tiles spill): the tile that gives a subdomain closest to 16 full tiles
+        if (q.pk) return -1000000000LL + (rs == 8 ? 100 * std::llabs(nbulk_ - 16) + k_ : (k_ <= 16 ? 16 - k_ : k_));
         if (q.cl > 1) return 200000000LL + q.cl * 1000 + k_;
         if (q.csm) return ((q.ws && k_ <= 16) ? 100000000LL : 300000000LL) + k_ * 100 + (1 - q.ws);
         return ((long long)(1 - q.ws) * 1000000 + dk * 1000 + k_) * 10 - q.minb;

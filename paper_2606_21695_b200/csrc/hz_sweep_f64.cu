@@ -47,12 +47,12 @@ namespace hz {
 
 // K(P, M, MAXT): several small subdomains per block (hz_sweep_pack.cuh), square tiles
 #define HZ_PK_TABLE_F64(K) \
-  K(1, 4, 128)             \
-  K(1, 2, 128)             \
-  K(2, 2, 128)             \
-  K(2, 1, 128)             \
-  K(3, 1, 128)             \
-  K(4, 1, 128)
+  K(1, 4, 256)             \
+  K(1, 2, 256)             \
+  K(2, 2, 256)             \
+  K(2, 1, 256)             \
+  K(3, 1, 256)             \
+  K(4, 1, 256)
 
 #define X_ENTRY(P, MX, MY, CSM, MAXT, MINB) \
   {P, MX, MY, CSM, MAXT, 0, MINB, 1, (const void *)k_sweep_tile<double, P, MX, MY, (CSM != 0), MAXT, MINB>},

@@ -138,3 +138,25 @@ def test_reference_arm_prints_contract_line():
     line = json.loads(out.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["cpu_baseline"]["kind"] == "oracle"
     assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["value"] > 0
+    assert line["cpu_baseline"]["cores"] == os.cpu_count()          # one oracle process per host core
+
+
+def test_the_oracle_window_of_bench_reproduces_the_full_problem():
+    """bench.py times the oracle on the lower-left window of the workload's subdomains (a full-size config-5 oracle
+    state would be 65 536 subdomains); a subdomain's DDM cycle in the window is that of the full problem."""
+    sys.path.insert(0, ROOT)
+    import bench
+    from oracle import hz_oracle as O
+    from paper_2606_21695_b200.inputs import make_config
+    inp = make_config(3, n=48)                                      # 6x6 subdomains of 8x8 elements
+    w = bench._oracle_window(inp, 2)
+    pr = O.Problem(inp.nx, inp.ny, inp.p, inp.x0, inp.y0, inp.x1, inp.y1, inp.c_nodes, inp.omega, inp.f_re.astype(complex))
+    st = O.ddm_setup(pr, inp.sx, inp.sy, inp.cfl_frac)
+    prw = O.Problem(w["nx"], w["ny"], w["p"], w["x0"], w["y0"], w["x1"], w["y1"], w["c"], w["omega"], w["f"].astype(complex))
+    n_t = O.choose_nt(w["p"], w["hx"], w["hy"], w["c_max"], w["omega"], w["cfl"])
+    assert n_t == st.tab.n_t
+    stw = O.ddm_setup(prw, w["sx"], w["sy"], w["cfl"], n_t=n_t)
+    for lw, l in ((0, 0), (1, 1), (2, inp.sx), (3, inp.sx + 1)):
+        uw, _ = O.ddm_cycle(stw, lw, 2, True)
+        u, _ = O.ddm_cycle(st, l, 2, True)
+        assert np.linalg.norm(uw - u) <= 1e-12 * np.linalg.norm(u)

@@ -119,7 +119,12 @@ def test_ddm_converges_to_the_direct_solve_and_single_subdomain_is_plain_wavehol
     for _ in range(3):
         st = O.ddm_solve(pr, 2, 2, 2, 100, 5, state=st)
         errs.append(np.linalg.norm(O.ddm_gather(st) - uref) / np.linalg.norm(uref))
-    assert errs[2] < 1e-4 and errs[1] < 0.5 * errs[0] and errs[2] < 0.5 * errs[1], errs   # linear convergence
+    # The absolute pin is errs[2] < 1e-4 against the direct solve.  The two ratio checks only assert LINEAR convergence
+    # of the relaxed fixed-point iteration (PAPER.md:85-90 gives no rate): per 100 sweeps the error must at least halve.
+    # The first version of this pin asked for a factor 0.3, which was a guess at the rate of this particular 2x2x2 case
+    # (measured 0.19 and 0.33: the second ratio misses 0.3) and not something the paper or the method fixes; 0.5 still
+    # fails a stagnating iteration (reading R12: rho = 1 stagnates, rho = 0.5 converges).
+    assert errs[2] < 1e-4 and errs[1] < 0.5 * errs[0] and errs[2] < 0.5 * errs[1], errs
     # L = 1: one sweep is n_wh WaveHoltz iterations on the whole box
     st1 = O.ddm_solve(pr, 1, 1, 1, 1, 3)
     A, M, H, b = O.assemble_global(pr)
