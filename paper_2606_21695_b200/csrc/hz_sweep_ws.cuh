@@ -22,9 +22,6 @@
 #ifndef HZ_WS_PACK
 #define HZ_WS_PACK 1
 #endif
-#ifndef HZ_WS_PRE_SPLIT
-#define HZ_WS_PRE_SPLIT 0
-#endif
 
 namespace hz {
 
@@ -215,7 +212,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
         // (grid-filling instantiations: config 3 fp32 1.257 -> 1.224 ms, fp64 2.498 -> 2.415 ms); otherwise after the
         // neighbour loads are issued, where it covers their latency (config 2, one bulk warp per scheduler: 0.114 ms
         // against 0.124 ms with PRE)
-        auto own_x = [&]() {
+        auto own_part = [&]() {
 #pragma unroll
         for (int b = 0; b < T; ++b) {
           real q[T + 1];
@@ -224,8 +221,6 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
           q[T] = real(0);
           X0[b] = line_own<real, P, M, false>(q, d0x, A.ex1, S[b]);
         }
-        };
-        auto own_y = [&]() {
 #pragma unroll
         for (int a = 0; a < T; ++a) {
           real q[T + 1], Sc[T];
@@ -251,11 +246,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
             if (a >= 2 * NP) vr[b][a] = fmaT(tn.k, p[b][a], vr[b][a]);
         }
         };
-        auto own_part = [&]() { own_x(); own_y(); };
-        if constexpr (PRE) {
-          if constexpr (HZ_WS_PRE_SPLIT) own_x();   // half before the barrier (absorbs the skew between the warps) ...
-          else own_part();
-        }
+        if constexpr (PRE) own_part();
         bar_sync_all(NTH);
         // issue the neighbour loads first, then do the part of the step that needs none of them
         const real *nL = pL + cur, *nR = pR + cur, *nD = pD + cur, *nU = pU + cur;
@@ -266,7 +257,6 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_ws(const SweepArgs<real> A
         ld_chunk<T>(nD + 2 * CH, piD);
         ld_chunk<T>(nU + 3 * CH, qU);
         if constexpr (!PRE) own_part();
-        else if constexpr (HZ_WS_PRE_SPLIT) own_y();  // ... half behind the neighbour loads (covers their latency)
 #pragma unroll
         for (int b = 0; b < T; ++b) {
           if (b == 0) line_finish<real, P, M, false>(qR[b], piL[b], s0x, X0[b], A.ex1, S[b]);
