@@ -602,6 +602,18 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
       shape(G, &nthr, &sm);
       if (G < 2) return false;
       ntv_pack = q.ntx * q.nty;
+    } else if (t.cl > 1 && t.ws) {
+      // cluster kernel with warp-specialised edge pieces (hz_sweep_cw.cuh): the full-tile columns are cut into t.cl strips
+      if (no_cl || n_t > kTabCMax || q.ntx - 1 < t.cl) return false;
+      const int nbc = q.ntx - 1, nbr = q.nty - 1, wmax = (nbc + t.cl - 1) / t.cl, nel = nbr + wmax + 1;
+      nthr = roundup(wmax * nbr, 32) + roundup(nel, 32);
+      const size_t v16 = 16 / rs;
+      const size_t chx = ((size_t)q.TX + v16 - 1) / v16 * v16, chy = ((size_t)q.TY + v16 - 1) / v16 * v16;
+      size_t rsw = 2 * chx + 2 * chy;
+      if ((rsw / v16) % 2 == 0) rsw += v16;
+      const size_t nep = ((size_t)nel + v16 - 1) / v16 * v16;
+      const size_t bufw = ((size_t)(wmax + 1) * q.nty + 2) * rsw + 2 * nep, hs = 2 * (size_t)nbr * chy + 2 * v16;
+      sm = (2 * bufw + 2 * hs) * rs + 16;
     } else if (t.cl > 1) {
       if (no_cl || n_t > kTabCMax || q.ntx < t.cl) return false;
       const int wmax = (q.ntx + t.cl - 1) / t.cl;
@@ -689,7 +701,8 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
         // (-1) several small subdomains per block, whenever a subdomain has at most 16 full tiles; largest tile <= 16 DOFs
         // fp32: the largest tile; fp64 (16-DOF tiles spill): the tile that gives a subdomain closest to 16 full tiles
         if (q.pk) return -1000000000LL + (rs == 8 ? 100 * std::llabs(nbulk_ - 16) + k_ : (k_ <= 16 ? 16 - k_ : k_));
-        if (q.cl > 1) return 200000000LL + q.cl * 1000 + k_;
+        // (2) clusters, smallest first; at equal size the warp-specialised cluster kernel, larger tile first
+        if (q.cl > 1) return 200000000LL + q.cl * 1000 + (q.ws ? 100 - k_ : 500 + k_);
         if (q.csm) return ((q.ws && k_ <= 16) ? 100000000LL : 300000000LL) + k_ * 100 + (1 - q.ws);
         return ((long long)(1 - q.ws) * 1000000 + dk * 1000 + k_) * 10 - q.minb;
       };
@@ -715,7 +728,7 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
     // warp-role order of k_sweep_ws: a 3-warp block (2 bulk + 1 edge) puts its edge warp in the middle, so that the bulk
     // warps of the blocks resident on an SM (consecutive hardware warp slots, slot mod 4 = sub-partition) spread evenly
     // over the 4 schedulers (measured: config 2 fp32 0.147 -> 0.111 ms per sweep, config 3 fp32 1.273 -> 1.241 ms)
-    ctx->worder = fl.warp_order > 0 ? fl.warp_order - 1 : ((ctx->ws && bl.threads == 96) ? 1 : 0);
+    ctx->worder = fl.warp_order > 0 ? fl.warp_order - 1 : ((ctx->ws && ctx->cl == 1 && bl.threads == 96) ? 1 : 0);
   } else if (streamed) {
     lay.variant = 2; lay.NT = N < 1024 ? roundup(N, 32) : 1024; lay.NS = roundup(N, 32); lay.TX = lay.TY = 1;
     lay.ntx = lay.nty = 0;

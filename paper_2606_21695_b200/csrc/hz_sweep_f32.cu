@@ -53,6 +53,15 @@ namespace hz {
   K(3, 1, 256)             \
   K(4, 1, 256)
 
+// CW(P, MX, MY, CL, MAXT, MINB): cluster of CL CTAs per subdomain, warp-specialised edge pieces (hz_sweep_cw.cuh)
+#define HZ_CW_TABLE_F32(CW) \
+  CW(3, 2, 1, 2, 320, 1)   \
+  CW(3, 2, 1, 4, 192, 1)   \
+  CW(3, 2, 1, 8, 352, 1)   \
+  CW(2, 2, 2, 4, 320, 1)   \
+  CW(4, 1, 1, 4, 320, 1)   \
+  CW(4, 1, 1, 16, 352, 1)
+
 #define X_ENTRY(P, MX, MY, CSM, MAXT, MINB) \
   {P, MX, MY, CSM, MAXT, 0, MINB, 1, (const void *)k_sweep_tile<float, P, MX, MY, (CSM != 0), MAXT, MINB>},
 #define W_ENTRY(P, M, CSM, MAXT, MINB) \
@@ -60,7 +69,9 @@ namespace hz {
 #define C_ENTRY(P, MX, MY, CL, MAXT, MINB) \
   {P, MX, MY, 0, MAXT, 0, MINB, CL, (const void *)k_sweep_cl<float, P, MX, MY, CL, MAXT, MINB>},
 #define K_ENTRY(P, M, MAXT) {P, M, M, 0, MAXT, 1, 1, 1, (const void *)k_sweep_pack<float, P, M, MAXT>, 1},
-static const TileEntry kTilesF32[] = {HZ_WS_TABLE_F32(W_ENTRY) HZ_TILE_TABLE_F32(X_ENTRY) HZ_CL_TABLE_F32(C_ENTRY) HZ_PK_TABLE_F32(K_ENTRY)};
+#define CW_ENTRY(P, MX, MY, CL, MAXT, MINB) \
+  {P, MX, MY, 0, MAXT, 1, MINB, CL, (const void *)k_sweep_cw<float, P, MX, MY, CL, MAXT, MINB>},
+static const TileEntry kTilesF32[] = {HZ_CW_TABLE_F32(CW_ENTRY) HZ_WS_TABLE_F32(W_ENTRY) HZ_TILE_TABLE_F32(X_ENTRY) HZ_CL_TABLE_F32(C_ENTRY) HZ_PK_TABLE_F32(K_ENTRY)};
 #undef K_ENTRY
 #undef C_ENTRY
 #undef X_ENTRY

@@ -54,6 +54,13 @@ namespace hz {
   K(3, 1, 256)             \
   K(4, 1, 256)
 
+// CW(P, MX, MY, CL, MAXT, MINB): cluster of CL CTAs per subdomain, warp-specialised edge pieces (hz_sweep_cw.cuh)
+#define HZ_CW_TABLE_F64(CW) \
+  CW(3, 1, 1, 4, 320, 1)   \
+  CW(3, 1, 1, 16, 352, 1)  \
+  CW(2, 1, 1, 8, 608, 1)   \
+  CW(4, 1, 1, 8, 192, 1)
+
 #define X_ENTRY(P, MX, MY, CSM, MAXT, MINB) \
   {P, MX, MY, CSM, MAXT, 0, MINB, 1, (const void *)k_sweep_tile<double, P, MX, MY, (CSM != 0), MAXT, MINB>},
 #define W_ENTRY(P, M, CSM, MAXT, MINB) \
@@ -61,7 +68,9 @@ namespace hz {
 #define C_ENTRY(P, MX, MY, CL, MAXT, MINB) \
   {P, MX, MY, 0, MAXT, 0, MINB, CL, (const void *)k_sweep_cl<double, P, MX, MY, CL, MAXT, MINB>},
 #define K_ENTRY(P, M, MAXT) {P, M, M, 0, MAXT, 1, 1, 1, (const void *)k_sweep_pack<double, P, M, MAXT>, 1},
-static const TileEntry kTilesF64[] = {HZ_WS_TABLE_F64(W_ENTRY) HZ_TILE_TABLE_F64(X_ENTRY) HZ_CL_TABLE_F64(C_ENTRY) HZ_PK_TABLE_F64(K_ENTRY)};
+#define CW_ENTRY(P, MX, MY, CL, MAXT, MINB) \
+  {P, MX, MY, 0, MAXT, 1, MINB, CL, (const void *)k_sweep_cw<double, P, MX, MY, CL, MAXT, MINB>},
+static const TileEntry kTilesF64[] = {HZ_CW_TABLE_F64(CW_ENTRY) HZ_WS_TABLE_F64(W_ENTRY) HZ_TILE_TABLE_F64(X_ENTRY) HZ_CL_TABLE_F64(C_ENTRY) HZ_PK_TABLE_F64(K_ENTRY)};
 #undef K_ENTRY
 #undef C_ENTRY
 #undef X_ENTRY

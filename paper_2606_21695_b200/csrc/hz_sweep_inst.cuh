@@ -6,6 +6,7 @@
 #include "hz_sweep.cuh"
 #include "hz_sweep_stream.cuh"
 #include "hz_sweep_cl.cuh"
+#include "hz_sweep_cw.cuh"
 #include "hz_sweep_pack.cuh"
 #include "hz_sweep_tile.cuh"
 #include "hz_sweep_ws.cuh"

@@ -350,19 +350,24 @@ def test_more_than_256_time_steps_uses_the_shared_memory_table():
     assert g["info"].n_t > 256 and g["info"].dofs_per_thread == 1
 
 
-@pytest.mark.parametrize("prec,cl", [(hz.HZ_F64, 2), (hz.HZ_F64, 4), (hz.HZ_F32, 2), (hz.HZ_F32, 8), (hz.HZ_F64, 16)])
-def test_cluster_kernel_matches_the_oracle(prec, cl):
-    """Thread-block-cluster variant (hz_sweep_cl.cuh): the subdomain's tile grid is cut into column strips, one CTA
-    each, with the strip-boundary chunks pushed through DSMEM.  Forced here on small subdomains (the automatic choice
-    only uses it when one SM cannot hold the state)."""
-    g = check_case(make_config(2, n=32, sub_elems=16 if cl >= 8 else None), prec, 9, n_outer=3, n_wh=2, flags=dict(cluster=cl))
+@pytest.mark.parametrize("prec,cl,k", [(hz.HZ_F64, 2, 9), (hz.HZ_F64, 4, 9), (hz.HZ_F32, 2, 9), (hz.HZ_F32, 8, 9), (hz.HZ_F64, 16, 9),
+                                       (hz.HZ_F32, 2, 18), (hz.HZ_F32, 4, 18), (hz.HZ_F32, 8, 18)])
+def test_cluster_kernel_matches_the_oracle(prec, cl, k):
+    """Thread-block-cluster variants: the subdomain's tile grid is cut into column strips, one CTA each, with the
+    strip-boundary chunks pushed through DSMEM.  k_sweep_cl (hz_sweep_cl.cuh; fp32 k = 9 with 2 or 8 CTAs, fp64 with 2)
+    and k_sweep_cw (hz_sweep_cw.cuh: warp-specialised edge pieces; fp32 with 6x3 tiles, k = 18, fp64 k = 9 with 4 or 16
+    CTAs).  Forced here on small subdomains (the automatic choice only uses clusters when one SM cannot hold the state)."""
+    g = check_case(make_config(2, n=32, sub_elems=16 if cl >= 8 or k == 18 else None), prec, k, n_outer=3, n_wh=2,
+                   flags=dict(cluster=cl))
     assert g["info"].cluster_size == cl
     if cl >= 8:      # 16 (beyond the portable size: opt-in attribute) and 8 need at least that many tile columns
         return
     inp = hetero_inputs(12, 4, 3, 2, 2, seed=55)      # 6x2-element subdomains: strips of unequal width
     rng = np.random.default_rng(12)
     bc = [rng.standard_normal(n) + 1j * rng.standard_normal(n) for n in (inp.npy, inp.npy, inp.npx, inp.npx)]
-    g = check_case(inp, prec, 9, n_outer=3, n_wh=2, warm=False, bc=bc, flags=dict(cluster=cl))
+    if k == 18 and cl > 3:
+        return                                        # 3 columns of 6x3 tiles: at most 3 strips
+    g = check_case(inp, prec, k, n_outer=3, n_wh=2, warm=False, bc=bc, flags=dict(cluster=cl))
     assert g["info"].cluster_size == cl
 
 
@@ -397,13 +402,14 @@ def test_stream_of_sources_matches_the_sequential_calls_bit_for_bit():
             hz.hz_destroy(ctx)
 
 
-@pytest.mark.parametrize("prec,cl", [(hz.HZ_F32, 2), (hz.HZ_F32, 4), (hz.HZ_F32, 8), (hz.HZ_F64, 2), (hz.HZ_F64, 4),
-                                     (hz.HZ_F64, 8), (hz.HZ_F64, 16)])      # every p = 3 cluster size that is compiled
-def test_cluster_halo_protocol_stress(prec, cl):
+@pytest.mark.parametrize("prec,cl,k", [(hz.HZ_F32, 2, 9), (hz.HZ_F32, 4, 9), (hz.HZ_F32, 8, 9), (hz.HZ_F64, 2, 9), (hz.HZ_F64, 4, 9),
+                                       (hz.HZ_F64, 8, 9), (hz.HZ_F64, 16, 9), (hz.HZ_F32, 2, 18), (hz.HZ_F32, 4, 18),
+                                       (hz.HZ_F32, 8, 18)])      # every p = 3 cluster shape that is compiled
+def test_cluster_halo_protocol_stress(prec, cl, k):
     """compute-sanitizer is closed on this GPU pool, so the two-slot halo protocol of hz_sweep_cl.cuh (st.async pushes
     into the adjacent CTA's shared memory, mbarrier transaction counts, no cluster barrier in the time loop) is
-    stressed instead: many time steps with strips of UNEQUAL width (17 tile columns over cl CTAs; some strips are a
-    single column at cl = 16), 20 repeats that must be bit-identical (a race shows as run-to-run noise), and the
+    stressed instead, for k_sweep_cl and k_sweep_cw (k = 18, and fp64 with 4 or 16 CTAs): many time steps with strips of
+    UNEQUAL width (17, resp. 16 or 8, tile columns over cl CTAs; some strips are a single column), 20 repeats that must be bit-identical (a race shows as run-to-run noise), and the
     result must agree with the single-CTA kernel's to rounding (its edge pieces associate their sums differently)."""
     _require_cuda()
     inp = make_config(2, n=32, sub_elems=16)
@@ -411,7 +417,7 @@ def test_cluster_halo_protocol_stress(prec, cl):
     dt = torch.float64 if prec == hz.HZ_F64 else torch.float32
 
     def run(flags, reps):
-        ctx, info = hz.setup_from_inputs(inp, prec, 9, **flags)
+        ctx, info = hz.setup_from_inputs(inp, prec, k if flags.get("cluster", 0) > 1 else 9, **flags)
         try:
             outs = []
             for _ in range(reps):
