@@ -39,9 +39,12 @@ E2E_SOURCES = 12  # sources of the end-to-end leg (independent of --steps)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel: STORED figures from one
 # `ncu --set full` capture each (not measured in this run); the summaries are in profiles/.
 STORED_TRAFFIC = {
+    "config5_p3_s8_f32": {"bytes": 1.525e9, "from": "profiles/r02_a_sweep_ws_cfg5_f32.md", "captured": "round 2"},
+    "config5_p3_s8_f64": {"bytes": 2.848e9, "from": "profiles/r02_b_sweep_ws_cfg5_f64.md", "captured": "round 2"},
     "config3_p3_s8_f32": {"bytes": 72.3e6, "from": "profiles/r01_b_sweep_ws_cfg3_f32.md", "captured": "round 1"},
     "config3_p3_s8_f64": {"bytes": 140.1e6, "from": "profiles/r01_c_sweep_ws_cfg3_f64.md", "captured": "round 1"},
-    "config4_p3_s32_f32": {"bytes": 242.7e6, "from": "profiles/r01_e_sweep_cl_cfg4_f32.md", "captured": "round 1"},
+    "config4_p3_s32_f32": {"bytes": 234.5e6, "from": "profiles/r02_c_sweep_cw_cfg4_f32.md", "captured": "round 2"},
+    "config4_p3_s32_f64": {"bytes": 500.5e6, "from": "profiles/r02_d_sweep_cw_cfg4_f64.md", "captured": "round 2"},
 }
 
 
@@ -493,7 +496,7 @@ def run_b200(args):
                        "parallelism": "replicas only (one independent problem per GPU)" if world > 1 else "1 GPU"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu,
             "extras": extras}
-    print(json.dumps(line), flush=True)
+    print(json.dumps(_finite(line), allow_nan=False), flush=True)
     if world > 1:
         dist.destroy_process_group()
 
@@ -501,19 +504,19 @@ def run_b200(args):
 # ---------------------------------------------------------------------------------------------------
 # secondary measurements (N = 1 only): the other configs, time to solution, the comparator, F3 / F4
 # ---------------------------------------------------------------------------------------------------
-def time_to_solution(hz, inp, prec_name, tol, every, nmax, stream, driver="fixed_point", restart=50):
+def time_to_solution(hz, inp, prec_name, tol, every, nmax, stream, driver="fixed_point", restart=50, n_wh=2):
     """DDM time-to-solution (BASELINE.json metric 1): global relative residual (hz_residual, fp64) to `tol`,
     n_wh = 2, rho = 0.5, warm start.  fixed_point: hz_ddm_solve with CUDA-graph replay between residual checks;
     mixed: hz_ddm_solve_mixed (fp32 sweeps on the correction, fp64 state); gmres: hz_ddm_solve_gmres."""
-    out = {"tol": tol, "n_wh": 2, "relax": 0.5, "driver": driver}
+    out = {"tol": tol, "n_wh": n_wh, "relax": 0.5, "driver": driver}
     if driver == "mixed":
         lo, _ = hz.setup_from_inputs(inp, hz.HZ_F32, 0)
         hi, _ = hz.setup_from_inputs(inp, hz.HZ_F64, 0)
         try:
             m = every
-            hz.hz_ddm_solve_mixed(lo, hi, 1, m, n_wh=2, reset_state=True, stream=stream)           # allocation, warm-up
+            hz.hz_ddm_solve_mixed(lo, hi, 1, m, n_wh=n_wh, reset_state=True, stream=stream)           # allocation, warm-up
             t0 = time.perf_counter()
-            s = hz.hz_ddm_solve_mixed(lo, hi, max(1, nmax // m), m, n_wh=2, relax=0.5, tol=tol, check_every=2,
+            s = hz.hz_ddm_solve_mixed(lo, hi, max(1, nmax // m), m, n_wh=n_wh, relax=0.5, tol=tol, check_every=2,
                                       reset_state=True, stream=stream)
             out.update(sweeps=s.sweeps_lo + s.sweeps_hi, sweeps_fp32=s.sweeps_lo, sweeps_fp64=s.sweeps_hi,
                        rel_residual=s.rel_residual, device_ms=s.total_ms, wall_ms=(time.perf_counter() - t0) * 1e3,
@@ -525,18 +528,19 @@ def time_to_solution(hz, inp, prec_name, tol, every, nmax, stream, driver="fixed
     ctx, pinfo = hz.setup_from_inputs(inp, hz.HZ_F32 if prec_name == "f32" else hz.HZ_F64, 0)
     try:
         if driver == "gmres":
-            hz.hz_ddm_solve_gmres(ctx, 3, n_wh=2, restart=restart, stream=stream)                  # allocation, warm-up
+            hz.hz_ddm_solve_gmres(ctx, 3, n_wh=n_wh, restart=restart, stream=stream)                  # allocation, warm-up
             t0 = time.perf_counter()
-            s = hz.hz_ddm_solve_gmres(ctx, nmax, n_wh=2, relax=0.5, restart=restart, tol=tol, reset_state=True, stream=stream)
+            s = hz.hz_ddm_solve_gmres(ctx, nmax, n_wh=n_wh, relax=0.5, restart=restart, tol=tol, reset_state=True, stream=stream)
             out.update(sweeps=s.sweeps_done, cycles=s.cycles, rel_residual=s.rel_residual, device_ms=s.total_ms,
                        wall_ms=(time.perf_counter() - t0) * 1e3, restart=restart, reached=bool(s.rel_residual <= tol))
         else:
-            hz.hz_ddm_solve(ctx, every, n_wh=2, reset_state=True, use_graph=True, stream=stream)   # graph capture, warm-up
+            hz.hz_ddm_solve(ctx, every, n_wh=n_wh, reset_state=True, use_graph=True, stream=stream)   # graph capture, warm-up
             t0 = time.perf_counter()
-            s = hz.hz_ddm_solve(ctx, nmax, n_wh=2, warm_start=True, relax=0.5, tol=tol, check_every=every,
+            s = hz.hz_ddm_solve(ctx, nmax, n_wh=n_wh, warm_start=True, relax=0.5, tol=tol, check_every=every,
                                 reset_state=True, use_graph=True, stream=stream)
             out.update(sweeps=s.n_outer_done, rel_residual=s.rel_residual, device_ms=s.total_ms,
-                       wall_ms=(time.perf_counter() - t0) * 1e3, cuda_graph=True, reached=bool(s.rel_residual <= tol))
+                       wall_ms=(time.perf_counter() - t0) * 1e3, cuda_graph=True, reached=bool(s.rel_residual <= tol),
+                       diverged=bool(not (s.rel_residual == s.rel_residual) or s.rel_residual > 1e3))
     finally:
         hz.hz_destroy(ctx)
     return out
@@ -614,12 +618,23 @@ def minres_vs_waveholtz(hz, torch, inp, prec_name, stream, max_nwh=4096):
     finally:
         hz.hz_destroy(ctx)
     ctx2, info2 = hz.setup_from_inputs(inp, prec, 0)
+    mk = None
     try:
         hz.hz_ddm_solve(ctx2, 0, reset_state=True, stream=stream)
         tk = timed(ctx2, hi)
+        try:   # MINRES in the same register-blocked layout (k_minres_tile), where the tile is one it is compiled for
+            hz.hz_ddm_solve(ctx2, 0, reset_state=True, stream=stream)
+            hz.hz_set_subdomain_state(ctx2, None, lam0.data_ptr(), stream=stream)
+            hz.hz_minres_cycle(ctx2, info2.blocks, tol, 100000, stream=stream)
+            mk, _, resk = hz.hz_minres_cycle(ctx2, info2.blocks, tol, 100000, stream=stream)
+        except hz.HzError:
+            mk = None
     finally:
         hz.hz_destroy(ctx2)
-    return {"p": inp.p, "sub_side": inp.nx // inp.sx, "dofs_per_sub": info.dofs_per_sub, "blocks": info.blocks,
+    extra = {} if mk is None else {"minres_ms_register_blocked": mk.kernel_ms, "minres_iters_mean_register_blocked": mk.iters_mean,
+                                   "minres_true_residual_register_blocked": float(resk.max()),
+                                   "speedup_same_layout_register_blocked": mk.kernel_ms / tk}
+    return {**extra, "p": inp.p, "sub_side": inp.nx // inp.sx, "dofs_per_sub": info.dofs_per_sub, "blocks": info.blocks,
             "prec": prec_name, "minres_iters_mean": mi.iters_mean, "minres_iters_max": mi.iters_max,
             "minres_true_residual": float(res.max()), "minres_ms": mi.kernel_ms, "n_wh": hi,
             "waveholtz_ms_one_dof_per_thread": t1, "waveholtz_ms_register_blocked": tk,
@@ -670,6 +685,13 @@ def run_extras(hz, torch, args, flush, stream, sampler):
     for cfg, pr, tol, every, nmax, drv in tts:
         key = f"config{cfg}_{'f32_sweeps_f64_state' if drv == 'mixed' else pr}_time_to_solution" + ("" if drv != "gmres" else "_gmres")
         leg(key, lambda: time_to_solution(hz, get(cfg), pr, tol, every, nmax, stream, drv))
+    # one WaveHoltz iteration per sweep (warm start): more sweeps, each half as long (n_wh in {1, 2})
+    # (config 3 diverges with n_wh = 1: one WaveHoltz iteration per sweep is too loose an inner solve there; the entry
+    # is kept, with a small sweep budget, so that the line shows it)
+    for cfg, pr, every, nmax, drv in ((3, "f64", 50, 1000, "fixed_point"), (4, "f32", 50, 6000, "fixed_point"),
+                                      (4, "f64", 50, 6000, "fixed_point")):
+        key = f"config{cfg}_{'f32_sweeps_f64_state' if drv == 'mixed' else pr}_time_to_solution_n_wh_1"
+        leg(key, lambda: time_to_solution(hz, get(cfg), pr, 1e-4, every, nmax, stream, drv, n_wh=1))
     inputs.clear()
 
     leg("paper_style_cycle_512_p3_f32", lambda: paper_style_cycle(hz, torch, stream, flush))
@@ -789,36 +811,43 @@ def run_tables(args):
                 for pr in ("f32", "f64"):
                     rate_row(5, pr, 0, n=(6144 // p) // sc // s * s, p=p, s=s, reps=2, distort=0.2)
     elif which == "tts":
-        print("| cfg | arithmetic | tol | driver | sweeps | residual reached | device ms | note |")
-        print("|---|---|---|---|---|---|---|---|")
+        print("| cfg | arithmetic | tol | driver | n_wh | sweeps | residual reached | device ms | note |")
+        print("|---|---|---|---|---|---|---|---|---|")
         for cfg in (1, 2, 3, 4):
             inp = make_config(cfg)
             every = 10 if cfg == 1 else 50
             tol_hi = 1e-8 if cfg == 1 else 1e-4
-            rows = [("f64", tol_hi, "fixed_point"), ("f32", 1e-4, "fixed_point"), ("f32", tol_hi, "mixed"),
-                    ("f64", tol_hi, "gmres"), ("f32", 1e-4, "gmres")]
-            for pr, tol, drv in rows:
-                r = time_to_solution(hz, inp, pr, tol, 25 if drv == "mixed" else every, 20000 if drv != "gmres" else 4000,
-                                     stream, drv, restart=50 if cfg <= 2 else 100)
+            rows = [("f64", tol_hi, "fixed_point", 2), ("f32", 1e-4, "fixed_point", 2), ("f32", tol_hi, "mixed", 2),
+                    ("f64", tol_hi, "fixed_point", 1), ("f32", tol_hi, "mixed", 1),
+                    ("f64", tol_hi, "gmres", 2), ("f32", 1e-4, "gmres", 2)]
+            for pr, tol, drv, nwh in rows:
+                r = time_to_solution(hz, inp, pr, tol, 25 if drv == "mixed" else every, 40000 if drv != "gmres" else 4000,
+                                     stream, drv, restart=50 if cfg <= 2 else 100, n_wh=nwh)
                 arith = "fp32 sweeps, fp64 state" if drv == "mixed" else pr
                 note = "" if r["reached"] else "NOT reached"
                 if drv == "mixed":
                     note += f" {r['sweeps_fp32']} fp32 + {r['sweeps_fp64']} fp64 sweeps"
-                print(f"| {cfg} | {arith} | {tol:g} | {drv} | {r['sweeps']} | {r['rel_residual']:.2e} | {r['device_ms']:.1f} | {note} |",
+                print(f"| {cfg} | {arith} | {tol:g} | {drv} | {nwh} | {r['sweeps']} | {r['rel_residual']:.2e} | {r['device_ms']:.1f} | {note} |",
                       flush=True)
     elif which == "minres":
-        print("| mesh | p | sub side | DOF/sub | blocks | prec | MINRES iters (mean / max) | MINRES true res | MINRES ms | n_wh | "
-              "WaveHoltz ms, 1 DOF/thread | WaveHoltz ms, register-blocked | speedup same layout | speedup best |")
-        print("|" + "---|" * 14)
+        print("| mesh | p | sub side | DOF/sub | blocks | prec | MINRES iters (mean / max) | MINRES true res | MINRES ms, 1 DOF/thread | "
+              "MINRES ms, register-blocked | n_wh | WaveHoltz ms, 1 DOF/thread | WaveHoltz ms, register-blocked | "
+              "speedup, both 1 DOF/thread | speedup, both register-blocked | speedup best vs best |")
+        print("|" + "---|" * 16)
         for cfg, n, sides in ((5, 2048 // args.scale, (4, 8)), (3, 256, (4, 8, 10))):
             for s in sides:
                 inp = make_config(cfg, n=n - n % s, p=3, sub_elems=s)
                 for pr in ("f32", "f64"):
                     r = minres_vs_waveholtz(hz, torch, inp, pr, stream)
+                    mrb = r.get("minres_ms_register_blocked")
+                    best_m = min(r["minres_ms"], mrb) if mrb else r["minres_ms"]
+                    best_w = min(r["waveholtz_ms_one_dof_per_thread"], r["waveholtz_ms_register_blocked"])
                     print(f"| {inp.nx}x{inp.ny} | 3 | {s} | {r['dofs_per_sub']} | {r['blocks']} | {pr} | {r['minres_iters_mean']:.0f} / "
-                          f"{r['minres_iters_max']} | {r['minres_true_residual']:.1e} | {r['minres_ms']:.2f} | {r['n_wh']} | "
+                          f"{r['minres_iters_max']} | {r['minres_true_residual']:.1e} | {r['minres_ms']:.2f} | "
+                          f"{'%.2f' % mrb if mrb else 'n/a'} | {r['n_wh']} | "
                           f"{r['waveholtz_ms_one_dof_per_thread']:.2f} | {r['waveholtz_ms_register_blocked']:.2f} "
-                          f"({r['register_blocked_kernel']}) | {r['speedup_same_layout']:.1f}x | {r['speedup_best']:.1f}x |", flush=True)
+                          f"({r['register_blocked_kernel']}) | {r['speedup_same_layout']:.1f}x | "
+                          f"{'%.1fx' % r['speedup_same_layout_register_blocked'] if mrb else 'n/a'} | {best_m / best_w:.1f}x |", flush=True)
     elif which == "3d":
         from paper_2606_21695_b200 import hz3
         from paper_2606_21695_b200.inputs import make_config_3d
@@ -845,6 +874,17 @@ def run_tables(args):
                               f"{r.sweep_ms_total / 3 / op:.1f} |", flush=True)
                     finally:
                         hz3.hz3_destroy(c3)
+
+
+def _finite(o):
+    """JSON has no NaN / Infinity: a diverged or missing number is reported as null."""
+    if isinstance(o, float):
+        return o if o == o and abs(o) != float("inf") else None
+    if isinstance(o, dict):
+        return {k: _finite(v) for k, v in o.items()}
+    if isinstance(o, (list, tuple)):
+        return [_finite(v) for v in o]
+    return o
 
 
 def main():

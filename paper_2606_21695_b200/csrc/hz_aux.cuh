@@ -198,22 +198,32 @@ struct Ref1D {
 constexpr int kHelmBX = 32, kHelmBY = 8;
 inline size_t helm_smem(int P, size_t elem) { return 2 * (size_t)((kHelmBX + 1) * P + 1) * ((kHelmBY + 1) * P + 1) * elem; }
 
+// asynchronous global -> shared copy of one 4- or 8-byte element (cp.async, no register staging: the whole patch of a
+// block is in flight at once); pred = false writes zeros (src-size 0)
+template <int BYTES>
+__device__ __forceinline__ void cp_async_elem(void *dst_smem, const void *src, bool pred) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(dst_smem);
+  const int sz = pred ? BYTES : 0;
+  asm volatile("cp.async.ca.shared.global [%0], [%1], %2, %3;" ::"r"(d), "l"(src), "n"(BYTES), "r"(sz) : "memory");
+}
+
 // MODE 0: residual of (4): block partial sums of |b - (A - i w H - w^2 M) u|^2 and |b|^2 -> part (hz_residual)
 // MODE 1: operator evaluation y = (A - i w H - w^2 M) u written to y (re | im planes) -- the paper's "operator time"
 //         kernel, in the arithmetic `acc` of the DDM cycle it normalises
 // u: re | im planes of type inT.  k2: w^2 / c^2 per node in `acc` precision (MODE 1) or NULL (then c, fp64, is read).
-// The block stages the u patch ((32+1)P+1) x ((8+1)P+1) through shared memory with coalesced row loads; every thread
-// then applies the two 1-D element operators to its P x P nodes from shared memory (3P^2 + 2P reads per plane for P^2
-// nodes instead of 2(2P+1) P^2), compile-time P, coefficients in the constant bank.
+// The block stages the u patch ((32+1)P+1) x ((8+1)P+1) into shared memory with cp.async (element data staged
+// asynchronously, north_star (b): this is the one kernel of the path that streams per-element data from HBM); every
+// thread then applies the two 1-D element operators to its P x P nodes from shared memory (3P^2 + 2P reads per plane
+// for P^2 nodes instead of 2(2P+1) P^2), compile-time P, coefficients in the constant bank.
 template <typename inT, typename acc, int P, int MODE>
-__global__ void __launch_bounds__(kHelmBX *kHelmBY) k_helm(Geo g, Ref1D ref, const double *__restrict__ c,
-                                                            const acc *__restrict__ k2, const double *__restrict__ f_re,
-                                                            const double *__restrict__ f_im, const double *__restrict__ bc,
-                                                            const inT *__restrict__ u, double *__restrict__ part,
-                                                            acc *__restrict__ y) {
+__global__ void __launch_bounds__(kHelmBX *kHelmBY, 2) k_helm(Geo g, Ref1D ref, const double *__restrict__ c,
+                                                               const acc *__restrict__ k2, const double *__restrict__ f_re,
+                                                               const double *__restrict__ f_im, const double *__restrict__ bc,
+                                                               const inT *__restrict__ u, double *__restrict__ part,
+                                                               acc *__restrict__ y) {
   constexpr int PW = (kHelmBX + 1) * P + 1, PH = (kHelmBY + 1) * P + 1;
   extern __shared__ __align__(16) unsigned char helm_raw[];
-  acc *sr = reinterpret_cast<acc *>(helm_raw), *si = sr + PW * PH;
+  inT *sr = reinterpret_cast<inT *>(helm_raw), *si = sr + PW * PH;
   const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * kHelmBX + tx;
   const int ex = blockIdx.x * kHelmBX + tx, ey = blockIdx.y * kHelmBY + ty;
   const int I0 = blockIdx.x * kHelmBX * P - P, J0 = blockIdx.y * kHelmBY * P - P;  // patch origin
@@ -223,9 +233,10 @@ __global__ void __launch_bounds__(kHelmBX *kHelmBY) k_helm(Geo g, Ref1D ref, con
     const int I = I0 + px, J = J0 + py;
     const bool in = I >= 0 && I < g.npx && J >= 0 && J < g.npy;
     const size_t n = (size_t)(in ? J : 0) * g.npx + (in ? I : 0);
-    sr[q] = in ? (acc)u[n] : acc(0);
-    si[q] = in ? (acc)u[total + n] : acc(0);
+    cp_async_elem<sizeof(inT)>(sr + q, u + n, in);
+    cp_async_elem<sizeof(inT)>(si + q, u + total + n, in);
   }
+  asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
   __syncthreads();
   double r2 = 0.0, b2 = 0.0;
   if (ex <= g.nx && ey <= g.ny) {
@@ -242,40 +253,40 @@ __global__ void __launch_bounds__(kHelmBX *kHelmBY) k_helm(Geo g, Ref1D ref, con
       for (int a = 0; a < P; ++a) {
         if (a > 0 && !hasR) break;
         const acc wx = a == 0 ? (acc)((hasL ? ref.w[P] : 0.0) + (hasR ? ref.w[0] : 0.0)) : (acc)ref.w[a];
-        const acc *rr = sr + (by + b) * PW + bx, *ri = si + (by + b) * PW + bx;   // row of this node, at the tile's x origin
-        const acc *cr = sr + by * PW + bx + a, *ci = si + by * PW + bx + a;       // column of this node, at the tile's y origin
+        const inT *rr = sr + (by + b) * PW + bx, *ri = si + (by + b) * PW + bx;   // row of this node, at the tile's x origin
+        const inT *cr = sr + by * PW + bx + a, *ci = si + by * PW + bx + a;       // column of this node, at the tile's y origin
         acc kxr = 0, kxi = 0, kyr = 0, kyi = 0;
         if (a == 0) {   // node shared by the element on the left (its row P) and this one (row 0), where they exist
 #pragma unroll
           for (int cc = 0; cc <= P; ++cc) {
             const acc kl = hasL ? (acc)ref.K[P][cc] : acc(0), kr = hasR ? (acc)ref.K[0][cc] : acc(0);
-            kxr += kl * rr[cc - P] + kr * rr[cc];
-            kxi += kl * ri[cc - P] + kr * ri[cc];
+            kxr += kl * (acc)rr[cc - P] + kr * (acc)rr[cc];
+            kxi += kl * (acc)ri[cc - P] + kr * (acc)ri[cc];
           }
         } else {
 #pragma unroll
           for (int cc = 0; cc <= P; ++cc) {
-            kxr += (acc)ref.K[a][cc] * rr[cc];
-            kxi += (acc)ref.K[a][cc] * ri[cc];
+            kxr += (acc)ref.K[a][cc] * (acc)rr[cc];
+            kxi += (acc)ref.K[a][cc] * (acc)ri[cc];
           }
         }
         if (b == 0) {
 #pragma unroll
           for (int cc = 0; cc <= P; ++cc) {
             const acc kd = hasD ? (acc)ref.K[P][cc] : acc(0), ku = hasU ? (acc)ref.K[0][cc] : acc(0);
-            kyr += kd * cr[(cc - P) * PW] + ku * cr[cc * PW];
-            kyi += kd * ci[(cc - P) * PW] + ku * ci[cc * PW];
+            kyr += kd * (acc)cr[(cc - P) * PW] + ku * (acc)cr[cc * PW];
+            kyi += kd * (acc)ci[(cc - P) * PW] + ku * (acc)ci[cc * PW];
           }
         } else {
 #pragma unroll
           for (int cc = 0; cc <= P; ++cc) {
-            kyr += (acc)ref.K[b][cc] * cr[cc * PW];
-            kyi += (acc)ref.K[b][cc] * ci[cc * PW];
+            kyr += (acc)ref.K[b][cc] * (acc)cr[cc * PW];
+            kyi += (acc)ref.K[b][cc] * (acc)ci[cc * PW];
           }
         }
         const int I = ex * P + a, J = ey * P + b;
         const size_t n = (size_t)J * g.npx + I;
-        const acc u_r = rr[a], u_i = ri[a];
+        const acc u_r = (acc)rr[a], u_i = (acc)ri[a];
         const acc Aur = ax_ * wy * kxr + ay_ * wx * kyr, Aui = ax_ * wy * kxi + ay_ * wx * kyi;
         const acc m = mh * wx * wy;
         acc kk;   // w^2 / c^2

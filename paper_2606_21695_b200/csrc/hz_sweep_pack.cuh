@@ -15,8 +15,11 @@
 
 namespace hz {
 
+#ifndef HZ_PK_MINB
+#define HZ_PK_MINB 1
+#endif
 template <typename real, int P, int M, int MAXT>
-__global__ void __launch_bounds__(MAXT, 1) k_sweep_pack(const SweepArgs<real> A, const __grid_constant__ TabC<real> TC) {
+__global__ void __launch_bounds__(MAXT, HZ_PK_MINB) k_sweep_pack(const SweepArgs<real> A, const __grid_constant__ TabC<real> TC) {
   constexpr int T = M * P;
   constexpr int V16 = 16 / (int)sizeof(real);
   constexpr int CH = (T + V16 - 1) / V16 * V16;
