@@ -289,7 +289,7 @@ cudaError_t launch_helm(hz_ctx *ctx, const acc *k2, const void *u_dev, double *p
   }
   const Geo g = make_geo(ctx);
   const dim3 grid((ctx->nx + 1 + kHelmBX - 1) / kHelmBX, (ctx->ny + 1 + kHelmBY - 1) / kHelmBY), block(kHelmBX, kHelmBY);
-  const size_t sm = helm_smem(ctx->p, sizeof(inT));
+  const size_t sm = helm_smem(ctx->p, sizeof(inT), MODE == 1 ? sizeof(acc) : 0);
   void (*fn)(Geo, Ref1D, const double *, const acc *, const double *, const double *, const double *, const inT *, double *, acc *) = nullptr;
   switch (ctx->p) {
     case 1: fn = k_helm<inT, acc, 1, MODE>; break;

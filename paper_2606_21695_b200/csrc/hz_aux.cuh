@@ -196,7 +196,10 @@ struct Ref1D {
 // Launch shape of k_helm: a block of HB_X x HB_Y threads, one thread per ELEMENT (its P x P lower-left nodes, as in the
 // sweep kernels; the phantom elements nx / ny own the last node column / row), and its shared-memory patch.
 constexpr int kHelmBX = 32, kHelmBY = 8;
-inline size_t helm_smem(int P, size_t elem) { return 2 * (size_t)((kHelmBX + 1) * P + 1) * ((kHelmBY + 1) * P + 1) * elem; }
+// shared memory: the u patch (re, im) of the input type; MODE 1 adds the w^2/c^2 values of the block's own nodes
+inline size_t helm_smem(int P, size_t elem_in, size_t elem_k2) {
+  return 2 * (size_t)((kHelmBX + 1) * P + 1) * ((kHelmBY + 1) * P + 1) * elem_in + (size_t)kHelmBX * P * kHelmBY * P * elem_k2;
+}
 
 // asynchronous global -> shared copy of one 4- or 8-byte element (cp.async, no register staging: the whole patch of a
 // block is in flight at once); pred = false writes zeros (src-size 0)
@@ -222,8 +225,10 @@ __global__ void __launch_bounds__(kHelmBX *kHelmBY, 2) k_helm(Geo g, Ref1D ref, 
                                                                const inT *__restrict__ u, double *__restrict__ part,
                                                                acc *__restrict__ y) {
   constexpr int PW = (kHelmBX + 1) * P + 1, PH = (kHelmBY + 1) * P + 1;
+  constexpr int OW = kHelmBX * P, OH = kHelmBY * P;   // the block's own nodes (patch coordinates [P, P+OW) x [P, P+OH))
   extern __shared__ __align__(16) unsigned char helm_raw[];
   inT *sr = reinterpret_cast<inT *>(helm_raw), *si = sr + PW * PH;
+  acc *sk = reinterpret_cast<acc *>(si + PW * PH);    // MODE 1: w^2/c^2 of the own nodes, staged like the patch
   const int tx = threadIdx.x, ty = threadIdx.y, tid = ty * kHelmBX + tx;
   const int ex = blockIdx.x * kHelmBX + tx, ey = blockIdx.y * kHelmBY + ty;
   const int I0 = blockIdx.x * kHelmBX * P - P, J0 = blockIdx.y * kHelmBY * P - P;  // patch origin
@@ -236,9 +241,23 @@ __global__ void __launch_bounds__(kHelmBX *kHelmBY, 2) k_helm(Geo g, Ref1D ref, 
     cp_async_elem<sizeof(inT)>(sr + q, u + n, in);
     cp_async_elem<sizeof(inT)>(si + q, u + total + n, in);
   }
+  if (MODE == 1) {
+    for (int q = tid; q < OW * OH; q += kHelmBX * kHelmBY) {
+      const int I = I0 + P + q % OW, J = J0 + P + q / OW;
+      const bool in = I < g.npx && J < g.npy;
+      cp_async_elem<sizeof(acc)>(sk + q, k2 + (in ? (size_t)J * g.npx + I : 0), in);
+    }
+  }
   asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
   __syncthreads();
   double r2 = 0.0, b2 = 0.0;
+  acc outr[MODE == 1 ? P : 1][MODE == 1 ? P : 1], outi[MODE == 1 ? P : 1][MODE == 1 ? P : 1];
+  if (MODE == 1) {
+#pragma unroll
+    for (int b = 0; b < P; ++b)
+#pragma unroll
+      for (int a = 0; a < P; ++a) outr[b][a] = outi[b][a] = acc(0);
+  }
   if (ex <= g.nx && ey <= g.ny) {
     const bool hasL = ex > 0, hasR = ex < g.nx, hasD = ey > 0, hasU = ey < g.ny;
     const acc ax_ = (acc)(g.hy / g.hx), ay_ = (acc)(g.hx / g.hy);
@@ -291,14 +310,14 @@ __global__ void __launch_bounds__(kHelmBX *kHelmBY, 2) k_helm(Geo g, Ref1D ref, 
         const acc m = mh * wx * wy;
         acc kk;   // w^2 / c^2
         double cj = 0.0;
-        if (k2) kk = k2[n];
+        if (MODE == 1) kk = sk[(ty * P + b) * OW + tx * P + a];
         else { cj = c[n]; kk = (acc)(g.omega * g.omega / (cj * cj)); }
         const bool onb = I == 0 || I == g.npx - 1 || J == 0 || J == g.npy - 1;
         acc wH = 0;
         double bre = 0.0, bim = 0.0;
         if (MODE == 0) { bre = f_re[n] * (double)m; bim = f_im ? f_im[n] * (double)m : 0.0; }
         if (onb) {   // impedance term and datum of eq. (1b) on the outer boundary only
-          if (k2) cj = c[n];
+          if (MODE == 1) cj = c[n];
           const double sWE = 0.5 * g.hy * (double)wy, sSN = 0.5 * g.hx * (double)wx;
           double H = 0.0;
           if (I == 0) { H += sWE / cj; if (MODE == 0 && bc) { bre += sWE * bc[(0 * 2 + 0) * g.EB + J]; bim += sWE * bc[(0 * 2 + 1) * g.EB + J]; } }
@@ -310,14 +329,35 @@ __global__ void __launch_bounds__(kHelmBX *kHelmBY, 2) k_helm(Geo g, Ref1D ref, 
         // (A - i w H - w^2 M) u = (A u_r - w2M u_r + wH u_i) + i (A u_i - w2M u_i - wH u_r)
         const acc w2M = kk * m;
         const acc yr = Aur - w2M * u_r + wH * u_i, yi = Aui - w2M * u_i - wH * u_r;
-        if (MODE == 1) {
-          y[n] = yr;
-          y[total + n] = yi;
+        if (MODE == 1) {   // kept in registers until every thread has read the patch, then staged for coalesced stores
+          outr[b][a] = yr;
+          outi[b][a] = yi;
         } else {
           const double rr_ = bre - (double)yr, ri_ = bim - (double)yi;
           r2 += rr_ * rr_ + ri_ * ri_;
           b2 += bre * bre + bim * bim;
         }
+      }
+    }
+  }
+  if (MODE == 1) {
+    // y of the own nodes goes through shared memory (the patch is dead now) so that the global stores are whole rows
+    acc *yo_r = reinterpret_cast<acc *>(helm_raw), *yo_i = yo_r + OW * OH;
+    __syncthreads();
+#pragma unroll
+    for (int b = 0; b < P; ++b)
+#pragma unroll
+      for (int a = 0; a < P; ++a) {
+        yo_r[(ty * P + b) * OW + tx * P + a] = outr[b][a];
+        yo_i[(ty * P + b) * OW + tx * P + a] = outi[b][a];
+      }
+    __syncthreads();
+    for (int q = tid; q < OW * OH; q += kHelmBX * kHelmBY) {
+      const int I = I0 + P + q % OW, J = J0 + P + q / OW;
+      if (I < g.npx && J < g.npy) {
+        const size_t n = (size_t)J * g.npx + I;
+        y[n] = yo_r[q];
+        y[total + n] = yo_i[q];
       }
     }
   }
