@@ -261,17 +261,7 @@ def peak_tflops(prec_name, sm_mhz=SM_MHZ):
 
 
 def kernel_name(pinfo, quads=False):
-    if quads:
-        return "k_sweep_quad"
-    if getattr(pinfo, "subs_per_block", 1) > 1:
-        return "k_sweep_pack"
-    if pinfo.cluster_size > 1:
-        return "k_sweep_cl"
-    if pinfo.dofs_per_thread == 1:
-        return "k_sweep_dof"
-    if pinfo.dofs_per_thread == -1:
-        return "k_sweep_stream"
-    return "k_sweep_ws" if pinfo.tile_mx == pinfo.tile_my else "k_sweep_tile"
+    return pinfo.kernel.decode()
 
 
 def fma_probe(kind, stream):

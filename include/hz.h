@@ -104,6 +104,7 @@ typedef struct {
   double dt, theta, sigma; /* dt = T/n_t; theta = tan(w dt/2)/w; sigma = 2 sin(w dt/2)/w */
   size_t smem_bytes;       /* dynamic shared memory per block */
   size_t workspace_bytes;  /* device bytes the context allocated for this partition */
+  char kernel[24];         /* name of the sweep kernel the partition launches, e.g. "k_sweep_ws" (NUL-terminated) */
 } hz_part_info;
 
 /* ---------------------------------------------------------------------------------------------

@@ -810,6 +810,12 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
     inf.subs_per_block = ctx->lay.variant == 1 ? ctx->pack : 1;
     inf.dt = ctx->dt; inf.theta = ctx->theta; inf.sigma = ctx->sigma;
     inf.smem_bytes = ctx->launch.smem; inf.workspace_bytes = ws;
+    const char *kn = "k_sweep_dof";
+    if (ctx->lay.variant == 3) kn = "k_sweep_quad";
+    else if (ctx->lay.variant == 2) kn = "k_sweep_stream";
+    else if (ctx->lay.variant == 1)
+      kn = ctx->pack > 1 ? "k_sweep_pack" : (ctx->cl > 1 ? (ctx->ws ? "k_sweep_cw" : "k_sweep_cl") : (ctx->ws ? "k_sweep_ws" : "k_sweep_tile"));
+    std::snprintf(inf.kernel, sizeof(inf.kernel), "%s", kn);
     *info_out = inf;
   }
   return HZ_OK;

@@ -31,7 +31,7 @@ class hz_part_info(C.Structure):
                 ("edge_stride", C.c_int), ("threads_per_block", C.c_int), ("blocks", C.c_int),
                 ("dofs_per_thread", C.c_int), ("tile_mx", C.c_int), ("tile_my", C.c_int), ("cluster_size", C.c_int),
                 ("subs_per_block", C.c_int), ("dt", C.c_double), ("theta", C.c_double), ("sigma", C.c_double),
-                ("smem_bytes", C.c_size_t), ("workspace_bytes", C.c_size_t)]
+                ("smem_bytes", C.c_size_t), ("workspace_bytes", C.c_size_t), ("kernel", C.c_char * 24)]
 
 
 class hz_part_flags(C.Structure):
