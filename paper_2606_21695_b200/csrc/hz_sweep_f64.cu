@@ -25,6 +25,8 @@ namespace hz {
   W(3, 1, 0, 128, 1)       \
   W(3, 1, 0, 320, 1)       \
   W(3, 1, 1, 512, 1)       \
+  W(4, 1, 1, 128, 1)       \
+  W(4, 1, 0, 128, 1)       \
   W(4, 1, 1, 320, 1)
 
 // C(P, MX, MY, CL, MAXT, MINB): cluster of CL CTAs per subdomain, coefficients in registers
@@ -57,6 +59,7 @@ namespace hz {
 // CW(P, MX, MY, CL, MAXT, MINB): cluster of CL CTAs per subdomain, warp-specialised edge pieces (hz_sweep_cw.cuh)
 #define HZ_CW_TABLE_F64(CW) \
   CW(3, 1, 1, 4, 320, 1)   \
+  CW(1, 4, 4, 2, 192, 1)   \
   CW(3, 1, 1, 16, 352, 1)  \
   CW(2, 1, 1, 8, 608, 1)   \
   CW(4, 1, 1, 8, 192, 1)
