@@ -571,6 +571,10 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
       const int NB = (q.ntx - 1) * (q.nty - 1), NE = q.ntx + q.nty - 1;
       if (n_t > kTabCMax) return false;
       if (NB > 16 || fl.pack == 1) return false;   // packing only pays below one warp of full tiles
+      // own part of a step before (pk = 2) or after (pk = 1) the block barrier: measured per shape on config 5
+      // (hz_sweep_pack.cuh, profiles/r02_config_sweep.md)
+      const bool pre = NB < 16 || t.mx == 1 || (rs == 8 && P == 1);
+      if ((t.pk == 2) != pre) return false;
       auto gcd = [](int a, int b) { while (b) { const int r = a % b; a = b; b = r; } return a; };
       const size_t v16 = 16 / rs;
       const size_t chx = ((size_t)q.TX + v16 - 1) / v16 * v16, chy = ((size_t)q.TY + v16 - 1) / v16 * v16;

@@ -99,7 +99,8 @@ struct TileEntry {
   int minb;                  // __launch_bounds__ min blocks per SM (register cap = 64K / (minb * maxt))
   int cl;                    // > 1: thread-block-cluster kernel (hz_sweep_cl.cuh), CTAs per subdomain
   const void *fn;
-  int pk;                    // 1: packed small-subdomain kernel (hz_sweep_pack.cuh), several subdomains per block
+  int pk;                    // > 0: packed small-subdomain kernel (hz_sweep_pack.cuh), several subdomains per block;
+                             // 2: its PRE instantiation (own part of a step before the block barrier)
 };
 
 struct SweepLaunch {

@@ -17,7 +17,11 @@ namespace hz {
 
 // (a register cap for two blocks of 256 threads per SM gains 5-10 % on the 4-tile subdomains and loses 10-45 % on the
 // 16-tile ones and in fp64: not used)
-template <typename real, int P, int M, int MAXT>
+// PRE: the neighbour-independent part of a step (own-tile line sums, the cos-filter sum of Re u) runs BEFORE the block
+// barrier, as in k_sweep_cw, so the wait overlaps arithmetic: faster where a subdomain has fewer than 16 full tiles
+// (one or two bulk warps per block), at M = 1 and in fp64 at p = 1; slower for the 16-tile M > 1 shapes, which keep
+// the order of k_sweep_ws (profiles/r02_config_sweep.md).  Same sums, same association: results are bit-identical.
+template <typename real, int P, int M, int MAXT, bool PRE>
 __global__ void __launch_bounds__(MAXT, 1) k_sweep_pack(const SweepArgs<real> A, const __grid_constant__ TabC<real> TC) {
   constexpr int T = M * P;
   constexpr int V16 = 16 / (int)sizeof(real);
@@ -153,15 +157,16 @@ __global__ void __launch_bounds__(MAXT, 1) k_sweep_pack(const SweepArgs<real> A,
           st_chunk<T>(my + 2 * CH, oPY);
           st_chunk<T>(my + 3 * CH, oRY);
         }
-        bar_sync_all(NTH);
-        real qR[T], piL[T], qU[T], piD[T];
-        ld_chunk<T>(pL + cur, piL);
-        ld_chunk<T>(pR + cur + CH, qR);
-        ld_chunk<T>(pD + cur + 2 * CH, piD);
-        ld_chunk<T>(pU + cur + 3 * CH, qU);
-        cur = BUFW - cur;
         const Tab4<real> tn = TC.t[nu];
         real S[T][T], X0[T], Y0[T];
+        real qR[T], piL[T], qU[T], piD[T];
+        if (!PRE) {
+          bar_sync_all(NTH);
+          ld_chunk<T>(pL + cur, piL);
+          ld_chunk<T>(pR + cur + CH, qR);
+          ld_chunk<T>(pD + cur + 2 * CH, piD);
+          ld_chunk<T>(pU + cur + 3 * CH, qU);
+        }
 #pragma unroll
         for (int b = 0; b < T; ++b) {
           real q[T + 1];
@@ -185,6 +190,14 @@ __global__ void __launch_bounds__(MAXT, 1) k_sweep_pack(const SweepArgs<real> A,
         for (int b = 0; b < T; ++b)
 #pragma unroll
           for (int a = 0; a < T; ++a) vr[b][a] = fmaT(tn.k, p[b][a], vr[b][a]);
+        if (PRE) {
+          bar_sync_all(NTH);
+          ld_chunk<T>(pL + cur, piL);
+          ld_chunk<T>(pR + cur + CH, qR);
+          ld_chunk<T>(pD + cur + 2 * CH, piD);
+          ld_chunk<T>(pU + cur + 3 * CH, qU);
+        }
+        cur = BUFW - cur;
 #pragma unroll
         for (int b = 0; b < T; ++b) {
           if (b == 0) line_finish<real, P, M, false>(qR[b], piL[b], s0x, X0[b], A.ex1, S[b]);
