@@ -328,6 +328,34 @@ hz_status hz_minres_cycle(hz_ctx *ctx, const hz_minres_opts *opts, int *iters_ou
  * accumulated in fp64.  u_dev: DEVICE, layout as u_out, of precision u_prec.  Synchronises `stream`. */
 hz_status hz_residual(hz_ctx *ctx, const void *u_dev, hz_prec u_prec, double *rel_residual, void *stream);
 
+/* ---------------------------------------------------------------------------------------------
+ * hz_residual_static — hz_residual for callers that cannot allocate (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): the same kernels (k_helm / k_residual_quad block partial sums, fp64
+ * reduction), but the partial sums live in a file-scope `static __device__` array of the library
+ * instead of the context's lazily allocated buffers, the result stays on the DEVICE, and the call neither allocates,
+ * frees, copies to the host nor synchronises: it only enqueues work on `stream`.
+ *
+ *   ctx               a context of hz_mesh_setup / hz_mesh_setup_quads (its device arrays c, f, bc are the inputs);
+ *                     hz_partition is not needed.  The context's device must be current.
+ *   u_dev             DEVICE, layout as u_out (re plane then im plane), of precision u_prec.
+ *   rel_residual_dev  DEVICE, 1 double, owned by the caller: receives ||b - (A - i w H - w^2 M) u|| / ||b||
+ *                     (bit-identical to hz_residual) once the work enqueued on `stream` has run.
+ * Limit: the mesh may need at most HZ_RESIDUAL_STATIC_MAX_BLOCKS partial-sum blocks (uniform meshes: one per patch
+ * of 32 x 8 elements, ceil((nx+1)/32) * ceil((ny+1)/8); general quads: one per 256 nodes), i.e. 4 MiB + 256 bytes of
+ * device memory, which EVERY GPU that loads the library holds until the process exits.  That covers all BASELINE.json
+ * configs (config 5 at p = 1: 148 417 blocks).  Larger meshes: HZ_EINVAL with a message (use hz_residual).
+ * The array is shared by all contexts and calls of the process on one device and keeps the last call's contents
+ * (the slots a call reads are cleared first, on `stream`): calls that overlap on the GPU (different streams, or
+ * several host threads without stream ordering) RACE on it; calls ordered on one stream are safe, as are different devices.
+ * hz_residual_static_setup resolves the array's device address for the CURRENT device (cudaGetSymbolAddress; cached per
+ * device).  Call it once per device at set-up, e.g. before stream capture begins; hz_residual_static does the same
+ * on first use otherwise.  Errors: HZ_ECUDA with the CUDA message.
+ * ------------------------------------------------------------------------------------------- */
+#define HZ_RESIDUAL_STATIC_MAX_BLOCKS 262144
+int hz_residual_static_max_blocks(void);
+hz_status hz_residual_static_setup(hz_ctx *ctx);
+hz_status hz_residual_static(hz_ctx *ctx, const void *u_dev, hz_prec u_prec, double *rel_residual_dev, void *stream);
+
 /* Raw state for parity tests.  u_sub_dev: DEVICE or NULL, doubles [blocks][2][dofs_per_sub]
  * (re then im, local node (I,J) at J*edge_nodes_x+I).  lambda_dev: DEVICE or NULL, doubles
  * [blocks][4][2][edge_stride] (current lambda^n; zeros on physical sides). */

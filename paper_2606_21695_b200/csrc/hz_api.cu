@@ -5,6 +5,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -1489,6 +1490,95 @@ hz_status hz_residual(hz_ctx *ctx, const void *u_dev, hz_prec u_prec, double *re
   hz_status st = residual_impl(ctx, u_dev, u_prec, &rel, (cudaStream_t)stream);
   if (st != HZ_OK) return st;
   *rel_residual = rel;
+  return HZ_OK;
+}
+
+}  // extern "C"
+
+// ---------------------------------------------------------------------------------------------
+// hz_residual_static: hz_residual without any allocation (include/hz.h).  The block partial sums of k_helm /
+// k_residual_quad and the reduced pair live in a file-scope device array instead of the context's lazily
+// cudaMalloc'ed buffers.  In HOST code `g_res_static` is only the symbol's host-side stand-in, not a device address:
+// the address the kernels get is resolved once per device with cudaGetSymbolAddress (that device current).
+// ---------------------------------------------------------------------------------------------
+static __device__ __align__(256) double g_res_static[2 * (size_t)HZ_RESIDUAL_STATIC_MAX_BLOCKS + 32];
+constexpr int kStaticMaxDevices = 64;
+static double *g_res_static_ptr[kStaticMaxDevices] = {};
+static std::mutex g_res_static_mu;
+
+// device address of g_res_static on the CURRENT device (resolved on first use, then cached)
+static cudaError_t res_static_address(double **out) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kStaticMaxDevices) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lk(g_res_static_mu);
+  if (!g_res_static_ptr[dev]) {
+    void *q = nullptr;
+    e = cudaGetSymbolAddress(&q, g_res_static);
+    if (e != cudaSuccess) return e;
+    if (!q) return cudaErrorInvalidSymbol;
+    g_res_static_ptr[dev] = static_cast<double *>(q);
+  }
+  *out = g_res_static_ptr[dev];
+  return cudaSuccess;
+}
+
+// rel = sqrt(|r|^2 / |b|^2) (|b| = 0: sqrt(|r|^2)), the last step of residual_impl, on the device
+static __global__ void k_rel_from_sums(const double *__restrict__ red, double *__restrict__ out) {
+  if (threadIdx.x == 0 && blockIdx.x == 0) out[0] = red[1] > 0.0 ? sqrt(red[0] / red[1]) : sqrt(red[0]);
+}
+
+extern "C" {
+
+int hz_residual_static_max_blocks(void) { return HZ_RESIDUAL_STATIC_MAX_BLOCKS; }
+
+hz_status hz_residual_static_setup(hz_ctx *ctx) {
+  if (!ctx) return HZ_EINVAL;
+  double *scratch = nullptr;
+  HZ_CUDA(res_static_address(&scratch));
+  return HZ_OK;
+}
+
+hz_status hz_residual_static(hz_ctx *ctx, const void *u_dev, hz_prec u_prec, double *rel_residual_dev, void *stream) {
+  if (!ctx) return HZ_EINVAL;
+  if (!u_dev || !rel_residual_dev) return fail(ctx, HZ_EINVAL, "hz_residual_static: NULL u_dev or rel_residual_dev");
+  if (u_prec != HZ_F32 && u_prec != HZ_F64) return fail(ctx, HZ_EINVAL, "hz_residual_static: bad precision");
+  cudaStream_t st = (cudaStream_t)stream;
+  const long long total = (long long)ctx->npx * ctx->npy;
+  const int bs = 256;
+  const long long nb = ctx->general ? (total + bs - 1) / bs
+                                    : (long long)((ctx->nx + 1 + kHelmBX - 1) / kHelmBX) * ((ctx->ny + 1 + kHelmBY - 1) / kHelmBY);
+  if (nb > HZ_RESIDUAL_STATIC_MAX_BLOCKS) {
+    char msg[192];
+    std::snprintf(msg, sizeof(msg), "hz_residual_static: the mesh needs %lld partial-sum blocks, the static scratch holds %d "
+                  "(HZ_RESIDUAL_STATIC_MAX_BLOCKS); use hz_residual", nb, HZ_RESIDUAL_STATIC_MAX_BLOCKS);
+    return fail(ctx, HZ_EINVAL, msg);
+  }
+  double *part = nullptr;
+  HZ_CUDA(res_static_address(&part));
+  double *red = part + 2 * (size_t)HZ_RESIDUAL_STATIC_MAX_BLOCKS;
+  // the array keeps the previous call's contents: the slots this call reads start at zero
+  HZ_CUDA(cudaMemsetAsync(part, 0, (size_t)2 * nb * sizeof(double), st));
+  HZ_CUDA(cudaMemsetAsync(red, 0, 2 * sizeof(double), st));
+  if (ctx->general) {
+    Geo g = make_geo(ctx);
+    if (u_prec == HZ_F32)
+      k_residual_quad<float><<<(unsigned)nb, bs, 0, st>>>(g, ctx->refq, ctx->d_vx, ctx->d_vy, ctx->d_c, ctx->d_fre, ctx->d_fim,
+                                                          ctx->d_bc, (const float *)u_dev, part);
+    else
+      k_residual_quad<double><<<(unsigned)nb, bs, 0, st>>>(g, ctx->refq, ctx->d_vx, ctx->d_vy, ctx->d_c, ctx->d_fre, ctx->d_fim,
+                                                           ctx->d_bc, (const double *)u_dev, part);
+    HZ_CUDA(cudaGetLastError());
+  } else if (u_prec == HZ_F32) {
+    HZ_CUDA((launch_helm<float, double, 0>(ctx, nullptr, u_dev, part, nullptr, st)));
+  } else {
+    HZ_CUDA((launch_helm<double, double, 0>(ctx, nullptr, u_dev, part, nullptr, st)));
+  }
+  k_reduce2<<<1, 1024, 0, st>>>(part, (int)nb, red);
+  HZ_CUDA(cudaGetLastError());
+  k_rel_from_sums<<<1, 32, 0, st>>>(red, rel_residual_dev);
+  HZ_CUDA(cudaGetLastError());
   return HZ_OK;
 }
 

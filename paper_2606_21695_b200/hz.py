@@ -23,7 +23,8 @@ STATUS_NAMES = {0: "HZ_OK", 1: "HZ_EINVAL", 2: "HZ_ENOMEM", 3: "HZ_ECUDA", 4: "H
 # every symbol include/hz.h declares
 EXPORTS = ("hz_mesh_setup", "hz_mesh_setup_quads", "hz_set_source", "hz_partition", "hz_partition_ex", "hz_ddm_solve",
            "hz_operator_time", "hz_ddm_solve_sources", "hz_ddm_solve_gmres", "hz_ddm_solve_mixed", "hz_minres_cycle",
-           "hz_residual", "hz_get_subdomain_state", "hz_set_subdomain_state", "hz_last_error", "hz_destroy")
+           "hz_residual", "hz_residual_static_max_blocks", "hz_residual_static_setup", "hz_residual_static",
+           "hz_get_subdomain_state", "hz_set_subdomain_state", "hz_last_error", "hz_destroy")
 
 
 class hz_part_info(C.Structure):
@@ -118,6 +119,10 @@ def lib():
     L.hz_ddm_solve_gmres.argtypes = [vp, C.POINTER(hz_gmres_opts), vp, C.POINTER(hz_gmres_info), vp]
     L.hz_minres_cycle.argtypes = [vp, C.POINTER(hz_minres_opts), vp, vp, C.POINTER(hz_minres_info), vp]
     L.hz_residual.argtypes = [vp, vp, ip, dp, vp]
+    L.hz_residual_static_max_blocks.argtypes = []
+    L.hz_residual_static_max_blocks.restype = C.c_int
+    L.hz_residual_static_setup.argtypes = [vp]
+    L.hz_residual_static.argtypes = [vp, vp, ip, vp, vp]
     L.hz_get_subdomain_state.argtypes = [vp, vp, vp, vp]
     L.hz_set_subdomain_state.argtypes = [vp, vp, vp, vp]
     L.hz_last_error.argtypes = [vp]
@@ -277,6 +282,16 @@ def hz_residual(ctx, u_ptr, u_prec, stream=None):
     r = C.c_double()
     _check(ctx, lib().hz_residual(ctx, C.c_void_p(u_ptr), u_prec, C.byref(r), C.c_void_p(stream) if stream else None))
     return r.value
+
+
+def hz_residual_static_setup(ctx):
+    _check(ctx, lib().hz_residual_static_setup(ctx))
+
+
+def hz_residual_static(ctx, u_ptr, u_prec, rel_ptr, stream=None):
+    """No allocation, no host copy, no synchronisation: the relative residual lands in the device double at rel_ptr."""
+    _check(ctx, lib().hz_residual_static(ctx, C.c_void_p(u_ptr), u_prec, C.c_void_p(rel_ptr),
+                                         C.c_void_p(stream) if stream else None))
 
 
 def hz_get_subdomain_state(ctx, u_sub_ptr=None, lambda_ptr=None, stream=None):
