@@ -283,25 +283,62 @@ cudaError_t launch_gather(const hz_ctx *c, void *out, int prec_out, cudaStream_t
 // launches k_helm<inT, acc, P, MODE> on the whole mesh (hz_aux.cuh)
 template <typename inT, typename acc, int MODE>
 cudaError_t launch_helm(hz_ctx *ctx, const acc *k2, const void *u_dev, double *part, acc *y, cudaStream_t st) {
-  Ref1D ref{};
-  for (int a = 0; a <= ctx->p; ++a) {
-    ref.w[a] = ctx->gll.w[a];
-    for (int b = 0; b <= ctx->p; ++b) ref.K[a][b] = ctx->gll.K[a][b];
+  HelmC<acc> hc{};
+  const int P_ = ctx->p;
+  for (int a = 0; a <= P_; ++a) {
+    hc.w[a] = (acc)ctx->gll.w[a];
+    hc.wa[a] = (acc)(a == 0 ? ctx->gll.w[0] + ctx->gll.w[P_] : ctx->gll.w[a]);
+    for (int b = 0; b <= P_; ++b) {
+      hc.kx[a][b] = (acc)(ctx->hy / ctx->hx * ctx->gll.K[a][b]);
+      hc.ky[a][b] = (acc)(ctx->hx / ctx->hy * ctx->gll.K[a][b]);
+    }
   }
+  hc.mh = (acc)(0.25 * ctx->hx * ctx->hy);
+  for (int cc = -P_; cc <= P_; ++cc) {   // assembled row of a node shared by two elements
+    const double kl = cc <= 0 ? ctx->gll.K[P_][cc + P_] : 0.0, kr = cc >= 0 ? ctx->gll.K[0][cc] : 0.0;
+    hc.kx0[cc + P_] = (acc)(ctx->hy / ctx->hx * (kl + kr));
+    hc.ky0[cc + P_] = (acc)(ctx->hx / ctx->hy * (kl + kr));
+  }
+  for (int b = 0; b < P_; ++b)
+    for (int a = 0; a < P_; ++a) {
+      const double wa_ = a == 0 ? ctx->gll.w[0] + ctx->gll.w[P_] : ctx->gll.w[a], wb_ = b == 0 ? ctx->gll.w[0] + ctx->gll.w[P_] : ctx->gll.w[b];
+      hc.wm[b][a] = (acc)(0.25 * ctx->hx * ctx->hy * wa_ * wb_);
+    }
   const Geo g = make_geo(ctx);
-  const dim3 grid((ctx->nx + 1 + kHelmBX - 1) / kHelmBX, (ctx->ny + 1 + kHelmBY - 1) / kHelmBY), block(kHelmBX, kHelmBY);
+  const HelmGrid hg = helm_grid(ctx->nx, ctx->ny, ctx->p);
+  const dim3 block(kHelmBX, kHelmBY);
   const size_t sm = helm_smem(ctx->p, sizeof(inT), MODE == 1 ? sizeof(acc) : 0);
-  void (*fn)(Geo, Ref1D, const double *, const acc *, const double *, const double *, const double *, const inT *, double *, acc *) = nullptr;
+  using fe_t = void (*)(Geo, const HelmGrid, const HelmC<acc>, const double *, const acc *, const double *, const double *,
+                        const double *, const inT *, double *, acc *);
+  using ft_t = void (*)(Geo, const HelmGrid, const HelmC<acc>, const double *, const acc *, const double *, const double *,
+                        const inT *, double *, acc *);
+  fe_t fi = nullptr;   // patches strictly inside the mesh, cp.async staging
+  ft_t ft = nullptr;   // the same with TMA bulk-copy staging: the fp64 operator at P >= 3 (hz_aux.cuh)
+  fe_t fe = nullptr;   // the ring of patches that touch the mesh boundary
+  constexpr bool kTma = MODE == 1 && sizeof(inT) == 8;
   switch (ctx->p) {
-    case 1: fn = k_helm<inT, acc, 1, MODE>; break;
-    case 2: fn = k_helm<inT, acc, 2, MODE>; break;
-    case 3: fn = k_helm<inT, acc, 3, MODE>; break;
-    case 4: fn = k_helm<inT, acc, 4, MODE>; break;
+    case 1: fi = k_helm<inT, acc, 1, MODE, false>; fe = k_helm<inT, acc, 1, MODE, true>; break;
+    case 2: fi = k_helm<inT, acc, 2, MODE, false>; fe = k_helm<inT, acc, 2, MODE, true>; break;
+    case 3: fi = k_helm<inT, acc, 3, MODE, false>; fe = k_helm<inT, acc, 3, MODE, true>; if constexpr (kTma) ft = k_helm_tma<inT, acc, 3, 1>; break;
+    case 4: fi = k_helm<inT, acc, 4, MODE, false>; fe = k_helm<inT, acc, 4, MODE, true>; if constexpr (kTma) ft = k_helm_tma<inT, acc, 4, 1>; break;
     default: return cudaErrorInvalidValue;
   }
-  cudaError_t e = cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+  const size_t smt = helm_tma_smem(ctx->p, sizeof(inT), sizeof(acc));
+  cudaError_t e = cudaFuncSetAttribute(fi, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
   if (e != cudaSuccess) return e;
-  fn<<<grid, block, sm, st>>>(g, ref, ctx->d_c, k2, ctx->d_fre, ctx->d_fim, ctx->d_bc, (const inT *)u_dev, part, y);
+  e = cudaFuncSetAttribute(fe, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+  if (e != cudaSuccess) return e;
+  if (ft) {
+    e = cudaFuncSetAttribute(ft, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smt);
+    if (e != cudaSuccess) return e;
+  }
+  const int nix = hg.bxh - 1, niy = hg.byh - 1, nring = hg.gx * hg.gy - nix * niy;
+  if (nix > 0 && niy > 0) {
+    if (ft) ft<<<dim3(nix, niy), block, smt, st>>>(g, hg, hc, ctx->d_c, k2, ctx->d_fre, ctx->d_fim, (const inT *)u_dev, part, y);
+    else fi<<<dim3(nix, niy), block, sm, st>>>(g, hg, hc, ctx->d_c, k2, ctx->d_fre, ctx->d_fim, ctx->d_bc, (const inT *)u_dev, part, y);
+  }
+  if (nring > 0)
+    fe<<<dim3(nring), block, sm, st>>>(g, hg, hc, ctx->d_c, k2, ctx->d_fre, ctx->d_fim, ctx->d_bc, (const inT *)u_dev, part, y);
   return cudaGetLastError();
 }
 
