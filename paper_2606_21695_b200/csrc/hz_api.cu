@@ -69,6 +69,8 @@ struct hz_ctx {
   void *d_bbf_zero = nullptr;  // all-zero load of the homogeneous sweep (hz_ddm_solve_mixed), allocated on first use
   void *d_mix = nullptr;       // hz_ddm_solve_mixed: hi context: X_old (n_state doubles); lo context: D (n_state floats)
   double *d_wxl = nullptr, *d_wyl = nullptr;
+  int *d_sxp = nullptr, *d_syp = nullptr;           // x / y part of Layout::slot per local node column / row (k_build)
+  GatherLine *d_gcol = nullptr, *d_grow = nullptr;  // k_gather's line tables (per global node column / row)
   double *d_part = nullptr, *d_red = nullptr, *d_ures = nullptr;
   void *d_opk2 = nullptr, *d_opy = nullptr;  // hz_operator_time: w^2/c^2 and the output vector, in precision op_prec
   int op_prec = -1;
@@ -128,7 +130,7 @@ void free_partition(hz_ctx *c) {
   if (c->d_G) { cudaFree(c->d_G); c->d_G = nullptr; }
   void **ptrs[] = {&c->d_tab, &c->d_gamma, &c->d_alpha, &c->d_bbf_re, &c->d_bbf_im, &c->d_lam, &c->d_bbf_zero, &c->d_mix,
                    &c->d_g, &c->d_k2, &c->d_bs, &c->d_bandx, &c->d_bandy, &c->d_scr, (void **)&c->d_wxl, (void **)&c->d_wyl,
-                   (void **)&c->d_part, (void **)&c->d_red, (void **)&c->d_ures};
+                   (void **)&c->d_part, (void **)&c->d_red, (void **)&c->d_ures, (void **)&c->d_gcol, (void **)&c->d_grow, (void **)&c->d_sxp, (void **)&c->d_syp};
   for (void **q : ptrs) { if (*q) cudaFree(*q); *q = nullptr; }
   c->part = false;
   c->ws_bytes = 0;
@@ -166,7 +168,10 @@ hz_status run_build(hz_ctx *ctx, int only_source, cudaStream_t st, const double 
     }
     return HZ_OK;
   }
-  k_build<real><<<nb, bs, 0, st>>>(make_geo(ctx), ctx->lay, ctx->d_c, f_re, ctx->d_fim, ctx->d_bc, ctx->d_wxl,
+  auto magic = [](unsigned long long d) { return d <= 1 ? 0ull : ~0ull / d + 1ull; };   // ceil(2^64 / d), d >= 2
+  BuildIdx bi{magic((unsigned long long)ctx->lay.lnx * ctx->lay.lny), magic((unsigned long long)ctx->lay.lnx),
+              magic((unsigned long long)ctx->sx), ctx->d_sxp, ctx->d_syp};
+  k_build<real><<<nb, bs, 0, st>>>(make_geo(ctx), ctx->lay, bi, ctx->d_c, f_re, ctx->d_fim, ctx->d_bc, ctx->d_wxl,
                                    ctx->d_wyl, (real *)ctx->d_gamma, (real *)ctx->d_alpha, (real *)ctx->d_bbf_re,
                                    (real *)ctx->d_bbf_im, (real *)ctx->d_k2, (real *)ctx->d_bs, only_source);
   HZ_CUDA(cudaGetLastError());
@@ -264,20 +269,64 @@ cudaError_t launch_exchange(const hz_ctx *c, double rho, cudaStream_t st) {
   return cudaGetLastError();
 }
 
-// gather into `out` of type outT (precision prec_out)
+// gather into `out` of type outT (precision prec_out); the line tables are built by hz_partition (upload_gather_tables)
 cudaError_t launch_gather(const hz_ctx *c, void *out, int prec_out, cudaStream_t st) {
-  const long long total = (long long)c->npx * c->npy;
   const int bs = 256;
-  const unsigned nb = (unsigned)((total + bs - 1) / bs);
-  const Geo g = make_geo(c);
+  const dim3 grid((unsigned)((c->npx + bs - 1) / bs), (unsigned)c->npy);
+  const size_t NS = (size_t)c->lay.NS;
   if (c->prec == HZ_F32) {
-    if (prec_out == HZ_F32) k_gather<float, float><<<nb, bs, 0, st>>>(g, c->lay, (const float *)c->d_usub, (float *)out);
-    else k_gather<float, double><<<nb, bs, 0, st>>>(g, c->lay, (const float *)c->d_usub, (double *)out);
+    if (prec_out == HZ_F32) k_gather<float, float><<<grid, bs, 0, st>>>(c->npx, c->npy, c->sx, NS, c->d_gcol, c->d_grow, (const float *)c->d_usub, (float *)out);
+    else k_gather<float, double><<<grid, bs, 0, st>>>(c->npx, c->npy, c->sx, NS, c->d_gcol, c->d_grow, (const float *)c->d_usub, (double *)out);
   } else {
-    if (prec_out == HZ_F32) k_gather<double, float><<<nb, bs, 0, st>>>(g, c->lay, (const double *)c->d_usub, (float *)out);
-    else k_gather<double, double><<<nb, bs, 0, st>>>(g, c->lay, (const double *)c->d_usub, (double *)out);
+    if (prec_out == HZ_F32) k_gather<double, float><<<grid, bs, 0, st>>>(c->npx, c->npy, c->sx, NS, c->d_gcol, c->d_grow, (const double *)c->d_usub, (float *)out);
+    else k_gather<double, double><<<grid, bs, 0, st>>>(c->npx, c->npy, c->sx, NS, c->d_gcol, c->d_grow, (const double *)c->d_usub, (double *)out);
   }
   return cudaGetLastError();
+}
+
+// the per-column / per-row tables of k_gather (hz_aux.cuh): which subdomain(s) hold global node line I (J) and where
+cudaError_t upload_gather_tables(hz_ctx *c) {
+  const Geo g = make_geo(c);
+  auto fill = [&](int np, int n_el, int q, int r, int mul, bool xdir, std::vector<GatherLine> *t) {
+    t->resize(np);
+    for (int I = 0; I < np; ++I) {
+      const int eh = I / g.p > n_el - 1 ? n_el - 1 : I / g.p;
+      const int i1 = sub_of_elem(q, r, eh);
+      const bool shared = I == sub_off(q, r, i1) * g.p && i1 > 0;
+      auto part = [&](int k) {   // x (y) part of Layout::slot of this line in subdomain column (row) k
+        const int loc = I - sub_off(q, r, k) * g.p;
+        return xdir ? c->lay.slot(loc, 0) : c->lay.slot(0, loc);
+      };
+      GatherLine L;
+      L.s1 = i1 * mul;
+      L.p1 = part(i1);
+      L.p0 = shared ? part(i1 - 1) : 0;
+      L.n = shared ? 2 : 1;
+      (*t)[I] = L;
+    }
+  };
+  std::vector<GatherLine> tx, ty;
+  fill(c->npx, c->nx, g.exq, g.exr, 1, true, &tx);
+  fill(c->npy, c->ny, g.eyq, g.eyr, c->sx, false, &ty);
+  cudaError_t e = cudaMalloc((void **)&c->d_gcol, tx.size() * sizeof(GatherLine));
+  if (e != cudaSuccess) return e;
+  e = cudaMalloc((void **)&c->d_grow, ty.size() * sizeof(GatherLine));
+  if (e != cudaSuccess) return e;
+  e = cudaMemcpy(c->d_gcol, tx.data(), tx.size() * sizeof(GatherLine), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) return e;
+  e = cudaMemcpy(c->d_grow, ty.data(), ty.size() * sizeof(GatherLine), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) return e;
+  // k_build's separable slot tables
+  std::vector<int> sxp(c->lay.lnx), syp(c->lay.lny);
+  for (int i = 0; i < c->lay.lnx; ++i) sxp[i] = c->lay.slot(i, 0);
+  for (int j = 0; j < c->lay.lny; ++j) syp[j] = c->lay.slot(0, j);
+  e = cudaMalloc((void **)&c->d_sxp, sxp.size() * sizeof(int));
+  if (e != cudaSuccess) return e;
+  e = cudaMalloc((void **)&c->d_syp, syp.size() * sizeof(int));
+  if (e != cudaSuccess) return e;
+  e = cudaMemcpy(c->d_sxp, sxp.data(), sxp.size() * sizeof(int), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) return e;
+  return cudaMemcpy(c->d_syp, syp.data(), syp.size() * sizeof(int), cudaMemcpyHostToDevice);
 }
 
 // launches k_helm<inT, acc, P, MODE> on the whole mesh (hz_aux.cuh)
@@ -837,6 +886,7 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
   }
   HZ_CUDA(upload_as<double>(wxl, (void **)&ctx->d_wxl));
   HZ_CUDA(upload_as<double>(wyl, (void **)&ctx->d_wyl));
+  HZ_CUDA(upload_gather_tables(ctx));
   ctx->ws_bytes = ws;
   ctx->part = true;
   hz_status st = prec == HZ_F32 ? run_build<float>(ctx, 0, 0) : run_build<double>(ctx, 0, 0);

@@ -27,8 +27,15 @@ __host__ __device__ inline int sub_of_elem(int q, int r, int e) {
 // One thread per (subdomain, local node).  wxl/wyl: assembled reference GLL weights of the ex (ey)
 // elements of a subdomain side.  Everything is computed in fp64 and rounded once.
 // ---------------------------------------------------------------------------------------------
+// Index arithmetic without divisions: gid -> (subdomain, row, column) by multiplication with host-computed
+// reciprocals (floor(x / d) = umul64hi(x, ceil(2^64 / d)) exactly for x, d < 2^32), the slot from the separable
+// tables sxp[i] + syp[j] of Layout::slot; one reciprocal of c and one of the denominator instead of six divisions.
+struct BuildIdx {
+  unsigned long long magN, magLnx, magSx;   // ceil(2^64 / N), ceil(2^64 / lnx), ceil(2^64 / sx)
+  const int *sxp, *syp;              // [lnx], [lny]: x and y part of Layout::slot
+};
 template <typename real>
-__global__ void k_build(Geo g, Layout lay, const double *__restrict__ c, const double *__restrict__ f_re,
+__global__ void k_build(Geo g, Layout lay, BuildIdx bi, const double *__restrict__ c, const double *__restrict__ f_re,
                         const double *__restrict__ f_im, const double *__restrict__ bc, const double *__restrict__ wxl,
                         const double *__restrict__ wyl, real *gamma, real *alpha, real *bbf_re, real *bbf_im,
                         real *k2edge, real *bs, int only_source) {
@@ -36,25 +43,25 @@ __global__ void k_build(Geo g, Layout lay, const double *__restrict__ c, const d
   const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const long long total = (long long)g.sx * g.sy * N;
   if (gid >= total) return;
-  const int l = (int)(gid / N), q = (int)(gid - (long long)l * N);
-  const int i = q % lay.lnx, j = q / lay.lnx;
-  const int six = l % g.sx, siy = l / g.sx;
+  const int l = (int)__umul64hi((unsigned long long)gid, bi.magN), q = (int)(gid - (long long)l * N);
+  const int j = (int)__umul64hi((unsigned long long)q, bi.magLnx), i = q - j * lay.lnx;
+  const int siy = g.sx == 1 ? l : (int)__umul64hi((unsigned long long)l, bi.magSx), six = l - siy * g.sx;
   const int I = six * g.ex * g.p + i, J = siy * g.ey * g.p + j;
   const size_t gn = (size_t)J * g.npx + I;
-  const double cj = c[gn];
+  const double cj = c[gn], rc = 1.0 / cj;
   const double m = 0.25 * g.hx * g.hy * wxl[i] * wyl[j];  // local lumped mass (geometric)
-  const double M = m / (cj * cj);
+  const double M = m * rc * rc;
   // impedance weight on the WHOLE subdomain boundary: interfaces carry the same operator as the
   // outer boundary
   const bool onW = i == 0, onE = i == lay.lnx - 1, onS = j == 0, onN = j == lay.lny - 1;
   const double sWE = 0.5 * g.hy * wyl[j], sSN = 0.5 * g.hx * wxl[i];
   double H = 0.0;
-  if (onW) H += sWE / cj;
-  if (onE) H += sWE / cj;
-  if (onS) H += sSN / cj;
-  if (onN) H += sSN / cj;
-  const double den = M + g.theta * H;
-  const double beta = g.sigma / den;
+  if (onW) H += sWE * rc;
+  if (onE) H += sWE * rc;
+  if (onS) H += sSN * rc;
+  if (onN) H += sSN * rc;
+  const double den = M + g.theta * H, rden = 1.0 / den;
+  const double beta = g.sigma * rden;
   // load: f(x_j) m_j (+ the outer-boundary datum lambda of eq. (1b) on physical sides)
   double bre = f_re[gn] * m, bim = f_im ? f_im[gn] * m : 0.0;
   if (bc) {
@@ -63,14 +70,14 @@ __global__ void k_build(Geo g, Layout lay, const double *__restrict__ c, const d
     if (onS && siy == 0) { bre += sSN * bc[(2 * 2 + 0) * g.EB + I]; bim += sSN * bc[(2 * 2 + 1) * g.EB + I]; }
     if (onN && siy == g.sy - 1) { bre += sSN * bc[(3 * 2 + 0) * g.EB + I]; bim += sSN * bc[(3 * 2 + 1) * g.EB + I]; }
   }
-  const size_t o = (size_t)l * lay.NS + lay.slot(i, j);
+  const size_t o = (size_t)l * lay.NS + bi.sxp[i] + bi.syp[j];
   bbf_re[o] = (real)(beta * bre);
   if (bbf_im) bbf_im[o] = (real)(beta * bim);
   if (only_source) return;
   gamma[o] = (real)(beta * m);
-  alpha[o] = (real)((M - g.theta * H) / den);
+  alpha[o] = (real)((M - g.theta * H) * rden);
   const size_t eb = (size_t)l * 4 * g.E;
-  const double k2 = 2.0 * g.omega / cj;
+  const double k2 = 2.0 * g.omega * rc;
   if (onW) { k2edge[eb + 0 * g.E + j] = (real)k2; bs[eb + 0 * g.E + j] = (real)(beta * sWE); }
   if (onE) { k2edge[eb + 1 * g.E + j] = (real)k2; bs[eb + 1 * g.E + j] = (real)(beta * sWE); }
   if (onS) { k2edge[eb + 2 * g.E + i] = (real)k2; bs[eb + 2 * g.E + i] = (real)(beta * sSN); }
@@ -157,29 +164,37 @@ __global__ void k_exchange(int sx, int sy, int E, int ex_nodes, int ey_nodes, re
 // A7 / R19: global nodal field, mean of the copies at nodes shared by several subdomains, summed in
 // the fixed order (iy ascending, ix ascending).
 // ---------------------------------------------------------------------------------------------
+// Layout::slot is separable: slot(i, j) = sx(i) + sy(j).  The host tabulates, for every GLOBAL node column I (row J),
+// the subdomain column (row) that owns the element having it as a lower node, the x (y) part of the slot there and, at a
+// node shared with the subdomain column (row) before, the part there: no divisions in the kernel, and the mean over
+// 1, 2 or 4 copies is a multiplication by an exact power of two.
+struct GatherLine {
+  int s1;     // subdomain column ix1 (x table) / iy1 * sx (y table): the last subdomain that holds the line
+  int p1;     // slot part of the line in that subdomain
+  int p0;     // slot part in the subdomain before (valid if n == 2)
+  int n;      // 1 or 2 copies along this direction
+};
 template <typename real, typename outT>
-__global__ void k_gather(Geo g, Layout lay, const real *__restrict__ u_sub, outT *__restrict__ u_out) {
-  const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  const long long total = (long long)g.npx * g.npy;
-  if (gid >= total) return;
-  const int I = (int)(gid % g.npx), J = (int)(gid / g.npx);
-  // the subdomain column (row) of the element that has this node as a lower node, and the one before at a shared node
-  const int ehx = I / g.p > g.nx - 1 ? g.nx - 1 : I / g.p, ehy = J / g.p > g.ny - 1 ? g.ny - 1 : J / g.p;
-  const int ix1 = sub_of_elem(g.exq, g.exr, ehx), iy1 = sub_of_elem(g.eyq, g.eyr, ehy);
-  const int ix0 = (I == sub_off(g.exq, g.exr, ix1) * g.p && ix1 > 0) ? ix1 - 1 : ix1;
-  const int iy0 = (J == sub_off(g.eyq, g.eyr, iy1) * g.p && iy1 > 0) ? iy1 - 1 : iy1;
+__global__ void __launch_bounds__(256) k_gather(int npx, int npy, int sxg, size_t NS, const GatherLine *__restrict__ colx,
+                                                const GatherLine *__restrict__ rowy, const real *__restrict__ u_sub,
+                                                outT *__restrict__ u_out) {
+  const int I = blockIdx.x * blockDim.x + threadIdx.x, J = blockIdx.y;
+  if (I >= npx) return;
+  const GatherLine cx = colx[I], ry = rowy[J];
+  const size_t total = (size_t)npx * npy, gid = (size_t)J * npx + I;
   double sr = 0.0, si = 0.0;
-  int cnt = 0;
-  for (int iy = iy0; iy <= iy1; ++iy)
-    for (int ix = ix0; ix <= ix1; ++ix) {
-      const int l = iy * g.sx + ix;
-      const int s = lay.slot(I - sub_off(g.exq, g.exr, ix) * g.p, J - sub_off(g.eyq, g.eyr, iy) * g.p);
-      sr += (double)u_sub[(size_t)l * 2 * lay.NS + s];
-      si += (double)u_sub[(size_t)l * 2 * lay.NS + lay.NS + s];
-      ++cnt;
+  // fixed order: iy ascending, ix ascending (reading R19)
+  for (int ky = ry.n - 1; ky >= 0; --ky) {
+    const int ly = ry.s1 - ky * sxg, py = ky ? ry.p0 : ry.p1;
+    for (int kx = cx.n - 1; kx >= 0; --kx) {
+      const size_t o = (size_t)(ly + cx.s1 - kx) * 2 * NS + (size_t)(py + (kx ? cx.p0 : cx.p1));
+      sr += (double)u_sub[o];
+      si += (double)u_sub[o + NS];
     }
-  u_out[gid] = (outT)(sr / cnt);
-  u_out[total + gid] = (outT)(si / cnt);
+  }
+  const double w = 1.0 / (double)(cx.n * ry.n);   // 1, 1/2, 1/4: exact
+  u_out[gid] = (outT)(sr * w);
+  u_out[total + gid] = (outT)(si * w);
 }
 
 // ---------------------------------------------------------------------------------------------
