@@ -450,7 +450,7 @@ __device__ __forceinline__ void helm_tile_int(const Geo &g, const HelmC<acc> &hc
 // Blocks strictly inside the mesh (all but the outermost ring) take a path without bounds checks, one-sided weights or
 // boundary terms.  Several blocks per SM (helm_minb) overlap one block's staging with another's arithmetic.
 template <typename inT, typename acc, int P, int MODE, bool EDGE>
-__global__ void __launch_bounds__(kHelmBX *kHelmBY, EDGE ? 1 : helm_minb<acc, P, MODE>())
+__global__ void __launch_bounds__(kHelmBX *kHelmBY, EDGE ? (MODE == 1 && P <= 3 ? 3 : 2) : helm_minb<acc, P, MODE>())
     k_helm(Geo g, const HelmGrid hg, const __grid_constant__ HelmC<acc> hc, const double *__restrict__ c, const acc *__restrict__ k2,
            const double *__restrict__ f_re, const double *__restrict__ f_im, const double *__restrict__ bc,
            const inT *__restrict__ u, double *__restrict__ part, acc *__restrict__ y) {

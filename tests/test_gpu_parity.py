@@ -463,11 +463,14 @@ def test_graph_is_rebuilt_when_a_complex_source_arrives():
 
 
 @pytest.mark.parametrize("prec", [hz.HZ_F64, hz.HZ_F32])
-@pytest.mark.parametrize("p,nx,ny", [(1, 37, 9), (2, 33, 11), (3, 35, 10), (4, 34, 9)])
+@pytest.mark.parametrize("p,nx,ny", [(1, 37, 9), (2, 33, 11), (3, 35, 10), (4, 34, 9),
+                                     (1, 101, 27), (2, 99, 26), (3, 70, 20), (4, 100, 27), (3, 131, 35)])
 def test_global_operator_kernel_matches_the_assembled_matrix(p, nx, ny, prec):
     """hz_operator_time's kernel (the paper's "operator" of PAPER.md:223; the residual kernel's other mode): y =
     (A - i w H - w^2 M) u on a random complex vector against the oracle's assembled sparse matrix.  The mesh spans
-    several 32x8-element blocks of the kernel with ragged tails in both directions."""
+    several 32x8-element blocks of the kernel with ragged tails in both directions; the larger meshes have patches
+    strictly inside the mesh, which run the interior kernels (cp.async staging; TMA bulk copies for fp64 at p >= 3), the
+    smaller ones only the general kernel of the boundary ring.  The residual mode is checked against the same matrix."""
     _require_cuda()
     inp = hetero_inputs(nx, ny, p, 1, 1, seed=300 + p)
     pr = problem_from(inp)
@@ -486,5 +489,10 @@ def test_global_operator_kernel_matches_the_assembled_matrix(p, nx, ny, prec):
         assert ms > 0
         y = yd.double().cpu().numpy()
         assert rel(y[:nn] + 1j * y[nn:], y_o) <= (1e-13 if prec == hz.HZ_F64 else 2e-6)
+        # residual mode of the same kernels: || b - Z u || / || b || with u in the precision `prec`
+        ur = ud.double().cpu().numpy()
+        want = np.linalg.norm(b - Z @ (ur[:nn] + 1j * ur[nn:])) / np.linalg.norm(b)
+        got = hz.hz_residual(ctx, ud.data_ptr(), prec)
+        assert abs(got - want) <= 1e-9 * want
     finally:
         hz.hz_destroy(ctx)
