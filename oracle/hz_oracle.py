@@ -550,18 +550,19 @@ def ddm_mixed_solve(pr: Problem, sx: int, sy: int, n_cycles: int, m_inner: int, 
 # vector (real parts, then imaginary parts) with the Euclidean inner product.
 # Restarted GMRES(m) on (I - T) x = c: Arnoldi with modified Gram-Schmidt, least-squares problem
 # by Givens rotations (Saad & Schultz 1986, in its textbook form).  Each Arnoldi step costs one sweep.
-def ddm_pack(st: DDMState) -> np.ndarray:
+def ddm_pack(st: DDMState, with_u: bool = True) -> np.ndarray:
     parts = []
     for l, sd in enumerate(st.subs):
         for side in range(4):
             if sd.neighbour[side] >= 0:
                 parts.append(st.lam[l][side])
-    parts += st.u
+    if with_u:
+        parts += st.u
     z = np.concatenate(parts)
     return np.concatenate([z.real, z.imag])
 
 
-def ddm_unpack(st: DDMState, x: np.ndarray) -> None:
+def ddm_unpack(st: DDMState, x: np.ndarray, with_u: bool = True) -> None:
     h = len(x) // 2
     z = x[:h] + 1j * x[h:]
     o = 0
@@ -571,26 +572,38 @@ def ddm_unpack(st: DDMState, x: np.ndarray) -> None:
                 n = len(st.lam[l][side])
                 st.lam[l][side] = z[o:o + n].copy()
                 o += n
+    if not with_u:
+        return
     for l in range(len(st.subs)):
         n = len(st.u[l])
         st.u[l] = z[o:o + n].copy()
         o += n
 
 
+# Krylov iteration on lambda ALONE (the fixed-point iteration on the interface data "accelerated with a
+# Krylov space method").  With a COLD start (Algorithm 1 as printed, u^(0) = 0) and a
+# fixed number n_wh of WaveHoltz iterations, one sweep is an affine, real-linear map lambda -> G lambda + d of the
+# interface data alone (u_l is an output, not a state), so GMRES on (I - G) lambda = d needs basis vectors of the size of
+# the interfaces only.  Its fixed point is the DDM fixed point of the INEXACT subdomain solver (n_wh WaveHoltz iterations
+# from zero); it tends to the discrete solution as n_wh grows.  After the iteration the field is u_l(lambda) by one more
+# cycle at fixed lambda, optionally polished by `n_polish` further warm-started WaveHoltz iterations at that lambda.
 def ddm_gmres(pr: Problem, sx: int, sy: int, n_wh: int, relax: float, restart: int, n_steps: int,
-              cfl_frac: float = 0.5, tol: float = 0.0):
+              cfl_frac: float = 0.5, tol: float = 0.0, lambda_only: bool = False, n_polish: int = 0):
     """Runs `n_steps` Arnoldi steps in total (restarting every `restart` steps) of GMRES on
     (I - T) x = c from x = 0 and leaves the final iterate in the returned state.
     Returns (state, history) with history[k] = relative LINEAR residual ||c - (I-T)x_k|| / ||c||
-    after k steps, as estimated by the Givens recurrence.  Stops early when that drops to `tol`."""
+    after k steps, as estimated by the Givens recurrence.  Stops early when that drops to `tol`.
+    lambda_only: x = lambda and the sweeps are cold-started (see above); the returned state then holds
+    u_l = n_wh (+ n_polish warm-started) WaveHoltz iterations for the final lambda."""
     st = ddm_setup(pr, sx, sy, cfl_frac)
+    with_u = not lambda_only
 
     def F(x):
-        ddm_unpack(st, x)
-        ddm_sweep(st, n_wh, True, relax)
-        return ddm_pack(st)
+        ddm_unpack(st, x, with_u)
+        ddm_sweep(st, n_wh, with_u, relax)
+        return ddm_pack(st, with_u)
 
-    x = np.zeros_like(ddm_pack(st))
+    x = np.zeros_like(ddm_pack(st, with_u))
     c = F(x)
     cnorm = float(np.linalg.norm(c))
     hist = [1.0]
@@ -631,7 +644,13 @@ def ddm_gmres(pr: Problem, sx: int, sy: int, n_wh: int, relax: float, restart: i
             x = x + y[i] * V[i]
         if tol > 0 and hist[-1] <= tol:
             break
-    ddm_unpack(st, x)
+    ddm_unpack(st, x, with_u)
+    if lambda_only:                                         # u_l(lambda) at the final lambda (lambda itself is not advanced)
+        for l in range(len(st.subs)):
+            st.u[l], _ = ddm_cycle(st, l, n_wh, False)
+        if n_polish > 0:
+            for l in range(len(st.subs)):
+                st.u[l], _ = ddm_cycle(st, l, n_polish, True)
     return st, hist
 
 
