@@ -497,7 +497,9 @@ def run_b200(args):
 def time_to_solution(hz, inp, prec_name, tol, every, nmax, stream, driver="fixed_point", restart=50, n_wh=2):
     """DDM time-to-solution (BASELINE.json metric 1): global relative residual (hz_residual, fp64) to `tol`,
     n_wh = 2, rho = 0.5, warm start.  fixed_point: hz_ddm_solve with CUDA-graph replay between residual checks;
-    mixed: hz_ddm_solve_mixed (fp32 sweeps on the correction, fp64 state); gmres: hz_ddm_solve_gmres."""
+    mixed: hz_ddm_solve_mixed (fp32 sweeps on the correction, fp64 state); gmres: hz_ddm_solve_gmres on the joint state;
+    gmres_lambda: hz_ddm_solve_gmres on lambda alone (cold-started sweeps of n_wh WaveHoltz iterations, rho = 1,
+    basis of `restart` interface-sized vectors: no restart in practice)."""
     out = {"tol": tol, "n_wh": n_wh, "relax": 0.5, "driver": driver}
     if driver == "mixed":
         lo, _ = hz.setup_from_inputs(inp, hz.HZ_F32, 0)
@@ -517,7 +519,16 @@ def time_to_solution(hz, inp, prec_name, tol, every, nmax, stream, driver="fixed
         return out
     ctx, pinfo = hz.setup_from_inputs(inp, hz.HZ_F32 if prec_name == "f32" else hz.HZ_F64, 0)
     try:
-        if driver == "gmres":
+        if driver == "gmres_lambda":
+            hz.hz_ddm_solve_gmres(ctx, 3, n_wh=n_wh, relax=1.0, restart=restart, lambda_only=True, stream=stream)   # allocation, warm-up
+            t0 = time.perf_counter()
+            s = hz.hz_ddm_solve_gmres(ctx, nmax, n_wh=n_wh, relax=1.0, restart=restart, lin_tol=0.02 * tol, reset_state=True,
+                                      lambda_only=True, stream=stream)
+            out.update(relax=1.0, sweeps=s.sweeps_done, waveholtz_iterations=s.sweeps_done * n_wh, cycles=s.cycles,
+                       lin_residual=s.lin_residual, rel_residual=s.rel_residual, device_ms=s.total_ms,
+                       wall_ms=(time.perf_counter() - t0) * 1e3, restart=restart, krylov_mb=s.krylov_bytes / 1e6,
+                       reached=bool(s.rel_residual <= tol))
+        elif driver == "gmres":
             hz.hz_ddm_solve_gmres(ctx, 3, n_wh=n_wh, restart=restart, stream=stream)                  # allocation, warm-up
             t0 = time.perf_counter()
             s = hz.hz_ddm_solve_gmres(ctx, nmax, n_wh=n_wh, relax=0.5, restart=restart, tol=tol, reset_state=True, stream=stream)
@@ -682,6 +693,12 @@ def run_extras(hz, torch, args, flush, stream, sampler):
                                       (4, "f64", 50, 6000, "fixed_point")):
         key = f"config{cfg}_{'f32_sweeps_f64_state' if drv == 'mixed' else pr}_time_to_solution_n_wh_1"
         leg(key, lambda: time_to_solution(hz, get(cfg), pr, 1e-4, every, nmax, stream, drv, n_wh=1))
+    # Krylov iteration on lambda alone (cold-started sweeps, interface-sized basis, no restart): config 2 to
+    # the shared tolerance with 20 WaveHoltz iterations per sweep; config 3 with a bounded step count (it does not get there)
+    leg("config2_f64_time_to_solution_gmres_lambda_only",
+        lambda: time_to_solution(hz, get(2), "f64", 1e-4, 0, 400, stream, "gmres_lambda", restart=400, n_wh=20))
+    leg("config3_f64_gmres_lambda_only_300_steps",
+        lambda: time_to_solution(hz, get(3), "f64", 1e-4, 0, 300, stream, "gmres_lambda", restart=300, n_wh=16))
     inputs.clear()
 
     leg("paper_style_cycle_512_p3_f32", lambda: paper_style_cycle(hz, torch, stream, flush))
@@ -809,10 +826,14 @@ def run_tables(args):
             tol_hi = 1e-8 if cfg == 1 else 1e-4
             rows = [("f64", tol_hi, "fixed_point", 2), ("f32", 1e-4, "fixed_point", 2), ("f32", tol_hi, "mixed", 2),
                     ("f64", tol_hi, "fixed_point", 1), ("f32", tol_hi, "mixed", 1),
-                    ("f64", tol_hi, "gmres", 2), ("f32", 1e-4, "gmres", 2)]
+                    ("f64", tol_hi, "gmres", 2), ("f32", 1e-4, "gmres", 2),
+                    ("f64", tol_hi, "gmres_lambda", {1: 40, 2: 20, 3: 16, 4: 16}[cfg])]
             for pr, tol, drv, nwh in rows:
-                r = time_to_solution(hz, inp, pr, tol, 25 if drv == "mixed" else every, 40000 if drv != "gmres" else 4000,
-                                     stream, drv, restart=50 if cfg <= 2 else 100, n_wh=nwh)
+                if drv == "gmres_lambda":
+                    r = time_to_solution(hz, inp, pr, tol, 0, 1000 if cfg <= 3 else 400, stream, drv, restart=1000 if cfg <= 3 else 400, n_wh=nwh)
+                else:
+                    r = time_to_solution(hz, inp, pr, tol, 25 if drv == "mixed" else every, 40000 if drv != "gmres" else 4000,
+                                         stream, drv, restart=50 if cfg <= 2 else 100, n_wh=nwh)
                 arith = "fp32 sweeps, fp64 state" if drv == "mixed" else pr
                 note = "" if r["reached"] else "NOT reached"
                 if drv == "mixed":

@@ -231,6 +231,14 @@ hz_status hz_ddm_solve_sources(hz_ctx *ctx, const hz_solve_opts *opts, int n_src
  * kernel, exactly as in hz_ddm_solve) is an affine, real-linear map x -> T x + c of the joint state
  * x = (lambda, u_l); restarted GMRES(restart) solves (I - T) x = c, one sweep per Arnoldi step (classical
  * Gram-Schmidt applied twice, Givens rotations on the host).  The fixed point is the DDM fixed point.
+ *
+ * lambda_only = 1: the Krylov iteration on lambda ALONE.  With cold-started sweeps (u^(0) = 0, Algorithm 1 as printed,
+ * PAPER.md:164) and a fixed n_wh, lambda -> G lambda + d is an affine map of the interface data alone, so the basis
+ * vectors have the size of the interfaces (about 1/25 of the joint state at 625 DOFs per subdomain) and a large
+ * `restart` is cheap.  Its fixed point is the DDM fixed point of the INEXACT subdomain solver (n_wh WaveHoltz
+ * iterations from zero): n_wh sets the attainable Helmholtz residual (about 0.55^n_wh on 8x8-element subdomains).
+ * The field returned is u_l(lambda) from one more sweep kernel at the final lambda (lambda not advanced), followed by
+ * n_polish warm-started WaveHoltz iterations at that lambda.
  * ------------------------------------------------------------------------------------------- */
 typedef struct {
   int n_wh;        /* WaveHoltz iterations per sweep (>= 1) */
@@ -244,6 +252,8 @@ typedef struct {
   int reset_state; /* 1: start from x = 0; 0: start from the context's current (lambda, u_l) */
   double *lin_history; /* HOST or NULL: receives the relative linear residual after each Arnoldi step */
   int history_len;     /* capacity of lin_history */
+  int lambda_only;     /* 0: x = (lambda, u_l), warm-started sweeps; 1: x = lambda, cold-started sweeps (see above) */
+  int n_polish;        /* lambda_only: WaveHoltz iterations added to u_l at the final lambda (>= 0) */
 } hz_gmres_opts;
 
 typedef struct {

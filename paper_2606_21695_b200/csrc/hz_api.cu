@@ -86,6 +86,7 @@ struct hz_ctx {
   double *d_kpart = nullptr;
   int kry_vecs = 0;
   long long n_state = 0;
+  long long kry_len = 0;  // length of the Krylov vectors d_kry was allocated for
   cudaGraphExec_t g_exec = nullptr;
   cudaStream_t cap_stream = nullptr;  // capture happens on this private stream (the legacy default stream cannot capture)
   // hz_ddm_solve_sources: copy-in / copy-out streams, double-buffered staging and the events that order them
@@ -124,7 +125,7 @@ void free_partition(hz_ctx *c) {
   if (c->d_mr) { cudaFree(c->d_mr); c->d_mr = nullptr; }
   if (c->d_mr_iters) { cudaFree(c->d_mr_iters); c->d_mr_iters = nullptr; }
   if (c->d_mr_res) { cudaFree(c->d_mr_res); c->d_mr_res = nullptr; }
-  if (c->d_kry) { cudaFree(c->d_kry); c->d_kry = nullptr; c->kry_vecs = 0; }
+  if (c->d_kry) { cudaFree(c->d_kry); c->d_kry = nullptr; c->kry_vecs = 0; c->kry_len = 0; }
   if (c->d_kpart) { cudaFree(c->d_kpart); c->d_kpart = nullptr; }
   if (c->g_exec) { cudaGraphExecDestroy(c->g_exec); c->g_exec = nullptr; }
   if (c->d_G) { cudaFree(c->d_G); c->d_G = nullptr; }
@@ -1196,28 +1197,45 @@ namespace {
 
 template <typename real>
 hz_status gmres_impl(hz_ctx *ctx, const hz_gmres_opts *o, void *u_out, hz_gmres_info *info, cudaStream_t st) {
-  const long long n = ctx->n_state;
+  // lambda_only: the vectors are the lambda part of the joint state (the first L*8*E reals of d_lam), sweeps cold-started
+  const bool lam_only = o->lambda_only != 0;
+  const long long n = lam_only ? (long long)ctx->L * 8 * ctx->E : ctx->n_state;
   const int m = o->restart;
   const int nvec = m + 3;  // V_0..V_m, c, x
   const size_t rs = sizeof(real);
   const int bs = 256, nblk = 592;  // 4 blocks per SM on 148 SMs
-  if (!ctx->d_kry || ctx->kry_vecs < nvec) {
+  if (!ctx->d_kry || ctx->kry_vecs < nvec || ctx->kry_len < n) {
     if (ctx->d_kry) cudaFree(ctx->d_kry);
     if (ctx->d_kpart) cudaFree(ctx->d_kpart);
     ctx->d_kry = nullptr; ctx->d_kpart = nullptr; ctx->kry_vecs = 0;
     HZ_CUDA(cudaMalloc(&ctx->d_kry, (size_t)nvec * n * rs));
     HZ_CUDA(cudaMalloc((void **)&ctx->d_kpart, ((size_t)(m + 2) * nblk + 2 * (m + 2)) * sizeof(double)));
     ctx->kry_vecs = nvec;
+    ctx->kry_len = n;
   }
   real *V = (real *)ctx->d_kry, *cvec = V + (size_t)(m + 1) * n, *x = cvec + n, *state = (real *)ctx->d_lam;
   double *part = ctx->d_kpart, *dres = part + (size_t)(m + 2) * nblk, *dcoef = dres + (m + 2);
   hz_solve_opts so{};
-  so.n_wh = o->n_wh; so.warm_start = 1; so.relax = o->relax;
+  so.n_wh = o->n_wh; so.warm_start = lam_only ? 0 : 1; so.relax = o->relax;
   int sweeps = 0;
   auto sweep = [&]() -> cudaError_t {
     cudaError_t e = launch_sweep(ctx, &so, st);
     if (e == cudaSuccess) e = launch_exchange(ctx, o->relax, st);
     ++sweeps;
+    return e;
+  };
+  // lambda_only: u_l of the lambda now in the state -- the sweep kernel without the exchange (lambda is not advanced),
+  // then n_polish warm-started WaveHoltz iterations at that lambda
+  auto materialise = [&]() -> cudaError_t {
+    if (!lam_only) return cudaSuccess;
+    cudaError_t e = launch_sweep(ctx, &so, st);
+    ++sweeps;
+    if (e == cudaSuccess && o->n_polish > 0) {
+      hz_solve_opts sp = so;
+      sp.n_wh = o->n_polish; sp.warm_start = 1;
+      e = launch_sweep(ctx, &sp, st);
+      ++sweeps;
+    }
     return e;
   };
   std::vector<double> hbuf(m + 2);
@@ -1327,6 +1345,7 @@ hz_status gmres_impl(hz_ctx *ctx, const hz_gmres_opts *o, void *u_out, hz_gmres_
     if (o->lin_tol > 0.0 && lin <= o->lin_tol) finished = true;
     if (o->tol > 0.0 && lin <= lin_target) {
       HZ_CUDA(cudaMemcpyAsync(state, x, n * rs, cudaMemcpyDeviceToDevice, st));
+      HZ_CUDA(materialise());
       HZ_CUDA(launch_gather(ctx, ctx->d_ures, HZ_F64, st));
       hz_status s2 = residual_impl(ctx, ctx->d_ures, HZ_F64, &rel, st);
       if (s2 != HZ_OK) return s2;
@@ -1336,6 +1355,7 @@ hz_status gmres_impl(hz_ctx *ctx, const hz_gmres_opts *o, void *u_out, hz_gmres_
   }
   // leave the iterate in the context's state, report its Helmholtz residual
   HZ_CUDA(cudaMemcpyAsync(state, x, n * rs, cudaMemcpyDeviceToDevice, st));
+  HZ_CUDA(materialise());
   HZ_CUDA(launch_gather(ctx, ctx->d_ures, HZ_F64, st));
   {
     hz_status s2 = residual_impl(ctx, ctx->d_ures, HZ_F64, &rel, st);
@@ -1560,8 +1580,8 @@ extern "C" hz_status hz_ddm_solve_gmres(hz_ctx *ctx, const hz_gmres_opts *opts, 
   if (!opts) return fail(ctx, HZ_EINVAL, "hz_ddm_solve_gmres: NULL opts");
   if (!ctx->part) return fail(ctx, HZ_ESTATE, "hz_ddm_solve_gmres: call hz_partition first");
   if (opts->n_wh < 1 || !(opts->relax > 0.0) || opts->relax > 1.0 || opts->restart < 1 || opts->restart > 1000 ||
-      opts->max_steps < 0 || (opts->lin_history && opts->history_len < 0))
-    return fail(ctx, HZ_EINVAL, "hz_ddm_solve_gmres: need n_wh >= 1, relax in (0,1], 1 <= restart <= 1000, max_steps >= 0");
+      opts->max_steps < 0 || (opts->lin_history && opts->history_len < 0) || opts->n_polish < 0)
+    return fail(ctx, HZ_EINVAL, "hz_ddm_solve_gmres: need n_wh >= 1, relax in (0,1], 1 <= restart <= 1000, max_steps >= 0, n_polish >= 0");
   cudaStream_t st = (cudaStream_t)stream;
   return ctx->prec == HZ_F32 ? gmres_impl<float>(ctx, opts, u_out, info, st) : gmres_impl<double>(ctx, opts, u_out, info, st);
 }

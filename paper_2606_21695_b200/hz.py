@@ -70,7 +70,8 @@ class hz_solve_info(C.Structure):
 class hz_gmres_opts(C.Structure):
     _fields_ = [("n_wh", C.c_int), ("relax", C.c_double), ("restart", C.c_int), ("max_steps", C.c_int),
                 ("lin_tol", C.c_double), ("tol", C.c_double), ("reset_state", C.c_int),
-                ("lin_history", C.POINTER(C.c_double)), ("history_len", C.c_int)]
+                ("lin_history", C.POINTER(C.c_double)), ("history_len", C.c_int), ("lambda_only", C.c_int),
+                ("n_polish", C.c_int)]
 
 
 class hz_gmres_info(C.Structure):
@@ -254,11 +255,12 @@ def hz_ddm_solve_sources(ctx, f_host_ptrs, u_host_ptrs, n_outer=1, n_wh=5, warm_
 
 
 def hz_ddm_solve_gmres(ctx, max_steps, n_wh=2, relax=0.5, restart=50, lin_tol=0.0, tol=0.0, reset_state=True,
-                       u_out_ptr=None, stream=None, want_history=False):
+                       u_out_ptr=None, stream=None, want_history=False, lambda_only=False, n_polish=0):
     """-> hz_gmres_info (and the per-step relative linear residuals if want_history)."""
     hist = (C.c_double * max(1, int(max_steps)))() if want_history else None
     opts = hz_gmres_opts(int(n_wh), float(relax), int(restart), int(max_steps), float(lin_tol), float(tol),
-                         int(bool(reset_state)), hist if want_history else None, int(max_steps) if want_history else 0)
+                         int(bool(reset_state)), hist if want_history else None, int(max_steps) if want_history else 0,
+                         int(bool(lambda_only)), int(n_polish))
     info = hz_gmres_info()
     _check(ctx, lib().hz_ddm_solve_gmres(ctx, C.byref(opts), C.c_void_p(u_out_ptr) if u_out_ptr else None,
                                          C.byref(info), C.c_void_p(stream) if stream else None))

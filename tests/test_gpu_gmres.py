@@ -76,3 +76,39 @@ def test_gmres_continues_from_the_current_state():
         assert b.rel_residual < a.rel_residual
     finally:
         hz.hz_destroy(ctx)
+
+
+# ---------------------------------------------------------------- Krylov iteration on lambda alone (lambda_only = 1)
+@pytest.mark.parametrize("prec,k,tol", [(hz.HZ_F64, 0, 1e-9), (hz.HZ_F64, 1, 1e-9), (hz.HZ_F32, 0, 1e-4)])
+def test_lambda_only_gmres_iterates_match_the_oracle(prec, k, tol):
+    """Same Arnoldi step counts (two restarts inside the run), cold-started sweeps of 3 WaveHoltz iterations, the field
+    polished by 2 more at the final lambda: lambda, u_l and the residual history against oracle.ddm_gmres(lambda_only)."""
+    if not torch.cuda.is_available():
+        pytest.fail("CUDA device required")
+    inp = make_config(2, n=24)           # 3x3 subdomains of 8x8 elements, Y-guide
+    steps, restart = 14, 6
+    st, hist_o = O.ddm_gmres(problem_from(inp), inp.sx, inp.sy, 3, 0.5, restart=restart, n_steps=steps, lambda_only=True,
+                             n_polish=2)
+    g = gpu_gmres(inp, prec, k, max_steps=steps, n_wh=3, relax=0.5, restart=restart, lambda_only=True, n_polish=2)
+    assert g["ginfo"].steps_done == steps and g["ginfo"].cycles == 3
+    u_o, lam_o = oracle_state_arrays(st)
+    assert rel(g["lam"], lam_o) <= tol, rel(g["lam"], lam_o)
+    assert rel(g["usub"], u_o) <= tol, rel(g["usub"], u_o)
+    assert np.allclose(g["hist"], hist_o[1:], rtol=max(tol, 1e-9) * 100, atol=0)
+    r_o = O.residual(problem_from(inp), O.ddm_gather(st))
+    assert abs(g["ginfo"].rel_residual - r_o) <= (1e-6 if prec == hz.HZ_F64 else 1e-2) * r_o
+    # the basis vectors have the size of the interface data, not of the joint state
+    assert g["ginfo"].krylov_bytes * 5 < (restart + 3) * g["usub"].size * (8 if prec == hz.HZ_F64 else 4)
+
+
+def test_lambda_only_gmres_reaches_the_direct_solution_with_tight_subdomain_solves():
+    """Config 1, rho = 1 (eq. (2) literally), 40 cold-started WaveHoltz iterations per sweep: the fixed point of the
+    lambda-only map is then the discrete solution to 1e-8 (oracle pin of the same statement)."""
+    if not torch.cuda.is_available():
+        pytest.fail("CUDA device required")
+    inp = make_config(1)
+    ustar = O.direct_solve(problem_from(inp))
+    g = gpu_gmres(inp, hz.HZ_F64, 0, max_steps=60, n_wh=40, relax=1.0, restart=60, lambda_only=True)
+    assert g["ginfo"].lin_residual <= 1e-8        # (the oracle's history stagnates at 3.5e-9: the Krylov space is exhausted)
+    assert rel(g["u"], ustar) < 1e-8
+    assert g["ginfo"].rel_residual < 1e-7
