@@ -656,7 +656,7 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
     int G = 1;
     if (t.pk) {
       // G subdomains per block: the G*NB full tiles fill whole bulk warps (hz_sweep_pack.cuh)
-      const int NB = (q.ntx - 1) * (q.nty - 1), NE = q.ntx + q.nty - 1;
+      const int NB = (q.ntx - 1) * (q.nty - 1), NE = q.ntx + q.nty - 2;   // (the last top piece carries the corner node)
       if (n_t > kTabCMax) return false;
       if (NB > 16 || fl.pack == 1) return false;   // packing only pays below one warp of full tiles
       // own part of a step before (pk = 2) or after (pk = 1) the block barrier: measured per shape on config 5
@@ -667,7 +667,7 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
       const size_t v16 = 16 / rs;
       const size_t chx = ((size_t)q.TX + v16 - 1) / v16 * v16, chy = ((size_t)q.TY + v16 - 1) / v16 * v16;
       const size_t rsw = 2 * chx + 2 * chy + v16;  // square tiles: 4 chunks + 16 bytes
-      const size_t nep = ((size_t)NE + v16 - 1) / v16 * v16;
+      const size_t nep = ((size_t)NE + 1 + v16 - 1) / v16 * v16;
       auto shape = [&](int g, int *thr, size_t *smb) {
         *thr = roundup(g * NB, 32) + roundup(g * NE, 32);
         *smb = 2 * ((size_t)g * ((size_t)(q.ntx * q.nty + 1) * rsw + 2 * nep) + rsw) * rs;

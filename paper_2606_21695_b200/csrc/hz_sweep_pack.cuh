@@ -15,6 +15,11 @@
 
 namespace hz {
 
+// a product that the compiler may not contract into a following addition (keeps the corner node's sums in the
+// association the piece code uses: mul, then add)
+__device__ __forceinline__ float mul_rn(float a, float b) { return __fmul_rn(a, b); }
+__device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(a, b); }
+
 // (a register cap for two blocks of 256 threads per SM gains 5-10 % on the 4-tile subdomains and loses 10-45 % on the
 // 16-tile ones and in fp64: not used)
 // PRE: the neighbour-independent part of a step (own-tile line sums, the cos-filter sum of Re u) runs BEFORE the block
@@ -31,9 +36,9 @@ __global__ void __launch_bounds__(MAXT, 1) k_sweep_pack(const SweepArgs<real> A,
   const int NTH = blockDim.x, h = threadIdx.x, G = A.pack;
   const int ntx = A.lay.ntx, nty = A.lay.nty, NTV = A.lay.NT, NS = A.lay.NS;
   const int lnx = A.lay.lnx, lny = A.lay.lny;
-  const int NB = (ntx - 1) * (nty - 1), NE = ntx + nty - 1;
+  const int NB = (ntx - 1) * (nty - 1), NE = ntx + nty - 2;   // edge pieces per subdomain (the last top piece also owns the corner node)
   const int bulkW = (G * NB + 31) & ~31;         // lanes of the bulk warps
-  const int NEP = (NE + V16 - 1) / V16 * V16;
+  const int NEP = (NE + 1 + V16 - 1) / V16 * V16;   // PA / RA entries: one per piece + the corner node's raw value
   const int ZR = NTV;                            // the zero record of a slice
   const int EAO = (NTV + 1) * RS;                // in a slice, after the records: PA[NEP] | RA[NEP]
   const int SW = EAO + 2 * NEP;                  // words per subdomain slice
@@ -267,8 +272,10 @@ __global__ void __launch_bounds__(MAXT, 1) k_sweep_pack(const SweepArgs<real> A,
   } else {
     // ============================ edge pieces: one line of T nodes per lane ============================
     // piece e < nty-1: right piece, virtual tile (ntx-1, e), nodes (lnx-1, e*T + n), "along" = y.
-    // piece e >= nty-1: top piece, virtual tile (e-(nty-1), nty-1), nodes (tx*T + n, lny-1), "along" = x;
-    //                   the last one (tx = ntx-1) is the corner and owns node 0 only.
+    // piece e >= nty-1: top piece, virtual tile (e-(nty-1), nty-1), nodes (tx*T + n, lny-1), "along" = x.
+    // The corner node (lnx-1, lny-1) -- node 0 of virtual tile (ntx-1, nty-1) -- has no lane of its own: the lane of the
+    // LAST top piece (tx = ntx-2) carries it as one extra node (same operations, same association as a piece of its
+    // own would apply), so that a subdomain has ntx + nty - 2 pieces: 16 at 8x8 tiles, two subdomains per edge warp.
     const int eh = h - bulkW;
     const int g = eh / NE, e = eh - g * NE;
     const int l = blockIdx.x * G + g;
@@ -289,8 +296,12 @@ __global__ void __launch_bounds__(MAXT, 1) k_sweep_pack(const SweepArgs<real> A,
     real *pPAout = !act ? scr : ((!top && ty == nty - 2) ? sl + v * RS + 2 * CH : sl + EAO + e);
     real *pRAout = !act ? scr + 1 : sl + EAO + NEP + e;
     const real *pP = hasP ? sl + EAO + e - 1 : sl + ZR * RS;
-    const real *pN = hasN ? sl + EAO + NEP + ((!top && ty == nty - 2) ? NE - 1 : e + 1) : sl + ZR * RS;
+    const real *pN = hasN ? sl + EAO + NEP + ((!top && ty == nty - 2) ? NE : e + 1) : sl + ZR * RS;   // RA[NE]: the corner node
     const real *pC = sl + (act ? v - sc : ZR) * RS + oPC;
+    const bool isLT = act && top && tx == ntx - 2;       // carries the corner node
+    const int vC = (nty - 1) * ntx + ntx - 1;            // the corner's virtual tile
+    real *pRAc = isLT ? sl + EAO + NEP + NE : scr + 2;   // its raw value, read by the last right piece and by this lane
+    const real *pCc = sl + (isLT ? vC - ntx : ZR) * RS + 2 * CH;   // the last right piece's partial (element 0 of its PY chunk)
     Elem1D<real> ka;  // coefficients along
 #pragma unroll
     for (int c = 0; c <= P; ++c) {
@@ -324,7 +335,6 @@ __global__ void __launch_bounds__(MAXT, 1) k_sweep_pack(const SweepArgs<real> A,
     const int len1 = top ? lnx : lny;
     int side2 = -1, idx2 = 0;
     if (act && top && tx == 0 && six > 0) { side2 = kSideW; idx2 = lny - 1; }
-    if (act && top && tx == ntx - 1 && six < A.sx - 1) { side2 = kSideE; idx2 = lny - 1; }
     if (act && !top && ty == 0 && siy > 0) { side2 = kSideS; idx2 = lnx - 1; }
 #pragma unroll
     for (int n = 0; n < T; ++n) {
@@ -340,6 +350,27 @@ __global__ void __launch_bounds__(MAXT, 1) k_sweep_pack(const SweepArgs<real> A,
       bbr[0] = fmaT(s, A.lam[lbase + (side2 * 2 + 0) * A.E + idx2], bbr[0]);
       bbi[0] = fmaT(s, A.lam[lbase + (side2 * 2 + 1) * A.E + idx2], bbi[0]);
     }
+    // the corner node: on side N (if that is an interface) at index lnx-1 and on side E at index lny-1
+    real pc = 0, pdc = 0, vrc = 0, vic = 0, urc = 0, uic = 0, gamc = 0, bbrc = 0, alc_ = 0, bbic = 0;
+    const size_t oC = (size_t)lc * NS + vC;
+    const bool cN = isLT && siy < A.sy - 1, cE = isLT && six < A.sx - 1;
+    if (isLT) {
+      gamc = A.gamma[oC]; bbrc = A.bbf_re[oC]; alc_ = A.alpha[oC];
+      bbic = A.bbf_im ? A.bbf_im[oC] : real(0);
+      urc = A.warm ? A.u_sub[(size_t)lc * 2 * NS + vC] : real(0);
+      uic = A.warm ? A.u_sub[(size_t)lc * 2 * NS + NS + vC] : real(0);
+      if (cN) {
+        const real s = A.bs[ebase + kSideN * A.E + lnx - 1];
+        bbrc = fmaT(s, A.lam[lbase + (kSideN * 2 + 0) * A.E + lnx - 1], bbrc);
+        bbic = fmaT(s, A.lam[lbase + (kSideN * 2 + 1) * A.E + lnx - 1], bbic);
+      }
+      if (cE) {
+        const real s = A.bs[ebase + kSideE * A.E + lny - 1];
+        bbrc = fmaT(s, A.lam[lbase + (kSideE * 2 + 0) * A.E + lny - 1], bbrc);
+        bbic = fmaT(s, A.lam[lbase + (kSideE * 2 + 1) * A.E + lny - 1], bbic);
+      }
+    }
+    const real d0ac = real(0) + A.ex1.kp[P];   // along x: only the element before the corner exists
     bar_sync_all(NTH);
 
     int cur = 0;
@@ -352,19 +383,27 @@ __global__ void __launch_bounds__(MAXT, 1) k_sweep_pack(const SweepArgs<real> A,
         vr[n] = t0.k * p[n];
         vi[n] = t0.kh * pd[n];
       }
+      pc = urc;
+      pdc = A.omega * (uic * A.cos_h - urc * A.sin_h);
+      vrc = t0.k * pc;
+      vic = t0.kh * pdc;
 #pragma unroll 1
       for (int nu = 1; nu < A.n_t; ++nu) {
         real q[T + 1];
 #pragma unroll
         for (int n = 0; n < T; ++n) { p[n] = fmaT(sigma, pd[n], p[n]); q[n] = p[n]; }
         q[T] = real(0);
-        pPAout[cur] = line_partial<real, P, M>(q, ka);
+        const real pa = line_partial<real, P, M>(q, ka);
+        pPAout[cur] = pa;
         pRAout[cur] = p[0];
         st_chunk<T>(pRaw + cur, p);
+        pc = fmaT(sigma, pdc, pc);
+        pRAc[cur] = pc;
         bar_sync_all(NTH);
         const real qN = pN[cur], piP = pP[cur];
         real piC[T];
         ld_chunk<T>(pC + cur, piC);
+        const real piCc = pCc[cur];
         cur = BUFW - cur;
         const Tab4<real> tn = TC.t[nu];
         real S[T];
@@ -382,11 +421,37 @@ __global__ void __launch_bounds__(MAXT, 1) k_sweep_pack(const SweepArgs<real> A,
           pd[n] = fmaT(al[n], pd[n], x);
           vi[n] = fmaT(tn.kh, pd[n], vi[n]);
         }
+        if (isLT) {   // the corner node: along x after the last top piece (its partial `pa`), across y after the last right piece
+          const real cownc = d0c * pc;
+          vrc = fmaT(tn.k, pc, vrc);
+          real Sc = real(2) * (mul_rn(d0ac, pc) + pa);
+          Sc = fmaT(s0c, cownc + piCc, Sc);
+          real x = fmaT(-gamc, Sc, bbrc * tn.c);
+          x = fmaT(bbic, tn.s, x);
+          pdc = fmaT(alc_, pdc, x);
+          vic = fmaT(tn.kh, pdc, vic);
+        }
       }
 #pragma unroll
       for (int n = 0; n < T; ++n) {
         ur[n] = A.two_over_nt * vr[n];
         ui[n] = A.two_over_nt * vi[n];
+      }
+      urc = A.two_over_nt * vrc;
+      uic = A.two_over_nt * vic;
+    }
+    if (isLT) {
+      A.u_sub[(size_t)l * 2 * NS + vC] = urc;
+      A.u_sub[(size_t)l * 2 * NS + NS + vC] = uic;
+      if (cN) {
+        const real k2 = A.k2edge[ebase + kSideN * A.E + lnx - 1];
+        A.gout[lbase + (kSideN * 2 + 0) * A.E + lnx - 1] = fmaT(k2, uic, -A.lam[lbase + (kSideN * 2 + 0) * A.E + lnx - 1]);
+        A.gout[lbase + (kSideN * 2 + 1) * A.E + lnx - 1] = fmaT(-k2, urc, -A.lam[lbase + (kSideN * 2 + 1) * A.E + lnx - 1]);
+      }
+      if (cE) {
+        const real k2 = A.k2edge[ebase + kSideE * A.E + lny - 1];
+        A.gout[lbase + (kSideE * 2 + 0) * A.E + lny - 1] = fmaT(k2, uic, -A.lam[lbase + (kSideE * 2 + 0) * A.E + lny - 1]);
+        A.gout[lbase + (kSideE * 2 + 1) * A.E + lny - 1] = fmaT(-k2, urc, -A.lam[lbase + (kSideE * 2 + 1) * A.E + lny - 1]);
       }
     }
     if (act) {
@@ -394,7 +459,7 @@ __global__ void __launch_bounds__(MAXT, 1) k_sweep_pack(const SweepArgs<real> A,
       for (int n = 0; n < T; ++n) {
         const size_t o = (size_t)(top ? n : n * T) * NTV + v;
         const int idx = ta * T + n;
-        if (idx < len1) {   // (the corner piece owns node 0 only)
+        if (idx < len1) {
           A.u_sub[(size_t)l * 2 * NS + o] = ur[n];
           A.u_sub[(size_t)l * 2 * NS + NS + o] = ui[n];
         }
