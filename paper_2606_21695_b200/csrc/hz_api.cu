@@ -658,11 +658,20 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
       // G subdomains per block: the G*NB full tiles fill whole bulk warps (hz_sweep_pack.cuh)
       const int NB = (q.ntx - 1) * (q.nty - 1), NE = q.ntx + q.nty - 2;   // (the last top piece carries the corner node)
       if (n_t > kTabCMax) return false;
-      if (NB > 16 || fl.pack == 1) return false;   // packing only pays below one warp of full tiles
-      // own part of a step before (pk = 2) or after (pk = 1) the block barrier: measured per shape on config 5
-      // (hz_sweep_pack.cuh, profiles/r02_config_sweep.md)
-      const bool pre = NB < 16 || t.mx == 1 || (rs == 8 && P == 1);
-      if ((t.pk == 2) != pre) return false;
+      if (fl.pack == 1) return false;
+      // pk = 3: TWO subdomains of up to 64 full tiles per block, their 2 x (ntx + nty - 2) <= 32 edge pieces in ONE edge
+      // warp (the headline shape: 8 x 8 tiles); only when the grid still fills the register-capped occupancy
+      const bool pair = t.pk == 3;
+      if (pair) {
+        if (NB <= 16 || NB > 64 || 2 * NE > 32 || (fl.pack > 1 && fl.pack != 2)) return false;
+        if (fl.pack == 0 && (Lsel + 1) / 2 < (long long)sm_count * t.minb) return false;
+      } else {
+        if (NB > 16) return false;   // packing several subdomains per warp only pays below one warp of full tiles
+        // own part of a step before (pk = 2) or after (pk = 1) the block barrier: measured per shape on config 5
+        // (hz_sweep_pack.cuh, profiles/r02_config_sweep.md)
+        const bool pre = NB < 16 || t.mx == 1 || (rs == 8 && P == 1);
+        if ((t.pk == 2) != pre) return false;
+      }
       auto gcd = [](int a, int b) { while (b) { const int r = a % b; a = b; b = r; } return a; };
       const size_t v16 = 16 / rs;
       const size_t chx = ((size_t)q.TX + v16 - 1) / v16 * v16, chy = ((size_t)q.TY + v16 - 1) / v16 * v16;
@@ -672,7 +681,9 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
         *thr = roundup(g * NB, 32) + roundup(g * NE, 32);
         *smb = 2 * ((size_t)g * ((size_t)(q.ntx * q.nty + 1) * rsw + 2 * nep) + rsw) * rs;
       };
-      if (fl.pack > 1) {
+      if (pair) {
+        G = 2;
+      } else if (fl.pack > 1) {
         G = fl.pack;
       } else {
         G = 32 / gcd(32, NB);                        // smallest G that fills the bulk warps ...

@@ -68,12 +68,17 @@ namespace hz {
   {P, M, M, CSM, MAXT, 1, MINB, 1, (const void *)k_sweep_ws<float, P, M, (CSM != 0), MAXT, MINB>},
 #define C_ENTRY(P, MX, MY, CL, MAXT, MINB) \
   {P, MX, MY, 0, MAXT, 0, MINB, CL, (const void *)k_sweep_cl<float, P, MX, MY, CL, MAXT, MINB>},
+// K2(P, M, MAXT, MINB): two 64-tile subdomains per block sharing one edge warp (pk = 3)
+#define HZ_PK2_TABLE_F32(K2) \
+  K2(3, 1, 160, 4)
+#define K2_ENTRY(P, M, MAXT, MINB) \
+  {P, M, M, 0, MAXT, 1, MINB, 1, (const void *)k_sweep_pack<float, P, M, MAXT, true, MINB>, 3},
 #define K_ENTRY(P, M, MAXT)                                                          \
   {P, M, M, 0, MAXT, 1, 1, 1, (const void *)k_sweep_pack<float, P, M, MAXT, false>, 1}, \
   {P, M, M, 0, MAXT, 1, 1, 1, (const void *)k_sweep_pack<float, P, M, MAXT, true>, 2},
 #define CW_ENTRY(P, MX, MY, CL, MAXT, MINB) \
   {P, MX, MY, 0, MAXT, 1, MINB, CL, (const void *)k_sweep_cw<float, P, MX, MY, CL, MAXT, MINB>},
-static const TileEntry kTilesF32[] = {HZ_CW_TABLE_F32(CW_ENTRY) HZ_WS_TABLE_F32(W_ENTRY) HZ_TILE_TABLE_F32(X_ENTRY) HZ_CL_TABLE_F32(C_ENTRY) HZ_PK_TABLE_F32(K_ENTRY)};
+static const TileEntry kTilesF32[] = {HZ_CW_TABLE_F32(CW_ENTRY) HZ_WS_TABLE_F32(W_ENTRY) HZ_TILE_TABLE_F32(X_ENTRY) HZ_CL_TABLE_F32(C_ENTRY) HZ_PK_TABLE_F32(K_ENTRY) HZ_PK2_TABLE_F32(K2_ENTRY)};
 #undef K_ENTRY
 #undef C_ENTRY
 #undef X_ENTRY

@@ -11,6 +11,7 @@
 // unrounded tile count as their stride (Layout::NT = ntx*nty), so a 25-DOF subdomain occupies 36 slots, not 128.
 // One named barrier per time step for the whole block: all subdomains share N_t and run in lockstep.
 #pragma once
+#include <type_traits>
 #include "hz_line.cuh"
 
 namespace hz {
@@ -26,9 +27,15 @@ __device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(
 // barrier, as in k_sweep_cw, so the wait overlaps arithmetic: faster where a subdomain has fewer than 16 full tiles
 // (one or two bulk warps per block), at M = 1 and in fp64 at p = 1; slower for the 16-tile M > 1 shapes, which keep
 // the order of k_sweep_ws (profiles/r02_config_sweep.md).  Same sums, same association: results are bit-identical.
-template <typename real, int P, int M, int MAXT, bool PRE>
-__global__ void __launch_bounds__(MAXT, 1) k_sweep_pack(const SweepArgs<real> A, const __grid_constant__ TabC<real> TC) {
+// MINB > 1: register-capped instantiation for TWO 64-tile subdomains per block (4 bulk warps + ONE edge warp of 2 x 16
+// pieces, instead of two blocks of 2 bulk warps + 1 half-empty edge warp each): the edge warp's instruction stream is
+// then paid once per two subdomains.  In fp32 it also issues the element-wise updates as packed pairs (FFMA2), as
+// k_sweep_ws does.
+template <typename real, int P, int M, int MAXT, bool PRE, int MINB = 1>
+__global__ void __launch_bounds__(MAXT, MINB) k_sweep_pack(const SweepArgs<real> A, const __grid_constant__ TabC<real> TC) {
   constexpr int T = M * P;
+  constexpr bool PK = std::is_same<real, float>::value && MINB > 1 && T >= 2;
+  constexpr int NP = PK ? T / 2 : 0;
   constexpr int V16 = 16 / (int)sizeof(real);
   constexpr int CH = (T + V16 - 1) / V16 * V16;
   constexpr int RS = 4 * CH + V16;  // record: PX | RX | PY | RY + 16 bytes (odd number of 16-byte units)
@@ -133,9 +140,18 @@ __global__ void __launch_bounds__(MAXT, 1) k_sweep_pack(const SweepArgs<real> A,
 #pragma unroll 1
       for (int nu = 1; nu < A.n_t; ++nu) {
 #pragma unroll
-        for (int b = 0; b < T; ++b)
+        for (int b = 0; b < T; ++b) {
+          if constexpr (PK) {
 #pragma unroll
-          for (int a = 0; a < T; ++a) p[b][a] = fmaT(sigma, pd[b][a], p[b][a]);
+            for (int j = 0; j < NP; ++j) {
+              const int a = 2 * j;
+              un2(fmaT(mk2(sigma, sigma), mk2(pd[b][a], pd[b][a + 1]), mk2(p[b][a], p[b][a + 1])), p[b][a], p[b][a + 1]);
+            }
+          }
+#pragma unroll
+          for (int a = 0; a < T; ++a)
+            if (a >= 2 * NP) p[b][a] = fmaT(sigma, pd[b][a], p[b][a]);
+        }
         {
           real *my = pMy + cur;
           real oPX[T], oRX[T], oPY[T], oRY[T];
@@ -192,9 +208,18 @@ __global__ void __launch_bounds__(MAXT, 1) k_sweep_pack(const SweepArgs<real> A,
           for (int b = 1; b < T; ++b) S[b][a] = Sc[b];
         }
 #pragma unroll
-        for (int b = 0; b < T; ++b)
+        for (int b = 0; b < T; ++b) {
+          if constexpr (PK) {
 #pragma unroll
-          for (int a = 0; a < T; ++a) vr[b][a] = fmaT(tn.k, p[b][a], vr[b][a]);
+            for (int j = 0; j < NP; ++j) {
+              const int a = 2 * j;
+              un2(fmaT(mk2(tn.k, tn.k), mk2(p[b][a], p[b][a + 1]), mk2(vr[b][a], vr[b][a + 1])), vr[b][a], vr[b][a + 1]);
+            }
+          }
+#pragma unroll
+          for (int a = 0; a < T; ++a)
+            if (a >= 2 * NP) vr[b][a] = fmaT(tn.k, p[b][a], vr[b][a]);
+        }
         if (PRE) {
           bar_sync_all(NTH);
           ld_chunk<T>(pL + cur, piL);
@@ -231,8 +256,17 @@ __global__ void __launch_bounds__(MAXT, 1) k_sweep_pack(const SweepArgs<real> A,
             } else {  // interior of the subdomain: alpha = 1, Im b = 0
               pd[b][a] = fmaT(r_, tn.c, fmaT(-g_, S[b][a], pd[b][a]));
             }
-            vi[b][a] = fmaT(tn.kh, pd[b][a], vi[b][a]);
+            if (a >= 2 * NP) vi[b][a] = fmaT(tn.kh, pd[b][a], vi[b][a]);
           }
+        if constexpr (PK) {
+#pragma unroll
+          for (int b = 0; b < T; ++b)
+#pragma unroll
+            for (int j = 0; j < NP; ++j) {
+              const int a = 2 * j;
+              un2(fmaT(mk2(tn.kh, tn.kh), mk2(pd[b][a], pd[b][a + 1]), mk2(vi[b][a], vi[b][a + 1])), vi[b][a], vi[b][a + 1]);
+            }
+        }
       }
 #pragma unroll
       for (int b = 0; b < T; ++b)
