@@ -68,9 +68,13 @@ namespace hz {
   {P, M, M, CSM, MAXT, 1, MINB, 1, (const void *)k_sweep_ws<float, P, M, (CSM != 0), MAXT, MINB>},
 #define C_ENTRY(P, MX, MY, CL, MAXT, MINB) \
   {P, MX, MY, 0, MAXT, 0, MINB, CL, (const void *)k_sweep_cl<float, P, MX, MY, CL, MAXT, MINB>},
-// K2(P, M, MAXT, MINB): two 64-tile subdomains per block sharing one edge warp (pk = 3)
+// K2(P, M, MAXT, MINB): two 64-tile subdomains per block sharing one edge warp (pk = 3).  Measured on config 5 against
+// k_sweep_ws: p = 3 side 8 18.92 -> 17.39 ms, p = 1 side 32 11.33 -> 9.23 ms; p = 4 side 8 (19.50 -> 20.57) and p = 2
+// side 16 (12.30 -> 12.67) are slower that way and keep k_sweep_ws.  Register cap of the p = 3 entry: 4 blocks per SM
+// (96 registers) 17.39 ms, 3 blocks 18.31 ms, 5 blocks 20.90 ms
 #define HZ_PK2_TABLE_F32(K2) \
-  K2(3, 1, 160, 4)
+  K2(3, 1, 160, 4)         \
+  K2(1, 4, 160, 2)
 #define K2_ENTRY(P, M, MAXT, MINB) \
   {P, M, M, 0, MAXT, 1, MINB, 1, (const void *)k_sweep_pack<float, P, M, MAXT, true, MINB>, 3},
 #define K_ENTRY(P, M, MAXT)                                                          \

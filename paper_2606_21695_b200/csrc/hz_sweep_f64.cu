@@ -70,9 +70,13 @@ namespace hz {
   {P, M, M, CSM, MAXT, 1, MINB, 1, (const void *)k_sweep_ws<double, P, M, (CSM != 0), MAXT, MINB>},
 #define C_ENTRY(P, MX, MY, CL, MAXT, MINB) \
   {P, MX, MY, 0, MAXT, 0, MINB, CL, (const void *)k_sweep_cl<double, P, MX, MY, CL, MAXT, MINB>},
-// K2(P, M, MAXT, MINB): two 64-tile subdomains per block sharing one edge warp (pk = 3)
+// K2(P, M, MAXT, MINB): two 64-tile subdomains per block sharing one edge warp (pk = 3).  Measured on config 5 against
+// k_sweep_ws: p = 3 side 8 37.27 -> 35.01 ms, p = 2 side 16 40.36 -> 37.30 ms; p = 4 side 8 (61.1 -> 64.7) and p = 1
+// side 32 (26.0 -> 27.3) are slower that way and keep k_sweep_ws.  Register cap of the p = 3 entry: 2 blocks per SM
+// (168 registers) 35.0 ms, 3 blocks 39.2 ms, uncapped 39.8 ms
 #define HZ_PK2_TABLE_F64(K2) \
-  K2(3, 1, 160, 2)
+  K2(3, 1, 160, 2)         \
+  K2(2, 2, 160, 1)
 #define K2_ENTRY(P, M, MAXT, MINB) \
   {P, M, M, 0, MAXT, 1, MINB, 1, (const void *)k_sweep_pack<double, P, M, MAXT, true, MINB>, 3},
 #define K_ENTRY(P, M, MAXT)                                                          \
