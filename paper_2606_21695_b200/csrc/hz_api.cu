@@ -664,6 +664,7 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
       const bool pair = t.pk == 3;
       if (pair) {
         if (NB <= 16 || NB > 64 || 2 * NE > 32 || (fl.pack > 1 && fl.pack != 2)) return false;
+        if (t.ntx > 0 && (q.ntx != t.ntx || q.nty != t.ntx)) return false;   // compiled for that tile grid
         if (fl.pack == 0 && (Lsel + 1) / 2 < (long long)sm_count * t.minb) return false;
       } else {
         if (NB > 16) return false;   // packing several subdomains per warp only pays below one warp of full tiles
@@ -679,7 +680,8 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
       const size_t nep = ((size_t)NE + 1 + v16 - 1) / v16 * v16;
       auto shape = [&](int g, int *thr, size_t *smb) {
         *thr = roundup(g * NB, 32) + roundup(g * NE, 32);
-        *smb = 2 * ((size_t)g * ((size_t)(q.ntx * q.nty + 1) * rsw + 2 * nep) + rsw) * rs;
+        // per buffer: g slices of (padded record grid + zero record + PA | RA) and the scratch region of the idle lanes
+        *smb = 2 * ((size_t)g * ((size_t)((q.ntx + 1) * (q.nty + 1) + 1) * rsw + 2 * nep) + (size_t)(2 * (q.ntx + 1) + 3) * rsw) * rs;
       };
       if (pair) {
         G = 2;

@@ -101,6 +101,8 @@ struct TileEntry {
   const void *fn;
   int pk;                    // > 0: packed small-subdomain kernel (hz_sweep_pack.cuh), several subdomains per block;
                              // 2: its PRE instantiation (own part of a step before the block barrier)
+                             // 3: two subdomains of up to 64 full tiles per block (one shared edge warp)
+  int ntx;                   // pk = 3: > 0: compiled for ntx = nty = this many thread tiles per side
 };
 
 struct SweepLaunch {

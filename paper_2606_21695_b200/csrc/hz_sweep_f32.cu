@@ -76,7 +76,7 @@ namespace hz {
   K2(3, 1, 160, 4)         \
   K2(1, 4, 160, 2)
 #define K2_ENTRY(P, M, MAXT, MINB) \
-  {P, M, M, 0, MAXT, 1, MINB, 1, (const void *)k_sweep_pack<float, P, M, MAXT, true, MINB>, 3},
+  {P, M, M, 0, MAXT, 1, MINB, 1, (const void *)k_sweep_pack<float, P, M, MAXT, true, MINB, 9>, 3, 9},
 #define K_ENTRY(P, M, MAXT)                                                          \
   {P, M, M, 0, MAXT, 1, 1, 1, (const void *)k_sweep_pack<float, P, M, MAXT, false>, 1}, \
   {P, M, M, 0, MAXT, 1, 1, 1, (const void *)k_sweep_pack<float, P, M, MAXT, true>, 2},

@@ -78,7 +78,7 @@ namespace hz {
   K2(3, 1, 160, 2)         \
   K2(2, 2, 160, 1)
 #define K2_ENTRY(P, M, MAXT, MINB) \
-  {P, M, M, 0, MAXT, 1, MINB, 1, (const void *)k_sweep_pack<double, P, M, MAXT, true, MINB>, 3},
+  {P, M, M, 0, MAXT, 1, MINB, 1, (const void *)k_sweep_pack<double, P, M, MAXT, true, MINB, 9>, 3, 9},
 #define K_ENTRY(P, M, MAXT)                                                          \
   {P, M, M, 0, MAXT, 1, 1, 1, (const void *)k_sweep_pack<double, P, M, MAXT, false>, 1}, \
   {P, M, M, 0, MAXT, 1, 1, 1, (const void *)k_sweep_pack<double, P, M, MAXT, true>, 2},

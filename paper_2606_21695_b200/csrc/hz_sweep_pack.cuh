@@ -31,7 +31,12 @@ __device__ __forceinline__ double mul_rn(double a, double b) { return __dmul_rn(
 // pieces, instead of two blocks of 2 bulk warps + 1 half-empty edge warp each): the edge warp's instruction stream is
 // then paid once per two subdomains.  In fp32 it also issues the element-wise updates as packed pairs (FFMA2), as
 // k_sweep_ws does.
-template <typename real, int P, int M, int MAXT, bool PRE, int MINB = 1>
+// Records live on a PADDED grid of (ntx + 1) x (nty + 1) per subdomain: virtual tile (tx, ty) at index (ty + 1)(ntx + 1) +
+// tx + 1, column -1 and row -1 never written (zero).  Every full tile then finds its four neighbours at the same offsets
+// from its own record (-1, +1, -(ntx+1), +(ntx+1) records), so the time loop keeps ONE pointer per thread (own record in
+// the current buffer) instead of five; NTX > 0 fixes ntx = nty = NTX at compile time and the offsets become immediates
+// of the load instructions (17 of 181 instructions per step were address arithmetic).
+template <typename real, int P, int M, int MAXT, bool PRE, int MINB = 1, int NTX = 0>
 __global__ void __launch_bounds__(MAXT, MINB) k_sweep_pack(const SweepArgs<real> A, const __grid_constant__ TabC<real> TC) {
   constexpr int T = M * P;
   constexpr bool PK = std::is_same<real, float>::value && MINB > 1 && T >= 2;
@@ -41,17 +46,18 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_pack(const SweepArgs<real>
   constexpr int RS = 4 * CH + V16;  // record: PX | RX | PY | RY + 16 bytes (odd number of 16-byte units)
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int NTH = blockDim.x, h = threadIdx.x, G = A.pack;
-  const int ntx = A.lay.ntx, nty = A.lay.nty, NTV = A.lay.NT, NS = A.lay.NS;
+  const int ntx = NTX > 0 ? NTX : A.lay.ntx, nty = NTX > 0 ? NTX : A.lay.nty, NTV = A.lay.NT, NS = A.lay.NS;
   const int lnx = A.lay.lnx, lny = A.lay.lny;
   const int NB = (ntx - 1) * (nty - 1), NE = ntx + nty - 2;   // edge pieces per subdomain (the last top piece also owns the corner node)
+  const int NXP = ntx + 1, NREC = NXP * (nty + 1);            // padded record grid
   const int bulkW = (G * NB + 31) & ~31;         // lanes of the bulk warps
   const int NEP = (NE + 1 + V16 - 1) / V16 * V16;   // PA / RA entries: one per piece + the corner node's raw value
-  const int ZR = NTV;                            // the zero record of a slice
-  const int EAO = (NTV + 1) * RS;                // in a slice, after the records: PA[NEP] | RA[NEP]
+  const int ZR = NREC;                           // the zero record of a slice (edge pieces without a neighbour along)
+  const int EAO = (NREC + 1) * RS;               // in a slice, after the records: PA[NEP] | RA[NEP]
   const int SW = EAO + 2 * NEP;                  // words per subdomain slice
-  const int BUFW = G * SW + RS;                  // per buffer: G slices + one scratch record for idle lanes
+  const int BUFW = G * SW + (2 * NXP + 3) * RS;  // per buffer: G slices + a scratch region for idle lanes
   real *xb = reinterpret_cast<real *>(smem_raw);
-  const int SCRo = G * SW;                       // offset of the scratch record
+  const int SCRo = G * SW + (NXP + 1) * RS;      // the scratch record: the middle of that region (its neighbour offsets stay inside)
 
   for (int q = h; q < 2 * BUFW; q += NTH) xb[q] = real(0);
   const real sigma = A.sigma;
@@ -64,10 +70,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_pack(const SweepArgs<real>
     const int tx = act ? t % (ntx - 1) : 0, ty = act ? t / (ntx - 1) : 0;
     const int v = ty * ntx + tx;
     real *sl = xb + (act ? g : 0) * SW;          // this subdomain's slice (buffer 0)
-    real *pMy = act ? sl + v * RS : xb + SCRo;
-    const real *pL = sl + ((act && tx > 0) ? v - 1 : ZR) * RS, *pR = sl + (act ? v + 1 : ZR) * RS;
-    const real *pD = sl + ((act && ty > 0) ? v - ntx : ZR) * RS, *pU = sl + (act ? v + ntx : ZR) * RS;
-    real *pMyRX = pMy + CH;
+    real *pMy = act ? sl + ((ty + 1) * NXP + tx + 1) * RS : xb + SCRo;
+    const int oD = NXP * RS;                     // record offset of the tile above / below
     const bool hasL = tx > 0, hasD = ty > 0;
     const real d0x = A.ex1.k0[0] + (hasL ? A.ex1.kp[P] : real(0));
     const real d0y = A.ey1.k0[0] + (hasD ? A.ey1.kp[P] : real(0));
@@ -178,15 +182,16 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_pack(const SweepArgs<real>
           st_chunk<T>(my + 2 * CH, oPY);
           st_chunk<T>(my + 3 * CH, oRY);
         }
+        const real *mr = pMy + cur;
         const Tab4<real> tn = TC.t[nu];
         real S[T][T], X0[T], Y0[T];
         real qR[T], piL[T], qU[T], piD[T];
         if (!PRE) {
           bar_sync_all(NTH);
-          ld_chunk<T>(pL + cur, piL);
-          ld_chunk<T>(pR + cur + CH, qR);
-          ld_chunk<T>(pD + cur + 2 * CH, piD);
-          ld_chunk<T>(pU + cur + 3 * CH, qU);
+          ld_chunk<T>(mr - RS, piL);
+          ld_chunk<T>(mr + RS + CH, qR);
+          ld_chunk<T>(mr - oD + 2 * CH, piD);
+          ld_chunk<T>(mr + oD + 3 * CH, qU);
         }
 #pragma unroll
         for (int b = 0; b < T; ++b) {
@@ -222,10 +227,10 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_pack(const SweepArgs<real>
         }
         if (PRE) {
           bar_sync_all(NTH);
-          ld_chunk<T>(pL + cur, piL);
-          ld_chunk<T>(pR + cur + CH, qR);
-          ld_chunk<T>(pD + cur + 2 * CH, piD);
-          ld_chunk<T>(pU + cur + 3 * CH, qU);
+          ld_chunk<T>(mr - RS, piL);
+          ld_chunk<T>(mr + RS + CH, qR);
+          ld_chunk<T>(mr - oD + 2 * CH, piD);
+          ld_chunk<T>(mr + oD + 3 * CH, qU);
         }
         cur = BUFW - cur;
 #pragma unroll
@@ -317,25 +322,26 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_pack(const SweepArgs<real>
     const bool top = act && e >= nty - 1;
     const int tx = !act ? 0 : (top ? e - (nty - 1) : ntx - 1);
     const int ty = !act ? 0 : (top ? nty - 1 : e);
-    const int v = ty * ntx + tx;
+    const int v = ty * ntx + tx;                          // slot in the per-node global arrays
+    const int vq = (ty + 1) * NXP + tx + 1;               // record index (padded grid)
     const int ta = top ? tx : ty, nta = top ? ntx : nty;  // position / count along the line direction
-    const int sc = top ? ntx : 1;                         // virtual-tile stride across
+    const int sc = top ? NXP : 1;                         // record stride across
     const int oRC = top ? 3 * CH : CH, oPC = top ? 2 * CH : 0;
     const bool hasP = act && ta > 0, hasN = act && ta < nta - 1;
     real *sl = xb + (act ? g : 0) * SW;
     real *scr = xb + SCRo;
-    real *pRaw = act ? sl + v * RS + oRC : scr;
+    real *pRaw = act ? sl + vq * RS + oRC : scr;
     // along-the-edge exchange through the compact arrays PA[e], RA[e].  The last right piece's partial sum has one
     // reader, the corner, which reads it as a chunk: it goes to element 0 of that piece's own PY chunk.
-    real *pPAout = !act ? scr : ((!top && ty == nty - 2) ? sl + v * RS + 2 * CH : sl + EAO + e);
+    real *pPAout = !act ? scr : ((!top && ty == nty - 2) ? sl + vq * RS + 2 * CH : sl + EAO + e);
     real *pRAout = !act ? scr + 1 : sl + EAO + NEP + e;
     const real *pP = hasP ? sl + EAO + e - 1 : sl + ZR * RS;
     const real *pN = hasN ? sl + EAO + NEP + ((!top && ty == nty - 2) ? NE : e + 1) : sl + ZR * RS;   // RA[NE]: the corner node
-    const real *pC = sl + (act ? v - sc : ZR) * RS + oPC;
+    const real *pC = sl + (act ? vq - sc : ZR) * RS + oPC;
     const bool isLT = act && top && tx == ntx - 2;       // carries the corner node
     const int vC = (nty - 1) * ntx + ntx - 1;            // the corner's virtual tile
     real *pRAc = isLT ? sl + EAO + NEP + NE : scr + 2;   // its raw value, read by the last right piece and by this lane
-    const real *pCc = sl + (isLT ? vC - ntx : ZR) * RS + 2 * CH;   // the last right piece's partial (element 0 of its PY chunk)
+    const real *pCc = sl + (isLT ? (nty - 1) * NXP + ntx : ZR) * RS + 2 * CH;   // the last right piece's partial (element 0 of its PY chunk)
     Elem1D<real> ka;  // coefficients along
 #pragma unroll
     for (int c = 0; c <= P; ++c) {
