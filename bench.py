@@ -39,10 +39,10 @@ E2E_SOURCES = 12  # sources of the end-to-end leg (independent of --steps)
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel: STORED figures from one
 # `ncu --set full` capture each (not measured in this run); the summaries are in profiles/.
 STORED_TRAFFIC = {
-    "config5_p3_s8_f32": {"bytes": 1.525e9, "from": "profiles/r02_a_sweep_ws_cfg5_f32.md", "captured": "round 2"},
-    "config5_p3_s8_f64": {"bytes": 2.848e9, "from": "profiles/r02_b_sweep_ws_cfg5_f64.md", "captured": "round 2"},
-    "config3_p3_s8_f32": {"bytes": 72.3e6, "from": "profiles/r01_b_sweep_ws_cfg3_f32.md", "captured": "round 1"},
-    "config3_p3_s8_f64": {"bytes": 140.1e6, "from": "profiles/r01_c_sweep_ws_cfg3_f64.md", "captured": "round 1"},
+    "config5_p3_s8_f32": {"bytes": 1.376e9, "from": "profiles/r02_k_sweep_pack_cfg5_f32.md", "captured": "round 2"},
+    "config5_p3_s8_f64": {"bytes": 2.753e9, "from": "profiles/r02_l_sweep_pack_cfg5_f64.md", "captured": "round 2"},
+    "config3_p3_s8_f32": {"bytes": 62.5e6, "from": "profiles/r02_m_sweep_pack_cfg3_f32.md", "captured": "round 2"},
+    "config3_p3_s8_f64": {"bytes": 137.6e6, "from": "profiles/r02_n_sweep_pack_cfg3_f64.md", "captured": "round 2"},
     "config4_p3_s32_f32": {"bytes": 234.5e6, "from": "profiles/r02_c_sweep_cw_cfg4_f32.md", "captured": "round 2"},
     "config4_p3_s32_f64": {"bytes": 500.5e6, "from": "profiles/r02_d_sweep_cw_cfg4_f64.md", "captured": "round 2"},
 }
@@ -313,7 +313,16 @@ def sweep_rate(hz, inp, prec_name, k, flush, stream, steps=4, warmup=2, **flags)
         tot, swp, exc, _, units = time_sweeps(hz, ctx, steps, warmup, flush, stream)
         rate = units / (sum(swp) * 1e-3)
         quads = inp.vx is not None
-        return {"dof_steps_per_s_sweep_kernel": rate, "sweep_ms": sum(swp) / steps, "exchange_ms": sum(exc) / steps,
+        extra = {}
+        if pinfo.dofs_per_thread == 1 and not quads:
+            # the one-DOF-per-thread layout fetches every operand of the line stencils from shared memory: 2(2p+1) loads and
+            # 1 store per DOF-step; its roofline is the shared-memory pipe (128 B per clock and SM), north_star: "or the
+            # stated L1/shared-bandwidth roofline if that binds"
+            words = 4 * inp.p + 3
+            smem_peak = SMS * 128.0 * SM_MHZ * 1e6
+            extra = {"shared_memory_words_per_dof_step": words,
+                     "frac_of_shared_memory_roofline": rate * words * (4 if prec_name == "f32" else 8) / smem_peak}
+        return {**extra, "dof_steps_per_s_sweep_kernel": rate, "sweep_ms": sum(swp) / steps, "exchange_ms": sum(exc) / steps,
                 "frac_of_derived_peak": rate * flops_per_dof_step(inp.p, quads) / (peak_tflops(prec_name) * 1e12),
                 "kernel": kernel_name(pinfo, quads), "dofs_per_thread": pinfo.dofs_per_thread,
                 "cluster_size": pinfo.cluster_size, "subs_per_block": pinfo.subs_per_block,

@@ -56,6 +56,7 @@ struct hz_ctx {
   bool part = false;
   int sx = 0, sy = 0, ex = 0, ey = 0, L = 0, E = 0, prec = 0;
   int mx = 0, my = 0, csm = 0, ws = 0, cl = 1, entry = -1, pack = 1;
+  int pk = 0;             // the partition launches k_sweep_pack (TileEntry::pk of the chosen entry)
   Layout lay{};
   SweepLaunch launch{};
   hz_part_flags flags{};  // variant-choice controls of the last hz_partition_ex
@@ -91,6 +92,9 @@ struct hz_ctx {
   cudaStream_t cap_stream = nullptr;  // capture happens on this private stream (the legacy default stream cannot capture)
   // hz_ddm_solve_sources: copy-in / copy-out streams, double-buffered staging and the events that order them
   cudaStream_t s_in = nullptr, s_out = nullptr;
+  // the boundary-ring kernel of the global operator runs beside the interior kernel on a stream of its own (fork / join by events)
+  cudaStream_t s_ring = nullptr;
+  cudaEvent_t ev_rfork = nullptr, ev_rjoin = nullptr;
   double *d_fstage[2] = {nullptr, nullptr};
   void *d_ubuf[2] = {nullptr, nullptr};
   size_t ubuf_bytes = 0;
@@ -331,8 +335,10 @@ cudaError_t upload_gather_tables(hz_ctx *c) {
 }
 
 // launches k_helm<inT, acc, P, MODE> on the whole mesh (hz_aux.cuh)
+// overlap_ring: launch the ring kernel on ctx->s_ring, concurrent with the interior kernel (they write disjoint outputs);
+// false = both on `st`, nothing created (hz_residual_static)
 template <typename inT, typename acc, int MODE>
-cudaError_t launch_helm(hz_ctx *ctx, const acc *k2, const void *u_dev, double *part, acc *y, cudaStream_t st) {
+cudaError_t launch_helm(hz_ctx *ctx, const acc *k2, const void *u_dev, double *part, acc *y, cudaStream_t st, bool overlap_ring = true) {
   HelmC<acc> hc{};
   const int P_ = ctx->p;
   for (int a = 0; a <= P_; ++a) {
@@ -383,12 +389,31 @@ cudaError_t launch_helm(hz_ctx *ctx, const acc *k2, const void *u_dev, double *p
     if (e != cudaSuccess) return e;
   }
   const int nix = hg.bxh - 1, niy = hg.byh - 1, nring = hg.gx * hg.gy - nix * niy;
+  const bool both = nix > 0 && niy > 0 && nring > 0;
+  cudaStream_t sr = st;
+  if (both && overlap_ring) {
+    if (!ctx->s_ring) {
+      e = cudaStreamCreateWithFlags(&ctx->s_ring, cudaStreamNonBlocking);
+      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_rfork, cudaEventDisableTiming);
+      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_rjoin, cudaEventDisableTiming);
+      if (e != cudaSuccess) return e;
+    }
+    e = cudaEventRecord(ctx->ev_rfork, st);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(ctx->s_ring, ctx->ev_rfork, 0);
+    if (e != cudaSuccess) return e;
+    sr = ctx->s_ring;
+  }
+  if (nring > 0)
+    fe<<<dim3(nring), block, sm, sr>>>(g, hg, hc, ctx->d_c, k2, ctx->d_fre, ctx->d_fim, ctx->d_bc, (const inT *)u_dev, part, y);
   if (nix > 0 && niy > 0) {
     if (ft) ft<<<dim3(nix, niy), block, smt, st>>>(g, hg, hc, ctx->d_c, k2, ctx->d_fre, ctx->d_fim, (const inT *)u_dev, part, y);
     else fi<<<dim3(nix, niy), block, sm, st>>>(g, hg, hc, ctx->d_c, k2, ctx->d_fre, ctx->d_fim, ctx->d_bc, (const inT *)u_dev, part, y);
   }
-  if (nring > 0)
-    fe<<<dim3(nring), block, sm, st>>>(g, hg, hc, ctx->d_c, k2, ctx->d_fre, ctx->d_fim, ctx->d_bc, (const inT *)u_dev, part, y);
+  if (sr != st) {
+    e = cudaEventRecord(ctx->ev_rjoin, sr);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ctx->ev_rjoin, 0);
+    if (e != cudaSuccess) return e;
+  }
   return cudaGetLastError();
 }
 
@@ -606,6 +631,7 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
   ctx->flags = fl;
   ctx->worder = 0;
   ctx->pack = 1;
+  ctx->pk = 0;
   const int P = ctx->p;
   // ex, ey: elements per subdomain side; for a ragged partition (general quads only, reading R25) the maximum
   ctx->sx = sx; ctx->sy = sy; ctx->ex = (ctx->nx + sx - 1) / sx; ctx->ey = (ctx->ny + sy - 1) / sy;
@@ -661,11 +687,16 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
       if (fl.pack == 1) return false;
       // pk = 3: TWO subdomains of up to 64 full tiles per block, their 2 x (ntx + nty - 2) <= 32 edge pieces in ONE edge
       // warp (the headline shape: 8 x 8 tiles); only when the grid still fills the register-capped occupancy
-      const bool pair = t.pk == 3;
+      // pk = 4: ONE larger subdomain per block through the same kernel (the corner node on the last top piece: 32 edge
+      // pieces = one edge warp at 16 x 16 tiles, where k_sweep_ws needs two)
+      const bool pair = t.pk == 3, single = t.pk == 4;
       if (pair) {
         if (NB <= 16 || NB > 64 || 2 * NE > 32 || (fl.pack > 1 && fl.pack != 2)) return false;
         if (t.ntx > 0 && (q.ntx != t.ntx || q.nty != t.ntx)) return false;   // compiled for that tile grid
         if (fl.pack == 0 && (Lsel + 1) / 2 < (long long)sm_count * t.minb) return false;
+      } else if (single) {
+        if (NB <= 64 || fl.pack > 1) return false;
+        if (t.ntx > 0 && (q.ntx != t.ntx || q.nty != t.ntx)) return false;
       } else {
         if (NB > 16) return false;   // packing several subdomains per warp only pays below one warp of full tiles
         // own part of a step before (pk = 2) or after (pk = 1) the block barrier: measured per shape on config 5
@@ -683,8 +714,8 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
         // per buffer: g slices of (padded record grid + zero record + PA | RA) and the scratch region of the idle lanes
         *smb = 2 * ((size_t)g * ((size_t)((q.ntx + 1) * (q.nty + 1) + 1) * rsw + 2 * nep) + (size_t)(2 * (q.ntx + 1) + 3) * rsw) * rs;
       };
-      if (pair) {
-        G = 2;
+      if (pair || single) {
+        G = pair ? 2 : 1;
       } else if (fl.pack > 1) {
         G = fl.pack;
       } else {
@@ -705,7 +736,7 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
         }
       }
       shape(G, &nthr, &sm);
-      if (G < 2) return false;
+      if (G < 2 && !single) return false;
       ntv_pack = q.ntx * q.nty;
     } else if (t.cl > 1 && t.ws) {
       // cluster kernel with warp-specialised edge pieces (hz_sweep_cw.cuh): the full-tile columns are cut into t.cl strips
@@ -829,6 +860,7 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
     ctx->mx = tiles[best].mx; ctx->my = tiles[best].my; ctx->csm = tiles[best].csm; ctx->ws = tiles[best].ws;
     ctx->cl = tiles[best].cl;
     ctx->pack = tiles[best].pk ? bpack : 1;
+    ctx->pk = tiles[best].pk;
     ctx->entry = best;
     // warp-role order of k_sweep_ws: a 3-warp block (2 bulk + 1 edge) puts its edge warp in the middle, so that the bulk
     // warps of the blocks resident on an SM (consecutive hardware warp slots, slot mod 4 = sub-partition) spread evenly
@@ -920,7 +952,7 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
     if (ctx->lay.variant == 3) kn = "k_sweep_quad";
     else if (ctx->lay.variant == 2) kn = "k_sweep_stream";
     else if (ctx->lay.variant == 1)
-      kn = ctx->pack > 1 ? "k_sweep_pack" : (ctx->cl > 1 ? (ctx->ws ? "k_sweep_cw" : "k_sweep_cl") : (ctx->ws ? "k_sweep_ws" : "k_sweep_tile"));
+      kn = ctx->pk ? "k_sweep_pack" : (ctx->cl > 1 ? (ctx->ws ? "k_sweep_cw" : "k_sweep_cl") : (ctx->ws ? "k_sweep_ws" : "k_sweep_tile"));
     std::snprintf(inf.kernel, sizeof(inf.kernel), "%s", kn);
     *info_out = inf;
   }
@@ -1691,9 +1723,9 @@ hz_status hz_residual_static(hz_ctx *ctx, const void *u_dev, hz_prec u_prec, dou
                                                            ctx->d_bc, (const double *)u_dev, part);
     HZ_CUDA(cudaGetLastError());
   } else if (u_prec == HZ_F32) {
-    HZ_CUDA((launch_helm<float, double, 0>(ctx, nullptr, u_dev, part, nullptr, st)));
+    HZ_CUDA((launch_helm<float, double, 0>(ctx, nullptr, u_dev, part, nullptr, st, false)));
   } else {
-    HZ_CUDA((launch_helm<double, double, 0>(ctx, nullptr, u_dev, part, nullptr, st)));
+    HZ_CUDA((launch_helm<double, double, 0>(ctx, nullptr, u_dev, part, nullptr, st, false)));
   }
   k_reduce2<<<1, 1024, 0, st>>>(part, (int)nb, red);
   HZ_CUDA(cudaGetLastError());
@@ -1754,6 +1786,9 @@ void hz_destroy(hz_ctx *ctx) {
   if (!ctx) return;
   free_partition(ctx);
   if (ctx->cap_stream) cudaStreamDestroy(ctx->cap_stream);
+  if (ctx->s_ring) cudaStreamDestroy(ctx->s_ring);
+  if (ctx->ev_rfork) cudaEventDestroy(ctx->ev_rfork);
+  if (ctx->ev_rjoin) cudaEventDestroy(ctx->ev_rjoin);
   if (ctx->s_in) cudaStreamDestroy(ctx->s_in);
   if (ctx->s_out) cudaStreamDestroy(ctx->s_out);
   for (int b = 0; b < 2; ++b) {

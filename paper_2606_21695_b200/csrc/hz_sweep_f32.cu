@@ -77,12 +77,20 @@ namespace hz {
   K2(1, 4, 160, 2)
 #define K2_ENTRY(P, M, MAXT, MINB) \
   {P, M, M, 0, MAXT, 1, MINB, 1, (const void *)k_sweep_pack<float, P, M, MAXT, true, MINB, 9>, 3, 9},
+// K4(P, M, MAXT, PRE): one subdomain of 16 x 16 tiles per block through the packed kernel (pk = 4: the corner node rides on
+// the last top piece, so the 32 edge pieces fill ONE edge warp where k_sweep_ws needs two).  Measured on config 5 against
+// k_sweep_ws: p = 1 side 64 12.83 -> 9.92 ms; p = 3 side 16 (18.74 -> 20.88), p = 4 side 16 (20.14 -> 21.11) and p = 2
+// side 32 (12.23 -> 13.55) are slower and keep k_sweep_ws
+#define HZ_PK4_TABLE_F32(K4) \
+  K4(1, 4, 288, false)
+#define K4_ENTRY(P, M, MAXT, PRE) \
+  {P, M, M, 0, MAXT, 1, 1, 1, (const void *)k_sweep_pack<float, P, M, MAXT, PRE, 1, 17>, 4, 17},
 #define K_ENTRY(P, M, MAXT)                                                          \
   {P, M, M, 0, MAXT, 1, 1, 1, (const void *)k_sweep_pack<float, P, M, MAXT, false>, 1}, \
   {P, M, M, 0, MAXT, 1, 1, 1, (const void *)k_sweep_pack<float, P, M, MAXT, true>, 2},
 #define CW_ENTRY(P, MX, MY, CL, MAXT, MINB) \
   {P, MX, MY, 0, MAXT, 1, MINB, CL, (const void *)k_sweep_cw<float, P, MX, MY, CL, MAXT, MINB>},
-static const TileEntry kTilesF32[] = {HZ_CW_TABLE_F32(CW_ENTRY) HZ_WS_TABLE_F32(W_ENTRY) HZ_TILE_TABLE_F32(X_ENTRY) HZ_CL_TABLE_F32(C_ENTRY) HZ_PK_TABLE_F32(K_ENTRY) HZ_PK2_TABLE_F32(K2_ENTRY)};
+static const TileEntry kTilesF32[] = {HZ_CW_TABLE_F32(CW_ENTRY) HZ_WS_TABLE_F32(W_ENTRY) HZ_TILE_TABLE_F32(X_ENTRY) HZ_CL_TABLE_F32(C_ENTRY) HZ_PK_TABLE_F32(K_ENTRY) HZ_PK2_TABLE_F32(K2_ENTRY) HZ_PK4_TABLE_F32(K4_ENTRY)};
 #undef K_ENTRY
 #undef C_ENTRY
 #undef X_ENTRY

@@ -79,12 +79,22 @@ namespace hz {
   K2(2, 2, 160, 1)
 #define K2_ENTRY(P, M, MAXT, MINB) \
   {P, M, M, 0, MAXT, 1, MINB, 1, (const void *)k_sweep_pack<double, P, M, MAXT, true, MINB, 9>, 3, 9},
+// K4(P, M, MAXT, PRE): one subdomain of 16 x 16 tiles per block through the packed kernel (pk = 4: the corner node rides on
+// the last top piece, so the 32 edge pieces fill ONE edge warp where k_sweep_ws needs two).  Measured on config 5 against
+// k_sweep_ws / k_sweep_cw: p = 3 side 16 38.15 -> 35.96 ms, p = 4 side 16 72.24 -> 68.09 ms (own part before the barrier),
+// p = 1 side 64 34.84 (cluster of 2) -> 30.15 ms; p = 2 side 32 (35.51 -> 39.08) is slower and keeps k_sweep_ws
+#define HZ_PK4_TABLE_F64(K4) \
+  K4(3, 1, 288, false)     \
+  K4(4, 1, 288, true)      \
+  K4(1, 4, 288, true)
+#define K4_ENTRY(P, M, MAXT, PRE) \
+  {P, M, M, 0, MAXT, 1, 1, 1, (const void *)k_sweep_pack<double, P, M, MAXT, PRE, 1, 17>, 4, 17},
 #define K_ENTRY(P, M, MAXT)                                                          \
   {P, M, M, 0, MAXT, 1, 1, 1, (const void *)k_sweep_pack<double, P, M, MAXT, false>, 1}, \
   {P, M, M, 0, MAXT, 1, 1, 1, (const void *)k_sweep_pack<double, P, M, MAXT, true>, 2},
 #define CW_ENTRY(P, MX, MY, CL, MAXT, MINB) \
   {P, MX, MY, 0, MAXT, 1, MINB, CL, (const void *)k_sweep_cw<double, P, MX, MY, CL, MAXT, MINB>},
-static const TileEntry kTilesF64[] = {HZ_CW_TABLE_F64(CW_ENTRY) HZ_WS_TABLE_F64(W_ENTRY) HZ_TILE_TABLE_F64(X_ENTRY) HZ_CL_TABLE_F64(C_ENTRY) HZ_PK_TABLE_F64(K_ENTRY) HZ_PK2_TABLE_F64(K2_ENTRY)};
+static const TileEntry kTilesF64[] = {HZ_CW_TABLE_F64(CW_ENTRY) HZ_WS_TABLE_F64(W_ENTRY) HZ_TILE_TABLE_F64(X_ENTRY) HZ_CL_TABLE_F64(C_ENTRY) HZ_PK_TABLE_F64(K_ENTRY) HZ_PK2_TABLE_F64(K2_ENTRY) HZ_PK4_TABLE_F64(K4_ENTRY)};
 #undef K_ENTRY
 #undef C_ENTRY
 #undef X_ENTRY
