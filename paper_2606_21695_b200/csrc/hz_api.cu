@@ -57,6 +57,7 @@ struct hz_ctx {
   int sx = 0, sy = 0, ex = 0, ey = 0, L = 0, E = 0, prec = 0;
   int mx = 0, my = 0, csm = 0, ws = 0, cl = 1, entry = -1, pack = 1;
   int pk = 0;             // the partition launches k_sweep_pack (TileEntry::pk of the chosen entry)
+  int cmerge = 0;         // k_sweep_pack: the corner node rides on the last top piece (SweepArgs::cmerge)
   Layout lay{};
   SweepLaunch launch{};
   hz_part_flags flags{};  // variant-choice controls of the last hz_partition_ex
@@ -229,7 +230,7 @@ SweepArgs<real> make_args(const hz_ctx *c, const hz_solve_opts *o, bool homog = 
   }
   a.worder = c->worder;
   a.fused = 0; a.relax = (real)o->relax; a.g_prev = nullptr; a.lam_rw = nullptr;
-  a.pack = c->pack; a.L = c->L;
+  a.pack = c->pack; a.L = c->L; a.cmerge = c->cmerge;
   return a;
 }
 
@@ -632,6 +633,7 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
   ctx->worder = 0;
   ctx->pack = 1;
   ctx->pk = 0;
+  ctx->cmerge = 0;
   const int P = ctx->p;
   // ex, ey: elements per subdomain side; for a ragged partition (general quads only, reading R25) the maximum
   ctx->sx = sx; ctx->sy = sy; ctx->ex = (ctx->nx + sx - 1) / sx; ctx->ey = (ctx->ny + sy - 1) / sy;
@@ -659,7 +661,7 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
   const size_t smem_cap = 227 * 1024;
   Layout lay{};
   lay.lnx = lnx; lay.lny = lny;
-  int best = -1, bpack = 1;
+  int best = -1, bpack = 1, bcm = 0;
   SweepLaunch bl{};
   Layout blay{};
   int sm_count = 148, dev = 0;
@@ -667,7 +669,7 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
   const bool no_ws = fl.no_warp_spec != 0, no_cl = fl.cluster == -1, no_regcap = fl.no_reg_cap != 0;
   const int force_cl = fl.cluster > 1 ? fl.cluster : 0;
   const long long Lsel = fl.grid_blocks > 0 ? fl.grid_blocks : (long long)sx * sy;  // grid size the choice assumes
-  auto tile_fit = [&](const TileEntry &t, Layout *lo, SweepLaunch *la, int *gsel) -> bool {
+  auto tile_fit = [&](const TileEntry &t, Layout *lo, SweepLaunch *la, int *gsel, int *cmsel) -> bool {
     if (t.p != P || ctx->ex % t.mx || ctx->ey % t.my) return false;
     if (force_cl > 1 && t.cl != force_cl) return false;
     if (fl.pack > 1 && !t.pk) return false;
@@ -682,7 +684,13 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
     int G = 1;
     if (t.pk) {
       // G subdomains per block: the G*NB full tiles fill whole bulk warps (hz_sweep_pack.cuh)
-      const int NB = (q.ntx - 1) * (q.nty - 1), NE = q.ntx + q.nty - 2;   // (the last top piece carries the corner node)
+      // corner node on the last top piece's lane (one edge piece fewer per subdomain) or as a piece of its own: measured per
+      // shape on config 5 (A/B on one box, round 2): merging wins for the two-subdomain and 16x16-tile entries, in fp32 for the
+      // 1-tile subdomains and at p = 4 (22.4 against 26.4 ms), in fp64 everywhere except p = 3 (50.0 against 47.0 ms); it loses
+      // in fp32 at p = 1, 2 with 16 tiles (15.5 against 12.1 ms, 19.2 against 16.2 ms)
+      const int NB = (q.ntx - 1) * (q.nty - 1);
+      const bool cmerge = t.pk >= 3 || (rs == 4 ? (NB == 1 || P == 4) : P != 3);
+      const int NE = q.ntx + q.nty - (cmerge ? 2 : 1);
       if (n_t > kTabCMax) return false;
       if (fl.pack == 1) return false;
       // pk = 3: TWO subdomains of up to 64 full tiles per block, their 2 x (ntx + nty - 2) <= 32 edge pieces in ONE edge
@@ -712,7 +720,9 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
       auto shape = [&](int g, int *thr, size_t *smb) {
         *thr = roundup(g * NB, 32) + roundup(g * NE, 32);
         // per buffer: g slices of (padded record grid + zero record + PA | RA) and the scratch region of the idle lanes
-        *smb = 2 * ((size_t)g * ((size_t)((q.ntx + 1) * (q.nty + 1) + 1) * rsw + 2 * nep) + (size_t)(2 * (q.ntx + 1) + 3) * rsw) * rs;
+        const bool pad = t.ntx > 0;   // compile-time tile grid: padded record grid (hz_sweep_pack.cuh)
+        const size_t nrec = pad ? (size_t)(q.ntx + 1) * (q.nty + 1) : (size_t)q.ntx * q.nty, nscr = pad ? 2 * (size_t)(q.ntx + 1) + 3 : 1;
+        *smb = 2 * ((size_t)g * ((nrec + 1) * rsw + 2 * nep) + nscr * rsw) * rs;
       };
       if (pair || single) {
         G = pair ? 2 : 1;
@@ -781,6 +791,7 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
     if (sm > smem_cap) return false;
     *lo = q; la->blocks = t.pk ? (ctx->L + G - 1) / G : ctx->L * t.cl; la->threads = nthr; la->smem = sm;
     if (gsel) *gsel = G;
+    if (cmsel) *cmsel = t.pk ? ((t.pk >= 3 || (rs == 4 ? ((q.ntx - 1) * (q.nty - 1) == 1 || P == 4) : P != 3)) ? 1 : 0) : 0;
     if (t.cl > 1 && !cluster_schedulable(t, *la)) return false;  // e.g. a GPC that cannot co-schedule t.cl such CTAs
     return true;
   };
@@ -817,8 +828,8 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
       const int k = t.mx * P * t.my * P;
       if (dofs_per_thread > 1 && k != dofs_per_thread) continue;
       Layout lo; SweepLaunch la;
-      int gsel = 1;
-      if (!tile_fit(t, &lo, &la, &gsel)) continue;
+      int gsel = 1, cmsel = 0;
+      if (!tile_fit(t, &lo, &la, &gsel, &cmsel)) continue;
       // prefer the warp-specialised kernel, then register-resident coefficients, then the smaller tile
       // (more threads, better latency hiding); among otherwise equal instantiations take the
       // register-capped one (higher occupancy, a few spills) only when the grid can fill that occupancy
@@ -845,7 +856,7 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
       const long long score = score_of(t);
       const long long bscore = best < 0 ? 0 : score_of(tiles[best]);
       if (best < 0 || score < bscore) {
-        best = i; blay = lo; bl = la; bpack = gsel;
+        best = i; blay = lo; bl = la; bpack = gsel; bcm = cmsel;
       }
     }
     if (best < 0 && dofs_per_thread > 1)
@@ -861,6 +872,7 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
     ctx->cl = tiles[best].cl;
     ctx->pack = tiles[best].pk ? bpack : 1;
     ctx->pk = tiles[best].pk;
+    ctx->cmerge = bcm;
     ctx->entry = best;
     // warp-role order of k_sweep_ws: a 3-warp block (2 bulk + 1 edge) puts its edge warp in the middle, so that the bulk
     // warps of the blocks resident on an SM (consecutive hardware warp slots, slot mod 4 = sub-partition) spread evenly

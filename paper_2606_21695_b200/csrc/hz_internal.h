@@ -82,6 +82,7 @@ struct SweepArgs {
   const real *g_prev;
   real *lam_rw;
   int pack;  // packed small-subdomain kernel (hz_sweep_pack.cuh): subdomains per thread block
+  int cmerge;  // packed kernel: 1 = the corner node rides on the last top piece's lane (one edge piece fewer per subdomain)
   int L;     // number of subdomains
 };
 

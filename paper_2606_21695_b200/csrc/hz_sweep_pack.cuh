@@ -48,16 +48,23 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_pack(const SweepArgs<real>
   const int NTH = blockDim.x, h = threadIdx.x, G = A.pack;
   const int ntx = NTX > 0 ? NTX : A.lay.ntx, nty = NTX > 0 ? NTX : A.lay.nty, NTV = A.lay.NT, NS = A.lay.NS;
   const int lnx = A.lay.lnx, lny = A.lay.lny;
-  const int NB = (ntx - 1) * (nty - 1), NE = ntx + nty - 2;   // edge pieces per subdomain (the last top piece also owns the corner node)
-  const int NXP = ntx + 1, NREC = NXP * (nty + 1);            // padded record grid
+  // edge pieces per subdomain: cmerge = 1: the last top piece also owns the corner node; 0: the corner is a piece of its own
+  // (which of the two is faster depends on the shape: hz_partition decides from the config-5 measurements)
+  const bool cm = A.cmerge != 0;
+  const int NB = (ntx - 1) * (nty - 1), NE = ntx + nty - (cm ? 2 : 1);
+  // PAD (the compile-time tile grids): padded record grid; otherwise the compact grid ntx x nty with one zero record per
+  // slice standing in for the missing neighbours (a 25-DOF subdomain has 4 records: padding would double its slice and
+  // halve the blocks per SM)
+  constexpr bool PAD = NTX > 0;
+  const int NXP = PAD ? ntx + 1 : ntx, NREC = PAD ? NXP * (nty + 1) : ntx * nty;
   const int bulkW = (G * NB + 31) & ~31;         // lanes of the bulk warps
   const int NEP = (NE + 1 + V16 - 1) / V16 * V16;   // PA / RA entries: one per piece + the corner node's raw value
   const int ZR = NREC;                           // the zero record of a slice (edge pieces without a neighbour along)
   const int EAO = (NREC + 1) * RS;               // in a slice, after the records: PA[NEP] | RA[NEP]
   const int SW = EAO + 2 * NEP;                  // words per subdomain slice
-  const int BUFW = G * SW + (2 * NXP + 3) * RS;  // per buffer: G slices + a scratch region for idle lanes
+  const int BUFW = G * SW + (PAD ? 2 * NXP + 3 : 1) * RS;  // per buffer: G slices + a scratch region for idle lanes
   real *xb = reinterpret_cast<real *>(smem_raw);
-  const int SCRo = G * SW + (NXP + 1) * RS;      // the scratch record: the middle of that region (its neighbour offsets stay inside)
+  const int SCRo = G * SW + (PAD ? NXP + 1 : 0) * RS;   // the scratch record: the middle of that region (its neighbour offsets stay inside)
 
   for (int q = h; q < 2 * BUFW; q += NTH) xb[q] = real(0);
   const real sigma = A.sigma;
@@ -70,8 +77,14 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_pack(const SweepArgs<real>
     const int tx = act ? t % (ntx - 1) : 0, ty = act ? t / (ntx - 1) : 0;
     const int v = ty * ntx + tx;
     real *sl = xb + (act ? g : 0) * SW;          // this subdomain's slice (buffer 0)
-    real *pMy = act ? sl + ((ty + 1) * NXP + tx + 1) * RS : xb + SCRo;
-    const int oD = NXP * RS;                     // record offset of the tile above / below
+    const int vq = PAD ? (ty + 1) * NXP + tx + 1 : v;   // record index
+    real *pMy = act ? sl + vq * RS : xb + SCRo;
+    // word offsets of the four neighbour records from the own one: constants on the padded grid; on the compact grid the
+    // slice's zero record stands in for a missing neighbour (idle lanes read their own scratch record)
+    const int oL = PAD ? -RS : (!act ? 0 : (tx > 0 ? -RS : (ZR - vq) * RS));
+    const int oR = PAD ? RS : (!act ? 0 : RS);
+    const int oDn = PAD ? -NXP * RS : (!act ? 0 : (ty > 0 ? -NXP * RS : (ZR - vq) * RS));
+    const int oUp = PAD ? NXP * RS : (!act ? 0 : NXP * RS);
     const bool hasL = tx > 0, hasD = ty > 0;
     const real d0x = A.ex1.k0[0] + (hasL ? A.ex1.kp[P] : real(0));
     const real d0y = A.ey1.k0[0] + (hasD ? A.ey1.kp[P] : real(0));
@@ -188,10 +201,10 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_pack(const SweepArgs<real>
         real qR[T], piL[T], qU[T], piD[T];
         if (!PRE) {
           bar_sync_all(NTH);
-          ld_chunk<T>(mr - RS, piL);
-          ld_chunk<T>(mr + RS + CH, qR);
-          ld_chunk<T>(mr - oD + 2 * CH, piD);
-          ld_chunk<T>(mr + oD + 3 * CH, qU);
+          ld_chunk<T>(mr + oL, piL);
+          ld_chunk<T>(mr + oR + CH, qR);
+          ld_chunk<T>(mr + oDn + 2 * CH, piD);
+          ld_chunk<T>(mr + oUp + 3 * CH, qU);
         }
 #pragma unroll
         for (int b = 0; b < T; ++b) {
@@ -227,10 +240,10 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_pack(const SweepArgs<real>
         }
         if (PRE) {
           bar_sync_all(NTH);
-          ld_chunk<T>(mr - RS, piL);
-          ld_chunk<T>(mr + RS + CH, qR);
-          ld_chunk<T>(mr - oD + 2 * CH, piD);
-          ld_chunk<T>(mr + oD + 3 * CH, qU);
+          ld_chunk<T>(mr + oL, piL);
+          ld_chunk<T>(mr + oR + CH, qR);
+          ld_chunk<T>(mr + oDn + 2 * CH, piD);
+          ld_chunk<T>(mr + oUp + 3 * CH, qU);
         }
         cur = BUFW - cur;
 #pragma unroll
@@ -323,7 +336,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_pack(const SweepArgs<real>
     const int tx = !act ? 0 : (top ? e - (nty - 1) : ntx - 1);
     const int ty = !act ? 0 : (top ? nty - 1 : e);
     const int v = ty * ntx + tx;                          // slot in the per-node global arrays
-    const int vq = (ty + 1) * NXP + tx + 1;               // record index (padded grid)
+    const int vq = PAD ? (ty + 1) * NXP + tx + 1 : v;     // record index
     const int ta = top ? tx : ty, nta = top ? ntx : nty;  // position / count along the line direction
     const int sc = top ? NXP : 1;                         // record stride across
     const int oRC = top ? 3 * CH : CH, oPC = top ? 2 * CH : 0;
@@ -336,12 +349,12 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_pack(const SweepArgs<real>
     real *pPAout = !act ? scr : ((!top && ty == nty - 2) ? sl + vq * RS + 2 * CH : sl + EAO + e);
     real *pRAout = !act ? scr + 1 : sl + EAO + NEP + e;
     const real *pP = hasP ? sl + EAO + e - 1 : sl + ZR * RS;
-    const real *pN = hasN ? sl + EAO + NEP + ((!top && ty == nty - 2) ? NE : e + 1) : sl + ZR * RS;   // RA[NE]: the corner node
+    const real *pN = hasN ? sl + EAO + NEP + ((!top && ty == nty - 2) ? ntx + nty - 2 : e + 1) : sl + ZR * RS;   // RA[ntx+nty-2]: the corner node
     const real *pC = sl + (act ? vq - sc : ZR) * RS + oPC;
-    const bool isLT = act && top && tx == ntx - 2;       // carries the corner node
+    const bool isLT = cm && act && top && tx == ntx - 2;  // carries the corner node
     const int vC = (nty - 1) * ntx + ntx - 1;            // the corner's virtual tile
-    real *pRAc = isLT ? sl + EAO + NEP + NE : scr + 2;   // its raw value, read by the last right piece and by this lane
-    const real *pCc = sl + (isLT ? (nty - 1) * NXP + ntx : ZR) * RS + 2 * CH;   // the last right piece's partial (element 0 of its PY chunk)
+    real *pRAc = isLT ? sl + EAO + NEP + ntx + nty - 2 : scr + 2;   // its raw value, read by the last right piece and by this lane
+    const real *pCc = sl + (isLT ? (PAD ? (nty - 1) * NXP + ntx : vC - ntx) : ZR) * RS + 2 * CH;   // the last right piece's partial (element 0 of its PY chunk)
     Elem1D<real> ka;  // coefficients along
 #pragma unroll
     for (int c = 0; c <= P; ++c) {
@@ -375,6 +388,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_pack(const SweepArgs<real>
     const int len1 = top ? lnx : lny;
     int side2 = -1, idx2 = 0;
     if (act && top && tx == 0 && six > 0) { side2 = kSideW; idx2 = lny - 1; }
+    if (act && top && tx == ntx - 1 && six < A.sx - 1) { side2 = kSideE; idx2 = lny - 1; }   // (the corner as a piece of its own)
     if (act && !top && ty == 0 && siy > 0) { side2 = kSideS; idx2 = lnx - 1; }
 #pragma unroll
     for (int n = 0; n < T; ++n) {
