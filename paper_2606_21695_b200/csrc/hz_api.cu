@@ -758,7 +758,8 @@ hz_status hz_partition_ex(hz_ctx *ctx, int sx, int sy, hz_transmission tc, hz_pr
       size_t rsw = 2 * chx + 2 * chy;
       if ((rsw / v16) % 2 == 0) rsw += v16;
       const size_t nep = ((size_t)nel + v16 - 1) / v16 * v16;
-      const size_t bufw = ((size_t)(wmax + 1) * q.nty + 2) * rsw + 2 * nep, hs = 2 * (size_t)nbr * chy + 2 * v16;
+      // per buffer: the padded record grid (wmax + 2) x (nty + 1) + the scratch region of the idle lanes + PA | RA; the scalar halo slots of the top pieces
+      const size_t bufw = ((size_t)(wmax + 2) * (q.nty + 1) + 2 * (size_t)(q.nty + 1) + 1) * rsw + 2 * nep, hs = 2 * v16;
       sm = (2 * bufw + 2 * hs) * rs + 16;
     } else if (t.cl > 1) {
       if (no_cl || n_t > kTabCMax || q.ntx < t.cl) return false;

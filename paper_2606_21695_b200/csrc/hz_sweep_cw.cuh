@@ -58,16 +58,27 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_cw(const SweepArgs<real> A
   const int bulkW = (wmax * NBR + 31) & ~31;          // bulk lanes (uniform over the cluster)
   const int NEL = NBR + wmax + 1;                     // edge lanes of the last CTA: right pieces | top pieces | corner
   const int NEP = (NEL + V16 - 1) / V16 * V16;
-  const int NREC = (wmax + 1) * nty;                  // records: local tile column c (0..wloc; wloc = the right pieces) x nty
-  const int ZR = NREC, SCR = NREC + 1;
-  const int EAO = (NREC + 2) * RS;                    // after the records: PA[NEP] | RA[NEP] of the edge lanes
+  // Records on a PADDED grid of (wmax + 2) columns x (nty + 1) rows: local tile column c at grid column c + 1, tile row t at
+  // grid row t + 1; grid row 0 is never written (zero: no tile below), grid column 0 and the column after the strip are the
+  // HALO columns the adjacent CTAs push into (zero where the subdomain ends; in the last CTA the column after the strip is the
+  // right pieces' own).  Every full tile finds its four neighbours at the same offsets from its own record, so the time loop
+  // keeps one pointer per thread (own record, current buffer) instead of five and no per-source buffer stride.
+  const int NYP = nty + 1;
+  const int NREC = (wmax + 2) * NYP;
+  // idle lanes own the middle record of a scratch region behind the grid (their neighbour offsets stay inside it); grid record
+  // (column 0, row 0) is never written and serves as the zero record
+  const int SCR = NREC + NYP, ZR = 0;
+  const int EAO = (NREC + 2 * NYP + 1) * RS;          // after the records: PA[NEP] | RA[NEP] of the edge lanes
   const int BUFW = EAO + 2 * NEP;
-  const int HS = 2 * NBR * CHY + 2 * V16;             // halo slots per buffer: haloL[NBR][CHY] | haloR[NBR][CHY] | PAh | RAh
+  const int HS = 2 * V16;                             // halo scalars per buffer (top pieces across a cut): PAh | RAh
   real *xb = reinterpret_cast<real *>(smem_raw);
   real *halo = xb + 2 * BUFW;
   const unsigned mbar0 = (unsigned)__cvta_generic_to_shared(halo + 2 * HS);
   const unsigned hbase = (unsigned)__cvta_generic_to_shared(halo);
-  const int oHL = 0, oHR = NBR * CHY, oPAh = 2 * NBR * CHY, oRAh = 2 * NBR * CHY + V16;
+  const unsigned xbase = (unsigned)__cvta_generic_to_shared(xb);
+  const int oPAh = 0, oRAh = V16;
+  const int wlocP = wq + (rk - 1 < wrem ? 1 : 0);    // strip width of the previous CTA
+  auto recq = [&](int c, int t) { return (c + 1) * NYP + t + 1; };   // record of local tile column c, tile row t
 
   for (int q = h; q < 2 * BUFW + 2 * HS; q += NTH) xb[q] = real(0);
   if (h == 0) {
@@ -87,18 +98,15 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_cw(const SweepArgs<real> A
     const int txl = act ? h / NBR : 0, ty = act ? h - txl * NBR : 0;
     const int tx = c0 + txl;
     const int v = tx * nty + ty;                      // slot in the per-node global arrays
-    const int rec = txl * nty + ty;
+    const int rec = recq(txl, ty);
     const bool remL = act && txl == 0 && rk > 0, remR = act && txl == wloc - 1 && !lastc;
     const bool hasL = tx > 0, hasD = ty > 0;
     real *pMy = xb + (act ? rec : SCR) * RS;
-    const real *pL = remL ? halo + oHL + ty * CHY : xb + ((act && txl > 0) ? rec - nty : ZR) * RS + oPX;
-    const real *pR = remR ? halo + oHR + ty * CHY : xb + (act ? rec + nty : ZR) * RS + oRX;
-    const real *pD = xb + ((act && hasD) ? rec - 1 : ZR) * RS + oPY;
-    const real *pU = xb + (act ? rec + 1 : ZR) * RS + oRY;
-    const int strL = remL ? HS : BUFW, strR = remR ? HS : BUFW;   // distance between the two buffers of that source
+    const int oX = NYP * RS;                          // record offset of the tile column to the right / left
     const bool wwait = __any_sync(0xffffffffu, remL || remR);
-    const unsigned pushR = remR ? mapa_cluster(hbase + (unsigned)(oHL + ty * CHY) * RB, rk + 1) : 0u;
-    const unsigned pushL = remL ? mapa_cluster(hbase + (unsigned)(oHR + ty * CHY) * RB, rk - 1) : 0u;
+    // what the tile across the cut needs goes into the adjacent CTA's halo column, at the chunk its reader loads
+    const unsigned pushR = remR ? mapa_cluster(xbase + (unsigned)(recq(-1, ty) * RS + oPX) * RB, rk + 1) : 0u;
+    const unsigned pushL = remL ? mapa_cluster(xbase + (unsigned)(recq(wlocP, ty) * RS + oRX) * RB, rk - 1) : 0u;
     const unsigned mbR = remR ? mapa_cluster(mbar0, rk + 1) : 0u, mbL = remL ? mapa_cluster(mbar0, rk - 1) : 0u;
     const real d0x = A.ex1.k0[0] + (hasL ? A.ex1.kp[P] : real(0));
     const real d0y = A.ey1.k0[0] + (hasD ? A.ey1.kp[P] : real(0));
@@ -198,9 +206,9 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_cw(const SweepArgs<real> A
           st_chunk<TY>(my + oRX, vRX);
           st_chunk<TX>(my + oPY, vPY);
           st_chunk<TX>(my + oRY, vRY);
-          // strip boundary: push what the tile across the cut needs into the adjacent CTA's halo slot
-          if (remR) push_chunk<TY>(pushR + (unsigned)(bsel * HS) * RB, mbR + 8u * bsel, vPX);
-          if (remL) push_chunk<TY>(pushL + (unsigned)(bsel * HS) * RB, mbL + 8u * bsel, vRX);
+          // strip boundary: push what the tile across the cut needs into the adjacent CTA's halo column (same buffer)
+          if (remR) push_chunk<TY>(pushR + (unsigned)cur * RB, mbR + 8u * bsel, vPX);
+          if (remL) push_chunk<TY>(pushL + (unsigned)cur * RB, mbL + 8u * bsel, vRX);
         }
         if (h == 0) mbar_arm(mbar0 + 8u * bsel, tx_bytes);
         const Tab4<real> tn = TC.t[nu];
@@ -234,10 +242,11 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_cw(const SweepArgs<real> A
         if (bsel) ph1 ^= 1u;
         else ph0 ^= 1u;
         real qR[TY], piL[TY], qU[TX], piD[TX];
-        ld_chunk<TY>(pL + bsel * strL, piL);
-        ld_chunk<TY>(pR + bsel * strR, qR);
-        ld_chunk<TX>(pD + cur, piD);
-        ld_chunk<TX>(pU + cur, qU);
+        const real *mr = pMy + cur;
+        ld_chunk<TY>(mr - oX + oPX, piL);
+        ld_chunk<TY>(mr + oX + oRX, qR);
+        ld_chunk<TX>(mr - RS + oPY, piD);
+        ld_chunk<TX>(mr + RS + oRY, qU);
         cur = BUFW - cur;
         bsel ^= 1;
 #pragma unroll
@@ -323,7 +332,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_cw(const SweepArgs<real> A
     const int tx = top ? c0 + txl : ntx - 1;           // (the corner: c0 + wloc = ntx - 1 in the last CTA)
     const int ty = top ? nty - 1 : (isR ? e : 0);
     const int v = tx * nty + ty;
-    const int rec = txl * nty + ty;
+    const int rec = recq(txl, ty);
     const int ta = top ? tx : ty, nta = top ? ntx : nty;
     const bool hasP = act && ta > 0, hasN = act && ta < nta - 1;
     // along-the-edge neighbours across a strip cut (top pieces only)
@@ -337,7 +346,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_cw(const SweepArgs<real> A
     const real *pN = remN ? halo + oRAh : (hasN ? xb + EAO + NEP + (lastR ? NBR + wloc : e + 1) : xb + ZR * RS);
     const int strP = remP ? HS : BUFW, strN = remN ? HS : BUFW;
     // partial sums from the tile across: bulk tile below (its PY) / to the left (its PX); for the corner the last right piece
-    const real *pC = xb + (act ? (top ? rec - 1 : rec - nty) : ZR) * RS + (top ? oPY : oPX);
+    const real *pC = xb + (act ? (top ? rec - 1 : rec - NYP) : ZR) * RS + (top ? oPY : oPX);
     const bool wwait = __any_sync(0xffffffffu, remP || remN);
     const unsigned pushPA = remN ? mapa_cluster(hbase + (unsigned)oPAh * RB, rk + 1) : 0u;   // my partial -> next CTA's first top piece
     const unsigned pushRA = remP ? mapa_cluster(hbase + (unsigned)oRAh * RB, rk - 1) : 0u;   // my raw p[0] -> previous CTA's last top piece
