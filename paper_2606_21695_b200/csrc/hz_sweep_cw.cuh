@@ -163,7 +163,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_cw(const SweepArgs<real> A
     cluster_sync_all();  // every CTA's mbarriers and zeroed buffers exist before anyone pushes
 
     int cur = 0, bsel = 0;
-    unsigned ph0 = 0, ph1 = 0;
+    unsigned nstep = 0;   // time steps done: barrier nstep & 1 is in its phase (nstep >> 1)
     for (int m = 0; m < A.n_wh; ++m) {
       const Tab4<real> t0 = TC.t[0];
 #pragma unroll
@@ -207,10 +207,12 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_cw(const SweepArgs<real> A
           st_chunk<TX>(my + oPY, vPY);
           st_chunk<TX>(my + oRY, vRY);
           // strip boundary: push what the tile across the cut needs into the adjacent CTA's halo column (same buffer)
-          if (remR) push_chunk<TY>(pushR + (unsigned)cur * RB, mbR + 8u * bsel, vPX);
-          if (remL) push_chunk<TY>(pushL + (unsigned)cur * RB, mbL + 8u * bsel, vRX);
+          if (h == 0) mbar_arm(mbar0 + 8u * bsel, tx_bytes);   // (arming from the edge warp instead measured 4 % slower in fp32)
+          if (remR || remL) {
+            if (remR) push_chunk<TY>(pushR + (unsigned)cur * RB, mbR + 8u * bsel, vPX);
+            if (remL) push_chunk<TY>(pushL + (unsigned)cur * RB, mbL + 8u * bsel, vRX);
+          }
         }
-        if (h == 0) mbar_arm(mbar0 + 8u * bsel, tx_bytes);
         const Tab4<real> tn = TC.t[nu];
         real S[TY][TX], X0[TY], Y0[TX];
         // the neighbour-independent part of the step, in front of the barrier
@@ -238,9 +240,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_cw(const SweepArgs<real> A
 #pragma unroll
           for (int a = 0; a < TX; ++a) vr[b][a] = fmaT(tn.k, p[b][a], vr[b][a]);
         __syncthreads();
-        if (wwait) mbar_wait_parity(mbar0 + 8u * bsel, bsel ? ph1 : ph0);
-        if (bsel) ph1 ^= 1u;
-        else ph0 ^= 1u;
+        if (wwait) mbar_wait_parity(mbar0 + 8u * bsel, (nstep >> 1) & 1u);
+        ++nstep;
         real qR[TY], piL[TY], qU[TX], piD[TX];
         const real *mr = pMy + cur;
         ld_chunk<TY>(mr - oX + oPX, piL);
@@ -436,7 +437,7 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_cw(const SweepArgs<real> A
     using MYt = std::integral_constant<int, MY>;
 
     int cur = 0, bsel = 0;
-    unsigned ph0 = 0, ph1 = 0;
+    unsigned nstep = 0;   // time steps done: barrier nstep & 1 is in its phase (nstep >> 1)
     for (int m = 0; m < A.n_wh; ++m) {
       const Tab4<real> t0 = TC.t[0];
 #pragma unroll
@@ -452,9 +453,8 @@ __global__ void __launch_bounds__(MAXT, MINB) k_sweep_cw(const SweepArgs<real> A
         else publish(MYt{}, A.ey1, cur, bsel);
         __syncwarp();   // the two piece kinds reconverge before the (aligned) block barrier
         __syncthreads();
-        if (wwait) mbar_wait_parity(mbar0 + 8u * bsel, bsel ? ph1 : ph0);
-        if (bsel) ph1 ^= 1u;
-        else ph0 ^= 1u;
+        if (wwait) mbar_wait_parity(mbar0 + 8u * bsel, (nstep >> 1) & 1u);
+        ++nstep;
         const Tab4<real> tn = TC.t[nu];
         if (top) finish(MXt{}, A.ex1, cur, bsel, tn);
         else finish(MYt{}, A.ey1, cur, bsel, tn);
