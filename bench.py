@@ -43,8 +43,8 @@ STORED_TRAFFIC = {
     "config5_p3_s8_f64": {"bytes": 2.753e9, "from": "profiles/r02_l_sweep_pack_cfg5_f64.md", "captured": "round 2"},
     "config3_p3_s8_f32": {"bytes": 62.5e6, "from": "profiles/r02_m_sweep_pack_cfg3_f32.md", "captured": "round 2"},
     "config3_p3_s8_f64": {"bytes": 137.6e6, "from": "profiles/r02_n_sweep_pack_cfg3_f64.md", "captured": "round 2"},
-    "config4_p3_s32_f32": {"bytes": 237.9e6, "from": "profiles/r02_c_sweep_cw_cfg4_f32.md", "captured": "round 2"},
-    "config4_p3_s32_f64": {"bytes": 500.1e6, "from": "profiles/r02_d_sweep_cw_cfg4_f64.md", "captured": "round 2"},
+    "config4_p3_s32_f32": {"bytes": 238.3e6, "from": "profiles/r02_c_sweep_cw_cfg4_f32.md", "captured": "round 2"},
+    "config4_p3_s32_f64": {"bytes": 501.2e6, "from": "profiles/r02_d_sweep_cw_cfg4_f64.md", "captured": "round 2"},
 }
 
 
