@@ -755,7 +755,10 @@ def run_extras(hz, torch, args, flush, stream, sampler):
                 rate = r.dof_timesteps / (r.sweep_ms_total * 1e-3)
                 r3[name + "_f32"] = {"dof_steps_per_s_sweep_kernel": rate, "sweep_ms": r.sweep_ms_total / 3, "n_t": info3.n_t,
                                      "nodes_per_thread": info3.nodes_per_thread, "blocks": info3.blocks,
-                                     "frac_of_derived_peak": rate * 2 * (3 * (p + 2) + 5) / (peak_tflops("f32") * 1e12)}
+                                     "frac_of_derived_peak": rate * 2 * (3 * (p + 2) + 5) / (peak_tflops("f32") * 1e12),
+                                     # the column kernel reads the x and y stencil operands from shared memory: 2(2p+1) loads
+                                     # + 1 store per DOF-step against 128 B per clock and SM (its binding roofline)
+                                     "frac_of_shared_memory_roofline": rate * (4 * p + 3) * 4 / (SMS * 128.0 * SM_MHZ * 1e6)}
             finally:
                 hz3.hz3_destroy(c3)
         return r3
