@@ -81,8 +81,12 @@ namespace hz {
 // the last top piece, so the 32 edge pieces fill ONE edge warp where k_sweep_ws needs two).  Measured on config 5 against
 // k_sweep_ws: p = 1 side 64 12.83 -> 9.92 ms; p = 3 side 16 (18.74 -> 20.88), p = 4 side 16 (20.14 -> 21.11) and p = 2
 // side 32 (12.23 -> 13.55) are slower and keep k_sweep_ws
-#define HZ_PK4_TABLE_F32(K4) \
+#define HZ_PK4_TABLE_F32(K4, K4B) \
+  K4B(3, 1, 288, true, 2)  \
   K4(1, 4, 288, false)
+// K4B: the same with a register cap for MINB blocks per SM (and, in fp32, the FFMA2 updates)
+#define K4B_ENTRY(P, M, MAXT, PRE, MINB) \
+  {P, M, M, 0, MAXT, 1, MINB, 1, (const void *)k_sweep_pack<float, P, M, MAXT, PRE, MINB, 17>, 4, 17},
 #define K4_ENTRY(P, M, MAXT, PRE) \
   {P, M, M, 0, MAXT, 1, 1, 1, (const void *)k_sweep_pack<float, P, M, MAXT, PRE, 1, 17>, 4, 17},
 #define K_ENTRY(P, M, MAXT)                                                          \
@@ -90,7 +94,7 @@ namespace hz {
   {P, M, M, 0, MAXT, 1, 1, 1, (const void *)k_sweep_pack<float, P, M, MAXT, true>, 2},
 #define CW_ENTRY(P, MX, MY, CL, MAXT, MINB) \
   {P, MX, MY, 0, MAXT, 1, MINB, CL, (const void *)k_sweep_cw<float, P, MX, MY, CL, MAXT, MINB>},
-static const TileEntry kTilesF32[] = {HZ_CW_TABLE_F32(CW_ENTRY) HZ_WS_TABLE_F32(W_ENTRY) HZ_TILE_TABLE_F32(X_ENTRY) HZ_CL_TABLE_F32(C_ENTRY) HZ_PK_TABLE_F32(K_ENTRY) HZ_PK2_TABLE_F32(K2_ENTRY) HZ_PK4_TABLE_F32(K4_ENTRY)};
+static const TileEntry kTilesF32[] = {HZ_CW_TABLE_F32(CW_ENTRY) HZ_WS_TABLE_F32(W_ENTRY) HZ_TILE_TABLE_F32(X_ENTRY) HZ_CL_TABLE_F32(C_ENTRY) HZ_PK_TABLE_F32(K_ENTRY) HZ_PK2_TABLE_F32(K2_ENTRY) HZ_PK4_TABLE_F32(K4_ENTRY, K4B_ENTRY)};
 #undef K_ENTRY
 #undef C_ENTRY
 #undef X_ENTRY
